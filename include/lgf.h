@@ -1,0 +1,138 @@
+/* lgf.h -- C ABI of the B200 (sm_100a) Fourier-accelerated Landau gauge fixer.
+ *
+ * Method: arXiv 1301.3460, "Landau gauge fixing on the lattice using GPU's".  The library
+ * maximises, on a 4-D periodic SU(3) lattice,
+ *
+ *     F_U[g] = (1/(N_d N_c V)) sum_x sum_mu Re Tr[ g(x) U_mu(x) g^dag(x+mu) ]
+ *
+ * with the steepest-descent method with Fourier acceleration, run parameters alpha and
+ * theta < theta_tol, links stored as 12 reals (two rows) or 18 reals.
+ * One iteration (BASELINE.json north_star steps 1-4):
+ *   S1  Delta(x) = A - A^dag - (1/3)Tr(A - A^dag),  A = sum_mu [U_mu(x-mu) - U_mu(x)];
+ *       theta = (1/(N_c V)) sum_x Tr[Delta Delta^dag];  F = (1/(N_d N_c V)) sum_x sum_mu Re Tr U_mu(x)
+ *   S2  X = IFFT[ (p2max/p2) FFT[Delta] ],  p2(n) = sum_mu 4 sin^2(pi n_mu/L_mu), p2max = 16, zero mode 0
+ *   S3  g(x) = rowGramSchmidt(1 + (alpha/2) X(x)), third row conj(u x v)
+ *   S4  U_mu(x) <- g(x) U_mu(x) g^dag(x+mu)   (all x, mu simultaneously)
+ *   S5  stop when theta < theta_tol (strict)
+ *
+ * Conventions
+ *   - Host/device link arrays ("canonical order"): double [V][4][3][3][2], i.e. links[x][mu][row][col][re,im],
+ *     site index x = x0 + L0*(x1 + L1*(x2 + L2*x3)) (x0 fastest), periodic boundaries.  Always 18 reals per
+ *     link on this boundary, whatever the internal storage.
+ *   - Every pointer argument says whether it is HOST or DEVICE memory.  The caller owns every pointer it
+ *     passes; the context never keeps a caller pointer after the call returns, except the workspace and
+ *     stream given to lgf_create_ex, which must outlive the context.
+ *   - Every call returns lgf_status.  No exceptions, no exit(), nothing is printed.  Out-parameters are
+ *     written only when the call returns LGF_OK or LGF_NOT_CONVERGED.
+ *   - Calls are synchronous for the host: on return the results are final.  Internally all work is ordered
+ *     on the context's CUDA stream.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with LGF_ERR_CUDA.
+ *   - Supported sizes: each L_mu a power of two, 4 <= L_mu <= 128, L0*L1 <= 4096 and L2*L3 <= 4096
+ *     (shared-memory tile limits of the FFT passes); otherwise LGF_ERR_UNSUPPORTED.
+ */
+#ifndef LGF_H
+#define LGF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lgf_ctx lgf_ctx; /* opaque; owns its device buffers unless a workspace was supplied */
+
+typedef enum {
+    LGF_OK = 0,
+    LGF_ERR_INVALID_ARG = 1,
+    LGF_ERR_UNSUPPORTED = 2,
+    LGF_ERR_OOM = 3,
+    LGF_ERR_CUDA = 4,
+    LGF_ERR_NOT_LOADED = 5,
+    LGF_ERR_NUMERIC = 6,      /* theta or F became non-finite */
+    LGF_NOT_CONVERGED = 100   /* non-fatal: max_iter reached, state and outputs valid */
+} lgf_status;
+
+typedef enum { LGF_FP64 = 0, LGF_FP32 = 1 /* not built yet: LGF_ERR_UNSUPPORTED */ } lgf_precision;
+typedef enum { LGF_STORE_18 = 18, LGF_STORE_12 = 12 } lgf_storage;
+
+/* Bytes of device workspace a context for these parameters needs (0 if the parameters are unsupported). */
+size_t lgf_workspace_bytes(const int dims[4], lgf_precision p, lgf_storage s);
+
+/* Create a context.  dims: HOST, {L0,L1,L2,L3}.  The library allocates its own device memory (cudaMalloc)
+ * on the current device and creates its own stream. */
+lgf_status lgf_create(const int dims[4], lgf_precision p, lgf_storage s, lgf_ctx **out);
+
+/* Same, but all device memory comes from dev_workspace (DEVICE pointer, 256-byte aligned, at least
+ * lgf_workspace_bytes() bytes) and all work is ordered on cuda_stream (a cudaStream_t cast to void*; NULL is
+ * the default stream).  This is how a framework (e.g. PyTorch) lends memory and a stream. */
+lgf_status lgf_create_ex(const int dims[4], lgf_precision p, lgf_storage s,
+                         void *dev_workspace, size_t workspace_bytes, void *cuda_stream, lgf_ctx **out);
+
+void lgf_destroy(lgf_ctx *ctx);
+
+/* Load links.  host_links: HOST, canonical order, V*4*18 doubles.  Stored as given -- no reprojection; in
+ * 12-real storage rows 0,1 are kept and row 2 is dropped (it is rebuilt as conj(row0 x row1) on use). */
+lgf_status lgf_load_links(lgf_ctx *ctx, const double *host_links);
+/* Same from DEVICE memory (canonical order). */
+lgf_status lgf_load_links_device(lgf_ctx *ctx, const double *dev_links);
+
+/* Read the links back, canonical order, always full 18 reals per link (row 2 rebuilt in 12-real storage). */
+lgf_status lgf_get_links(lgf_ctx *ctx, double *host_links);
+lgf_status lgf_get_links_device(lgf_ctx *ctx, double *dev_links);
+
+/* Apply exactly n iterations S1-S4 with step alpha (no stop test), then measure once more.
+ * F, theta (HOST, may be NULL): the functional and theta of the links AFTER the n-th update.  n >= 0. */
+lgf_status lgf_iterate(lgf_ctx *ctx, int n, double alpha, double *F, double *theta);
+
+/* Iterate until theta < theta_tol (strict) or max_iter updates.  n_iter (HOST): number of link updates applied
+ * before the first measurement with theta < theta_tol (0 if the links already satisfy it).  F, theta: that
+ * measurement.  Returns LGF_OK, or LGF_NOT_CONVERGED when max_iter updates did not reach theta_tol. */
+lgf_status lgf_fix(lgf_ctx *ctx, double alpha, double theta_tol, int max_iter,
+                   int *n_iter, double *F, double *theta);
+
+/* F, theta and the average plaquette of the current links; no state change.  Any out pointer may be NULL. */
+lgf_status lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette);
+
+/* (F_k, theta_k) of the measurements made by the last lgf_iterate/lgf_fix call, k = 0..min(n_iter, cap-1);
+ * hist: HOST, 2*capacity doubles; *n_out receives how many pairs were written. */
+lgf_status lgf_get_history(lgf_ctx *ctx, double *hist, int capacity, int *n_out);
+
+/* Stage read-outs for kernel-level parity tests.  Each writes a full anti-Hermitian 3x3 field, HOST,
+ * double [V][3][3][2], computed by the hot-path kernels from the current links (links unchanged):
+ *   LGF_FIELD_DELTA  Delta(x) of step S1;   LGF_FIELD_X  X(x) of step S2;
+ *   LGF_FIELD_G      g(x) of step S3 for the given alpha (a special unitary field, not anti-Hermitian). */
+typedef enum { LGF_FIELD_DELTA = 0, LGF_FIELD_X = 1, LGF_FIELD_G = 2 } lgf_field;
+lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *host_field);
+
+/* Kernel selection (for ncu comparisons; results are identical up to rounding order).
+ *   LGF_OPT_FUSE_DELTA_FFT  1: Delta is computed inside FFT pass A (default when the plane fits), 0: separate kernel
+ *   LGF_OPT_STORE_G         1: pass C stores g(x) and the update reads it, 0: the update recomputes g from X
+ *   LGF_OPT_GRAPH           1: replay iterations through a CUDA graph (default), 0: plain launches
+ *   LGF_OPT_BATCH           iterations enqueued between two reads of the device stop flag (default 8) */
+typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3 } lgf_option;
+lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
+lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
+
+/* Per-kernel device timing.  lgf_set_profiling(ctx,1) brackets every kernel launch with CUDA events on the
+ * context's stream (plain launches, no graph); lgf_get_profile returns, per kernel slot i < LGF_MAX_KERNELS,
+ * the accumulated milliseconds and launch counts since profiling was enabled.  names via lgf_kernel_name. */
+#define LGF_MAX_KERNELS 16
+lgf_status lgf_set_profiling(lgf_ctx *ctx, int on);
+lgf_status lgf_get_profile(lgf_ctx *ctx, double ms[LGF_MAX_KERNELS], long long launches[LGF_MAX_KERNELS]);
+const char *lgf_kernel_name(int slot);
+
+/* Total number of this library's kernels launched by the context since creation. */
+long long lgf_launch_count(lgf_ctx *ctx);
+
+/* Stream copy yardstick: copies `bytes` (multiple of 16) from dev_src to dev_dst (DEVICE) `reps` times with the
+ * library's own double2 streaming kernel on cuda_stream and returns the average milliseconds per copy in *ms
+ * (HOST).  This is the "measured copy-kernel peak" of the north star: GB/s = 2*bytes/ms/1e6. */
+lgf_status lgf_copy_peak(void *dev_dst, const void *dev_src, size_t bytes, int reps, void *cuda_stream, double *ms);
+
+const char *lgf_status_string(lgf_status s);
+const char *lgf_last_error(lgf_ctx *ctx); /* detail of the last LGF_ERR_CUDA (static or ctx-owned string) */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LGF_H */

@@ -1,0 +1,128 @@
+// fft_tile.cuh -- in-place power-of-two FFTs along one axis of a shared-memory tile (fp64, sm_100a).
+//
+// Forward transforms are decimation-in-frequency: natural order in, DIGIT-REVERSED order out.  Inverse
+// transforms are the exact stage-by-stage inverses (decimation-in-time, conjugate twiddles), so they take
+// digit-reversed order in and give natural order out.  Between the two, the p2max/p2 filter is applied at
+// the stored (digit-reversed) positions using per-axis tables built in the same order (host side,
+// lgf_api.cu: stored_freq()).  No reordering pass and no ping-pong buffer is ever needed.
+//
+// Stage radices for a sub-length N = 2^lgN:  radix 4 when lgN is 2 or 4, radix 2 when lgN is 1, else radix 8
+// (L = 4:[4]  8:[8]  16:[4,4]  32:[8,4]  64:[8,8]  128:[8,4,4]).  The last forward stage has unit twiddles.
+#pragma once
+#include "su3.cuh"
+
+namespace lgf {
+
+__host__ __device__ __forceinline__ int stage_lg_radix(int lgN) { return (lgN == 1) ? 1 : ((lgN == 2 || lgN == 4) ? 2 : 3); }
+
+// One axis transform inside a tile.  Work items are (iA, q, iB): iA the fastest thread index over a
+// non-transformed tile axis (stride strideA, 2^lgA values), q the butterfly inside a line, iB the slow
+// non-transformed axis.
+struct AxisXf {
+    int lgL;       // log2 of the transform length
+    int strideK;   // element stride along the transformed axis
+    int lgA, strideA;
+    int nB, strideB;
+    const cplx* tw;  // shared-memory table tw[k] = exp(-2 pi i k / L), k < L
+};
+
+template <bool INV> __device__ __forceinline__ cplx mul_i(cplx a) {  // forward: * (-i); inverse: * (+i)
+    return INV ? mk(-a.y, a.x) : mk(a.y, -a.x);
+}
+
+template <bool INV> __device__ __forceinline__ void bfly2(cplx& a, cplx& b) { cplx t = csub(a, b); a = cadd(a, b); b = t; }
+
+// y_m = sum_k x_k W4^{mk}, W4 = exp(-+ 2 pi i/4)
+template <bool INV> __device__ __forceinline__ void bfly4(cplx& x0, cplx& x1, cplx& x2, cplx& x3) {
+    cplx t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), t3 = mul_i<INV>(csub(x1, x3));
+    x0 = cadd(t0, t2); x2 = csub(t0, t2); x1 = cadd(t1, t3); x3 = csub(t1, t3);
+}
+
+template <bool INV> __device__ __forceinline__ void bfly8(cplx (&v)[8]) {
+    // even/odd split: E = DFT4(v0,v2,v4,v6), O = DFT4(v1,v3,v5,v7); y_m = E_m + W8^m O_m, y_{m+4} = E_m - W8^m O_m
+    bfly4<INV>(v[0], v[2], v[4], v[6]);   // now v0,v2,v4,v6 = E_0..E_3
+    bfly4<INV>(v[1], v[3], v[5], v[7]);   // now v1,v3,v5,v7 = O_0..O_3
+    const double h = 0.70710678118654752440;
+    cplx o1 = v[3], o2 = v[5], o3 = v[7];
+    // W8^1 = h(1 -+ i), W8^2 = -+ i, W8^3 = h(-1 -+ i)
+    cplx w1 = INV ? mk(h * (o1.x - o1.y), h * (o1.x + o1.y)) : mk(h * (o1.x + o1.y), h * (o1.y - o1.x));
+    cplx w2 = mul_i<INV>(o2);
+    cplx w3 = INV ? mk(-h * (o3.x + o3.y), h * (o3.x - o3.y)) : mk(h * (o3.y - o3.x), -h * (o3.x + o3.y));
+    cplx e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
+    v[0] = cadd(e0, o0); v[4] = csub(e0, o0);
+    v[1] = cadd(e1, w1); v[5] = csub(e1, w1);
+    v[2] = cadd(e2, w2); v[6] = csub(e2, w2);
+    v[3] = cadd(e3, w3); v[7] = csub(e3, w3);
+}
+
+template <int R, bool INV> __device__ __forceinline__ void bfly(cplx (&v)[R]) {
+    if constexpr (R == 2) bfly2<INV>(v[0], v[1]);
+    if constexpr (R == 4) bfly4<INV>(v[0], v[1], v[2], v[3]);
+    if constexpr (R == 8) bfly8<INV>(v);
+}
+
+// One radix-R stage on sub-blocks of length N = 2^lgN for every line of the tile.  The caller syncs.
+template <int R, bool INV>
+__device__ __forceinline__ void fft_stage(cplx* __restrict__ t, const AxisXf& a, int lgN) {
+    constexpr int lgR = (R == 8) ? 3 : (R == 4 ? 2 : 1);
+    const int lgs = lgN - lgR;            // s = N/R: stride between the R inputs of one butterfly
+    const int lgQ = a.lgL - lgR;          // butterflies per line
+    const int nwork = a.nB << (a.lgA + lgQ);
+    const int twsh = a.lgL - lgN;         // W_N^k = tw[k << twsh]
+    const int ss = a.strideK << lgs;
+    for (int w = threadIdx.x; w < nwork; w += blockDim.x) {
+        const int iA = w & ((1 << a.lgA) - 1);
+        const int q = (w >> a.lgA) & ((1 << lgQ) - 1);
+        const int iB = w >> (a.lgA + lgQ);
+        const int j = q & ((1 << lgs) - 1);
+        const int b = q >> lgs;
+        cplx* p = t + iA * a.strideA + iB * a.strideB + ((b << lgN) + j) * a.strideK;
+        cplx v[R];
+#pragma unroll
+        for (int m = 0; m < R; m++) v[m] = p[m * ss];
+        if (INV) {
+            if (lgs > 0) {
+#pragma unroll
+                for (int m = 1; m < R; m++) v[m] = cmulc(v[m], a.tw[(j * m) << twsh]);
+            }
+            bfly<R, true>(v);
+        } else {
+            bfly<R, false>(v);
+            if (lgs > 0) {
+#pragma unroll
+                for (int m = 1; m < R; m++) v[m] = cmul(v[m], a.tw[(j * m) << twsh]);
+            }
+        }
+#pragma unroll
+        for (int m = 0; m < R; m++) p[m * ss] = v[m];
+    }
+}
+
+template <bool INV> __device__ __forceinline__ void fft_stage_dispatch(cplx* t, const AxisXf& a, int lgN) {
+    const int lgR = stage_lg_radix(lgN);
+    if (lgR == 3) fft_stage<8, INV>(t, a, lgN);
+    else if (lgR == 2) fft_stage<4, INV>(t, a, lgN);
+    else fft_stage<2, INV>(t, a, lgN);
+}
+
+// Forward (DIF) transform of every line along the axis; ends with __syncthreads().
+__device__ __forceinline__ void fft_axis_forward(cplx* t, const AxisXf& a) {
+    int lgN = a.lgL;
+    while (lgN > 0) {
+        fft_stage_dispatch<false>(t, a, lgN);
+        __syncthreads();
+        lgN -= stage_lg_radix(lgN);
+    }
+}
+// Inverse (DIT) transform: the forward stages undone in reverse order; ends with __syncthreads().
+__device__ __forceinline__ void fft_axis_inverse(cplx* t, const AxisXf& a) {
+    int seq[8];
+    int n = 0, lgN = a.lgL;
+    while (lgN > 0) { seq[n++] = lgN; lgN -= stage_lg_radix(lgN); }
+    for (int k = n - 1; k >= 0; k--) {
+        fft_stage_dispatch<true>(t, a, seq[k]);
+        __syncthreads();
+    }
+}
+
+}  // namespace lgf

@@ -1,0 +1,636 @@
+// lgf_api.cu -- host side of the C ABI declared in include/lgf.h: context, workspace carving, FFT tables,
+// the iteration driver (device-side stop flag, CUDA-graph replay) and the boundary copies.
+// There is deliberately no CPU fallback: every compute entry point needs a CUDA device.
+#include "../../include/lgf.h"
+#include "kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace lgf;
+
+namespace {
+
+enum KernelSlot {
+    K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
+    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_NSLOTS
+};
+const char* const kKernelNames[LGF_MAX_KERNELS] = {
+    "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
+    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "", "", ""};
+
+constexpr int HIST_CAP = 1 << 16;
+constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
+constexpr int MAX_SMEM = 200 * 1024;
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {   // offsets into the workspace
+    size_t links, field, gbuf, partials, ctl, hist, tables, scratch, staging, total;
+    int n_partials;
+    long long stage_sites;
+};
+
+bool dims_ok(const int dims[4], int lg[4]) {
+    for (int k = 0; k < 4; k++) {
+        int L = dims[k];
+        if (L < 4 || L > 128 || (L & (L - 1))) return false;
+        int l = 0; while ((1 << l) < L) l++;
+        lg[k] = l;
+    }
+    if ((long long)dims[0] * dims[1] > 4096 || (long long)dims[2] * dims[3] > 4096) return false;
+    return true;
+}
+
+Layout make_layout(const int dims[4], int NC) {
+    Layout o;
+    const long long V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
+    size_t off = 0;
+    o.links = off; off = align_up(off + (size_t)V * 4 * NC * 16, 256);
+    o.field = off; off = align_up(off + (size_t)V * 4 * 16, 256);
+    o.gbuf = off; off = align_up(off + (size_t)V * 6 * 16, 256);
+    o.n_partials = (int)(V / 128);
+    o.partials = off; off = align_up(off + (size_t)o.n_partials * 16, 256);
+    o.ctl = off; off = align_up(off + sizeof(Ctl), 256);
+    o.hist = off; off = align_up(off + (size_t)HIST_CAP * 16, 256);
+    o.tables = off; off = align_up(off + 4 * 128 * 16 + 4 * 128 * 8, 256);
+    o.scratch = off; off = align_up(off + 256, 256);
+    o.stage_sites = V < STAGE_SITES ? V : STAGE_SITES;
+    o.staging = off; off = align_up(off + (size_t)o.stage_sites * 4 * 9 * 16, 256);
+    o.total = off;
+    return o;
+}
+
+// frequency index held at stored position p after the forward DIF stages of fft_tile.cuh
+int stored_freq(int p, int lgL) {
+    int n = 0, mult = 1, lgN = lgL;
+    while (lgN > 0) {
+        const int lgR = stage_lg_radix(lgN);
+        const int lgs = lgN - lgR;
+        const int m = p >> lgs;
+        p &= (1 << lgs) - 1;
+        n += m * mult;
+        mult <<= lgR;
+        lgN -= lgR;
+    }
+    return n;
+}
+
+}  // namespace
+
+struct lgf_ctx {
+    Geom G;
+    int NC;                 // 6 or 9
+    Layout lay;
+    char* ws;               // workspace base (device)
+    bool own_ws, own_stream;
+    cudaStream_t stream;
+    cplx *links, *field, *gbuf, *staging;
+    double2 *partials, *hist;
+    Ctl* ctl;
+    FftTables T;
+    Ctl* h_ctl;             // pinned
+    bool loaded;
+    // options
+    int opt_fuse, opt_store_g, opt_graph, opt_batch;
+    // derived launch parameters
+    int fft01_ncomp_fused_ok, fft01_ncomp, fft01_threads, fft23_lgC, fft23_S1, fft23_S2, fft23_threads;
+    size_t smem01_fused, smem01, smem23;
+    // graph cache
+    cudaGraphExec_t graph_exec;
+    int graph_key;
+    // profiling
+    int profiling;
+    cudaEvent_t ev0, ev1;
+    double prof_ms[LGF_MAX_KERNELS];
+    long long prof_n[LGF_MAX_KERNELS];
+    long long launches;
+    std::string err;
+    bool capturing;
+};
+
+namespace {
+
+#define CK(call)                                                                                           \
+    do {                                                                                                   \
+        cudaError_t e_ = (call);                                                                           \
+        if (e_ != cudaSuccess) {                                                                           \
+            char b_[512];                                                                                  \
+            snprintf(b_, sizeof b_, "%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            c->err = b_;                                                                                   \
+            return LGF_ERR_CUDA;                                                                           \
+        }                                                                                                  \
+    } while (0)
+
+// Launch bookkeeping: counts every kernel; in profiling mode brackets it with events and accumulates its time.
+struct LaunchScope {
+    lgf_ctx* c; int slot;
+    LaunchScope(lgf_ctx* c_, int s) : c(c_), slot(s) {
+        if (c->profiling && !c->capturing) cudaEventRecord(c->ev0, c->stream);
+    }
+    ~LaunchScope() {
+        if (!c->capturing) c->launches++;
+        if (c->profiling && !c->capturing) {
+            cudaEventRecord(c->ev1, c->stream);
+            cudaEventSynchronize(c->ev1);
+            float ms = 0; cudaEventElapsedTime(&ms, c->ev0, c->ev1);
+            c->prof_ms[slot] += ms; c->prof_n[slot]++;
+        }
+    }
+};
+
+template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
+    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+lgf_status setup_kernels(lgf_ctx* c) {
+    const Geom& G = c->G;
+    const int nP = G.L[0] * G.L[1];
+    auto smem01 = [&](int ncomp) { return (size_t)((G.L[0] + 1) * G.L[1] * ncomp + G.L[0] + G.L[1]) * 16; };
+    c->fft01_ncomp_fused_ok = smem01(4) <= (size_t)MAX_SMEM;
+    c->smem01_fused = smem01(4);
+    int ncomp = 4;
+    while (ncomp > 1 && smem01(ncomp) > 100 * 1024) ncomp >>= 1;
+    c->fft01_ncomp = ncomp;
+    c->smem01 = smem01(ncomp);
+    int th = nP * 4 / 8; if (th > 256) th = 256; if (th < 32) th = 32;
+    c->fft01_threads = th;
+    // axes 2,3: chunk of x0
+    const int n23 = G.L[2] * G.L[3];
+    int lgC = 3; if (lgC > G.lg[0]) lgC = G.lg[0];
+    while (lgC > 1 && ((size_t)n23 << lgC) * 16 > 64 * 1024) lgC--;
+    if (((size_t)n23 << lgC) * 16 > (size_t)MAX_SMEM - 8192) lgC = 0;
+    c->fft23_lgC = lgC;
+    const int C0 = 1 << lgC;
+    c->fft23_S1 = C0;
+    c->fft23_S2 = C0 * G.L[2] + (C0 < 8 ? C0 : 0);
+    c->smem23 = (size_t)(c->fft23_S2 * G.L[3] + G.L[2] + G.L[3]) * 16 + (size_t)(G.L[2] + G.L[3]) * 8;
+    if (c->smem23 > (size_t)MAX_SMEM || c->smem01 > (size_t)MAX_SMEM) return LGF_ERR_UNSUPPORTED;
+    th = (n23 << lgC) / 8; if (th > 256) th = 256; if (th < 32) th = 32;
+    c->fft23_threads = th;
+
+    CK(set_smem(k_fft01<MODE_FWD, 6>, c->smem01));
+    CK(set_smem(k_fft01<MODE_INV, 6>, c->smem01));
+    CK(set_smem(k_fft23_mid, c->smem23));
+    if (c->fft01_ncomp_fused_ok) {
+        CK(set_smem(k_fft01<MODE_DELTA_FWD, 6>, c->smem01_fused));
+        CK(set_smem(k_fft01<MODE_DELTA_FWD, 9>, c->smem01_fused));
+        CK(set_smem(k_fft01<MODE_INV_G, 6>, c->smem01_fused));
+    }
+    return LGF_OK;
+}
+
+lgf_status build_tables(lgf_ctx* c) {
+    std::vector<double> tw(4 * 128 * 2, 0.0), s(4 * 128, 0.0);
+    const long double pi = 3.141592653589793238462643383279502884L;
+    for (int mu = 0; mu < 4; mu++) {
+        const int L = c->G.L[mu];
+        for (int k = 0; k < L; k++) {
+            long double a = 2.0L * pi * (long double)k / (long double)L;
+            double cr = (double)cosl(a), sr = (double)sinl(a);
+            if ((4 * k) % L == 0) { const int q = 4 * k / L; const double cc[4] = {1, 0, -1, 0}, ss[4] = {0, 1, 0, -1}; cr = cc[q]; sr = ss[q]; }
+            tw[(mu * 128 + k) * 2] = cr; tw[(mu * 128 + k) * 2 + 1] = -sr;
+        }
+        for (int p = 0; p < L; p++) {
+            const int n = stored_freq(p, c->G.lg[mu]);
+            long double sn = sinl(pi * (long double)n / (long double)L);
+            s[mu * 128 + p] = (n == 0) ? 0.0 : (double)(4.0L * sn * sn);
+        }
+    }
+    char* tb = c->ws + c->lay.tables;
+    CK(cudaMemcpyAsync(tb, tw.data(), tw.size() * 8, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(tb + 4 * 128 * 16, s.data(), s.size() * 8, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    for (int mu = 0; mu < 4; mu++) {
+        c->T.tw[mu] = reinterpret_cast<const cplx*>(tb) + mu * 128;
+        c->T.s[mu] = reinterpret_cast<const double*>(tb + 4 * 128 * 16) + mu * 128;
+    }
+    return LGF_OK;
+}
+
+// ---- kernel launchers ---------------------------------------------------------------------------------------
+template <int NC> void launch_delta(lgf_ctx* c) {
+    LaunchScope ls(c, K_DELTA);
+    k_delta<NC><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, c->field, c->partials, c->G, c->ctl);
+}
+template <int MODE, int NC> void launch_fft01(lgf_ctx* c, int slot, double half_alpha) {
+    LaunchScope ls(c, slot);
+    const bool fused = (MODE == MODE_DELTA_FWD || MODE == MODE_INV_G);
+    const int ncomp = fused ? 4 : c->fft01_ncomp;
+    const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3] * (4 / ncomp));
+    k_fft01<MODE, NC><<<grid, c->fft01_threads, fused ? c->smem01_fused : c->smem01, c->stream>>>(
+        c->field, c->links, c->gbuf, c->partials, c->G, c->T, ncomp, half_alpha, c->ctl);
+}
+void launch_fft23(lgf_ctx* c) {
+    LaunchScope ls(c, K_FFT23_MID);
+    const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fft23_lgC));
+    k_fft23_mid<<<grid, c->fft23_threads, c->smem23, c->stream>>>(c->field, c->G, c->T, c->fft23_lgC, c->fft23_S1, c->fft23_S2,
+                                                                   16.0 / (double)c->G.V, c->ctl);
+}
+void launch_finalize(lgf_ctx* c, int n_partials) {
+    LaunchScope ls(c, K_FINALIZE);
+    k_finalize<<<1, 256, 0, c->stream>>>(c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V));
+}
+template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
+    LaunchScope ls(c, SG ? K_UPDATE_G : K_UPDATE_X);
+    k_update<NC, SG><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
+}
+
+bool use_fused(const lgf_ctx* c) { return c->opt_fuse && c->fft01_ncomp_fused_ok; }
+bool use_store_g(const lgf_ctx* c) { return c->opt_store_g && c->fft01_ncomp_fused_ok; }
+
+// S1 (+ pass A) and the reduction.  Returns the number of partials written.
+template <int NC> void enqueue_head(lgf_ctx* c) {
+    int np;
+    if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
+    else { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fft01<MODE_FWD, 6>(c, K_FFT01_FWD, 0.0); }
+    launch_finalize(c, np);
+}
+// pass B, pass C, update
+template <int NC> void enqueue_tail(lgf_ctx* c, double half_alpha) {
+    launch_fft23(c);
+    if (use_store_g(c)) { launch_fft01<MODE_INV_G, 6>(c, K_FFT01_INV_G, half_alpha); launch_update<NC, 1>(c, half_alpha); }
+    else { launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, half_alpha); launch_update<NC, 0>(c, half_alpha); }
+}
+void enqueue_body(lgf_ctx* c, double half_alpha) {
+    if (c->NC == 6) { enqueue_head<6>(c); enqueue_tail<6>(c, half_alpha); }
+    else { enqueue_head<9>(c); enqueue_tail<9>(c, half_alpha); }
+}
+
+lgf_status reset_ctl(lgf_ctx* c, double tol, int max_iter) {
+    Ctl h; memset(&h, 0, sizeof h);
+    h.theta_tol = tol; h.max_iter = max_iter; h.hist_cap = HIST_CAP;
+    *c->h_ctl = h;
+    CK(cudaMemcpyAsync(c->ctl, c->h_ctl, sizeof(Ctl), cudaMemcpyHostToDevice, c->stream));
+    return LGF_OK;
+}
+lgf_status read_ctl(lgf_ctx* c) {
+    CK(cudaMemcpyAsync(c->h_ctl, c->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return LGF_OK;
+}
+
+// Enqueue `nb` iteration bodies: a replay of the cached CUDA graph of opt_batch bodies when nb matches, else plain launches.
+lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
+    const bool graph_ok = c->opt_graph && !c->profiling && nb == c->opt_batch;
+    if (!graph_ok) {
+        for (int i = 0; i < nb; i++) enqueue_body(c, half_alpha);
+        CK(cudaGetLastError());
+        return LGF_OK;
+    }
+    // alpha enters the graph as a kernel argument, so it is part of the key
+    union { double d; unsigned long long u; } au; au.d = half_alpha;
+    const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (nb << 8);
+    if (!c->graph_exec || c->graph_key != key) {
+        if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+        cudaGraph_t g = nullptr;
+        CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+        c->capturing = true;   // LaunchScope neither counts nor times captured launches
+        for (int i = 0; i < nb; i++) enqueue_body(c, half_alpha);
+        c->capturing = false;
+        CK(cudaStreamEndCapture(c->stream, &g));
+        CK(cudaGraphInstantiate(&c->graph_exec, g, 0));
+        cudaGraphDestroy(g);
+        c->graph_key = key;
+    }
+    CK(cudaGraphLaunch(c->graph_exec, c->stream));
+    c->launches += (long long)nb * (use_fused(c) ? 5 : 6);
+    return LGF_OK;
+}
+
+// Shared driver of lgf_iterate (tol < 0: never) and lgf_fix.
+lgf_status run(lgf_ctx* c, double alpha, double tol, int max_iter, bool poll) {
+    lgf_status st = reset_ctl(c, tol, max_iter);
+    if (st != LGF_OK) return st;
+    const double ha = 0.5 * alpha;
+    long long bodies_left = (long long)max_iter + 1;
+    while (bodies_left > 0) {
+        int nb = (int)(bodies_left < c->opt_batch ? bodies_left : c->opt_batch);
+        st = enqueue_bodies(c, nb, ha);
+        if (st != LGF_OK) return st;
+        bodies_left -= nb;
+        if (poll || bodies_left == 0) {
+            st = read_ctl(c);
+            if (st != LGF_OK) return st;
+            if (c->h_ctl->done) break;
+        }
+    }
+    if (c->h_ctl->nonfinite) return LGF_ERR_NUMERIC;
+    return LGF_OK;
+}
+
+lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* wsp, size_t ws_bytes, void* stream, bool own, lgf_ctx** out) {
+    if (!dims || !out) return LGF_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (p != LGF_FP64 && p != LGF_FP32) return LGF_ERR_INVALID_ARG;
+    if (s != LGF_STORE_12 && s != LGF_STORE_18) return LGF_ERR_INVALID_ARG;
+    for (int k = 0; k < 4; k++) if (dims[k] < 1) return LGF_ERR_INVALID_ARG;
+    if (p != LGF_FP64) return LGF_ERR_UNSUPPORTED;
+    int lg[4];
+    if (!dims_ok(dims, lg)) return LGF_ERR_UNSUPPORTED;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return LGF_ERR_CUDA;   // no CPU fallback
+
+    lgf_ctx* c = new (std::nothrow) lgf_ctx();
+    if (!c) return LGF_ERR_OOM;
+    int shv = 0;
+    for (int k = 0; k < 4; k++) { c->G.L[k] = dims[k]; c->G.lg[k] = lg[k]; c->G.sh[k] = shv; shv += lg[k]; }
+    c->G.V = 1LL << shv;
+    c->NC = (s == LGF_STORE_12) ? 6 : 9;
+    c->lay = make_layout(dims, c->NC);
+    c->own_ws = own; c->own_stream = own;
+    c->loaded = false;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8;
+    c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
+    c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr;
+    memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
+
+    auto fail = [&](lgf_status st) { lgf_destroy(c); return st; };
+    if (own) {
+        if (cudaMalloc(&c->ws, c->lay.total) != cudaSuccess) { cudaGetLastError(); return fail(LGF_ERR_OOM); }
+        if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(LGF_ERR_CUDA);
+    } else {
+        if (!wsp || ((size_t)wsp & 255) || ws_bytes < c->lay.total) return fail(LGF_ERR_INVALID_ARG);
+        c->ws = static_cast<char*>(wsp);
+        c->stream = static_cast<cudaStream_t>(stream);
+    }
+    c->links = reinterpret_cast<cplx*>(c->ws + c->lay.links);
+    c->field = reinterpret_cast<cplx*>(c->ws + c->lay.field);
+    c->gbuf = reinterpret_cast<cplx*>(c->ws + c->lay.gbuf);
+    c->staging = reinterpret_cast<cplx*>(c->ws + c->lay.staging);
+    c->partials = reinterpret_cast<double2*>(c->ws + c->lay.partials);
+    c->hist = reinterpret_cast<double2*>(c->ws + c->lay.hist);
+    c->ctl = reinterpret_cast<Ctl*>(c->ws + c->lay.ctl);
+    if (cudaHostAlloc(&c->h_ctl, sizeof(Ctl), cudaHostAllocDefault) != cudaSuccess) return fail(LGF_ERR_OOM);
+    if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) return fail(LGF_ERR_CUDA);
+    lgf_status st = setup_kernels(c);
+    if (st != LGF_OK) return fail(st);
+    st = build_tables(c);
+    if (st != LGF_OK) return fail(st);
+    st = reset_ctl(c, -1.0, 0);
+    if (st != LGF_OK) return fail(st);
+    *out = c;
+    return LGF_OK;
+}
+
+lgf_status load_from_device_chunks(lgf_ctx* c, const double* src, bool src_is_host) {
+    const long long V = c->G.V, S = c->lay.stage_sites;
+    for (long long off = 0; off < V; off += S) {
+        const long long n = (V - off < S) ? V - off : S;
+        const cplx* aos;
+        if (src_is_host) {
+            CK(cudaMemcpyAsync(c->staging, src + off * 72, (size_t)n * 576, cudaMemcpyHostToDevice, c->stream));
+            aos = c->staging;
+        } else aos = reinterpret_cast<const cplx*>(src) + off * 36;
+        {
+            LaunchScope ls(c, K_LAYOUT_IN);
+            const unsigned grid = (unsigned)((n * 4 + 255) / 256);
+            if (c->NC == 6) k_layout_in<6><<<grid, 256, 0, c->stream>>>(aos, c->links, V, off, n);
+            else k_layout_in<9><<<grid, 256, 0, c->stream>>>(aos, c->links, V, off, n);
+        }
+        CK(cudaGetLastError());
+    }
+    CK(cudaStreamSynchronize(c->stream));
+    c->loaded = true;
+    return LGF_OK;
+}
+
+lgf_status get_to_chunks(lgf_ctx* c, double* dst, bool dst_is_host) {
+    const long long V = c->G.V, S = c->lay.stage_sites;
+    for (long long off = 0; off < V; off += S) {
+        const long long n = (V - off < S) ? V - off : S;
+        cplx* aos = dst_is_host ? c->staging : reinterpret_cast<cplx*>(dst) + off * 36;
+        {
+            LaunchScope ls(c, K_LAYOUT_OUT);
+            const unsigned grid = (unsigned)((n * 4 + 255) / 256);
+            if (c->NC == 6) k_layout_out<6><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n);
+            else k_layout_out<9><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n);
+        }
+        CK(cudaGetLastError());
+        if (dst_is_host) CK(cudaMemcpyAsync(dst + off * 72, c->staging, (size_t)n * 576, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CK(cudaStreamSynchronize(c->stream));
+    return LGF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t lgf_workspace_bytes(const int dims[4], lgf_precision p, lgf_storage s) {
+    int lg[4];
+    if (!dims || p != LGF_FP64 || (s != LGF_STORE_12 && s != LGF_STORE_18) || !dims_ok(dims, lg)) return 0;
+    return make_layout(dims, s == LGF_STORE_12 ? 6 : 9).total;
+}
+
+lgf_status lgf_create(const int dims[4], lgf_precision p, lgf_storage s, lgf_ctx** out) {
+    return create_impl(dims, p, s, nullptr, 0, nullptr, true, out);
+}
+lgf_status lgf_create_ex(const int dims[4], lgf_precision p, lgf_storage s, void* ws, size_t bytes, void* stream, lgf_ctx** out) {
+    return create_impl(dims, p, s, ws, bytes, stream, false, out);
+}
+
+void lgf_destroy(lgf_ctx* c) {
+    if (!c) return;
+    if (c->stream) cudaStreamSynchronize(c->stream);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->h_ctl) cudaFreeHost(c->h_ctl);
+    if (c->own_ws && c->ws) cudaFree(c->ws);
+    if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
+    delete c;
+}
+
+lgf_status lgf_load_links(lgf_ctx* c, const double* host_links) {
+    if (!c || !host_links) return LGF_ERR_INVALID_ARG;
+    return load_from_device_chunks(c, host_links, true);
+}
+lgf_status lgf_load_links_device(lgf_ctx* c, const double* dev_links) {
+    if (!c || !dev_links) return LGF_ERR_INVALID_ARG;
+    return load_from_device_chunks(c, dev_links, false);
+}
+lgf_status lgf_get_links(lgf_ctx* c, double* host_links) {
+    if (!c || !host_links) return LGF_ERR_INVALID_ARG;
+    if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    return get_to_chunks(c, host_links, true);
+}
+lgf_status lgf_get_links_device(lgf_ctx* c, double* dev_links) {
+    if (!c || !dev_links) return LGF_ERR_INVALID_ARG;
+    if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    return get_to_chunks(c, dev_links, false);
+}
+
+lgf_status lgf_iterate(lgf_ctx* c, int n, double alpha, double* F, double* theta) {
+    if (!c || n < 0 || !(alpha > 0.0) || !std::isfinite(alpha)) return LGF_ERR_INVALID_ARG;
+    if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    lgf_status st = run(c, alpha, -1.0, n, false);
+    if (st != LGF_OK) return st;
+    if (F) *F = c->h_ctl->F;
+    if (theta) *theta = c->h_ctl->theta;
+    return LGF_OK;
+}
+
+lgf_status lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int* n_iter, double* F, double* theta) {
+    if (!c || max_iter < 0 || !(alpha > 0.0) || !std::isfinite(alpha) || !(theta_tol >= 0.0)) return LGF_ERR_INVALID_ARG;
+    if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    lgf_status st = run(c, alpha, theta_tol, max_iter, true);
+    if (st != LGF_OK) return st;
+    if (n_iter) *n_iter = c->h_ctl->iters;
+    if (F) *F = c->h_ctl->F;
+    if (theta) *theta = c->h_ctl->theta;
+    return c->h_ctl->converged ? LGF_OK : LGF_NOT_CONVERGED;
+}
+
+lgf_status lgf_measure(lgf_ctx* c, double* F, double* theta, double* plaq) {
+    if (!c) return LGF_ERR_INVALID_ARG;
+    if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    lgf_status st = reset_ctl(c, -1.0, 0);
+    if (st != LGF_OK) return st;
+    if (c->NC == 6) launch_delta<6>(c); else launch_delta<9>(c);
+    launch_finalize(c, (int)(c->G.V / 128));
+    {
+        LaunchScope ls(c, K_PLAQUETTE);
+        if (c->NC == 6) k_plaquette<6><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, c->partials, c->G);
+        else k_plaquette<9><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, c->partials, c->G);
+    }
+    double* sums = reinterpret_cast<double*>(c->ws + c->lay.scratch);
+    {
+        LaunchScope ls(c, K_MISC);
+        k_sum_partials<<<1, 256, 0, c->stream>>>(c->partials, (int)(c->G.V / 128), sums);
+    }
+    CK(cudaGetLastError());
+    double h[2];
+    CK(cudaMemcpyAsync(h, sums, 16, cudaMemcpyDeviceToHost, c->stream));
+    st = read_ctl(c);
+    if (st != LGF_OK) return st;
+    if (c->h_ctl->nonfinite) return LGF_ERR_NUMERIC;
+    if (F) *F = c->h_ctl->F;
+    if (theta) *theta = c->h_ctl->theta;
+    if (plaq) *plaq = h[0] / (18.0 * (double)c->G.V);
+    return LGF_OK;
+}
+
+lgf_status lgf_get_history(lgf_ctx* c, double* hist, int capacity, int* n_out) {
+    if (!c || !hist || capacity < 0 || !n_out) return LGF_ERR_INVALID_ARG;
+    int n = c->h_ctl->n_meas; if (n > HIST_CAP) n = HIST_CAP; if (n > capacity) n = capacity;
+    if (n > 0) {
+        CK(cudaMemcpyAsync(hist, c->hist, (size_t)n * 16, cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+    }
+    *n_out = n;
+    return LGF_OK;
+}
+
+lgf_status lgf_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host_field) {
+    if (!c || !host_field) return LGF_ERR_INVALID_ARG;
+    if (which != LGF_FIELD_DELTA && which != LGF_FIELD_X && which != LGF_FIELD_G) return LGF_ERR_INVALID_ARG;
+    if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    lgf_status st = reset_ctl(c, -1.0, 1 << 30);
+    if (st != LGF_OK) return st;
+    const double ha = 0.5 * alpha;
+    bool g_from_buf = false;
+    if (which == LGF_FIELD_DELTA) {
+        if (c->NC == 6) launch_delta<6>(c); else launch_delta<9>(c);
+    } else {
+        if (c->NC == 6) enqueue_head<6>(c); else enqueue_head<9>(c);
+        launch_fft23(c);
+        if (which == LGF_FIELD_G && use_store_g(c)) { launch_fft01<MODE_INV_G, 6>(c, K_FFT01_INV_G, ha); g_from_buf = true; }
+        else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, ha);
+    }
+    CK(cudaGetLastError());
+    const long long V = c->G.V;
+    const long long S = c->lay.stage_sites * 4;   // staging holds 4*9 complex per site -> 4x as many 3x3 matrices
+    for (long long off = 0; off < V; off += S) {
+        const long long n = (V - off < S) ? V - off : S;
+        {
+            LaunchScope ls(c, K_MISC);
+            const unsigned grid = (unsigned)((n + 255) / 256);
+            if (which == LGF_FIELD_G) k_unpack_g<<<grid, 256, 0, c->stream>>>(g_from_buf ? c->gbuf : c->field, g_from_buf ? 0 : 1, ha, c->staging, V, off, n);
+            else k_unpack_field<<<grid, 256, 0, c->stream>>>(c->field, c->staging, V, off, n);
+        }
+        CK(cudaGetLastError());
+        CK(cudaMemcpyAsync(host_field + off * 18, c->staging, (size_t)n * 144, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CK(cudaStreamSynchronize(c->stream));
+    return LGF_OK;
+}
+
+lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
+    if (!c) return LGF_ERR_INVALID_ARG;
+    switch (opt) {
+        case LGF_OPT_FUSE_DELTA_FFT: c->opt_fuse = value ? 1 : 0; break;
+        case LGF_OPT_STORE_G: c->opt_store_g = value ? 1 : 0; break;
+        case LGF_OPT_GRAPH: c->opt_graph = value ? 1 : 0; break;
+        case LGF_OPT_BATCH: if (value < 1 || value > 1024) return LGF_ERR_INVALID_ARG; c->opt_batch = value; break;
+        default: return LGF_ERR_INVALID_ARG;
+    }
+    return LGF_OK;
+}
+lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
+    if (!c || !value) return LGF_ERR_INVALID_ARG;
+    switch (opt) {
+        case LGF_OPT_FUSE_DELTA_FFT: *value = use_fused(c); break;
+        case LGF_OPT_STORE_G: *value = use_store_g(c); break;
+        case LGF_OPT_GRAPH: *value = c->opt_graph; break;
+        case LGF_OPT_BATCH: *value = c->opt_batch; break;
+        default: return LGF_ERR_INVALID_ARG;
+    }
+    return LGF_OK;
+}
+
+lgf_status lgf_set_profiling(lgf_ctx* c, int on) {
+    if (!c) return LGF_ERR_INVALID_ARG;
+    c->profiling = on ? 1 : 0;
+    memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
+    return LGF_OK;
+}
+lgf_status lgf_get_profile(lgf_ctx* c, double ms[LGF_MAX_KERNELS], long long n[LGF_MAX_KERNELS]) {
+    if (!c || !ms || !n) return LGF_ERR_INVALID_ARG;
+    memcpy(ms, c->prof_ms, sizeof c->prof_ms); memcpy(n, c->prof_n, sizeof c->prof_n);
+    return LGF_OK;
+}
+const char* lgf_kernel_name(int slot) { return (slot >= 0 && slot < LGF_MAX_KERNELS) ? kKernelNames[slot] : ""; }
+long long lgf_launch_count(lgf_ctx* c) { return c ? c->launches : 0; }
+
+lgf_status lgf_copy_peak(void* dst, const void* src, size_t bytes, int reps, void* stream, double* ms) {
+    if (!dst || !src || !ms || reps < 1 || bytes < 16 || (bytes & 15)) return LGF_ERR_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return LGF_ERR_CUDA;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const long long n = (long long)(bytes / 16);
+    const unsigned grid = (unsigned)(sms * 8);
+    k_copy<<<grid, 256, 0, s>>>((double2*)dst, (const double2*)src, n);   // warm-up
+    cudaEventRecord(a, s);
+    for (int i = 0; i < reps; i++) k_copy<<<grid, 256, 0, s>>>((double2*)dst, (const double2*)src, n);
+    cudaEventRecord(b, s);
+    cudaError_t e = cudaEventSynchronize(b);
+    float t = 0; cudaEventElapsedTime(&t, a, b);
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return LGF_ERR_CUDA;
+    *ms = (double)t / reps;
+    return LGF_OK;
+}
+
+const char* lgf_status_string(lgf_status s) {
+    switch (s) {
+        case LGF_OK: return "ok";
+        case LGF_ERR_INVALID_ARG: return "invalid argument";
+        case LGF_ERR_UNSUPPORTED: return "unsupported lattice size or precision";
+        case LGF_ERR_OOM: return "out of memory";
+        case LGF_ERR_CUDA: return "CUDA error (or no CUDA device: there is no CPU fallback)";
+        case LGF_ERR_NOT_LOADED: return "links not loaded";
+        case LGF_ERR_NUMERIC: return "theta or F is not finite";
+        case LGF_NOT_CONVERGED: return "max_iter reached before theta < theta_tol";
+    }
+    return "unknown status";
+}
+const char* lgf_last_error(lgf_ctx* c) { return c ? c->err.c_str() : ""; }
+
+}  // extern "C"

@@ -1,0 +1,136 @@
+// su3.cuh -- register-level complex 3x3 algebra for the gauge-fixing kernels (fp64, sm_100a).
+// Complex numbers are double2 (x = re, y = im).  Everything is __forceinline__ so that unused rows
+// and entries are dead-code eliminated in each kernel.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace lgf {
+
+typedef double2 cplx;
+
+__device__ __forceinline__ cplx mk(double a, double b) { return make_double2(a, b); }
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return mk(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return mk(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cconj(cplx a) { return mk(a.x, -a.y); }
+__device__ __forceinline__ cplx cscale(cplx a, double s) { return mk(a.x * s, a.y * s); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+// a * conj(b)
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b) { return mk(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }
+// conj(a) * b
+__device__ __forceinline__ cplx ccmul(cplx a, cplx b) { return mk(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }
+// c + a*b
+__device__ __forceinline__ cplx cfma(cplx a, cplx b, cplx c) {
+    return mk(fma(a.x, b.x, fma(-a.y, b.y, c.x)), fma(a.x, b.y, fma(a.y, b.x, c.y)));
+}
+// c + a*conj(b)
+__device__ __forceinline__ cplx cfmac(cplx a, cplx b, cplx c) {
+    return mk(fma(a.x, b.x, fma(a.y, b.y, c.x)), fma(a.y, b.x, fma(-a.x, b.y, c.y)));
+}
+// c - a*b
+__device__ __forceinline__ cplx cfnma(cplx a, cplx b, cplx c) {
+    return mk(fma(-a.x, b.x, fma(a.y, b.y, c.x)), fma(-a.x, b.y, fma(-a.y, b.x, c.y)));
+}
+__device__ __forceinline__ double cnorm2(cplx a) { return fma(a.x, a.x, a.y * a.y); }
+
+// Row 2 of a special unitary matrix from rows 0,1: row2 = conj(row0 x row1)  ("12 real
+// number representation").  u[0..2] = row 0, u[3..5] = row 1, u[6..8] = row 2.
+__device__ __forceinline__ void third_row(cplx (&u)[9]) {
+    u[6] = cconj(cfnma(u[2], u[4], cmul(u[1], u[5])));
+    u[7] = cconj(cfnma(u[0], u[5], cmul(u[2], u[3])));
+    u[8] = cconj(cfnma(u[1], u[3], cmul(u[0], u[4])));
+}
+
+// 128-bit loads/stores of one complex double
+__device__ __forceinline__ cplx ldg2(const cplx* p) { return __ldg(p); }
+
+// Load link (x, mu) from the structure-of-arrays store: entry c of direction mu is the V-array at
+// links + (mu*NC + c)*V, NC = 6 (12-real: rows 0,1) or 9 (18-real).  Row 2 is rebuilt for NC = 6.
+template <int NC>
+__device__ __forceinline__ void load_link(const cplx* __restrict__ links, long long V, int mu, long long x, cplx (&u)[9]) {
+    const cplx* p = links + (long long)(mu * NC) * V + x;
+#pragma unroll
+    for (int c = 0; c < NC; c++) u[c] = ldg2(p + (long long)c * V);
+    if (NC == 6) third_row(u);
+}
+template <int NC>
+__device__ __forceinline__ void store_link(cplx* __restrict__ links, long long V, int mu, long long x, const cplx (&u)[9]) {
+    cplx* p = links + (long long)(mu * NC) * V + x;
+#pragma unroll
+    for (int c = 0; c < NC; c++) p[(long long)c * V] = u[c];
+}
+
+// S3: g = rowGramSchmidt(M), M = 1 + (alpha/2) X, X given by its packed independent components
+//   f0 = X01, f1 = X02, f2 = X12, f3 = (Im X00, Im X11);  X_ji = -conj(X_ij), X anti-Hermitian traceless.
+// Only rows 0 and 1 of M enter; row 2 of g is conj(u x v).  ha = alpha/2.   [north_star step 3]
+__device__ __forceinline__ void build_g(cplx f0, cplx f1, cplx f2, cplx f3, double ha, cplx (&g)[9]) {
+    cplx m00 = mk(1.0, ha * f3.x), m01 = cscale(f0, ha), m02 = cscale(f1, ha);
+    cplx m10 = mk(-ha * f0.x, ha * f0.y), m11 = mk(1.0, ha * f3.y), m12 = cscale(f2, ha);
+    double n0 = cnorm2(m00) + cnorm2(m01) + cnorm2(m02);
+    double r0 = 1.0 / sqrt(n0);
+    g[0] = cscale(m00, r0); g[1] = cscale(m01, r0); g[2] = cscale(m02, r0);
+    // <u, M1> = sum_j conj(u_j) M1_j
+    cplx ip = ccmul(g[0], m10);
+    ip = cadd(ip, ccmul(g[1], m11));
+    ip = cadd(ip, ccmul(g[2], m12));
+    cplx v0 = cfnma(ip, g[0], m10), v1 = cfnma(ip, g[1], m11), v2 = cfnma(ip, g[2], m12);
+    double n1 = cnorm2(v0) + cnorm2(v1) + cnorm2(v2);
+    double r1 = 1.0 / sqrt(n1);
+    g[3] = cscale(v0, r1); g[4] = cscale(v1, r1); g[5] = cscale(v2, r1);
+    third_row(g);
+}
+
+// S4 for one link: r = g * U * gp^dag.  NROWS = 2 computes rows 0,1 only (12-real storage).
+template <int NROWS>
+__device__ __forceinline__ void rotate_link(const cplx (&g)[9], const cplx (&u)[9], const cplx (&gp)[9], cplx (&r)[9]) {
+#pragma unroll
+    for (int i = 0; i < NROWS; i++) {
+        cplx t[3];
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            cplx s = cmul(g[3 * i + 0], u[j]);
+            s = cfma(g[3 * i + 1], u[3 + j], s);
+            s = cfma(g[3 * i + 2], u[6 + j], s);
+            t[j] = s;
+        }
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            cplx s = cmulc(t[0], gp[3 * j + 0]);
+            s = cfmac(t[1], gp[3 * j + 1], s);
+            s = cfmac(t[2], gp[3 * j + 2], s);
+            r[3 * i + j] = s;
+        }
+    }
+}
+
+// Lattice geometry: every L_mu is a power of two, x = x0 + L0*(x1 + L1*(x2 + L2*x3)).
+struct Geom {
+    int L[4];
+    int lg[4];    // log2 L
+    int sh[4];    // log2 stride of axis mu (sum of lg of lower axes)
+    long long V;
+};
+__device__ __forceinline__ int coord(const Geom& G, long long x, int mu) { return (int)(x >> G.sh[mu]) & (G.L[mu] - 1); }
+__device__ __forceinline__ long long fwd(const Geom& G, long long x, int mu) {
+    int c = coord(G, x, mu);
+    return (c == G.L[mu] - 1) ? x - ((long long)(G.L[mu] - 1) << G.sh[mu]) : x + (1LL << G.sh[mu]);
+}
+__device__ __forceinline__ long long bwd(const Geom& G, long long x, int mu) {
+    int c = coord(G, x, mu);
+    return (c == 0) ? x + ((long long)(G.L[mu] - 1) << G.sh[mu]) : x - (1LL << G.sh[mu]);
+}
+
+// Device-resident control block shared by all kernels of one context.
+struct Ctl {
+    double F, theta;       // last measurement (S1)
+    double theta_tol;      // S5: stop when theta < theta_tol; negative = never
+    int max_iter;          // stop after this many updates
+    int done;              // 1: every later kernel exits at once, the link state is frozen
+    int converged;         // 1: stopped by theta < theta_tol
+    int iters;             // link updates applied so far
+    int nonfinite;         // theta or F not finite
+    int n_meas;            // measurements made (index into the history)
+    int hist_cap;
+    unsigned int ticket;   // block counter of the fused reduction
+};
+
+}  // namespace lgf
