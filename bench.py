@@ -1,0 +1,326 @@
+#!/usr/bin/env python
+"""bench.py -- Fourier-accelerated Landau gauge-fixing throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2b] [--inner 100] [--impl ours|reference]
+
+A "step" is one lgf_iterate(inner, alpha = 0.08) call on one resident lattice: `inner` full iterations
+(S1 Delta/theta/F, S2 FFT + p2max/p2 filter + inverse FFT, S3 g build, S4 link update, S5 bookkeeping) plus the
+closing measurement (reading A5).  metric = iterations/s at 32^4 SU(3) fp64, 12-real storage (config C2b of
+BASELINE.json configs[2]); value = N * K * inner / (max over ranks of the CUDA-event time of the K steps).
+N > 1: one independent configuration per GPU (replicas, weak scaling), no collective on the
+data path.  The JSON line also carries: e2e (host buffers through the C ABI), roofline (dominant kernel, live
+CUDA-event timing), kernels (every kernel), iteration (whole-iteration HBM fraction), time_to_theta (lgf_fix),
+cpu_baseline (the oracle timed on the host cores), clocks, gpu_launches.
+
+--impl reference times the CPU oracle (oracle/, radix-2 FFT mode) on the host cores on the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+ALPHA = 0.08
+THETA_TOL = 1e-15
+METRIC = "FA gauge-fix iterations/s at 32^4 SU(3) fp64"
+UNIT = "iterations/s"
+
+# Algorithmic HBM bytes per site per launch of each hot-path kernel:
+# links cost 16*NC bytes per direction (NC = 6 two-row, 9 full), the packed field 64 B/site.
+def kernel_bytes_per_site(nc: int) -> dict:
+    lk = 4 * nc * 16
+    return {
+        "k_fft01_delta_fwd": lk + 64,        # read own links once (backward neighbours: cache), write Delta~ field
+        "k_delta": lk + 64,
+        "k_fft01_fwd": 128,
+        "k_fft23_mid": 128,                  # read + write the field (forward, filter, inverse on chip)
+        "k_fft01_inv": 128,
+        "k_fft01_inv_g": 64 + 96,
+        "k_update_x": 64 + 2 * lk,           # read X once (neighbours: cache), read + write links
+        "k_update_g": 96 + 2 * lk,
+        "k_finalize": 0,
+    }
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                       "-lms", "200"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        time.sleep(0.25)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name).read().strip().splitlines() if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for k, nm in enumerate(names):
+                if len(r) > 3 + k and r[3 + k].strip().lower() == "active":
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_links(workload: str, rank: int):
+    import ensembles as E
+    cfg = dict(E.CONFIGS[workload])
+    if cfg["kind"] == "pure_gauge":
+        U = E.pure_gauge(cfg["dims"], cfg["seed"], cfg.get("stream", 0) + 16 * rank)
+    else:
+        U = E.noisy(cfg["dims"], cfg["seed"], cfg["eps"], cfg.get("stream", 0) + 16 * rank)   # rank r: its own configuration
+    return U, cfg
+
+
+def dims_name(dims):
+    return "x".join(str(d) for d in dims)
+
+
+# ---------------------------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    U, cfg = make_links(args.workload, 0)
+    dims, storage = cfg["dims"], cfg["storage"]
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    o.load(U)
+    V = int(np.prod(dims))
+    per_step = max(1, min(args.inner, int(round(2.0e6 / V)) or 1))     # bounded sample: ~2 iterations at 32^4
+    for _ in range(args.warmup):
+        o.iterate(1, ALPHA)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.iterate(per_step, ALPHA)
+    dt = time.perf_counter() - t0
+    val = args.steps * per_step / dt
+    cores = oracle.num_threads()
+    sample = f"{per_step} iteration(s) per step of {args.workload} ({dims_name(dims)}, {storage}-real), oracle radix-2 FFT mode"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, alpha=0.08", "iterations_per_step": per_step},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import paper_1301_3460_b200 as lgf
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    U, cfg = make_links(args.workload, rank)
+    dims, storage = cfg["dims"], cfg["storage"]
+    V = int(np.prod(dims))
+    nc = 6 if storage == 12 else 9
+    inner = args.inner
+    # pinned host copies for the end-to-end leg
+    h_in = torch.from_numpy(U.view(np.float64).reshape(-1)).pin_memory()
+    h_out = torch.empty_like(h_in).pin_memory()
+    del U
+
+    gf = lgf.GaugeFixer(dims, storage)
+    gf.load_links(h_in.numpy())
+    _, _, plaq = gf.measure()
+    stream = gf.stream            # the context's own torch stream: every kernel and copy is ordered on it
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            fn()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        barrier()
+        return max_over_ranks(e0.elapsed_time(e1))       # ms
+
+    # ---- device-resident throughput (links already in HBM)
+    sampler = ClockSampler(local) if rank == 0 else None
+    n0 = gf.launch_count()
+    res = {}
+
+    def step():
+        res["F"], res["theta"] = gf.iterate(inner, ALPHA)
+
+    for _ in range(args.warmup):
+        step()
+    n_before = gf.launch_count()
+    ms = timed(step, args.steps, 0)
+    launches = gf.launch_count() - n_before
+    clocks = sampler.stop() if sampler else None
+    value = world * args.steps * inner / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers: H2D of the links, the iterations, D2H of the result
+    def step_e2e():
+        gf.load_links(h_in.numpy())
+        gf.iterate(inner, ALPHA)
+        gf.get_links(h_out.numpy().view(np.complex128).reshape(V, 4, 3, 3))
+
+    e2e_steps = max(2, min(args.steps, 5))
+    ms_e2e = timed(step_e2e, e2e_steps, 1)
+    e2e_value = world * e2e_steps * inner / (ms_e2e * 1e-3)
+
+    line = None
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        kb = kernel_bytes_per_site(nc)
+        # ---- per-kernel device times: CUDA events around every launch on the library's stream (plain launches)
+        gf.load_links(h_in.numpy())
+        gf.iterate(10, ALPHA)
+        gf.set_profiling(True)
+        gf.iterate(inner, ALPHA)
+        prof = gf.get_profile()
+        gf.set_profiling(False)
+        kernels = {}
+        tot_ms = sum(v["ms"] for v in prof.values())
+        for name, v in prof.items():
+            us = v["ms"] / v["launches"] * 1e3
+            b = kb.get(name, 0) * V
+            kernels[name] = {"launches": v["launches"], "avg_us": us, "share": v["ms"] / tot_ms,
+                             "bytes_per_launch": b, "gbs": b / us / 1e3 if us > 0 else None,
+                             "frac": (b / us / 1e3) / peak if us > 0 else None}
+        dom = max((k for k in kernels if kb.get(k, 0) > 0), key=lambda k: prof[k]["ms"])
+        try:
+            copy_gbs = lgf.copy_peak_gbs(1 << 30, 10)
+        except Exception:
+            copy_gbs = None
+        iter_bytes = sum(kb[k] for k in ("k_fft01_delta_fwd", "k_fft23_mid", "k_fft01_inv", "k_update_x")) * V \
+            if (gf.get_option(lgf.LGF_OPT_FUSE_DELTA_FFT) and not gf.get_option(lgf.LGF_OPT_STORE_G)) else \
+            sum(kb[k] * V for k in kernels if k in kb)
+        it_s_1 = value / world
+        # ---- time to theta < 1e-15 (lgf_fix, links resident, all syncs included)
+        gf.load_links(h_in.numpy())
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        r = gf.fix(ALPHA, THETA_TOL, 100000)
+        torch.cuda.synchronize()
+        ttt = {"ms": (time.perf_counter() - t0) * 1e3, "n_iter": r["n_iter"], "status": r["status"], "F": r["F"],
+               "theta": r["theta"], "plaquette": plaq, "ensemble": args.workload}
+        # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            import oracle
+            o = oracle.Oracle(dims, storage, fft_mode=1)
+            o.load(h_in.numpy().view(np.complex128).reshape(V, 4, 3, 3))
+            n_cpu = max(1, int(round(10.0 * (1 << 20) / V)))
+            o.iterate(1, ALPHA)
+            t0 = time.perf_counter()
+            o.iterate(n_cpu, ALPHA)
+            dt = time.perf_counter() - t0
+            cpu = {"value": n_cpu / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                   "sample": f"{n_cpu} iterations of {args.workload} ({dims_name(dims)}, {storage}-real), oracle radix-2 FFT mode, after 1 warm-up"}
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, eps={cfg.get('eps')}, seed={cfg['seed']}, alpha=0.08",
+                       "iterations_per_step": inner, "l2": "inputs larger than L2 (links %.0f MB + field %.0f MB per GPU)" % (V * nc * 64 / 1e6, V * 64 / 1e6),
+                       "parallelism": "replicas" if world > 1 else "single"},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": V * 576, "d2h_bytes_per_step": V * 576 + 16,
+                    "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                         "frac": kernels[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                         "bytes_per_launch": kernels[dom]["bytes_per_launch"], "avg_us": kernels[dom]["avg_us"],
+                         "copy_kernel_gbs": copy_gbs},
+            "iteration": {"bytes_per_site": iter_bytes // V, "bytes": iter_bytes, "gbs": iter_bytes * it_s_1 / 1e9,
+                          "frac_of_measured": iter_bytes * it_s_1 / 1e9 / peak, "frac_of_spec_8000": iter_bytes * it_s_1 / 1e9 / 8000.0},
+            "kernels": kernels,
+            "time_to_theta": ttt,
+            "cpu_baseline": cpu,
+            "final": {"F": res["F"], "theta": res["theta"]},
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--inner", type=int, default=100, help="iterations per step (one lgf_iterate call)")
+    ap.add_argument("--workload", default="C2b", help="ensemble name from ensembles.CONFIGS (C2b = 32^4, eps 0.35)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                   # timing rule: at least 3 warm-up steps
+    sys.exit(run_reference(args) if args.impl == "reference" else run_ours(args))
+
+
+if __name__ == "__main__":
+    main()

@@ -76,8 +76,8 @@ class Oracle:
             raise ValueError("orc_create failed")
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            lib().orc_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.orc_destroy(self._h)
             self._h = None
 
     def set_variant(self, accel: int = 1, exp_sign: int = -1):

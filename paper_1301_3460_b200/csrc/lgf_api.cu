@@ -53,7 +53,8 @@ Layout make_layout(const int dims[4], int NC) {
     o.links = off; off = align_up(off + (size_t)V * 4 * NC * 16, 256);
     o.field = off; off = align_up(off + (size_t)V * 4 * 16, 256);
     o.gbuf = off; off = align_up(off + (size_t)V * 6 * 16, 256);
-    o.n_partials = (int)(V / 128);
+    o.n_partials = (int)(V / 128);                       // k_delta / k_plaquette: one per 128-site block
+    if (o.n_partials < dims[2] * dims[3]) o.n_partials = dims[2] * dims[3];   // fused pass A: one per (x2,x3) plane
     o.partials = off; off = align_up(off + (size_t)o.n_partials * 16, 256);
     o.ctl = off; off = align_up(off + sizeof(Ctl), 256);
     o.hist = off; off = align_up(off + (size_t)HIST_CAP * 16, 256);
@@ -276,7 +277,8 @@ lgf_status read_ctl(lgf_ctx* c) {
 
 // Enqueue `nb` iteration bodies: a replay of the cached CUDA graph of opt_batch bodies when nb matches, else plain launches.
 lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
-    const bool graph_ok = c->opt_graph && !c->profiling && nb == c->opt_batch;
+    // the legacy default stream cannot be captured: plain launches there
+    const bool graph_ok = c->opt_graph && !c->profiling && nb == c->opt_batch && c->stream != nullptr && c->stream != cudaStreamLegacy;
     if (!graph_ok) {
         for (int i = 0; i < nb; i++) enqueue_body(c, half_alpha);
         CK(cudaGetLastError());
@@ -292,9 +294,10 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
         c->capturing = true;   // LaunchScope neither counts nor times captured launches
         for (int i = 0; i < nb; i++) enqueue_body(c, half_alpha);
         c->capturing = false;
-        CK(cudaStreamEndCapture(c->stream, &g));
-        CK(cudaGraphInstantiate(&c->graph_exec, g, 0));
+        CK(cudaStreamEndCapture(c->stream, &g));   // a failed capture is ended (and reported) here
+        cudaError_t ge = cudaGraphInstantiate(&c->graph_exec, g, 0);
         cudaGraphDestroy(g);
+        if (ge != cudaSuccess) { c->graph_exec = nullptr; CK(ge); }
         c->graph_key = key;
     }
     CK(cudaGraphLaunch(c->graph_exec, c->stream));

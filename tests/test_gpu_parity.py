@@ -1,0 +1,346 @@
+"""GPU parity: the CUDA path (through the C ABI of include/lgf.h) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are the north star's (BASELINE.json) with reading A14 for theta
+(DESIGN.md "Readings"): |dF| <= 1e-12, |dtheta| <= 1e-9 * max(theta_ref, 1e-15), links <= 1e-11, iteration
+count exact (A19).  Kernel-level stages use the tighter bounds of SURVEY.md section 7 step 4/5.
+"""
+import numpy as np
+import pytest
+
+import ensembles as E
+import oracle
+import paper_1301_3460_b200 as lgf
+
+pytestmark = pytest.mark.gpu
+
+ALPHA = 0.08
+TOL = 1e-15
+
+F_TOL = 1e-12
+LINK_TOL = 1e-11
+
+
+def theta_close(t_gpu, t_ref):
+    return abs(t_gpu - t_ref) <= 1e-9 * max(t_ref, TOL)
+
+
+def all_variants(gf):
+    """Every kernel selection the library offers: (fuse Delta into FFT pass A, store g, CUDA graph)."""
+    out = []
+    for fuse in (1, 0):
+        for store_g in (0, 1):
+            for graph in (1, 0):
+                out.append((fuse, store_g, graph))
+    return out
+
+
+def set_variant(gf, v):
+    gf.set_option(lgf.LGF_OPT_FUSE_DELTA_FFT, v[0])
+    gf.set_option(lgf.LGF_OPT_STORE_G, v[1])
+    gf.set_option(lgf.LGF_OPT_GRAPH, v[2])
+
+
+# ------------------------------------------------------------------ boundary: load -> get
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (4, 8, 16, 4)])
+def test_load_get_roundtrip(dims):
+    U = E.noisy(dims, 41, 0.3)
+    g18 = lgf.GaugeFixer(dims, 18)
+    g18.load_links(U)
+    assert np.array_equal(g18.get_links(), U)                      # 18-real: bit exact
+    g12 = lgf.GaugeFixer(dims, 12)
+    bad = U.copy()
+    bad[:, :, 2, :] = 7.0                                           # row 2 must be ignored on load (A9)
+    g12.load_links(bad)
+    out = g12.get_links()
+    assert np.array_equal(out[:, :, :2], U[:, :, :2])               # rows 0,1 bit exact
+    assert np.abs(out[:, :, 2] - U[:, :, 2]).max() < 1e-15          # row 2 rebuilt
+    # float64 [V,4,3,3,2] view is accepted as well
+    g18.load_links(E.as_real(U))
+    assert np.array_equal(g18.get_links(), U)
+    # the library-owned workspace/stream flavour (lgf_create) gives the same bytes
+    g3 = lgf.GaugeFixer(dims, 18, use_torch_workspace=False)
+    g3.load_links(U)
+    assert np.array_equal(g3.get_links(), U)
+
+
+def test_device_pointer_load_and_get():
+    import torch
+    dims = (8, 4, 8, 4)
+    U = E.noisy(dims, 42, 0.3)
+    d_in = torch.from_numpy(E.as_real(U).copy()).cuda()
+    d_out = torch.zeros_like(d_in)
+    gf = lgf.GaugeFixer(dims, 12)
+    gf.load_links_device(d_in.data_ptr())
+    gf.get_links_device(d_out.data_ptr())
+    torch.cuda.synchronize()
+    got = E.as_complex(d_out.cpu().numpy())
+    assert np.array_equal(got[:, :, :2], U[:, :, :2])
+    assert np.abs(got - U).max() < 1e-15
+
+
+# ------------------------------------------------------------------ kernel-level stages (S1, S2, S3, S4)
+STAGE_CASES = [
+    ((8, 8, 8, 8), 18), ((8, 8, 8, 8), 12), ((16, 16, 16, 16), 12),
+    ((8, 8, 16, 32), 12), ((4, 8, 16, 32), 18), ((32, 4, 8, 4), 12), ((4, 4, 4, 4), 12), ((16, 32, 4, 8), 18),
+]
+
+
+@pytest.mark.parametrize("dims,storage", STAGE_CASES)
+def test_stage_parity_delta_X_g_update(dims, storage):
+    U = E.noisy(dims, 43, 0.35)
+    o = oracle.Oracle(dims, storage)
+    o.load(U)
+    D_ref, X_ref, g_ref = o.delta(), o.fa_field(), o.g_field(ALPHA)
+    F_ref, th_ref = o.measure()
+    o.iterate(1, ALPHA)
+    U1_ref = o.get()
+    F1_ref, th1_ref = o.measure()
+    xs = np.abs(X_ref).max()
+
+    gf = lgf.GaugeFixer(dims, storage)
+    for v in all_variants(gf):
+        gf.load_links(U)
+        set_variant(gf, v)
+        F, th, _ = gf.measure()
+        assert abs(F - F_ref) <= 1e-14, v
+        assert abs(th - th_ref) <= 1e-12 * th_ref, v
+        D = gf.get_field(lgf.LGF_FIELD_DELTA)
+        assert np.abs(D - D_ref).max() <= 1e-14 * max(1.0, np.abs(D_ref).max()), v
+        X = gf.get_field(lgf.LGF_FIELD_X)
+        assert np.abs(X - X_ref).max() <= 1e-13 * xs, v
+        g = gf.get_field(lgf.LGF_FIELD_G, ALPHA)
+        assert np.abs(g - g_ref).max() <= 1e-13, v
+        assert np.array_equal(gf.get_links()[:, :, :2], U[:, :, :2]), v     # read-outs do not change the links
+        F1, th1 = gf.iterate(1, ALPHA)
+        assert abs(F1 - F1_ref) <= 1e-13, v
+        assert abs(th1 - th1_ref) <= 1e-11 * th1_ref, v
+        assert np.abs(gf.get_links() - U1_ref).max() <= 1e-13, v
+
+
+# ------------------------------------------------------------------ trajectories (configs C0, C1 of BASELINE.json)
+def oracle_trajectory(U, dims, storage, checkpoints, fft_mode):
+    """F_k, theta_k for k = 0..max(checkpoints) and the links at each checkpoint."""
+    o = oracle.Oracle(dims, storage, fft_mode=fft_mode)
+    o.load(U)
+    hist, links, done = [], {}, 0
+    for cp in checkpoints:
+        r = o.fix(ALPHA, 0.0, cp - done, history=True)      # theta < 0 never holds: exactly cp-done updates
+        assert r["status"] == 100
+        h = r["history"]
+        hist.extend(h[:-1] if cp != checkpoints[-1] else h)
+        links[cp] = o.get()
+        done = cp
+    return np.array(hist), links
+
+
+def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
+    U, cfg = E.make_config(name)
+    dims, storage = cfg["dims"], cfg["storage"]
+    hist_ref, links_ref = oracle_trajectory(U, dims, storage, checkpoints, fft_mode)
+    n_ref = int(np.argmax(hist_ref[:, 1] < TOL))
+    assert hist_ref[n_ref, 1] < TOL, "oracle did not converge inside the trajectory"
+
+    gf = lgf.GaugeFixer(dims, storage)
+    for v in [(1, 0, 1), (0, 1, 0)]:
+        set_variant(gf, v)
+        gf.load_links(U)
+        done = 0
+        hist = []
+        for cp in checkpoints:
+            F, th = gf.iterate(cp - done, ALPHA)
+            h = gf.get_history()
+            assert len(h) == cp - done + 1
+            assert h[-1, 0] == F and h[-1, 1] == th
+            hist.extend(h[:-1] if cp != checkpoints[-1] else h)
+            done = cp
+            # north star: |dF| <= 1e-12, theta (A14), links <= 1e-11 after 10 and 100 iterations
+            assert abs(F - hist_ref[cp, 0]) <= F_TOL, (name, v, cp)
+            assert theta_close(th, hist_ref[cp, 1]), (name, v, cp, th, hist_ref[cp, 1])
+            assert np.abs(gf.get_links() - links_ref[cp]).max() <= LINK_TOL, (name, v, cp)
+        hist = np.array(hist)
+        assert np.abs(hist[:, 0] - hist_ref[:, 0]).max() <= F_TOL
+        for k in range(len(hist)):
+            assert theta_close(hist[k, 1], hist_ref[k, 1]), (name, v, k, hist[k, 1], hist_ref[k, 1])
+        # the stop iteration: lgf_fix from the same start
+        gf.load_links(U)
+        r = gf.fix(ALPHA, TOL, 1000)
+        assert r["status"] == lgf.LGF_OK
+        assert r["n_iter"] == n_ref, (name, v, r, n_ref)                     # A19: exact
+        assert abs(r["F"] - hist_ref[n_ref, 0]) <= F_TOL
+        assert theta_close(r["theta"], hist_ref[n_ref, 1])
+        assert r["theta"] < TOL
+        assert np.abs(gf.get_links() - oracle_links_at(U, dims, storage, n_ref, fft_mode)).max() <= LINK_TOL
+    return hist_ref, n_ref
+
+
+_cache = {}
+
+
+def oracle_links_at(U, dims, storage, n, fft_mode):
+    key = (id(U), n)
+    if key not in _cache:
+        o = oracle.Oracle(dims, storage, fft_mode=fft_mode)
+        o.load(U)
+        o.iterate(n, ALPHA)
+        _cache.clear()
+        _cache[key] = o.get()
+    return _cache[key]
+
+
+def test_trajectory_C0_pure_gauge_fixed_point():
+    hist_ref, n_ref = check_trajectory("C0", fft_mode=0)
+    assert abs(hist_ref[n_ref, 0] - 1.0) < 1e-13          # closed-form fixed point F = 1 (P14)
+
+
+def test_trajectory_C1():
+    check_trajectory("C1", fft_mode=1)
+
+
+def test_C1_ten_iterations_against_the_naive_dft_oracle():
+    U, cfg = E.make_config("C1")
+    o = oracle.Oracle(cfg["dims"], cfg["storage"], fft_mode=0)      # the definition
+    o.load(U)
+    F_ref, th_ref = o.iterate(10, ALPHA)
+    gf = lgf.GaugeFixer(cfg["dims"], cfg["storage"])
+    gf.load_links(U)
+    F, th = gf.iterate(10, ALPHA)
+    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
+    assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
+
+
+# ------------------------------------------------------------------ invariants through the GPU path alone
+@pytest.mark.parametrize("storage", [12, 18])
+def test_gpu_invariants_plaquette_unitarity_monotone(storage):
+    dims = (16, 8, 8, 16)
+    U = E.noisy(dims, 44, 0.45)
+    gf = lgf.GaugeFixer(dims, storage)
+    gf.load_links(U)
+    _, _, p0 = gf.measure()
+    o = oracle.Oracle(dims, storage)
+    o.load(U)
+    assert abs(p0 - o.plaquette()) < 1e-13
+    r = gf.fix(ALPHA, TOL, 500)
+    assert r["status"] == lgf.LGF_OK
+    h = gf.get_history()
+    assert len(h) == r["n_iter"] + 1
+    F, th = h[:, 0], h[:, 1]
+    assert np.all((F[1:] - F[:-1])[th[:-1] > 1e-25] >= -1e-14)     # monotone F at alpha = 0.08 (NS; A17)
+    assert th[-1] < TOL and np.all(th[:-1] >= TOL)                   # strict stop, count = updates applied
+    _, _, p1 = gf.measure()
+    assert abs(p1 - p0) < 1e-12                                      # gauge invariance of the plaquette (NS)
+    Uf = gf.get_links()
+    I = np.eye(3)
+    assert np.abs(Uf @ Uf.conj().swapaxes(-1, -2) - I).max() < 1e-13
+    assert np.abs(np.linalg.det(Uf) - 1).max() < 1e-13
+
+
+# ------------------------------------------------------------------ edge and degenerate cases
+def test_edge_cases():
+    dims = (8, 8, 8, 8)
+    U = E.noisy(dims, 45, 0.3)
+    gf = lgf.GaugeFixer(dims, 12)
+    L = lgf.lib()
+    import ctypes as C
+    F = C.c_double()
+    # before load
+    assert L.lgf_iterate(gf._h, 1, 0.08, C.byref(F), C.byref(F)) == lgf.LGF_ERR_NOT_LOADED
+    assert L.lgf_fix(gf._h, 0.08, 1e-15, 10, None, None, None) == lgf.LGF_ERR_NOT_LOADED
+    assert L.lgf_measure(gf._h, None, None, None) == lgf.LGF_ERR_NOT_LOADED
+    buf = np.empty(4096 * 72)
+    assert L.lgf_get_links(gf._h, buf.ctypes.data) == lgf.LGF_ERR_NOT_LOADED
+    gf.load_links(U)
+    # bad arguments
+    assert L.lgf_iterate(gf._h, -1, 0.08, None, None) == lgf.LGF_ERR_INVALID_ARG
+    assert L.lgf_iterate(gf._h, 1, 0.0, None, None) == lgf.LGF_ERR_INVALID_ARG
+    assert L.lgf_iterate(gf._h, 1, float("nan"), None, None) == lgf.LGF_ERR_INVALID_ARG
+    assert L.lgf_fix(gf._h, 0.08, -1.0, 10, None, None, None) == lgf.LGF_ERR_INVALID_ARG
+    assert L.lgf_fix(gf._h, 0.08, 1e-15, -1, None, None, None) == lgf.LGF_ERR_INVALID_ARG
+    # n = 0: a pure measurement, links untouched (A5)
+    o = oracle.Oracle(dims, 12)
+    o.load(U)
+    F0, th0 = o.measure()
+    Fg, thg = gf.iterate(0, ALPHA)
+    assert abs(Fg - F0) <= 1e-14 and abs(thg - th0) <= 1e-12 * th0
+    assert np.array_equal(gf.get_links()[:, :, :2], U[:, :, :2])
+    # max_iter = 0 -> NOT_CONVERGED with the initial measurement, links untouched
+    r = gf.fix(ALPHA, TOL, 0)
+    assert r["status"] == lgf.LGF_NOT_CONVERGED and r["n_iter"] == 0 and abs(r["F"] - F0) <= 1e-14
+    assert np.array_equal(gf.get_links()[:, :, :2], U[:, :, :2])
+    # max_iter smaller than needed, batch boundaries: counts are exact for every batch size
+    for batch in (1, 3, 8):
+        gf.set_option(lgf.LGF_OPT_BATCH, batch)
+        gf.load_links(U)
+        r = gf.fix(ALPHA, TOL, 7)
+        assert r["status"] == lgf.LGF_NOT_CONVERGED and r["n_iter"] == 7
+    o.iterate(7, ALPHA)
+    assert np.abs(gf.get_links() - o.get()).max() <= 1e-12
+    gf.set_option(lgf.LGF_OPT_BATCH, 8)
+    # fix on already fixed links returns 0 updates (A5) and leaves them alone
+    r = gf.fix(ALPHA, TOL, 500)
+    assert r["status"] == lgf.LGF_OK
+    Ufix = gf.get_links()
+    r2 = gf.fix(ALPHA, TOL, 500)
+    assert r2["status"] == lgf.LGF_OK and r2["n_iter"] == 0
+    assert np.array_equal(gf.get_links(), Ufix)
+    # a loose tolerance stops earlier, at the oracle's iteration
+    gf.load_links(U)
+    r3 = gf.fix(ALPHA, 1e-6, 500)
+    o2 = oracle.Oracle(dims, 12)
+    o2.load(U)
+    assert r3["n_iter"] == o2.fix(ALPHA, 1e-6, 500)["n_iter"]
+
+
+def test_identity_links_are_a_fixed_point():
+    dims = (4, 8, 4, 8)
+    V = 1024
+    U = np.broadcast_to(np.eye(3, dtype=np.complex128), (V, 4, 3, 3)).copy()
+    for storage in (12, 18):
+        gf = lgf.GaugeFixer(dims, storage)
+        gf.load_links(U)
+        F, th = gf.iterate(3, ALPHA)
+        assert F == 1.0 and th == 0.0
+        assert np.array_equal(gf.get_links(), U)
+        r = gf.fix(ALPHA, TOL, 10)
+        assert r["n_iter"] == 0 and r["status"] == lgf.LGF_OK
+
+
+def test_nonfinite_links_are_reported():
+    dims = (4, 4, 4, 4)
+    U = E.noisy(dims, 46, 0.3)
+    U[17, 2, 0, 1] = np.nan
+    gf = lgf.GaugeFixer(dims, 18)
+    gf.load_links(U)
+    with pytest.raises(lgf.LgfError) as ei:
+        gf.iterate(2, ALPHA)
+    assert ei.value.status == lgf.LGF_ERR_NUMERIC
+
+
+def test_largest_axis_and_smallest_lattice():
+    # L = 128 on one axis (the library's maximum) and the 4^4 minimum; oracle in FFT mode for the long axis
+    for dims in [(128, 4, 4, 4), (4, 4, 4, 128), (4, 128, 4, 4), (4, 4, 128, 4)]:
+        U = E.noisy(dims, 47, 0.3)
+        o = oracle.Oracle(dims, 12, fft_mode=1)
+        o.load(U)
+        F_ref, th_ref = o.iterate(3, ALPHA)
+        gf = lgf.GaugeFixer(dims, 12)
+        gf.load_links(U)
+        F, th = gf.iterate(3, ALPHA)
+        assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref), dims
+        assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL, dims
+
+
+def test_launch_count_and_profile():
+    dims = (8, 8, 8, 8)
+    U = E.noisy(dims, 48, 0.3)
+    gf = lgf.GaugeFixer(dims, 12)
+    gf.load_links(U)
+    n0 = gf.launch_count()
+    gf.iterate(8, ALPHA)
+    per_body = 5 if gf.get_option(lgf.LGF_OPT_FUSE_DELTA_FFT) else 6
+    assert gf.launch_count() - n0 == 9 * per_body
+    gf.set_profiling(True)
+    gf.iterate(4, ALPHA)
+    prof = gf.get_profile()
+    gf.set_profiling(False)
+    assert prof["k_fft23_mid"]["launches"] == 5 and prof["k_update_x"]["launches"] == 5
+    assert all(v["ms"] > 0 for v in prof.values())
+    assert lgf.copy_peak_gbs(1 << 28, 3) > 500.0
