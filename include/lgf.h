@@ -108,8 +108,11 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_FUSE_DELTA_FFT  1: Delta is computed inside FFT pass A (default when the plane fits), 0: separate kernel
  *   LGF_OPT_STORE_G         1: pass C stores g(x) and the update reads it, 0: the update recomputes g from X
  *   LGF_OPT_GRAPH           1: replay iterations through a CUDA graph (default), 0: plain launches
- *   LGF_OPT_BATCH           iterations enqueued between two reads of the device stop flag (default 8) */
-typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3 } lgf_option;
+ *   LGF_OPT_BATCH           iterations enqueued between two reads of the device stop flag (default 8)
+ *   LGF_OPT_FAST_FFT        1 (default): use the compile-time-sized FFT passes where the lattice allows (extents 16 or
+ *                           32 on the axis pair of a pass), 0: always the generic passes.  lgf_get_option returns a
+ *                           bit mask of the passes that run fast: 1 pass A (fused Delta), 2 pass B, 4 pass C */
+typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

@@ -6,14 +6,20 @@
 // the stored (digit-reversed) positions using per-axis tables built in the same order (host side,
 // lgf_api.cu: stored_freq()).  No reordering pass and no ping-pong buffer is ever needed.
 //
-// Stage radices for a sub-length N = 2^lgN:  radix 4 when lgN is 2 or 4, radix 2 when lgN is 1, else radix 8
-// (L = 4:[4]  8:[8]  16:[4,4]  32:[8,4]  64:[8,8]  128:[8,4,4]).  The last forward stage has unit twiddles.
+// Stage radices (the "plan" of an axis, AxisPlan) are fixed per axis by the host (lgf_api.cu make_plan):
+//   "a" axes (0 and 2):  L = 4:[4]  8:[8]  16:[4,4]  32:[8,4]  64:[8,8]  128:[8,4,4]
+//   "b" axes (1 and 3):  the same except 32:[4,8], so that the last a-stage and the first b-stage of a 32x32 or
+//   16x16 tile are both radix 4 and can be fused into one 16-point register block (fft_fast.cuh).
+// The last forward stage has unit twiddles.
 #pragma once
 #include "su3.cuh"
 
 namespace lgf {
 
-__host__ __device__ __forceinline__ int stage_lg_radix(int lgN) { return (lgN == 1) ? 1 : ((lgN == 2 || lgN == 4) ? 2 : 3); }
+struct AxisPlan {
+    int nst;       // number of stages
+    int lgr[3];    // log2 radix of each forward stage, in forward order
+};
 
 // One axis transform inside a tile.  Work items are (iA, q, iB): iA the fastest thread index over a
 // non-transformed tile axis (stride strideA, 2^lgA values), q the butterfly inside a line, iB the slow
@@ -24,6 +30,7 @@ struct AxisXf {
     int lgA, strideA;
     int nB, strideB;
     const cplx* tw;  // shared-memory table tw[k] = exp(-2 pi i k / L), k < L
+    AxisPlan plan;
 };
 
 template <bool INV> __device__ __forceinline__ cplx mul_i(cplx a) {  // forward: * (-i); inverse: * (+i)
@@ -98,8 +105,7 @@ __device__ __forceinline__ void fft_stage(cplx* __restrict__ t, const AxisXf& a,
     }
 }
 
-template <bool INV> __device__ __forceinline__ void fft_stage_dispatch(cplx* t, const AxisXf& a, int lgN) {
-    const int lgR = stage_lg_radix(lgN);
+template <bool INV> __device__ __forceinline__ void fft_stage_dispatch(cplx* t, const AxisXf& a, int lgN, int lgR) {
     if (lgR == 3) fft_stage<8, INV>(t, a, lgN);
     else if (lgR == 2) fft_stage<4, INV>(t, a, lgN);
     else fft_stage<2, INV>(t, a, lgN);
@@ -108,19 +114,18 @@ template <bool INV> __device__ __forceinline__ void fft_stage_dispatch(cplx* t, 
 // Forward (DIF) transform of every line along the axis; ends with __syncthreads().
 __device__ __forceinline__ void fft_axis_forward(cplx* t, const AxisXf& a) {
     int lgN = a.lgL;
-    while (lgN > 0) {
-        fft_stage_dispatch<false>(t, a, lgN);
+    for (int k = 0; k < a.plan.nst; k++) {
+        fft_stage_dispatch<false>(t, a, lgN, a.plan.lgr[k]);
         __syncthreads();
-        lgN -= stage_lg_radix(lgN);
+        lgN -= a.plan.lgr[k];
     }
 }
 // Inverse (DIT) transform: the forward stages undone in reverse order; ends with __syncthreads().
 __device__ __forceinline__ void fft_axis_inverse(cplx* t, const AxisXf& a) {
-    int seq[8];
-    int n = 0, lgN = a.lgL;
-    while (lgN > 0) { seq[n++] = lgN; lgN -= stage_lg_radix(lgN); }
-    for (int k = n - 1; k >= 0; k--) {
-        fft_stage_dispatch<true>(t, a, seq[k]);
+    int lgN = 0;
+    for (int k = a.plan.nst - 1; k >= 0; k--) {
+        lgN += a.plan.lgr[k];
+        fft_stage_dispatch<true>(t, a, lgN, a.plan.lgr[k]);
         __syncthreads();
     }
 }

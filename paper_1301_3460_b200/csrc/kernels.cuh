@@ -114,6 +114,7 @@ __global__ void __launch_bounds__(256) k_finalize(const double2* __restrict__ pa
 struct FftTables {          // device pointers to per-axis tables (built on the host in long double)
     const cplx* tw[4];      // tw[mu][k] = exp(-2 pi i k / L_mu)
     const double* s[4];     // s[mu][p] = 4 sin^2(pi n/L_mu), n = frequency stored at position p after the forward DIF
+    AxisPlan plan[4];       // stage radices of each axis (fft_tile.cuh)
 };
 
 enum { MODE_FWD = 0, MODE_INV = 1, MODE_DELTA_FWD = 2, MODE_INV_G = 3 };
@@ -169,8 +170,8 @@ __global__ void __launch_bounds__(256) k_fft01(cplx* __restrict__ field, const c
     __syncthreads();
 
     AxisXf a0, a1;
-    a0.lgL = G.lg[0]; a0.strideK = 1;  a0.lgA = G.lg[1]; a0.strideA = S1; a0.nB = ncomp; a0.strideB = S2; a0.tw = tw0;
-    a1.lgL = G.lg[1]; a1.strideK = S1; a1.lgA = G.lg[0]; a1.strideA = 1;  a1.nB = ncomp; a1.strideB = S2; a1.tw = tw1;
+    a0.lgL = G.lg[0]; a0.strideK = 1;  a0.lgA = G.lg[1]; a0.strideA = S1; a0.nB = ncomp; a0.strideB = S2; a0.tw = tw0; a0.plan = T.plan[0];
+    a1.lgL = G.lg[1]; a1.strideK = S1; a1.lgA = G.lg[0]; a1.strideA = 1;  a1.nB = ncomp; a1.strideB = S2; a1.tw = tw1; a1.plan = T.plan[1];
     if (MODE == MODE_FWD || MODE == MODE_DELTA_FWD) {
         fft_axis_forward(tile, a0);
         fft_axis_forward(tile, a1);
@@ -230,8 +231,8 @@ __global__ void __launch_bounds__(256) k_fft23_mid(cplx* __restrict__ field, Geo
     __syncthreads();
 
     AxisXf a2, a3;
-    a2.lgL = G.lg[2]; a2.strideK = S1; a2.lgA = lgC; a2.strideA = 1; a2.nB = L3; a2.strideB = S2; a2.tw = tw2;
-    a3.lgL = G.lg[3]; a3.strideK = S2; a3.lgA = lgC; a3.strideA = 1; a3.nB = L2; a3.strideB = S1; a3.tw = tw3;
+    a2.lgL = G.lg[2]; a2.strideK = S1; a2.lgA = lgC; a2.strideA = 1; a2.nB = L3; a2.strideB = S2; a2.tw = tw2; a2.plan = T.plan[2];
+    a3.lgL = G.lg[3]; a3.strideK = S2; a3.lgA = lgC; a3.strideA = 1; a3.nB = L2; a3.strideB = S1; a3.tw = tw3; a3.plan = T.plan[3];
     fft_axis_forward(tile, a2);
     fft_axis_forward(tile, a3);
 

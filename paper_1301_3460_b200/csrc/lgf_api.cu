@@ -3,6 +3,7 @@
 // There is deliberately no CPU fallback: every compute entry point needs a CUDA device.
 #include "../../include/lgf.h"
 #include "kernels.cuh"
+#include "fft_fast.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -17,11 +18,11 @@ namespace {
 
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
-    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_NSLOTS
+    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_NSLOTS
 };
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
-    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "", "", ""};
+    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv"};
 
 constexpr int HIST_CAP = 1 << 16;
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
@@ -66,11 +67,24 @@ Layout make_layout(const int dims[4], int NC) {
     return o;
 }
 
-// frequency index held at stored position p after the forward DIF stages of fft_tile.cuh
-int stored_freq(int p, int lgL) {
-    int n = 0, mult = 1, lgN = lgL;
+// Stage radices of an axis of length 2^lgL; b_axis: axes 1 and 3 (see fft_tile.cuh).
+AxisPlan make_plan(int lgL, bool b_axis) {
+    AxisPlan p; p.nst = 0; p.lgr[0] = p.lgr[1] = p.lgr[2] = 0;
+    if (lgL == 5 && b_axis) { p.nst = 2; p.lgr[0] = 2; p.lgr[1] = 3; return p; }
+    int lgN = lgL;
     while (lgN > 0) {
-        const int lgR = stage_lg_radix(lgN);
+        const int lgR = (lgN == 1) ? 1 : ((lgN == 2 || lgN == 4) ? 2 : 3);
+        p.lgr[p.nst++] = lgR;
+        lgN -= lgR;
+    }
+    return p;
+}
+
+// frequency index held at stored position p after the forward DIF stages of fft_tile.cuh
+int stored_freq(int p, int lgL, const AxisPlan& plan) {
+    int n = 0, mult = 1, lgN = lgL;
+    for (int k = 0; k < plan.nst; k++) {
+        const int lgR = plan.lgr[k];
         const int lgs = lgN - lgR;
         const int m = p >> lgs;
         p &= (1 << lgs) - 1;
@@ -97,7 +111,11 @@ struct lgf_ctx {
     Ctl* h_ctl;             // pinned
     bool loaded;
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast;
+    // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
+    bool fast_a, fast_b, fast_c;
+    size_t smem_fa, smem_fb, smem_fc;
+    int fb_lgC;
     // derived launch parameters
     int fft01_ncomp_fused_ok, fft01_ncomp, fft01_threads, fft23_lgC, fft23_S1, fft23_S2, fft23_threads;
     size_t smem01_fused, smem01, smem23;
@@ -148,6 +166,72 @@ template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
     return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
+// ---- fast (compile-time-sized) FFT passes: the lattices they cover, and their launchers -----------------------
+constexpr int FA_NT = 256;
+// (lg of the fast axis, lg of the slow axis) pairs instantiated for each pass
+#define LGF_FAST_PAIRS(X) X(4, 4) X(4, 5) X(5, 4) X(5, 5)
+constexpr int fast_mid_lgC(int lga, int lgb) { return (lga + lgb >= 10) ? 2 : 3; }   // x0 chunk: tile <= 64 KB
+bool fast_pair(int lga, int lgb) {
+#define X(A, B) if (lga == A && lgb == B) return true;
+    LGF_FAST_PAIRS(X)
+#undef X
+    return false;
+}
+size_t smem_fast_plane(int lga, int lgb, int ncomp) { return (size_t)(((1 << lga) + 1) * (1 << lgb) * ncomp + (1 << lga) + (1 << lgb)) * 16; }
+size_t smem_fast_mid(int lga, int lgb, int lgC) {
+    const int C0 = 1 << lgC, S2 = C0 * (1 << lga) + (C0 < 8 ? C0 : 0);
+    return (size_t)(S2 * (1 << lgb) + (1 << lga) + (1 << lgb)) * 16 + (size_t)((1 << lga) + (1 << lgb)) * 8;
+}
+
+template <int NC> void launch_fa_delta_fwd(lgf_ctx* c) {
+    LaunchScope ls(c, K_FA_DELTA_FWD);
+    const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        k_fa_delta_fwd<A, B, NC, FA_NT><<<grid, FA_NT, c->smem_fa, c->stream>>>(c->links, c->field, c->partials, c->G, c->T, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+void launch_fa_inv(lgf_ctx* c) {
+    LaunchScope ls(c, K_FA_INV);
+    const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        k_fa_inv<A, B, 4, FA_NT><<<grid, FA_NT, c->smem_fc, c->stream>>>(c->field, c->G, c->T, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+void launch_fa_mid(lgf_ctx* c) {
+    LaunchScope ls(c, K_FA_MID);
+    const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
+    const double scale = 16.0 / (double)c->G.V;
+#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
+        k_fa_mid<A, B, fast_mid_lgC(A, B), FA_NT><<<grid, FA_NT, c->smem_fb, c->stream>>>(c->field, c->G, c->T, scale, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+
+lgf_status setup_fast(lgf_ctx* c) {
+    const Geom& G = c->G;
+    c->fast_a = c->fast_c = fast_pair(G.lg[0], G.lg[1]);
+    c->fast_b = fast_pair(G.lg[2], G.lg[3]);
+    c->fb_lgC = fast_mid_lgC(G.lg[2], G.lg[3]);
+    if (c->fb_lgC > G.lg[0]) c->fast_b = false;          // the x0 extent must hold one chunk
+    c->smem_fa = c->smem_fc = smem_fast_plane(G.lg[0], G.lg[1], 4);
+    c->smem_fb = smem_fast_mid(G.lg[2], G.lg[3], c->fb_lgC);
+    if (c->fast_a) {
+#define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
+            CK(set_smem(k_fa_delta_fwd<A, B, 6, FA_NT>, c->smem_fa)); CK(set_smem(k_fa_delta_fwd<A, B, 9, FA_NT>, c->smem_fa)); \
+            CK(set_smem(k_fa_inv<A, B, 4, FA_NT>, c->smem_fc)); }
+        LGF_FAST_PAIRS(X)
+#undef X
+    }
+    if (c->fast_b) {
+#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), FA_NT>, c->smem_fb));
+        LGF_FAST_PAIRS(X)
+#undef X
+    }
+    return LGF_OK;
+}
+
 lgf_status setup_kernels(lgf_ctx* c) {
     const Geom& G = c->G;
     const int nP = G.L[0] * G.L[1];
@@ -182,11 +266,12 @@ lgf_status setup_kernels(lgf_ctx* c) {
         CK(set_smem(k_fft01<MODE_DELTA_FWD, 9>, c->smem01_fused));
         CK(set_smem(k_fft01<MODE_INV_G, 6>, c->smem01_fused));
     }
-    return LGF_OK;
+    return setup_fast(c);
 }
 
 lgf_status build_tables(lgf_ctx* c) {
     std::vector<double> tw(4 * 128 * 2, 0.0), s(4 * 128, 0.0);
+    for (int mu = 0; mu < 4; mu++) c->T.plan[mu] = make_plan(c->G.lg[mu], (mu & 1) != 0);
     const long double pi = 3.141592653589793238462643383279502884L;
     for (int mu = 0; mu < 4; mu++) {
         const int L = c->G.L[mu];
@@ -197,7 +282,7 @@ lgf_status build_tables(lgf_ctx* c) {
             tw[(mu * 128 + k) * 2] = cr; tw[(mu * 128 + k) * 2 + 1] = -sr;
         }
         for (int p = 0; p < L; p++) {
-            const int n = stored_freq(p, c->G.lg[mu]);
+            const int n = stored_freq(p, c->G.lg[mu], c->T.plan[mu]);
             long double sn = sinl(pi * (long double)n / (long double)L);
             s[mu * 128 + p] = (n == 0) ? 0.0 : (double)(4.0L * sn * sn);
         }
@@ -243,19 +328,25 @@ template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
 
 bool use_fused(const lgf_ctx* c) { return c->opt_fuse && c->fft01_ncomp_fused_ok; }
 bool use_store_g(const lgf_ctx* c) { return c->opt_store_g && c->fft01_ncomp_fused_ok; }
+bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a && use_fused(c); }
+bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
+bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c && !use_store_g(c); }
 
 // S1 (+ pass A) and the reduction.  Returns the number of partials written.
 template <int NC> void enqueue_head(lgf_ctx* c) {
     int np;
-    if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
+    if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
+    else if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
     else { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fft01<MODE_FWD, 6>(c, K_FFT01_FWD, 0.0); }
     launch_finalize(c, np);
 }
 // pass B, pass C, update
+void launch_mid(lgf_ctx* c) { if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c); }
+void launch_inv_x(lgf_ctx* c) { if (use_fast_c(c)) launch_fa_inv(c); else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, 0.0); }
 template <int NC> void enqueue_tail(lgf_ctx* c, double half_alpha) {
-    launch_fft23(c);
+    launch_mid(c);
     if (use_store_g(c)) { launch_fft01<MODE_INV_G, 6>(c, K_FFT01_INV_G, half_alpha); launch_update<NC, 1>(c, half_alpha); }
-    else { launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, half_alpha); launch_update<NC, 0>(c, half_alpha); }
+    else { launch_inv_x(c); launch_update<NC, 0>(c, half_alpha); }
 }
 void enqueue_body(lgf_ctx* c, double half_alpha) {
     if (c->NC == 6) { enqueue_head<6>(c); enqueue_tail<6>(c, half_alpha); }
@@ -286,7 +377,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     }
     // alpha enters the graph as a kernel argument, so it is part of the key
     union { double d; unsigned long long u; } au; au.d = half_alpha;
-    const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (nb << 8);
+    const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^ (nb << 8);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -347,7 +438,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1;
     c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
     c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
@@ -541,9 +632,9 @@ lgf_status lgf_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host
         if (c->NC == 6) launch_delta<6>(c); else launch_delta<9>(c);
     } else {
         if (c->NC == 6) enqueue_head<6>(c); else enqueue_head<9>(c);
-        launch_fft23(c);
+        launch_mid(c);
         if (which == LGF_FIELD_G && use_store_g(c)) { launch_fft01<MODE_INV_G, 6>(c, K_FFT01_INV_G, ha); g_from_buf = true; }
-        else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, ha);
+        else launch_inv_x(c);
     }
     CK(cudaGetLastError());
     const long long V = c->G.V;
@@ -570,6 +661,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_STORE_G: c->opt_store_g = value ? 1 : 0; break;
         case LGF_OPT_GRAPH: c->opt_graph = value ? 1 : 0; break;
         case LGF_OPT_BATCH: if (value < 1 || value > 1024) return LGF_ERR_INVALID_ARG; c->opt_batch = value; break;
+        case LGF_OPT_FAST_FFT: c->opt_fast = value ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
@@ -581,6 +673,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_STORE_G: *value = use_store_g(c); break;
         case LGF_OPT_GRAPH: *value = c->opt_graph; break;
         case LGF_OPT_BATCH: *value = c->opt_batch; break;
+        case LGF_OPT_FAST_FFT: *value = (use_fast_a(c) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | (use_fast_c(c) ? 4 : 0); break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;

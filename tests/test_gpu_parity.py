@@ -24,12 +24,16 @@ def theta_close(t_gpu, t_ref):
 
 
 def all_variants(gf):
-    """Every kernel selection the library offers: (fuse Delta into FFT pass A, store g, CUDA graph)."""
+    """Every kernel selection the library offers:
+    (fuse Delta into FFT pass A, store g, CUDA graph, compile-time-sized FFT passes)."""
+    if gf.V > (1 << 18):
+        return [(1, 0, 1, 1), (1, 0, 0, 0), (0, 1, 1, 1), (0, 0, 0, 0)]
     out = []
-    for fuse in (1, 0):
-        for store_g in (0, 1):
-            for graph in (1, 0):
-                out.append((fuse, store_g, graph))
+    for fast in (1, 0):
+        for fuse in (1, 0):
+            for store_g in (0, 1):
+                for graph in (1, 0):
+                    out.append((fuse, store_g, graph, fast))
     return out
 
 
@@ -37,6 +41,7 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_FUSE_DELTA_FFT, v[0])
     gf.set_option(lgf.LGF_OPT_STORE_G, v[1])
     gf.set_option(lgf.LGF_OPT_GRAPH, v[2])
+    gf.set_option(lgf.LGF_OPT_FAST_FFT, v[3] if len(v) > 3 else 1)
 
 
 # ------------------------------------------------------------------ boundary: load -> get
@@ -86,6 +91,7 @@ def test_device_pointer_load_and_get():
 STAGE_CASES = [
     ((8, 8, 8, 8), 18), ((8, 8, 8, 8), 12), ((16, 16, 16, 16), 12),
     ((8, 8, 16, 32), 12), ((4, 8, 16, 32), 18), ((32, 4, 8, 4), 12), ((4, 4, 4, 4), 12), ((16, 32, 4, 8), 18),
+    ((32, 16, 16, 32), 12), ((16, 32, 32, 16), 18), ((32, 32, 16, 16), 12), ((16, 16, 32, 32), 18), ((32, 32, 32, 32), 12),
 ]
 
 
@@ -145,7 +151,7 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
     assert hist_ref[n_ref, 1] < TOL, "oracle did not converge inside the trajectory"
 
     gf = lgf.GaugeFixer(dims, storage)
-    for v in [(1, 0, 1), (0, 1, 0)]:
+    for v in [(1, 0, 1, 1), (0, 1, 0, 0)]:
         set_variant(gf, v)
         gf.load_links(U)
         done = 0
@@ -349,3 +355,13 @@ def test_launch_count_and_profile():
     assert prof["k_fft23_mid"]["launches"] == 5 and prof["k_update_x"]["launches"] == 5
     assert all(v["ms"] > 0 for v in prof.values())
     assert lgf.copy_peak_gbs(1 << 28, 3) > 500.0
+
+
+def test_fast_fft_pass_selection():
+    """Which lattices run the compile-time-sized passes (bit mask: 1 pass A, 2 pass B, 4 pass C)."""
+    for dims, mask in [((32, 32, 32, 32), 7), ((16, 16, 16, 16), 7), ((16, 32, 32, 16), 7), ((8, 8, 16, 32), 2),
+                       ((16, 32, 4, 8), 5), ((4, 8, 16, 32), 0), ((8, 8, 8, 8), 0)]:
+        gf = lgf.GaugeFixer(dims, 12)
+        assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
+        gf.set_option(lgf.LGF_OPT_FAST_FFT, 0)
+        assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == 0
