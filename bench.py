@@ -49,6 +49,10 @@ def kernel_bytes_per_site(nc: int) -> dict:
         "k_update_x": 64 + 2 * lk,           # read X once (neighbours: cache), read + write links
         "k_update_g": 96 + 2 * lk,
         "k_finalize": 0,
+        # compile-time-sized passes (fft_fast.cuh): same traffic as the generic passes they replace
+        "k_fa_delta_fwd": lk + 64,
+        "k_fa_mid": 128,
+        "k_fa_inv": 128,
     }
 
 
@@ -253,9 +257,8 @@ def run_ours(args):
             copy_gbs = lgf.copy_peak_gbs(1 << 30, 10)
         except Exception:
             copy_gbs = None
-        iter_bytes = sum(kb[k] for k in ("k_fft01_delta_fwd", "k_fft23_mid", "k_fft01_inv", "k_update_x")) * V \
-            if (gf.get_option(lgf.LGF_OPT_FUSE_DELTA_FFT) and not gf.get_option(lgf.LGF_OPT_STORE_G)) else \
-            sum(kb[k] * V for k in kernels if k in kb)
+        # bytes of one iteration = the kernels that actually ran (each launched once per iteration)
+        iter_bytes = sum(kb[k] * V for k in kernels if k in kb)
         it_s_1 = value / world
         # ---- time to theta < 1e-15 (lgf_fix, links resident, all syncs included)
         gf.load_links(h_in.numpy())
