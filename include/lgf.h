@@ -111,15 +111,20 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_BATCH           iterations enqueued between two reads of the device stop flag (default 8)
  *   LGF_OPT_FAST_FFT        1 (default): use the compile-time-sized FFT passes where the lattice allows (extents 16 or
  *                           32 on the axis pair of a pass), 0: always the generic passes.  lgf_get_option returns a
- *                           bit mask of the passes that run fast: 1 pass A (fused Delta), 2 pass B, 4 pass C */
-typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4 } lgf_option;
+ *                           bit mask of the passes that run fast: 1 pass A (fused Delta), 2 pass B, 4 pass C
+ *   LGF_OPT_FUSE_UPDATE     1 (default): where the compile-time-sized passes cover the (x0,x1) plane, S3/S4 of one iteration
+ *                           are fused with S1 and FFT pass A of the next (double-buffered links, g stored by pass C:
+ *                           the links cross HBM twice per iteration instead of three times), 0: separate kernels.
+ *                           lgf_get_option returns whether the fused path is the one that runs. */
+typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
+               LGF_OPT_FUSE_UPDATE = 5 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 
 /* Per-kernel device timing.  lgf_set_profiling(ctx,1) brackets every kernel launch with CUDA events on the
  * context's stream (plain launches, no graph); lgf_get_profile returns, per kernel slot i < LGF_MAX_KERNELS,
  * the accumulated milliseconds and launch counts since profiling was enabled.  names via lgf_kernel_name. */
-#define LGF_MAX_KERNELS 16
+#define LGF_MAX_KERNELS 24
 lgf_status lgf_set_profiling(lgf_ctx *ctx, int on);
 lgf_status lgf_get_profile(lgf_ctx *ctx, double ms[LGF_MAX_KERNELS], long long launches[LGF_MAX_KERNELS]);
 const char *lgf_kernel_name(int slot);

@@ -19,7 +19,7 @@ __all__ = [
     "LgfError", "lib", "library_path", "GaugeFixer", "copy_peak_gbs",
     "LGF_OK", "LGF_NOT_CONVERGED", "LGF_FP64", "LGF_FP32", "LGF_STORE_12", "LGF_STORE_18",
     "LGF_FIELD_DELTA", "LGF_FIELD_X", "LGF_FIELD_G",
-    "LGF_OPT_FUSE_DELTA_FFT", "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_FAST_FFT",
+    "LGF_OPT_FUSE_DELTA_FFT", "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_FAST_FFT", "LGF_OPT_FUSE_UPDATE",
     "EXPORTS",
 ]
 
@@ -34,8 +34,8 @@ LGF_NOT_CONVERGED = 100
 LGF_FP64, LGF_FP32 = 0, 1
 LGF_STORE_18, LGF_STORE_12 = 18, 12
 LGF_FIELD_DELTA, LGF_FIELD_X, LGF_FIELD_G = 0, 1, 2
-LGF_OPT_FUSE_DELTA_FFT, LGF_OPT_STORE_G, LGF_OPT_GRAPH, LGF_OPT_BATCH, LGF_OPT_FAST_FFT = 0, 1, 2, 3, 4
-LGF_MAX_KERNELS = 16
+LGF_OPT_FUSE_DELTA_FFT, LGF_OPT_STORE_G, LGF_OPT_GRAPH, LGF_OPT_BATCH, LGF_OPT_FAST_FFT, LGF_OPT_FUSE_UPDATE = 0, 1, 2, 3, 4, 5
+LGF_MAX_KERNELS = 24
 
 # every symbol include/lgf.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [
@@ -63,7 +63,8 @@ class LgfError(RuntimeError):
 
 
 def library_path() -> str:
-    return os.path.join(_HERE, "liblgf.so")
+    """The in-tree library; LGF_LIBRARY points at another build of the same sources (kernel A/B timing)."""
+    return os.environ.get("LGF_LIBRARY") or os.path.join(_HERE, "liblgf.so")
 
 
 def lib():

@@ -16,6 +16,17 @@
 #include <type_traits>
 #include "kernels.cuh"
 
+// resident CTAs per SM the passes are compiled for (register cap = 65536 / (NT * MINB))
+#ifndef LGF_FA_MINB_DELTA
+#define LGF_FA_MINB_DELTA 1
+#endif
+#ifndef LGF_FA_MINB_MID
+#define LGF_FA_MINB_MID 1
+#endif
+#ifndef LGF_FA_MINB_INV
+#define LGF_FA_MINB_INV 1
+#endif
+
 namespace lgf {
 
 // Two-stage plan of an axis of length 2^LG (LG = 4, 5, 6); B = axis 1 or 3.  Must agree with make_plan().
@@ -142,9 +153,53 @@ __device__ __forceinline__ void plane_middle(cplx* __restrict__ t, const cplx* _
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Forward FFT over axes 0,1 of the 4 component tiles t[c][x1][x0] (row stride L0+1), last stage written straight
+// to field (component c at field + c*V, plane base xbase).  The tile must be complete (caller syncs before).
+template <int LG0, int LG1, int NT>
+__device__ __forceinline__ void plane_forward_store(cplx* __restrict__ tile, const cplx* __restrict__ tw0, const cplx* __restrict__ tw1,
+                                                    cplx* __restrict__ field, long long V, long long xbase) {
+    using PA = Plan2<LG0, false>;
+    using PB = Plan2<LG1, true>;
+    constexpr int L0 = PA::L, L1 = PB::L, S = L0 + 1, SC = S * L1;
+    // a stage 1: points a = ja + m R2, twiddles tw0[k ja]; lanes over rows
+    {
+        constexpr int NW = 4 * PA::R2 * L1;
+#pragma unroll
+        for (int w0 = 0; w0 < NW; w0 += NT) {
+            const int w = w0 + threadIdx.x;
+            if (NW % NT == 0 || w < NW) {
+                const int xb = w % L1, ja = (w / L1) % PA::R2, c = w / (L1 * PA::R2);
+                stage_smem<PA::R1, false, true>(tile + c * SC + xb * S + ja, PA::R2, tw0, ja);
+            }
+        }
+        __syncthreads();
+    }
+    plane_middle<LG0, LG1, 4, NT, false>(tile, tw1);
+    // b stage 2 (no twiddles) -> global; lanes over x0: coalesced
+    {
+        constexpr int NW = 4 * L0 * PB::R1;
+#pragma unroll
+        for (int w0 = 0; w0 < NW; w0 += NT) {
+            const int w = w0 + threadIdx.x;
+            if (NW % NT == 0 || w < NW) {
+                const int xa = w % L0, bb = (w / L0) % PB::R1, c = w / (L0 * PB::R1);
+                const cplx* p = tile + c * SC + (bb * PB::R2) * S + xa;
+                cplx v[PB::R2];
+#pragma unroll
+                for (int m = 0; m < PB::R2; m++) v[m] = p[m * S];
+                bfly<PB::R2, false>(v);
+                cplx* gq = field + (long long)c * V + xbase + ((bb * PB::R2) << LG0) + xa;
+#pragma unroll
+                for (int m = 0; m < PB::R2; m++) gq[m << LG0] = v[m];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Pass A: S1 (Delta, theta/F partials) + forward FFT over axes 0,1 of one (x2,x3) plane, all 4 components.
 template <int LG0, int LG1, int NC, int NT>
-__global__ void __launch_bounds__(NT) k_fa_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
+__global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
                                                      Geom G, FftTables T, const Ctl* __restrict__ ctl) {
     if (ctl->done) return;
     using PA = Plan2<LG0, false>;
@@ -174,44 +229,16 @@ __global__ void __launch_bounds__(NT) k_fa_delta_fwd(const cplx* __restrict__ li
     if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
     __syncthreads();
 
-    // a stage 1: points a = ja + m R2, twiddles tw0[k ja]; lanes over rows
-    {
-        constexpr int NW = 4 * PA::R2 * L1;
-#pragma unroll
-        for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
-            if (NW % NT == 0 || w < NW) {
-                const int xb = w % L1, ja = (w / L1) % PA::R2, c = w / (L1 * PA::R2);
-                stage_smem<PA::R1, false, true>(tile + c * SC + xb * S + ja, PA::R2, tw0, ja);
-            }
-        }
-        __syncthreads();
-    }
-    plane_middle<LG0, LG1, 4, NT, false>(tile, tw1);
-    // b stage 2 (no twiddles) -> global; lanes over x0: coalesced
-    {
-        constexpr int NW = 4 * L0 * PB::R1;
-#pragma unroll
-        for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
-            if (NW % NT == 0 || w < NW) {
-                const int xa = w % L0, bb = (w / L0) % PB::R1, c = w / (L0 * PB::R1);
-                const cplx* p = tile + c * SC + (bb * PB::R2) * S + xa;
-                cplx v[PB::R2];
-#pragma unroll
-                for (int m = 0; m < PB::R2; m++) v[m] = p[m * S];
-                bfly<PB::R2, false>(v);
-                cplx* gq = field + (long long)c * G.V + xbase + ((bb * PB::R2) << LG0) + xa;
-#pragma unroll
-                for (int m = 0; m < PB::R2; m++) gq[m << LG0] = v[m];
-            }
-        }
-    }
+    plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, xbase);
 }
 
 // Pass C: inverse FFT over axes 1,0 of one (x2,x3) plane for NCOMP components (blockIdx.x = plane * (4/NCOMP) + group).
-template <int LG0, int LG1, int NCOMP, int NT>
-__global__ void __launch_bounds__(NT) k_fa_inv(cplx* __restrict__ field, Geom G, FftTables T, const Ctl* __restrict__ ctl) {
+// WRITE_G (NCOMP = 4): the last stage stays in the tile and the pass ends in S3, g(x) = GramSchmidt(1 + (alpha/2) X(x)),
+// rows 0,1 written to gbuf (6 V-arrays) instead of X to field.
+template <int LG0, int LG1, int NCOMP, int NT, bool WRITE_G>
+__global__ void __launch_bounds__(NT, LGF_FA_MINB_INV) k_fa_inv(cplx* __restrict__ field, cplx* __restrict__ gbuf, double half_alpha, Geom G, FftTables T,
+                                                                const Ctl* __restrict__ ctl) {
+    static_assert(!WRITE_G || NCOMP == 4, "g needs all four components of X");
     if (ctl->done) return;
     using PA = Plan2<LG0, false>;
     using PB = Plan2<LG1, true>;
@@ -248,6 +275,29 @@ __global__ void __launch_bounds__(NT) k_fa_inv(cplx* __restrict__ field, Geom G,
         __syncthreads();
     }
     plane_middle<LG0, LG1, NCOMP, NT, true>(tile, tw1);
+    if constexpr (WRITE_G) {
+        // a stage 1 inverse in place (lanes over rows: odd stride, conflict-free), then S3 per site
+        constexpr int NW = NCOMP * PA::R2 * L1;
+#pragma unroll
+        for (int w0 = 0; w0 < NW; w0 += NT) {
+            const int w = w0 + threadIdx.x;
+            if (NW % NT == 0 || w < NW) {
+                const int xb = w % L1, ja = (w / L1) % PA::R2, c = w / (L1 * PA::R2);
+                stage_smem<PA::R1, true, true>(tile + c * SC + xb * S + ja, PA::R2, tw0, ja);
+            }
+        }
+        __syncthreads();
+        constexpr int nP = L0 * L1;
+#pragma unroll 1
+        for (int e = threadIdx.x; e < nP; e += NT) {
+            const int o = (e & (L0 - 1)) + (e >> LG0) * S;
+            cplx g[9];
+            build_g(tile[o], tile[SC + o], tile[2 * SC + o], tile[3 * SC + o], half_alpha, g);
+#pragma unroll
+            for (int c = 0; c < 6; c++) gbuf[(long long)c * G.V + xbase + e] = g[c];
+        }
+        return;
+    }
     // a stage 1 inverse (twiddles conj tw0[k ja]) -> global.  Lane order: each quarter-warp reads conflict-free and
     // each warp store covers whole 64 B (R2 = 4) or 128 B (R2 = 8) segments.
     {
@@ -276,7 +326,7 @@ __global__ void __launch_bounds__(NT) k_fa_inv(cplx* __restrict__ field, Geom G,
 // Pass B: forward over axes 2,3, filter, inverse over axes 3,2, for a chunk of C0 = 2^LGC consecutive x0 at fixed
 // (component, x1).  tile[i3][i2][i0], S1 = C0, S2 = C0*L2 (+C0 when C0 < 8: keeps quarter-warps conflict-free).
 template <int LG2, int LG3, int LGC, int NT>
-__global__ void __launch_bounds__(NT) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+__global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
     if (ctl->done) return;
     using PA = Plan2<LG2, false>;
     using PB = Plan2<LG3, true>;

@@ -92,7 +92,10 @@ __global__ void __launch_bounds__(128) k_delta(const cplx* __restrict__ links, c
 // ------------------------------------------------------------------------------------------------ S5
 // One block.  Sums the partials in a fixed order (strided per thread, then tree), writes F, theta, history,
 // and raises the stop flag: theta < theta_tol (converged), or max_iter updates applied, or non-finite.
-__global__ void __launch_bounds__(256) k_finalize(const double2* __restrict__ partials, int n, Ctl* ctl, double2* hist, double inv3V, double inv12V) {
+// advance != 0: the measured links are the result of an update applied by the same iteration body (fused update,
+// fused_update.cuh): count it and make the buffer it wrote the current one.
+__global__ void __launch_bounds__(256) k_finalize(const double2* __restrict__ partials, int n, Ctl* ctl, double2* hist, double inv3V, double inv12V,
+                                                  int advance) {
     if (ctl->done) return;
     __shared__ double red[64];
     double a = 0, b = 0;
@@ -101,6 +104,7 @@ __global__ void __launch_bounds__(256) k_finalize(const double2* __restrict__ pa
     if (threadIdx.x == 0) {
         const double theta = a * inv3V, F = b * inv12V;
         ctl->theta = theta; ctl->F = F;
+        if (advance) { ctl->iters = ctl->iters + 1; ctl->parity = ctl->parity ^ 1; }
         const int k = ctl->n_meas;
         if (k < ctl->hist_cap) hist[k] = make_double2(F, theta);
         ctl->n_meas = k + 1;

@@ -4,6 +4,7 @@
 #include "../../include/lgf.h"
 #include "kernels.cuh"
 #include "fft_fast.cuh"
+#include "fused_update.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -18,11 +19,12 @@ namespace {
 
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
-    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_NSLOTS
+    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE, K_NSLOTS
 };
+static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
-    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv"};
+    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd"};
 
 constexpr int HIST_CAP = 1 << 16;
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
@@ -32,6 +34,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {   // offsets into the workspace
     size_t links, field, gbuf, partials, ctl, hist, tables, scratch, staging, total;
+    size_t link_buf;        // bytes of one link buffer; the links region holds two (fused update: read one, write the other)
     int n_partials;
     long long stage_sites;
 };
@@ -51,7 +54,8 @@ Layout make_layout(const int dims[4], int NC) {
     Layout o;
     const long long V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
     size_t off = 0;
-    o.links = off; off = align_up(off + (size_t)V * 4 * NC * 16, 256);
+    o.link_buf = align_up((size_t)V * 4 * NC * 16, 256);
+    o.links = off; off += 2 * o.link_buf;
     o.field = off; off = align_up(off + (size_t)V * 4 * 16, 256);
     o.gbuf = off; off = align_up(off + (size_t)V * 6 * 16, 256);
     o.n_partials = (int)(V / 128);                       // k_delta / k_plaquette: one per 128-site block
@@ -111,10 +115,11 @@ struct lgf_ctx {
     Ctl* h_ctl;             // pinned
     bool loaded;
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update;
+    int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
     bool fast_a, fast_b, fast_c;
-    size_t smem_fa, smem_fb, smem_fc;
+    size_t smem_fa, smem_fb, smem_fc, smem_fu;
     int fb_lgC;
     // derived launch parameters
     int fft01_ncomp_fused_ok, fft01_ncomp, fft01_threads, fft23_lgC, fft23_S1, fft23_S2, fft23_threads;
@@ -145,6 +150,8 @@ namespace {
         }                                                                                                  \
     } while (0)
 
+cplx* cur_links(const lgf_ctx* c) { return c->links + (size_t)c->parity * (c->lay.link_buf / 16); }
+
 // Launch bookkeeping: counts every kernel; in profiling mode brackets it with events and accumulates its time.
 struct LaunchScope {
     lgf_ctx* c; int slot;
@@ -162,7 +169,12 @@ struct LaunchScope {
     }
 };
 
+#ifndef LGF_CARVEOUT
+#define LGF_CARVEOUT 0
+#endif
 template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
+    // prefer the largest shared-memory carveout: the tile passes are limited by resident CTAs, not by L1
+    if (LGF_CARVEOUT) cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, LGF_CARVEOUT);
     return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
@@ -187,7 +199,7 @@ template <int NC> void launch_fa_delta_fwd(lgf_ctx* c) {
     LaunchScope ls(c, K_FA_DELTA_FWD);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_delta_fwd<A, B, NC, FA_NT><<<grid, FA_NT, c->smem_fa, c->stream>>>(c->links, c->field, c->partials, c->G, c->T, c->ctl);
+        k_fa_delta_fwd<A, B, NC, FA_NT><<<grid, FA_NT, c->smem_fa, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -195,7 +207,25 @@ void launch_fa_inv(lgf_ctx* c) {
     LaunchScope ls(c, K_FA_INV);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_inv<A, B, 4, FA_NT><<<grid, FA_NT, c->smem_fc, c->stream>>>(c->field, c->G, c->T, c->ctl);
+        k_fa_inv<A, B, 4, FA_NT, false><<<grid, FA_NT, c->smem_fc, c->stream>>>(c->field, nullptr, 0.0, c->G, c->T, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+void launch_fa_inv_g(lgf_ctx* c, double half_alpha) {
+    LaunchScope ls(c, K_FA_INV_G);
+    const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        k_fa_inv<A, B, 4, FA_NT, true><<<grid, FA_NT, c->smem_fc, c->stream>>>(c->field, c->gbuf, half_alpha, c->G, c->T, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+// S3/S4 of this iteration + S1 and pass A of the next (fused_update.cuh); reads link buffer Ctl::parity, writes the other
+template <int NC> void launch_fu_update(lgf_ctx* c) {
+    LaunchScope ls(c, K_FU_UPDATE);
+    const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
+    const long long stride = (long long)(c->lay.link_buf / 16);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        k_fu_update_delta_fwd<A, B, NC, LGF_FU_NT><<<grid, LGF_FU_NT, c->smem_fu, c->stream>>>(c->links, stride, c->gbuf, c->field, c->partials, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -215,12 +245,13 @@ lgf_status setup_fast(lgf_ctx* c) {
     c->fast_b = fast_pair(G.lg[2], G.lg[3]);
     c->fb_lgC = fast_mid_lgC(G.lg[2], G.lg[3]);
     if (c->fb_lgC > G.lg[0]) c->fast_b = false;          // the x0 extent must hold one chunk
-    c->smem_fa = c->smem_fc = smem_fast_plane(G.lg[0], G.lg[1], 4);
+    c->smem_fa = c->smem_fc = c->smem_fu = smem_fast_plane(G.lg[0], G.lg[1], 4);
     c->smem_fb = smem_fast_mid(G.lg[2], G.lg[3], c->fb_lgC);
     if (c->fast_a) {
 #define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
             CK(set_smem(k_fa_delta_fwd<A, B, 6, FA_NT>, c->smem_fa)); CK(set_smem(k_fa_delta_fwd<A, B, 9, FA_NT>, c->smem_fa)); \
-            CK(set_smem(k_fa_inv<A, B, 4, FA_NT>, c->smem_fc)); }
+            CK(set_smem(k_fa_inv<A, B, 4, FA_NT, false>, c->smem_fc)); CK(set_smem(k_fa_inv<A, B, 4, FA_NT, true>, c->smem_fc)); \
+            CK(set_smem(k_fu_update_delta_fwd<A, B, 6, LGF_FU_NT>, c->smem_fu)); CK(set_smem(k_fu_update_delta_fwd<A, B, 9, LGF_FU_NT>, c->smem_fu)); }
         LGF_FAST_PAIRS(X)
 #undef X
     }
@@ -301,7 +332,7 @@ lgf_status build_tables(lgf_ctx* c) {
 // ---- kernel launchers ---------------------------------------------------------------------------------------
 template <int NC> void launch_delta(lgf_ctx* c) {
     LaunchScope ls(c, K_DELTA);
-    k_delta<NC><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, c->field, c->partials, c->G, c->ctl);
+    k_delta<NC><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->ctl);
 }
 template <int MODE, int NC> void launch_fft01(lgf_ctx* c, int slot, double half_alpha) {
     LaunchScope ls(c, slot);
@@ -309,7 +340,7 @@ template <int MODE, int NC> void launch_fft01(lgf_ctx* c, int slot, double half_
     const int ncomp = fused ? 4 : c->fft01_ncomp;
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3] * (4 / ncomp));
     k_fft01<MODE, NC><<<grid, c->fft01_threads, fused ? c->smem01_fused : c->smem01, c->stream>>>(
-        c->field, c->links, c->gbuf, c->partials, c->G, c->T, ncomp, half_alpha, c->ctl);
+        c->field, cur_links(c), c->gbuf, c->partials, c->G, c->T, ncomp, half_alpha, c->ctl);
 }
 void launch_fft23(lgf_ctx* c) {
     LaunchScope ls(c, K_FFT23_MID);
@@ -317,13 +348,13 @@ void launch_fft23(lgf_ctx* c) {
     k_fft23_mid<<<grid, c->fft23_threads, c->smem23, c->stream>>>(c->field, c->G, c->T, c->fft23_lgC, c->fft23_S1, c->fft23_S2,
                                                                    16.0 / (double)c->G.V, c->ctl);
 }
-void launch_finalize(lgf_ctx* c, int n_partials) {
+void launch_finalize(lgf_ctx* c, int n_partials, int advance = 0) {
     LaunchScope ls(c, K_FINALIZE);
-    k_finalize<<<1, 256, 0, c->stream>>>(c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V));
+    k_finalize<<<1, 256, 0, c->stream>>>(c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), advance);
 }
 template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
     LaunchScope ls(c, SG ? K_UPDATE_G : K_UPDATE_X);
-    k_update<NC, SG><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
+    k_update<NC, SG><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(cur_links(c), SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
 }
 
 bool use_fused(const lgf_ctx* c) { return c->opt_fuse && c->fft01_ncomp_fused_ok; }
@@ -331,6 +362,7 @@ bool use_store_g(const lgf_ctx* c) { return c->opt_store_g && c->fft01_ncomp_fus
 bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a && use_fused(c); }
 bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
 bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c && !use_store_g(c); }
+bool use_fused_update(const lgf_ctx* c) { return c->opt_fuse_update && c->opt_fast && c->fast_a; }
 
 // S1 (+ pass A) and the reduction.  Returns the number of partials written.
 template <int NC> void enqueue_head(lgf_ctx* c) {
@@ -349,13 +381,22 @@ template <int NC> void enqueue_tail(lgf_ctx* c, double half_alpha) {
     else { launch_inv_x(c); launch_update<NC, 0>(c, half_alpha); }
 }
 void enqueue_body(lgf_ctx* c, double half_alpha) {
+    if (use_fused_update(c)) {
+        // pass B, pass C ending in g, then update + next Delta + next pass A, and the measurement of the updated links
+        launch_mid(c);
+        launch_fa_inv_g(c, half_alpha);
+        if (c->NC == 6) launch_fu_update<6>(c); else launch_fu_update<9>(c);
+        launch_finalize(c, c->G.L[2] * c->G.L[3], 1);
+        return;
+    }
     if (c->NC == 6) { enqueue_head<6>(c); enqueue_tail<6>(c, half_alpha); }
     else { enqueue_head<9>(c); enqueue_tail<9>(c, half_alpha); }
 }
+int launches_per_body(const lgf_ctx* c) { return use_fused_update(c) ? 4 : (use_fused(c) ? 5 : 6); }
 
 lgf_status reset_ctl(lgf_ctx* c, double tol, int max_iter) {
     Ctl h; memset(&h, 0, sizeof h);
-    h.theta_tol = tol; h.max_iter = max_iter; h.hist_cap = HIST_CAP;
+    h.theta_tol = tol; h.max_iter = max_iter; h.hist_cap = HIST_CAP; h.parity = c->parity;
     *c->h_ctl = h;
     CK(cudaMemcpyAsync(c->ctl, c->h_ctl, sizeof(Ctl), cudaMemcpyHostToDevice, c->stream));
     return LGF_OK;
@@ -363,6 +404,7 @@ lgf_status reset_ctl(lgf_ctx* c, double tol, int max_iter) {
 lgf_status read_ctl(lgf_ctx* c) {
     CK(cudaMemcpyAsync(c->h_ctl, c->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
+    c->parity = c->h_ctl->parity;
     return LGF_OK;
 }
 
@@ -377,7 +419,9 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     }
     // alpha enters the graph as a kernel argument, so it is part of the key
     union { double d; unsigned long long u; } au; au.d = half_alpha;
-    const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^ (nb << 8);
+    // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
+    const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -392,7 +436,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
         c->graph_key = key;
     }
     CK(cudaGraphLaunch(c->graph_exec, c->stream));
-    c->launches += (long long)nb * (use_fused(c) ? 5 : 6);
+    c->launches += (long long)nb * launches_per_body(c);
     return LGF_OK;
 }
 
@@ -402,6 +446,13 @@ lgf_status run(lgf_ctx* c, double alpha, double tol, int max_iter, bool poll) {
     if (st != LGF_OK) return st;
     const double ha = 0.5 * alpha;
     long long bodies_left = (long long)max_iter + 1;
+    if (use_fused_update(c)) {
+        // measurement 0 (S1 + pass A of the first iteration); every later measurement is made by the fused update
+        if (c->NC == 6) enqueue_head<6>(c); else enqueue_head<9>(c);
+        CK(cudaGetLastError());
+        bodies_left = max_iter;
+        if (bodies_left == 0) { st = read_ctl(c); if (st != LGF_OK) return st; }
+    }
     while (bodies_left > 0) {
         int nb = (int)(bodies_left < c->opt_batch ? bodies_left : c->opt_batch);
         st = enqueue_bodies(c, nb, ha);
@@ -438,7 +489,8 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 1;
+    c->parity = 0;
     c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
     c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
@@ -473,6 +525,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
 
 lgf_status load_from_device_chunks(lgf_ctx* c, const double* src, bool src_is_host) {
     const long long V = c->G.V, S = c->lay.stage_sites;
+    c->parity = 0;          // a load fills link buffer 0
     for (long long off = 0; off < V; off += S) {
         const long long n = (V - off < S) ? V - off : S;
         const cplx* aos;
@@ -501,8 +554,8 @@ lgf_status get_to_chunks(lgf_ctx* c, double* dst, bool dst_is_host) {
         {
             LaunchScope ls(c, K_LAYOUT_OUT);
             const unsigned grid = (unsigned)((n * 4 + 255) / 256);
-            if (c->NC == 6) k_layout_out<6><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n);
-            else k_layout_out<9><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n);
+            if (c->NC == 6) k_layout_out<6><<<grid, 256, 0, c->stream>>>(cur_links(c), aos, V, off, n);
+            else k_layout_out<9><<<grid, 256, 0, c->stream>>>(cur_links(c), aos, V, off, n);
         }
         CK(cudaGetLastError());
         if (dst_is_host) CK(cudaMemcpyAsync(dst + off * 72, c->staging, (size_t)n * 576, cudaMemcpyDeviceToHost, c->stream));
@@ -589,8 +642,8 @@ lgf_status lgf_measure(lgf_ctx* c, double* F, double* theta, double* plaq) {
     launch_finalize(c, (int)(c->G.V / 128));
     {
         LaunchScope ls(c, K_PLAQUETTE);
-        if (c->NC == 6) k_plaquette<6><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, c->partials, c->G);
-        else k_plaquette<9><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, c->partials, c->G);
+        if (c->NC == 6) k_plaquette<6><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(cur_links(c), c->partials, c->G);
+        else k_plaquette<9><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(cur_links(c), c->partials, c->G);
     }
     double* sums = reinterpret_cast<double*>(c->ws + c->lay.scratch);
     {
@@ -662,6 +715,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_GRAPH: c->opt_graph = value ? 1 : 0; break;
         case LGF_OPT_BATCH: if (value < 1 || value > 1024) return LGF_ERR_INVALID_ARG; c->opt_batch = value; break;
         case LGF_OPT_FAST_FFT: c->opt_fast = value ? 1 : 0; break;
+        case LGF_OPT_FUSE_UPDATE: c->opt_fuse_update = value ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
@@ -674,6 +728,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_GRAPH: *value = c->opt_graph; break;
         case LGF_OPT_BATCH: *value = c->opt_batch; break;
         case LGF_OPT_FAST_FFT: *value = (use_fast_a(c) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | (use_fast_c(c) ? 4 : 0); break;
+        case LGF_OPT_FUSE_UPDATE: *value = use_fused_update(c) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;

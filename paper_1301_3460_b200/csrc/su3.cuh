@@ -131,6 +131,7 @@ struct Ctl {
     int n_meas;            // measurements made (index into the history)
     int hist_cap;
     unsigned int ticket;   // block counter of the fused reduction
+    int parity;            // which of the two link buffers holds the current links (fused update: flipped per update)
 };
 
 }  // namespace lgf

@@ -42,7 +42,8 @@ def test_workspace_bytes_and_supported_sizes():
     V = 32 ** 4
     n12 = L.lgf_workspace_bytes(d(32, 32, 32, 32), lgf.LGF_FP64, lgf.LGF_STORE_12)
     n18 = L.lgf_workspace_bytes(d(32, 32, 32, 32), lgf.LGF_FP64, lgf.LGF_STORE_18)
-    assert n12 >= V * (384 + 64) and n18 - n12 == V * 192     # links 384 / 576 B per site
+    # links 384 / 576 B per site, two buffers (the fused update reads one and writes the other)
+    assert n12 >= V * (2 * 384 + 64) and n18 - n12 == 2 * V * 192
     assert L.lgf_workspace_bytes(d(64, 64, 64, 64), lgf.LGF_FP64, lgf.LGF_STORE_12) >= 64 ** 4 * 448
     assert L.lgf_workspace_bytes(d(32, 32, 32, 64), lgf.LGF_FP64, lgf.LGF_STORE_12) > 0
     assert L.lgf_workspace_bytes(d(8, 8, 8, 8), lgf.LGF_FP64, lgf.LGF_STORE_18) > 0

@@ -25,15 +25,16 @@ def theta_close(t_gpu, t_ref):
 
 def all_variants(gf):
     """Every kernel selection the library offers:
-    (fuse Delta into FFT pass A, store g, CUDA graph, compile-time-sized FFT passes)."""
+    (fuse Delta into FFT pass A, store g, CUDA graph, compile-time-sized FFT passes, fused update + next Delta)."""
     if gf.V > (1 << 18):
-        return [(1, 0, 1, 1), (1, 0, 0, 0), (0, 1, 1, 1), (0, 0, 0, 0)]
+        return [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 0, 0, 0), (0, 1, 1, 1, 0), (0, 0, 0, 0, 0)]
     out = []
     for fast in (1, 0):
         for fuse in (1, 0):
             for store_g in (0, 1):
                 for graph in (1, 0):
-                    out.append((fuse, store_g, graph, fast))
+                    out.append((fuse, store_g, graph, fast, 0))
+    out += [(1, 0, 1, 1, 1), (1, 0, 0, 1, 1)]       # the fused update needs the fast passes; the other switches do not enter
     return out
 
 
@@ -41,7 +42,8 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_FUSE_DELTA_FFT, v[0])
     gf.set_option(lgf.LGF_OPT_STORE_G, v[1])
     gf.set_option(lgf.LGF_OPT_GRAPH, v[2])
-    gf.set_option(lgf.LGF_OPT_FAST_FFT, v[3] if len(v) > 3 else 1)
+    gf.set_option(lgf.LGF_OPT_FAST_FFT, v[3])
+    gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, v[4])
 
 
 # ------------------------------------------------------------------ boundary: load -> get
@@ -151,7 +153,7 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
     assert hist_ref[n_ref, 1] < TOL, "oracle did not converge inside the trajectory"
 
     gf = lgf.GaugeFixer(dims, storage)
-    for v in [(1, 0, 1, 1), (0, 1, 0, 0)]:
+    for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (0, 1, 0, 0, 0)]:
         set_variant(gf, v)
         gf.load_links(U)
         done = 0
@@ -355,6 +357,55 @@ def test_launch_count_and_profile():
     assert prof["k_fft23_mid"]["launches"] == 5 and prof["k_update_x"]["launches"] == 5
     assert all(v["ms"] > 0 for v in prof.values())
     assert lgf.copy_peak_gbs(1 << 28, 3) > 500.0
+
+
+def test_fused_update_buffers_and_counts():
+    """The fused update double-buffers the links: whatever the parity after a call, every later call --
+    read-back, measurement, stage read-out, more iterations on either path, a reload -- sees the current links."""
+    dims, storage = (16, 16, 16, 16), 12
+    U = E.noisy(dims, 49, 0.35)
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    gf = lgf.GaugeFixer(dims, storage)
+    assert gf.get_option(lgf.LGF_OPT_FUSE_UPDATE) == 1
+    gf.load_links(U)
+    o.load(U)
+    n0 = gf.launch_count()
+    F, th = gf.iterate(3, ALPHA)                          # odd: the current links are in the second buffer
+    assert gf.launch_count() - n0 == 2 + 4 * 3            # measurement 0 (2 kernels) + 3 bodies of 4
+    F_ref, th_ref = o.iterate(3, ALPHA)
+    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
+    U3 = gf.get_links()
+    assert np.abs(U3 - o.get()).max() <= LINK_TOL
+    Fm, thm, _ = gf.measure()
+    assert abs(Fm - F) <= 1e-14 and abs(thm - th) <= 1e-12 * th
+    assert np.abs(gf.get_field(lgf.LGF_FIELD_DELTA) - o.delta()).max() <= 1e-13
+    F0, th0 = gf.iterate(0, ALPHA)
+    assert abs(F0 - F) <= 1e-14
+    gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, 0)             # separate kernels continue from the second buffer, in place
+    F, th = gf.iterate(2, ALPHA)
+    F_ref, th_ref = o.iterate(2, ALPHA)
+    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
+    gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, 1)
+    F, th = gf.iterate(4, ALPHA)
+    F_ref, th_ref = o.iterate(4, ALPHA)
+    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
+    assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
+    gf.load_links(U)                                      # a reload starts from buffer 0 again
+    assert np.array_equal(gf.get_links()[:, :, :2], U[:, :, :2])
+    r = gf.fix(ALPHA, TOL, 1000)
+    o.load(U)
+    r_ref = o.fix(ALPHA, TOL, 1000)
+    assert r["status"] == lgf.LGF_OK and r["n_iter"] == r_ref["n_iter"]
+    assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
+    h = gf.get_history()
+    assert len(h) == r["n_iter"] + 1 and h[-1, 1] < TOL and np.all(h[:-1, 1] >= TOL)
+    # profile names of the fused path
+    gf.set_profiling(True)
+    gf.iterate(2, ALPHA)
+    prof = gf.get_profile()
+    gf.set_profiling(False)
+    assert prof["k_fu_update_delta_fwd"]["launches"] == 2 and prof["k_fa_inv_g"]["launches"] == 2
+    assert prof["k_fa_delta_fwd"]["launches"] == 1 and prof["k_finalize"]["launches"] == 3
 
 
 def test_fast_fft_pass_selection():
