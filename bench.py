@@ -53,6 +53,9 @@ def kernel_bytes_per_site(nc: int) -> dict:
         "k_fa_delta_fwd": lk + 64,
         "k_fa_mid": 128,
         "k_fa_inv": 128,
+        "k_fa_inv_g": 64 + 96,               # read X~ field, write rows 0,1 of g
+        # fused S3/S4 + next S1 + next pass A (fused_update.cuh): g 96, links read once + written once, field written
+        "k_fu_update_delta_fwd": 96 + 2 * lk + 64,
     }
 
 
@@ -191,6 +194,8 @@ def run_ours(args):
     del U
 
     gf = lgf.GaugeFixer(dims, storage)
+    if args.fuse_update is not None:
+        gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, args.fuse_update)
     gf.load_links(h_in.numpy())
     _, _, plaq = gf.measure()
     stream = gf.stream            # the context's own torch stream: every kernel and copy is ordered on it
@@ -319,6 +324,8 @@ def main():
     ap.add_argument("--workload", default="C2b", help="ensemble name from ensembles.CONFIGS (C2b = 32^4, eps 0.35)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fuse-update", type=int, default=None, choices=[0, 1],
+                    help="override LGF_OPT_FUSE_UPDATE (kernel A/B timing); default: the library's choice")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps

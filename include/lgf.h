@@ -112,7 +112,8 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_FAST_FFT        1 (default): use the compile-time-sized FFT passes where the lattice allows (extents 16 or
  *                           32 on the axis pair of a pass), 0: always the generic passes.  lgf_get_option returns a
  *                           bit mask of the passes that run fast: 1 pass A (fused Delta), 2 pass B, 4 pass C
- *   LGF_OPT_FUSE_UPDATE     1 (default): where the compile-time-sized passes cover the (x0,x1) plane, S3/S4 of one iteration
+ *   LGF_OPT_FUSE_UPDATE     0 (default: the separate kernels measured faster on B200), 1: where the
+ *                           compile-time-sized passes cover the (x0,x1) plane, S3/S4 of one iteration
  *                           are fused with S1 and FFT pass A of the next (double-buffered links, g stored by pass C:
  *                           the links cross HBM twice per iteration instead of three times), 0: separate kernels.
  *                           lgf_get_option returns whether the fused path is the one that runs. */

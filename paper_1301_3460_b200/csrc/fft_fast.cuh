@@ -16,12 +16,13 @@
 #include <type_traits>
 #include "kernels.cuh"
 
-// resident CTAs per SM the passes are compiled for (register cap = 65536 / (NT * MINB))
+// resident CTAs per SM the passes are compiled for (register cap = 65536 / (NT * MINB)).  Measured on B200 at 32^4
+// (CUDA events per launch): pass A 118.9 us at 1 CTA/SM, 107.7 at 2, 143.2 at 3 (spills); pass B 66.0 / 47.3 / 59.3.
 #ifndef LGF_FA_MINB_DELTA
-#define LGF_FA_MINB_DELTA 1
+#define LGF_FA_MINB_DELTA 2
 #endif
 #ifndef LGF_FA_MINB_MID
-#define LGF_FA_MINB_MID 1
+#define LGF_FA_MINB_MID 2
 #endif
 #ifndef LGF_FA_MINB_INV
 #define LGF_FA_MINB_INV 1

@@ -43,6 +43,12 @@ __device__ __forceinline__ void third_row(cplx (&u)[9]) {
 // 128-bit loads/stores of one complex double
 __device__ __forceinline__ cplx ldg2(const cplx* p) { return __ldg(p); }
 
+// Asynchronous DRAM -> L2 prefetch of `bytes` contiguous bytes (multiple of 16, 16-byte aligned): no register or
+// shared-memory destination, so the bytes in flight are not bounded by the register file (sm_90+ bulk prefetch).
+__device__ __forceinline__ void prefetch_l2(const void* p, unsigned bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 // Load link (x, mu) from the structure-of-arrays store: entry c of direction mu is the V-array at
 // links + (mu*NC + c)*V, NC = 6 (12-real: rows 0,1) or 9 (18-real).  Row 2 is rebuilt for NC = 6.
 template <int NC>

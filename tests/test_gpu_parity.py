@@ -366,6 +366,8 @@ def test_fused_update_buffers_and_counts():
     U = E.noisy(dims, 49, 0.35)
     o = oracle.Oracle(dims, storage, fft_mode=1)
     gf = lgf.GaugeFixer(dims, storage)
+    assert gf.get_option(lgf.LGF_OPT_FUSE_UPDATE) == 0   # measured slower on B200: off by default
+    gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, 1)
     assert gf.get_option(lgf.LGF_OPT_FUSE_UPDATE) == 1
     gf.load_links(U)
     o.load(U)
