@@ -116,9 +116,19 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *                           compile-time-sized passes cover the (x0,x1) plane, S3/S4 of one iteration
  *                           are fused with S1 and FFT pass A of the next (double-buffered links, g stored by pass C:
  *                           the links cross HBM twice per iteration instead of three times), 0: separate kernels.
- *                           lgf_get_option returns whether the fused path is the one that runs. */
+ *                           lgf_get_option returns whether the fused path is the one that runs.
+ *   LGF_OPT_PINGPONG        bit mask (1 pass A, 2 pass B, 4 pass C): run that compile-time-sized pass as a
+ *                           persistent kernel, one CTA per SM, whose two thread groups alternate their global-memory
+ *                           and shared-memory phases (fft_fast.cuh); 0 bits: one work item per CTA.
+ *                           lgf_get_option returns the mask of the passes that run this way.  Default 0: measured on
+ *                           B200 the strict alternation is slower for pass A and neutral for B and C.
+ *   LGF_OPT_FUSE_FINALIZE   1: with the compile-time-sized pass A, the CTA that finishes S1 last also does the final
+ *                           theta/F reduction and the S5 stop test (one launch fewer per iteration; the summation
+ *                           order, hence the result, is that of the separate k_finalize), 0 (default: the gpu-scope
+ *                           fence it needs costs pass A more than the launch it saves): k_finalize.
+ *                           lgf_get_option returns whether it applies. */
 typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
-               LGF_OPT_FUSE_UPDATE = 5 } lgf_option;
+               LGF_OPT_FUSE_UPDATE = 5, LGF_OPT_PINGPONG = 6, LGF_OPT_FUSE_FINALIZE = 7 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

@@ -30,6 +30,14 @@
 
 namespace lgf {
 
+// A group of NT threads that works on one tile: thread index within the group and the named barrier the group
+// synchronises on.  A whole CTA is the group {threadIdx.x, 0} (bar.sync 0 over all threads = __syncthreads());
+// the ping-pong kernels of fft_pp.cuh run two groups per CTA on barriers 1 and 2.
+struct Grp { int tid; int bar; };
+template <int NT> __device__ __forceinline__ void gsync(const Grp& g) {
+    asm volatile("bar.sync %0, %1;" ::"r"(g.bar), "n"(NT) : "memory");
+}
+
 // Two-stage plan of an axis of length 2^LG (LG = 4, 5, 6); B = axis 1 or 3.  Must agree with make_plan().
 template <int LG, bool B> struct Plan2 {
     static_assert(LG >= 4 && LG <= 6, "fast FFT passes cover L = 16, 32, 64");
@@ -104,9 +112,9 @@ __device__ __forceinline__ void block_smem(cplx* __restrict__ p, int sa, int sb,
 // ---------------------------------------------------------------------------------------------------------------
 // The middle stages of a 2-D transform of NCOMP tiles t[c][b][a] (row stride S odd, component stride SC), i.e.
 // everything between the first stage of axis a and the last stage of axis b (forward), or the mirror (inverse).
-// Ends with __syncthreads().
+// Ends with a group barrier.
 template <int LGA, int LGB, int NCOMP, int NT, bool INV>
-__device__ __forceinline__ void plane_middle(cplx* __restrict__ t, const cplx* __restrict__ twb) {
+__device__ __forceinline__ void plane_middle(cplx* __restrict__ t, const cplx* __restrict__ twb, const Grp& g) {
     using PA = Plan2<LGA, false>;
     using PB = Plan2<LGB, true>;
     constexpr int LA = PA::L, LB = PB::L, S = LA + 1, SC = S * LB;
@@ -115,39 +123,39 @@ __device__ __forceinline__ void plane_middle(cplx* __restrict__ t, const cplx* _
         constexpr int NW = NCOMP * PA::R1 * PB::R2;
 #pragma unroll
         for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
+            const int w = w0 + g.tid;
             if (NW % NT == 0 || w < NW) {
                 const int jb = w % PB::R2, ba = (w / PB::R2) % PA::R1, c = w / (PB::R2 * PA::R1);
                 block_smem<PA::R2, PB::R1, INV>(t + c * SC + jb * S + ba * PA::R2, 1, PB::R2 * S, twb, jb);
             }
         }
-        __syncthreads();
+        gsync<NT>(g);
     } else {
         // a stage 2 (contiguous sub-blocks of R2 points, no twiddles): lanes over rows
         auto a2 = [&]() {
             constexpr int NW = NCOMP * PA::R1 * LB;
 #pragma unroll
             for (int w0 = 0; w0 < NW; w0 += NT) {
-                const int w = w0 + threadIdx.x;
+                const int w = w0 + g.tid;
                 if (NW % NT == 0 || w < NW) {
                     const int xb = w % LB, ba = (w / LB) % PA::R1, c = w / (LB * PA::R1);
                     stage_smem<PA::R2, INV, false>(t + c * SC + xb * S + ba * PA::R2, 1, nullptr, 0);
                 }
             }
-            __syncthreads();
+            gsync<NT>(g);
         };
         // b stage 1 (sub-length LB, twiddles tw[k jb]): lanes over columns
         auto b1 = [&]() {
             constexpr int NW = NCOMP * LA * PB::R2;
 #pragma unroll
             for (int w0 = 0; w0 < NW; w0 += NT) {
-                const int w = w0 + threadIdx.x;
+                const int w = w0 + g.tid;
                 if (NW % NT == 0 || w < NW) {
                     const int xa = w % LA, jb = (w / LA) % PB::R2, c = w / (LA * PB::R2);
                     stage_smem<PB::R1, INV, true>(t + c * SC + jb * S + xa, PB::R2 * S, twb, jb);
                 }
             }
-            __syncthreads();
+            gsync<NT>(g);
         };
         if constexpr (INV) { b1(); a2(); } else { a2(); b1(); }
     }
@@ -158,7 +166,7 @@ __device__ __forceinline__ void plane_middle(cplx* __restrict__ t, const cplx* _
 // to field (component c at field + c*V, plane base xbase).  The tile must be complete (caller syncs before).
 template <int LG0, int LG1, int NT>
 __device__ __forceinline__ void plane_forward_store(cplx* __restrict__ tile, const cplx* __restrict__ tw0, const cplx* __restrict__ tw1,
-                                                    cplx* __restrict__ field, long long V, long long xbase) {
+                                                    cplx* __restrict__ field, long long V, long long xbase, const Grp& g) {
     using PA = Plan2<LG0, false>;
     using PB = Plan2<LG1, true>;
     constexpr int L0 = PA::L, L1 = PB::L, S = L0 + 1, SC = S * L1;
@@ -167,21 +175,21 @@ __device__ __forceinline__ void plane_forward_store(cplx* __restrict__ tile, con
         constexpr int NW = 4 * PA::R2 * L1;
 #pragma unroll
         for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
+            const int w = w0 + g.tid;
             if (NW % NT == 0 || w < NW) {
                 const int xb = w % L1, ja = (w / L1) % PA::R2, c = w / (L1 * PA::R2);
                 stage_smem<PA::R1, false, true>(tile + c * SC + xb * S + ja, PA::R2, tw0, ja);
             }
         }
-        __syncthreads();
+        gsync<NT>(g);
     }
-    plane_middle<LG0, LG1, 4, NT, false>(tile, tw1);
+    plane_middle<LG0, LG1, 4, NT, false>(tile, tw1, g);
     // b stage 2 (no twiddles) -> global; lanes over x0: coalesced
     {
         constexpr int NW = 4 * L0 * PB::R1;
 #pragma unroll
         for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
+            const int w = w0 + g.tid;
             if (NW % NT == 0 || w < NW) {
                 const int xa = w % L0, bb = (w / L0) % PB::R1, c = w / (L0 * PB::R1);
                 const cplx* p = tile + c * SC + (bb * PB::R2) * S + xa;
@@ -191,34 +199,39 @@ __device__ __forceinline__ void plane_forward_store(cplx* __restrict__ tile, con
                 bfly<PB::R2, false>(v);
                 cplx* gq = field + (long long)c * V + xbase + ((bb * PB::R2) << LG0) + xa;
 #pragma unroll
-                for (int m = 0; m < PB::R2; m++) gq[m << LG0] = v[m];
+                for (int m = 0; m < PB::R2; m++) st_field(gq + (m << LG0), v[m]);
             }
         }
     }
 }
 
+// Sum of two values over a group of NT threads in a fixed order (warp shuffle tree, then warp 0 of the group over the
+// warp partials); result valid in group thread 0.  red: 64 doubles of the group's own.  Contains one group barrier.
+template <int NT>
+__device__ __forceinline__ void group_sum2(double& a, double& b, double* red, const Grp& g) {
+    a = warp_sum(a); b = warp_sum(b);
+    const int w = g.tid >> 5, l = g.tid & 31;
+    constexpr int nw = NT / 32;
+    if (l == 0) { red[w] = a; red[32 + w] = b; }
+    gsync<NT>(g);
+    if (w == 0) {
+        a = (l < nw) ? red[l] : 0.0;
+        b = (l < nw) ? red[32 + l] : 0.0;
+        a = warp_sum(a); b = warp_sum(b);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
-// Pass A: S1 (Delta, theta/F partials) + forward FFT over axes 0,1 of one (x2,x3) plane, all 4 components.
+// Pass A, memory phase: S1 of one (x2,x3) plane -> the 4 component tiles, theta/F partial of the plane -> partials.
+// Ends with a group barrier (the tile is complete).
 template <int LG0, int LG1, int NC, int NT>
-__global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
-                                                     Geom G, FftTables T, const Ctl* __restrict__ ctl) {
-    if (ctl->done) return;
-    using PA = Plan2<LG0, false>;
-    using PB = Plan2<LG1, true>;
-    constexpr int L0 = PA::L, L1 = PB::L, S = L0 + 1, SC = S * L1, nP = L0 * L1;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx* tile = reinterpret_cast<cplx*>(smem_raw);
-    cplx* tw0 = tile + 4 * SC;
-    cplx* tw1 = tw0 + L0;
-    __shared__ double red[64];
-    const long long xbase = (long long)blockIdx.x << (LG0 + LG1);
-
-    for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
-    for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
-
+__device__ __forceinline__ void pass_a_delta(const cplx* __restrict__ links, const Geom& G, int plane, cplx* __restrict__ tile, double* red,
+                                             double2* __restrict__ partials, const Grp& g) {
+    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1, nP = L0 * L1;
+    const long long xbase = (long long)plane << (LG0 + LG1);
     double th = 0, fs = 0;
 #pragma unroll 1
-    for (int e = threadIdx.x; e < nP; e += NT) {
+    for (int e = g.tid; e < nP; e += NT) {
         cplx f0, f1, f2, f3;
         double t_, f_;
         delta_site<NC>(links, G, xbase + e, f0, f1, f2, f3, t_, f_);
@@ -226,24 +239,155 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cp
         const int o = (e & (L0 - 1)) + (e >> LG0) * S;
         tile[o] = f0; tile[SC + o] = f1; tile[2 * SC + o] = f2; tile[3 * SC + o] = f3;
     }
-    block_sum2(th, fs, red);     // contains a __syncthreads() after the tile writes
-    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
-    __syncthreads();
+    group_sum2<NT>(th, fs, red, g);     // its barrier also orders the tile writes
+    if (g.tid == 0) partials[plane] = make_double2(th, fs);
+    gsync<NT>(g);
+}
 
-    plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, xbase);
+// S5 inside pass A: the CTA that takes the last ticket sums the plane partials in the order k_finalize uses (strided per
+// thread, then the fixed tree: the result is bit-identical), writes F, theta and the history and raises the stop flag.
+// Every CTA of the grid has passed its ctl->done test by then, and the next kernel starts after this one ends.
+struct FinArgs { double2* hist; double inv3V, inv12V; int on; };
+template <int NT>
+__device__ __forceinline__ void finalize_last_cta(const double2* partials, int n, Ctl* ctl, const FinArgs& fa, double* red) {
+    __shared__ int is_last;
+    if (threadIdx.x == 0) {
+        __threadfence();                                   // this CTA's partial is visible before its ticket
+        is_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    double a = 0, b = 0;
+    for (int i = threadIdx.x; i < n; i += NT) { const double2 p = __ldcg(partials + i); a += p.x; b += p.y; }
+    block_sum2(a, b, red);
+    if (threadIdx.x == 0) {
+        const double theta = a * fa.inv3V, F = b * fa.inv12V;
+        ctl->theta = theta; ctl->F = F; ctl->ticket = 0;
+        const int k = ctl->n_meas;
+        if (k < ctl->hist_cap) fa.hist[k] = make_double2(F, theta);
+        ctl->n_meas = k + 1;
+        if (!(isfinite(theta) && isfinite(F))) { ctl->nonfinite = 1; ctl->done = 1; }
+        else if (theta < ctl->theta_tol) { ctl->converged = 1; ctl->done = 1; }
+        else if (ctl->iters >= ctl->max_iter) { ctl->done = 1; }
+    }
+    __syncthreads();
+}
+
+// Pass A: S1 (Delta, theta/F partials) + forward FFT over axes 0,1 of one (x2,x3) plane, all 4 components.
+template <int LG0, int LG1, int NC, int NT>
+__global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
+                                                     Geom G, FftTables T, Ctl* ctl, FinArgs fa) {
+    if (ctl->done) return;
+    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw);
+    cplx* tw0 = tile + 4 * SC;
+    cplx* tw1 = tw0 + L0;
+    __shared__ double red[64];
+    const Grp g{(int)threadIdx.x, 0};
+    for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
+    for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
+    pass_a_delta<LG0, LG1, NC, NT>(links, G, blockIdx.x, tile, red, partials, g);
+    if (fa.on) finalize_last_cta<NT>(partials, gridDim.x, ctl, fa, red);
+    plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)blockIdx.x << (LG0 + LG1), g);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Pass C, memory phase: X~ of one plane (NCOMP components from fbase) -> inverse b stage 2 (no twiddles) -> tile.
+// Ends with a group barrier.
+template <int LG0, int LG1, int NCOMP, int NT>
+__device__ __forceinline__ void pass_c_load(const cplx* __restrict__ fbase, long long V, cplx* __restrict__ tile, const Grp& g) {
+    using PB = Plan2<LG1, true>;
+    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
+    constexpr int NW = NCOMP * L0 * PB::R1;
+#pragma unroll
+    for (int w0 = 0; w0 < NW; w0 += NT) {
+        const int w = w0 + g.tid;
+        if (NW % NT == 0 || w < NW) {
+            const int xa = w % L0, bb = (w / L0) % PB::R1, c = w / (L0 * PB::R1);
+            const cplx* gq = fbase + (long long)c * V + ((bb * PB::R2) << LG0) + xa;
+            cplx v[PB::R2];
+#pragma unroll
+            for (int m = 0; m < PB::R2; m++) v[m] = ld_field(gq + (m << LG0));
+            bfly<PB::R2, true>(v);
+            cplx* p = tile + c * SC + (bb * PB::R2) * S + xa;
+#pragma unroll
+            for (int m = 0; m < PB::R2; m++) p[m * S] = v[m];
+        }
+    }
+    gsync<NT>(g);
+}
+
+// Pass C, on-chip phase: the remaining inverse stages of axes 1,0; X -> field (in place), or with WRITE_G the pass ends
+// in S3, g(x) = GramSchmidt(1 + (alpha/2) X(x)), rows 0,1 written to gbuf (6 V-arrays) at gbase = gbuf + xbase.
+template <int LG0, int LG1, int NCOMP, int NT, bool WRITE_G>
+__device__ __forceinline__ void pass_c_finish(cplx* __restrict__ fbase, cplx* __restrict__ gbase, double half_alpha, long long V, cplx* __restrict__ tile,
+                                              const cplx* __restrict__ tw0, const cplx* __restrict__ tw1, const Grp& g) {
+    using PA = Plan2<LG0, false>;
+    using PB = Plan2<LG1, true>;
+    constexpr int L0 = PA::L, L1 = PB::L, S = L0 + 1, SC = S * L1;
+    plane_middle<LG0, LG1, NCOMP, NT, true>(tile, tw1, g);
+    if constexpr (WRITE_G) {
+        // a stage 1 inverse in place (lanes over rows: odd stride, conflict-free), then S3 per site
+        constexpr int NW = NCOMP * PA::R2 * L1;
+#pragma unroll
+        for (int w0 = 0; w0 < NW; w0 += NT) {
+            const int w = w0 + g.tid;
+            if (NW % NT == 0 || w < NW) {
+                const int xb = w % L1, ja = (w / L1) % PA::R2, c = w / (L1 * PA::R2);
+                stage_smem<PA::R1, true, true>(tile + c * SC + xb * S + ja, PA::R2, tw0, ja);
+            }
+        }
+        gsync<NT>(g);
+        constexpr int nP = L0 * L1;
+#pragma unroll 1
+        for (int e = g.tid; e < nP; e += NT) {
+            const int o = (e & (L0 - 1)) + (e >> LG0) * S;
+            cplx gm[9];
+            build_g(tile[o], tile[SC + o], tile[2 * SC + o], tile[3 * SC + o], half_alpha, gm);
+#pragma unroll
+            for (int c = 0; c < 6; c++) gbase[(long long)c * V + e] = gm[c];
+        }
+    } else {
+        // a stage 1 inverse (twiddles conj tw0[k ja]) -> global.  Lane order (R2 = 4): a quarter-warp is 4 consecutive ja
+        // (one 64 B segment) of two rows 4 apart: its shared-memory reads are conflict-free (16-byte bank group =
+        // (xb + ja + 4m) mod 8 with the odd row stride) and its global store touches 2 lines, 8 per warp instruction.
+        // (Lanes over 8 rows first, as in the first version, made every quarter-warp touch 8 lines: ncu showed the pass
+        // bound by L1TEX data-pipe wavefronts, 32.7 k global per SM against 10.6 k now.)  R2 = 8: 128 B per quarter-warp.
+        constexpr int NW = NCOMP * PA::R2 * L1;
+#pragma unroll
+        for (int w0 = 0; w0 < NW; w0 += NT) {
+            const int w = w0 + g.tid;
+            if (NW % NT == 0 || w < NW) {
+                int ja, xb;
+                if constexpr (PA::R2 >= 8) { ja = w % PA::R2; xb = (w / PA::R2) % L1; }
+                else {
+                    static_assert(PA::R2 == 4, "lane order below");
+                    const int t = w >> 2;
+                    ja = w & 3; xb = (((t >> 1) & 3) | ((t & 1) << 2)) + 8 * ((t >> 3) % (L1 / 8));
+                }
+                const int c = w / (PA::R2 * L1);
+                const cplx* p = tile + c * SC + xb * S + ja;
+                cplx v[PA::R1];
+#pragma unroll
+                for (int m = 0; m < PA::R1; m++) v[m] = p[m * PA::R2];
+                stage_regs<PA::R1, true, true>(v, tw0, ja);
+                cplx* gq = fbase + (long long)c * V + (xb << LG0) + ja;
+#pragma unroll
+                for (int m = 0; m < PA::R1; m++) st_field(gq + m * PA::R2, v[m]);
+            }
+        }
+    }
 }
 
 // Pass C: inverse FFT over axes 1,0 of one (x2,x3) plane for NCOMP components (blockIdx.x = plane * (4/NCOMP) + group).
-// WRITE_G (NCOMP = 4): the last stage stays in the tile and the pass ends in S3, g(x) = GramSchmidt(1 + (alpha/2) X(x)),
-// rows 0,1 written to gbuf (6 V-arrays) instead of X to field.
 template <int LG0, int LG1, int NCOMP, int NT, bool WRITE_G>
 __global__ void __launch_bounds__(NT, LGF_FA_MINB_INV) k_fa_inv(cplx* __restrict__ field, cplx* __restrict__ gbuf, double half_alpha, Geom G, FftTables T,
                                                                 const Ctl* __restrict__ ctl) {
     static_assert(!WRITE_G || NCOMP == 4, "g needs all four components of X");
     if (ctl->done) return;
-    using PA = Plan2<LG0, false>;
-    using PB = Plan2<LG1, true>;
-    constexpr int L0 = PA::L, L1 = PB::L, S = L0 + 1, SC = S * L1;
+    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* tile = reinterpret_cast<cplx*>(smem_raw);
     cplx* tw0 = tile + NCOMP * SC;
@@ -251,129 +395,72 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_INV) k_fa_inv(cplx* __restrict
     constexpr int NG = 4 / NCOMP;
     const long long xbase = (long long)(blockIdx.x / NG) << (LG0 + LG1);
     cplx* fbase = field + (long long)((blockIdx.x % NG) * NCOMP) * G.V + xbase;
-
+    const Grp g{(int)threadIdx.x, 0};
     for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
     for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
-
-    // global -> b stage 2 inverse (no twiddles) -> tile; lanes over x0
-    {
-        constexpr int NW = NCOMP * L0 * PB::R1;
-#pragma unroll
-        for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
-            if (NW % NT == 0 || w < NW) {
-                const int xa = w % L0, bb = (w / L0) % PB::R1, c = w / (L0 * PB::R1);
-                const cplx* gq = fbase + (long long)c * G.V + ((bb * PB::R2) << LG0) + xa;
-                cplx v[PB::R2];
-#pragma unroll
-                for (int m = 0; m < PB::R2; m++) v[m] = gq[m << LG0];
-                bfly<PB::R2, true>(v);
-                cplx* p = tile + c * SC + (bb * PB::R2) * S + xa;
-#pragma unroll
-                for (int m = 0; m < PB::R2; m++) p[m * S] = v[m];
-            }
-        }
-        __syncthreads();
-    }
-    plane_middle<LG0, LG1, NCOMP, NT, true>(tile, tw1);
-    if constexpr (WRITE_G) {
-        // a stage 1 inverse in place (lanes over rows: odd stride, conflict-free), then S3 per site
-        constexpr int NW = NCOMP * PA::R2 * L1;
-#pragma unroll
-        for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
-            if (NW % NT == 0 || w < NW) {
-                const int xb = w % L1, ja = (w / L1) % PA::R2, c = w / (L1 * PA::R2);
-                stage_smem<PA::R1, true, true>(tile + c * SC + xb * S + ja, PA::R2, tw0, ja);
-            }
-        }
-        __syncthreads();
-        constexpr int nP = L0 * L1;
-#pragma unroll 1
-        for (int e = threadIdx.x; e < nP; e += NT) {
-            const int o = (e & (L0 - 1)) + (e >> LG0) * S;
-            cplx g[9];
-            build_g(tile[o], tile[SC + o], tile[2 * SC + o], tile[3 * SC + o], half_alpha, g);
-#pragma unroll
-            for (int c = 0; c < 6; c++) gbuf[(long long)c * G.V + xbase + e] = g[c];
-        }
-        return;
-    }
-    // a stage 1 inverse (twiddles conj tw0[k ja]) -> global.  Lane order: each quarter-warp reads conflict-free and
-    // each warp store covers whole 64 B (R2 = 4) or 128 B (R2 = 8) segments.
-    {
-        constexpr int NW = NCOMP * PA::R2 * L1;
-#pragma unroll
-        for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
-            if (NW % NT == 0 || w < NW) {
-                int ja, xb;
-                if constexpr (PA::R2 >= 8) { ja = w % PA::R2; xb = (w / PA::R2) % L1; }
-                else { ja = (w / 8) % PA::R2; xb = (w % 8) + 8 * ((w / (8 * PA::R2)) % (L1 / 8)); }
-                const int c = w / (PA::R2 * L1);
-                const cplx* p = tile + c * SC + xb * S + ja;
-                cplx v[PA::R1];
-#pragma unroll
-                for (int m = 0; m < PA::R1; m++) v[m] = p[m * PA::R2];
-                stage_regs<PA::R1, true, true>(v, tw0, ja);
-                cplx* gq = fbase + (long long)c * G.V + (xb << LG0) + ja;
-#pragma unroll
-                for (int m = 0; m < PA::R1; m++) gq[m * PA::R2] = v[m];
-            }
-        }
-    }
+    pass_c_load<LG0, LG1, NCOMP, NT>(fbase, G.V, tile, g);      // its barrier also publishes the twiddles
+    pass_c_finish<LG0, LG1, NCOMP, NT, WRITE_G>(fbase, WRITE_G ? gbuf + xbase : nullptr, half_alpha, G.V, tile, tw0, tw1, g);
 }
 
-// Pass B: forward over axes 2,3, filter, inverse over axes 3,2, for a chunk of C0 = 2^LGC consecutive x0 at fixed
-// (component, x1).  tile[i3][i2][i0], S1 = C0, S2 = C0*L2 (+C0 when C0 < 8: keeps quarter-warps conflict-free).
+// ---------------------------------------------------------------------------------------------------------------
+// Pass B works on the (x2,x3) extent of one (component, x1, chunk of C0 = 2^LGC consecutive x0):
+// tile[i3][i2][i0], S1 = C0, S2 = C0*L2 (+C0 when C0 < 8: keeps quarter-warps conflict-free).
+// Work item index = chunk + nChunks*(x1 + L1*comp).
+template <int LG2, int LGC> struct MidGeom {
+    static constexpr int L2 = 1 << LG2, C0 = 1 << LGC, S1 = C0, S2 = C0 * L2 + (C0 < 8 ? C0 : 0);
+};
+struct MidItem {
+    cplx* gp;        // field + comp*V + chunk*C0 + x1*L0 + i0
+    double s01;      // s[0][x0] + s[1][x1] of this thread's x0
+};
+template <int LGC>
+__device__ __forceinline__ MidItem mid_item(cplx* __restrict__ field, const Geom& G, const FftTables& T, int item, int i0) {
+    const int lgChunks = G.lg[0] - LGC;
+    const int chunk = item & ((1 << lgChunks) - 1);
+    const int x1 = (item >> lgChunks) & (G.L[1] - 1);
+    const int comp = item >> (lgChunks + G.lg[1]);
+    MidItem it;
+    it.gp = field + (long long)comp * G.V + (chunk << LGC) + ((long long)x1 << G.sh[1]) + i0;
+    it.s01 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1];
+    return it;
+}
+
+// Pass B, memory phase: global -> axis-2 stage 1 (points i2 = ja + m R2, twiddles tw2[k ja]) -> tile.  Ends with a
+// group barrier.  tl = tile + i0.
 template <int LG2, int LG3, int LGC, int NT>
-__global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
-    if (ctl->done) return;
+__device__ __forceinline__ void pass_b_load(const cplx* __restrict__ gp, int sh2, int sh3, cplx* __restrict__ tl, const cplx* __restrict__ tw2, const Grp& g) {
     using PA = Plan2<LG2, false>;
     using PB = Plan2<LG3, true>;
-    constexpr int L2 = PA::L, L3 = PB::L, C0 = 1 << LGC, S1 = C0, S2 = C0 * L2 + (C0 < 8 ? C0 : 0);
-    static_assert(NT % C0 == 0, "a thread keeps its x0 offset");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx* tile = reinterpret_cast<cplx*>(smem_raw);
-    cplx* tw2 = tile + S2 * L3;
-    cplx* tw3 = tw2 + L2;
-    double* s2 = reinterpret_cast<double*>(tw3 + L3);
-    double* s3 = s2 + L2;
-
-    const int lgChunks = G.lg[0] - LGC;
-    const int chunk = blockIdx.x & ((1 << lgChunks) - 1);
-    const int x1 = (blockIdx.x >> lgChunks) & (G.L[1] - 1);
-    const int comp = blockIdx.x >> (lgChunks + G.lg[1]);
-    const int i0 = threadIdx.x % C0;
-    cplx* gp = field + (long long)comp * G.V + (chunk << LGC) + ((long long)x1 << G.sh[1]) + i0;
-    cplx* tl = tile + i0;
-    const int sh2 = G.sh[2], sh3 = G.sh[3];
-
-    for (int i = threadIdx.x; i < L2; i += NT) { tw2[i] = T.tw[2][i]; s2[i] = T.s[2][i]; }
-    for (int i = threadIdx.x; i < L3; i += NT) { tw3[i] = T.tw[3][i]; s3[i] = T.s[3][i]; }
-    const double s01 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1];
-    __syncthreads();
-
-    // global -> axis-2 stage 1 (points i2 = ja + m R2, twiddles tw2[k ja]) -> tile
-    {
-        constexpr int NW = C0 * PA::R2 * L3;
+    using MG = MidGeom<LG2, LGC>;
+    constexpr int L3 = PB::L, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
+    constexpr int NW = C0 * PA::R2 * L3;
 #pragma unroll
-        for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
-            if (NW % NT == 0 || w < NW) {
-                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
-                const cplx* gq = gp + ((long long)ja << sh2) + ((long long)i3 << sh3);
-                cplx v[PA::R1];
+    for (int w0 = 0; w0 < NW; w0 += NT) {
+        const int w = w0 + g.tid;
+        if (NW % NT == 0 || w < NW) {
+            const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+            const cplx* gq = gp + ((long long)ja << sh2) + ((long long)i3 << sh3);
+            cplx v[PA::R1];
 #pragma unroll
-                for (int m = 0; m < PA::R1; m++) v[m] = gq[(long long)(m * PA::R2) << sh2];
-                stage_regs<PA::R1, false, true>(v, tw2, ja);
-                cplx* p = tl + ja * S1 + i3 * S2;
+            for (int m = 0; m < PA::R1; m++) v[m] = ld_field(gq + ((long long)(m * PA::R2) << sh2));
+            stage_regs<PA::R1, false, true>(v, tw2, ja);
+            cplx* p = tl + ja * S1 + i3 * S2;
 #pragma unroll
-                for (int m = 0; m < PA::R1; m++) p[m * PA::R2 * S1] = v[m];
-            }
+            for (int m = 0; m < PA::R1; m++) p[m * PA::R2 * S1] = v[m];
         }
-        __syncthreads();
     }
+    gsync<NT>(g);
+}
+
+// Pass B, on-chip phase: the remaining forward stages, the p2max/p2 filter, the inverse stages, last one -> global.
+template <int LG2, int LG3, int LGC, int NT>
+__device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01, int sh2, int sh3, double scale, cplx* __restrict__ tl,
+                                              const cplx* __restrict__ tw2, const cplx* __restrict__ tw3, const double* __restrict__ s2,
+                                              const double* __restrict__ s3, const Grp& g) {
+    using PA = Plan2<LG2, false>;
+    using PB = Plan2<LG3, true>;
+    using MG = MidGeom<LG2, LGC>;
+    constexpr int L2 = PA::L, L3 = PB::L, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
     // middle stages, forward and (after the filter) inverse
     auto middle = [&](auto inv_tag) {
         constexpr bool INV = decltype(inv_tag)::value;
@@ -381,37 +468,37 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict
             constexpr int NW = C0 * PB::R2 * PA::R1;
 #pragma unroll
             for (int w0 = 0; w0 < NW; w0 += NT) {
-                const int w = w0 + threadIdx.x;
+                const int w = w0 + g.tid;
                 if (NW % NT == 0 || w < NW) {
                     const int jb = (w / C0) % PB::R2, ba = w / (C0 * PB::R2);
                     block_smem<PA::R2, PB::R1, INV>(tl + ba * PA::R2 * S1 + jb * S2, S1, PB::R2 * S2, tw3, jb);
                 }
             }
-            __syncthreads();
+            gsync<NT>(g);
         } else {
             auto a2 = [&]() {
                 constexpr int NW = C0 * PA::R1 * L3;
 #pragma unroll
                 for (int w0 = 0; w0 < NW; w0 += NT) {
-                    const int w = w0 + threadIdx.x;
+                    const int w = w0 + g.tid;
                     if (NW % NT == 0 || w < NW) {
                         const int ba = (w / C0) % PA::R1, i3 = w / (C0 * PA::R1);
                         stage_smem<PA::R2, INV, false>(tl + ba * PA::R2 * S1 + i3 * S2, S1, nullptr, 0);
                     }
                 }
-                __syncthreads();
+                gsync<NT>(g);
             };
             auto b1 = [&]() {
                 constexpr int NW = C0 * L2 * PB::R2;
 #pragma unroll
                 for (int w0 = 0; w0 < NW; w0 += NT) {
-                    const int w = w0 + threadIdx.x;
+                    const int w = w0 + g.tid;
                     if (NW % NT == 0 || w < NW) {
                         const int i2 = (w / C0) % L2, jb = w / (C0 * L2);
                         stage_smem<PB::R1, INV, true>(tl + i2 * S1 + jb * S2, PB::R2 * S2, tw3, jb);
                     }
                 }
-                __syncthreads();
+                gsync<NT>(g);
             };
             if constexpr (INV) { b1(); a2(); } else { a2(); b1(); }
         }
@@ -423,7 +510,7 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict
         constexpr int NW = C0 * L2 * PB::R1;
 #pragma unroll
         for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
+            const int w = w0 + g.tid;
             if (NW % NT == 0 || w < NW) {
                 const int i2 = (w / C0) % L2, bb = w / (C0 * L2);
                 cplx* p = tl + i2 * S1 + (bb * PB::R2) * S2;
@@ -443,7 +530,7 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict
                 for (int m = 0; m < PB::R2; m++) p[m * S2] = v[m];
             }
         }
-        __syncthreads();
+        gsync<NT>(g);
     }
     middle(std::true_type{});
     // tile -> axis-2 stage 1 inverse -> global
@@ -451,7 +538,7 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict
         constexpr int NW = C0 * PA::R2 * L3;
 #pragma unroll
         for (int w0 = 0; w0 < NW; w0 += NT) {
-            const int w = w0 + threadIdx.x;
+            const int w = w0 + g.tid;
             if (NW % NT == 0 || w < NW) {
                 const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
                 const cplx* p = tl + ja * S1 + i3 * S2;
@@ -461,8 +548,171 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict
                 stage_regs<PA::R1, true, true>(v, tw2, ja);
                 cplx* gq = gp + ((long long)ja << sh2) + ((long long)i3 << sh3);
 #pragma unroll
-                for (int m = 0; m < PA::R1; m++) gq[(long long)(m * PA::R2) << sh2] = v[m];
+                for (int m = 0; m < PA::R1; m++) st_field(gq + ((long long)(m * PA::R2) << sh2), v[m]);
             }
+        }
+    }
+}
+
+// Pass B: forward over axes 2,3, filter, inverse over axes 3,2, one work item per CTA.
+template <int LG2, int LG3, int LGC, int NT>
+__global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+    if (ctl->done) return;
+    using MG = MidGeom<LG2, LGC>;
+    constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0;
+    static_assert(NT % C0 == 0, "a thread keeps its x0 offset");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw);
+    cplx* tw2 = tile + MG::S2 * L3;
+    cplx* tw3 = tw2 + L2;
+    double* s2 = reinterpret_cast<double*>(tw3 + L3);
+    double* s3 = s2 + L2;
+    const Grp g{(int)threadIdx.x, 0};
+    const int i0 = threadIdx.x % C0;
+    const MidItem it = mid_item<LGC>(field, G, T, blockIdx.x, i0);
+    for (int i = threadIdx.x; i < L2; i += NT) { tw2[i] = T.tw[2][i]; s2[i] = T.s[2][i]; }
+    for (int i = threadIdx.x; i < L3; i += NT) { tw3[i] = T.tw[3][i]; s3[i] = T.s[3][i]; }
+    __syncthreads();
+    pass_b_load<LG2, LG3, LGC, NT>(it.gp, G.sh[2], G.sh[3], tile + i0, tw2, g);
+    pass_b_finish<LG2, LG3, LGC, NT>(it.gp, it.s01, G.sh[2], G.sh[3], scale, tile + i0, tw2, tw3, s2, s3, g);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Ping-pong persistent passes.  With one work item per CTA every resident CTA starts together and stays in phase:
+// all of them read global memory at once, then all of them sit in the shared-memory stages with HBM idle (measured
+// on B200 at 32^4: pass A takes 17.2 us per plane per SM at 1 CTA/SM and 2 x 15.6 at 2 CTAs/SM, i.e. the phases add
+// instead of overlapping).  Here one CTA per SM runs two groups of NT threads, each with its own tile, which take the
+// CTA's work items alternately and pass a token so that their MEMORY phases alternate: while group 0 is in the
+// on-chip stages of item k, group 1 is loading item k+1.  The token is a pair of named barriers (3: "group 0 may
+// load", 4: "group 1 may load"): bar.sync by the waiting group, bar.arrive by the releasing one.
+// Work items of CTA b: b, b + gridDim, b + 2 gridDim, ...  (148 CTAs x 6.92 planes at 32^4: 7 rounds, 1 % tail).
+#ifndef LGF_PP_TOKEN
+#define LGF_PP_TOKEN 1
+#endif
+#ifndef LGF_PP_PREFETCH
+#define LGF_PP_PREFETCH 0
+#endif
+template <int NT> struct PingPong {
+    int grp;
+    __device__ __forceinline__ void acquire(int round) const {
+        if (!LGF_PP_TOKEN) return;
+        if (grp == 1 || round > 0) asm volatile("bar.sync %0, %1;" ::"r"(3 + grp), "n"(2 * NT) : "memory");
+    }
+    // last: no later acquire of the other group will consume this release
+    __device__ __forceinline__ void release(bool last) const {
+        if (!LGF_PP_TOKEN) return;
+        if (grp == 0 || !last) asm volatile("bar.arrive %0, %1;" ::"r"(3 + (grp ^ 1)), "n"(2 * NT) : "memory");
+    }
+};
+
+template <int LG0, int LG1, int NC, int NT>
+__global__ void __launch_bounds__(2 * NT, 1) k_pp_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
+                                                            Geom G, FftTables T, const Ctl* __restrict__ ctl) {
+    if (ctl->done) return;
+    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red2[2][64];
+    const int grp = threadIdx.x / NT;
+    const Grp g{(int)threadIdx.x % NT, 1 + grp};
+    const PingPong<NT> pp{grp};
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw) + grp * 4 * SC;
+    cplx* tw0 = reinterpret_cast<cplx*>(smem_raw) + 8 * SC;
+    cplx* tw1 = tw0 + L0;
+    for (int i = threadIdx.x; i < L0; i += 2 * NT) tw0[i] = T.tw[0][i];
+    for (int i = threadIdx.x; i < L1; i += 2 * NT) tw1[i] = T.tw[1][i];
+    __syncthreads();
+    const int n_all = G.L[2] * G.L[3];
+    const int n_items = (n_all - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int rounds = (n_items + 1) >> 1;
+#pragma unroll 1
+    for (int r = 0; r < rounds; r++) {
+        const int k = 2 * r + grp;
+        const bool active = k < n_items;
+        const int plane = blockIdx.x + k * gridDim.x;
+        pp.acquire(r);
+        if (active) pass_a_delta<LG0, LG1, NC, NT>(links, G, plane, tile, red2[grp], partials, g);
+        pp.release(r == rounds - 1);
+        if (LGF_PP_PREFETCH && k + 2 < n_items && g.tid < 4 * NC) {
+            // DRAM -> L2 prefetch of the group's next plane (4*NC contiguous runs of L0*L1 entries) while it transforms this one
+            const long long xn = (long long)(plane + 2 * (int)gridDim.x) << (LG0 + LG1);
+            prefetch_l2(links + (long long)g.tid * G.V + xn, (unsigned)(L0 * L1 * sizeof(cplx)));
+        }
+        if (active) {
+            plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)plane << (LG0 + LG1), g);
+            gsync<NT>(g);      // the tile is free for the group's next item
+        }
+    }
+}
+
+template <int LG0, int LG1, int NT>
+__global__ void __launch_bounds__(2 * NT, 1) k_pp_inv(cplx* __restrict__ field, Geom G, FftTables T, const Ctl* __restrict__ ctl) {
+    if (ctl->done) return;
+    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int grp = threadIdx.x / NT;
+    const Grp g{(int)threadIdx.x % NT, 1 + grp};
+    const PingPong<NT> pp{grp};
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw) + grp * 4 * SC;
+    cplx* tw0 = reinterpret_cast<cplx*>(smem_raw) + 8 * SC;
+    cplx* tw1 = tw0 + L0;
+    for (int i = threadIdx.x; i < L0; i += 2 * NT) tw0[i] = T.tw[0][i];
+    for (int i = threadIdx.x; i < L1; i += 2 * NT) tw1[i] = T.tw[1][i];
+    __syncthreads();
+    const int n_all = G.L[2] * G.L[3];
+    const int n_items = (n_all - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int rounds = (n_items + 1) >> 1;
+#pragma unroll 1
+    for (int r = 0; r < rounds; r++) {
+        const int k = 2 * r + grp;
+        const bool active = k < n_items;
+        cplx* fbase = field + ((long long)(blockIdx.x + k * gridDim.x) << (LG0 + LG1));
+        pp.acquire(r);
+        if (active) pass_c_load<LG0, LG1, 4, NT>(fbase, G.V, tile, g);
+        pp.release(r == rounds - 1);
+        if (active) {
+            pass_c_finish<LG0, LG1, 4, NT, false>(fbase, nullptr, 0.0, G.V, tile, tw0, tw1, g);
+            gsync<NT>(g);
+        }
+    }
+}
+
+template <int LG2, int LG3, int LGC, int NT>
+__global__ void __launch_bounds__(2 * NT, 1) k_pp_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+    if (ctl->done) return;
+    using MG = MidGeom<LG2, LGC>;
+    constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, TILE = MG::S2 * L3;
+    static_assert(NT % C0 == 0, "a thread keeps its x0 offset");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int grp = threadIdx.x / NT;
+    const Grp g{(int)threadIdx.x % NT, 1 + grp};
+    const PingPong<NT> pp{grp};
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw) + grp * TILE;
+    cplx* tw2 = reinterpret_cast<cplx*>(smem_raw) + 2 * TILE;
+    cplx* tw3 = tw2 + L2;
+    double* s2 = reinterpret_cast<double*>(tw3 + L3);
+    double* s3 = s2 + L2;
+    for (int i = threadIdx.x; i < L2; i += 2 * NT) { tw2[i] = T.tw[2][i]; s2[i] = T.s[2][i]; }
+    for (int i = threadIdx.x; i < L3; i += 2 * NT) { tw3[i] = T.tw[3][i]; s3[i] = T.s[3][i]; }
+    __syncthreads();
+    const int i0 = g.tid % C0;
+    const int n_all = 4 * G.L[1] * (G.L[0] >> LGC);
+    const int n_items = (n_all - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int rounds = (n_items + 1) >> 1;
+    const int sh2 = G.sh[2], sh3 = G.sh[3];
+#pragma unroll 1
+    for (int r = 0; r < rounds; r++) {
+        const int k = 2 * r + grp;
+        const bool active = k < n_items;
+        MidItem it;
+        pp.acquire(r);
+        if (active) {
+            it = mid_item<LGC>(field, G, T, blockIdx.x + k * gridDim.x, i0);
+            pass_b_load<LG2, LG3, LGC, NT>(it.gp, sh2, sh3, tile + i0, tw2, g);
+        }
+        pp.release(r == rounds - 1);
+        if (active) {
+            pass_b_finish<LG2, LG3, LGC, NT>(it.gp, it.s01, sh2, sh3, scale, tile + i0, tw2, tw3, s2, s3, g);
+            gsync<NT>(g);
         }
     }
 }

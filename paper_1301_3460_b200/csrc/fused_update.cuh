@@ -211,7 +211,7 @@ __global__ void __launch_bounds__(NT, LGF_FU_MINB) k_fu_update_delta_fwd(cplx* _
     if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
     __syncthreads();
 
-    plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, V, xbase);
+    plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, V, xbase, Grp{(int)threadIdx.x, 0});
 }
 
 }  // namespace lgf

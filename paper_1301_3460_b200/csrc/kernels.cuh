@@ -267,8 +267,14 @@ __global__ void __launch_bounds__(256) k_fft23_mid(cplx* __restrict__ field, Geo
 // One thread per site.  STORE_G = 0: g(x) and g(x+mu) are rebuilt from the packed X field (5 Gram-Schmidt per
 // site, 64 B/site read once from HBM, neighbours from L1/L2).  STORE_G = 1: rows 0,1 of g are read from gbuf
 // (96 B/site) and row 2 is rebuilt.  Each link (x,mu) is read and written by exactly one thread: in place.
+#ifndef LGF_UPD_NT
+#define LGF_UPD_NT 128
+#endif
+#ifndef LGF_UPD_MINB
+#define LGF_UPD_MINB 3
+#endif
 template <int NC, int STORE_G>
-__global__ void __launch_bounds__(128) k_update(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G, double half_alpha, Ctl* ctl) {
+__global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G, double half_alpha, Ctl* ctl) {
     if (ctl->done) return;
     const long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long V = G.V;
@@ -278,7 +284,7 @@ __global__ void __launch_bounds__(128) k_update(cplx* __restrict__ links, const 
         for (int c = 0; c < 6; c++) g[c] = ldg2(src + (long long)c * V + x);
         third_row(g);
     } else {
-        build_g(ldg2(src + x), ldg2(src + V + x), ldg2(src + 2 * V + x), ldg2(src + 3 * V + x), half_alpha, g);
+        build_g(ldc_field(src + x), ldc_field(src + V + x), ldc_field(src + 2 * V + x), ldc_field(src + 3 * V + x), half_alpha, g);
     }
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) {
@@ -290,7 +296,7 @@ __global__ void __launch_bounds__(128) k_update(cplx* __restrict__ links, const 
             for (int c = 0; c < 6; c++) gp[c] = ldg2(src + (long long)c * V + xf);
             third_row(gp);
         } else {
-            build_g(ldg2(src + xf), ldg2(src + V + xf), ldg2(src + 2 * V + xf), ldg2(src + 3 * V + xf), half_alpha, gp);
+            build_g(ldc_field(src + xf), ldc_field(src + V + xf), ldc_field(src + 2 * V + xf), ldc_field(src + 3 * V + xf), half_alpha, gp);
         }
         rotate_link<(NC == 6) ? 2 : 3>(g, u, gp, r);
         store_link<NC>(links, V, mu, x, r);

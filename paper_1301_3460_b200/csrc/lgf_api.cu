@@ -19,12 +19,14 @@ namespace {
 
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
-    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE, K_NSLOTS
+    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE,
+    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
-    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd"};
+    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd",
+    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv"};
 
 constexpr int HIST_CAP = 1 << 16;
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
@@ -115,11 +117,12 @@ struct lgf_ctx {
     Ctl* h_ctl;             // pinned
     bool loaded;
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin;
+    int sms;                // SMs of the device: grid of the persistent passes
     int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
-    bool fast_a, fast_b, fast_c;
-    size_t smem_fa, smem_fb, smem_fc, smem_fu;
+    bool fast_a, fast_b, fast_c, pp_b_ok;
+    size_t smem_fa, smem_fb, smem_fc, smem_fu, smem_pa, smem_pb;
     int fb_lgC;
     // derived launch parameters
     int fft01_ncomp_fused_ok, fft01_ncomp, fft01_threads, fft23_lgC, fft23_S1, fft23_S2, fft23_threads;
@@ -182,7 +185,14 @@ template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
 constexpr int FA_NT = 256;
 // (lg of the fast axis, lg of the slow axis) pairs instantiated for each pass
 #define LGF_FAST_PAIRS(X) X(4, 4) X(4, 5) X(5, 4) X(5, 5)
-constexpr int fast_mid_lgC(int lga, int lgb) { return (lga + lgb >= 10) ? 2 : 3; }   // x0 chunk: tile <= 64 KB
+#ifndef LGF_FB_LGC55
+#define LGF_FB_LGC55 2
+#endif
+#ifndef LGF_FB_NT
+#define LGF_FB_NT 256
+#endif
+constexpr int FB_NT = LGF_FB_NT;
+constexpr int fast_mid_lgC(int lga, int lgb) { return (lga + lgb >= 10) ? LGF_FB_LGC55 : 3; }   // x0 chunk: tile <= 64 KB
 bool fast_pair(int lga, int lgb) {
 #define X(A, B) if (lga == A && lgb == B) return true;
     LGF_FAST_PAIRS(X)
@@ -195,11 +205,13 @@ size_t smem_fast_mid(int lga, int lgb, int lgC) {
     return (size_t)(S2 * (1 << lgb) + (1 << lga) + (1 << lgb)) * 16 + (size_t)((1 << lga) + (1 << lgb)) * 8;
 }
 
-template <int NC> void launch_fa_delta_fwd(lgf_ctx* c) {
+// fin: the last CTA also does S5 (no k_finalize launch)
+template <int NC> void launch_fa_delta_fwd(lgf_ctx* c, bool fin) {
     LaunchScope ls(c, K_FA_DELTA_FWD);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
+    const FinArgs fa{c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), fin ? 1 : 0};
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_delta_fwd<A, B, NC, FA_NT><<<grid, FA_NT, c->smem_fa, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->T, c->ctl);
+        k_fa_delta_fwd<A, B, NC, FA_NT><<<grid, FA_NT, c->smem_fa, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->T, c->ctl, fa);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -234,7 +246,35 @@ void launch_fa_mid(lgf_ctx* c) {
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
     const double scale = 16.0 / (double)c->G.V;
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        k_fa_mid<A, B, fast_mid_lgC(A, B), FA_NT><<<grid, FA_NT, c->smem_fb, c->stream>>>(c->field, c->G, c->T, scale, c->ctl);
+        k_fa_mid<A, B, fast_mid_lgC(A, B), FB_NT><<<grid, FB_NT, c->smem_fb, c->stream>>>(c->field, c->G, c->T, scale, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+
+// persistent ping-pong forms of the three passes (fft_fast.cuh): one CTA per SM, two groups of FA_NT threads
+unsigned pp_grid(const lgf_ctx* c, long long items) { return (unsigned)(items < c->sms ? items : c->sms); }
+template <int NC> void launch_pp_delta_fwd(lgf_ctx* c) {
+    LaunchScope ls(c, K_PP_DELTA_FWD);
+    const unsigned grid = pp_grid(c, c->G.L[2] * c->G.L[3]);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        k_pp_delta_fwd<A, B, NC, FA_NT><<<grid, 2 * FA_NT, c->smem_pa, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->T, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+void launch_pp_inv(lgf_ctx* c) {
+    LaunchScope ls(c, K_PP_INV);
+    const unsigned grid = pp_grid(c, c->G.L[2] * c->G.L[3]);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        k_pp_inv<A, B, FA_NT><<<grid, 2 * FA_NT, c->smem_pa, c->stream>>>(c->field, c->G, c->T, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+void launch_pp_mid(lgf_ctx* c) {
+    LaunchScope ls(c, K_PP_MID);
+    const unsigned grid = pp_grid(c, 4LL * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
+    const double scale = 16.0 / (double)c->G.V;
+#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
+        k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT><<<grid, 2 * FA_NT, c->smem_pb, c->stream>>>(c->field, c->G, c->T, scale, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -247,16 +287,23 @@ lgf_status setup_fast(lgf_ctx* c) {
     if (c->fb_lgC > G.lg[0]) c->fast_b = false;          // the x0 extent must hold one chunk
     c->smem_fa = c->smem_fc = c->smem_fu = smem_fast_plane(G.lg[0], G.lg[1], 4);
     c->smem_fb = smem_fast_mid(G.lg[2], G.lg[3], c->fb_lgC);
+    // two tiles + one set of tables
+    c->smem_pa = 2 * c->smem_fa - (size_t)(G.L[0] + G.L[1]) * 16;
+    c->smem_pb = 2 * c->smem_fb - ((size_t)(G.L[2] + G.L[3]) * 16 + (size_t)(G.L[2] + G.L[3]) * 8);
+    c->pp_b_ok = c->smem_pb <= (size_t)227 * 1024;
     if (c->fast_a) {
 #define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
             CK(set_smem(k_fa_delta_fwd<A, B, 6, FA_NT>, c->smem_fa)); CK(set_smem(k_fa_delta_fwd<A, B, 9, FA_NT>, c->smem_fa)); \
             CK(set_smem(k_fa_inv<A, B, 4, FA_NT, false>, c->smem_fc)); CK(set_smem(k_fa_inv<A, B, 4, FA_NT, true>, c->smem_fc)); \
-            CK(set_smem(k_fu_update_delta_fwd<A, B, 6, LGF_FU_NT>, c->smem_fu)); CK(set_smem(k_fu_update_delta_fwd<A, B, 9, LGF_FU_NT>, c->smem_fu)); }
+            CK(set_smem(k_fu_update_delta_fwd<A, B, 6, LGF_FU_NT>, c->smem_fu)); CK(set_smem(k_fu_update_delta_fwd<A, B, 9, LGF_FU_NT>, c->smem_fu)); \
+            CK(set_smem(k_pp_delta_fwd<A, B, 6, FA_NT>, c->smem_pa)); CK(set_smem(k_pp_delta_fwd<A, B, 9, FA_NT>, c->smem_pa)); \
+            CK(set_smem(k_pp_inv<A, B, FA_NT>, c->smem_pa)); }
         LGF_FAST_PAIRS(X)
 #undef X
     }
     if (c->fast_b) {
-#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), FA_NT>, c->smem_fb));
+#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) { CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), FB_NT>, c->smem_fb)); \
+            if (c->pp_b_ok) CK(set_smem(k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, c->smem_pb)); }
         LGF_FAST_PAIRS(X)
 #undef X
     }
@@ -354,7 +401,7 @@ void launch_finalize(lgf_ctx* c, int n_partials, int advance = 0) {
 }
 template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
     LaunchScope ls(c, SG ? K_UPDATE_G : K_UPDATE_X);
-    k_update<NC, SG><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(cur_links(c), SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
+    k_update<NC, SG><<<(unsigned)(c->G.V / LGF_UPD_NT), LGF_UPD_NT, 0, c->stream>>>(cur_links(c), SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
 }
 
 bool use_fused(const lgf_ctx* c) { return c->opt_fuse && c->fft01_ncomp_fused_ok; }
@@ -363,18 +410,24 @@ bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a && use_fused
 bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
 bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c && !use_store_g(c); }
 bool use_fused_update(const lgf_ctx* c) { return c->opt_fuse_update && c->opt_fast && c->fast_a; }
+bool use_pp_a(const lgf_ctx* c) { return (c->opt_pingpong & 1) && use_fast_a(c); }
+bool use_pp_b(const lgf_ctx* c) { return (c->opt_pingpong & 2) && use_fast_b(c) && c->pp_b_ok; }
+bool use_pp_c(const lgf_ctx* c) { return (c->opt_pingpong & 4) && use_fast_c(c); }
 
 // S1 (+ pass A) and the reduction.  Returns the number of partials written.
 template <int NC> void enqueue_head(lgf_ctx* c) {
     int np;
-    if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
+    if (use_pp_a(c)) { launch_pp_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
+    else if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c, c->opt_fuse_fin != 0); if (c->opt_fuse_fin) return; np = c->G.L[2] * c->G.L[3]; }
     else if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
     else { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fft01<MODE_FWD, 6>(c, K_FFT01_FWD, 0.0); }
     launch_finalize(c, np);
 }
 // pass B, pass C, update
-void launch_mid(lgf_ctx* c) { if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c); }
-void launch_inv_x(lgf_ctx* c) { if (use_fast_c(c)) launch_fa_inv(c); else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, 0.0); }
+void launch_mid(lgf_ctx* c) { if (use_pp_b(c)) launch_pp_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c); }
+void launch_inv_x(lgf_ctx* c) {
+    if (use_pp_c(c)) launch_pp_inv(c); else if (use_fast_c(c)) launch_fa_inv(c); else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, 0.0);
+}
 template <int NC> void enqueue_tail(lgf_ctx* c, double half_alpha) {
     launch_mid(c);
     if (use_store_g(c)) { launch_fft01<MODE_INV_G, 6>(c, K_FFT01_INV_G, half_alpha); launch_update<NC, 1>(c, half_alpha); }
@@ -392,7 +445,8 @@ void enqueue_body(lgf_ctx* c, double half_alpha) {
     if (c->NC == 6) { enqueue_head<6>(c); enqueue_tail<6>(c, half_alpha); }
     else { enqueue_head<9>(c); enqueue_tail<9>(c, half_alpha); }
 }
-int launches_per_body(const lgf_ctx* c) { return use_fused_update(c) ? 4 : (use_fused(c) ? 5 : 6); }
+bool use_fused_fin(const lgf_ctx* c) { return c->opt_fuse_fin && use_fast_a(c) && !use_pp_a(c); }
+int launches_per_body(const lgf_ctx* c) { return use_fused_update(c) ? 4 : (use_fused_fin(c) ? 4 : (use_fused(c) ? 5 : 6)); }
 
 lgf_status reset_ctl(lgf_ctx* c, double tol, int max_iter) {
     Ctl h; memset(&h, 0, sizeof h);
@@ -421,7 +475,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -489,7 +543,8 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0;
+    { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
     c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
     c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr;
@@ -716,6 +771,8 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_BATCH: if (value < 1 || value > 1024) return LGF_ERR_INVALID_ARG; c->opt_batch = value; break;
         case LGF_OPT_FAST_FFT: c->opt_fast = value ? 1 : 0; break;
         case LGF_OPT_FUSE_UPDATE: c->opt_fuse_update = value ? 1 : 0; break;
+        case LGF_OPT_PINGPONG: if (value < 0 || value > 7) return LGF_ERR_INVALID_ARG; c->opt_pingpong = value; break;
+        case LGF_OPT_FUSE_FINALIZE: c->opt_fuse_fin = value ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
@@ -729,6 +786,8 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_BATCH: *value = c->opt_batch; break;
         case LGF_OPT_FAST_FFT: *value = (use_fast_a(c) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | (use_fast_c(c) ? 4 : 0); break;
         case LGF_OPT_FUSE_UPDATE: *value = use_fused_update(c) ? 1 : 0; break;
+        case LGF_OPT_PINGPONG: *value = (use_pp_a(c) ? 1 : 0) | (use_pp_b(c) ? 2 : 0) | (use_pp_c(c) ? 4 : 0); break;
+        case LGF_OPT_FUSE_FINALIZE: *value = use_fused_fin(c) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;

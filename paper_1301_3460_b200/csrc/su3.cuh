@@ -43,6 +43,48 @@ __device__ __forceinline__ void third_row(cplx (&u)[9]) {
 // 128-bit loads/stores of one complex double
 __device__ __forceinline__ cplx ldg2(const cplx* p) { return __ldg(p); }
 
+// L2 residency control (createpolicy + ld/st .L2::cache_hint).  The packed field (64 B/site: 67 MB at 32^4) is
+// touched by every kernel of an iteration and fits the 126 MB L2; the links (384 B/site) are streamed once per
+// kernel and do not.  LGF_L2HINT bit 0: field accesses evict_last; bit 1: link accesses evict_first.
+#ifndef LGF_L2HINT
+#define LGF_L2HINT 0
+#endif
+__device__ __forceinline__ unsigned long long l2_policy_last() {
+    unsigned long long p; asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_first() {
+    unsigned long long p; asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ cplx ld_hint(const cplx* p, unsigned long long pol) {
+    cplx v; asm volatile("ld.global.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol)); return v;
+}
+__device__ __forceinline__ cplx ldnc_hint(const cplx* p, unsigned long long pol) {
+    cplx v; asm("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol)); return v;
+}
+__device__ __forceinline__ void st_hint(cplx* p, cplx v, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+// field (Delta~ / X~ / X) accesses: ld_field where the same kernel later overwrites the location (plain load),
+// ldc_field where the field is read-only for the kernel (non-coherent path)
+__device__ __forceinline__ cplx ld_field(const cplx* p) {
+    if (LGF_L2HINT & 1) return ld_hint(p, l2_policy_last());
+    return *p;
+}
+__device__ __forceinline__ cplx ldc_field(const cplx* p) {
+    if (LGF_L2HINT & 1) return ldnc_hint(p, l2_policy_last());
+    return __ldg(p);
+}
+__device__ __forceinline__ void st_field(cplx* p, cplx v) {
+    if (LGF_L2HINT & 1) st_hint(p, v, l2_policy_last()); else *p = v;
+}
+__device__ __forceinline__ cplx ld_lnk(const cplx* p) {
+    if (LGF_L2HINT & 2) return ldnc_hint(p, l2_policy_first());
+    return __ldg(p);
+}
+__device__ __forceinline__ void st_lnk(cplx* p, cplx v) {
+    if (LGF_L2HINT & 2) st_hint(p, v, l2_policy_first()); else *p = v;
+}
+
 // Asynchronous DRAM -> L2 prefetch of `bytes` contiguous bytes (multiple of 16, 16-byte aligned): no register or
 // shared-memory destination, so the bytes in flight are not bounded by the register file (sm_90+ bulk prefetch).
 __device__ __forceinline__ void prefetch_l2(const void* p, unsigned bytes) {
@@ -55,14 +97,14 @@ template <int NC>
 __device__ __forceinline__ void load_link(const cplx* __restrict__ links, long long V, int mu, long long x, cplx (&u)[9]) {
     const cplx* p = links + (long long)(mu * NC) * V + x;
 #pragma unroll
-    for (int c = 0; c < NC; c++) u[c] = ldg2(p + (long long)c * V);
+    for (int c = 0; c < NC; c++) u[c] = ld_lnk(p + (long long)c * V);
     if (NC == 6) third_row(u);
 }
 template <int NC>
 __device__ __forceinline__ void store_link(cplx* __restrict__ links, long long V, int mu, long long x, const cplx (&u)[9]) {
     cplx* p = links + (long long)(mu * NC) * V + x;
 #pragma unroll
-    for (int c = 0; c < NC; c++) p[(long long)c * V] = u[c];
+    for (int c = 0; c < NC; c++) st_lnk(p + (long long)c * V, u[c]);
 }
 
 // S3: g = rowGramSchmidt(M), M = 1 + (alpha/2) X, X given by its packed independent components

@@ -25,9 +25,10 @@ def theta_close(t_gpu, t_ref):
 
 def all_variants(gf):
     """Every kernel selection the library offers:
-    (fuse Delta into FFT pass A, store g, CUDA graph, compile-time-sized FFT passes, fused update + next Delta)."""
+    (fuse Delta into FFT pass A, store g, CUDA graph, compile-time-sized FFT passes, fused update + next Delta
+    [, ping-pong mask of the persistent passes; default 0 [, S5 inside pass A; default 0]])."""
     if gf.V > (1 << 18):
-        return [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 0, 0, 0), (0, 1, 1, 1, 0), (0, 0, 0, 0, 0)]
+        return [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 0, 0), (0, 1, 1, 1, 0), (0, 0, 0, 0, 0)]
     out = []
     for fast in (1, 0):
         for fuse in (1, 0):
@@ -35,6 +36,8 @@ def all_variants(gf):
                 for graph in (1, 0):
                     out.append((fuse, store_g, graph, fast, 0))
     out += [(1, 0, 1, 1, 1), (1, 0, 0, 1, 1)]       # the fused update needs the fast passes; the other switches do not enter
+    # the persistent ping-pong passes, all or one at a time; S5 inside pass A
+    out += [(1, 0, 1, 1, 0, 7), (0, 0, 0, 1, 0, 7), (1, 0, 1, 1, 0, 1), (1, 0, 1, 1, 0, 2), (1, 0, 0, 1, 0, 4), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 1, 0, 0, 1)]
     return out
 
 
@@ -44,6 +47,8 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_GRAPH, v[2])
     gf.set_option(lgf.LGF_OPT_FAST_FFT, v[3])
     gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, v[4])
+    gf.set_option(lgf.LGF_OPT_PINGPONG, v[5] if len(v) > 5 else 0)
+    gf.set_option(lgf.LGF_OPT_FUSE_FINALIZE, v[6] if len(v) > 6 else 0)
 
 
 # ------------------------------------------------------------------ boundary: load -> get
@@ -153,7 +158,7 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
     assert hist_ref[n_ref, 1] < TOL, "oracle did not converge inside the trajectory"
 
     gf = lgf.GaugeFixer(dims, storage)
-    for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (0, 1, 0, 0, 0)]:
+    for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (0, 1, 0, 0, 0)]:
         set_variant(gf, v)
         gf.load_links(U)
         done = 0
@@ -373,7 +378,8 @@ def test_fused_update_buffers_and_counts():
     o.load(U)
     n0 = gf.launch_count()
     F, th = gf.iterate(3, ALPHA)                          # odd: the current links are in the second buffer
-    assert gf.launch_count() - n0 == 2 + 4 * 3            # measurement 0 (2 kernels) + 3 bodies of 4
+    head = 1 if gf.get_option(lgf.LGF_OPT_FUSE_FINALIZE) else 2
+    assert gf.launch_count() - n0 == head + 4 * 3         # measurement 0 (pass A [+ k_finalize]) + 3 bodies of 4
     F_ref, th_ref = o.iterate(3, ALPHA)
     assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
     U3 = gf.get_links()
@@ -416,5 +422,11 @@ def test_fast_fft_pass_selection():
                        ((16, 32, 4, 8), 5), ((4, 8, 16, 32), 0), ((8, 8, 8, 8), 0)]:
         gf = lgf.GaugeFixer(dims, 12)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
+        assert gf.get_option(lgf.LGF_OPT_PINGPONG) == 0, dims
+        gf.set_option(lgf.LGF_OPT_PINGPONG, 7)
+        assert gf.get_option(lgf.LGF_OPT_PINGPONG) == mask, dims      # every fast pass has a persistent form
+        gf.set_option(lgf.LGF_OPT_PINGPONG, 2)
+        assert gf.get_option(lgf.LGF_OPT_PINGPONG) == (mask & 2), dims
         gf.set_option(lgf.LGF_OPT_FAST_FFT, 0)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == 0
+        assert gf.get_option(lgf.LGF_OPT_PINGPONG) == 0
