@@ -48,6 +48,7 @@ def kernel_bytes_per_site(nc: int) -> dict:
         "k_fft01_inv_g": 64 + 96,
         "k_update_x": 64 + 2 * lk,           # read X once (neighbours: cache), read + write links
         "k_update_g": 96 + 2 * lk,
+        "k_update_quad": 64 + 2 * lk,        # same traffic as k_update_x, one thread per link
         "k_finalize": 0,
         # compile-time-sized passes (fft_fast.cuh): same traffic as the generic passes they replace
         "k_fa_delta_fwd": lk + 64,

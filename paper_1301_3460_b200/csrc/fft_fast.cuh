@@ -286,10 +286,23 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cp
     cplx* tw1 = tw0 + L0;
     __shared__ double red[64];
     const Grp g{(int)threadIdx.x, 0};
+#if defined(LGF_A_PREFETCH) && LGF_A_PREFETCH
+    if (threadIdx.x < 4 * NC)     // experiment: DRAM -> L2 bulk prefetch of the CTA's own plane
+        prefetch_l2(links + (long long)threadIdx.x * G.V + ((long long)blockIdx.x << (LG0 + LG1)), (unsigned)(L0 * L1 * sizeof(cplx)));
+#endif
     for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
     for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
+#if defined(LGF_DBG_A) && LGF_DBG_A == 2      // timing experiment: no S1 (tile filled with constants)
+    for (int e = threadIdx.x; e < 4 * SC; e += NT) tile[e] = mk(1e-3 * (e & 15), 1e-3);
+    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(1.0, 1.0);
+    __syncthreads();
+#else
     pass_a_delta<LG0, LG1, NC, NT>(links, G, blockIdx.x, tile, red, partials, g);
+#endif
     if (fa.on) finalize_last_cta<NT>(partials, gridDim.x, ctl, fa, red);
+#if defined(LGF_DBG_A) && LGF_DBG_A == 1      // timing experiment: no FFT, no field store
+    return;
+#endif
     plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)blockIdx.x << (LG0 + LG1), g);
 }
 

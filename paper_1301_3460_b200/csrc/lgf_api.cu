@@ -20,13 +20,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE,
-    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_NSLOTS
+    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd",
-    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv"};
+    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad"};
 
 constexpr int HIST_CAP = 1 << 16;
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
@@ -117,7 +117,7 @@ struct lgf_ctx {
     Ctl* h_ctl;             // pinned
     bool loaded;
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad;
     int sms;                // SMs of the device: grid of the persistent passes
     int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
@@ -182,7 +182,15 @@ template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
 }
 
 // ---- fast (compile-time-sized) FFT passes: the lattices they cover, and their launchers -----------------------
-constexpr int FA_NT = 256;
+#ifndef LGF_FA_NT
+#define LGF_FA_NT 256
+#endif
+#ifndef LGF_FC_NT
+#define LGF_FC_NT 256
+#endif
+constexpr int FA_NT = 256;            // group size of the ping-pong passes
+constexpr int FAD_NT = LGF_FA_NT;     // threads per CTA of pass A (k_fa_delta_fwd)
+constexpr int FC_NT = LGF_FC_NT;      // threads per CTA of pass C (k_fa_inv)
 // (lg of the fast axis, lg of the slow axis) pairs instantiated for each pass
 #define LGF_FAST_PAIRS(X) X(4, 4) X(4, 5) X(5, 4) X(5, 5)
 #ifndef LGF_FB_LGC55
@@ -211,7 +219,7 @@ template <int NC> void launch_fa_delta_fwd(lgf_ctx* c, bool fin) {
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
     const FinArgs fa{c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), fin ? 1 : 0};
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_delta_fwd<A, B, NC, FA_NT><<<grid, FA_NT, c->smem_fa, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->T, c->ctl, fa);
+        k_fa_delta_fwd<A, B, NC, FAD_NT><<<grid, FAD_NT, c->smem_fa, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->T, c->ctl, fa);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -219,7 +227,7 @@ void launch_fa_inv(lgf_ctx* c) {
     LaunchScope ls(c, K_FA_INV);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_inv<A, B, 4, FA_NT, false><<<grid, FA_NT, c->smem_fc, c->stream>>>(c->field, nullptr, 0.0, c->G, c->T, c->ctl);
+        k_fa_inv<A, B, 4, FC_NT, false><<<grid, FC_NT, c->smem_fc, c->stream>>>(c->field, nullptr, 0.0, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -227,7 +235,7 @@ void launch_fa_inv_g(lgf_ctx* c, double half_alpha) {
     LaunchScope ls(c, K_FA_INV_G);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_inv<A, B, 4, FA_NT, true><<<grid, FA_NT, c->smem_fc, c->stream>>>(c->field, c->gbuf, half_alpha, c->G, c->T, c->ctl);
+        k_fa_inv<A, B, 4, FC_NT, true><<<grid, FC_NT, c->smem_fc, c->stream>>>(c->field, c->gbuf, half_alpha, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -293,8 +301,8 @@ lgf_status setup_fast(lgf_ctx* c) {
     c->pp_b_ok = c->smem_pb <= (size_t)227 * 1024;
     if (c->fast_a) {
 #define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
-            CK(set_smem(k_fa_delta_fwd<A, B, 6, FA_NT>, c->smem_fa)); CK(set_smem(k_fa_delta_fwd<A, B, 9, FA_NT>, c->smem_fa)); \
-            CK(set_smem(k_fa_inv<A, B, 4, FA_NT, false>, c->smem_fc)); CK(set_smem(k_fa_inv<A, B, 4, FA_NT, true>, c->smem_fc)); \
+            CK(set_smem(k_fa_delta_fwd<A, B, 6, FAD_NT>, c->smem_fa)); CK(set_smem(k_fa_delta_fwd<A, B, 9, FAD_NT>, c->smem_fa)); \
+            CK(set_smem(k_fa_inv<A, B, 4, FC_NT, false>, c->smem_fc)); CK(set_smem(k_fa_inv<A, B, 4, FC_NT, true>, c->smem_fc)); \
             CK(set_smem(k_fu_update_delta_fwd<A, B, 6, LGF_FU_NT>, c->smem_fu)); CK(set_smem(k_fu_update_delta_fwd<A, B, 9, LGF_FU_NT>, c->smem_fu)); \
             CK(set_smem(k_pp_delta_fwd<A, B, 6, FA_NT>, c->smem_pa)); CK(set_smem(k_pp_delta_fwd<A, B, 9, FA_NT>, c->smem_pa)); \
             CK(set_smem(k_pp_inv<A, B, FA_NT>, c->smem_pa)); }
@@ -400,6 +408,11 @@ void launch_finalize(lgf_ctx* c, int n_partials, int advance = 0) {
     k_finalize<<<1, 256, 0, c->stream>>>(c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), advance);
 }
 template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
+    if (!SG && c->opt_quad) {
+        LaunchScope ls(c, K_UPDATE_QUAD);
+        k_update_quad<NC><<<(unsigned)(c->G.V / 32), 128, 0, c->stream>>>(cur_links(c), c->field, c->G, half_alpha, c->ctl);
+        return;
+    }
     LaunchScope ls(c, SG ? K_UPDATE_G : K_UPDATE_X);
     k_update<NC, SG><<<(unsigned)(c->G.V / LGF_UPD_NT), LGF_UPD_NT, 0, c->stream>>>(cur_links(c), SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
 }
@@ -475,7 +488,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -543,7 +556,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
     c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
@@ -773,6 +786,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_FUSE_UPDATE: c->opt_fuse_update = value ? 1 : 0; break;
         case LGF_OPT_PINGPONG: if (value < 0 || value > 7) return LGF_ERR_INVALID_ARG; c->opt_pingpong = value; break;
         case LGF_OPT_FUSE_FINALIZE: c->opt_fuse_fin = value ? 1 : 0; break;
+        case LGF_OPT_QUAD_UPDATE: c->opt_quad = value ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
@@ -788,6 +802,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_FUSE_UPDATE: *value = use_fused_update(c) ? 1 : 0; break;
         case LGF_OPT_PINGPONG: *value = (use_pp_a(c) ? 1 : 0) | (use_pp_b(c) ? 2 : 0) | (use_pp_c(c) ? 4 : 0); break;
         case LGF_OPT_FUSE_FINALIZE: *value = use_fused_fin(c) ? 1 : 0; break;
+        case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
