@@ -130,10 +130,14 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_QUAD_UPDATE     1 (default): S3+S4 with one thread per link, the four directions of 32 sites per CTA, g(x)
  *                           taken from the thread that built it as g((x-0)+0) (4 Gram-Schmidt per site, k_update_quad),
  *                           0: one thread per site (5 Gram-Schmidt per site, k_update).  Applies when g is recomputed
- *                           from X (LGF_OPT_STORE_G = 0, LGF_OPT_FUSE_UPDATE = 0); lgf_get_option returns whether it runs. */
+ *                           from X (LGF_OPT_STORE_G = 0, LGF_OPT_FUSE_UPDATE = 0); lgf_get_option returns whether it runs.
+ *   LGF_OPT_PDL             1 (default): the kernels of an iteration are launched with programmatic dependent launch
+ *                           (each waits on the device for the complete end of its predecessor, so results are
+ *                           unchanged; launch latency and CTA ramp-up overlap the predecessor's tail), 0: plain
+ *                           stream-ordered launches. */
 typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
                LGF_OPT_FUSE_UPDATE = 5, LGF_OPT_PINGPONG = 6, LGF_OPT_FUSE_FINALIZE = 7,
-               LGF_OPT_QUAD_UPDATE = 8 } lgf_option;
+               LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

@@ -21,6 +21,11 @@
 #ifndef LGF_FA_MINB_DELTA
 #define LGF_FA_MINB_DELTA 2
 #endif
+// 1: pass A runs its middle stages as two 8-point-or-smaller stages instead of one 16-point register block (fewer
+// registers per thread, one more shared-memory round trip)
+#ifndef LGF_FA_NOBLOCK16
+#define LGF_FA_NOBLOCK16 0
+#endif
 #ifndef LGF_FA_MINB_MID
 #define LGF_FA_MINB_MID 2
 #endif
@@ -118,7 +123,7 @@ __device__ __forceinline__ void plane_middle(cplx* __restrict__ t, const cplx* _
     using PA = Plan2<LGA, false>;
     using PB = Plan2<LGB, true>;
     constexpr int LA = PA::L, LB = PB::L, S = LA + 1, SC = S * LB;
-    if constexpr (PA::R2 * PB::R1 <= 16) {
+    if constexpr (PA::R2 * PB::R1 <= 16 && !(LGF_FA_NOBLOCK16 && !INV)) {
         // lanes run over jb (rows, odd stride S: conflict-free), then over the a-blocks
         constexpr int NW = NCOMP * PA::R1 * PB::R2;
 #pragma unroll
@@ -278,6 +283,7 @@ __device__ __forceinline__ void finalize_last_cta(const double2* partials, int n
 template <int LG0, int LG1, int NC, int NT>
 __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
                                                      Geom G, FftTables T, Ctl* ctl, FinArgs fa) {
+    pdl_enter();
     if (ctl->done) return;
     constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -399,6 +405,7 @@ template <int LG0, int LG1, int NCOMP, int NT, bool WRITE_G>
 __global__ void __launch_bounds__(NT, LGF_FA_MINB_INV) k_fa_inv(cplx* __restrict__ field, cplx* __restrict__ gbuf, double half_alpha, Geom G, FftTables T,
                                                                 const Ctl* __restrict__ ctl) {
     static_assert(!WRITE_G || NCOMP == 4, "g needs all four components of X");
+    pdl_enter();
     if (ctl->done) return;
     constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -570,6 +577,7 @@ __device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01,
 // Pass B: forward over axes 2,3, filter, inverse over axes 3,2, one work item per CTA.
 template <int LG2, int LG3, int LGC, int NT>
 __global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+    pdl_enter();
     if (ctl->done) return;
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0;
@@ -621,6 +629,7 @@ template <int NT> struct PingPong {
 template <int LG0, int LG1, int NC, int NT>
 __global__ void __launch_bounds__(2 * NT, 1) k_pp_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
                                                             Geom G, FftTables T, const Ctl* __restrict__ ctl) {
+    pdl_enter();
     if (ctl->done) return;
     constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -659,6 +668,7 @@ __global__ void __launch_bounds__(2 * NT, 1) k_pp_delta_fwd(const cplx* __restri
 
 template <int LG0, int LG1, int NT>
 __global__ void __launch_bounds__(2 * NT, 1) k_pp_inv(cplx* __restrict__ field, Geom G, FftTables T, const Ctl* __restrict__ ctl) {
+    pdl_enter();
     if (ctl->done) return;
     constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -691,6 +701,7 @@ __global__ void __launch_bounds__(2 * NT, 1) k_pp_inv(cplx* __restrict__ field, 
 
 template <int LG2, int LG3, int LGC, int NT>
 __global__ void __launch_bounds__(2 * NT, 1) k_pp_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+    pdl_enter();
     if (ctl->done) return;
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, TILE = MG::S2 * L3;

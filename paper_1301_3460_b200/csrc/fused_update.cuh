@@ -58,6 +58,7 @@ template <int LG0, int LG1, int NC, int NT>
 __global__ void __launch_bounds__(NT, LGF_FU_MINB) k_fu_update_delta_fwd(cplx* __restrict__ links2, long long buf_stride, const cplx* __restrict__ gbuf,
                                                                          cplx* __restrict__ field, double2* __restrict__ partials, Geom G, FftTables T,
                                                                          const Ctl* __restrict__ ctl) {
+    pdl_enter();
     if (ctl->done) return;
     using PA = Plan2<LG0, false>;
     using PB = Plan2<LG1, true>;

@@ -83,6 +83,7 @@ __device__ __forceinline__ void delta_site(const cplx* __restrict__ links, const
 template <int NC>
 __global__ void __launch_bounds__(128) k_delta(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
                                                Geom G, const Ctl* __restrict__ ctl) {
+    pdl_enter();
     if (ctl->done) return;
     __shared__ double red[64];
     const long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -101,6 +102,7 @@ __global__ void __launch_bounds__(128) k_delta(const cplx* __restrict__ links, c
 // fused_update.cuh): count it and make the buffer it wrote the current one.
 __global__ void __launch_bounds__(256) k_finalize(const double2* __restrict__ partials, int n, Ctl* ctl, double2* hist, double inv3V, double inv12V,
                                                   int advance) {
+    pdl_enter();
     if (ctl->done) return;
     __shared__ double red[64];
     double a = 0, b = 0;
@@ -137,6 +139,7 @@ template <int MODE, int NC>
 __global__ void __launch_bounds__(256) k_fft01(cplx* __restrict__ field, const cplx* __restrict__ links, cplx* __restrict__ gbuf,
                                                double2* __restrict__ partials, Geom G, FftTables T, int ncomp, double half_alpha,
                                                const Ctl* __restrict__ ctl) {
+    pdl_enter();
     if (ctl->done) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int L0 = G.L[0], L1 = G.L[1];
@@ -210,6 +213,7 @@ __global__ void __launch_bounds__(256) k_fft01(cplx* __restrict__ field, const c
 // tile[x3][x2][i0].  scale = 16/V folds p2max and the 1/V of the inverse transform.          [north_star step 2]
 __global__ void __launch_bounds__(256) k_fft23_mid(cplx* __restrict__ field, Geom G, FftTables T, int lgC, int S1, int S2, double scale,
                                                    const Ctl* __restrict__ ctl) {
+    pdl_enter();
     if (ctl->done) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int L2 = G.L[2], L3 = G.L[3];
@@ -280,6 +284,7 @@ __global__ void __launch_bounds__(256) k_fft23_mid(cplx* __restrict__ field, Geo
 #endif
 template <int NC, int STORE_G>
 __global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G, double half_alpha, Ctl* ctl) {
+    pdl_enter();
     if (ctl->done) return;
     const long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long V = G.V;
@@ -320,6 +325,7 @@ __global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __res
 #endif
 template <int NC>
 __global__ void __launch_bounds__(128, LGF_UPDQ_MINB) k_update_quad(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G, double half_alpha, Ctl* ctl) {
+    pdl_enter();
     if (ctl->done) return;
     __shared__ cplx sg[9][32];
     const int lane = threadIdx.x & 31, mu = threadIdx.x >> 5;

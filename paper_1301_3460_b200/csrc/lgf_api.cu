@@ -117,7 +117,7 @@ struct lgf_ctx {
     Ctl* h_ctl;             // pinned
     bool loaded;
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl;
     int sms;                // SMs of the device: grid of the persistent passes
     int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
@@ -172,6 +172,19 @@ struct LaunchScope {
     }
 };
 
+// Launch of an iteration-body kernel: with opt_pdl the launch carries the programmatic-stream-serialization attribute
+// (the kernels call pdl_enter(), su3.cuh); stream capture turns it into a programmatic graph edge.
+template <typename... KArgs, typename... Args>
+void launch_k(lgf_ctx* c, void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = c->opt_pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 #ifndef LGF_CARVEOUT
 #define LGF_CARVEOUT 0
 #endif
@@ -219,7 +232,7 @@ template <int NC> void launch_fa_delta_fwd(lgf_ctx* c, bool fin) {
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
     const FinArgs fa{c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), fin ? 1 : 0};
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_delta_fwd<A, B, NC, FAD_NT><<<grid, FAD_NT, c->smem_fa, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->T, c->ctl, fa);
+        launch_k(c, k_fa_delta_fwd<A, B, NC, FAD_NT>, grid, FAD_NT, c->smem_fa, cur_links(c), c->field, c->partials, c->G, c->T, c->ctl, fa);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -227,7 +240,7 @@ void launch_fa_inv(lgf_ctx* c) {
     LaunchScope ls(c, K_FA_INV);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_inv<A, B, 4, FC_NT, false><<<grid, FC_NT, c->smem_fc, c->stream>>>(c->field, nullptr, 0.0, c->G, c->T, c->ctl);
+        launch_k(c, k_fa_inv<A, B, 4, FC_NT, false>, grid, FC_NT, c->smem_fc, c->field, nullptr, 0.0, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -235,7 +248,7 @@ void launch_fa_inv_g(lgf_ctx* c, double half_alpha) {
     LaunchScope ls(c, K_FA_INV_G);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fa_inv<A, B, 4, FC_NT, true><<<grid, FC_NT, c->smem_fc, c->stream>>>(c->field, c->gbuf, half_alpha, c->G, c->T, c->ctl);
+        launch_k(c, k_fa_inv<A, B, 4, FC_NT, true>, grid, FC_NT, c->smem_fc, c->field, c->gbuf, half_alpha, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -245,7 +258,7 @@ template <int NC> void launch_fu_update(lgf_ctx* c) {
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
     const long long stride = (long long)(c->lay.link_buf / 16);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_fu_update_delta_fwd<A, B, NC, LGF_FU_NT><<<grid, LGF_FU_NT, c->smem_fu, c->stream>>>(c->links, stride, c->gbuf, c->field, c->partials, c->G, c->T, c->ctl);
+        launch_k(c, k_fu_update_delta_fwd<A, B, NC, LGF_FU_NT>, grid, LGF_FU_NT, c->smem_fu, c->links, stride, c->gbuf, c->field, c->partials, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -254,7 +267,7 @@ void launch_fa_mid(lgf_ctx* c) {
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
     const double scale = 16.0 / (double)c->G.V;
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        k_fa_mid<A, B, fast_mid_lgC(A, B), FB_NT><<<grid, FB_NT, c->smem_fb, c->stream>>>(c->field, c->G, c->T, scale, c->ctl);
+        launch_k(c, k_fa_mid<A, B, fast_mid_lgC(A, B), FB_NT>, grid, FB_NT, c->smem_fb, c->field, c->G, c->T, scale, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -265,7 +278,7 @@ template <int NC> void launch_pp_delta_fwd(lgf_ctx* c) {
     LaunchScope ls(c, K_PP_DELTA_FWD);
     const unsigned grid = pp_grid(c, c->G.L[2] * c->G.L[3]);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_pp_delta_fwd<A, B, NC, FA_NT><<<grid, 2 * FA_NT, c->smem_pa, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->T, c->ctl);
+        launch_k(c, k_pp_delta_fwd<A, B, NC, FA_NT>, grid, 2 * FA_NT, c->smem_pa, cur_links(c), c->field, c->partials, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -273,7 +286,7 @@ void launch_pp_inv(lgf_ctx* c) {
     LaunchScope ls(c, K_PP_INV);
     const unsigned grid = pp_grid(c, c->G.L[2] * c->G.L[3]);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        k_pp_inv<A, B, FA_NT><<<grid, 2 * FA_NT, c->smem_pa, c->stream>>>(c->field, c->G, c->T, c->ctl);
+        launch_k(c, k_pp_inv<A, B, FA_NT>, grid, 2 * FA_NT, c->smem_pa, c->field, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -282,7 +295,7 @@ void launch_pp_mid(lgf_ctx* c) {
     const unsigned grid = pp_grid(c, 4LL * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
     const double scale = 16.0 / (double)c->G.V;
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT><<<grid, 2 * FA_NT, c->smem_pb, c->stream>>>(c->field, c->G, c->T, scale, c->ctl);
+        launch_k(c, k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, grid, 2 * FA_NT, c->smem_pb, c->field, c->G, c->T, scale, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -387,34 +400,34 @@ lgf_status build_tables(lgf_ctx* c) {
 // ---- kernel launchers ---------------------------------------------------------------------------------------
 template <int NC> void launch_delta(lgf_ctx* c) {
     LaunchScope ls(c, K_DELTA);
-    k_delta<NC><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(cur_links(c), c->field, c->partials, c->G, c->ctl);
+    launch_k(c, k_delta<NC>, (unsigned)(c->G.V / 128), 128, 0, cur_links(c), c->field, c->partials, c->G, c->ctl);
 }
 template <int MODE, int NC> void launch_fft01(lgf_ctx* c, int slot, double half_alpha) {
     LaunchScope ls(c, slot);
     const bool fused = (MODE == MODE_DELTA_FWD || MODE == MODE_INV_G);
     const int ncomp = fused ? 4 : c->fft01_ncomp;
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3] * (4 / ncomp));
-    k_fft01<MODE, NC><<<grid, c->fft01_threads, fused ? c->smem01_fused : c->smem01, c->stream>>>(
+    launch_k(c, k_fft01<MODE, NC>, grid, c->fft01_threads, fused ? c->smem01_fused : c->smem01, 
         c->field, cur_links(c), c->gbuf, c->partials, c->G, c->T, ncomp, half_alpha, c->ctl);
 }
 void launch_fft23(lgf_ctx* c) {
     LaunchScope ls(c, K_FFT23_MID);
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fft23_lgC));
-    k_fft23_mid<<<grid, c->fft23_threads, c->smem23, c->stream>>>(c->field, c->G, c->T, c->fft23_lgC, c->fft23_S1, c->fft23_S2,
+    launch_k(c, k_fft23_mid, grid, c->fft23_threads, c->smem23, c->field, c->G, c->T, c->fft23_lgC, c->fft23_S1, c->fft23_S2,
                                                                    16.0 / (double)c->G.V, c->ctl);
 }
 void launch_finalize(lgf_ctx* c, int n_partials, int advance = 0) {
     LaunchScope ls(c, K_FINALIZE);
-    k_finalize<<<1, 256, 0, c->stream>>>(c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), advance);
+    launch_k(c, k_finalize, 1, 256, 0, c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), advance);
 }
 template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
     if (!SG && c->opt_quad) {
         LaunchScope ls(c, K_UPDATE_QUAD);
-        k_update_quad<NC><<<(unsigned)(c->G.V / 32), 128, 0, c->stream>>>(cur_links(c), c->field, c->G, half_alpha, c->ctl);
+        launch_k(c, k_update_quad<NC>, (unsigned)(c->G.V / 32), 128, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl);
         return;
     }
     LaunchScope ls(c, SG ? K_UPDATE_G : K_UPDATE_X);
-    k_update<NC, SG><<<(unsigned)(c->G.V / LGF_UPD_NT), LGF_UPD_NT, 0, c->stream>>>(cur_links(c), SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
+    launch_k(c, k_update<NC, SG>, (unsigned)(c->G.V / LGF_UPD_NT), LGF_UPD_NT, 0, cur_links(c), SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
 }
 
 bool use_fused(const lgf_ctx* c) { return c->opt_fuse && c->fft01_ncomp_fused_ok; }
@@ -488,7 +501,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -556,7 +569,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
     c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
@@ -787,6 +800,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_PINGPONG: if (value < 0 || value > 7) return LGF_ERR_INVALID_ARG; c->opt_pingpong = value; break;
         case LGF_OPT_FUSE_FINALIZE: c->opt_fuse_fin = value ? 1 : 0; break;
         case LGF_OPT_QUAD_UPDATE: c->opt_quad = value ? 1 : 0; break;
+        case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
@@ -802,6 +816,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_FUSE_UPDATE: *value = use_fused_update(c) ? 1 : 0; break;
         case LGF_OPT_PINGPONG: *value = (use_pp_a(c) ? 1 : 0) | (use_pp_b(c) ? 2 : 0) | (use_pp_c(c) ? 4 : 0); break;
         case LGF_OPT_FUSE_FINALIZE: *value = use_fused_fin(c) ? 1 : 0; break;
+        case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }

@@ -167,6 +167,16 @@ __device__ __forceinline__ long long bwd(const Geom& G, long long x, int mu) {
     return (c == 0) ? x + ((long long)(G.L[mu] - 1) << G.sh[mu]) : x - (1LL << G.sh[mu]);
 }
 
+// Programmatic dependent launch (sm_90+): every kernel of the iteration lets its successor be scheduled as soon as
+// all of its own CTAs have started (launch_dependents), and itself waits for the complete, flushed end of its
+// predecessor (wait) before it touches global memory -- so stream order is kept, and what overlaps is the launch
+// latency and CTA ramp-up of kernel n+1 with the tail of kernel n.  Both are no-ops when the launch does not carry
+// the programmatic-serialization attribute.
+__device__ __forceinline__ void pdl_enter() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // Device-resident control block shared by all kernels of one context.
 struct Ctl {
     double F, theta;       // last measurement (S1)
