@@ -109,8 +109,8 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_STORE_G         1: pass C stores g(x) and the update reads it, 0: the update recomputes g from X
  *   LGF_OPT_GRAPH           1: replay iterations through a CUDA graph (default), 0: plain launches
  *   LGF_OPT_BATCH           iterations enqueued between two reads of the device stop flag (default 8)
- *   LGF_OPT_FAST_FFT        1 (default): use the compile-time-sized FFT passes where the lattice allows (extents 16 or
- *                           32 on the axis pair of a pass), 0: always the generic passes.  lgf_get_option returns a
+ *   LGF_OPT_FAST_FFT        1 (default): use the compile-time-sized FFT passes where the lattice allows (extents 16,
+ *                           32 or 64 on the axis pair of a pass; a 64 extent in the (x0,x1) plane keeps S1 separate), 0: always the generic passes.  lgf_get_option returns a
  *                           bit mask of the passes that run fast: 1 pass A (fused Delta), 2 pass B, 4 pass C
  *   LGF_OPT_FUSE_UPDATE     0 (default: the separate kernels measured faster on B200), 1: where the
  *                           compile-time-sized passes cover the (x0,x1) plane, S3/S4 of one iteration

@@ -169,7 +169,7 @@ __device__ __forceinline__ void plane_middle(cplx* __restrict__ t, const cplx* _
 // ---------------------------------------------------------------------------------------------------------------
 // Forward FFT over axes 0,1 of the 4 component tiles t[c][x1][x0] (row stride L0+1), last stage written straight
 // to field (component c at field + c*V, plane base xbase).  The tile must be complete (caller syncs before).
-template <int LG0, int LG1, int NT>
+template <int LG0, int LG1, int NT, int NCOMP = 4>
 __device__ __forceinline__ void plane_forward_store(cplx* __restrict__ tile, const cplx* __restrict__ tw0, const cplx* __restrict__ tw1,
                                                     cplx* __restrict__ field, long long V, long long xbase, const Grp& g) {
     using PA = Plan2<LG0, false>;
@@ -177,7 +177,7 @@ __device__ __forceinline__ void plane_forward_store(cplx* __restrict__ tile, con
     constexpr int L0 = PA::L, L1 = PB::L, S = L0 + 1, SC = S * L1;
     // a stage 1: points a = ja + m R2, twiddles tw0[k ja]; lanes over rows
     {
-        constexpr int NW = 4 * PA::R2 * L1;
+        constexpr int NW = NCOMP * PA::R2 * L1;
 #pragma unroll
         for (int w0 = 0; w0 < NW; w0 += NT) {
             const int w = w0 + g.tid;
@@ -188,10 +188,10 @@ __device__ __forceinline__ void plane_forward_store(cplx* __restrict__ tile, con
         }
         gsync<NT>(g);
     }
-    plane_middle<LG0, LG1, 4, NT, false>(tile, tw1, g);
+    plane_middle<LG0, LG1, NCOMP, NT, false>(tile, tw1, g);
     // b stage 2 (no twiddles) -> global; lanes over x0: coalesced
     {
-        constexpr int NW = 4 * L0 * PB::R1;
+        constexpr int NW = NCOMP * L0 * PB::R1;
 #pragma unroll
         for (int w0 = 0; w0 < NW; w0 += NT) {
             const int w = w0 + g.tid;
@@ -310,6 +310,32 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cp
     return;
 #endif
     plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)blockIdx.x << (LG0 + LG1), g);
+}
+
+// Pass A without S1, for planes whose four component tiles do not fit one SM (64 x 64, 32 x 64): forward FFT over axes
+// 0,1 of NCOMP components of one plane, Delta read from field (written by k_delta).  blockIdx.x = plane * (4/NCOMP) + group.
+template <int LG0, int LG1, int NCOMP, int NT>
+__global__ void __launch_bounds__(NT, 2) k_fa_fwd(cplx* __restrict__ field, Geom G, FftTables T, const Ctl* __restrict__ ctl) {
+    pdl_enter();
+    if (ctl->done) return;
+    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1, nP = L0 * L1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw);
+    cplx* tw0 = tile + NCOMP * SC;
+    cplx* tw1 = tw0 + L0;
+    constexpr int NG = 4 / NCOMP;
+    const long long xbase = (long long)(blockIdx.x / NG) << (LG0 + LG1);
+    cplx* fbase = field + (long long)((blockIdx.x % NG) * NCOMP) * G.V;
+    const Grp g{(int)threadIdx.x, 0};
+    for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
+    for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
+#pragma unroll 4
+    for (int e = threadIdx.x; e < NCOMP * nP; e += NT) {
+        const int c = e >> (LG0 + LG1), r = e & (nP - 1);
+        tile[c * SC + (r & (L0 - 1)) + (r >> LG0) * S] = ld_field(fbase + (long long)c * G.V + xbase + r);
+    }
+    __syncthreads();
+    plane_forward_store<LG0, LG1, NT, NCOMP>(tile, tw0, tw1, fbase, G.V, xbase, g);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -576,7 +602,7 @@ __device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01,
 
 // Pass B: forward over axes 2,3, filter, inverse over axes 3,2, one work item per CTA.
 template <int LG2, int LG3, int LGC, int NT>
-__global__ void __launch_bounds__(NT, LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+__global__ void __launch_bounds__(NT, (NT > 256) ? 1 : LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
     pdl_enter();
     if (ctl->done) return;
     using MG = MidGeom<LG2, LGC>;

@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(128) k_delta(const cplx* __restrict__ links, c
 // and raises the stop flag: theta < theta_tol (converged), or max_iter updates applied, or non-finite.
 // advance != 0: the measured links are the result of an update applied by the same iteration body (fused update,
 // fused_update.cuh): count it and make the buffer it wrote the current one.
-__global__ void __launch_bounds__(256) k_finalize(const double2* __restrict__ partials, int n, Ctl* ctl, double2* hist, double inv3V, double inv12V,
+__global__ void __launch_bounds__(1024) k_finalize(const double2* __restrict__ partials, int n, Ctl* ctl, double2* hist, double inv3V, double inv12V,
                                                   int advance) {
     pdl_enter();
     if (ctl->done) return;
@@ -317,39 +317,37 @@ __global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __res
 // One thread per link, four warps per CTA = the four directions of 32 consecutive sites.  Thread (x, mu) builds
 // g(x+mu) only; g(x) is what the mu = 0 thread of the site x-0 built (its forward neighbour is x), handed over
 // through shared memory: 4 Gram-Schmidt per site instead of 5 (one thread per site) or 8 (k_update_link).
-// Needs L0 <= 32 so that the x0 row of a site lies inside its warp; longer rows: the mu = 0 warp builds g(x) too.
+// A CTA covers whole x0 rows (NS = max(32, L0) sites, 4 NS threads), so the site x-0 is always in the same CTA.
 // Measured on B200 at 32^4 (CUDA events per launch): 149 us at 5 CTAs/SM (96 registers), 157 at 4, 157 at 6 (spills),
 // against 161 for one thread per site (k_update<NC,0>, 12 warps/SM); the IEEE 1/sqrt costs nothing measurable.
+#ifndef LGF_UPDQ_MINB64
+#define LGF_UPDQ_MINB64 3
+#endif
 #ifndef LGF_UPDQ_MINB
 #define LGF_UPDQ_MINB 5
 #endif
-template <int NC>
-__global__ void __launch_bounds__(128, LGF_UPDQ_MINB) k_update_quad(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G, double half_alpha, Ctl* ctl) {
+template <int NC, int NS>      // NS = sites per CTA = max(32, L0): 4 * NS threads, thread = (mu, site)
+__global__ void __launch_bounds__(4 * NS, (NS == 32) ? LGF_UPDQ_MINB : ((NS == 64) ? LGF_UPDQ_MINB64 : 1)) k_update_quad(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G,
+                                                                                       double half_alpha, Ctl* ctl) {
     pdl_enter();
     if (ctl->done) return;
-    __shared__ cplx sg[9][32];
-    const int lane = threadIdx.x & 31, mu = threadIdx.x >> 5;
+    __shared__ cplx sg[9][NS];
+    const int st = threadIdx.x % NS, mu = threadIdx.x / NS;
     const long long V = G.V;
-    const long long x = (long long)blockIdx.x * 32 + lane;
+    const long long x = (long long)blockIdx.x * NS + st;
     const long long xf = fwd(G, x, mu);
     cplx g[9], gp[9], u[9], r[9];
     load_link<NC>(links, V, mu, x, u);
     build_g(ldc_field(src + xf), ldc_field(src + V + xf), ldc_field(src + 2 * V + xf), ldc_field(src + 3 * V + xf), half_alpha, gp);
     if (mu == 0) {
-        if (G.L[0] <= 32) {
-            const int m = G.L[0] - 1;
-            const int dst = (lane & ~m) | ((lane + 1) & m);      // the lane of site x+0 (same row, periodic)
+        const int m = G.L[0] - 1;                             // L0 <= NS: the x0 row of a site lies inside its CTA
+        const int dst = (st & ~m) | ((st + 1) & m);           // the slot of site x+0 (same row, periodic)
 #pragma unroll
-            for (int c = 0; c < 9; c++) sg[c][dst] = gp[c];
-        } else {
-            build_g(ldc_field(src + x), ldc_field(src + V + x), ldc_field(src + 2 * V + x), ldc_field(src + 3 * V + x), half_alpha, g);
-#pragma unroll
-            for (int c = 0; c < 9; c++) sg[c][lane] = g[c];
-        }
+        for (int c = 0; c < 9; c++) sg[c][dst] = gp[c];
     }
     __syncthreads();
 #pragma unroll
-    for (int c = 0; c < 9; c++) g[c] = sg[c][lane];
+    for (int c = 0; c < 9; c++) g[c] = sg[c][st];
     rotate_link<(NC == 6) ? 2 : 3>(g, u, gp, r);
     store_link<NC>(links, V, mu, x, r);
     if (x == 0 && mu == 0) ctl->iters = ctl->iters + 1;

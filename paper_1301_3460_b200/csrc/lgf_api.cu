@@ -20,13 +20,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE,
-    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_NSLOTS
+    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd",
-    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad"};
+    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad", "k_fa_fwd1", "k_fa_inv1"};
 
 constexpr int HIST_CAP = 1 << 16;
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
@@ -121,8 +121,8 @@ struct lgf_ctx {
     int sms;                // SMs of the device: grid of the persistent passes
     int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
-    bool fast_a, fast_b, fast_c, pp_b_ok;
-    size_t smem_fa, smem_fb, smem_fc, smem_fu, smem_pa, smem_pb;
+    bool fast_a, fast_b, fast_c, pp_b_ok, big_p;
+    size_t smem_fa, smem_fb, smem_fc, smem_fu, smem_pa, smem_pb, smem_p1;
     int fb_lgC;
     // derived launch parameters
     int fft01_ncomp_fused_ok, fft01_ncomp, fft01_threads, fft23_lgC, fft23_S1, fft23_S2, fft23_threads;
@@ -213,10 +213,30 @@ constexpr int FC_NT = LGF_FC_NT;      // threads per CTA of pass C (k_fa_inv)
 #define LGF_FB_NT 256
 #endif
 constexpr int FB_NT = LGF_FB_NT;
-constexpr int fast_mid_lgC(int lga, int lgb) { return (lga + lgb >= 10) ? LGF_FB_LGC55 : 3; }   // x0 chunk: tile <= 64 KB
+// 64 extents: the (x0,x1) plane passes take one component per CTA (S1 stays a separate kernel: four 64 x 64 tiles do
+// not fit one SM), the (x2,x3) pass takes a shorter x0 chunk
+#define LGF_BIG_PAIRS(X) X(5, 6) X(6, 5) X(6, 6)
+#ifndef LGF_FB_LGC11
+#define LGF_FB_LGC11 2
+#endif
+#ifndef LGF_FB_LGC12
+#define LGF_FB_LGC12 1
+#endif
+// x0 chunk of pass B (2^lgC sites): tile = 2^(lga+lgb+lgC) * 16 B
+constexpr int fast_mid_lgC(int lga, int lgb) {
+    return (lga + lgb <= 9) ? 3 : ((lga + lgb == 10) ? LGF_FB_LGC55 : ((lga + lgb == 11) ? LGF_FB_LGC11 : LGF_FB_LGC12));
+}
+// threads per CTA of pass B: one 512-thread CTA per SM when the tile is above 100 KB, else 2 x 256
+constexpr int fast_mid_nt(int lga, int lgb) { return ((16 << (lga + lgb + fast_mid_lgC(lga, lgb))) > 100 * 1024) ? 512 : FB_NT; }
 bool fast_pair(int lga, int lgb) {
 #define X(A, B) if (lga == A && lgb == B) return true;
     LGF_FAST_PAIRS(X)
+#undef X
+    return false;
+}
+bool big_pair(int lga, int lgb) {
+#define X(A, B) if (lga == A && lgb == B) return true;
+    LGF_BIG_PAIRS(X)
 #undef X
     return false;
 }
@@ -252,6 +272,23 @@ void launch_fa_inv_g(lgf_ctx* c, double half_alpha) {
     LGF_FAST_PAIRS(X)
 #undef X
 }
+// planes with a 64 extent: one component per CTA
+void launch_fa_fwd1(lgf_ctx* c) {
+    LaunchScope ls(c, K_FA_FWD1);
+    const unsigned grid = (unsigned)(4 * c->G.L[2] * c->G.L[3]);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        launch_k(c, k_fa_fwd<A, B, 1, FC_NT>, grid, FC_NT, c->smem_p1, c->field, c->G, c->T, c->ctl);
+    LGF_BIG_PAIRS(X)
+#undef X
+}
+void launch_fa_inv1(lgf_ctx* c) {
+    LaunchScope ls(c, K_FA_INV1);
+    const unsigned grid = (unsigned)(4 * c->G.L[2] * c->G.L[3]);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        launch_k(c, k_fa_inv<A, B, 1, FC_NT, false>, grid, FC_NT, c->smem_p1, c->field, nullptr, 0.0, c->G, c->T, c->ctl);
+    LGF_BIG_PAIRS(X)
+#undef X
+}
 // S3/S4 of this iteration + S1 and pass A of the next (fused_update.cuh); reads link buffer Ctl::parity, writes the other
 template <int NC> void launch_fu_update(lgf_ctx* c) {
     LaunchScope ls(c, K_FU_UPDATE);
@@ -267,8 +304,8 @@ void launch_fa_mid(lgf_ctx* c) {
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
     const double scale = 16.0 / (double)c->G.V;
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        launch_k(c, k_fa_mid<A, B, fast_mid_lgC(A, B), FB_NT>, grid, FB_NT, c->smem_fb, c->field, c->G, c->T, scale, c->ctl);
-    LGF_FAST_PAIRS(X)
+        launch_k(c, k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, grid, fast_mid_nt(A, B), c->smem_fb, c->field, c->G, c->T, scale, c->ctl);
+    LGF_FAST_PAIRS(X) LGF_BIG_PAIRS(X)
 #undef X
 }
 
@@ -303,7 +340,9 @@ void launch_pp_mid(lgf_ctx* c) {
 lgf_status setup_fast(lgf_ctx* c) {
     const Geom& G = c->G;
     c->fast_a = c->fast_c = fast_pair(G.lg[0], G.lg[1]);
-    c->fast_b = fast_pair(G.lg[2], G.lg[3]);
+    c->fast_b = fast_pair(G.lg[2], G.lg[3]) || big_pair(G.lg[2], G.lg[3]);
+    c->big_p = big_pair(G.lg[0], G.lg[1]);               // plane passes with one component per CTA, S1 separate
+    c->smem_p1 = smem_fast_plane(G.lg[0], G.lg[1], 1);
     c->fb_lgC = fast_mid_lgC(G.lg[2], G.lg[3]);
     if (c->fb_lgC > G.lg[0]) c->fast_b = false;          // the x0 extent must hold one chunk
     c->smem_fa = c->smem_fc = c->smem_fu = smem_fast_plane(G.lg[0], G.lg[1], 4);
@@ -311,7 +350,7 @@ lgf_status setup_fast(lgf_ctx* c) {
     // two tiles + one set of tables
     c->smem_pa = 2 * c->smem_fa - (size_t)(G.L[0] + G.L[1]) * 16;
     c->smem_pb = 2 * c->smem_fb - ((size_t)(G.L[2] + G.L[3]) * 16 + (size_t)(G.L[2] + G.L[3]) * 8);
-    c->pp_b_ok = c->smem_pb <= (size_t)227 * 1024;
+    c->pp_b_ok = c->smem_pb <= (size_t)227 * 1024 && fast_pair(G.lg[2], G.lg[3]);
     if (c->fast_a) {
 #define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
             CK(set_smem(k_fa_delta_fwd<A, B, 6, FAD_NT>, c->smem_fa)); CK(set_smem(k_fa_delta_fwd<A, B, 9, FAD_NT>, c->smem_fa)); \
@@ -323,9 +362,18 @@ lgf_status setup_fast(lgf_ctx* c) {
 #undef X
     }
     if (c->fast_b) {
-#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) { CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), FB_NT>, c->smem_fb)); \
+#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) { CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb)); \
             if (c->pp_b_ok) CK(set_smem(k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, c->smem_pb)); }
         LGF_FAST_PAIRS(X)
+#undef X
+#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb));
+        LGF_BIG_PAIRS(X)
+#undef X
+    }
+    if (c->big_p) {
+#define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
+            CK(set_smem(k_fa_fwd<A, B, 1, FC_NT>, c->smem_p1)); CK(set_smem(k_fa_inv<A, B, 1, FC_NT, false>, c->smem_p1)); }
+        LGF_BIG_PAIRS(X)
 #undef X
     }
     return LGF_OK;
@@ -418,12 +466,14 @@ void launch_fft23(lgf_ctx* c) {
 }
 void launch_finalize(lgf_ctx* c, int n_partials, int advance = 0) {
     LaunchScope ls(c, K_FINALIZE);
-    launch_k(c, k_finalize, 1, 256, 0, c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), advance);
+    launch_k(c, k_finalize, 1, n_partials > 8192 ? 1024 : 256, 0, c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), advance);
 }
 template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
     if (!SG && c->opt_quad) {
         LaunchScope ls(c, K_UPDATE_QUAD);
-        launch_k(c, k_update_quad<NC>, (unsigned)(c->G.V / 32), 128, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl);
+        if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32>, (unsigned)(c->G.V / 32), 128, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl);
+        else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64>, (unsigned)(c->G.V / 64), 256, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl);
+        else launch_k(c, k_update_quad<NC, 128>, (unsigned)(c->G.V / 128), 512, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl);
         return;
     }
     LaunchScope ls(c, SG ? K_UPDATE_G : K_UPDATE_X);
@@ -436,6 +486,7 @@ bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a && use_fused
 bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
 bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c && !use_store_g(c); }
 bool use_fused_update(const lgf_ctx* c) { return c->opt_fuse_update && c->opt_fast && c->fast_a; }
+bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p && !use_store_g(c); }
 bool use_pp_a(const lgf_ctx* c) { return (c->opt_pingpong & 1) && use_fast_a(c); }
 bool use_pp_b(const lgf_ctx* c) { return (c->opt_pingpong & 2) && use_fast_b(c) && c->pp_b_ok; }
 bool use_pp_c(const lgf_ctx* c) { return (c->opt_pingpong & 4) && use_fast_c(c); }
@@ -445,6 +496,7 @@ template <int NC> void enqueue_head(lgf_ctx* c) {
     int np;
     if (use_pp_a(c)) { launch_pp_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
     else if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c, c->opt_fuse_fin != 0); if (c->opt_fuse_fin) return; np = c->G.L[2] * c->G.L[3]; }
+    else if (use_big_p(c)) { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fa_fwd1(c); }
     else if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
     else { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fft01<MODE_FWD, 6>(c, K_FFT01_FWD, 0.0); }
     launch_finalize(c, np);
@@ -452,7 +504,8 @@ template <int NC> void enqueue_head(lgf_ctx* c) {
 // pass B, pass C, update
 void launch_mid(lgf_ctx* c) { if (use_pp_b(c)) launch_pp_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c); }
 void launch_inv_x(lgf_ctx* c) {
-    if (use_pp_c(c)) launch_pp_inv(c); else if (use_fast_c(c)) launch_fa_inv(c); else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, 0.0);
+    if (use_pp_c(c)) launch_pp_inv(c); else if (use_fast_c(c)) launch_fa_inv(c); else if (use_big_p(c)) launch_fa_inv1(c);
+    else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, 0.0);
 }
 template <int NC> void enqueue_tail(lgf_ctx* c, double half_alpha) {
     launch_mid(c);
@@ -472,7 +525,11 @@ void enqueue_body(lgf_ctx* c, double half_alpha) {
     else { enqueue_head<9>(c); enqueue_tail<9>(c, half_alpha); }
 }
 bool use_fused_fin(const lgf_ctx* c) { return c->opt_fuse_fin && use_fast_a(c) && !use_pp_a(c); }
-int launches_per_body(const lgf_ctx* c) { return use_fused_update(c) ? 4 : (use_fused_fin(c) ? 4 : (use_fused(c) ? 5 : 6)); }
+int launches_per_body(const lgf_ctx* c) {
+    if (use_fused_update(c) || use_fused_fin(c)) return 4;
+    if (use_big_p(c) && !use_fast_a(c) && !use_pp_a(c)) return 6;
+    return use_fused(c) ? 5 : 6;
+}
 
 lgf_status reset_ctl(lgf_ctx* c, double tol, int max_iter) {
     Ctl h; memset(&h, 0, sizeof h);
@@ -812,7 +869,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_STORE_G: *value = use_store_g(c); break;
         case LGF_OPT_GRAPH: *value = c->opt_graph; break;
         case LGF_OPT_BATCH: *value = c->opt_batch; break;
-        case LGF_OPT_FAST_FFT: *value = (use_fast_a(c) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | (use_fast_c(c) ? 4 : 0); break;
+        case LGF_OPT_FAST_FFT: *value = ((use_fast_a(c) || use_big_p(c)) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | ((use_fast_c(c) || use_big_p(c)) ? 4 : 0); break;
         case LGF_OPT_FUSE_UPDATE: *value = use_fused_update(c) ? 1 : 0; break;
         case LGF_OPT_PINGPONG: *value = (use_pp_a(c) ? 1 : 0) | (use_pp_b(c) ? 2 : 0) | (use_pp_c(c) ? 4 : 0); break;
         case LGF_OPT_FUSE_FINALIZE: *value = use_fused_fin(c) ? 1 : 0; break;

@@ -101,6 +101,8 @@ def test_device_pointer_load_and_get():
 # ------------------------------------------------------------------ kernel-level stages (S1, S2, S3, S4)
 STAGE_CASES = [
     ((8, 8, 8, 8), 18), ((8, 8, 8, 8), 12), ((16, 16, 16, 16), 12),
+    # 64 extents (the shapes of C3, C4 on small companions): one-component plane passes, short-chunk pass B
+    ((64, 64, 4, 4), 12), ((4, 4, 64, 64), 18), ((32, 64, 4, 8), 12), ((64, 32, 8, 4), 18), ((8, 4, 32, 64), 12), ((4, 8, 64, 32), 12),
     ((8, 8, 16, 32), 12), ((4, 8, 16, 32), 18), ((32, 4, 8, 4), 12), ((4, 4, 4, 4), 12), ((16, 32, 4, 8), 18),
     ((32, 16, 16, 32), 12), ((16, 32, 32, 16), 18), ((32, 32, 16, 16), 12), ((16, 16, 32, 32), 18), ((32, 32, 32, 32), 12),
 ]
@@ -418,6 +420,14 @@ def test_fused_update_buffers_and_counts():
     gf.set_profiling(False)
     assert prof["k_fu_update_delta_fwd"]["launches"] == 2 and prof["k_fa_inv_g"]["launches"] == 2
     assert prof["k_fa_delta_fwd"]["launches"] == 1 and prof["k_finalize"]["launches"] == 3
+
+
+def test_fast_fft_pass_selection_64_extents():
+    """64 extents: plane passes with one component per CTA (bits 1 and 4), pass B with a short x0 chunk (bit 2)."""
+    for dims, mask in [((64, 64, 4, 4), 5), ((4, 4, 64, 64), 2), ((32, 64, 32, 64), 7), ((8, 8, 64, 32), 2), ((64, 32, 16, 16), 7)]:
+        gf = lgf.GaugeFixer(dims, 12)
+        assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
+        gf.destroy()
 
 
 def test_fast_fft_pass_selection():
