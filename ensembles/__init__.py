@@ -41,6 +41,7 @@ __all__ = [
     "abelian",
     "as_real",
     "as_complex",
+    "device_su3",
 ]
 
 # Gell-Mann matrices lambda_1..lambda_8
@@ -180,3 +181,33 @@ def as_real(U: np.ndarray) -> np.ndarray:
 def as_complex(R: np.ndarray) -> np.ndarray:
     R = np.ascontiguousarray(R, dtype=np.float64)
     return R.view(np.complex128).reshape(R.shape[:-1])
+
+
+def device_su3(dims, seed: int, spread: float = 0.15):
+    """Seeded random SU(3) links generated ON THE CUDA DEVICE (torch), for lattices too large to build with numpy
+    in test time (64^4: 67 M links).  U = rows of GramSchmidt(1 + spread * G), G complex Gaussian, third row the
+    conjugate cross product -- smooth-ish links near the identity, no gauge structure.  Returns a torch complex128
+    tensor [V, 4, 3, 3] in the canonical order of include/lgf.h.  Inputs only: nothing of the method is here.
+    These are not the BASELINE.json ensembles (those are `noisy`/`pure_gauge`); they serve property and
+    sampled-site parity tests and kernel timing at sizes where the host generator takes minutes."""
+    import torch
+    V = volume(dims)
+    gen = torch.Generator(device="cuda")
+    gen.manual_seed(int(seed))
+    n = V * 4
+    U = torch.empty(n, 3, 3, dtype=torch.complex128, device="cuda")
+    chunk = 1 << 22
+    for o in range(0, n, chunk):
+        m = min(chunk, n - o)
+        A = torch.randn(m, 2, 3, 2, dtype=torch.float64, device="cuda", generator=gen)
+        A = torch.view_as_complex(A) * spread
+        A[:, 0, 0] += 1
+        A[:, 1, 1] += 1
+        u = A[:, 0]
+        u = u / u.abs().pow(2).sum(-1, keepdim=True).sqrt()
+        v = A[:, 1] - (u.conj() * A[:, 1]).sum(-1, keepdim=True) * u
+        v = v / v.abs().pow(2).sum(-1, keepdim=True).sqrt()
+        U[o:o + m, 0] = u
+        U[o:o + m, 1] = v
+        U[o:o + m, 2] = torch.linalg.cross(u, v).conj()
+    return U.reshape(V, 4, 3, 3)

@@ -219,6 +219,98 @@ def test_trajectory_C1():
     check_trajectory("C1", fft_mode=1)
 
 
+def test_trajectory_C2b_headline_config():
+    """BASELINE.json configs[2], eps = 0.35 (the workload bench.py times): F, theta, links after 10 and 100 iterations
+    and the stop iteration, against the oracle (radix-2 FFT mode, itself pinned to the naive DFT on CPU)."""
+    check_trajectory("C2b", fft_mode=1)
+
+
+def test_trajectory_C3_anisotropic():
+    """BASELINE.json configs[3], 32^3 x 64: uneven FFT axes, non-cubic p^2 filter, 64-extent pass B."""
+    check_trajectory("C3", fft_mode=1, checkpoints=(10, 60))
+
+
+# ------------------------------------------------------------------ full-size lattices on sampled sites
+def _site_coords(x, dims):
+    c = []
+    for L in dims:
+        c.append(x % L)
+        x //= L
+    return c
+
+
+def _site_index(c, dims):
+    x, m = 0, 1
+    for k, L in zip(c, dims):
+        x += (k % L) * m
+        m *= L
+    return x
+
+
+@pytest.mark.parametrize("dims", [(64, 64, 64, 64), (32, 32, 32, 64)])
+def test_full_size_sampled_sites_and_invariants(dims):
+    """C4 / C3 shapes at full size, where the oracle cannot run the whole lattice in test time: every stage is checked
+    on sampled sites against what the oracle computes site by site, plus properties that hold at any size.
+      S1: Delta(x) from the oracle on a 4^4 carrier lattice holding the 8 links of x (the stencil is local);
+      S2: -Laplacian X = p2max * Delta, since p2max/p^2 inverts the eigenvalues 4 sin^2(pi n/L) of the lattice Laplacian;
+      S3+S4: U' = g(x) U g(x+mu)^dagger with g = oracle.project(X) on the sampled sites;
+      theta from the full Delta field; plaquette invariance; F monotone."""
+    import torch
+    V = int(np.prod(dims))
+    Ud = E.device_su3(dims, seed=5, spread=0.15)
+    gf = lgf.GaugeFixer(dims, 12)
+    gf.load_links_device(Ud.data_ptr())
+    F0, th0, plaq0 = gf.measure()
+    D = gf.get_field(lgf.LGF_FIELD_DELTA)
+    X = gf.get_field(lgf.LGF_FIELD_X)
+    assert abs(np.einsum("xij,xij->", D.conj(), D).real / (3.0 * V) - th0) <= 1e-12 * th0      # theta = (1/3V) sum Tr D D^dag
+    rng = np.random.default_rng(11)
+    sites = [int(v) for v in rng.integers(0, V, 48)] + [0, V - 1, dims[0] - 1, V - dims[0]]      # corners: every wrap
+    ident = np.broadcast_to(np.eye(3, dtype=np.complex128), (256, 4, 3, 3)).copy()
+    carrier = (4, 4, 4, 4)
+    y = _site_index((1, 1, 1, 1), carrier)
+    o4 = oracle.Oracle(carrier, 12)
+    xs = np.abs(X).max()
+    for x in sites:
+        c = _site_coords(x, dims)
+        nb_f = [_site_index([c[k] + (1 if k == mu else 0) for k in range(4)], dims) for mu in range(4)]
+        nb_b = [_site_index([c[k] - (1 if k == mu else 0) for k in range(4)], dims) for mu in range(4)]
+        idx = torch.tensor([x] + nb_b, device="cuda")
+        Ul = Ud[idx].cpu().numpy()                                  # links of x and of its 4 backward neighbours
+        # S1 on the carrier lattice: A(y) = sum_mu [U_mu(y-mu) - U_mu(y)] touches exactly these 8 links
+        W = ident.copy()
+        W[y] = Ul[0]
+        for mu in range(4):
+            yb = _site_index([1 - (1 if k == mu else 0) for k in range(4)], carrier)
+            W[yb, mu] = Ul[1 + mu, mu]
+        o4.load(W)
+        assert np.abs(o4.delta()[y] - D[x]).max() <= 1e-14 * max(1.0, np.abs(D[x]).max()), (dims, x)
+        # S2: sum_mu [2 X(x) - X(x+mu) - X(x-mu)] = 16 Delta(x)
+        lap = sum(2.0 * X[x] - X[nb_f[mu]] - X[nb_b[mu]] for mu in range(4))
+        assert np.abs(lap - 16.0 * D[x]).max() <= 1e-11 * max(xs, 1.0), (dims, x)
+    # S3 + S4 on the sampled sites
+    F1, th1 = gf.iterate(1, ALPHA)
+    U1 = torch.empty_like(Ud)
+    gf.get_links_device(U1.data_ptr())
+    torch.cuda.synchronize()
+    for x in sites[:24] + sites[-4:]:
+        c = _site_coords(x, dims)
+        nb_f = [_site_index([c[k] + (1 if k == mu else 0) for k in range(4)], dims) for mu in range(4)]
+        g = oracle.project(np.ascontiguousarray(X[[x] + nb_f]), ALPHA)
+        Ux = Ud[x].cpu().numpy()
+        got = U1[x].cpu().numpy()
+        for mu in range(4):
+            want = g[0] @ Ux[mu] @ g[1 + mu].conj().T
+            want[2] = np.conj(np.cross(want[0], want[1]))           # 12-real storage (O6)
+            assert np.abs(got[mu] - want).max() <= 1e-13, (dims, x, mu)
+    assert F1 >= F0 - 1e-14
+    F3, th3 = gf.iterate(2, ALPHA)
+    assert F3 >= F1 - 1e-14
+    _, _, plaq3 = gf.measure()
+    assert abs(plaq3 - plaq0) <= 1e-12                              # gauge invariance of the plaquette
+    gf.destroy()
+
+
 def test_C1_ten_iterations_against_the_naive_dft_oracle():
     U, cfg = E.make_config("C1")
     o = oracle.Oracle(cfg["dims"], cfg["storage"], fft_mode=0)      # the definition

@@ -110,6 +110,33 @@ def haar_links_8():
     return dims, U
 
 
+def test_P18_filter_inverts_the_lattice_laplacian():
+    """p^2(n) = sum_mu 4 sin^2(pi n_mu/L_mu) are the eigenvalues of minus the nearest-neighbour lattice Laplacian, so the
+    Fourier-accelerated field obeys, site by site and with no transform in sight,
+        sum_mu [2 X(x) - X(x+mu) - X(x-mu)] = p2max * (Delta(x) - mean Delta) = 16 Delta(x)       (P4: mean Delta = 0).
+    Fixes the filter (every p^2 term, p2max, the zero mode), the 1/V of the inverse transform and the axis/wrap
+    handling of S2 together, on an anisotropic lattice, in both FFT modes."""
+    dims = (4, 8, 6, 4)
+    U = E.noisy(dims, 21, 0.4)
+    for mode in ((0, 1) if all((d & (d - 1)) == 0 for d in dims) else (0,)):
+        o = oracle.Oracle(dims, 18, fft_mode=mode)
+        o.load(U)
+        D = o.delta().reshape(dims[::-1] + (3, 3))
+        X = o.fa_field().reshape(dims[::-1] + (3, 3))
+        lap = np.zeros_like(X)
+        for ax in range(4):
+            lap += 2.0 * X - np.roll(X, 1, axis=ax) - np.roll(X, -1, axis=ax)
+        assert np.abs(lap - 16.0 * D).max() <= 1e-12 * np.abs(X).max()
+    dims = (8, 4, 4, 16)
+    U = E.noisy(dims, 22, 0.4)
+    o = oracle.Oracle(dims, 12, fft_mode=1)
+    o.load(U)
+    D = o.delta().reshape(dims[::-1] + (3, 3))
+    X = o.fa_field().reshape(dims[::-1] + (3, 3))
+    lap = sum(2.0 * X - np.roll(X, 1, axis=ax) - np.roll(X, -1, axis=ax) for ax in range(4))
+    assert np.abs(lap - 16.0 * D).max() <= 1e-12 * np.abs(X).max()
+
+
 def test_P3_P4_delta_traceless_antihermitian_zero_sum(haar_links_8):
     dims, U = haar_links_8
     o = oracle.Oracle(dims, 18)
