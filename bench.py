@@ -68,6 +68,20 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic(kernel: str):
+    """DRAM bytes (read + write) per launch of `kernel` from the committed ncu --set full capture
+    (profiles/r01_ncu_traffic.csv; the command that made it is in profiles/r01_README.md), or None."""
+    import csv
+    try:
+        with open(os.path.join(ROOT, "profiles", "r01_ncu_traffic.csv")) as f:
+            for r in csv.DictReader(f):
+                if r["kernel"] == kernel:
+                    return int(r["dram_read_bytes"]) + int(r["dram_write_bytes"])
+    except Exception:
+        pass
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -299,7 +313,8 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                         "frac": kernels[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                         "frac": kernels[dom]["frac"], "traffic": ncu_traffic(dom) if args.workload.startswith("C2") else None,
+                         "traffic_source": "profiles/r01_ncu_traffic.csv (ncu --set full, one launch, cold caches)", "peak_source": peak_src,
                          "bytes_per_launch": kernels[dom]["bytes_per_launch"], "avg_us": kernels[dom]["avg_us"],
                          "copy_kernel_gbs": copy_gbs},
             "iteration": {"bytes_per_site": iter_bytes // V, "bytes": iter_bytes, "gbs": iter_bytes * it_s_1 / 1e9,

@@ -133,6 +133,8 @@ struct lgf_ctx {
     // profiling
     int profiling;
     cudaEvent_t ev0, ev1;
+    std::vector<cudaEvent_t> ev_pool;   // profiling: event pairs recorded around launches, resolved in batches
+    std::vector<int> ev_slot;           // kernel slot of each recorded pair
     double prof_ms[LGF_MAX_KERNELS];
     long long prof_n[LGF_MAX_KERNELS];
     long long launches;
@@ -155,19 +157,37 @@ namespace {
 
 cplx* cur_links(const lgf_ctx* c) { return c->links + (size_t)c->parity * (c->lay.link_buf / 16); }
 
-// Launch bookkeeping: counts every kernel; in profiling mode brackets it with events and accumulates its time.
+// Profiling: resolve the event pairs recorded so far (one synchronisation for the whole batch, so the kernels run
+// back to back on the device and the pairs measure device time, not launch latency).
+constexpr size_t PROF_PAIRS = 1024;
+void prof_flush(lgf_ctx* c) {
+    if (c->ev_slot.empty()) return;
+    cudaStreamSynchronize(c->stream);
+    for (size_t i = 0; i < c->ev_slot.size(); i++) {
+        float ms = 0;
+        if (cudaEventElapsedTime(&ms, c->ev_pool[2 * i], c->ev_pool[2 * i + 1]) == cudaSuccess) {
+            c->prof_ms[c->ev_slot[i]] += ms; c->prof_n[c->ev_slot[i]]++;
+        }
+    }
+    c->ev_slot.clear();
+}
+// Launch bookkeeping: counts every kernel; in profiling mode brackets it with a pair of events.
 struct LaunchScope {
-    lgf_ctx* c; int slot;
-    LaunchScope(lgf_ctx* c_, int s) : c(c_), slot(s) {
-        if (c->profiling && !c->capturing) cudaEventRecord(c->ev0, c->stream);
+    lgf_ctx* c; int slot; bool rec;
+    LaunchScope(lgf_ctx* c_, int s) : c(c_), slot(s), rec(false) {
+        if (c->profiling && !c->capturing) {
+            if (c->ev_slot.size() >= PROF_PAIRS) prof_flush(c);
+            const size_t i = c->ev_slot.size();
+            while (c->ev_pool.size() < 2 * (i + 1)) { cudaEvent_t e = nullptr; if (cudaEventCreate(&e) != cudaSuccess) return; c->ev_pool.push_back(e); }
+            cudaEventRecord(c->ev_pool[2 * i], c->stream);
+            rec = true;
+        }
     }
     ~LaunchScope() {
         if (!c->capturing) c->launches++;
-        if (c->profiling && !c->capturing) {
-            cudaEventRecord(c->ev1, c->stream);
-            cudaEventSynchronize(c->ev1);
-            float ms = 0; cudaEventElapsedTime(&ms, c->ev0, c->ev1);
-            c->prof_ms[slot] += ms; c->prof_n[slot]++;
+        if (rec) {
+            cudaEventRecord(c->ev_pool[2 * c->ev_slot.size() + 1], c->stream);
+            c->ev_slot.push_back(slot);
         }
     }
 };
@@ -723,6 +743,7 @@ void lgf_destroy(lgf_ctx* c) {
     if (!c) return;
     if (c->stream) cudaStreamSynchronize(c->stream);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     if (c->h_ctl) cudaFreeHost(c->h_ctl);
@@ -882,12 +903,14 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
 
 lgf_status lgf_set_profiling(lgf_ctx* c, int on) {
     if (!c) return LGF_ERR_INVALID_ARG;
+    prof_flush(c);
     c->profiling = on ? 1 : 0;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
     return LGF_OK;
 }
 lgf_status lgf_get_profile(lgf_ctx* c, double ms[LGF_MAX_KERNELS], long long n[LGF_MAX_KERNELS]) {
     if (!c || !ms || !n) return LGF_ERR_INVALID_ARG;
+    prof_flush(c);
     memcpy(ms, c->prof_ms, sizeof c->prof_ms); memcpy(n, c->prof_n, sizeof c->prof_n);
     return LGF_OK;
 }
