@@ -49,6 +49,8 @@ def kernel_bytes_per_site(nc: int) -> dict:
         "k_update_x": 64 + 2 * lk,           # read X once (neighbours: cache), read + write links
         "k_update_g": 96 + 2 * lk,
         "k_update_quad": 64 + 2 * lk,        # same traffic as k_update_x, one thread per link
+        "k_fa_fwd1": 128,                    # 64-extent planes: forward axes 0,1 from/to the field, one component per CTA
+        "k_fa_inv1": 128,
         "k_finalize": 0,
         # compile-time-sized passes (fft_fast.cuh): same traffic as the generic passes they replace
         "k_fa_delta_fwd": lk + 64,
@@ -198,20 +200,37 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
-    U, cfg = make_links(args.workload, rank)
+    import ensembles as E
+    device_links = args.links == "device"
+    if device_links:
+        # seeded links generated on the device (ensembles.device_su3): for the large shapes (C3, C4), whose host recipe
+        # takes minutes; throughput does not depend on the configuration.  No end-to-end leg, no CPU baseline.
+        cfg = dict(E.CONFIGS[args.workload])
+        U = None
+    else:
+        U, cfg = make_links(args.workload, rank)
     dims, storage = cfg["dims"], cfg["storage"]
     V = int(np.prod(dims))
     nc = 6 if storage == 12 else 9
     inner = args.inner
-    # pinned host copies for the end-to-end leg
-    h_in = torch.from_numpy(U.view(np.float64).reshape(-1)).pin_memory()
-    h_out = torch.empty_like(h_in).pin_memory()
-    del U
-
     gf = lgf.GaugeFixer(dims, storage)
     if args.fuse_update is not None:
         gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, args.fuse_update)
-    gf.load_links(h_in.numpy())
+    if device_links:
+        d_in = E.device_su3(dims, cfg["seed"] + 100 * rank, 0.15)
+        h_in = h_out = None
+
+        def reload():
+            gf.load_links_device(d_in.data_ptr())
+    else:
+        # pinned host copies for the end-to-end leg
+        h_in = torch.from_numpy(U.view(np.float64).reshape(-1)).pin_memory()
+        h_out = torch.empty_like(h_in).pin_memory()
+        del U
+
+        def reload():
+            gf.load_links(h_in.numpy())
+    reload()
     _, _, plaq = gf.measure()
     stream = gf.stream            # the context's own torch stream: every kernel and copy is ordered on it
 
@@ -250,15 +269,18 @@ def run_ours(args):
         gf.get_links(h_out.numpy().view(np.complex128).reshape(V, 4, 3, 3))
 
     e2e_steps = max(2, min(args.steps, 5))
-    ms_e2e = timed(step_e2e, e2e_steps, 1)
-    e2e_value = world * e2e_steps * inner / (ms_e2e * 1e-3)
+    if device_links:
+        ms_e2e, e2e_value = None, None
+    else:
+        ms_e2e = timed(step_e2e, e2e_steps, 1)
+        e2e_value = world * e2e_steps * inner / (ms_e2e * 1e-3)
 
     line = None
     if rank == 0:
         peak, peak_src = measured_peak()
         kb = kernel_bytes_per_site(nc)
         # ---- per-kernel device times: CUDA events around every launch on the library's stream (plain launches)
-        gf.load_links(h_in.numpy())
+        reload()
         gf.iterate(10, ALPHA)
         gf.set_profiling(True)
         gf.iterate(inner, ALPHA)
@@ -281,7 +303,7 @@ def run_ours(args):
         iter_bytes = sum(kb[k] * V for k in kernels if k in kb)
         it_s_1 = value / world
         # ---- time to theta < 1e-15 (lgf_fix, links resident, all syncs included)
-        gf.load_links(h_in.numpy())
+        reload()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
         r = gf.fix(ALPHA, THETA_TOL, 100000)
@@ -290,7 +312,7 @@ def run_ours(args):
                "theta": r["theta"], "plaquette": plaq, "ensemble": args.workload}
         # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample
         cpu = None
-        if world == 1 and not args.no_cpu_baseline:
+        if world == 1 and not args.no_cpu_baseline and not device_links:
             import oracle
             o = oracle.Oracle(dims, storage, fft_mode=1)
             o.load(h_in.numpy().view(np.complex128).reshape(V, 4, 3, 3))
@@ -305,11 +327,11 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, eps={cfg.get('eps')}, seed={cfg['seed']}, alpha=0.08",
+            "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, " + ("device-generated links (ensembles.device_su3)" if device_links else f"eps={cfg.get('eps')}") + f", seed={cfg['seed']}, alpha=0.08",
                        "iterations_per_step": inner, "l2": "inputs larger than L2 (links %.0f MB + field %.0f MB per GPU)" % (V * nc * 64 / 1e6, V * 64 / 1e6),
                        "parallelism": "replicas" if world > 1 else "single"},
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": V * 576, "d2h_bytes_per_step": V * 576 + 16,
-                    "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
+            "e2e": None if device_links else {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": V * 576, "d2h_bytes_per_step": V * 576 + 16,
+                                              "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
@@ -340,6 +362,9 @@ def main():
     ap.add_argument("--workload", default="C2b", help="ensemble name from ensembles.CONFIGS (C2b = 32^4, eps 0.35)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--links", default="host", choices=["host", "device"],
+                    help="host: the seeded BASELINE.json ensemble built with numpy (default); device: seeded links generated on the GPU "
+                         "(large shapes C3, C4; no e2e leg, no CPU baseline)")
     ap.add_argument("--fuse-update", type=int, default=None, choices=[0, 1],
                     help="override LGF_OPT_FUSE_UPDATE (kernel A/B timing); default: the library's choice")
     args = ap.parse_args()
