@@ -297,8 +297,9 @@ def run_ours(args):
         dom = max((k for k in kernels if kb.get(k, 0) > 0), key=lambda k: prof[k]["ms"])
         try:
             copy_gbs = lgf.copy_peak_gbs(1 << 30, 10)
+            stream_gbs = {"read": lgf.stream_peak_gbs(V, False, 10), "read_write_in_place": lgf.stream_peak_gbs(V, True, 10)}
         except Exception:
-            copy_gbs = None
+            copy_gbs, stream_gbs = None, None
         # bytes of one iteration = the kernels that actually ran (each launched once per iteration)
         iter_bytes = sum(kb[k] * V for k in kernels if k in kb)
         it_s_1 = value / world
@@ -338,7 +339,7 @@ def run_ours(args):
                          "frac": kernels[dom]["frac"], "traffic": ncu_traffic(dom) if args.workload.startswith("C2") else None,
                          "traffic_source": "profiles/r01_ncu_traffic.csv (ncu --set full, one launch, cold caches)", "peak_source": peak_src,
                          "bytes_per_launch": kernels[dom]["bytes_per_launch"], "avg_us": kernels[dom]["avg_us"],
-                         "copy_kernel_gbs": copy_gbs},
+                         "copy_kernel_gbs": copy_gbs, "stream_yardstick_gbs": stream_gbs},
             "iteration": {"bytes_per_site": iter_bytes // V, "bytes": iter_bytes, "gbs": iter_bytes * it_s_1 / 1e9,
                           "frac_of_measured": iter_bytes * it_s_1 / 1e9 / peak, "frac_of_spec_8000": iter_bytes * it_s_1 / 1e9 / 8000.0},
             "kernels": kernels,

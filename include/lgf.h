@@ -157,6 +157,13 @@ long long lgf_launch_count(lgf_ctx *ctx);
  * (HOST).  This is the "measured copy-kernel peak" of the north star: GB/s = 2*bytes/ms/1e6. */
 lgf_status lgf_copy_peak(void *dev_dst, const void *dev_src, size_t bytes, int reps, void *cuda_stream, double *ms);
 
+/* Second yardstick: the access pattern of the link kernels without their arithmetic.  dev_buf, DEVICE, holds 24 arrays
+ * of n_sites double2 (24 * 16 * n_sites bytes: the 12-real link store of n_sites sites); one thread per site reads its
+ * entry of each array (write = 0) or reads it and writes it back in place (write = 1), 128 threads per CTA.  n_sites a
+ * multiple of 128.  *ms, HOST, receives the mean time of one of `reps` launches after one warm-up; bytes moved per
+ * launch: 384 * n_sites * (1 + write).  Same errors as lgf_copy_peak. */
+lgf_status lgf_stream_peak(void *dev_buf, size_t n_sites, int write, int reps, void *cuda_stream, double *ms);
+
 const char *lgf_status_string(lgf_status s);
 const char *lgf_last_error(lgf_ctx *ctx); /* detail of the last LGF_ERR_CUDA (static or ctx-owned string) */
 

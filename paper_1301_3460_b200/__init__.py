@@ -16,7 +16,7 @@ import os
 import numpy as np
 
 __all__ = [
-    "LgfError", "lib", "library_path", "GaugeFixer", "copy_peak_gbs",
+    "LgfError", "lib", "library_path", "GaugeFixer", "copy_peak_gbs", "stream_peak_gbs",
     "LGF_OK", "LGF_NOT_CONVERGED", "LGF_FP64", "LGF_FP32", "LGF_STORE_12", "LGF_STORE_18",
     "LGF_FIELD_DELTA", "LGF_FIELD_X", "LGF_FIELD_G",
     "LGF_OPT_FUSE_DELTA_FFT", "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_FAST_FFT", "LGF_OPT_FUSE_UPDATE",
@@ -44,7 +44,7 @@ EXPORTS = [
     "lgf_workspace_bytes", "lgf_create", "lgf_create_ex", "lgf_destroy", "lgf_load_links", "lgf_load_links_device",
     "lgf_get_links", "lgf_get_links_device", "lgf_iterate", "lgf_fix", "lgf_measure", "lgf_get_history",
     "lgf_get_field", "lgf_set_option", "lgf_get_option", "lgf_set_profiling", "lgf_get_profile", "lgf_kernel_name",
-    "lgf_launch_count", "lgf_copy_peak", "lgf_status_string", "lgf_last_error",
+    "lgf_launch_count", "lgf_copy_peak", "lgf_stream_peak", "lgf_status_string", "lgf_last_error",
 ]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -108,6 +108,7 @@ def lib():
     L.lgf_launch_count.restype = C.c_longlong
     L.lgf_launch_count.argtypes = [P]
     L.lgf_copy_peak.argtypes = [P, P, C.c_size_t, C.c_int, P, D]
+    L.lgf_stream_peak.argtypes = [P, C.c_size_t, C.c_int, C.c_int, P, D]
     L.lgf_status_string.restype = C.c_char_p
     L.lgf_status_string.argtypes = [C.c_int]
     L.lgf_last_error.restype = C.c_char_p
@@ -290,3 +291,15 @@ def copy_peak_gbs(nbytes: int = 1 << 30, reps: int = 10) -> float:
     if st != LGF_OK:
         raise LgfError(st, "lgf_copy_peak")
     return 2.0 * nbytes / ms.value / 1e6
+
+
+def stream_peak_gbs(n_sites: int = 1 << 20, write: bool = False, reps: int = 10) -> float:
+    """GB/s of the 24-stream yardstick (lgf_stream_peak): the link kernels' access pattern without their arithmetic."""
+    import torch
+    a = torch.zeros(n_sites * 24 * 2, dtype=torch.float64, device="cuda")
+    ms = C.c_double()
+    s = torch.cuda.current_stream()
+    st = lib().lgf_stream_peak(C.c_void_p(a.data_ptr()), n_sites, 1 if write else 0, reps, C.c_void_p(s.cuda_stream), C.byref(ms))
+    if st != LGF_OK:
+        raise LgfError(st, "lgf_stream_peak")
+    return 384.0 * n_sites * (2 if write else 1) / ms.value / 1e6

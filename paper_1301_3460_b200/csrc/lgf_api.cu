@@ -938,6 +938,27 @@ lgf_status lgf_copy_peak(void* dst, const void* src, size_t bytes, int reps, voi
     return LGF_OK;
 }
 
+lgf_status lgf_stream_peak(void* buf, size_t n_sites, int write, int reps, void* stream, double* ms) {
+    if (!buf || !ms || reps < 1 || n_sites < 128 || (n_sites & 127)) return LGF_ERR_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return LGF_ERR_CUDA;
+    double2* p = static_cast<double2*>(buf);
+    const unsigned grid = (unsigned)(n_sites / 128);
+    const long long V = (long long)n_sites;
+    for (int i = -1; i < reps; i++) {
+        if (i == 0) cudaEventRecord(a, s);
+        if (write) k_streams<1><<<grid, 128, 0, s>>>(p, V, p); else k_streams<0><<<grid, 128, 0, s>>>(p, V, p);
+    }
+    cudaEventRecord(b, s);
+    cudaError_t e = cudaEventSynchronize(b);
+    float t = 0; cudaEventElapsedTime(&t, a, b);
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return LGF_ERR_CUDA;
+    *ms = (double)t / reps;
+    return LGF_OK;
+}
+
 const char* lgf_status_string(lgf_status s) {
     switch (s) {
         case LGF_OK: return "ok";

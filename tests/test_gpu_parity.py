@@ -460,6 +460,7 @@ def test_launch_count_and_profile():
     assert prof["k_fft23_mid"]["launches"] == 5 and prof["k_update_quad"]["launches"] == 5
     assert all(v["ms"] > 0 for v in prof.values())
     assert lgf.copy_peak_gbs(1 << 28, 3) > 500.0
+    assert lgf.stream_peak_gbs(1 << 18, False, 3) > 500.0 and lgf.stream_peak_gbs(1 << 18, True, 3) > 500.0
 
 
 def test_fused_update_buffers_and_counts():
