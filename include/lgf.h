@@ -134,10 +134,14 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_PDL             1 (default): the kernels of an iteration are launched with programmatic dependent launch
  *                           (each waits on the device for the complete end of its predecessor, so results are
  *                           unchanged; launch latency and CTA ramp-up overlap the predecessor's tail), 0: plain
- *                           stream-ordered launches. */
+ *                           stream-ordered launches.
+ *   LGF_OPT_FOURIER_ACCEL   1 (default): the paper's method, X = IFFT[(p2max/p2) FFT[Delta]].  0: plain steepest
+ *                           descent, X = Delta (the method Fourier acceleration is measured against, PAPER.md:41 refs
+ *                           [1],[2]): S2 drops out, an iteration is S1, S5, S3+S4.  Converges for alpha < 2/p2max = 1/8,
+ *                           with a rate that degrades with the volume (critical slowing down). */
 typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
                LGF_OPT_FUSE_UPDATE = 5, LGF_OPT_PINGPONG = 6, LGF_OPT_FUSE_FINALIZE = 7,
-               LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9 } lgf_option;
+               LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9, LGF_OPT_FOURIER_ACCEL = 10 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

@@ -117,7 +117,7 @@ struct lgf_ctx {
     Ctl* h_ctl;             // pinned
     bool loaded;
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel;
     int sms;                // SMs of the device: grid of the persistent passes
     int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
@@ -505,7 +505,7 @@ bool use_store_g(const lgf_ctx* c) { return c->opt_store_g && c->fft01_ncomp_fus
 bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a && use_fused(c); }
 bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
 bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c && !use_store_g(c); }
-bool use_fused_update(const lgf_ctx* c) { return c->opt_fuse_update && c->opt_fast && c->fast_a; }
+bool use_fused_update(const lgf_ctx* c) { return c->opt_accel && c->opt_fuse_update && c->opt_fast && c->fast_a; }
 bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p && !use_store_g(c); }
 bool use_pp_a(const lgf_ctx* c) { return (c->opt_pingpong & 1) && use_fast_a(c); }
 bool use_pp_b(const lgf_ctx* c) { return (c->opt_pingpong & 2) && use_fast_b(c) && c->pp_b_ok; }
@@ -533,6 +533,12 @@ template <int NC> void enqueue_tail(lgf_ctx* c, double half_alpha) {
     else { launch_inv_x(c); launch_update<NC, 0>(c, half_alpha); }
 }
 void enqueue_body(lgf_ctx* c, double half_alpha) {
+    if (!c->opt_accel) {
+        // plain steepest descent (no Fourier acceleration, PAPER.md:41 refs [1],[2]): X = Delta, so S2 drops out
+        if (c->NC == 6) { launch_delta<6>(c); launch_finalize(c, (int)(c->G.V / 128)); launch_update<6, 0>(c, half_alpha); }
+        else { launch_delta<9>(c); launch_finalize(c, (int)(c->G.V / 128)); launch_update<9, 0>(c, half_alpha); }
+        return;
+    }
     if (use_fused_update(c)) {
         // pass B, pass C ending in g, then update + next Delta + next pass A, and the measurement of the updated links
         launch_mid(c);
@@ -546,6 +552,7 @@ void enqueue_body(lgf_ctx* c, double half_alpha) {
 }
 bool use_fused_fin(const lgf_ctx* c) { return c->opt_fuse_fin && use_fast_a(c) && !use_pp_a(c); }
 int launches_per_body(const lgf_ctx* c) {
+    if (!c->opt_accel) return 3;
     if (use_fused_update(c) || use_fused_fin(c)) return 4;
     if (use_big_p(c) && !use_fast_a(c) && !use_pp_a(c)) return 6;
     return use_fused(c) ? 5 : 6;
@@ -578,7 +585,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -646,7 +653,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
     c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
@@ -840,7 +847,7 @@ lgf_status lgf_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host
     if (st != LGF_OK) return st;
     const double ha = 0.5 * alpha;
     bool g_from_buf = false;
-    if (which == LGF_FIELD_DELTA) {
+    if (which == LGF_FIELD_DELTA || !c->opt_accel) {       // plain steepest descent: X = Delta
         if (c->NC == 6) launch_delta<6>(c); else launch_delta<9>(c);
     } else {
         if (c->NC == 6) enqueue_head<6>(c); else enqueue_head<9>(c);
@@ -879,6 +886,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_FUSE_FINALIZE: c->opt_fuse_fin = value ? 1 : 0; break;
         case LGF_OPT_QUAD_UPDATE: c->opt_quad = value ? 1 : 0; break;
         case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
+        case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
@@ -895,6 +903,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_PINGPONG: *value = (use_pp_a(c) ? 1 : 0) | (use_pp_b(c) ? 2 : 0) | (use_pp_c(c) ? 4 : 0); break;
         case LGF_OPT_FUSE_FINALIZE: *value = use_fused_fin(c) ? 1 : 0; break;
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
+        case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }

@@ -311,6 +311,44 @@ def test_full_size_sampled_sites_and_invariants(dims):
     gf.destroy()
 
 
+@pytest.mark.parametrize("dims,storage", [((8, 8, 8, 8), 18), ((16, 16, 16, 16), 12), ((4, 8, 16, 4), 12)])
+def test_plain_steepest_descent_variant(dims, storage):
+    """LGF_OPT_FOURIER_ACCEL = 0 (X = Delta) against the oracle's unaccelerated variant:
+    trajectory, links, and the first-order rate dF/dalpha = theta/16 of pin P8."""
+    U = E.noisy(dims, 51, 0.3)
+    o = oracle.Oracle(dims, storage)
+    o.set_variant(accel=0)
+    o.load(U)
+    X_ref = o.fa_field()
+    r_ref = o.fix(ALPHA, 0.0, 20, history=True)
+    gf = lgf.GaugeFixer(dims, storage)
+    for quad in (1, 0):
+        gf.set_option(lgf.LGF_OPT_FOURIER_ACCEL, 0)
+        gf.set_option(lgf.LGF_OPT_QUAD_UPDATE, quad)
+        assert gf.get_option(lgf.LGF_OPT_FOURIER_ACCEL) == 0
+        gf.load_links(U)
+        assert np.abs(gf.get_field(lgf.LGF_FIELD_X) - X_ref).max() <= 1e-13 * np.abs(X_ref).max()
+        n0 = gf.launch_count()
+        F, th = gf.iterate(20, ALPHA)
+        assert gf.launch_count() - n0 == 3 * 21
+        h = gf.get_history()
+        href = np.array(r_ref["history"])
+        assert np.abs(h[:, 0] - href[:, 0]).max() <= F_TOL
+        assert all(theta_close(a, b) for a, b in zip(h[:, 1], href[:, 1]))
+        assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
+        assert np.all(np.diff(h[:, 0]) >= -1e-14)                       # F rises monotonically for alpha < 1/8
+    # pin P8 on the GPU: dF/dalpha at alpha -> 0 equals theta/16 without the filter
+    gf.load_links(U)
+    F0, th0, _ = gf.measure()
+    a = 1e-4
+    F1, _ = gf.iterate(1, a)
+    assert abs((F1 - F0) / a - th0 / 16.0) <= 2e-3 * th0 / 16.0
+    gf.set_option(lgf.LGF_OPT_FOURIER_ACCEL, 1)
+    gf.load_links(U)
+    F, th = gf.iterate(20, ALPHA)
+    assert th < href[-1, 1]                                              # Fourier acceleration converges faster
+
+
 def test_C1_ten_iterations_against_the_naive_dft_oracle():
     U, cfg = E.make_config("C1")
     o = oracle.Oracle(cfg["dims"], cfg["storage"], fft_mode=0)      # the definition
