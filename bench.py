@@ -37,28 +37,30 @@ UNIT = "iterations/s"
 
 # Algorithmic HBM bytes per site per launch of each hot-path kernel:
 # links cost 16*NC bytes per direction (NC = 6 two-row, 9 full), the packed field 64 B/site.
-def kernel_bytes_per_site(nc: int) -> dict:
-    lk = 4 * nc * 16
+def kernel_bytes_per_site(nc: int, cb: int = 16) -> dict:
+    """cb: bytes of one stored complex number (16 fp64, 8 fp32)."""
+    lk = 4 * nc * cb
+    fld, g = 4 * cb, 6 * cb
     return {
-        "k_fft01_delta_fwd": lk + 64,        # read own links once (backward neighbours: cache), write Delta~ field
-        "k_delta": lk + 64,
-        "k_fft01_fwd": 128,
-        "k_fft23_mid": 128,                  # read + write the field (forward, filter, inverse on chip)
-        "k_fft01_inv": 128,
-        "k_fft01_inv_g": 64 + 96,
-        "k_update_x": 64 + 2 * lk,           # read X once (neighbours: cache), read + write links
-        "k_update_g": 96 + 2 * lk,
-        "k_update_quad": 64 + 2 * lk,        # same traffic as k_update_x, one thread per link
-        "k_fa_fwd1": 128,                    # 64-extent planes: forward axes 0,1 from/to the field, one component per CTA
-        "k_fa_inv1": 128,
+        "k_fft01_delta_fwd": lk + fld,       # read own links once (backward neighbours: cache), write Delta~ field
+        "k_delta": lk + fld,
+        "k_fft01_fwd": 2 * fld,
+        "k_fft23_mid": 2 * fld,              # read + write the field (forward, filter, inverse on chip)
+        "k_fft01_inv": 2 * fld,
+        "k_fft01_inv_g": fld + g,
+        "k_update_x": fld + 2 * lk,          # read X once (neighbours: cache), read + write links
+        "k_update_g": g + 2 * lk,
+        "k_update_quad": fld + 2 * lk,       # same traffic as k_update_x, one thread per link
+        "k_fa_fwd1": 2 * fld,                # 64-extent planes: forward axes 0,1 from/to the field, one component per CTA
+        "k_fa_inv1": 2 * fld,
         "k_finalize": 0,
         # compile-time-sized passes (fft_fast.cuh): same traffic as the generic passes they replace
-        "k_fa_delta_fwd": lk + 64,
-        "k_fa_mid": 128,
-        "k_fa_inv": 128,
-        "k_fa_inv_g": 64 + 96,               # read X~ field, write rows 0,1 of g
-        # fused S3/S4 + next S1 + next pass A (fused_update.cuh): g 96, links read once + written once, field written
-        "k_fu_update_delta_fwd": 96 + 2 * lk + 64,
+        "k_fa_delta_fwd": lk + fld,
+        "k_fa_mid": 2 * fld,
+        "k_fa_inv": 2 * fld,
+        "k_fa_inv_g": fld + g,               # read X~ field, write rows 0,1 of g
+        # fused S3/S4 + next S1 + next pass A (fused_update.cuh): g, links read once + written once, field written
+        "k_fu_update_delta_fwd": g + 2 * lk + fld,
     }
 
 
@@ -213,7 +215,8 @@ def run_ours(args):
     V = int(np.prod(dims))
     nc = 6 if storage == 12 else 9
     inner = args.inner
-    gf = lgf.GaugeFixer(dims, storage)
+    fp32 = args.precision == "fp32"
+    gf = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_FP32 if fp32 else lgf.LGF_FP64)
     if args.fuse_update is not None:
         gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, args.fuse_update)
     if device_links:
@@ -278,7 +281,7 @@ def run_ours(args):
     line = None
     if rank == 0:
         peak, peak_src = measured_peak()
-        kb = kernel_bytes_per_site(nc)
+        kb = kernel_bytes_per_site(nc, 8 if fp32 else 16)
         # ---- per-kernel device times: CUDA events around every launch on the library's stream (plain launches)
         reload()
         gf.iterate(10, ALPHA)
@@ -307,10 +310,10 @@ def run_ours(args):
         reload()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        r = gf.fix(ALPHA, THETA_TOL, 100000)
+        r = gf.fix(ALPHA, 1e-10 if fp32 else THETA_TOL, 100000)      # fp32 bottoms out near theta = 1e-14
         torch.cuda.synchronize()
         ttt = {"ms": (time.perf_counter() - t0) * 1e3, "n_iter": r["n_iter"], "status": r["status"], "F": r["F"],
-               "theta": r["theta"], "plaquette": plaq, "ensemble": args.workload}
+               "theta": r["theta"], "theta_tol": 1e-10 if fp32 else THETA_TOL, "plaquette": plaq, "ensemble": args.workload}
         # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample
         cpu = None
         if world == 1 and not args.no_cpu_baseline and not device_links:
@@ -325,9 +328,9 @@ def run_ours(args):
             cpu = {"value": n_cpu / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                    "sample": f"{n_cpu} iterations of {args.workload} ({dims_name(dims)}, {storage}-real), oracle radix-2 FFT mode, after 1 warm-up"}
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "metric": METRIC.replace("fp64", "fp32") if fp32 else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64", "data": "synthetic",
+            "dtype": "f32" if fp32 else "f64", "data": "synthetic",
             "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, " + ("device-generated links (ensembles.device_su3)" if device_links else f"eps={cfg.get('eps')}") + f", seed={cfg['seed']}, alpha=0.08",
                        "iterations_per_step": inner, "l2": "inputs larger than L2 (links %.0f MB + field %.0f MB per GPU)" % (V * nc * 64 / 1e6, V * 64 / 1e6),
                        "parallelism": "replicas" if world > 1 else "single"},
@@ -336,7 +339,7 @@ def run_ours(args):
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                         "frac": kernels[dom]["frac"], "traffic": ncu_traffic(dom) if args.workload.startswith("C2") else None,
+                         "frac": kernels[dom]["frac"], "traffic": ncu_traffic(dom) if (args.workload.startswith("C2") and not fp32) else None,
                          "traffic_source": "profiles/r01_ncu_traffic.csv (ncu --set full, one launch, cold caches)", "peak_source": peak_src,
                          "bytes_per_launch": kernels[dom]["bytes_per_launch"], "avg_us": kernels[dom]["avg_us"],
                          "copy_kernel_gbs": copy_gbs, "stream_yardstick_gbs": stream_gbs},
@@ -363,6 +366,9 @@ def main():
     ap.add_argument("--workload", default="C2b", help="ensemble name from ensembles.CONFIGS (C2b = 32^4, eps 0.35)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
+                    help="fp64: the BASELINE.json metric (default); fp32: LGF_FP32 storage and arithmetic (SURVEY.md 8(f) NEXT-1), "
+                         "reported with dtype f32 and its own byte model; time_to_theta then stops at theta < 1e-10")
     ap.add_argument("--links", default="host", choices=["host", "device"],
                     help="host: the seeded BASELINE.json ensemble built with numpy (default); device: seeded links generated on the GPU "
                          "(large shapes C3, C4; no e2e leg, no CPU baseline)")

@@ -52,7 +52,12 @@ typedef enum {
     LGF_NOT_CONVERGED = 100   /* non-fatal: max_iter reached, state and outputs valid */
 } lgf_status;
 
-typedef enum { LGF_FP64 = 0, LGF_FP32 = 1 /* not built yet: LGF_ERR_UNSUPPORTED */ } lgf_precision;
+/* Precision of link storage and of the per-site arithmetic.  LGF_FP64: the paper's setting.
+ * LGF_FP32: links and field stored as float, every kernel computes in float; the
+ * lattice sums (theta, F) and the p^2 filter weights stay double.  Half the HBM bytes per iteration; theta bottoms out
+ * near 1e-12 (fp32 rounding of Delta), so theta < 1e-15 is not reachable in this precision alone.  Host- and
+ * device-side link and field arrays of this API are double in every precision (converted on load and on get). */
+typedef enum { LGF_FP64 = 0, LGF_FP32 = 1 } lgf_precision;
 typedef enum { LGF_STORE_18 = 18, LGF_STORE_12 = 12 } lgf_storage;
 
 /* Bytes of device workspace a context for these parameters needs (0 if the parameters are unsupported). */

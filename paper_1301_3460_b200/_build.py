@@ -13,8 +13,10 @@ DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "fft_tile.cuh",
     os.path.join(os.path.dirname(HERE), "include", "lgf.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-shared", "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v",
+    "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v",
 ]
+# lgf_api.cu is compiled twice: fp64 (public lgf_* entry points) and, with -DLGF_F32, fp32 (lgf32_* twins)
+OBJECTS = [("lgf_api_f64.o", []), ("lgf_api_f32.o", ["-DLGF_F32"])]
 
 
 def nvcc() -> str:
@@ -31,14 +33,25 @@ def up_to_date() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return OUT
-    cmd = [nvcc()] + NVCC_FLAGS + SOURCES + ["-o", OUT]
+    procs = []
+    for obj, extra in OBJECTS:
+        cmd = [nvcc()] + NVCC_FLAGS + extra + ["-c"] + SOURCES + ["-o", os.path.join(HERE, obj)]
+        procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
+    log = ""
+    for cmd, p in procs:
+        out, err = p.communicate()
+        log += "# " + " ".join(cmd) + "\n" + err
+        if verbose or p.returncode != 0:
+            sys.stderr.write(out + err)
+        if p.returncode != 0:
+            raise RuntimeError("nvcc failed: " + " ".join(cmd))
+    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared"] + [os.path.join(HERE, o) for o, _ in OBJECTS] + ["-o", OUT]
     res = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed: " + " ".join(cmd))
+        sys.stderr.write(res.stdout + res.stderr)
+        raise RuntimeError("link failed: " + " ".join(cmd))
     with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
-        f.write("# " + " ".join(cmd) + "\n" + res.stderr)
+        f.write(log)
     return OUT
 
 

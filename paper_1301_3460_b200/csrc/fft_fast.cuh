@@ -299,7 +299,7 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cp
     for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
     for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
 #if defined(LGF_DBG_A) && LGF_DBG_A == 2      // timing experiment: no S1 (tile filled with constants)
-    for (int e = threadIdx.x; e < 4 * SC; e += NT) tile[e] = mk(1e-3 * (e & 15), 1e-3);
+    for (int e = threadIdx.x; e < 4 * SC; e += NT) tile[e] = mk((real)(1e-3 * (e & 15)), (real)1e-3);
     if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(1.0, 1.0);
     __syncthreads();
 #else
@@ -390,7 +390,7 @@ __device__ __forceinline__ void pass_c_finish(cplx* __restrict__ fbase, cplx* __
         for (int e = g.tid; e < nP; e += NT) {
             const int o = (e & (L0 - 1)) + (e >> LG0) * S;
             cplx gm[9];
-            build_g(tile[o], tile[SC + o], tile[2 * SC + o], tile[3 * SC + o], half_alpha, gm);
+            build_g(tile[o], tile[SC + o], tile[2 * SC + o], tile[3 * SC + o], (real)half_alpha, gm);
 #pragma unroll
             for (int c = 0; c < 6; c++) gbase[(long long)c * V + e] = gm[c];
         }
@@ -569,7 +569,7 @@ __device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01,
                 for (int m = 0; m < PB::R2; m++) {
                     const double p2 = s012 + s3[bb * PB::R2 + m];
                     const double wgt = (p2 > 0.0) ? scale / p2 : 0.0;
-                    v[m] = cscale(v[m], wgt);
+                    v[m] = cscale(v[m], (real)wgt);
                 }
                 bfly<PB::R2, true>(v);
 #pragma unroll

@@ -49,7 +49,7 @@ template <bool INV> __device__ __forceinline__ void bfly8(cplx (&v)[8]) {
     // even/odd split: E = DFT4(v0,v2,v4,v6), O = DFT4(v1,v3,v5,v7); y_m = E_m + W8^m O_m, y_{m+4} = E_m - W8^m O_m
     bfly4<INV>(v[0], v[2], v[4], v[6]);   // now v0,v2,v4,v6 = E_0..E_3
     bfly4<INV>(v[1], v[3], v[5], v[7]);   // now v1,v3,v5,v7 = O_0..O_3
-    const double h = 0.70710678118654752440;
+    const real h = (real)0.70710678118654752440;
     cplx o1 = v[3], o2 = v[5], o3 = v[7];
     // W8^1 = h(1 -+ i), W8^2 = -+ i, W8^3 = h(-1 -+ i)
     cplx w1 = INV ? mk(h * (o1.x - o1.y), h * (o1.x + o1.y)) : mk(h * (o1.x + o1.y), h * (o1.y - o1.x));

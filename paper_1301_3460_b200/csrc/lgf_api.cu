@@ -2,6 +2,67 @@
 // the iteration driver (device-side stop flag, CUDA-graph replay) and the boundary copies.
 // There is deliberately no CPU fallback: every compute entry point needs a CUDA device.
 #include "../../include/lgf.h"
+
+// This file is compiled twice into liblgf.so: as it stands (fp64: real = double) and with -DLGF_F32 (fp32 storage and
+// arithmetic: real = float, lattice sums still double).  The fp32 build lives in its own namespace, has its own
+// context type and exports its entry points as lgf32_*; the fp64 entry points (the public lgf_* names) forward to
+// them when the context, or the precision argument of lgf_create*, says LGF_FP32.  Every context starts with its
+// precision, so the public opaque handle can be told apart.
+#ifdef LGF_F32
+#define lgf lgf32
+#define lgf_ctx lgf32_ctx
+#define lgf_workspace_bytes lgf32_workspace_bytes
+#define lgf_create_ex lgf32_create_ex
+#define lgf_create lgf32_create
+#define lgf_destroy lgf32_destroy
+#define lgf_load_links_device lgf32_load_links_device
+#define lgf_load_links lgf32_load_links
+#define lgf_get_links_device lgf32_get_links_device
+#define lgf_get_links lgf32_get_links
+#define lgf_iterate lgf32_iterate
+#define lgf_fix lgf32_fix
+#define lgf_measure lgf32_measure
+#define lgf_get_history lgf32_get_history
+#define lgf_get_field lgf32_get_field
+#define lgf_set_option lgf32_set_option
+#define lgf_get_option lgf32_get_option
+#define lgf_set_profiling lgf32_set_profiling
+#define lgf_get_profile lgf32_get_profile
+#define lgf_launch_count lgf32_launch_count
+#define lgf_last_error lgf32_last_error
+struct lgf_ctx;
+extern "C" void lgf_destroy(lgf_ctx* c);
+#define LGF_THIS_PREC LGF_FP32
+#define FWD32(call)
+#define FWD32V(call)
+#else
+#define LGF_THIS_PREC LGF_FP64
+extern "C" {
+size_t lgf32_workspace_bytes(const int dims[4], lgf_precision p, lgf_storage s);
+lgf_status lgf32_create(const int dims[4], lgf_precision p, lgf_storage s, lgf_ctx** out);
+lgf_status lgf32_create_ex(const int dims[4], lgf_precision p, lgf_storage s, void* ws, size_t bytes, void* stream, lgf_ctx** out);
+void lgf32_destroy(lgf_ctx* c);
+lgf_status lgf32_load_links(lgf_ctx* c, const double* host_links);
+lgf_status lgf32_load_links_device(lgf_ctx* c, const double* dev_links);
+lgf_status lgf32_get_links(lgf_ctx* c, double* host_links);
+lgf_status lgf32_get_links_device(lgf_ctx* c, double* dev_links);
+lgf_status lgf32_iterate(lgf_ctx* c, int n, double alpha, double* F, double* theta);
+lgf_status lgf32_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int* n_iter, double* F, double* theta);
+lgf_status lgf32_measure(lgf_ctx* c, double* F, double* theta, double* plaq);
+lgf_status lgf32_get_history(lgf_ctx* c, double* hist, int capacity, int* n_out);
+lgf_status lgf32_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host_field);
+lgf_status lgf32_set_option(lgf_ctx* c, lgf_option opt, int value);
+lgf_status lgf32_get_option(lgf_ctx* c, lgf_option opt, int* value);
+lgf_status lgf32_set_profiling(lgf_ctx* c, int on);
+lgf_status lgf32_get_profile(lgf_ctx* c, double ms[LGF_MAX_KERNELS], long long n[LGF_MAX_KERNELS]);
+long long lgf32_launch_count(lgf_ctx* c);
+const char* lgf32_last_error(lgf_ctx* c);
+}
+// forward to the fp32 twin when the context is an fp32 one (the precision is the first member of both context types)
+#define FWD32(call) if (c && *reinterpret_cast<const int*>(c) == (int)LGF_FP32) return call;
+#define FWD32V(call) if (c && *reinterpret_cast<const int*>(c) == (int)LGF_FP32) { call; return; }
+#endif
+
 #include "kernels.cuh"
 #include "fft_fast.cuh"
 #include "fused_update.cuh"
@@ -56,10 +117,10 @@ Layout make_layout(const int dims[4], int NC) {
     Layout o;
     const long long V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
     size_t off = 0;
-    o.link_buf = align_up((size_t)V * 4 * NC * 16, 256);
+    o.link_buf = align_up((size_t)V * 4 * NC * sizeof(cplx), 256);
     o.links = off; off += 2 * o.link_buf;
-    o.field = off; off = align_up(off + (size_t)V * 4 * 16, 256);
-    o.gbuf = off; off = align_up(off + (size_t)V * 6 * 16, 256);
+    o.field = off; off = align_up(off + (size_t)V * 4 * sizeof(cplx), 256);
+    o.gbuf = off; off = align_up(off + (size_t)V * 6 * sizeof(cplx), 256);
     o.n_partials = (int)(V / 128);                       // k_delta / k_plaquette: one per 128-site block
     if (o.n_partials < dims[2] * dims[3]) o.n_partials = dims[2] * dims[3];   // fused pass A: one per (x2,x3) plane
     o.partials = off; off = align_up(off + (size_t)o.n_partials * 16, 256);
@@ -104,13 +165,15 @@ int stored_freq(int p, int lgL, const AxisPlan& plan) {
 }  // namespace
 
 struct lgf_ctx {
+    int precision;          // LGF_FP64 or LGF_FP32: FIRST member of the context in both builds
     Geom G;
     int NC;                 // 6 or 9
     Layout lay;
     char* ws;               // workspace base (device)
     bool own_ws, own_stream;
     cudaStream_t stream;
-    cplx *links, *field, *gbuf, *staging;
+    cplx *links, *field, *gbuf;
+    dcplx* staging;         // host-facing double complex (AoS chunks of the boundary copies)
     double2 *partials, *hist;
     Ctl* ctl;
     FftTables T;
@@ -155,7 +218,7 @@ namespace {
         }                                                                                                  \
     } while (0)
 
-cplx* cur_links(const lgf_ctx* c) { return c->links + (size_t)c->parity * (c->lay.link_buf / 16); }
+cplx* cur_links(const lgf_ctx* c) { return c->links + (size_t)c->parity * (c->lay.link_buf / sizeof(cplx)); }
 
 // Profiling: resolve the event pairs recorded so far (one synchronisation for the whole batch, so the kernels run
 // back to back on the device and the pairs measure device time, not launch latency).
@@ -260,10 +323,10 @@ bool big_pair(int lga, int lgb) {
 #undef X
     return false;
 }
-size_t smem_fast_plane(int lga, int lgb, int ncomp) { return (size_t)(((1 << lga) + 1) * (1 << lgb) * ncomp + (1 << lga) + (1 << lgb)) * 16; }
+size_t smem_fast_plane(int lga, int lgb, int ncomp) { return (size_t)(((1 << lga) + 1) * (1 << lgb) * ncomp + (1 << lga) + (1 << lgb)) * sizeof(cplx); }
 size_t smem_fast_mid(int lga, int lgb, int lgC) {
     const int C0 = 1 << lgC, S2 = C0 * (1 << lga) + (C0 < 8 ? C0 : 0);
-    return (size_t)(S2 * (1 << lgb) + (1 << lga) + (1 << lgb)) * 16 + (size_t)((1 << lga) + (1 << lgb)) * 8;
+    return (size_t)(S2 * (1 << lgb) + (1 << lga) + (1 << lgb)) * sizeof(cplx) + (size_t)((1 << lga) + (1 << lgb)) * 8;
 }
 
 // fin: the last CTA also does S5 (no k_finalize launch)
@@ -313,7 +376,7 @@ void launch_fa_inv1(lgf_ctx* c) {
 template <int NC> void launch_fu_update(lgf_ctx* c) {
     LaunchScope ls(c, K_FU_UPDATE);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
-    const long long stride = (long long)(c->lay.link_buf / 16);
+    const long long stride = (long long)(c->lay.link_buf / sizeof(cplx));
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
         launch_k(c, k_fu_update_delta_fwd<A, B, NC, LGF_FU_NT>, grid, LGF_FU_NT, c->smem_fu, c->links, stride, c->gbuf, c->field, c->partials, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
@@ -368,8 +431,8 @@ lgf_status setup_fast(lgf_ctx* c) {
     c->smem_fa = c->smem_fc = c->smem_fu = smem_fast_plane(G.lg[0], G.lg[1], 4);
     c->smem_fb = smem_fast_mid(G.lg[2], G.lg[3], c->fb_lgC);
     // two tiles + one set of tables
-    c->smem_pa = 2 * c->smem_fa - (size_t)(G.L[0] + G.L[1]) * 16;
-    c->smem_pb = 2 * c->smem_fb - ((size_t)(G.L[2] + G.L[3]) * 16 + (size_t)(G.L[2] + G.L[3]) * 8);
+    c->smem_pa = 2 * c->smem_fa - (size_t)(G.L[0] + G.L[1]) * sizeof(cplx);
+    c->smem_pb = 2 * c->smem_fb - ((size_t)(G.L[2] + G.L[3]) * sizeof(cplx) + (size_t)(G.L[2] + G.L[3]) * 8);
     c->pp_b_ok = c->smem_pb <= (size_t)227 * 1024 && fast_pair(G.lg[2], G.lg[3]);
     if (c->fast_a) {
 #define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
@@ -402,7 +465,7 @@ lgf_status setup_fast(lgf_ctx* c) {
 lgf_status setup_kernels(lgf_ctx* c) {
     const Geom& G = c->G;
     const int nP = G.L[0] * G.L[1];
-    auto smem01 = [&](int ncomp) { return (size_t)((G.L[0] + 1) * G.L[1] * ncomp + G.L[0] + G.L[1]) * 16; };
+    auto smem01 = [&](int ncomp) { return (size_t)((G.L[0] + 1) * G.L[1] * ncomp + G.L[0] + G.L[1]) * sizeof(cplx); };
     c->fft01_ncomp_fused_ok = smem01(4) <= (size_t)MAX_SMEM;
     c->smem01_fused = smem01(4);
     int ncomp = 4;
@@ -420,7 +483,7 @@ lgf_status setup_kernels(lgf_ctx* c) {
     const int C0 = 1 << lgC;
     c->fft23_S1 = C0;
     c->fft23_S2 = C0 * G.L[2] + (C0 < 8 ? C0 : 0);
-    c->smem23 = (size_t)(c->fft23_S2 * G.L[3] + G.L[2] + G.L[3]) * 16 + (size_t)(G.L[2] + G.L[3]) * 8;
+    c->smem23 = (size_t)(c->fft23_S2 * G.L[3] + G.L[2] + G.L[3]) * sizeof(cplx) + (size_t)(G.L[2] + G.L[3]) * 8;
     if (c->smem23 > (size_t)MAX_SMEM || c->smem01 > (size_t)MAX_SMEM) return LGF_ERR_UNSUPPORTED;
     th = (n23 << lgC) / 8; if (th > 256) th = 256; if (th < 32) th = 32;
     c->fft23_threads = th;
@@ -437,7 +500,8 @@ lgf_status setup_kernels(lgf_ctx* c) {
 }
 
 lgf_status build_tables(lgf_ctx* c) {
-    std::vector<double> tw(4 * 128 * 2, 0.0), s(4 * 128, 0.0);
+    std::vector<real> tw(4 * 128 * 2, real(0));
+    std::vector<double> s(4 * 128, 0.0);
     for (int mu = 0; mu < 4; mu++) c->T.plan[mu] = make_plan(c->G.lg[mu], (mu & 1) != 0);
     const long double pi = 3.141592653589793238462643383279502884L;
     for (int mu = 0; mu < 4; mu++) {
@@ -446,7 +510,7 @@ lgf_status build_tables(lgf_ctx* c) {
             long double a = 2.0L * pi * (long double)k / (long double)L;
             double cr = (double)cosl(a), sr = (double)sinl(a);
             if ((4 * k) % L == 0) { const int q = 4 * k / L; const double cc[4] = {1, 0, -1, 0}, ss[4] = {0, 1, 0, -1}; cr = cc[q]; sr = ss[q]; }
-            tw[(mu * 128 + k) * 2] = cr; tw[(mu * 128 + k) * 2 + 1] = -sr;
+            tw[(mu * 128 + k) * 2] = (real)cr; tw[(mu * 128 + k) * 2 + 1] = (real)(-sr);
         }
         for (int p = 0; p < L; p++) {
             const int n = stored_freq(p, c->G.lg[mu], c->T.plan[mu]);
@@ -455,7 +519,7 @@ lgf_status build_tables(lgf_ctx* c) {
         }
     }
     char* tb = c->ws + c->lay.tables;
-    CK(cudaMemcpyAsync(tb, tw.data(), tw.size() * 8, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(tb, tw.data(), tw.size() * sizeof(real), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(tb + 4 * 128 * 16, s.data(), s.size() * 8, cudaMemcpyHostToDevice, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     for (int mu = 0; mu < 4; mu++) {
@@ -638,7 +702,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     if (p != LGF_FP64 && p != LGF_FP32) return LGF_ERR_INVALID_ARG;
     if (s != LGF_STORE_12 && s != LGF_STORE_18) return LGF_ERR_INVALID_ARG;
     for (int k = 0; k < 4; k++) if (dims[k] < 1) return LGF_ERR_INVALID_ARG;
-    if (p != LGF_FP64) return LGF_ERR_UNSUPPORTED;
+    if (p != LGF_THIS_PREC) return LGF_ERR_UNSUPPORTED;
     int lg[4];
     if (!dims_ok(dims, lg)) return LGF_ERR_UNSUPPORTED;
     int ndev = 0;
@@ -646,6 +710,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
 
     lgf_ctx* c = new (std::nothrow) lgf_ctx();
     if (!c) return LGF_ERR_OOM;
+    c->precision = (int)LGF_THIS_PREC;
     int shv = 0;
     for (int k = 0; k < 4; k++) { c->G.L[k] = dims[k]; c->G.lg[k] = lg[k]; c->G.sh[k] = shv; shv += lg[k]; }
     c->G.V = 1LL << shv;
@@ -672,7 +737,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->links = reinterpret_cast<cplx*>(c->ws + c->lay.links);
     c->field = reinterpret_cast<cplx*>(c->ws + c->lay.field);
     c->gbuf = reinterpret_cast<cplx*>(c->ws + c->lay.gbuf);
-    c->staging = reinterpret_cast<cplx*>(c->ws + c->lay.staging);
+    c->staging = reinterpret_cast<dcplx*>(c->ws + c->lay.staging);
     c->partials = reinterpret_cast<double2*>(c->ws + c->lay.partials);
     c->hist = reinterpret_cast<double2*>(c->ws + c->lay.hist);
     c->ctl = reinterpret_cast<Ctl*>(c->ws + c->lay.ctl);
@@ -693,11 +758,11 @@ lgf_status load_from_device_chunks(lgf_ctx* c, const double* src, bool src_is_ho
     c->parity = 0;          // a load fills link buffer 0
     for (long long off = 0; off < V; off += S) {
         const long long n = (V - off < S) ? V - off : S;
-        const cplx* aos;
+        const dcplx* aos;
         if (src_is_host) {
             CK(cudaMemcpyAsync(c->staging, src + off * 72, (size_t)n * 576, cudaMemcpyHostToDevice, c->stream));
             aos = c->staging;
-        } else aos = reinterpret_cast<const cplx*>(src) + off * 36;
+        } else aos = reinterpret_cast<const dcplx*>(src) + off * 36;
         {
             LaunchScope ls(c, K_LAYOUT_IN);
             const unsigned grid = (unsigned)((n * 4 + 255) / 256);
@@ -715,7 +780,7 @@ lgf_status get_to_chunks(lgf_ctx* c, double* dst, bool dst_is_host) {
     const long long V = c->G.V, S = c->lay.stage_sites;
     for (long long off = 0; off < V; off += S) {
         const long long n = (V - off < S) ? V - off : S;
-        cplx* aos = dst_is_host ? c->staging : reinterpret_cast<cplx*>(dst) + off * 36;
+        dcplx* aos = dst_is_host ? c->staging : reinterpret_cast<dcplx*>(dst) + off * 36;
         {
             LaunchScope ls(c, K_LAYOUT_OUT);
             const unsigned grid = (unsigned)((n * 4 + 255) / 256);
@@ -735,18 +800,28 @@ extern "C" {
 
 size_t lgf_workspace_bytes(const int dims[4], lgf_precision p, lgf_storage s) {
     int lg[4];
-    if (!dims || p != LGF_FP64 || (s != LGF_STORE_12 && s != LGF_STORE_18) || !dims_ok(dims, lg)) return 0;
+#ifndef LGF_F32
+    if (p == LGF_FP32) return lgf32_workspace_bytes(dims, p, s);
+#endif
+    if (!dims || p != LGF_THIS_PREC || (s != LGF_STORE_12 && s != LGF_STORE_18) || !dims_ok(dims, lg)) return 0;
     return make_layout(dims, s == LGF_STORE_12 ? 6 : 9).total;
 }
 
 lgf_status lgf_create(const int dims[4], lgf_precision p, lgf_storage s, lgf_ctx** out) {
+#ifndef LGF_F32
+    if (p == LGF_FP32) return lgf32_create(dims, p, s, out);
+#endif
     return create_impl(dims, p, s, nullptr, 0, nullptr, true, out);
 }
 lgf_status lgf_create_ex(const int dims[4], lgf_precision p, lgf_storage s, void* ws, size_t bytes, void* stream, lgf_ctx** out) {
+#ifndef LGF_F32
+    if (p == LGF_FP32) return lgf32_create_ex(dims, p, s, ws, bytes, stream, out);
+#endif
     return create_impl(dims, p, s, ws, bytes, stream, false, out);
 }
 
 void lgf_destroy(lgf_ctx* c) {
+    FWD32V(lgf32_destroy(c))
     if (!c) return;
     if (c->stream) cudaStreamSynchronize(c->stream);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
@@ -760,25 +835,30 @@ void lgf_destroy(lgf_ctx* c) {
 }
 
 lgf_status lgf_load_links(lgf_ctx* c, const double* host_links) {
+    FWD32(lgf32_load_links(c, host_links))
     if (!c || !host_links) return LGF_ERR_INVALID_ARG;
     return load_from_device_chunks(c, host_links, true);
 }
 lgf_status lgf_load_links_device(lgf_ctx* c, const double* dev_links) {
+    FWD32(lgf32_load_links_device(c, dev_links))
     if (!c || !dev_links) return LGF_ERR_INVALID_ARG;
     return load_from_device_chunks(c, dev_links, false);
 }
 lgf_status lgf_get_links(lgf_ctx* c, double* host_links) {
+    FWD32(lgf32_get_links(c, host_links))
     if (!c || !host_links) return LGF_ERR_INVALID_ARG;
     if (!c->loaded) return LGF_ERR_NOT_LOADED;
     return get_to_chunks(c, host_links, true);
 }
 lgf_status lgf_get_links_device(lgf_ctx* c, double* dev_links) {
+    FWD32(lgf32_get_links_device(c, dev_links))
     if (!c || !dev_links) return LGF_ERR_INVALID_ARG;
     if (!c->loaded) return LGF_ERR_NOT_LOADED;
     return get_to_chunks(c, dev_links, false);
 }
 
 lgf_status lgf_iterate(lgf_ctx* c, int n, double alpha, double* F, double* theta) {
+    FWD32(lgf32_iterate(c, n, alpha, F, theta))
     if (!c || n < 0 || !(alpha > 0.0) || !std::isfinite(alpha)) return LGF_ERR_INVALID_ARG;
     if (!c->loaded) return LGF_ERR_NOT_LOADED;
     lgf_status st = run(c, alpha, -1.0, n, false);
@@ -789,6 +869,7 @@ lgf_status lgf_iterate(lgf_ctx* c, int n, double alpha, double* F, double* theta
 }
 
 lgf_status lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int* n_iter, double* F, double* theta) {
+    FWD32(lgf32_fix(c, alpha, theta_tol, max_iter, n_iter, F, theta))
     if (!c || max_iter < 0 || !(alpha > 0.0) || !std::isfinite(alpha) || !(theta_tol >= 0.0)) return LGF_ERR_INVALID_ARG;
     if (!c->loaded) return LGF_ERR_NOT_LOADED;
     lgf_status st = run(c, alpha, theta_tol, max_iter, true);
@@ -800,6 +881,7 @@ lgf_status lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int
 }
 
 lgf_status lgf_measure(lgf_ctx* c, double* F, double* theta, double* plaq) {
+    FWD32(lgf32_measure(c, F, theta, plaq))
     if (!c) return LGF_ERR_INVALID_ARG;
     if (!c->loaded) return LGF_ERR_NOT_LOADED;
     lgf_status st = reset_ctl(c, -1.0, 0);
@@ -829,6 +911,7 @@ lgf_status lgf_measure(lgf_ctx* c, double* F, double* theta, double* plaq) {
 }
 
 lgf_status lgf_get_history(lgf_ctx* c, double* hist, int capacity, int* n_out) {
+    FWD32(lgf32_get_history(c, hist, capacity, n_out))
     if (!c || !hist || capacity < 0 || !n_out) return LGF_ERR_INVALID_ARG;
     int n = c->h_ctl->n_meas; if (n > HIST_CAP) n = HIST_CAP; if (n > capacity) n = capacity;
     if (n > 0) {
@@ -840,6 +923,7 @@ lgf_status lgf_get_history(lgf_ctx* c, double* hist, int capacity, int* n_out) {
 }
 
 lgf_status lgf_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host_field) {
+    FWD32(lgf32_get_field(c, which, alpha, host_field))
     if (!c || !host_field) return LGF_ERR_INVALID_ARG;
     if (which != LGF_FIELD_DELTA && which != LGF_FIELD_X && which != LGF_FIELD_G) return LGF_ERR_INVALID_ARG;
     if (!c->loaded) return LGF_ERR_NOT_LOADED;
@@ -874,6 +958,7 @@ lgf_status lgf_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host
 }
 
 lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
+    FWD32(lgf32_set_option(c, opt, value))
     if (!c) return LGF_ERR_INVALID_ARG;
     switch (opt) {
         case LGF_OPT_FUSE_DELTA_FFT: c->opt_fuse = value ? 1 : 0; break;
@@ -892,6 +977,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
     return LGF_OK;
 }
 lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
+    FWD32(lgf32_get_option(c, opt, value))
     if (!c || !value) return LGF_ERR_INVALID_ARG;
     switch (opt) {
         case LGF_OPT_FUSE_DELTA_FFT: *value = use_fused(c); break;
@@ -911,6 +997,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
 }
 
 lgf_status lgf_set_profiling(lgf_ctx* c, int on) {
+    FWD32(lgf32_set_profiling(c, on))
     if (!c) return LGF_ERR_INVALID_ARG;
     prof_flush(c);
     c->profiling = on ? 1 : 0;
@@ -918,14 +1005,21 @@ lgf_status lgf_set_profiling(lgf_ctx* c, int on) {
     return LGF_OK;
 }
 lgf_status lgf_get_profile(lgf_ctx* c, double ms[LGF_MAX_KERNELS], long long n[LGF_MAX_KERNELS]) {
+    FWD32(lgf32_get_profile(c, ms, n))
     if (!c || !ms || !n) return LGF_ERR_INVALID_ARG;
     prof_flush(c);
     memcpy(ms, c->prof_ms, sizeof c->prof_ms); memcpy(n, c->prof_n, sizeof c->prof_n);
     return LGF_OK;
 }
+#ifndef LGF_F32
 const char* lgf_kernel_name(int slot) { return (slot >= 0 && slot < LGF_MAX_KERNELS) ? kKernelNames[slot] : ""; }
-long long lgf_launch_count(lgf_ctx* c) { return c ? c->launches : 0; }
+#endif
+long long lgf_launch_count(lgf_ctx* c) {
+    FWD32(lgf32_launch_count(c))
+    return c ? c->launches : 0;
+}
 
+#ifndef LGF_F32
 lgf_status lgf_copy_peak(void* dst, const void* src, size_t bytes, int reps, void* stream, double* ms) {
     if (!dst || !src || !ms || reps < 1 || bytes < 16 || (bytes & 15)) return LGF_ERR_INVALID_ARG;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -981,6 +1075,10 @@ const char* lgf_status_string(lgf_status s) {
     }
     return "unknown status";
 }
-const char* lgf_last_error(lgf_ctx* c) { return c ? c->err.c_str() : ""; }
+#endif
+const char* lgf_last_error(lgf_ctx* c) {
+    FWD32(lgf32_last_error(c))
+    return c ? c->err.c_str() : "";
+}
 
 }  // extern "C"

@@ -1,18 +1,28 @@
 // su3.cuh -- register-level complex 3x3 algebra for the gauge-fixing kernels (fp64, sm_100a).
 // Complex numbers are double2 (x = re, y = im).  Everything is __forceinline__ so that unused rows
 // and entries are dead-code eliminated in each kernel.
+// Precision: the translation unit defines LGF_F32 for the fp32 build (real = float, cplx = float2, namespace renamed by
+// "#define lgf lgf32" in lgf_api.cu); default fp64.  Sums over the lattice (theta, F) and the p^2 filter weights stay
+// double in both builds.
 #pragma once
 #include <cuda_runtime.h>
 
 namespace lgf {
 
+#ifdef LGF_F32
+typedef float real;
+typedef float2 cplx;
+#else
+typedef double real;
 typedef double2 cplx;
+#endif
+typedef double2 dcplx;      // host-facing complex (the C ABI speaks double in every precision)
 
-__device__ __forceinline__ cplx mk(double a, double b) { return make_double2(a, b); }
+__device__ __forceinline__ cplx mk(real a, real b) { cplx r; r.x = a; r.y = b; return r; }
 __device__ __forceinline__ cplx cadd(cplx a, cplx b) { return mk(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ cplx csub(cplx a, cplx b) { return mk(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ cplx cconj(cplx a) { return mk(a.x, -a.y); }
-__device__ __forceinline__ cplx cscale(cplx a, double s) { return mk(a.x * s, a.y * s); }
+__device__ __forceinline__ cplx cscale(cplx a, real s) { return mk(a.x * s, a.y * s); }
 __device__ __forceinline__ cplx cmul(cplx a, cplx b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 // a * conj(b)
 __device__ __forceinline__ cplx cmulc(cplx a, cplx b) { return mk(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }
@@ -30,7 +40,7 @@ __device__ __forceinline__ cplx cfmac(cplx a, cplx b, cplx c) {
 __device__ __forceinline__ cplx cfnma(cplx a, cplx b, cplx c) {
     return mk(fma(-a.x, b.x, fma(a.y, b.y, c.x)), fma(-a.x, b.y, fma(-a.y, b.x, c.y)));
 }
-__device__ __forceinline__ double cnorm2(cplx a) { return fma(a.x, a.x, a.y * a.y); }
+__device__ __forceinline__ real cnorm2(cplx a) { return fma(a.x, a.x, a.y * a.y); }
 
 // Row 2 of a special unitary matrix from rows 0,1: row2 = conj(row0 x row1)  ("12 real
 // number representation").  u[0..2] = row 0, u[3..5] = row 1, u[6..8] = row 2.
@@ -49,12 +59,17 @@ __device__ __forceinline__ cplx ldg2(const cplx* p) { return __ldg(p); }
 #ifndef LGF_L2HINT
 #define LGF_L2HINT 0
 #endif
+#ifdef LGF_F32
+#undef LGF_L2HINT
+#define LGF_L2HINT 0        // the hinted accesses below are written for 16-byte complex
+#endif
 __device__ __forceinline__ unsigned long long l2_policy_last() {
     unsigned long long p; asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
 }
 __device__ __forceinline__ unsigned long long l2_policy_first() {
     unsigned long long p; asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
 }
+#ifndef LGF_F32
 __device__ __forceinline__ cplx ld_hint(const cplx* p, unsigned long long pol) {
     cplx v; asm volatile("ld.global.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol)); return v;
 }
@@ -64,6 +79,11 @@ __device__ __forceinline__ cplx ldnc_hint(const cplx* p, unsigned long long pol)
 __device__ __forceinline__ void st_hint(cplx* p, cplx v, unsigned long long pol) {
     asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
 }
+#else
+__device__ __forceinline__ cplx ld_hint(const cplx* p, unsigned long long) { return *p; }
+__device__ __forceinline__ cplx ldnc_hint(const cplx* p, unsigned long long) { return __ldg(p); }
+__device__ __forceinline__ void st_hint(cplx* p, cplx v, unsigned long long) { *p = v; }
+#endif
 // field (Delta~ / X~ / X) accesses: ld_field where the same kernel later overwrites the location (plain load),
 // ldc_field where the field is read-only for the kernel (non-coherent path)
 __device__ __forceinline__ cplx ld_field(const cplx* p) {
@@ -110,19 +130,19 @@ __device__ __forceinline__ void store_link(cplx* __restrict__ links, long long V
 // S3: g = rowGramSchmidt(M), M = 1 + (alpha/2) X, X given by its packed independent components
 //   f0 = X01, f1 = X02, f2 = X12, f3 = (Im X00, Im X11);  X_ji = -conj(X_ij), X anti-Hermitian traceless.
 // Only rows 0 and 1 of M enter; row 2 of g is conj(u x v).  ha = alpha/2.   [north_star step 3]
-__device__ __forceinline__ void build_g(cplx f0, cplx f1, cplx f2, cplx f3, double ha, cplx (&g)[9]) {
-    cplx m00 = mk(1.0, ha * f3.x), m01 = cscale(f0, ha), m02 = cscale(f1, ha);
-    cplx m10 = mk(-ha * f0.x, ha * f0.y), m11 = mk(1.0, ha * f3.y), m12 = cscale(f2, ha);
-    double n0 = cnorm2(m00) + cnorm2(m01) + cnorm2(m02);
-    double r0 = 1.0 / sqrt(n0);
+__device__ __forceinline__ void build_g(cplx f0, cplx f1, cplx f2, cplx f3, real ha, cplx (&g)[9]) {
+    cplx m00 = mk(real(1), ha * f3.x), m01 = cscale(f0, ha), m02 = cscale(f1, ha);
+    cplx m10 = mk(-ha * f0.x, ha * f0.y), m11 = mk(real(1), ha * f3.y), m12 = cscale(f2, ha);
+    real n0 = cnorm2(m00) + cnorm2(m01) + cnorm2(m02);
+    real r0 = real(1) / sqrt(n0);
     g[0] = cscale(m00, r0); g[1] = cscale(m01, r0); g[2] = cscale(m02, r0);
     // <u, M1> = sum_j conj(u_j) M1_j
     cplx ip = ccmul(g[0], m10);
     ip = cadd(ip, ccmul(g[1], m11));
     ip = cadd(ip, ccmul(g[2], m12));
     cplx v0 = cfnma(ip, g[0], m10), v1 = cfnma(ip, g[1], m11), v2 = cfnma(ip, g[2], m12);
-    double n1 = cnorm2(v0) + cnorm2(v1) + cnorm2(v2);
-    double r1 = 1.0 / sqrt(n1);
+    real n1 = cnorm2(v0) + cnorm2(v1) + cnorm2(v2);
+    real r1 = real(1) / sqrt(n1);
     g[3] = cscale(v0, r1); g[4] = cscale(v1, r1); g[5] = cscale(v2, r1);
     third_row(g);
 }

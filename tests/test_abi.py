@@ -47,10 +47,13 @@ def test_workspace_bytes_and_supported_sizes():
     assert L.lgf_workspace_bytes(d(64, 64, 64, 64), lgf.LGF_FP64, lgf.LGF_STORE_12) >= 64 ** 4 * 448
     assert L.lgf_workspace_bytes(d(32, 32, 32, 64), lgf.LGF_FP64, lgf.LGF_STORE_12) > 0
     assert L.lgf_workspace_bytes(d(8, 8, 8, 8), lgf.LGF_FP64, lgf.LGF_STORE_18) > 0
-    # unsupported: non power of two, too small, fp32 (not built), bad storage
+    # fp32 (LGF_FP32): half the link and field bytes
+    n12f = L.lgf_workspace_bytes(d(32, 32, 32, 32), lgf.LGF_FP32, lgf.LGF_STORE_12)
+    assert V * (2 * 192 + 32) <= n12f < n12 - V * 384
+    # unsupported: non power of two, too small, bad precision, bad storage
     assert L.lgf_workspace_bytes(d(12, 8, 8, 8), lgf.LGF_FP64, lgf.LGF_STORE_12) == 0
     assert L.lgf_workspace_bytes(d(2, 8, 8, 8), lgf.LGF_FP64, lgf.LGF_STORE_12) == 0
-    assert L.lgf_workspace_bytes(d(8, 8, 8, 8), lgf.LGF_FP32, lgf.LGF_STORE_12) == 0
+    assert L.lgf_workspace_bytes(d(8, 8, 8, 8), 7, lgf.LGF_STORE_12) == 0
     assert L.lgf_workspace_bytes(d(8, 8, 8, 8), lgf.LGF_FP64, 10) == 0
 
 
@@ -61,7 +64,10 @@ def test_argument_errors_before_any_device_work():
     assert L.lgf_create(None, 0, 12, C.byref(h)) == lgf.LGF_ERR_INVALID_ARG
     assert L.lgf_create(d, 7, 12, C.byref(h)) == lgf.LGF_ERR_INVALID_ARG
     assert L.lgf_create(d, 0, 13, C.byref(h)) == lgf.LGF_ERR_INVALID_ARG
-    assert L.lgf_create(d, lgf.LGF_FP32, 12, C.byref(h)) == lgf.LGF_ERR_UNSUPPORTED
+    st = L.lgf_create(d, lgf.LGF_FP32, 12, C.byref(h))            # fp32 is built: only the missing device can refuse it
+    assert st in (lgf.LGF_ERR_CUDA, lgf.LGF_OK)
+    if st == lgf.LGF_OK:
+        L.lgf_destroy(h)
     bad = (C.c_int * 4)(8, 8, 6, 8)
     assert L.lgf_create(bad, 0, 12, C.byref(h)) == lgf.LGF_ERR_UNSUPPORTED
     neg = (C.c_int * 4)(8, 8, -1, 8)

@@ -349,6 +349,66 @@ def test_plain_steepest_descent_variant(dims, storage):
     assert th < href[-1, 1]                                              # Fourier acceleration converges faster
 
 
+# ------------------------------------------------------------------ fp32
+EPS32 = 2.0 ** -24      # fp32 unit round-off
+
+
+@pytest.mark.parametrize("dims,storage", [((8, 8, 8, 8), 18), ((16, 16, 16, 16), 12), ((32, 16, 16, 32), 12), ((4, 8, 16, 4), 12),
+                                          ((64, 64, 4, 4), 12), ((8, 4, 32, 64), 12)])
+def test_fp32_stage_and_trajectory_against_the_fp64_oracle(dims, storage):
+    """LGF_FP32: same kernels instantiated for float storage and arithmetic, lattice sums in double.  The oracle stays
+    fp64 (it is the definition); the bounds are fp32 round-off times the operation counts of DESIGN.md section 7:
+    Delta (16 link terms) 8 eps, X (FFT of log2 V stages, filter <= p2max/p2min) 32 eps, g 32 eps, all relative to the
+    field maximum; F (a mean of O(1) terms, summed in double) 16 eps; links after k iterations 64 k eps."""
+    U = E.noisy(dims, 43, 0.35)
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    o.load(U)
+    D_ref, X_ref, g_ref = o.delta(), o.fa_field(), o.g_field(ALPHA)
+    F_ref, th_ref = o.measure()
+    r = o.fix(ALPHA, 0.0, 10, history=True)
+    href = np.array(r["history"])
+    U10 = o.get()
+    gf = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_FP32)
+    for v in [(1, 0, 1, 1, 0), (0, 0, 0, 0, 0, 0, 0, 0), (1, 1, 1, 1, 0), (1, 0, 1, 1, 0, 7)]:
+        set_variant(gf, v)
+        gf.load_links(U)
+        F, th, _ = gf.measure()
+        assert abs(F - F_ref) <= 16 * EPS32 and abs(th - th_ref) <= 16 * EPS32 * th_ref, v
+        assert np.abs(gf.get_field(lgf.LGF_FIELD_DELTA) - D_ref).max() <= 8 * EPS32 * np.abs(D_ref).max(), v
+        assert np.abs(gf.get_field(lgf.LGF_FIELD_X) - X_ref).max() <= 32 * EPS32 * np.abs(X_ref).max(), v
+        assert np.abs(gf.get_field(lgf.LGF_FIELD_G, ALPHA) - g_ref).max() <= 32 * EPS32, v
+        got = gf.get_links()
+        assert np.abs(got[:, :, :2] - U[:, :, :2]).max() <= EPS32, v          # stored as float: one rounding
+        F10, th10 = gf.iterate(10, ALPHA)
+        h = gf.get_history()
+        assert np.abs(h[:, 0] - href[:, 0]).max() <= 16 * EPS32, v
+        assert np.all(np.abs(h[:, 1] - href[:, 1]) <= 64 * EPS32 * href[:, 1]), v
+        assert np.abs(gf.get_links() - U10).max() <= 64 * 10 * EPS32, v
+
+
+def test_fp32_converges_to_its_rounding_floor_and_keeps_invariants():
+    """C1 in fp32: theta < 1e-10 is reached in the oracle's iteration count for that tolerance (+-1: the trajectories
+    differ at fp32 round-off), theta < 1e-15 is not reachable (floor ~1e-14: LGF_NOT_CONVERGED), F agrees with the fp64
+    fixed point to fp32 accuracy, the plaquette is invariant and the links stay unitary to fp32 accuracy."""
+    U, cfg = E.make_config("C1")
+    dims, storage = cfg["dims"], cfg["storage"]
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    o.load(U)
+    r_ref = o.fix(ALPHA, 1e-10, 1000)
+    gf = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_FP32)
+    gf.load_links(U)
+    _, _, plaq0 = gf.measure()
+    r = gf.fix(ALPHA, 1e-10, 1000)
+    assert r["status"] == lgf.LGF_OK and abs(r["n_iter"] - r_ref["n_iter"]) <= 1 and r["theta"] < 1e-10
+    assert abs(r["F"] - r_ref["F"]) <= 64 * EPS32
+    _, _, plaq1 = gf.measure()
+    assert abs(plaq1 - plaq0) <= 64 * EPS32
+    L = gf.get_links()
+    assert np.abs(np.einsum("xmij,xmkj->xmik", L, L.conj()) - np.eye(3)).max() <= 64 * r["n_iter"] * EPS32
+    r = gf.fix(ALPHA, TOL, 200)
+    assert r["status"] == lgf.LGF_NOT_CONVERGED and 1e-16 < r["theta"] < 1e-12
+
+
 def test_C1_ten_iterations_against_the_naive_dft_oracle():
     U, cfg = E.make_config("C1")
     o = oracle.Oracle(cfg["dims"], cfg["storage"], fft_mode=0)      # the definition
