@@ -314,6 +314,25 @@ def run_ours(args):
         torch.cuda.synchronize()
         ttt = {"ms": (time.perf_counter() - t0) * 1e3, "n_iter": r["n_iter"], "status": r["status"], "F": r["F"],
                "theta": r["theta"], "theta_tol": 1e-10 if fp32 else THETA_TOL, "plaquette": plaq, "ensemble": args.workload}
+        # ---- the same with LGF_MIXED (fp32 phase + fp64 polish), fp64 workloads only
+        if not fp32:
+            try:
+                gm = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_MIXED)
+                for _ in range(2):                       # first call: graph capture of both precisions
+                    if device_links:
+                        gm.load_links_device(d_in.data_ptr())
+                    else:
+                        gm.load_links(h_in.numpy())
+                    torch.cuda.synchronize()
+                    t0 = time.perf_counter()
+                    rm = gm.fix(ALPHA, THETA_TOL, 100000)
+                    torch.cuda.synchronize()
+                    tm = (time.perf_counter() - t0) * 1e3
+                ttt["mixed"] = {"ms": tm, "n_iter": rm["n_iter"], "fp32_iters": gm.get_option(lgf.LGF_OPT_MIXED_FP32_ITERS),
+                                "status": rm["status"], "F": rm["F"], "theta": rm["theta"]}
+                gm.destroy()
+            except Exception as e:                       # reported, never fatal for the headline number
+                ttt["mixed"] = {"error": str(e)}
         # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample
         cpu = None
         if world == 1 and not args.no_cpu_baseline and not device_links:

@@ -56,8 +56,14 @@ typedef enum {
  * LGF_FP32: links and field stored as float, every kernel computes in float; the
  * lattice sums (theta, F) and the p^2 filter weights stay double.  Half the HBM bytes per iteration; theta bottoms out
  * near 1e-12 (fp32 rounding of Delta), so theta < 1e-15 is not reachable in this precision alone.  Host- and
- * device-side link and field arrays of this API are double in every precision (converted on load and on get). */
-typedef enum { LGF_FP64 = 0, LGF_FP32 = 1 } lgf_precision;
+ * device-side link and field arrays of this API are double in every precision (converted on load and on get).
+ * LGF_MIXED: an fp64 context (everything above holds: fp64 links, fp64 lgf_iterate) whose lgf_fix runs in two phases:
+ * a float copy of the links is fixed in fp32 down to theta = max(theta_tol, 1e-12) while the update accumulates the
+ * total gauge transformation G(x); then the fp64 links receive U_mu(x) <- G(x) U_mu(x) G(x+mu)^dagger with G
+ * re-orthonormalised in double -- an exact gauge copy of the input, at the fp32 noise level of theta -- and the fp64
+ * iteration continues to theta_tol.  n_iter is the total; lgf_get_option(LGF_OPT_MIXED_FP32_ITERS) gives the fp32
+ * share; lgf_get_history covers the fp64 phase.  Needs the workspaces of both precisions. */
+typedef enum { LGF_FP64 = 0, LGF_FP32 = 1, LGF_MIXED = 2 } lgf_precision;
 typedef enum { LGF_STORE_18 = 18, LGF_STORE_12 = 12 } lgf_storage;
 
 /* Bytes of device workspace a context for these parameters needs (0 if the parameters are unsupported). */
@@ -146,7 +152,8 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *                           with a rate that degrades with the volume (critical slowing down). */
 typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
                LGF_OPT_FUSE_UPDATE = 5, LGF_OPT_PINGPONG = 6, LGF_OPT_FUSE_FINALIZE = 7,
-               LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9, LGF_OPT_FOURIER_ACCEL = 10 } lgf_option;
+               LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9, LGF_OPT_FOURIER_ACCEL = 10,
+               LGF_OPT_MIXED_FP32_ITERS = 11 /* read-only */ } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

@@ -326,9 +326,11 @@ __global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __res
 #ifndef LGF_UPDQ_MINB
 #define LGF_UPDQ_MINB 5
 #endif
-template <int NC, int NS>      // NS = sites per CTA = max(32, L0): 4 * NS threads, thread = (mu, site)
+// ACC: the mu = 1 thread of each site also accumulates the total gauge transformation, Gacc(x) <- g(x) Gacc(x)
+// (rows 0,1 in gacc, 6 V-arrays; mixed precision, lgf_api.cu): +2 x 6 complex per site.
+template <int NC, int NS, int ACC = 0>      // NS = sites per CTA = max(32, L0): 4 * NS threads, thread = (mu, site)
 __global__ void __launch_bounds__(4 * NS, (NS == 32) ? LGF_UPDQ_MINB : ((NS == 64) ? LGF_UPDQ_MINB64 : 1)) k_update_quad(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G,
-                                                                                       double half_alpha, Ctl* ctl) {
+                                                                                       double half_alpha, Ctl* ctl, cplx* __restrict__ gacc = nullptr) {
     pdl_enter();
     if (ctl->done) return;
     __shared__ cplx sg[9][NS];
@@ -350,8 +352,67 @@ __global__ void __launch_bounds__(4 * NS, (NS == 32) ? LGF_UPDQ_MINB : ((NS == 6
     for (int c = 0; c < 9; c++) g[c] = sg[c][st];
     rotate_link<(NC == 6) ? 2 : 3>(g, u, gp, r);
     store_link<NC>(links, V, mu, x, r);
+    if (ACC && mu == 1) {
+        cplx a[9];
+#pragma unroll
+        for (int c = 0; c < 6; c++) a[c] = gacc[(long long)c * V + x];
+        third_row(a);
+#pragma unroll
+        for (int i = 0; i < 2; i++)
+#pragma unroll
+            for (int j = 0; j < 3; j++) {
+                cplx t = cmul(g[3 * i], a[j]);
+                t = cfma(g[3 * i + 1], a[3 + j], t);
+                t = cfma(g[3 * i + 2], a[6 + j], t);
+                gacc[(long long)(3 * i + j) * V + x] = t;
+            }
+    }
     if (x == 0 && mu == 0) ctl->iters = ctl->iters + 1;
 }
+
+// Gacc(x) = 1 (rows 0,1)
+__global__ void __launch_bounds__(256) k_init_gacc(cplx* __restrict__ gacc, long long V) {
+    const long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (x >= V) return;
+#pragma unroll
+    for (int c = 0; c < 6; c++) gacc[(long long)c * V + x] = mk((c == 0 || c == 4) ? real(1) : real(0), real(0));
+}
+
+#ifndef LGF_F32
+// ---- mixed precision (fp64 build only): the fp32 shadow context works on a float copy of the links and accumulates
+// the gauge transformation; the fp64 links then receive it in one step, U_mu(x) <- G(x) U_mu(x) G(x+mu)^dagger, with G
+// re-orthonormalised in double, so the result is an exact (to fp64 rounding) gauge copy of the fp64 input.
+__global__ void __launch_bounds__(256) k_demote(const double2* __restrict__ src, float2* __restrict__ dst, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { const double2 v = __ldg(src + i); dst[i] = make_float2((float)v.x, (float)v.y); }
+}
+__device__ __forceinline__ void load_gacc64(const float2* __restrict__ gacc, long long V, long long x, cplx (&g)[9]) {
+    cplx m[6];
+#pragma unroll
+    for (int c = 0; c < 6; c++) { const float2 v = __ldg(gacc + (long long)c * V + x); m[c] = mk((double)v.x, (double)v.y); }
+    // row Gram-Schmidt in double (the same projection as S3), third row = conj(u x v)
+    const double r0 = 1.0 / sqrt(cnorm2(m[0]) + cnorm2(m[1]) + cnorm2(m[2]));
+    g[0] = cscale(m[0], r0); g[1] = cscale(m[1], r0); g[2] = cscale(m[2], r0);
+    cplx ip = ccmul(g[0], m[3]);
+    ip = cadd(ip, ccmul(g[1], m[4]));
+    ip = cadd(ip, ccmul(g[2], m[5]));
+    const cplx v0 = cfnma(ip, g[0], m[3]), v1 = cfnma(ip, g[1], m[4]), v2 = cfnma(ip, g[2], m[5]);
+    const double r1 = 1.0 / sqrt(cnorm2(v0) + cnorm2(v1) + cnorm2(v2));
+    g[3] = cscale(v0, r1); g[4] = cscale(v1, r1); g[5] = cscale(v2, r1);
+    third_row(g);
+}
+template <int NC>
+__global__ void __launch_bounds__(128) k_apply_gacc(cplx* __restrict__ links, const float2* __restrict__ gacc, Geom G) {
+    const int mu = blockIdx.x & 3;
+    const long long x = (long long)(blockIdx.x >> 2) * 128 + threadIdx.x;
+    cplx g[9], gp[9], u[9], r[9];
+    load_link<NC>(links, G.V, mu, x, u);
+    load_gacc64(gacc, G.V, x, g);
+    load_gacc64(gacc, G.V, fwd(G, x, mu), gp);
+    rotate_link<(NC == 6) ? 2 : 3>(g, u, gp, r);
+    store_link<NC>(links, G.V, mu, x, r);
+}
+#endif
 
 // ------------------------------------------------------------------------------------------------ boundary helpers
 // canonical [x][mu][3][3] complex (array of structs) -> structure of arrays; one thread per (x, mu)

@@ -57,6 +57,10 @@ lgf_status lgf32_set_profiling(lgf_ctx* c, int on);
 lgf_status lgf32_get_profile(lgf_ctx* c, double ms[LGF_MAX_KERNELS], long long n[LGF_MAX_KERNELS]);
 long long lgf32_launch_count(lgf_ctx* c);
 const char* lgf32_last_error(lgf_ctx* c);
+// mixed precision (internal, not in lgf.h): start an fp32 phase on links the caller writes to the returned device
+// buffer (float2 SoA, same order as the fp64 store) with the accumulated transformation reset to 1; and read it back
+void* lgf32_x_begin(lgf_ctx* c);
+void* lgf32_x_gacc(lgf_ctx* c);
 }
 // forward to the fp32 twin when the context is an fp32 one (the precision is the first member of both context types)
 #define FWD32(call) if (c && *reinterpret_cast<const int*>(c) == (int)LGF_FP32) return call;
@@ -179,6 +183,11 @@ struct lgf_ctx {
     FftTables T;
     Ctl* h_ctl;             // pinned
     bool loaded;
+    // mixed precision: the fp64 context owns an fp32 shadow context (same stream); the fp32 context accumulates G
+    lgf_ctx* shadow;        // fp64 build: opaque fp32 context, or nullptr
+    char* shadow_ws;        // its workspace when this context allocated it
+    int acc_g;              // fp32 build: the update also accumulates Gacc(x) <- g(x) Gacc(x) in gbuf
+    int mixed_n32;          // fp32 iterations of the last mixed lgf_fix
     // options
     int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel;
     int sms;                // SMs of the device: grid of the persistent passes
@@ -555,9 +564,15 @@ void launch_finalize(lgf_ctx* c, int n_partials, int advance = 0) {
 template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
     if (!SG && c->opt_quad) {
         LaunchScope ls(c, K_UPDATE_QUAD);
-        if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32>, (unsigned)(c->G.V / 32), 128, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl);
-        else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64>, (unsigned)(c->G.V / 64), 256, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl);
-        else launch_k(c, k_update_quad<NC, 128>, (unsigned)(c->G.V / 128), 512, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl);
+        cplx* const no_acc = nullptr;
+        if (c->acc_g) {
+            if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32, 1>, (unsigned)(c->G.V / 32), 128, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, c->gbuf);
+            else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64, 1>, (unsigned)(c->G.V / 64), 256, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, c->gbuf);
+            else launch_k(c, k_update_quad<NC, 128, 1>, (unsigned)(c->G.V / 128), 512, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, c->gbuf);
+        }
+        else if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32>, (unsigned)(c->G.V / 32), 128, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, no_acc);
+        else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64>, (unsigned)(c->G.V / 64), 256, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, no_acc);
+        else launch_k(c, k_update_quad<NC, 128>, (unsigned)(c->G.V / 128), 512, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, no_acc);
         return;
     }
     LaunchScope ls(c, SG ? K_UPDATE_G : K_UPDATE_X);
@@ -649,7 +664,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -699,7 +714,7 @@ lgf_status run(lgf_ctx* c, double alpha, double tol, int max_iter, bool poll) {
 lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* wsp, size_t ws_bytes, void* stream, bool own, lgf_ctx** out) {
     if (!dims || !out) return LGF_ERR_INVALID_ARG;
     *out = nullptr;
-    if (p != LGF_FP64 && p != LGF_FP32) return LGF_ERR_INVALID_ARG;
+    if (p != LGF_FP64 && p != LGF_FP32 && p != LGF_MIXED) return LGF_ERR_INVALID_ARG;
     if (s != LGF_STORE_12 && s != LGF_STORE_18) return LGF_ERR_INVALID_ARG;
     for (int k = 0; k < 4; k++) if (dims[k] < 1) return LGF_ERR_INVALID_ARG;
     if (p != LGF_THIS_PREC) return LGF_ERR_UNSUPPORTED;
@@ -721,6 +736,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
+    c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0;
     c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
     c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
@@ -802,20 +818,53 @@ size_t lgf_workspace_bytes(const int dims[4], lgf_precision p, lgf_storage s) {
     int lg[4];
 #ifndef LGF_F32
     if (p == LGF_FP32) return lgf32_workspace_bytes(dims, p, s);
+    if (p == LGF_MIXED) {
+        const size_t n64 = lgf_workspace_bytes(dims, LGF_FP64, s), n32 = lgf32_workspace_bytes(dims, LGF_FP32, s);
+        return (n64 && n32) ? align_up(n64, 256) + n32 : 0;
+    }
 #endif
     if (!dims || p != LGF_THIS_PREC || (s != LGF_STORE_12 && s != LGF_STORE_18) || !dims_ok(dims, lg)) return 0;
     return make_layout(dims, s == LGF_STORE_12 ? 6 : 9).total;
 }
 
+#ifndef LGF_F32
+// LGF_MIXED: an fp64 context that owns an fp32 shadow context on the same stream
+static lgf_status create_mixed(const int dims[4], lgf_storage s, void* ws, size_t bytes, void* stream, bool own, lgf_ctx** out) {
+    if (!dims || !out) return LGF_ERR_INVALID_ARG;
+    *out = nullptr;
+    const size_t n64 = lgf_workspace_bytes(dims, LGF_FP64, s), n32 = lgf32_workspace_bytes(dims, LGF_FP32, s);
+    lgf_ctx* c = nullptr;
+    lgf_status st;
+    if (own) st = create_impl(dims, LGF_FP64, s, nullptr, 0, nullptr, true, &c);
+    else {
+        if (n64 == 0 || n32 == 0) return create_impl(dims, LGF_FP64, s, ws, bytes, stream, false, &c);   // reports the argument error
+        if (!ws || bytes < align_up(n64, 256) + n32) return LGF_ERR_INVALID_ARG;
+        st = create_impl(dims, LGF_FP64, s, ws, align_up(n64, 256), stream, false, &c);
+    }
+    if (st != LGF_OK) return st;
+    char* ws32;
+    if (own) {
+        if (cudaMalloc(&c->shadow_ws, n32) != cudaSuccess) { cudaGetLastError(); lgf_destroy(c); return LGF_ERR_OOM; }
+        ws32 = c->shadow_ws;
+    } else ws32 = static_cast<char*>(ws) + align_up(n64, 256);
+    st = lgf32_create_ex(dims, LGF_FP32, s, ws32, n32, c->stream, &c->shadow);
+    if (st != LGF_OK) { c->shadow = nullptr; lgf_destroy(c); return st; }
+    *out = c;
+    return LGF_OK;
+}
+#endif
+
 lgf_status lgf_create(const int dims[4], lgf_precision p, lgf_storage s, lgf_ctx** out) {
 #ifndef LGF_F32
     if (p == LGF_FP32) return lgf32_create(dims, p, s, out);
+    if (p == LGF_MIXED) return create_mixed(dims, s, nullptr, 0, nullptr, true, out);
 #endif
     return create_impl(dims, p, s, nullptr, 0, nullptr, true, out);
 }
 lgf_status lgf_create_ex(const int dims[4], lgf_precision p, lgf_storage s, void* ws, size_t bytes, void* stream, lgf_ctx** out) {
 #ifndef LGF_F32
     if (p == LGF_FP32) return lgf32_create_ex(dims, p, s, ws, bytes, stream, out);
+    if (p == LGF_MIXED) return create_mixed(dims, s, ws, bytes, stream, false, out);
 #endif
     return create_impl(dims, p, s, ws, bytes, stream, false, out);
 }
@@ -824,6 +873,10 @@ void lgf_destroy(lgf_ctx* c) {
     FWD32V(lgf32_destroy(c))
     if (!c) return;
     if (c->stream) cudaStreamSynchronize(c->stream);
+#ifndef LGF_F32
+    if (c->shadow) lgf32_destroy(c->shadow);
+    if (c->shadow_ws) cudaFree(c->shadow_ws);
+#endif
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     if (c->ev0) cudaEventDestroy(c->ev0);
@@ -857,6 +910,17 @@ lgf_status lgf_get_links_device(lgf_ctx* c, double* dev_links) {
     return get_to_chunks(c, dev_links, false);
 }
 
+#ifdef LGF_F32
+void* lgf32_x_begin(lgf_ctx* c) {
+    c->parity = 0; c->loaded = true; c->acc_g = 1;
+    c->opt_quad = 1; c->opt_store_g = 0; c->opt_fuse_update = 0; c->opt_accel = 1;
+    LaunchScope ls(c, K_MISC);
+    k_init_gacc<<<(unsigned)((c->G.V + 255) / 256), 256, 0, c->stream>>>(c->gbuf, c->G.V);
+    return c->links;
+}
+void* lgf32_x_gacc(lgf_ctx* c) { return c->gbuf; }
+#endif
+
 lgf_status lgf_iterate(lgf_ctx* c, int n, double alpha, double* F, double* theta) {
     FWD32(lgf32_iterate(c, n, alpha, F, theta))
     if (!c || n < 0 || !(alpha > 0.0) || !std::isfinite(alpha)) return LGF_ERR_INVALID_ARG;
@@ -872,9 +936,35 @@ lgf_status lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int
     FWD32(lgf32_fix(c, alpha, theta_tol, max_iter, n_iter, F, theta))
     if (!c || max_iter < 0 || !(alpha > 0.0) || !std::isfinite(alpha) || !(theta_tol >= 0.0)) return LGF_ERR_INVALID_ARG;
     if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    int n32 = 0;
+#ifndef LGF_F32
+    if (c->shadow) {
+        // Mixed precision.  Phase 1: a float copy of the links is fixed in fp32 down to theta_sw (above the fp32 floor of
+        // ~1e-14) while the fp32 update accumulates the total transformation Gacc(x).  Phase 2: the fp64 links receive
+        // Gacc in one step (re-orthonormalised in double: an exact gauge copy of the input) and the fp64 iteration
+        // takes theta from the fp32 noise level to theta_tol.
+        const double theta_sw = theta_tol > 1e-12 ? theta_tol : 1e-12;
+        float2* l32 = static_cast<float2*>(lgf32_x_begin(c->shadow));
+        const long long n = 4LL * c->NC * c->G.V;
+        { LaunchScope ls(c, K_MISC); k_demote<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(cur_links(c), l32, n); }
+        CK(cudaGetLastError());
+        double F32v = 0, th32 = 0;
+        lgf_status s1 = lgf32_fix(c->shadow, alpha, theta_sw, max_iter, &n32, &F32v, &th32);
+        if (s1 != LGF_OK && s1 != LGF_NOT_CONVERGED) { c->err = std::string("fp32 phase: ") + lgf32_last_error(c->shadow); return s1; }
+        {
+            LaunchScope ls(c, K_MISC);
+            const float2* ga = static_cast<const float2*>(lgf32_x_gacc(c->shadow));
+            if (c->NC == 6) k_apply_gacc<6><<<(unsigned)(4 * (c->G.V / 128)), 128, 0, c->stream>>>(cur_links(c), ga, c->G);
+            else k_apply_gacc<9><<<(unsigned)(4 * (c->G.V / 128)), 128, 0, c->stream>>>(cur_links(c), ga, c->G);
+        }
+        CK(cudaGetLastError());
+        c->mixed_n32 = n32;
+        max_iter = max_iter > n32 ? max_iter - n32 : 0;
+    }
+#endif
     lgf_status st = run(c, alpha, theta_tol, max_iter, true);
     if (st != LGF_OK) return st;
-    if (n_iter) *n_iter = c->h_ctl->iters;
+    if (n_iter) *n_iter = n32 + c->h_ctl->iters;
     if (F) *F = c->h_ctl->F;
     if (theta) *theta = c->h_ctl->theta;
     return c->h_ctl->converged ? LGF_OK : LGF_NOT_CONVERGED;
@@ -990,6 +1080,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_FUSE_FINALIZE: *value = use_fused_fin(c) ? 1 : 0; break;
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
+        case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;
         case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;
     }

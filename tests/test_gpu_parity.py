@@ -409,6 +409,39 @@ def test_fp32_converges_to_its_rounding_floor_and_keeps_invariants():
     assert r["status"] == lgf.LGF_NOT_CONVERGED and 1e-16 < r["theta"] < 1e-12
 
 
+@pytest.mark.parametrize("name", ["C0", "C1"])
+def test_mixed_precision_fix_is_an_exact_gauge_copy_at_the_same_maximum(name):
+    """LGF_MIXED: fp32 phase with accumulated transformation, applied to the fp64 links in one step, fp64 polish.
+    The result must (i) reach theta < 1e-15, (ii) be a gauge copy of the input to fp64 accuracy (plaquette, unitarity),
+    (iii) sit at the maximum the oracle's fp64 trajectory reaches: same F to 1e-12 (the value of the functional at a
+    maximum does not depend on the path; the links themselves agree only up to one global SU(3) rotation, because the
+    iteration never fixes the zero mode and fp32 round-off lets it drift, so they are not compared element by element),
+    (iv) do most of its iterations in fp32."""
+    U, cfg = E.make_config(name)
+    dims, storage = cfg["dims"], cfg["storage"]
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    o.load(U)
+    r_ref = o.fix(ALPHA, TOL, 1000)
+    gf = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_MIXED)
+    gf.load_links(U)
+    _, _, plaq0 = gf.measure()
+    r = gf.fix(ALPHA, TOL, 1000)
+    n32 = gf.get_option(lgf.LGF_OPT_MIXED_FP32_ITERS)
+    assert r["status"] == lgf.LGF_OK and r["theta"] < TOL
+    assert 0 < n32 < r["n_iter"] <= r_ref["n_iter"] + 8 and r["n_iter"] - n32 <= 10       # most of the work in fp32
+    assert abs(r["F"] - r_ref["F"]) <= F_TOL
+    F1, th1, plaq1 = gf.measure()
+    assert abs(plaq1 - plaq0) <= 1e-12 and F1 == r["F"]
+    L = gf.get_links()
+    assert np.abs(np.einsum("xmij,xmkj->xmik", L, L.conj()) - np.eye(3)).max() <= 1e-13
+    # fp64 lgf_iterate on a mixed context is the plain fp64 path
+    gf.load_links(U)
+    o.load(U)
+    F, th = gf.iterate(3, ALPHA)
+    F_ref, th_ref = o.iterate(3, ALPHA)
+    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref) and np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
+
+
 def test_C1_ten_iterations_against_the_naive_dft_oracle():
     U, cfg = E.make_config("C1")
     o = oracle.Oracle(cfg["dims"], cfg["storage"], fft_mode=0)      # the definition
