@@ -216,7 +216,13 @@ def test_trajectory_C0_pure_gauge_fixed_point():
 
 
 def test_trajectory_C1():
-    check_trajectory("C1", fft_mode=1)
+    hist_ref, n_ref = check_trajectory("C1", fft_mode=1)
+    # the same trajectory as the stored oracle output (tests/golden, written by the oracle alone)
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_C1_trajectory.txt")
+    rows = np.array([[float(v) for v in ln.split()] for ln in open(path) if not ln.startswith("#")])
+    assert n_ref == len(rows) - 1
+    assert np.abs(hist_ref[: len(rows), 0] - rows[:, 1]).max() <= 1e-13
 
 
 def test_trajectory_C2b_headline_config():

@@ -448,3 +448,20 @@ def test_thread_count_independence():
         env = dict(os.environ, OMP_NUM_THREADS=nt)
         outs.append(subprocess.check_output([sys.executable, "-c", code], env=env, cwd=os.path.dirname(os.path.dirname(__file__))))
     assert outs[0] == outs[1]
+
+
+@pytest.mark.parametrize("name,fft_mode", [("C0", 0), ("C1", 1)])
+def test_golden_trajectories_are_what_the_oracle_computes(name, fft_mode):
+    """tests/golden/oracle_*_trajectory.txt (written by tests/golden/make_golden.py from the oracle alone) against the
+    oracle as it stands: a change of the oracle's arithmetic must show up here.  Rounding-level slack only."""
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", f"oracle_{name}_trajectory.txt")
+    rows = np.array([[float(v) for v in ln.split()] for ln in open(path) if not ln.startswith("#")])
+    U, cfg = E.make_config(name)
+    o = oracle.Oracle(cfg["dims"], cfg["storage"], fft_mode=fft_mode)
+    o.load(U)
+    r = o.fix(0.08, 1e-15, 1000, history=True)
+    h = np.array(r["history"])
+    assert len(h) == len(rows) and r["n_iter"] == len(rows) - 1
+    assert np.abs(h[:, 0] - rows[:, 1]).max() <= 1e-13
+    assert np.all(np.abs(h[:, 1] - rows[:, 2]) <= 1e-9 * np.maximum(rows[:, 2], 1e-15))
