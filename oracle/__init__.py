@@ -32,6 +32,7 @@ def lib():
         L.orc_create.argtypes = [I4, C.c_int, C.c_int]
         L.orc_destroy.argtypes = [P]
         L.orc_set_variant.argtypes = [P, C.c_int, C.c_int]
+        L.orc_set_gauge.argtypes = [P, C.c_int]
         L.orc_load.argtypes = [P, P]
         L.orc_get.argtypes = [P, P]
         L.orc_measure.argtypes = [P, D, D]
@@ -82,6 +83,10 @@ class Oracle:
 
     def set_variant(self, accel: int = 1, exp_sign: int = -1):
         lib().orc_set_variant(self._h, accel, exp_sign)
+
+    def set_gauge(self, nd: int = 4):
+        """nd = 4 Landau gauge (the paper); nd = 3 Coulomb gauge (gauge condition over mu = 0..2 only)."""
+        lib().orc_set_gauge(self._h, nd)
 
     def load(self, U):
         U = _c128(U)

@@ -153,15 +153,20 @@ void dft4(const Geometry& G, std::vector<cd>& f, int sign, int fft_mode) {
 }
 
 // w(n) = p2max / p2(n), p2max = 4 N_d = 16, w(0) = 0      [NS step 2]
-std::vector<double> fa_weights(const Geometry& G, int accel) {
+// nd = 4: Landau gauge (the paper).  nd = 3: Coulomb gauge (the variant of PAPER.md:41
+// refs [1],[2] with the sum over mu restricted to the spatial directions): p2 runs over axes 0..2, p2max = 4*3 = 12,
+// and the weight vanishes on the zero spatial momentum of every time slice (n0 = n1 = n2 = 0, any n3).  The weight
+// then does not depend on n3, so the 4-D transform pair acts as a 3-D transform pair on every time slice.
+std::vector<double> fa_weights(const Geometry& G, int accel, int nd = 4) {
     std::vector<double> w(G.V);
     const double pi = 3.14159265358979323846264338327950288;
     for (long n = 0; n < G.V; n++) {
         if (!accel) { w[n] = 1.0; continue; }
         int c[4]; G.coords(n, c);
         double p2 = 0;
-        for (int k = 0; k < 4; k++) { double s = std::sin(pi * (double)c[k] / (double)G.L[k]); p2 += 4.0 * s * s; }
-        w[n] = (n == 0) ? 0.0 : 16.0 / p2;
+        bool zero = true;
+        for (int k = 0; k < nd; k++) { double s = std::sin(pi * (double)c[k] / (double)G.L[k]); p2 += 4.0 * s * s; zero = zero && c[k] == 0; }
+        w[n] = zero ? 0.0 : (4.0 * nd) / p2;
     }
     return w;
 }
@@ -174,6 +179,7 @@ struct orc_ctx {
     int fft_mode;   // 0 naive DFT (definition), 1 radix-2 FFT
     int accel;      // 1 Fourier accelerated (paper), 0 plain steepest descent (pin P8 only)
     int exp_sign;   // -1: forward e^{-i..} (default); +1: swapped convention (pin P7 only)
+    int nd;         // directions in the gauge condition: 4 Landau (the paper), 3 Coulomb (mu = 0..2)
     std::vector<Mat> U;  // U[x*4+mu]
     bool loaded;
 };
@@ -183,7 +189,7 @@ namespace {
 // O1, per site
 inline Mat delta_site(const orc_ctx* c, long x) {
     Mat A = mat_zero();
-    for (int mu = 0; mu < 4; mu++) {
+    for (int mu = 0; mu < c->nd; mu++) {
         long xb = c->G.bwd(x, mu);
         A = mat_add(A, mat_sub(c->U[xb * 4 + mu], c->U[x * 4 + mu]));
     }
@@ -208,11 +214,11 @@ void measure(const orc_ctx* c, const std::vector<Mat>& D, double* F, double* the
         for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) s += std::norm(D[x].m[i][j]);   // Tr[Delta Delta^dag]
         th[x] = s;
         double f = 0;
-        for (int mu = 0; mu < 4; mu++) f += mat_tr(c->U[x * 4 + mu]).real();
+        for (int mu = 0; mu < c->nd; mu++) f += mat_tr(c->U[x * 4 + mu]).real();
         fs[x] = f;
     }
     *theta = csum(th) / (3.0 * (double)V);
-    *F = csum(fs) / (12.0 * (double)V);
+    *F = csum(fs) / (3.0 * (double)c->nd * (double)V);
 }
 
 // O3
@@ -220,7 +226,7 @@ void fa_field(const orc_ctx* c, const std::vector<Mat>& D, std::vector<Mat>& X) 
     const Geometry& G = c->G;
     const long V = G.V;
     X.resize(V);
-    std::vector<double> w = fa_weights(G, c->accel);
+    std::vector<double> w = fa_weights(G, c->accel, c->nd);
     std::vector<cd> f(V);
     for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) {
         for (long x = 0; x < V; x++) f[x] = D[x].m[i][j];
@@ -285,11 +291,12 @@ orc_ctx* orc_create(const int dims[4], int storage, int fft_mode) {
     if (storage != 12 && storage != 18) return nullptr;
     for (int k = 0; k < 4; k++) if (dims[k] < 1) return nullptr;
     orc_ctx* c = new orc_ctx;
-    c->G.set(dims); c->storage = storage; c->fft_mode = fft_mode; c->accel = 1; c->exp_sign = -1; c->loaded = false;
+    c->G.set(dims); c->storage = storage; c->fft_mode = fft_mode; c->accel = 1; c->exp_sign = -1; c->nd = 4; c->loaded = false;
     return c;
 }
 void orc_destroy(orc_ctx* c) { delete c; }
 void orc_set_variant(orc_ctx* c, int accel, int exp_sign) { c->accel = accel; c->exp_sign = exp_sign; }
+void orc_set_gauge(orc_ctx* c, int nd) { c->nd = (nd == 3) ? 3 : 4; }
 
 // links: [V][4][3][3][2] doubles, x0 fastest.  Stored as given (no reprojection, reading A9);
 // in 12-real mode row 2 is dropped and rebuilt from rows 0,1.
@@ -321,10 +328,10 @@ double orc_F_of_g(const orc_ctx* c, const double* g_in) {
     std::vector<double> fs(V);
     for (long x = 0; x < V; x++) {
         double f = 0;
-        for (int mu = 0; mu < 4; mu++) f += mat_tr(mat_mul(mat_mul(g[x], c->U[x * 4 + mu]), mat_dag(g[c->G.fwd(x, mu)]))).real();
+        for (int mu = 0; mu < c->nd; mu++) f += mat_tr(mat_mul(mat_mul(g[x], c->U[x * 4 + mu]), mat_dag(g[c->G.fwd(x, mu)]))).real();
         fs[x] = f;
     }
-    return csum(fs) / (12.0 * (double)V);
+    return csum(fs) / (3.0 * (double)c->nd * (double)V);
 }
 
 // iterate(n): (O1, O3-O6) n times, then O1 once more; returns F, theta of the links after the n-th update (A5)

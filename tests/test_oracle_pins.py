@@ -465,3 +465,68 @@ def test_golden_trajectories_are_what_the_oracle_computes(name, fft_mode):
     assert len(h) == len(rows) and r["n_iter"] == len(rows) - 1
     assert np.abs(h[:, 0] - rows[:, 1]).max() <= 1e-13
     assert np.all(np.abs(h[:, 1] - rows[:, 2]) <= 1e-9 * np.maximum(rows[:, 2], 1e-15))
+
+
+# ------------------------------------------------------------------ Coulomb-gauge variant of the oracle (nd = 3)
+def _coulomb(dims, storage=18, fft_mode=0):
+    o = oracle.Oracle(dims, storage, fft_mode=fft_mode)
+    o.set_gauge(3)
+    return o
+
+
+@pytest.mark.parametrize("dims,alpha", [((8, 8, 8, 4), 0.08), ((4, 8, 4, 8), 0.05)])
+def test_coulomb_linearised_rate(dims, alpha):
+    """Coulomb gauge (gauge condition over mu = 0..2): with p2max = 4*3 every mode of non-zero
+    spatial momentum contracts by (1 - 12 alpha) per iteration, so theta_{k+1}/theta_k = (1 - 12 alpha)^2; pins
+    p2max = 12, the restriction of p^2 to three axes, alpha/2, 1/V and the sign, as P9 does for Landau."""
+    V = int(np.prod(dims))
+    rng = np.random.Generator(np.random.Philox(key=[6, 1]))
+    h = E.expi_hermitian(E.gaussian_su3_algebra(rng, V), 1e-5)
+    U = np.stack([h @ dag(shift(h, dims, mu)) for mu in range(4)], axis=1)
+    o = _coulomb(dims)
+    o.load(U)
+    _, th0 = o.measure()
+    _, th1 = o.iterate(1, alpha)
+    _, th2 = o.iterate(1, alpha)
+    r = (1 - 12 * alpha) ** 2
+    assert abs(th1 / th0 - r) < 2e-3 * r
+    assert abs(th2 / th1 - r) < 2e-3 * r
+
+
+def test_coulomb_field_is_spatial_and_inverts_the_3d_laplacian():
+    """Delta and X of time slice t depend only on the spatial links of that slice; X obeys the 3-D version of P18,
+    sum_{mu<3} [2 X(x) - X(x+mu) - X(x-mu)] = 12 Delta(x); F counts three directions (identity links: F = 1)."""
+    dims = (4, 6, 4, 4)
+    U = E.noisy(dims, 31, 0.4)
+    o = _coulomb(dims)
+    o.load(U)
+    D = o.delta().reshape(dims[::-1] + (3, 3))
+    X = o.fa_field().reshape(dims[::-1] + (3, 3))
+    lap = sum(2.0 * X - np.roll(X, 1, axis=ax) - np.roll(X, -1, axis=ax) for ax in (1, 2, 3))     # axes x2, x1, x0
+    assert np.abs(lap - 12.0 * D).max() <= 1e-12 * np.abs(X).max()
+    assert np.abs(D.sum(axis=(1, 2, 3))).max() <= 1e-12                                            # per time slice
+    U2 = U.copy().reshape(dims[::-1] + (4, 3, 3))
+    U2[1] = E.noisy(dims, 32, 0.4).reshape(dims[::-1] + (4, 3, 3))[1]                              # another slice t = 1
+    U2[:, :, :, :, 3] = E.noisy(dims, 33, 0.4).reshape(dims[::-1] + (4, 3, 3))[:, :, :, :, 3]      # all temporal links
+    o.load(U2.reshape(-1, 4, 3, 3))
+    X2 = o.fa_field().reshape(dims[::-1] + (3, 3))
+    assert np.abs(X2[[0, 2, 3]] - X[[0, 2, 3]]).max() <= 1e-13 * np.abs(X).max()
+    ident = np.broadcast_to(np.eye(3, dtype=np.complex128), (int(np.prod(dims)), 4, 3, 3)).copy()
+    o.load(ident)
+    F, th = o.measure()
+    assert abs(F - 1.0) < 1e-15 and th == 0.0
+
+
+def test_coulomb_trajectory_invariants():
+    """F_C rises monotonically, the plaquette is invariant, links stay special unitary, theta falls below 1e-15."""
+    dims = (8, 8, 8, 4)
+    U = E.noisy(dims, 34, 0.3)
+    o = _coulomb(dims, storage=12, fft_mode=1)
+    o.load(U)
+    p0 = o.plaquette()
+    r = o.fix(0.08, 1e-15, 500, history=True)
+    h = np.array(r["history"])
+    assert r["status"] == 0 and h[-1, 1] < 1e-15
+    assert np.all(np.diff(h[:, 0]) >= -1e-14)
+    assert abs(o.plaquette() - p0) <= 1e-12
+    assert max(o.unitarity()) <= 1e-13
