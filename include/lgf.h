@@ -149,11 +149,16 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_FOURIER_ACCEL   1 (default): the paper's method, X = IFFT[(p2max/p2) FFT[Delta]].  0: plain steepest
  *                           descent, X = Delta (the method Fourier acceleration is measured against, PAPER.md:41 refs
  *                           [1],[2]): S2 drops out, an iteration is S1, S5, S3+S4.  Converges for alpha < 2/p2max = 1/8,
- *                           with a rate that degrades with the volume (critical slowing down). */
+ *                           with a rate that degrades with the volume (critical slowing down).
+ *   LGF_OPT_GAUGE_DIRECTIONS 4 (default): Landau gauge, the paper's problem.  3: Coulomb gauge -- the gauge
+ *                           condition, Delta, F (normalised by 3 N_c V) and p^2 run over mu = 0..2 only, p2max = 12, the
+ *                           spatial zero mode of every time slice is dropped, all four link directions are transformed.
+ *                           Same kernels; the transform along axis 3 is a no-op pair kept for simplicity.
+ *                           LGF_OPT_FUSE_UPDATE is Landau only and is ignored in Coulomb gauge. */
 typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
                LGF_OPT_FUSE_UPDATE = 5, LGF_OPT_PINGPONG = 6, LGF_OPT_FUSE_FINALIZE = 7,
                LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9, LGF_OPT_FOURIER_ACCEL = 10,
-               LGF_OPT_MIXED_FP32_ITERS = 11 /* read-only */ } lgf_option;
+               LGF_OPT_MIXED_FP32_ITERS = 11 /* read-only */, LGF_OPT_GAUGE_DIRECTIONS = 12 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

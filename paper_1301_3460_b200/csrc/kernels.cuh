@@ -60,6 +60,7 @@ __device__ __forceinline__ void delta_site(const cplx* __restrict__ links, const
     real i0 = 0, i1 = 0, i2 = 0, retr = 0;
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) {
+        if (mu >= G.nd) break;                       // Coulomb gauge: the condition runs over mu = 0..2
         cplx u[9];
         load_link<NC>(links, G.V, mu, x, u);
         retr += u[0].x + u[4].x + u[8].x;

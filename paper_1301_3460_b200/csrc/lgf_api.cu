@@ -342,7 +342,7 @@ size_t smem_fast_mid(int lga, int lgb, int lgC) {
 template <int NC> void launch_fa_delta_fwd(lgf_ctx* c, bool fin) {
     LaunchScope ls(c, K_FA_DELTA_FWD);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
-    const FinArgs fa{c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), fin ? 1 : 0};
+    const FinArgs fa{c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (3.0 * (double)c->G.nd * (double)c->G.V), fin ? 1 : 0};
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
         launch_k(c, k_fa_delta_fwd<A, B, NC, FAD_NT>, grid, FAD_NT, c->smem_fa, cur_links(c), c->field, c->partials, c->G, c->T, c->ctl, fa);
     LGF_FAST_PAIRS(X)
@@ -394,7 +394,7 @@ template <int NC> void launch_fu_update(lgf_ctx* c) {
 void launch_fa_mid(lgf_ctx* c) {
     LaunchScope ls(c, K_FA_MID);
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
-    const double scale = 16.0 / (double)c->G.V;
+    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
         launch_k(c, k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, grid, fast_mid_nt(A, B), c->smem_fb, c->field, c->G, c->T, scale, c->ctl);
     LGF_FAST_PAIRS(X) LGF_BIG_PAIRS(X)
@@ -422,7 +422,7 @@ void launch_pp_inv(lgf_ctx* c) {
 void launch_pp_mid(lgf_ctx* c) {
     LaunchScope ls(c, K_PP_MID);
     const unsigned grid = pp_grid(c, 4LL * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
-    const double scale = 16.0 / (double)c->G.V;
+    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
         launch_k(c, k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, grid, 2 * FA_NT, c->smem_pb, c->field, c->G, c->T, scale, c->ctl);
     LGF_FAST_PAIRS(X)
@@ -524,7 +524,7 @@ lgf_status build_tables(lgf_ctx* c) {
         for (int p = 0; p < L; p++) {
             const int n = stored_freq(p, c->G.lg[mu], c->T.plan[mu]);
             long double sn = sinl(pi * (long double)n / (long double)L);
-            s[mu * 128 + p] = (n == 0) ? 0.0 : (double)(4.0L * sn * sn);
+            s[mu * 128 + p] = (n == 0 || mu >= c->G.nd) ? 0.0 : (double)(4.0L * sn * sn);      // Coulomb: p2 over mu = 0..2
         }
     }
     char* tb = c->ws + c->lay.tables;
@@ -555,11 +555,11 @@ void launch_fft23(lgf_ctx* c) {
     LaunchScope ls(c, K_FFT23_MID);
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fft23_lgC));
     launch_k(c, k_fft23_mid, grid, c->fft23_threads, c->smem23, c->field, c->G, c->T, c->fft23_lgC, c->fft23_S1, c->fft23_S2,
-                                                                   16.0 / (double)c->G.V, c->ctl);
+                                                                   4.0 * (double)c->G.nd / (double)c->G.V, c->ctl);
 }
 void launch_finalize(lgf_ctx* c, int n_partials, int advance = 0) {
     LaunchScope ls(c, K_FINALIZE);
-    launch_k(c, k_finalize, 1, n_partials > 8192 ? 1024 : 256, 0, c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (12.0 * (double)c->G.V), advance);
+    launch_k(c, k_finalize, 1, n_partials > 8192 ? 1024 : 256, 0, c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (3.0 * (double)c->G.nd * (double)c->G.V), advance);
 }
 template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
     if (!SG && c->opt_quad) {
@@ -584,7 +584,7 @@ bool use_store_g(const lgf_ctx* c) { return c->opt_store_g && c->fft01_ncomp_fus
 bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a && use_fused(c); }
 bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
 bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c && !use_store_g(c); }
-bool use_fused_update(const lgf_ctx* c) { return c->opt_accel && c->opt_fuse_update && c->opt_fast && c->fast_a; }
+bool use_fused_update(const lgf_ctx* c) { return c->opt_accel && c->G.nd == 4 && c->opt_fuse_update && c->opt_fast && c->fast_a; }
 bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p && !use_store_g(c); }
 bool use_pp_a(const lgf_ctx* c) { return (c->opt_pingpong & 1) && use_fast_a(c); }
 bool use_pp_b(const lgf_ctx* c) { return (c->opt_pingpong & 2) && use_fast_b(c) && c->pp_b_ok; }
@@ -664,7 +664,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28) ^ ((c->G.nd == 3) << 29);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -729,6 +729,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     int shv = 0;
     for (int k = 0; k < 4; k++) { c->G.L[k] = dims[k]; c->G.lg[k] = lg[k]; c->G.sh[k] = shv; shv += lg[k]; }
     c->G.V = 1LL << shv;
+    c->G.nd = 4;
     c->NC = (s == LGF_STORE_12) ? 6 : 9;
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
@@ -913,7 +914,7 @@ lgf_status lgf_get_links_device(lgf_ctx* c, double* dev_links) {
 #ifdef LGF_F32
 void* lgf32_x_begin(lgf_ctx* c) {
     c->parity = 0; c->loaded = true; c->acc_g = 1;
-    c->opt_quad = 1; c->opt_store_g = 0; c->opt_fuse_update = 0; c->opt_accel = 1;
+    c->opt_quad = 1; c->opt_store_g = 0; c->opt_fuse_update = 0;
     LaunchScope ls(c, K_MISC);
     k_init_gacc<<<(unsigned)((c->G.V + 255) / 256), 256, 0, c->stream>>>(c->gbuf, c->G.V);
     return c->links;
@@ -1050,6 +1051,12 @@ lgf_status lgf_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host
 lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
     FWD32(lgf32_set_option(c, opt, value))
     if (!c) return LGF_ERR_INVALID_ARG;
+#ifndef LGF_F32
+    if (c->shadow && (opt == LGF_OPT_GAUGE_DIRECTIONS || opt == LGF_OPT_FOURIER_ACCEL)) {      // the method itself: both phases
+        lgf_status st = lgf32_set_option(c->shadow, opt, value);
+        if (st != LGF_OK) return st;
+    }
+#endif
     switch (opt) {
         case LGF_OPT_FUSE_DELTA_FFT: c->opt_fuse = value ? 1 : 0; break;
         case LGF_OPT_STORE_G: c->opt_store_g = value ? 1 : 0; break;
@@ -1062,6 +1069,13 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_QUAD_UPDATE: c->opt_quad = value ? 1 : 0; break;
         case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
+        case LGF_OPT_GAUGE_DIRECTIONS: {
+            if (value != 3 && value != 4) return LGF_ERR_INVALID_ARG;
+            c->G.nd = value;
+            lgf_status st = build_tables(c);         // the p2 table of axis 3 is zero in Coulomb gauge
+            if (st != LGF_OK) return st;
+            break;
+        }
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
@@ -1080,6 +1094,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_FUSE_FINALIZE: *value = use_fused_fin(c) ? 1 : 0; break;
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
+        case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;
         case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;

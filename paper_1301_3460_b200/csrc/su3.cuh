@@ -175,6 +175,7 @@ struct Geom {
     int L[4];
     int lg[4];    // log2 L
     int sh[4];    // log2 stride of axis mu (sum of lg of lower axes)
+    int nd;       // directions in the gauge condition: 4 Landau (the paper), 3 Coulomb (mu = 0..2)
     long long V;
 };
 __device__ __forceinline__ int coord(const Geom& G, long long x, int mu) { return (int)(x >> G.sh[mu]) & (G.L[mu] - 1); }

@@ -355,6 +355,57 @@ def test_plain_steepest_descent_variant(dims, storage):
     assert th < href[-1, 1]                                              # Fourier acceleration converges faster
 
 
+# ------------------------------------------------------------------ Coulomb gauge
+@pytest.mark.parametrize("dims,storage", [((8, 8, 8, 8), 18), ((16, 16, 16, 8), 12), ((32, 32, 16, 16), 12), ((4, 8, 16, 4), 12)])
+def test_coulomb_gauge_against_the_oracle(dims, storage):
+    """LGF_OPT_GAUGE_DIRECTIONS = 3: stages, trajectory, stop iteration against the oracle's Coulomb mode (pinned on the
+    CPU by the rate (1 - 12 alpha)^2, the 3-D Laplacian identity and slice locality); every kernel selection."""
+    U = E.noisy(dims, 61, 0.3)
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    o.set_gauge(3)
+    o.load(U)
+    D_ref, X_ref = o.delta(), o.fa_field()
+    F_ref, th_ref = o.measure()
+    r20 = o.fix(ALPHA, 0.0, 20, history=True)
+    href = np.array(r20["history"])
+    U20 = o.get()
+    o.load(U)
+    r_ref = o.fix(ALPHA, TOL, 1000)
+    gf = lgf.GaugeFixer(dims, storage)
+    gf.set_option(lgf.LGF_OPT_GAUGE_DIRECTIONS, 3)
+    assert gf.get_option(lgf.LGF_OPT_GAUGE_DIRECTIONS) == 3
+    for v in [(1, 0, 1, 1, 0), (0, 0, 0, 0, 0, 0, 0, 0), (0, 1, 1, 1, 0), (1, 0, 0, 1, 0, 7), (1, 0, 1, 1, 1)]:
+        set_variant(gf, v)
+        gf.load_links(U)
+        F, th, _ = gf.measure()
+        assert abs(F - F_ref) <= 1e-14 and abs(th - th_ref) <= 1e-12 * th_ref, v
+        assert np.abs(gf.get_field(lgf.LGF_FIELD_DELTA) - D_ref).max() <= 1e-14 * max(1.0, np.abs(D_ref).max()), v
+        assert np.abs(gf.get_field(lgf.LGF_FIELD_X) - X_ref).max() <= 1e-13 * np.abs(X_ref).max(), v
+        gf.iterate(20, ALPHA)
+        h = gf.get_history()
+        assert np.abs(h[:, 0] - href[:, 0]).max() <= F_TOL, v
+        assert all(theta_close(a, b) for a, b in zip(h[:, 1], href[:, 1])), v
+        assert np.abs(gf.get_links() - U20).max() <= LINK_TOL, v
+        gf.load_links(U)
+        r = gf.fix(ALPHA, TOL, 1000)
+        assert r["status"] == lgf.LGF_OK and r["n_iter"] == r_ref["n_iter"] and abs(r["F"] - r_ref["F"]) <= F_TOL, v
+    # mixed precision in Coulomb gauge: both phases use the restricted condition
+    gm = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_MIXED)
+    gm.set_option(lgf.LGF_OPT_GAUGE_DIRECTIONS, 3)
+    gm.load_links(U)
+    r = gm.fix(ALPHA, TOL, 1000)
+    assert r["status"] == lgf.LGF_OK and r["theta"] < TOL and abs(r["F"] - r_ref["F"]) <= 1e-10
+    # back to Landau on the same context
+    gf.set_option(lgf.LGF_OPT_GAUGE_DIRECTIONS, 4)
+    set_variant(gf, (1, 0, 1, 1, 0))
+    gf.load_links(U)
+    o.set_gauge(4)
+    o.load(U)
+    F, th = gf.iterate(3, ALPHA)
+    F_ref, th_ref = o.iterate(3, ALPHA)
+    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
+
+
 # ------------------------------------------------------------------ fp32 (SURVEY.md section 8(f) NEXT-1)
 EPS32 = 2.0 ** -24      # fp32 unit round-off
 
