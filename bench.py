@@ -126,13 +126,38 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+# ---------------------------------------------------------------------------------------------- replicas (N > 1)
+# The path does not shard without two all-to-all exchanges per iteration, so N GPUs fix N
+# independent configurations: no collective on the data path.  torch.distributed serves the barrier and the
+# max-over-ranks time only.  These three helpers are the whole multi-rank host logic; tests/test_replicas.py runs
+# them at world size 2 over gloo on the CPU.
+def rank_stream(cfg: dict, rank: int) -> int:
+    """Philox stream of rank `rank`: its own configuration of the same ensemble."""
+    return int(cfg.get("stream", 0)) + 16 * int(rank)
+
+
+def max_over_ranks(x: float, dist=None, device="cpu") -> float:
+    """The slowest rank's time: every multi-GPU number is the max over ranks of device times."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, steps: int, inner: int, ms: float) -> float:
+    """Iterations/s of the whole job: every rank did steps*inner iterations in the (max over ranks) time ms."""
+    return world * steps * inner / (ms * 1e-3)
+
+
 def make_links(workload: str, rank: int):
     import ensembles as E
     cfg = dict(E.CONFIGS[workload])
     if cfg["kind"] == "pure_gauge":
-        U = E.pure_gauge(cfg["dims"], cfg["seed"], cfg.get("stream", 0) + 16 * rank)
+        U = E.pure_gauge(cfg["dims"], cfg["seed"], rank_stream(cfg, rank))
     else:
-        U = E.noisy(cfg["dims"], cfg["seed"], cfg["eps"], cfg.get("stream", 0) + 16 * rank)   # rank r: its own configuration
+        U = E.noisy(cfg["dims"], cfg["seed"], cfg["eps"], rank_stream(cfg, rank))   # rank r: its own configuration
     return U, cfg
 
 
@@ -195,12 +220,8 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(x: float) -> float:
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    def max_ranks(x: float) -> float:
+        return max_over_ranks(x, dist, "cuda")
 
     import ensembles as E
     device_links = args.links == "device"
@@ -247,7 +268,7 @@ def run_ours(args):
             fn()
         e1.record(stream)
         barrier()
-        return max_over_ranks(e0.elapsed_time(e1))       # ms
+        return max_ranks(e0.elapsed_time(e1))       # ms
 
     # ---- device-resident throughput (links already in HBM)
     sampler = ClockSampler(local) if rank == 0 else None
@@ -263,7 +284,7 @@ def run_ours(args):
     ms = timed(step, args.steps, 0)
     launches = gf.launch_count() - n_before
     clocks = sampler.stop() if sampler else None
-    value = world * args.steps * inner / (ms * 1e-3)
+    value = whole_job_value(world, args.steps, inner, ms)
 
     # ---- end to end through the C ABI with host buffers: H2D of the links, the iterations, D2H of the result
     def step_e2e():
@@ -276,7 +297,7 @@ def run_ours(args):
         ms_e2e, e2e_value = None, None
     else:
         ms_e2e = timed(step_e2e, e2e_steps, 1)
-        e2e_value = world * e2e_steps * inner / (ms_e2e * 1e-3)
+        e2e_value = whole_job_value(world, e2e_steps, inner, ms_e2e)
 
     line = None
     if rank == 0:
