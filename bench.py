@@ -57,6 +57,7 @@ def kernel_bytes_per_site(nc: int, cb: int = 16) -> dict:
         # compile-time-sized passes (fft_fast.cuh): same traffic as the generic passes they replace
         "k_fa_delta_fwd": lk + fld,
         "k_fa_mid": 2 * fld,
+        "k_fr_mid": 2 * fld,                 # pass B with whole lines in registers: same traffic
         "k_fa_inv": 2 * fld,
         "k_fa_inv_g": fld + g,               # read X~ field, write rows 0,1 of g
         # fused S3/S4 + next S1 + next pass A (fused_update.cuh): g, links read once + written once, field written

@@ -154,18 +154,22 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *                           condition, Delta, F (normalised by 3 N_c V) and p^2 run over mu = 0..2 only, p2max = 12, the
  *                           spatial zero mode of every time slice is dropped, all four link directions are transformed.
  *                           Same kernels; the transform along axis 3 is a no-op pair kept for simplicity.
- *                           LGF_OPT_FUSE_UPDATE is Landau only and is ignored in Coulomb gauge. */
+ *                           LGF_OPT_FUSE_UPDATE is Landau only and is ignored in Coulomb gauge.
+ *   LGF_OPT_LINE_FFT        1 (default): FFT pass B on extents 16/32 keeps whole lines in registers (one thread = one line
+ *                           of an axis, twiddles as instruction operands; the tile is written and read twice per point
+ *                           instead of four times, two barriers instead of five; k_fr_mid), 0: the stage-wise pass B
+ *                           (k_fa_mid).  lgf_get_option returns whether it runs. */
 typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
                LGF_OPT_FUSE_UPDATE = 5, LGF_OPT_PINGPONG = 6, LGF_OPT_FUSE_FINALIZE = 7,
                LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9, LGF_OPT_FOURIER_ACCEL = 10,
-               LGF_OPT_MIXED_FP32_ITERS = 11 /* read-only */, LGF_OPT_GAUGE_DIRECTIONS = 12 } lgf_option;
+               LGF_OPT_MIXED_FP32_ITERS = 11 /* read-only */, LGF_OPT_GAUGE_DIRECTIONS = 12, LGF_OPT_LINE_FFT = 13 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 
 /* Per-kernel device timing.  lgf_set_profiling(ctx,1) brackets every kernel launch with CUDA events on the
  * context's stream (plain launches, no graph); lgf_get_profile returns, per kernel slot i < LGF_MAX_KERNELS,
  * the accumulated milliseconds and launch counts since profiling was enabled.  names via lgf_kernel_name. */
-#define LGF_MAX_KERNELS 24
+#define LGF_MAX_KERNELS 32
 lgf_status lgf_set_profiling(lgf_ctx *ctx, int on);
 lgf_status lgf_get_profile(lgf_ctx *ctx, double ms[LGF_MAX_KERNELS], long long launches[LGF_MAX_KERNELS]);
 const char *lgf_kernel_name(int slot);

@@ -624,6 +624,161 @@ __global__ void __launch_bounds__(NT, (NT > 256) ? 1 : LGF_FA_MINB_MID) k_fa_mid
     pass_b_finish<LG2, LG3, LGC, NT>(it.gp, it.s01, G.sh[2], G.sh[3], scale, tile + i0, tw2, tw3, s2, s3, g);
 }
 
+
+// ---------------------------------------------------------------------------------------------------------------
+// Pass B with whole lines in registers (extents 16 and 32).  A thread takes one line of the tile at a time and runs
+// the complete forward (or inverse) transform of that axis on it in registers -- same stages, radices and stored
+// order as the passes above (Plan2), twiddles from constant-memory tables with compile-time indices, so they are
+// instruction operands, not loads.  Per point the tile is written twice and read twice (the stage-wise pass B: four
+// times each) and the pass has two barriers instead of five.
+//   phase 1: axis-2 lines straight from global memory -> forward -> tile
+//   phase 2: axis-3 lines: forward, p2max/p2 filter, inverse, in place
+//   phase 3: axis-2 lines: inverse -> straight to global memory
+__constant__ real c_tw16[16][2] = {      // exp(-2 pi i k / 16), correctly rounded
+    {(real)1.0, (real)-0.0}, {(real)0.9238795325112867, (real)-0.3826834323650898},
+    {(real)0.7071067811865476, (real)-0.7071067811865476}, {(real)0.3826834323650898, (real)-0.9238795325112867},
+    {(real)0.0, (real)-1.0}, {(real)-0.3826834323650898, (real)-0.9238795325112867},
+    {(real)-0.7071067811865476, (real)-0.7071067811865476}, {(real)-0.9238795325112867, (real)-0.3826834323650898},
+    {(real)-1.0, (real)-0.0}, {(real)-0.9238795325112867, (real)0.3826834323650898},
+    {(real)-0.7071067811865476, (real)0.7071067811865476}, {(real)-0.3826834323650898, (real)0.9238795325112867},
+    {(real)0.0, (real)1.0}, {(real)0.3826834323650898, (real)0.9238795325112867},
+    {(real)0.7071067811865476, (real)0.7071067811865476}, {(real)0.9238795325112867, (real)0.3826834323650898},
+};
+__constant__ real c_tw32[32][2] = {      // exp(-2 pi i k / 32), correctly rounded
+    {(real)1.0, (real)-0.0}, {(real)0.9807852804032304, (real)-0.19509032201612828},
+    {(real)0.9238795325112867, (real)-0.3826834323650898}, {(real)0.8314696123025452, (real)-0.5555702330196022},
+    {(real)0.7071067811865476, (real)-0.7071067811865476}, {(real)0.5555702330196022, (real)-0.8314696123025452},
+    {(real)0.3826834323650898, (real)-0.9238795325112867}, {(real)0.19509032201612828, (real)-0.9807852804032304},
+    {(real)0.0, (real)-1.0}, {(real)-0.19509032201612828, (real)-0.9807852804032304},
+    {(real)-0.3826834323650898, (real)-0.9238795325112867}, {(real)-0.5555702330196022, (real)-0.8314696123025452},
+    {(real)-0.7071067811865476, (real)-0.7071067811865476}, {(real)-0.8314696123025452, (real)-0.5555702330196022},
+    {(real)-0.9238795325112867, (real)-0.3826834323650898}, {(real)-0.9807852804032304, (real)-0.19509032201612828},
+    {(real)-1.0, (real)-0.0}, {(real)-0.9807852804032304, (real)0.19509032201612828},
+    {(real)-0.9238795325112867, (real)0.3826834323650898}, {(real)-0.8314696123025452, (real)0.5555702330196022},
+    {(real)-0.7071067811865476, (real)0.7071067811865476}, {(real)-0.5555702330196022, (real)0.8314696123025452},
+    {(real)-0.3826834323650898, (real)0.9238795325112867}, {(real)-0.19509032201612828, (real)0.9807852804032304},
+    {(real)0.0, (real)1.0}, {(real)0.19509032201612828, (real)0.9807852804032304},
+    {(real)0.3826834323650898, (real)0.9238795325112867}, {(real)0.5555702330196022, (real)0.8314696123025452},
+    {(real)0.7071067811865476, (real)0.7071067811865476}, {(real)0.8314696123025452, (real)0.5555702330196022},
+    {(real)0.9238795325112867, (real)0.3826834323650898}, {(real)0.9807852804032304, (real)0.19509032201612828},
+};
+template <int LG> __device__ __forceinline__ cplx ctw(int k) {      // k is a compile-time constant after unrolling
+    if constexpr (LG == 4) return mk(c_tw16[k][0], c_tw16[k][1]);
+    else return mk(c_tw32[k][0], c_tw32[k][1]);
+}
+
+// Complete transform of one line of L = R1 R2 points in registers: the two stages of Plan2<LG, B>, in place, stored
+// (digit-reversed) order out of the forward transform and into the inverse one.
+template <int LG, bool B, bool INV>
+__device__ __forceinline__ void line_fft(cplx (&v)[1 << LG]) {
+    using P = Plan2<LG, B>;
+    auto stage1 = [&]() {        // points ja + m R2, twiddles W_L^{k ja}
+#pragma unroll
+        for (int ja = 0; ja < P::R2; ja++) {
+            cplx x[P::R1];
+#pragma unroll
+            for (int m = 0; m < P::R1; m++) x[m] = v[ja + m * P::R2];
+            if constexpr (INV) {
+#pragma unroll
+                for (int k = 1; k < P::R1; k++) if (ja) x[k] = cmulc(x[k], ctw<LG>(k * ja));
+                bfly<P::R1, true>(x);
+            } else {
+                bfly<P::R1, false>(x);
+#pragma unroll
+                for (int k = 1; k < P::R1; k++) if (ja) x[k] = cmul(x[k], ctw<LG>(k * ja));
+            }
+#pragma unroll
+            for (int m = 0; m < P::R1; m++) v[ja + m * P::R2] = x[m];
+        }
+    };
+    auto stage2 = [&]() {        // contiguous sub-blocks of R2 points, unit twiddles
+#pragma unroll
+        for (int ba = 0; ba < P::R1; ba++) {
+            cplx x[P::R2];
+#pragma unroll
+            for (int m = 0; m < P::R2; m++) x[m] = v[ba * P::R2 + m];
+            bfly<P::R2, INV>(x);
+#pragma unroll
+            for (int m = 0; m < P::R2; m++) v[ba * P::R2 + m] = x[m];
+        }
+    };
+    if constexpr (INV) { stage2(); stage1(); } else { stage1(); stage2(); }
+}
+
+#ifndef LGF_FR_NT
+#define LGF_FR_NT 128
+#endif
+#ifndef LGF_FR_MINB
+#define LGF_FR_MINB 2
+#endif
+template <int LG2, int LG3, int LGC, int NT>
+__global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+    pdl_enter();
+    if (ctl->done) return;
+    using MG = MidGeom<LG2, LGC>;
+    constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw);
+    double* s2 = reinterpret_cast<double*>(tile + S2 * L3);
+    double* s3 = s2 + L2;
+    for (int i = threadIdx.x; i < L2; i += NT) s2[i] = T.s[2][i];
+    for (int i = threadIdx.x; i < L3; i += NT) s3[i] = T.s[3][i];
+    const int lgChunks = G.lg[0] - LGC;
+    const int chunk = blockIdx.x & ((1 << lgChunks) - 1);
+    const int x1 = (blockIdx.x >> lgChunks) & (G.L[1] - 1);
+    const int comp = blockIdx.x >> (lgChunks + G.lg[1]);
+    cplx* gbase = field + (long long)comp * G.V + (chunk << LGC) + ((long long)x1 << G.sh[1]);
+    const int sh2 = G.sh[2], sh3 = G.sh[3];
+    // phase 1: lines along axis 2, one per (i0, i3)
+#pragma unroll 1
+    for (int ln = threadIdx.x; ln < C0 * L3; ln += NT) {
+        const int i0 = ln % C0, i3 = ln / C0;
+        const cplx* gq = gbase + i0 + ((long long)i3 << sh3);
+        cplx v[L2];
+#pragma unroll
+        for (int m = 0; m < L2; m++) v[m] = ld_field(gq + ((long long)m << sh2));
+        line_fft<LG2, false, false>(v);
+        cplx* p = tile + i0 + i3 * S2;
+#pragma unroll
+        for (int m = 0; m < L2; m++) p[m * S1] = v[m];
+    }
+    __syncthreads();
+    // phase 2: lines along axis 3, one per (i0, i2): forward, filter X~ = (p2max / (V p2)) Delta~ at the stored positions
+    // (zero mode -> 0), inverse                                                                  [north_star step 2]
+#pragma unroll 1
+    for (int ln = threadIdx.x; ln < C0 * L2; ln += NT) {
+        const int i0 = ln % C0, i2 = ln / C0;
+        cplx* p = tile + i0 + i2 * S1;
+        cplx v[L3];
+#pragma unroll
+        for (int m = 0; m < L3; m++) v[m] = p[m * S2];
+        line_fft<LG3, true, false>(v);
+        const double s012 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1] + s2[i2];
+#pragma unroll
+        for (int m = 0; m < L3; m++) {
+            const double p2 = s012 + s3[m];
+            v[m] = cscale(v[m], (real)((p2 > 0.0) ? scale / p2 : 0.0));
+        }
+        line_fft<LG3, true, true>(v);
+#pragma unroll
+        for (int m = 0; m < L3; m++) p[m * S2] = v[m];
+    }
+    __syncthreads();
+    // phase 3: lines along axis 2 again: inverse, straight to global memory
+#pragma unroll 1
+    for (int ln = threadIdx.x; ln < C0 * L3; ln += NT) {
+        const int i0 = ln % C0, i3 = ln / C0;
+        const cplx* p = tile + i0 + i3 * S2;
+        cplx v[L2];
+#pragma unroll
+        for (int m = 0; m < L2; m++) v[m] = p[m * S1];
+        line_fft<LG2, false, true>(v);
+        cplx* gq = gbase + i0 + ((long long)i3 << sh3);
+#pragma unroll
+        for (int m = 0; m < L2; m++) st_field(gq + ((long long)m << sh2), v[m]);
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // Ping-pong persistent passes.  With one work item per CTA every resident CTA starts together and stays in phase:
 // all of them read global memory at once, then all of them sit in the shared-memory stages with HBM idle (measured

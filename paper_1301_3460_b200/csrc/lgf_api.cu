@@ -85,13 +85,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE,
-    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_NSLOTS
+    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd",
-    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad", "k_fa_fwd1", "k_fa_inv1"};
+    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid"};
 
 constexpr int HIST_CAP = 1 << 16;
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
@@ -189,7 +189,7 @@ struct lgf_ctx {
     int acc_g;              // fp32 build: the update also accumulates Gacc(x) <- g(x) Gacc(x) in gbuf
     int mixed_n32;          // fp32 iterations of the last mixed lgf_fix
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel, opt_line;
     int sms;                // SMs of the device: grid of the persistent passes
     int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
@@ -401,6 +401,17 @@ void launch_fa_mid(lgf_ctx* c) {
 #undef X
 }
 
+// pass B with whole lines in registers (fft_fast.cuh k_fr_mid): 16/32 extents
+void launch_fr_mid(lgf_ctx* c) {
+    LaunchScope ls(c, K_FR_MID);
+    const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
+    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
+#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
+        launch_k(c, k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT>, grid, LGF_FR_NT, c->smem_fb, c->field, c->G, c->T, scale, c->ctl);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+
 // persistent ping-pong forms of the three passes (fft_fast.cuh): one CTA per SM, two groups of FA_NT threads
 unsigned pp_grid(const lgf_ctx* c, long long items) { return (unsigned)(items < c->sms ? items : c->sms); }
 template <int NC> void launch_pp_delta_fwd(lgf_ctx* c) {
@@ -455,6 +466,7 @@ lgf_status setup_fast(lgf_ctx* c) {
     }
     if (c->fast_b) {
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) { CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb)); \
+            CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT>, c->smem_fb)); \
             if (c->pp_b_ok) CK(set_smem(k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, c->smem_pb)); }
         LGF_FAST_PAIRS(X)
 #undef X
@@ -601,7 +613,17 @@ template <int NC> void enqueue_head(lgf_ctx* c) {
     launch_finalize(c, np);
 }
 // pass B, pass C, update
-void launch_mid(lgf_ctx* c) { if (use_pp_b(c)) launch_pp_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c); }
+bool use_line_b(const lgf_ctx* c) { return c->opt_line && use_fast_b(c) && fast_pair(c->G.lg[2], c->G.lg[3]); }
+void launch_mid_once(lgf_ctx* c);
+void launch_mid(lgf_ctx* c) {
+    launch_mid_once(c);
+#ifdef LGF_DBG_MID2          // timing experiment: a second pass B right behind the first (field then L2-resident)
+    launch_mid_once(c);
+#endif
+}
+void launch_mid_once(lgf_ctx* c) {
+    if (use_pp_b(c)) launch_pp_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
+}
 void launch_inv_x(lgf_ctx* c) {
     if (use_pp_c(c)) launch_pp_inv(c); else if (use_fast_c(c)) launch_fa_inv(c); else if (use_big_p(c)) launch_fa_inv1(c);
     else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, 0.0);
@@ -664,7 +686,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28) ^ ((c->G.nd == 3) << 29);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28) ^ ((c->G.nd == 3) << 29) ^ (c->opt_line << 30);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -734,7 +756,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_line = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
     c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0;
@@ -1069,6 +1091,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_QUAD_UPDATE: c->opt_quad = value ? 1 : 0; break;
         case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
+        case LGF_OPT_LINE_FFT: c->opt_line = value ? 1 : 0; break;
         case LGF_OPT_GAUGE_DIRECTIONS: {
             if (value != 3 && value != 4) return LGF_ERR_INVALID_ARG;
             c->G.nd = value;
@@ -1095,6 +1118,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
+        case LGF_OPT_LINE_FFT: *value = (use_line_b(c) && !use_pp_b(c)) ? 1 : 0; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;
         case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;

@@ -27,10 +27,10 @@ def all_variants(gf):
     """Every kernel selection the library offers:
     (fuse Delta into FFT pass A, store g, CUDA graph, compile-time-sized FFT passes, fused update + next Delta
     [, ping-pong mask of the persistent passes; default 0 [, S5 inside pass A; default 0
-    [, one thread per link in S3/S4; default 1]]])."""
+    [, one thread per link in S3/S4; default 1 [, pass B with whole lines in registers; default 1]]]])."""
     if gf.V > (1 << 18):
         return [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 0, 0), (0, 1, 1, 1, 0), (0, 0, 0, 0, 0),
-                (1, 0, 1, 1, 0, 0, 0, 0)]
+                (1, 0, 1, 1, 0, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 1, 0)]
     out = []
     for fast in (1, 0):
         for fuse in (1, 0):
@@ -41,6 +41,7 @@ def all_variants(gf):
     # the persistent ping-pong passes, all or one at a time; S5 inside pass A
     out += [(1, 0, 1, 1, 0, 7), (0, 0, 0, 1, 0, 7), (1, 0, 1, 1, 0, 1), (1, 0, 1, 1, 0, 2), (1, 0, 0, 1, 0, 4), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 1, 0, 0, 1)]
     out += [(1, 0, 1, 1, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]      # one thread per site in S3/S4
+    out += [(1, 0, 1, 1, 0, 0, 0, 1, 0), (0, 1, 0, 1, 0, 0, 0, 1, 0)]   # stage-wise pass B
     return out
 
 
@@ -53,6 +54,7 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_PINGPONG, v[5] if len(v) > 5 else 0)
     gf.set_option(lgf.LGF_OPT_FUSE_FINALIZE, v[6] if len(v) > 6 else 0)
     gf.set_option(lgf.LGF_OPT_QUAD_UPDATE, v[7] if len(v) > 7 else 1)
+    gf.set_option(lgf.LGF_OPT_LINE_FFT, v[8] if len(v) > 8 else 1)
 
 
 # ------------------------------------------------------------------ boundary: load -> get
@@ -164,7 +166,8 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
     assert hist_ref[n_ref, 1] < TOL, "oracle did not converge inside the trajectory"
 
     gf = lgf.GaugeFixer(dims, storage)
-    for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (0, 1, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 0)]:
+    for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (0, 1, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 0),
+              (1, 0, 1, 1, 0, 0, 0, 1, 0)]:
         set_variant(gf, v)
         gf.load_links(U)
         done = 0
