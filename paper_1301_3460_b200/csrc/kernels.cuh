@@ -96,6 +96,52 @@ __global__ void __launch_bounds__(128) k_delta(const cplx* __restrict__ links, c
     if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
 }
 
+// S1 with one thread per link pair: a CTA is 4 warps = the 4 directions of 32 consecutive sites.  Thread (x, mu) loads
+// U_mu(x-mu) and U_mu(x) (12 loads instead of 48 per thread: more resident warps, shorter dependency chains), forms the
+// packed contribution of the pair to Delta(x) and hands it over through shared memory; thread (x, c) then sums the four
+// directions of packed component c and writes it: 4 coalesced V-arrays.  In Coulomb gauge the mu = 3 warp contributes 0.
+#ifndef LGF_DELTAQ_MINB
+#define LGF_DELTAQ_MINB 8
+#endif
+template <int NC>
+__global__ void __launch_bounds__(128, LGF_DELTAQ_MINB) k_delta_quad(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
+                                                                    Geom G, const Ctl* __restrict__ ctl) {
+    pdl_enter();
+    if (ctl->done) return;
+    __shared__ cplx sc[4][4][32];          // [direction][packed component][site]
+    __shared__ double red[64];
+    const int lane = threadIdx.x & 31, mu = threadIdx.x >> 5;
+    double th = 0, fs = 0;
+#pragma unroll 1
+    for (int it = 0; it < 4; it++) {       // 4 groups of 32 sites per CTA: one partial per 128 sites, as k_delta
+        const long long x = ((long long)blockIdx.x * 4 + it) * 32 + lane;
+        cplx d01 = mk(0, 0), d02 = mk(0, 0), d12 = mk(0, 0);
+        real i0 = 0, i1 = 0, i2 = 0, retr = 0;
+        if (mu < G.nd) {
+            cplx u[9];
+            load_link<NC>(links, G.V, mu, x, u);
+            retr = u[0].x + u[4].x + u[8].x;
+            acc_link(u, real(-1), d01, d02, d12, i0, i1, i2);
+            load_link<NC>(links, G.V, mu, bwd(G, x, mu), u);
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
+        }
+        // the diagonal part is linear too: e_j = 2 i_j - (2/3)(i0 + i1 + i2)
+        const real tr3 = real(2.0 / 3.0) * (i0 + i1 + i2);
+        if (it) __syncthreads();           // the previous group's sums have been read
+        sc[mu][0][lane] = d01; sc[mu][1][lane] = d02; sc[mu][2][lane] = d12;
+        sc[mu][3][lane] = mk(real(2) * i0 - tr3, real(2) * i1 - tr3);
+        __syncthreads();
+        const int c = mu;                  // this thread now owns packed component c of site x
+        const cplx f = cadd(cadd(sc[0][c][lane], sc[1][c][lane]), cadd(sc[2][c][lane], sc[3][c][lane]));
+        field[(long long)c * G.V + x] = f;
+        if (c < 3) th += (double)(real(2) * cnorm2(f));
+        else { const real e2 = -(f.x + f.y); th += (double)(f.x * f.x + f.y * f.y + e2 * e2); }
+        fs += (double)retr;
+    }
+    block_sum2(th, fs, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
+}
+
 // ------------------------------------------------------------------------------------------------ S5
 // One block.  Sums the partials in a fixed order (strided per thread, then tree), writes F, theta, history,
 // and raises the stop flag: theta < theta_tol (converged), or max_iter updates applied, or non-finite.

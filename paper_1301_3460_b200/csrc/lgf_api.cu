@@ -189,7 +189,7 @@ struct lgf_ctx {
     int acc_g;              // fp32 build: the update also accumulates Gacc(x) <- g(x) Gacc(x) in gbuf
     int mixed_n32;          // fp32 iterations of the last mixed lgf_fix
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel, opt_line;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel, opt_line, opt_delta_quad;
     int sms;                // SMs of the device: grid of the persistent passes
     int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
@@ -553,6 +553,7 @@ lgf_status build_tables(lgf_ctx* c) {
 // ---- kernel launchers ---------------------------------------------------------------------------------------
 template <int NC> void launch_delta(lgf_ctx* c) {
     LaunchScope ls(c, K_DELTA);
+    if (c->opt_delta_quad) { launch_k(c, k_delta_quad<NC>, (unsigned)(c->G.V / 128), 128, 0, cur_links(c), c->field, c->partials, c->G, c->ctl); return; }
     launch_k(c, k_delta<NC>, (unsigned)(c->G.V / 128), 128, 0, cur_links(c), c->field, c->partials, c->G, c->ctl);
 }
 template <int MODE, int NC> void launch_fft01(lgf_ctx* c, int slot, double half_alpha) {
@@ -686,7 +687,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28) ^ ((c->G.nd == 3) << 29) ^ (c->opt_line << 30);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28) ^ ((c->G.nd == 3) << 29) ^ (c->opt_line << 30) ^ (c->opt_delta_quad << 19);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -756,7 +757,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_line = 1;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_line = 1; c->opt_delta_quad = 0;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
     c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0;
@@ -1092,6 +1093,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
         case LGF_OPT_LINE_FFT: c->opt_line = value ? 1 : 0; break;
+        case LGF_OPT_QUAD_DELTA: c->opt_delta_quad = value ? 1 : 0; break;
         case LGF_OPT_GAUGE_DIRECTIONS: {
             if (value != 3 && value != 4) return LGF_ERR_INVALID_ARG;
             c->G.nd = value;
@@ -1118,6 +1120,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
+        case LGF_OPT_QUAD_DELTA: *value = c->opt_delta_quad; break;
         case LGF_OPT_LINE_FFT: *value = (use_line_b(c) && !use_pp_b(c)) ? 1 : 0; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;
         case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;

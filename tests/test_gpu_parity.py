@@ -30,7 +30,7 @@ def all_variants(gf):
     [, one thread per link in S3/S4; default 1 [, pass B with whole lines in registers; default 1]]]])."""
     if gf.V > (1 << 18):
         return [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 0, 0), (0, 1, 1, 1, 0), (0, 0, 0, 0, 0),
-                (1, 0, 1, 1, 0, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 1, 0)]
+                (1, 0, 1, 1, 0, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 1, 0), (0, 0, 1, 1, 0, 0, 0, 1, 1, 1)]
     out = []
     for fast in (1, 0):
         for fuse in (1, 0):
@@ -42,6 +42,7 @@ def all_variants(gf):
     out += [(1, 0, 1, 1, 0, 7), (0, 0, 0, 1, 0, 7), (1, 0, 1, 1, 0, 1), (1, 0, 1, 1, 0, 2), (1, 0, 0, 1, 0, 4), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 1, 0, 0, 1)]
     out += [(1, 0, 1, 1, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]      # one thread per site in S3/S4
     out += [(1, 0, 1, 1, 0, 0, 0, 1, 0), (0, 1, 0, 1, 0, 0, 0, 1, 0)]   # stage-wise pass B
+    out += [(0, 0, 1, 1, 0, 0, 0, 1, 1, 1), (0, 0, 0, 0, 0, 0, 0, 0, 1, 1)]   # S1 as its own kernel with one thread per link pair
     return out
 
 
@@ -55,6 +56,7 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_FUSE_FINALIZE, v[6] if len(v) > 6 else 0)
     gf.set_option(lgf.LGF_OPT_QUAD_UPDATE, v[7] if len(v) > 7 else 1)
     gf.set_option(lgf.LGF_OPT_LINE_FFT, v[8] if len(v) > 8 else 1)
+    gf.set_option(lgf.LGF_OPT_QUAD_DELTA, v[9] if len(v) > 9 else 0)
 
 
 # ------------------------------------------------------------------ boundary: load -> get
