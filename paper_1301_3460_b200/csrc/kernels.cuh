@@ -53,14 +53,15 @@ __device__ __forceinline__ void acc_link(const cplx (&u)[9], real sg, cplx& d01,
 }
 
 // Delta(x) packed, plus this site's contributions to theta (Tr[Delta Delta^dag]) and F (sum_mu Re Tr U_mu(x)).
-template <int NC>
-__device__ __forceinline__ void delta_site(const cplx* __restrict__ links, const Geom& G, long long x,
-                                           cplx& f0, cplx& f1, cplx& f2, cplx& f3, double& th, double& fs) {
+// ND = directions of the gauge condition (4 Landau, 3 Coulomb), a template parameter so that the loop over mu unrolls
+// with all its loads free to be scheduled together (a run-time bound cost the fp32 pass A 17 %).
+template <int NC, int ND>
+__device__ __forceinline__ void delta_site_nd(const cplx* __restrict__ links, const Geom& G, long long x,
+                                              cplx& f0, cplx& f1, cplx& f2, cplx& f3, double& th, double& fs) {
     cplx d01 = mk(0, 0), d02 = mk(0, 0), d12 = mk(0, 0);
     real i0 = 0, i1 = 0, i2 = 0, retr = 0;
 #pragma unroll
-    for (int mu = 0; mu < 4; mu++) {
-        if (mu >= G.nd) break;                       // Coulomb gauge: the condition runs over mu = 0..2
+    for (int mu = 0; mu < ND; mu++) {
         cplx u[9];
         load_link<NC>(links, G.V, mu, x, u);
         retr += u[0].x + u[4].x + u[8].x;
@@ -79,6 +80,12 @@ __device__ __forceinline__ void delta_site(const cplx* __restrict__ links, const
     f0 = d01; f1 = d02; f2 = d12; f3 = mk(e0, e1);
     th = (double)(real(2) * (cnorm2(d01) + cnorm2(d02) + cnorm2(d12)) + e0 * e0 + e1 * e1 + e2 * e2);
     fs = (double)retr;
+}
+template <int NC>
+__device__ __forceinline__ void delta_site(const cplx* __restrict__ links, const Geom& G, long long x,
+                                           cplx& f0, cplx& f1, cplx& f2, cplx& f3, double& th, double& fs) {
+    if (G.nd == 4) delta_site_nd<NC, 4>(links, G, x, f0, f1, f2, f3, th, fs);
+    else delta_site_nd<NC, 3>(links, G, x, f0, f1, f2, f3, th, fs);      // Coulomb gauge: the condition runs over mu = 0..2
 }
 
 template <int NC>
