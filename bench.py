@@ -56,6 +56,7 @@ def kernel_bytes_per_site(nc: int, cb: int = 16) -> dict:
         "k_finalize": 0,
         # compile-time-sized passes (fft_fast.cuh): same traffic as the generic passes they replace
         "k_fa_delta_fwd": lk + fld,
+        "k_cl_delta_fwd": lk + fld,          # 64 x 64 planes: S1 + pass A on CTA pairs
         "k_fa_mid": 2 * fld,
         "k_fr_mid": 2 * fld,                 # pass B with whole lines in registers: same traffic
         "k_fa_inv": 2 * fld,

@@ -162,12 +162,16 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_QUAD_DELTA      1: where S1 is a kernel of its own (64-extent planes, LGF_OPT_FUSE_DELTA_FFT = 0, plain
  *                           steepest descent, lgf_measure) it runs with one thread per link pair (k_delta_quad:
  *                           4 directions x 32 sites per CTA step, contributions summed through shared memory),
- *                           0 (default; measured faster): one thread per site (k_delta). */
+ *                           0 (default; measured faster): one thread per site (k_delta).
+ *   LGF_OPT_CLUSTER_PASS_A  1 (default): on 64 x 64 (x0,x1) planes S1 is fused into FFT pass A on CTA pairs (thread-block
+ *                           clusters of 2: each CTA keeps two of the four component tiles and writes the other two
+ *                           into its partner's shared memory; k_cl_delta_fwd), needs LGF_OPT_FUSE_DELTA_FFT = 1;
+ *                           0: S1 as its own kernel + one-component plane passes.  get: whether it runs. */
 typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
                LGF_OPT_FUSE_UPDATE = 5, LGF_OPT_PINGPONG = 6, LGF_OPT_FUSE_FINALIZE = 7,
                LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9, LGF_OPT_FOURIER_ACCEL = 10,
                LGF_OPT_MIXED_FP32_ITERS = 11 /* read-only */, LGF_OPT_GAUGE_DIRECTIONS = 12, LGF_OPT_LINE_FFT = 13,
-               LGF_OPT_QUAD_DELTA = 14 } lgf_option;
+               LGF_OPT_QUAD_DELTA = 14, LGF_OPT_CLUSTER_PASS_A = 15 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

@@ -20,7 +20,7 @@ __all__ = [
     "LGF_OK", "LGF_NOT_CONVERGED", "LGF_FP64", "LGF_FP32", "LGF_MIXED", "LGF_STORE_12", "LGF_STORE_18",
     "LGF_FIELD_DELTA", "LGF_FIELD_X", "LGF_FIELD_G",
     "LGF_OPT_FUSE_DELTA_FFT", "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_FAST_FFT", "LGF_OPT_FUSE_UPDATE",
-    "LGF_OPT_PINGPONG", "LGF_OPT_FUSE_FINALIZE", "LGF_OPT_QUAD_UPDATE", "LGF_OPT_PDL", "LGF_OPT_FOURIER_ACCEL", "LGF_OPT_MIXED_FP32_ITERS", "LGF_OPT_GAUGE_DIRECTIONS", "LGF_OPT_LINE_FFT", "LGF_OPT_QUAD_DELTA",
+    "LGF_OPT_PINGPONG", "LGF_OPT_FUSE_FINALIZE", "LGF_OPT_QUAD_UPDATE", "LGF_OPT_PDL", "LGF_OPT_FOURIER_ACCEL", "LGF_OPT_MIXED_FP32_ITERS", "LGF_OPT_GAUGE_DIRECTIONS", "LGF_OPT_LINE_FFT", "LGF_OPT_QUAD_DELTA", "LGF_OPT_CLUSTER_PASS_A",
     "EXPORTS",
 ]
 
@@ -38,7 +38,7 @@ LGF_FIELD_DELTA, LGF_FIELD_X, LGF_FIELD_G = 0, 1, 2
 LGF_OPT_FUSE_DELTA_FFT, LGF_OPT_STORE_G, LGF_OPT_GRAPH, LGF_OPT_BATCH, LGF_OPT_FAST_FFT, LGF_OPT_FUSE_UPDATE = 0, 1, 2, 3, 4, 5
 LGF_OPT_PINGPONG, LGF_OPT_FUSE_FINALIZE, LGF_OPT_QUAD_UPDATE, LGF_OPT_PDL, LGF_OPT_FOURIER_ACCEL = 6, 7, 8, 9, 10
 LGF_OPT_MIXED_FP32_ITERS, LGF_OPT_GAUGE_DIRECTIONS, LGF_OPT_LINE_FFT = 11, 12, 13
-LGF_OPT_QUAD_DELTA = 14
+LGF_OPT_QUAD_DELTA, LGF_OPT_CLUSTER_PASS_A = 14, 15
 LGF_MAX_KERNELS = 32
 
 # every symbol include/lgf.h declares (checked by tests/test_abi.py against the header text)

@@ -14,6 +14,7 @@
 // folds into immediates.
 #pragma once
 #include <type_traits>
+#include <cooperative_groups.h>
 #include "kernels.cuh"
 
 // resident CTAs per SM the passes are compiled for (register cap = 65536 / (NT * MINB)).  Measured on B200 at 32^4
@@ -310,6 +311,52 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cp
     return;
 #endif
     plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)blockIdx.x << (LG0 + LG1), g);
+}
+
+// Pass A for 64 x 64 planes on a CTA PAIR (thread-block cluster of 2, distributed shared memory): the four component
+// tiles (266 KB) do not fit one SM, so CTA r of the pair keeps components 2r, 2r+1 (133 KB).  Each CTA computes S1 for
+// half of the plane's rows -- all four components of a site come out of the same eight links -- and writes the two
+// components its partner owns straight into the partner's tile (st.shared::cluster through map_shared_rank).  After
+// one cluster barrier each CTA transforms its two components.  S1 stays fused (no Delta round trip through HBM:
+// 1536 instead of 1664 B/site) and the links are still read once.  Two (theta, F) partials per plane.
+template <int LG0, int LG1, int NC, int NT>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NT, 1)
+k_cl_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials, Geom G, FftTables T,
+               const Ctl* __restrict__ ctl) {
+    pdl_enter();
+    if (ctl->done) return;                               // uniform over the grid: both CTAs of a pair leave together
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1, nP = L0 * L1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw);      // [2][L1][S]
+    cplx* tw0 = tile + 2 * SC;
+    cplx* tw1 = tw0 + L0;
+    __shared__ double red[64];
+    const int r = (int)cluster.block_rank();             // which half of the rows, which pair of components
+    cplx* peer = cluster.map_shared_rank(tile, r ^ 1);
+    const int plane = blockIdx.x >> 1;
+    const long long xbase = (long long)plane << (LG0 + LG1);
+    const Grp g{(int)threadIdx.x, 0};
+    for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
+    for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
+    double th = 0, fs = 0;
+#pragma unroll 1
+    for (int e = r * (nP / 2) + threadIdx.x; e < (r + 1) * (nP / 2); e += NT) {
+        cplx f[4];
+        double t_, f_;
+        delta_site<NC>(links, G, xbase + e, f[0], f[1], f[2], f[3], t_, f_);
+        th += t_; fs += f_;
+        const int o = (e & (L0 - 1)) + (e >> LG0) * S;
+        cplx* own = tile + o;
+        cplx* oth = peer + o;
+        if (r == 0) { own[0] = f[0]; own[SC] = f[1]; oth[0] = f[2]; oth[SC] = f[3]; }
+        else { oth[0] = f[0]; oth[SC] = f[1]; own[0] = f[2]; own[SC] = f[3]; }
+    }
+    block_sum2(th, fs, red);
+    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
+    cluster.sync();                                      // both halves of both tiles are in place (release/acquire)
+    plane_forward_store<LG0, LG1, NT, 2>(tile, tw0, tw1, field + (long long)(2 * r) * G.V, G.V, xbase, g);
 }
 
 // Pass A without S1, for planes whose four component tiles do not fit one SM (64 x 64, 32 x 64): forward FFT over axes

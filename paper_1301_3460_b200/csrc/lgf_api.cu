@@ -85,13 +85,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE,
-    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_NSLOTS
+    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd",
-    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid"};
+    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd"};
 
 constexpr int HIST_CAP = 1 << 16;
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
@@ -189,12 +189,12 @@ struct lgf_ctx {
     int acc_g;              // fp32 build: the update also accumulates Gacc(x) <- g(x) Gacc(x) in gbuf
     int mixed_n32;          // fp32 iterations of the last mixed lgf_fix
     // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel, opt_line, opt_delta_quad;
+    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel, opt_line, opt_delta_quad, opt_cluster;
     int sms;                // SMs of the device: grid of the persistent passes
     int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
     // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
-    bool fast_a, fast_b, fast_c, pp_b_ok, big_p;
-    size_t smem_fa, smem_fb, smem_fc, smem_fu, smem_pa, smem_pb, smem_p1;
+    bool fast_a, fast_b, fast_c, pp_b_ok, big_p, cl_ok;
+    size_t smem_fa, smem_fb, smem_fc, smem_fu, smem_pa, smem_pb, smem_p1, smem_cl;
     int fb_lgC;
     // derived launch parameters
     int fft01_ncomp_fused_ok, fft01_ncomp, fft01_threads, fft23_lgC, fft23_S1, fft23_S2, fft23_threads;
@@ -296,6 +296,10 @@ template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
 constexpr int FA_NT = 256;            // group size of the ping-pong passes
 constexpr int FAD_NT = LGF_FA_NT;     // threads per CTA of pass A (k_fa_delta_fwd)
 constexpr int FC_NT = LGF_FC_NT;      // threads per CTA of pass C (k_fa_inv)
+#ifndef LGF_CL_NT
+#define LGF_CL_NT 256
+#endif
+constexpr int CL_NT = LGF_CL_NT;      // threads per CTA of the CTA-pair pass A (k_cl_delta_fwd)
 // (lg of the fast axis, lg of the slow axis) pairs instantiated for each pass
 #define LGF_FAST_PAIRS(X) X(4, 4) X(4, 5) X(5, 4) X(5, 5)
 #ifndef LGF_FB_LGC55
@@ -363,6 +367,12 @@ void launch_fa_inv_g(lgf_ctx* c, double half_alpha) {
         launch_k(c, k_fa_inv<A, B, 4, FC_NT, true>, grid, FC_NT, c->smem_fc, c->field, c->gbuf, half_alpha, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
+}
+// 64 x 64 planes: S1 fused into pass A on CTA pairs (clusters of 2 sharing the four component tiles over DSMEM)
+template <int NC> void launch_cl_delta_fwd(lgf_ctx* c) {
+    LaunchScope ls(c, K_CL_DELTA_FWD);
+    const unsigned grid = (unsigned)(2 * c->G.L[2] * c->G.L[3]);
+    launch_k(c, k_cl_delta_fwd<6, 6, NC, CL_NT>, grid, CL_NT, c->smem_cl, cur_links(c), c->field, c->partials, c->G, c->T, c->ctl);
 }
 // planes with a 64 extent: one component per CTA
 void launch_fa_fwd1(lgf_ctx* c) {
@@ -473,6 +483,13 @@ lgf_status setup_fast(lgf_ctx* c) {
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb));
         LGF_BIG_PAIRS(X)
 #undef X
+    }
+    c->cl_ok = false;
+    if (c->big_p && G.lg[0] == 6 && G.lg[1] == 6) {
+        c->smem_cl = smem_fast_plane(6, 6, 2);
+        c->cl_ok = set_smem(k_cl_delta_fwd<6, 6, 6, CL_NT>, c->smem_cl) == cudaSuccess &&
+                   set_smem(k_cl_delta_fwd<6, 6, 9, CL_NT>, c->smem_cl) == cudaSuccess;
+        if (!c->cl_ok) cudaGetLastError();
     }
     if (c->big_p) {
 #define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
@@ -599,6 +616,7 @@ bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
 bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c && !use_store_g(c); }
 bool use_fused_update(const lgf_ctx* c) { return c->opt_accel && c->G.nd == 4 && c->opt_fuse_update && c->opt_fast && c->fast_a; }
 bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p && !use_store_g(c); }
+bool use_cluster_a(const lgf_ctx* c) { return use_big_p(c) && c->cl_ok && c->opt_cluster && c->opt_fuse; }
 bool use_pp_a(const lgf_ctx* c) { return (c->opt_pingpong & 1) && use_fast_a(c); }
 bool use_pp_b(const lgf_ctx* c) { return (c->opt_pingpong & 2) && use_fast_b(c) && c->pp_b_ok; }
 bool use_pp_c(const lgf_ctx* c) { return (c->opt_pingpong & 4) && use_fast_c(c); }
@@ -608,6 +626,7 @@ template <int NC> void enqueue_head(lgf_ctx* c) {
     int np;
     if (use_pp_a(c)) { launch_pp_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
     else if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c, c->opt_fuse_fin != 0); if (c->opt_fuse_fin) return; np = c->G.L[2] * c->G.L[3]; }
+    else if (use_cluster_a(c)) { launch_cl_delta_fwd<NC>(c); np = 2 * c->G.L[2] * c->G.L[3]; }
     else if (use_big_p(c)) { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fa_fwd1(c); }
     else if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
     else { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fft01<MODE_FWD, 6>(c, K_FFT01_FWD, 0.0); }
@@ -656,6 +675,7 @@ bool use_fused_fin(const lgf_ctx* c) { return c->opt_fuse_fin && use_fast_a(c) &
 int launches_per_body(const lgf_ctx* c) {
     if (!c->opt_accel) return 3;
     if (use_fused_update(c) || use_fused_fin(c)) return 4;
+    if (use_cluster_a(c)) return 5;
     if (use_big_p(c) && !use_fast_a(c) && !use_pp_a(c)) return 6;
     return use_fused(c) ? 5 : 6;
 }
@@ -687,7 +707,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     union { double d; unsigned long long u; } au; au.d = half_alpha;
     // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
     const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28) ^ ((c->G.nd == 3) << 29) ^ (c->opt_line << 30) ^ (c->opt_delta_quad << 19);
+                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28) ^ ((c->G.nd == 3) << 29) ^ (c->opt_line << 30) ^ (c->opt_delta_quad << 19) ^ (c->opt_cluster << 18);
     if (!c->graph_exec || c->graph_key != key) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -757,7 +777,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_line = 1; c->opt_delta_quad = 0;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_line = 1; c->opt_delta_quad = 0; c->opt_cluster = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
     c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0;
@@ -1094,6 +1114,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
         case LGF_OPT_LINE_FFT: c->opt_line = value ? 1 : 0; break;
         case LGF_OPT_QUAD_DELTA: c->opt_delta_quad = value ? 1 : 0; break;
+        case LGF_OPT_CLUSTER_PASS_A: c->opt_cluster = value ? 1 : 0; break;
         case LGF_OPT_GAUGE_DIRECTIONS: {
             if (value != 3 && value != 4) return LGF_ERR_INVALID_ARG;
             c->G.nd = value;
@@ -1121,6 +1142,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
         case LGF_OPT_QUAD_DELTA: *value = c->opt_delta_quad; break;
+        case LGF_OPT_CLUSTER_PASS_A: *value = use_cluster_a(c) ? 1 : 0; break;
         case LGF_OPT_LINE_FFT: *value = (use_line_b(c) && !use_pp_b(c)) ? 1 : 0; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;
         case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;

@@ -43,6 +43,7 @@ def all_variants(gf):
     out += [(1, 0, 1, 1, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]      # one thread per site in S3/S4
     out += [(1, 0, 1, 1, 0, 0, 0, 1, 0), (0, 1, 0, 1, 0, 0, 0, 1, 0)]   # stage-wise pass B
     out += [(0, 0, 1, 1, 0, 0, 0, 1, 1, 1), (0, 0, 0, 0, 0, 0, 0, 0, 1, 1)]   # S1 as its own kernel with one thread per link pair
+    out += [(1, 0, 1, 1, 0, 0, 0, 1, 1, 0, 0)]                               # 64 x 64 planes without the CTA-pair pass A
     return out
 
 
@@ -57,6 +58,7 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_QUAD_UPDATE, v[7] if len(v) > 7 else 1)
     gf.set_option(lgf.LGF_OPT_LINE_FFT, v[8] if len(v) > 8 else 1)
     gf.set_option(lgf.LGF_OPT_QUAD_DELTA, v[9] if len(v) > 9 else 0)
+    gf.set_option(lgf.LGF_OPT_CLUSTER_PASS_A, v[10] if len(v) > 10 else 1)
 
 
 # ------------------------------------------------------------------ boundary: load -> get
@@ -713,6 +715,7 @@ def test_fast_fft_pass_selection_64_extents():
     for dims, mask in [((64, 64, 4, 4), 5), ((4, 4, 64, 64), 2), ((32, 64, 32, 64), 7), ((8, 8, 64, 32), 2), ((64, 32, 16, 16), 7)]:
         gf = lgf.GaugeFixer(dims, 12)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
+        assert gf.get_option(lgf.LGF_OPT_CLUSTER_PASS_A) == (1 if dims[:2] == (64, 64) else 0), dims
         gf.destroy()
 
 
