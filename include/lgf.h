@@ -133,11 +133,14 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *                           and shared-memory phases (fft_fast.cuh); 0 bits: one work item per CTA.
  *                           lgf_get_option returns the mask of the passes that run this way.  Default 0: measured on
  *                           B200 the strict alternation is slower for pass A and neutral for B and C.
- *   LGF_OPT_FUSE_FINALIZE   1: with the compile-time-sized pass A, the CTA that finishes S1 last also does the final
- *                           theta/F reduction and the S5 stop test (one launch fewer per iteration; the summation
- *                           order, hence the result, is that of the separate k_finalize), 0 (default: the gpu-scope
- *                           fence it needs costs pass A more than the launch it saves): k_finalize.
- *                           lgf_get_option returns whether it applies.
+ *   LGF_OPT_FUSE_FINALIZE   where the final theta/F reduction and the S5 stop test run.  0: k_finalize, a one-CTA kernel
+ *                           between S1 and pass B.  2 (default): inside the first CTA of pass B, where pass B is one of
+ *                           the compile-time-sized kernels -- the partials are complete when pass B starts, pass B
+ *                           itself does not need the decision, pass C and the update see it: one launch fewer per
+ *                           iteration, no fence.  1: inside the CTA of the compile-time-sized pass A that finishes
+ *                           S1 last (needs a gpu-scope fence per CTA, which costs pass A more than the launch it
+ *                           saves).  Summation order as in k_finalize up to the CTA's thread count.
+ *                           lgf_get_option returns the mode that runs.
  *   LGF_OPT_QUAD_UPDATE     1 (default): S3+S4 with one thread per link, the four directions of 32 sites per CTA, g(x)
  *                           taken from the thread that built it as g((x-0)+0) (4 Gram-Schmidt per site, k_update_quad),
  *                           0: one thread per site (5 Gram-Schmidt per site, k_update).  Applies when g is recomputed

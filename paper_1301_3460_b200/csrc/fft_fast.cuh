@@ -254,16 +254,9 @@ __device__ __forceinline__ void pass_a_delta(const cplx* __restrict__ links, con
 // thread, then the fixed tree: the result is bit-identical), writes F, theta and the history and raises the stop flag.
 // Every CTA of the grid has passed its ctl->done test by then, and the next kernel starts after this one ends.
 struct FinArgs { double2* hist; double inv3V, inv12V; int on; };
+// The reduction and the S5 decision by one whole CTA (all its threads call this).
 template <int NT>
-__device__ __forceinline__ void finalize_last_cta(const double2* partials, int n, Ctl* ctl, const FinArgs& fa, double* red) {
-    __shared__ int is_last;
-    if (threadIdx.x == 0) {
-        __threadfence();                                   // this CTA's partial is visible before its ticket
-        is_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!is_last) return;
-    __threadfence();
+__device__ __forceinline__ void finalize_cta(const double2* partials, int n, Ctl* ctl, const FinArgs& fa, double* red) {
     double a = 0, b = 0;
     for (int i = threadIdx.x; i < n; i += NT) { const double2 p = __ldcg(partials + i); a += p.x; b += p.y; }
     block_sum2(a, b, red);
@@ -278,6 +271,27 @@ __device__ __forceinline__ void finalize_last_cta(const double2* partials, int n
         else if (ctl->iters >= ctl->max_iter) { ctl->done = 1; }
     }
     __syncthreads();
+}
+template <int NT>
+__device__ __forceinline__ void finalize_last_cta(const double2* partials, int n, Ctl* ctl, const FinArgs& fa, double* red) {
+    __shared__ int is_last;
+    if (threadIdx.x == 0) {
+        __threadfence();                                   // this CTA's partial is visible before its ticket
+        is_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    finalize_cta<NT>(partials, n, ctl, fa, red);
+}
+// S5 inside pass B (LGF_OPT_FUSE_FINALIZE = 2): the partials of pass A are complete when pass B starts, so its CTA 0 does
+// the reduction and the stop decision before its own tile -- no k_finalize launch, no fence.  Pass B itself never needs
+// the decision (it only transforms the scratch field; a CTA that already sees the flag may skip its tile, which nobody
+// reads once the flag is up); pass C and the update start after this kernel has ended and see it.
+template <int NT>
+__device__ __forceinline__ void finalize_in_pass_b(const double2* partials, const FinArgs& fa, Ctl* ctl) {
+    __shared__ double red_fin[64];
+    if (fa.on > 0 && blockIdx.x == 0) finalize_cta<NT>(partials, fa.on, ctl, fa, red_fin);
 }
 
 // Pass A: S1 (Delta, theta/F partials) + forward FFT over axes 0,1 of one (x2,x3) plane, all 4 components.
@@ -649,9 +663,10 @@ __device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01,
 
 // Pass B: forward over axes 2,3, filter, inverse over axes 3,2, one work item per CTA.
 template <int LG2, int LG3, int LGC, int NT>
-__global__ void __launch_bounds__(NT, (NT > 256) ? 1 : LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+__global__ void __launch_bounds__(NT, (NT > 256) ? 1 : LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
     if (ctl->done) return;
+    finalize_in_pass_b<NT>(partials, fa, ctl);           // fa.on = number of partials, 0: k_finalize ran
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0;
     static_assert(NT % C0 == 0, "a thread keeps its x0 offset");
@@ -759,9 +774,10 @@ __device__ __forceinline__ void line_fft(cplx (&v)[1 << LG]) {
 #define LGF_FR_MINB 2
 #endif
 template <int LG2, int LG3, int LGC, int NT>
-__global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
+__global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
     if (ctl->done) return;
+    finalize_in_pass_b<NT>(partials, fa, ctl);           // fa.on = number of partials, 0: k_finalize ran
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
     extern __shared__ __align__(16) unsigned char smem_raw[];

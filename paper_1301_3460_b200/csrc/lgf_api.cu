@@ -188,6 +188,7 @@ struct lgf_ctx {
     char* shadow_ws;        // its workspace when this context allocated it
     int acc_g;              // fp32 build: the update also accumulates Gacc(x) <- g(x) Gacc(x) in gbuf
     int mixed_n32;          // fp32 iterations of the last mixed lgf_fix
+    int pending_np;         // S5 inside pass B: partials of the S1 just enqueued that no k_finalize has reduced yet
     // options
     int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel, opt_line, opt_delta_quad, opt_cluster;
     int sms;                // SMs of the device: grid of the persistent passes
@@ -401,12 +402,19 @@ template <int NC> void launch_fu_update(lgf_ctx* c) {
     LGF_FAST_PAIRS(X)
 #undef X
 }
+// S5 inside pass B: the pending number of partials of the S1 that just ran (0: k_finalize already did it)
+FinArgs pending_fin(lgf_ctx* c) {
+    const FinArgs fa{c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (3.0 * (double)c->G.nd * (double)c->G.V), c->pending_np};
+    c->pending_np = 0;
+    return fa;
+}
 void launch_fa_mid(lgf_ctx* c) {
     LaunchScope ls(c, K_FA_MID);
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
     const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
+    const FinArgs fa = pending_fin(c);
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        launch_k(c, k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, grid, fast_mid_nt(A, B), c->smem_fb, c->field, c->G, c->T, scale, c->ctl);
+        launch_k(c, k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, grid, fast_mid_nt(A, B), c->smem_fb, c->field, c->G, c->T, scale, c->ctl, c->partials, fa);
     LGF_FAST_PAIRS(X) LGF_BIG_PAIRS(X)
 #undef X
 }
@@ -416,8 +424,9 @@ void launch_fr_mid(lgf_ctx* c) {
     LaunchScope ls(c, K_FR_MID);
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
     const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
+    const FinArgs fa = pending_fin(c);
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        launch_k(c, k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT>, grid, LGF_FR_NT, c->smem_fb, c->field, c->G, c->T, scale, c->ctl);
+        launch_k(c, k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT>, grid, LGF_FR_NT, c->smem_fb, c->field, c->G, c->T, scale, c->ctl, c->partials, fa);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -621,15 +630,18 @@ bool use_pp_a(const lgf_ctx* c) { return (c->opt_pingpong & 1) && use_fast_a(c);
 bool use_pp_b(const lgf_ctx* c) { return (c->opt_pingpong & 2) && use_fast_b(c) && c->pp_b_ok; }
 bool use_pp_c(const lgf_ctx* c) { return (c->opt_pingpong & 4) && use_fast_c(c); }
 
+// S5 inside pass B's first CTA: LGF_OPT_FUSE_FINALIZE = 2, where pass B is one of the compile-time-sized kernels
+bool use_fin_b(const lgf_ctx* c) { return c->opt_fuse_fin == 2 && c->opt_accel && use_fast_b(c) && !use_pp_b(c) && !use_fused_update(c); }
 // S1 (+ pass A) and the reduction.  Returns the number of partials written.
 template <int NC> void enqueue_head(lgf_ctx* c) {
     int np;
     if (use_pp_a(c)) { launch_pp_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
-    else if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c, c->opt_fuse_fin != 0); if (c->opt_fuse_fin) return; np = c->G.L[2] * c->G.L[3]; }
+    else if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c, c->opt_fuse_fin == 1); if (c->opt_fuse_fin == 1) return; np = c->G.L[2] * c->G.L[3]; }
     else if (use_cluster_a(c)) { launch_cl_delta_fwd<NC>(c); np = 2 * c->G.L[2] * c->G.L[3]; }
     else if (use_big_p(c)) { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fa_fwd1(c); }
     else if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
     else { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fft01<MODE_FWD, 6>(c, K_FFT01_FWD, 0.0); }
+    if (use_fin_b(c)) { c->pending_np = np; return; }     // pass B's CTA 0 reduces them (every head here is followed by a pass B)
     launch_finalize(c, np);
 }
 // pass B, pass C, update
@@ -671,13 +683,16 @@ void enqueue_body(lgf_ctx* c, double half_alpha) {
     if (c->NC == 6) { enqueue_head<6>(c); enqueue_tail<6>(c, half_alpha); }
     else { enqueue_head<9>(c); enqueue_tail<9>(c, half_alpha); }
 }
-bool use_fused_fin(const lgf_ctx* c) { return c->opt_fuse_fin && use_fast_a(c) && !use_pp_a(c); }
+bool use_fused_fin(const lgf_ctx* c) { return (c->opt_fuse_fin == 1 && use_fast_a(c) && !use_pp_a(c)) || use_fin_b(c); }
 int launches_per_body(const lgf_ctx* c) {
     if (!c->opt_accel) return 3;
-    if (use_fused_update(c) || use_fused_fin(c)) return 4;
-    if (use_cluster_a(c)) return 5;
-    if (use_big_p(c) && !use_fast_a(c) && !use_pp_a(c)) return 6;
-    return use_fused(c) ? 5 : 6;
+    if (use_fused_update(c)) return 4;
+    int n;                                               // with a k_finalize launch
+    if (use_pp_a(c) || use_fast_a(c) || use_cluster_a(c)) n = 5;
+    else if (use_big_p(c)) n = 6;
+    else n = use_fused(c) ? 5 : 6;
+    if (use_fused_fin(c)) n -= 1;                        // S5 inside pass A's last CTA or pass B's first
+    return n;
 }
 
 lgf_status reset_ctl(lgf_ctx* c, double tol, int max_iter) {
@@ -777,10 +792,10 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 0; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_line = 1; c->opt_delta_quad = 0; c->opt_cluster = 1;
+    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 2; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_line = 1; c->opt_delta_quad = 0; c->opt_cluster = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->parity = 0;
-    c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0;
+    c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0; c->pending_np = 0;
     c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
     c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
@@ -1108,7 +1123,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_FAST_FFT: c->opt_fast = value ? 1 : 0; break;
         case LGF_OPT_FUSE_UPDATE: c->opt_fuse_update = value ? 1 : 0; break;
         case LGF_OPT_PINGPONG: if (value < 0 || value > 7) return LGF_ERR_INVALID_ARG; c->opt_pingpong = value; break;
-        case LGF_OPT_FUSE_FINALIZE: c->opt_fuse_fin = value ? 1 : 0; break;
+        case LGF_OPT_FUSE_FINALIZE: if (value < 0 || value > 2) return LGF_ERR_INVALID_ARG; c->opt_fuse_fin = value; break;
         case LGF_OPT_QUAD_UPDATE: c->opt_quad = value ? 1 : 0; break;
         case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
@@ -1137,7 +1152,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_FAST_FFT: *value = ((use_fast_a(c) || use_big_p(c)) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | ((use_fast_c(c) || use_big_p(c)) ? 4 : 0); break;
         case LGF_OPT_FUSE_UPDATE: *value = use_fused_update(c) ? 1 : 0; break;
         case LGF_OPT_PINGPONG: *value = (use_pp_a(c) ? 1 : 0) | (use_pp_b(c) ? 2 : 0) | (use_pp_c(c) ? 4 : 0); break;
-        case LGF_OPT_FUSE_FINALIZE: *value = use_fused_fin(c) ? 1 : 0; break;
+        case LGF_OPT_FUSE_FINALIZE: *value = use_fin_b(c) ? 2 : ((c->opt_fuse_fin == 1 && use_fast_a(c) && !use_pp_a(c)) ? 1 : 0); break;
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;

@@ -26,7 +26,7 @@ def theta_close(t_gpu, t_ref):
 def all_variants(gf):
     """Every kernel selection the library offers:
     (fuse Delta into FFT pass A, store g, CUDA graph, compile-time-sized FFT passes, fused update + next Delta
-    [, ping-pong mask of the persistent passes; default 0 [, S5 inside pass A; default 0
+    [, ping-pong mask of the persistent passes; default 0 [, where S5 runs: 0 k_finalize, 1 pass A, 2 pass B; default 2
     [, one thread per link in S3/S4; default 1 [, pass B with whole lines in registers; default 1]]]])."""
     if gf.V > (1 << 18):
         return [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 0, 0), (0, 1, 1, 1, 0), (0, 0, 0, 0, 0),
@@ -40,7 +40,8 @@ def all_variants(gf):
     out += [(1, 0, 1, 1, 1), (1, 0, 0, 1, 1)]       # the fused update needs the fast passes; the other switches do not enter
     # the persistent ping-pong passes, all or one at a time; S5 inside pass A
     out += [(1, 0, 1, 1, 0, 7), (0, 0, 0, 1, 0, 7), (1, 0, 1, 1, 0, 1), (1, 0, 1, 1, 0, 2), (1, 0, 0, 1, 0, 4), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 1, 0, 0, 1)]
-    out += [(1, 0, 1, 1, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]      # one thread per site in S3/S4
+    out += [(1, 0, 1, 1, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]      # one thread per site in S3/S4 (and k_finalize)
+    out += [(1, 0, 1, 1, 0, 0, 0), (0, 0, 0, 1, 0, 0, 0), (1, 1, 1, 1, 0, 0, 0)]   # k_finalize as a kernel of its own
     out += [(1, 0, 1, 1, 0, 0, 0, 1, 0), (0, 1, 0, 1, 0, 0, 0, 1, 0)]   # stage-wise pass B
     out += [(0, 0, 1, 1, 0, 0, 0, 1, 1, 1), (0, 0, 0, 0, 0, 0, 0, 0, 1, 1)]   # S1 as its own kernel with one thread per link pair
     out += [(1, 0, 1, 1, 0, 0, 0, 1, 1, 0, 0)]                               # 64 x 64 planes without the CTA-pair pass A
@@ -54,7 +55,7 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_FAST_FFT, v[3])
     gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, v[4])
     gf.set_option(lgf.LGF_OPT_PINGPONG, v[5] if len(v) > 5 else 0)
-    gf.set_option(lgf.LGF_OPT_FUSE_FINALIZE, v[6] if len(v) > 6 else 0)
+    gf.set_option(lgf.LGF_OPT_FUSE_FINALIZE, v[6] if len(v) > 6 else 2)
     gf.set_option(lgf.LGF_OPT_QUAD_UPDATE, v[7] if len(v) > 7 else 1)
     gf.set_option(lgf.LGF_OPT_LINE_FFT, v[8] if len(v) > 8 else 1)
     gf.set_option(lgf.LGF_OPT_QUAD_DELTA, v[9] if len(v) > 9 else 0)
@@ -170,7 +171,7 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
     assert hist_ref[n_ref, 1] < TOL, "oracle did not converge inside the trajectory"
 
     gf = lgf.GaugeFixer(dims, storage)
-    for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (0, 1, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 0),
+    for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (1, 0, 1, 1, 0, 0, 0), (0, 1, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 0),
               (1, 0, 1, 1, 0, 0, 0, 1, 0)]:
         set_variant(gf, v)
         gf.load_links(U)
