@@ -27,6 +27,16 @@
 #ifndef LGF_FA_NOBLOCK16
 #define LGF_FA_NOBLOCK16 0
 #endif
+// 1: pass A prefetches the own links of a thread's next site into L2 (prefetch.global.L2) before it works on the current
+// one.  Measured on B200 at 32^4: fp32 61.5 against 65.8 us, fp64 115.5 against 106 us (the extra L1TEX requests cost
+// more than the latency they save) -- so it is on in the fp32 build only.
+#ifndef LGF_FA_PREFETCH_NEXT
+#ifdef LGF_F32
+#define LGF_FA_PREFETCH_NEXT 1
+#else
+#define LGF_FA_PREFETCH_NEXT 0
+#endif
+#endif
 #ifndef LGF_FA_MINB_MID
 #define LGF_FA_MINB_MID 2
 #endif
@@ -240,6 +250,13 @@ __device__ __forceinline__ void pass_a_delta(const cplx* __restrict__ links, con
     for (int e = g.tid; e < nP; e += NT) {
         cplx f0, f1, f2, f3;
         double t_, f_;
+#if LGF_FA_PREFETCH_NEXT
+        if (e + NT < nP) {               // own links of this thread's next site: DRAM -> L2 while this site is computed
+            const cplx* q = links + xbase + e + NT;
+#pragma unroll
+            for (int k = 0; k < 4 * NC; k++) prefetch_line_l2(q + (long long)k * G.V);
+        }
+#endif
         delta_site<NC>(links, G, xbase + e, f0, f1, f2, f3, t_, f_);
         th += t_; fs += f_;
         const int o = (e & (L0 - 1)) + (e >> LG0) * S;

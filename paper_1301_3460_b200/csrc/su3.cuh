@@ -111,6 +111,10 @@ __device__ __forceinline__ void prefetch_l2(const void* p, unsigned bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
+// Line prefetch into L2 (no destination register): used to pull a thread's NEXT site towards the SM while it works on
+// the current one, so that the later loads see L2 latency instead of DRAM latency.
+__device__ __forceinline__ void prefetch_line_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // Load link (x, mu) from the structure-of-arrays store: entry c of direction mu is the V-array at
 // links + (mu*NC + c)*V, NC = 6 (12-real: rows 0,1) or 9 (18-real).  Row 2 is rebuilt for NC = 6.
 template <int NC>
