@@ -374,6 +374,16 @@ __global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __res
 // A CTA covers whole x0 rows (NS = max(32, L0) sites, 4 NS threads), so the site x-0 is always in the same CTA.
 // Measured on B200 at 32^4 (CUDA events per launch): 149 us at 5 CTAs/SM (96 registers), 157 at 4, 157 at 6 (spills),
 // against 161 for one thread per site (k_update<NC,0>, 12 warps/SM); the IEEE 1/sqrt costs nothing measurable.
+// > 0: each thread prefetches into L2 the link its counterpart that many CTAs ahead will load.  Measured on B200 at 32^4
+// with 740 (= one resident wave of 5 CTAs x 148 SMs): fp32 83.7 against 87.7 us, fp64 148.3 against 145 us (1480: 153,
+// 2960: 169) -- on in the fp32 build only.
+#ifndef LGF_UPDQ_PREFETCH
+#ifdef LGF_F32
+#define LGF_UPDQ_PREFETCH 740
+#else
+#define LGF_UPDQ_PREFETCH 0
+#endif
+#endif
 #ifndef LGF_UPDQ_MINB64
 #define LGF_UPDQ_MINB64 3
 #endif
@@ -393,6 +403,16 @@ __global__ void __launch_bounds__(4 * NS, (NS == 32) ? LGF_UPDQ_MINB : ((NS == 6
     const long long x = (long long)blockIdx.x * NS + st;
     const long long xf = fwd(G, x, mu);
     cplx g[9], gp[9], u[9], r[9];
+#if LGF_UPDQ_PREFETCH
+    {   // the link this thread's counterpart LGF_UPDQ_PREFETCH CTAs ahead will load: DRAM -> L2 now
+        const long long xp = x + (long long)LGF_UPDQ_PREFETCH * NS;
+        if (xp < V) {
+            const cplx* q = links + (long long)(mu * NC) * V + xp;
+#pragma unroll
+            for (int c = 0; c < NC; c++) prefetch_line_l2(q + (long long)c * V);
+        }
+    }
+#endif
     load_link<NC>(links, V, mu, x, u);
     build_g(ldc_field(src + xf), ldc_field(src + V + xf), ldc_field(src + 2 * V + xf), ldc_field(src + 3 * V + xf), (real)half_alpha, gp);
     if (mu == 0) {
