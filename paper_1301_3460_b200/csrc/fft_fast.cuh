@@ -251,7 +251,7 @@ __device__ __forceinline__ void pass_a_delta(const cplx* __restrict__ links, con
         cplx f0, f1, f2, f3;
         double t_, f_;
 #if LGF_FA_PREFETCH_NEXT
-        if (e + NT < nP) {               // own links of this thread's next site: DRAM -> L2 while this site is computed
+        if (e + NT < nP && prefetch_lane()) {   // own links of this thread's next site: DRAM -> L2 while this site is computed
             const cplx* q = links + xbase + e + NT;
 #pragma unroll
             for (int k = 0; k < 4 * NC; k++) prefetch_line_l2(q + (long long)k * G.V);

@@ -406,7 +406,7 @@ __global__ void __launch_bounds__(4 * NS, (NS == 32) ? LGF_UPDQ_MINB : ((NS == 6
 #if LGF_UPDQ_PREFETCH
     {   // the link this thread's counterpart LGF_UPDQ_PREFETCH CTAs ahead will load: DRAM -> L2 now
         const long long xp = x + (long long)LGF_UPDQ_PREFETCH * NS;
-        if (xp < V) {
+        if (xp < V && prefetch_lane()) {
             const cplx* q = links + (long long)(mu * NC) * V + xp;
 #pragma unroll
             for (int c = 0; c < NC; c++) prefetch_line_l2(q + (long long)c * V);

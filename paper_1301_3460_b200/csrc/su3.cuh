@@ -114,6 +114,13 @@ __device__ __forceinline__ void prefetch_l2(const void* p, unsigned bytes) {
 // Line prefetch into L2 (no destination register): used to pull a thread's NEXT site towards the SM while it works on
 // the current one, so that the later loads see L2 latency instead of DRAM latency.
 __device__ __forceinline__ void prefetch_line_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// true for one lane per 128-byte line of consecutive complex numbers (lanes run over consecutive sites)
+#ifndef LGF_PF_ONE_PER_LINE
+#define LGF_PF_ONE_PER_LINE 0
+#endif
+__device__ __forceinline__ bool prefetch_lane() {
+    return !LGF_PF_ONE_PER_LINE || (threadIdx.x & (128 / (int)sizeof(cplx) - 1)) == 0;
+}
 
 // Load link (x, mu) from the structure-of-arrays store: entry c of direction mu is the V-array at
 // links + (mu*NC + c)*V, NC = 6 (12-real: rows 0,1) or 9 (18-real).  Row 2 is rebuilt for NC = 6.
