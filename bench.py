@@ -226,7 +226,7 @@ def run_ours(args):
         return max_over_ranks(x, dist, "cuda")
 
     import ensembles as E
-    device_links = args.links == "device"
+    device_links = args.links in ("device", "wilson")
     if device_links:
         # seeded links generated on the device (ensembles.device_su3): for the large shapes (C3, C4), whose host recipe
         # takes minutes; throughput does not depend on the configuration.  No end-to-end leg, no CPU baseline.
@@ -243,7 +243,10 @@ def run_ours(args):
     if args.fuse_update is not None:
         gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, args.fuse_update)
     if device_links:
-        d_in = E.device_su3(dims, cfg["seed"] + 100 * rank, 0.15)
+        if args.links == "wilson":
+            d_in = E.wilson(dims, args.beta, args.sweeps, cfg["seed"] + 100 * rank, device="cuda")
+        else:
+            d_in = E.device_su3(dims, cfg["seed"] + 100 * rank, 0.15)
         h_in = h_out = None
 
         def reload():
@@ -373,7 +376,7 @@ def run_ours(args):
             "metric": METRIC.replace("fp64", "fp32") if fp32 else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if fp32 else "f64", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, " + ("device-generated links (ensembles.device_su3)" if device_links else f"eps={cfg.get('eps')}") + f", seed={cfg['seed']}, alpha=0.08",
+            "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, " + ((f"Wilson-action heat bath beta={args.beta}, {args.sweeps} sweeps (ensembles.wilson)" if args.links == "wilson" else "device-generated links (ensembles.device_su3)") if device_links else f"eps={cfg.get('eps')}") + f", seed={cfg['seed']}, alpha=0.08",
                        "iterations_per_step": inner, "l2": "inputs larger than L2 (links %.0f MB + field %.0f MB per GPU)" % (V * nc * 64 / 1e6, V * 64 / 1e6),
                        "parallelism": "replicas" if world > 1 else "single"},
             "e2e": None if device_links else {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": V * 576, "d2h_bytes_per_step": V * 576 + 16,
@@ -411,9 +414,12 @@ def main():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
                     help="fp64: the BASELINE.json metric (default); fp32: LGF_FP32 storage and arithmetic (SURVEY.md 8(f) NEXT-1), "
                          "reported with dtype f32 and its own byte model; time_to_theta then stops at theta < 1e-10")
-    ap.add_argument("--links", default="host", choices=["host", "device"],
+    ap.add_argument("--beta", type=float, default=6.0, help="--links wilson: coupling of the Wilson action")
+    ap.add_argument("--sweeps", type=int, default=20, help="--links wilson: heat-bath sweeps from a cold start")
+    ap.add_argument("--links", default="host", choices=["host", "device", "wilson"],
                     help="host: the seeded BASELINE.json ensemble built with numpy (default); device: seeded links generated on the GPU "
-                         "(large shapes C3, C4; no e2e leg, no CPU baseline)")
+                         "(large shapes C3, C4; no e2e leg, no CPU baseline); wilson: a thermalised Wilson-action configuration generated on the GPU "
+                         "(ensembles.wilson: the kind of input the paper fixes), for time_to_theta on realistic links")
     ap.add_argument("--fuse-update", type=int, default=None, choices=[0, 1],
                     help="override LGF_OPT_FUSE_UPDATE (kernel A/B timing); default: the library's choice")
     args = ap.parse_args()

@@ -42,6 +42,7 @@ __all__ = [
     "as_real",
     "as_complex",
     "device_su3",
+    "wilson",
 ]
 
 # Gell-Mann matrices lambda_1..lambda_8
@@ -211,3 +212,11 @@ def device_su3(dims, seed: int, spread: float = 0.15):
         U[o:o + m, 1] = v
         U[o:o + m, 2] = torch.linalg.cross(u, v).conj()
     return U.reshape(V, 4, 3, 3)
+
+
+def wilson(dims, beta: float, sweeps: int, seed: int, device: str = "cpu", hot: bool = False):
+    """Thermalised Wilson-action configuration (ensembles/heatbath.py: Cabibbo-Marinari heat bath, Kennedy-Pendleton
+    SU(2) updates) -- the kind of input the paper fixes, at a beta of the caller's choice.  Returns a
+    torch complex128 tensor [V, 4, 3, 3] on `device` (use .cpu().numpy() for the host entry points)."""
+    from .heatbath import thermalise
+    return thermalise(dims, beta, sweeps, seed, device=device, hot=hot)

@@ -363,6 +363,38 @@ def test_plain_steepest_descent_variant(dims, storage):
     assert th < href[-1, 1]                                              # Fourier acceleration converges faster
 
 
+# ------------------------------------------------------------------ thermalised Wilson-action inputs
+@pytest.mark.parametrize("dims,beta", [((8, 8, 8, 8), 5.8), ((16, 16, 16, 16), 6.0)])
+def test_trajectory_on_thermalised_wilson_configuration(dims, beta):
+    """The kind of input the paper fixes (Wilson action): a heat-bath configuration (ensembles.wilson,
+    generated on the device, fed to both sides as the same host array).  Whole trajectory against the oracle with the
+    north-star tolerances -- here theta is far from its rounding floor for the whole run, so the relative theta bound
+    bites at every iteration -- the stop iteration exactly, the links at the end; mixed precision reaches the same F."""
+    from ensembles import heatbath as H
+    Ud = E.wilson(dims, beta, 20, 7, device="cuda")
+    assert 0.55 < H.average_plaquette(Ud, dims) < 0.62          # thermalised around beta = 6: 0.57 .. 0.60
+    U = Ud.cpu().numpy()
+    o = oracle.Oracle(dims, 12, fft_mode=1)
+    o.load(U)
+    r_ref = o.fix(ALPHA, TOL, 5000, history=True)
+    href = np.array(r_ref["history"])
+    assert r_ref["status"] == 0 and r_ref["n_iter"] > 30
+    gf = lgf.GaugeFixer(dims, 12)
+    for v in [(1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]:
+        set_variant(gf, v)
+        gf.load_links(U)
+        r = gf.fix(ALPHA, TOL, 5000)
+        h = gf.get_history()
+        assert r["status"] == lgf.LGF_OK and r["n_iter"] == r_ref["n_iter"], (v, r, r_ref["n_iter"])
+        assert len(h) == len(href) and np.abs(h[:, 0] - href[:, 0]).max() <= F_TOL, v
+        assert all(theta_close(a, b) for a, b in zip(h[:, 1], href[:, 1])), v
+        assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL, v
+    gm = lgf.GaugeFixer(dims, 12, precision=lgf.LGF_MIXED)
+    gm.load_links(U)
+    rm = gm.fix(ALPHA, TOL, 5000)
+    assert rm["status"] == lgf.LGF_OK and rm["theta"] < TOL and abs(rm["F"] - r_ref["F"]) <= 1e-11
+
+
 # ------------------------------------------------------------------ Coulomb gauge (SURVEY.md section 8(f) NEXT-3)
 @pytest.mark.parametrize("dims,storage", [((8, 8, 8, 8), 18), ((16, 16, 16, 8), 12), ((32, 32, 16, 16), 12), ((4, 8, 16, 4), 12)])
 def test_coulomb_gauge_against_the_oracle(dims, storage):
