@@ -364,15 +364,18 @@ def test_plain_steepest_descent_variant(dims, storage):
 
 
 # ------------------------------------------------------------------ thermalised Wilson-action inputs
-@pytest.mark.parametrize("dims,beta", [((8, 8, 8, 8), 5.8), ((16, 16, 16, 16), 6.0)])
-def test_trajectory_on_thermalised_wilson_configuration(dims, beta):
+@pytest.mark.parametrize("dims,beta,sweeps,seed", [((8, 8, 8, 8), 5.8, 20, 7), ((16, 16, 16, 16), 6.0, 20, 7),
+                                                  ((8, 8, 8, 8), 5.7, 40, 8), ((16, 16, 16, 16), 5.7, 40, 7)])
+def test_trajectory_on_thermalised_wilson_configuration(dims, beta, sweeps, seed):
     """The kind of input the paper fixes (Wilson action): a heat-bath configuration (ensembles.wilson,
     generated on the device, fed to both sides as the same host array).  Whole trajectory against the oracle with the
     north-star tolerances -- here theta is far from its rounding floor for the whole run, so the relative theta bound
-    bites at every iteration -- the stop iteration exactly, the links at the end; mixed precision reaches the same F."""
+    bites at every iteration -- the stop iteration exactly, the links at the end; mixed precision reaches the same F.
+    The beta = 5.7 cases are rough configurations that need 221 and 383 iterations: the trajectory stays within the
+    tolerances over hundreds of iterations (reading A16: the iteration is a well-conditioned map)."""
     from ensembles import heatbath as H
-    Ud = E.wilson(dims, beta, 20, 7, device="cuda")
-    assert 0.55 < H.average_plaquette(Ud, dims) < 0.62          # thermalised around beta = 6: 0.57 .. 0.60
+    Ud = E.wilson(dims, beta, sweeps, seed, device="cuda")
+    assert 0.53 < H.average_plaquette(Ud, dims) < 0.62          # thermalised around beta = 5.7 .. 6: 0.55 .. 0.60
     U = Ud.cpu().numpy()
     o = oracle.Oracle(dims, 12, fft_mode=1)
     o.load(U)
