@@ -304,7 +304,11 @@ constexpr int CL_NT = LGF_CL_NT;      // threads per CTA of the CTA-pair pass A 
 // (lg of the fast axis, lg of the slow axis) pairs instantiated for each pass
 #define LGF_FAST_PAIRS(X) X(4, 4) X(4, 5) X(5, 4) X(5, 5)
 #ifndef LGF_FB_LGC55
+#ifdef LGF_F32_LGC55
+#define LGF_FB_LGC55 LGF_F32_LGC55
+#else
 #define LGF_FB_LGC55 2
+#endif
 #endif
 #ifndef LGF_FB_NT
 #define LGF_FB_NT 256
