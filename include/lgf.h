@@ -156,7 +156,8 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_GAUGE_DIRECTIONS 4 (default): Landau gauge, the paper's problem.  3: Coulomb gauge -- the gauge
  *                           condition, Delta, F (normalised by 3 N_c V) and p^2 run over mu = 0..2 only, p2max = 12, the
  *                           spatial zero mode of every time slice is dropped, all four link directions are transformed.
- *                           Same kernels; the transform along axis 3 is a no-op pair kept for simplicity.
+ *                           Same kernels; the transform pair along axis 3 cancels -- k_fr_mid skips it (every axis-2 line
+ *                           is finished in registers), the other pass-B kernels keep it as a no-op pair.
  *                           LGF_OPT_FUSE_UPDATE is Landau only and is ignored in Coulomb gauge.
  *   LGF_OPT_LINE_FFT        1 (default): FFT pass B on extents 16/32 keeps whole lines in registers (one thread = one line
  *                           of an axis, twiddles as instruction operands; the tile is written and read twice per point

@@ -790,7 +790,7 @@ __device__ __forceinline__ void line_fft(cplx (&v)[1 << LG]) {
 #ifndef LGF_FR_MINB
 #define LGF_FR_MINB 2
 #endif
-template <int LG2, int LG3, int LGC, int NT>
+template <int LG2, int LG3, int LGC, int NT, bool COULOMB = false>
 __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
     if (ctl->done) return;
@@ -809,6 +809,30 @@ __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ f
     const int comp = blockIdx.x >> (lgChunks + G.lg[1]);
     cplx* gbase = field + (long long)comp * G.V + (chunk << LGC) + ((long long)x1 << G.sh[1]);
     const int sh2 = G.sh[2], sh3 = G.sh[3];
+    if constexpr (COULOMB) {
+        // Coulomb gauge: the filter does not depend on the axis-3 momentum, so the transform pair along axis 3 cancels and
+        // every axis-2 line is finished on its own: forward, filter, inverse in registers, no shared memory, no barrier
+        __syncthreads();                                     // s2 is complete
+#pragma unroll 1
+        for (int ln = threadIdx.x; ln < C0 * L3; ln += NT) {
+            const int i0 = ln % C0, i3 = ln / C0;
+            cplx* gq = gbase + i0 + ((long long)i3 << sh3);
+            cplx v[L2];
+#pragma unroll
+            for (int m = 0; m < L2; m++) v[m] = ld_field(gq + ((long long)m << sh2));
+            line_fft<LG2, false, false>(v);
+            const double s01 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1];
+#pragma unroll
+            for (int m = 0; m < L2; m++) {
+                const double p2 = s01 + s2[m];
+                v[m] = cscale(v[m], (real)((p2 > 0.0) ? scale * (double)L3 / p2 : 0.0));      // no 1/L3: axis 3 is not transformed
+            }
+            line_fft<LG2, false, true>(v);
+#pragma unroll
+            for (int m = 0; m < L2; m++) st_field(gq + ((long long)m << sh2), v[m]);
+        }
+        return;
+    }
     // phase 1: lines along axis 2, one per (i0, i3)
 #pragma unroll 1
     for (int ln = threadIdx.x; ln < C0 * L3; ln += NT) {

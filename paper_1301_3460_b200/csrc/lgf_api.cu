@@ -429,8 +429,9 @@ void launch_fr_mid(lgf_ctx* c) {
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
     const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
     const FinArgs fa = pending_fin(c);
-#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        launch_k(c, k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT>, grid, LGF_FR_NT, c->smem_fb, c->field, c->G, c->T, scale, c->ctl, c->partials, fa);
+#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) { \
+        if (c->G.nd == 3) launch_k(c, k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, true>, grid, LGF_FR_NT, c->smem_fb, c->field, c->G, c->T, scale, c->ctl, c->partials, fa); \
+        else launch_k(c, k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, false>, grid, LGF_FR_NT, c->smem_fb, c->field, c->G, c->T, scale, c->ctl, c->partials, fa); }
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -489,7 +490,8 @@ lgf_status setup_fast(lgf_ctx* c) {
     }
     if (c->fast_b) {
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) { CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb)); \
-            CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT>, c->smem_fb)); \
+            CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, false>, c->smem_fb)); \
+            CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, true>, c->smem_fb)); \
             if (c->pp_b_ok) CK(set_smem(k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, c->smem_pb)); }
         LGF_FAST_PAIRS(X)
 #undef X
