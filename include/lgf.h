@@ -162,7 +162,8 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_LINE_FFT        1 (default): FFT pass B on extents 16/32 keeps whole lines in registers (one thread = one line
  *                           of an axis, twiddles as instruction operands; the tile is written and read twice per point
  *                           instead of four times, two barriers instead of five; k_fr_mid), 0: the stage-wise pass B
- *                           (k_fa_mid).  lgf_get_option returns whether it runs.
+ *                           (k_fa_mid), 2: half a line per thread, lane pairs exchanging by shuffle (k_fh_mid; Landau
+ *                           only; measured slower).  lgf_get_option returns the form that runs.
  *   LGF_OPT_QUAD_DELTA      1: where S1 is a kernel of its own (64-extent planes, LGF_OPT_FUSE_DELTA_FFT = 0, plain
  *                           steepest descent, lgf_measure) it runs with one thread per link pair (k_delta_quad:
  *                           4 directions x 32 sites per CTA step, contributions summed through shared memory),

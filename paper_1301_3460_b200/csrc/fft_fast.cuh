@@ -884,6 +884,176 @@ __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ f
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Pass B with HALF a line per thread: two adjacent lanes (h = 0, 1) share a line of L = R1 R2 points.  Stage 1 needs no
+// exchange (lane h takes the butterflies ja in [h R2/2, (h+1) R2/2)); before stage 2 the pair swaps half of its values
+// through one round of shuffles so that lane h owns the complete blocks ba in [h R1/2, (h+1) R1/2).  Half the registers
+// of k_fr_mid per thread (16 points instead of 32), hence twice the resident warps.
+//   "stage-1 layout":  a[jl][k]  <->  position (h J + jl) + k R2,      J = R2/2, jl < J, k < R1
+//   "stage-2 layout":  b[kl][j]  <->  position (h K + kl) R2 + j,      K = R1/2, kl < K, j < R2
+template <int LG> __device__ __forceinline__ cplx ctw_rt(int k) {       // run-time index: constant-cache load
+    if constexpr (LG == 4) return mk(c_tw16[k][0], c_tw16[k][1]);
+    else return mk(c_tw32[k][0], c_tw32[k][1]);
+}
+__device__ __forceinline__ cplx shfl_pair(cplx v) {
+    return mk(__shfl_xor_sync(0xffffffffu, v.x, 1), __shfl_xor_sync(0xffffffffu, v.y, 1));
+}
+__device__ __forceinline__ cplx csel(bool c, cplx a, cplx b) { return mk(c ? a.x : b.x, c ? a.y : b.y); }
+
+template <int LG, bool B>
+__device__ __forceinline__ void half_fft_forward(const cplx (&a)[(1 << LG) / 2], cplx (&b)[(1 << LG) / 2], int h) {
+    using P = Plan2<LG, B>;
+    constexpr int R1 = P::R1, R2 = P::R2, J = R2 / 2, K = R1 / 2;
+    cplx s[J][R1];
+#pragma unroll
+    for (int jl = 0; jl < J; jl++) {
+        cplx x[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) x[k] = a[jl * R1 + k];
+        bfly<R1, false>(x);
+        const int ja = h * J + jl;
+#pragma unroll
+        for (int k = 1; k < R1; k++) x[k] = cmul(x[k], ctw_rt<LG>(k * ja));
+#pragma unroll
+        for (int k = 0; k < R1; k++) s[jl][k] = x[k];
+    }
+#pragma unroll
+    for (int kl = 0; kl < K; kl++) {
+        cplx x[R2];
+#pragma unroll
+        for (int jl = 0; jl < J; jl++) {
+            const cplx keep = csel(h, s[jl][K + kl], s[jl][kl]);
+            const cplx recv = shfl_pair(csel(h, s[jl][kl], s[jl][K + kl]));
+            x[jl] = csel(h, recv, keep);
+            x[J + jl] = csel(h, keep, recv);
+        }
+        bfly<R2, false>(x);
+#pragma unroll
+        for (int j = 0; j < R2; j++) b[kl * R2 + j] = x[j];
+    }
+}
+template <int LG, bool B>
+__device__ __forceinline__ void half_fft_inverse(const cplx (&b)[(1 << LG) / 2], cplx (&a)[(1 << LG) / 2], int h) {
+    using P = Plan2<LG, B>;
+    constexpr int R1 = P::R1, R2 = P::R2, J = R2 / 2, K = R1 / 2;
+    cplx s[J][R1];
+#pragma unroll
+    for (int kl = 0; kl < K; kl++) {
+        cplx x[R2];
+#pragma unroll
+        for (int j = 0; j < R2; j++) x[j] = b[kl * R2 + j];
+        bfly<R2, true>(x);
+#pragma unroll
+        for (int jl = 0; jl < J; jl++) {
+            const cplx keep = csel(h, x[J + jl], x[jl]);
+            const cplx recv = shfl_pair(csel(h, x[jl], x[J + jl]));
+            s[jl][kl] = csel(h, recv, keep);
+            s[jl][K + kl] = csel(h, keep, recv);
+        }
+    }
+#pragma unroll
+    for (int jl = 0; jl < J; jl++) {
+        cplx x[R1];
+#pragma unroll
+        for (int k = 0; k < R1; k++) x[k] = s[jl][k];
+        const int ja = h * J + jl;
+#pragma unroll
+        for (int k = 1; k < R1; k++) x[k] = cmulc(x[k], ctw_rt<LG>(k * ja));
+        bfly<R1, true>(x);
+#pragma unroll
+        for (int k = 0; k < R1; k++) a[jl * R1 + k] = x[k];
+    }
+}
+
+#ifndef LGF_FH_MINB
+#define LGF_FH_MINB 2
+#endif
+template <int LG2, int LG3, int LGC, int NT>
+__global__ void __launch_bounds__(NT, LGF_FH_MINB) k_fh_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
+    pdl_enter();
+    if (ctl->done) return;
+    finalize_in_pass_b<NT>(partials, fa, ctl);
+    using MG = MidGeom<LG2, LGC>;
+    using P2 = Plan2<LG2, false>;
+    using P3 = Plan2<LG3, true>;
+    constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
+    constexpr int J2 = P2::R2 / 2, K2 = P2::R1 / 2, J3 = P3::R2 / 2, K3 = P3::R1 / 2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw);
+    double* s2 = reinterpret_cast<double*>(tile + S2 * L3);
+    double* s3 = s2 + L2;
+    for (int i = threadIdx.x; i < L2; i += NT) s2[i] = T.s[2][i];
+    for (int i = threadIdx.x; i < L3; i += NT) s3[i] = T.s[3][i];
+    const int lgChunks = G.lg[0] - LGC;
+    const int chunk = blockIdx.x & ((1 << lgChunks) - 1);
+    const int x1 = (blockIdx.x >> lgChunks) & (G.L[1] - 1);
+    const int comp = blockIdx.x >> (lgChunks + G.lg[1]);
+    cplx* gbase = field + (long long)comp * G.V + (chunk << LGC) + ((long long)x1 << G.sh[1]);
+    const int sh2 = G.sh[2], sh3 = G.sh[3];
+    const int h = threadIdx.x & 1;
+    // phase 1: axis-2 lines, one per (i0, i3) and lane pair: global -> forward -> tile
+#pragma unroll 1
+    for (int ln = threadIdx.x >> 1; ln < C0 * L3; ln += NT / 2) {
+        const int i0 = ln % C0, i3 = ln / C0;
+        const cplx* gq = gbase + i0 + ((long long)i3 << sh3);
+        cplx a[L2 / 2], b[L2 / 2];
+#pragma unroll
+        for (int jl = 0; jl < J2; jl++)
+#pragma unroll
+            for (int k = 0; k < P2::R1; k++) a[jl * P2::R1 + k] = ld_field(gq + ((long long)((h * J2 + jl) + k * P2::R2) << sh2));
+        half_fft_forward<LG2, false>(a, b, h);
+        cplx* p = tile + i0 + i3 * S2;
+#pragma unroll
+        for (int kl = 0; kl < K2; kl++)
+#pragma unroll
+            for (int j = 0; j < P2::R2; j++) p[((h * K2 + kl) * P2::R2 + j) * S1] = b[kl * P2::R2 + j];
+    }
+    __syncthreads();
+    // phase 2: axis-3 lines, one per (i0, i2) and lane pair: forward, filter at the stored positions, inverse, in place
+#pragma unroll 1
+    for (int ln = threadIdx.x >> 1; ln < C0 * L2; ln += NT / 2) {
+        const int i0 = ln % C0, i2 = ln / C0;
+        cplx* p = tile + i0 + i2 * S1;
+        cplx a[L3 / 2], b[L3 / 2];
+#pragma unroll
+        for (int jl = 0; jl < J3; jl++)
+#pragma unroll
+            for (int k = 0; k < P3::R1; k++) a[jl * P3::R1 + k] = p[((h * J3 + jl) + k * P3::R2) * S2];
+        half_fft_forward<LG3, true>(a, b, h);
+        const double s012 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1] + s2[i2];
+#pragma unroll
+        for (int kl = 0; kl < K3; kl++)
+#pragma unroll
+            for (int j = 0; j < P3::R2; j++) {
+                const double p2 = s012 + s3[(h * K3 + kl) * P3::R2 + j];
+                b[kl * P3::R2 + j] = cscale(b[kl * P3::R2 + j], (real)((p2 > 0.0) ? scale / p2 : 0.0));
+            }
+        half_fft_inverse<LG3, true>(b, a, h);
+#pragma unroll
+        for (int jl = 0; jl < J3; jl++)
+#pragma unroll
+            for (int k = 0; k < P3::R1; k++) p[((h * J3 + jl) + k * P3::R2) * S2] = a[jl * P3::R1 + k];
+    }
+    __syncthreads();
+    // phase 3: axis-2 lines again: tile -> inverse -> global
+#pragma unroll 1
+    for (int ln = threadIdx.x >> 1; ln < C0 * L3; ln += NT / 2) {
+        const int i0 = ln % C0, i3 = ln / C0;
+        const cplx* p = tile + i0 + i3 * S2;
+        cplx a[L2 / 2], b[L2 / 2];
+#pragma unroll
+        for (int kl = 0; kl < K2; kl++)
+#pragma unroll
+            for (int j = 0; j < P2::R2; j++) b[kl * P2::R2 + j] = p[((h * K2 + kl) * P2::R2 + j) * S1];
+        half_fft_inverse<LG2, false>(b, a, h);
+        cplx* gq = gbase + i0 + ((long long)i3 << sh3);
+#pragma unroll
+        for (int jl = 0; jl < J2; jl++)
+#pragma unroll
+            for (int k = 0; k < P2::R1; k++) st_field(gq + ((long long)((h * J2 + jl) + k * P2::R2) << sh2), a[jl * P2::R1 + k]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Ping-pong persistent passes.  With one work item per CTA every resident CTA starts together and stays in phase:
 // all of them read global memory at once, then all of them sit in the shared-memory stages with HBM idle (measured
 // on B200 at 32^4: pass A takes 17.2 us per plane per SM at 1 CTA/SM and 2 x 15.6 at 2 CTAs/SM, i.e. the phases add

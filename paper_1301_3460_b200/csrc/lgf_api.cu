@@ -85,13 +85,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE,
-    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_NSLOTS
+    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_FH_MID, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd",
-    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd"};
+    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_fh_mid"};
 
 constexpr int HIST_CAP = 1 << 16;
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
@@ -424,6 +424,17 @@ void launch_fa_mid(lgf_ctx* c) {
 }
 
 // pass B with whole lines in registers (fft_fast.cuh k_fr_mid): 16/32 extents
+// pass B with half a line per thread (k_fh_mid): LGF_OPT_LINE_FFT = 2
+void launch_fh_mid(lgf_ctx* c) {
+    LaunchScope ls(c, K_FH_MID);
+    const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
+    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
+    const FinArgs fa = pending_fin(c);
+#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
+        launch_k(c, k_fh_mid<A, B, fast_mid_lgC(A, B), 256>, grid, 256, c->smem_fb, c->field, c->G, c->T, scale, c->ctl, c->partials, fa);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
 void launch_fr_mid(lgf_ctx* c) {
     LaunchScope ls(c, K_FR_MID);
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
@@ -491,6 +502,7 @@ lgf_status setup_fast(lgf_ctx* c) {
     if (c->fast_b) {
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) { CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb)); \
             CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, false>, c->smem_fb)); \
+            CK(set_smem(k_fh_mid<A, B, fast_mid_lgC(A, B), 256>, c->smem_fb)); \
             CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, true>, c->smem_fb)); \
             if (c->pp_b_ok) CK(set_smem(k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, c->smem_pb)); }
         LGF_FAST_PAIRS(X)
@@ -660,7 +672,7 @@ void launch_mid(lgf_ctx* c) {
 #endif
 }
 void launch_mid_once(lgf_ctx* c) {
-    if (use_pp_b(c)) launch_pp_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
+    if (use_pp_b(c)) launch_pp_mid(c); else if (use_line_b(c) && c->opt_line == 2 && c->G.nd == 4) launch_fh_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
 }
 void launch_inv_x(lgf_ctx* c) {
     if (use_pp_c(c)) launch_pp_inv(c); else if (use_fast_c(c)) launch_fa_inv(c); else if (use_big_p(c)) launch_fa_inv1(c);
@@ -1133,7 +1145,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_QUAD_UPDATE: c->opt_quad = value ? 1 : 0; break;
         case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
-        case LGF_OPT_LINE_FFT: c->opt_line = value ? 1 : 0; break;
+        case LGF_OPT_LINE_FFT: if (value < 0 || value > 2) return LGF_ERR_INVALID_ARG; c->opt_line = value; break;
         case LGF_OPT_QUAD_DELTA: c->opt_delta_quad = value ? 1 : 0; break;
         case LGF_OPT_CLUSTER_PASS_A: c->opt_cluster = value ? 1 : 0; break;
         case LGF_OPT_GAUGE_DIRECTIONS: {
@@ -1164,7 +1176,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
         case LGF_OPT_QUAD_DELTA: *value = c->opt_delta_quad; break;
         case LGF_OPT_CLUSTER_PASS_A: *value = use_cluster_a(c) ? 1 : 0; break;
-        case LGF_OPT_LINE_FFT: *value = (use_line_b(c) && !use_pp_b(c)) ? 1 : 0; break;
+        case LGF_OPT_LINE_FFT: *value = (use_line_b(c) && !use_pp_b(c)) ? ((c->opt_line == 2 && c->G.nd == 4) ? 2 : 1) : 0; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;
         case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;
         default: return LGF_ERR_INVALID_ARG;

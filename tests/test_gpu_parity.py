@@ -43,6 +43,7 @@ def all_variants(gf):
     out += [(1, 0, 1, 1, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]      # one thread per site in S3/S4 (and k_finalize)
     out += [(1, 0, 1, 1, 0, 0, 0), (0, 0, 0, 1, 0, 0, 0), (1, 1, 1, 1, 0, 0, 0)]   # k_finalize as a kernel of its own
     out += [(1, 0, 1, 1, 0, 0, 0, 1, 0), (0, 1, 0, 1, 0, 0, 0, 1, 0)]   # stage-wise pass B
+    out += [(1, 0, 1, 1, 0, 0, 2, 1, 2), (0, 0, 0, 1, 0, 0, 0, 1, 2)]   # pass B with half a line per thread
     out += [(0, 0, 1, 1, 0, 0, 0, 1, 1, 1), (0, 0, 0, 0, 0, 0, 0, 0, 1, 1)]   # S1 as its own kernel with one thread per link pair
     out += [(1, 0, 1, 1, 0, 0, 0, 1, 1, 0, 0)]                               # 64 x 64 planes without the CTA-pair pass A
     return out
@@ -172,7 +173,7 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
 
     gf = lgf.GaugeFixer(dims, storage)
     for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (1, 0, 1, 1, 0, 0, 0), (0, 1, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 0),
-              (1, 0, 1, 1, 0, 0, 0, 1, 0)]:
+              (1, 0, 1, 1, 0, 0, 0, 1, 0), (1, 0, 1, 1, 0, 0, 2, 1, 2)]:
         set_variant(gf, v)
         gf.load_links(U)
         done = 0
