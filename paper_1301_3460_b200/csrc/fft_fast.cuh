@@ -310,6 +310,15 @@ __device__ __forceinline__ void finalize_in_pass_b(const double2* partials, cons
     __shared__ double red_fin[64];
     if (fa.on > 0 && blockIdx.x == 0) finalize_cta<NT>(partials, fa.on, ctl, fa, red_fin);
 }
+// Entry test of the pass-B kernels.  With S5 inside pass B the stop flag can be raised by CTA 0 WHILE other CTAs of the
+// same kernel start, so the flag must be read once per CTA and broadcast: if every thread read it for itself, the
+// warps of one CTA could disagree and the CTA would hang at its next barrier.
+__device__ __forceinline__ bool pass_b_done(const Ctl* ctl) {
+    __shared__ int s_done;
+    if (threadIdx.x == 0) s_done = *reinterpret_cast<const volatile int*>(&ctl->done);
+    __syncthreads();
+    return s_done != 0;
+}
 
 // Pass A: S1 (Delta, theta/F partials) + forward FFT over axes 0,1 of one (x2,x3) plane, all 4 components.
 template <int LG0, int LG1, int NC, int NT>
@@ -682,7 +691,7 @@ __device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01,
 template <int LG2, int LG3, int LGC, int NT>
 __global__ void __launch_bounds__(NT, (NT > 256) ? 1 : LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
-    if (ctl->done) return;
+    if (pass_b_done(ctl)) return;
     finalize_in_pass_b<NT>(partials, fa, ctl);           // fa.on = number of partials, 0: k_finalize ran
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0;
@@ -793,7 +802,7 @@ __device__ __forceinline__ void line_fft(cplx (&v)[1 << LG]) {
 template <int LG2, int LG3, int LGC, int NT, bool COULOMB = false>
 __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
-    if (ctl->done) return;
+    if (pass_b_done(ctl)) return;
     finalize_in_pass_b<NT>(partials, fa, ctl);           // fa.on = number of partials, 0: k_finalize ran
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
@@ -970,7 +979,7 @@ __device__ __forceinline__ void half_fft_inverse(const cplx (&b)[(1 << LG) / 2],
 template <int LG2, int LG3, int LGC, int NT>
 __global__ void __launch_bounds__(NT, LGF_FH_MINB) k_fh_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
-    if (ctl->done) return;
+    if (pass_b_done(ctl)) return;
     finalize_in_pass_b<NT>(partials, fa, ctl);
     using MG = MidGeom<LG2, LGC>;
     using P2 = Plan2<LG2, false>;
