@@ -305,19 +305,26 @@ __device__ __forceinline__ void finalize_last_cta(const double2* partials, int n
 // the reduction and the stop decision before its own tile -- no k_finalize launch, no fence.  Pass B itself never needs
 // the decision (it only transforms the scratch field; a CTA that already sees the flag may skip its tile, which nobody
 // reads once the flag is up); pass C and the update start after this kernel has ended and see it.
+// Entry of the pass-B kernels.  With S5 inside pass B the stop flag can be raised by CTA 0 WHILE other CTAs of the same
+// kernel start, so a CTA must take ONE reading of it: thread 0 reads it at entry into shared memory, and the CTA acts on
+// it only behind its first regular barrier (PASS_B_EXIT_IF_DONE) -- if every thread read the flag for itself the warps
+// of a CTA could disagree and the CTA would hang at its next barrier, and a barrier of its own right behind
+// griddepcontrol.wait costs 60 us per iteration under programmatic dependent launch (measured).  What a CTA does before
+// that barrier only touches its shared-memory tile.  CTA 0 alone synchronises at once, because it has to know whether the
+// run is already over before it reduces the partials of the S1 that has just run (fa.on of them; 0: k_finalize did it).
 template <int NT>
-__device__ __forceinline__ void finalize_in_pass_b(const double2* partials, const FinArgs& fa, Ctl* ctl) {
+__device__ __forceinline__ void pass_b_entry(const double2* partials, const FinArgs& fa, Ctl* ctl, int* s_done) {
     __shared__ double red_fin[64];
-    if (fa.on > 0 && blockIdx.x == 0) finalize_cta<NT>(partials, fa.on, ctl, fa, red_fin);
-}
-// Entry test of the pass-B kernels.  With S5 inside pass B the stop flag can be raised by CTA 0 WHILE other CTAs of the
-// same kernel start, so the flag must be read once per CTA and broadcast: if every thread read it for itself, the
-// warps of one CTA could disagree and the CTA would hang at its next barrier.
-__device__ __forceinline__ bool pass_b_done(const Ctl* ctl) {
-    __shared__ int s_done;
-    if (threadIdx.x == 0) s_done = *reinterpret_cast<const volatile int*>(&ctl->done);
-    __syncthreads();
-    return s_done != 0;
+    // Every thread reads one word of the control block right behind griddepcontrol.wait and branches on it (hist_cap
+    // never changes while kernels run and is never negative).  Measured: without such a read the first instructions
+    // behind the wait are the field loads of phase 1 and the iteration takes 373 us under programmatic dependent
+    // launch; with it 310 us -- as with the per-thread "if (ctl->done) return" of the other kernels.
+    if (ctl->hist_cap < 0) return;
+    if (threadIdx.x == 0) *s_done = __ldcg(&ctl->done);
+    if (fa.on > 0 && blockIdx.x == 0) {
+        __syncthreads();
+        if (!*s_done) finalize_cta<NT>(partials, fa.on, ctl, fa, red_fin);
+    }
 }
 
 // Pass A: S1 (Delta, theta/F partials) + forward FFT over axes 0,1 of one (x2,x3) plane, all 4 components.
@@ -691,8 +698,8 @@ __device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01,
 template <int LG2, int LG3, int LGC, int NT>
 __global__ void __launch_bounds__(NT, (NT > 256) ? 1 : LGF_FA_MINB_MID) k_fa_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
-    if (pass_b_done(ctl)) return;
-    finalize_in_pass_b<NT>(partials, fa, ctl);           // fa.on = number of partials, 0: k_finalize ran
+    __shared__ int s_done;
+    pass_b_entry<NT>(partials, fa, ctl, &s_done);
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0;
     static_assert(NT % C0 == 0, "a thread keeps its x0 offset");
@@ -708,6 +715,7 @@ __global__ void __launch_bounds__(NT, (NT > 256) ? 1 : LGF_FA_MINB_MID) k_fa_mid
     for (int i = threadIdx.x; i < L2; i += NT) { tw2[i] = T.tw[2][i]; s2[i] = T.s[2][i]; }
     for (int i = threadIdx.x; i < L3; i += NT) { tw3[i] = T.tw[3][i]; s3[i] = T.s[3][i]; }
     __syncthreads();
+    if (s_done) return;                                  // one reading per CTA, behind a barrier (pass_b_entry)
     pass_b_load<LG2, LG3, LGC, NT>(it.gp, G.sh[2], G.sh[3], tile + i0, tw2, g);
     pass_b_finish<LG2, LG3, LGC, NT>(it.gp, it.s01, G.sh[2], G.sh[3], scale, tile + i0, tw2, tw3, s2, s3, g);
 }
@@ -802,8 +810,8 @@ __device__ __forceinline__ void line_fft(cplx (&v)[1 << LG]) {
 template <int LG2, int LG3, int LGC, int NT, bool COULOMB = false>
 __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
-    if (pass_b_done(ctl)) return;
-    finalize_in_pass_b<NT>(partials, fa, ctl);           // fa.on = number of partials, 0: k_finalize ran
+    __shared__ int s_done;
+    pass_b_entry<NT>(partials, fa, ctl, &s_done);
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -822,6 +830,7 @@ __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ f
         // Coulomb gauge: the filter does not depend on the axis-3 momentum, so the transform pair along axis 3 cancels and
         // every axis-2 line is finished on its own: forward, filter, inverse in registers, no shared memory, no barrier
         __syncthreads();                                     // s2 is complete
+        if (s_done) return;
 #pragma unroll 1
         for (int ln = threadIdx.x; ln < C0 * L3; ln += NT) {
             const int i0 = ln % C0, i3 = ln / C0;
@@ -856,6 +865,7 @@ __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ f
         for (int m = 0; m < L2; m++) p[m * S1] = v[m];
     }
     __syncthreads();
+    if (s_done) return;                                  // one reading per CTA, behind a barrier (pass_b_entry)
     // phase 2: lines along axis 3, one per (i0, i2): forward, filter X~ = (p2max / (V p2)) Delta~ at the stored positions
     // (zero mode -> 0), inverse                                                                  [north_star step 2]
 #pragma unroll 1
@@ -979,8 +989,8 @@ __device__ __forceinline__ void half_fft_inverse(const cplx (&b)[(1 << LG) / 2],
 template <int LG2, int LG3, int LGC, int NT>
 __global__ void __launch_bounds__(NT, LGF_FH_MINB) k_fh_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
     pdl_enter();
-    if (pass_b_done(ctl)) return;
-    finalize_in_pass_b<NT>(partials, fa, ctl);
+    __shared__ int s_done;
+    pass_b_entry<NT>(partials, fa, ctl, &s_done);
     using MG = MidGeom<LG2, LGC>;
     using P2 = Plan2<LG2, false>;
     using P3 = Plan2<LG3, true>;
@@ -1017,6 +1027,7 @@ __global__ void __launch_bounds__(NT, LGF_FH_MINB) k_fh_mid(cplx* __restrict__ f
             for (int j = 0; j < P2::R2; j++) p[((h * K2 + kl) * P2::R2 + j) * S1] = b[kl * P2::R2 + j];
     }
     __syncthreads();
+    if (s_done) return;
     // phase 2: axis-3 lines, one per (i0, i2) and lane pair: forward, filter at the stored positions, inverse, in place
 #pragma unroll 1
     for (int ln = threadIdx.x >> 1; ln < C0 * L2; ln += NT / 2) {
