@@ -364,6 +364,38 @@ def test_plain_steepest_descent_variant(dims, storage):
     assert th < href[-1, 1]                                              # Fourier acceleration converges faster
 
 
+# ------------------------------------------------------------------ many short runs across the kernel selections
+def test_kernel_selections_agree_over_many_configurations():
+    """Several hundred lgf_fix runs on seeded device-generated configurations: every kernel selection (pass B forms, where S5
+    runs, PDL, graph batching) must stop at the same iteration with the same F, and the mixed-precision run must reach
+    the same F.  The stop flag is raised and observed in a different kernel or CTA in each selection; this is the test
+    that goes through that transition many times (a per-thread read of the flag once hung an experimental build)."""
+    variants = [{}, {"LGF_OPT_LINE_FFT": 0}, {"LGF_OPT_LINE_FFT": 2}, {"LGF_OPT_FUSE_FINALIZE": 0}, {"LGF_OPT_FUSE_FINALIZE": 1},
+                {"LGF_OPT_PDL": 0}, {"LGF_OPT_BATCH": 1}, {"LGF_OPT_BATCH": 3}, {"LGF_OPT_GRAPH": 0}, {"LGF_OPT_QUAD_UPDATE": 0}]
+    for dims, nseeds in [((16, 16, 16, 16), 24), ((32, 32, 16, 16), 8), ((64, 64, 4, 4), 4)]:
+        gfs = []
+        for opts in variants:
+            g = lgf.GaugeFixer(dims, 12)
+            for k, v in opts.items():
+                g.set_option(getattr(lgf, k), v)
+            gfs.append(g)
+        gm = lgf.GaugeFixer(dims, 12, precision=lgf.LGF_MIXED)
+        for seed in range(nseeds):
+            Ud = E.device_su3(dims, 2000 + seed, 0.1 + 0.01 * (seed % 20))
+            ref = None
+            for opts, g in zip(variants, gfs):
+                g.load_links_device(Ud.data_ptr())
+                r = g.fix(ALPHA, TOL, 5000)
+                assert r["status"] == lgf.LGF_OK, (dims, seed, opts, r)
+                ref = ref or r
+                assert r["n_iter"] == ref["n_iter"] and abs(r["F"] - ref["F"]) <= 1e-13, (dims, seed, opts, r, ref)
+            gm.load_links_device(Ud.data_ptr())
+            rm = gm.fix(ALPHA, TOL, 5000)
+            assert rm["status"] == lgf.LGF_OK and abs(rm["F"] - ref["F"]) <= 1e-11, (dims, seed, rm, ref)
+        for g in gfs + [gm]:
+            g.destroy()
+
+
 # ------------------------------------------------------------------ thermalised Wilson-action inputs (SURVEY.md section 8(f) NEXT-4)
 @pytest.mark.parametrize("dims,beta,sweeps,seed", [((8, 8, 8, 8), 5.8, 20, 7), ((16, 16, 16, 16), 6.0, 20, 7),
                                                   ((8, 8, 8, 8), 5.7, 40, 8), ((16, 16, 16, 16), 5.7, 40, 7)])
