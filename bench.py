@@ -240,8 +240,6 @@ def run_ours(args):
     inner = args.inner
     fp32 = args.precision == "fp32"
     gf = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_FP32 if fp32 else lgf.LGF_FP64)
-    if args.fuse_update is not None:
-        gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, args.fuse_update)
     if device_links:
         if args.links == "wilson":
             d_in = E.wilson(dims, args.beta, args.sweeps, cfg["seed"] + 100 * rank, device="cuda")
@@ -420,8 +418,6 @@ def main():
                     help="host: the seeded BASELINE.json ensemble built with numpy (default); device: seeded links generated on the GPU "
                          "(large shapes C3, C4; no e2e leg, no CPU baseline); wilson: a thermalised Wilson-action configuration generated on the GPU "
                          "(ensembles.wilson: the kind of input the paper fixes), for time_to_theta on realistic links")
-    ap.add_argument("--fuse-update", type=int, default=None, choices=[0, 1],
-                    help="override LGF_OPT_FUSE_UPDATE (kernel A/B timing); default: the library's choice")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                   # timing rule: at least 3 warm-up steps

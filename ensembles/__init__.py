@@ -42,6 +42,7 @@ __all__ = [
     "as_real",
     "as_complex",
     "device_su3",
+    "noisy_device",
     "wilson",
 ]
 
@@ -212,6 +213,56 @@ def device_su3(dims, seed: int, spread: float = 0.15):
         U[o:o + m, 1] = v
         U[o:o + m, 2] = torch.linalg.cross(u, v).conj()
     return U.reshape(V, 4, 3, 3)
+
+
+def noisy_device(dims, seed: int, eps: float, stream: int = 0, device: str = "cuda", chunk: int = 1 << 22):
+    """The `noisy` recipe of BASELINE.json configs[1] -- U_mu(x) = h(x) exp(i eps H_mu(x)) h^dagger(x+mu), h Haar-random
+    SU(3), H = sum_a c_a lambda_a / 2 with c_a ~ N(0,1) (reading A12) -- generated with torch on `device`, for the
+    lattices whose numpy build takes minutes (C4: 64^4, 67 M links).  Same distribution as `noisy`, different random
+    stream (torch's Philox generator seeded with (seed, stream) instead of numpy's), and the two linear-algebra steps
+    are written as their closed forms so that they run as plain tensor ops: the QR of the Ginibre matrix with a
+    positive R diagonal IS column Gram-Schmidt, and exp(i eps H) is torch.linalg.matrix_exp.  Returns a torch
+    complex128 tensor [V, 4, 3, 3] in the canonical order of include/lgf.h; the caller copies it to the host once and
+    feeds the same array to the oracle and to lgf_load_links (reading A12b).  Inputs only."""
+    import torch
+    dims = tuple(int(v) for v in dims)
+    V = volume(dims)
+    gen = torch.Generator(device=device)
+    gen.manual_seed((int(seed) << 20) + int(stream))
+    gm = torch.from_numpy(_GM).to(device)
+    h = torch.empty(V, 3, 3, dtype=torch.complex128, device=device)
+    for a in range(0, V, chunk):
+        b = min(V, a + chunk)
+        z = torch.view_as_complex(torch.randn(b - a, 3, 3, 2, dtype=torch.float64, device=device, generator=gen))
+        # column Gram-Schmidt = QR with positive diag(R): Haar on U(3) (the phase fix of haar_su3); a second pass
+        # restores orthogonality to rounding where two Gaussian columns were nearly parallel
+        q = z
+        for _ in range(2):
+            q0 = q[:, :, 0] / q[:, :, 0].abs().pow(2).sum(-1, keepdim=True).sqrt()
+            v1 = q[:, :, 1] - (q0.conj() * q[:, :, 1]).sum(-1, keepdim=True) * q0
+            q1 = v1 / v1.abs().pow(2).sum(-1, keepdim=True).sqrt()
+            v2 = q[:, :, 2] - (q0.conj() * q[:, :, 2]).sum(-1, keepdim=True) * q0 - (q1.conj() * q[:, :, 2]).sum(-1, keepdim=True) * q1
+            q2 = v2 / v2.abs().pow(2).sum(-1, keepdim=True).sqrt()
+            q = torch.stack([q0, q1, q2], dim=-1)
+        det = torch.linalg.det(q)
+        h[a:b] = q * torch.exp(-1j * torch.angle(det) / 3.0)[:, None, None]
+    L0, L1, L2, L3 = dims
+    h4 = h.view(L3, L2, L1, L0, 3, 3)
+    U = torch.empty(V, 4, 3, 3, dtype=torch.complex128, device=device)
+    for mu in range(4):
+        hf = torch.roll(h4, -1, dims=3 - mu).reshape(V, 3, 3).conj().transpose(1, 2)      # h^dagger(x + mu)
+        for a in range(0, V, chunk):
+            b = min(V, a + chunk)
+            c = torch.randn(b - a, 8, dtype=torch.float64, device=device, generator=gen)
+            H = torch.einsum("na,aij->nij", c.to(torch.complex128), gm) * 0.5
+            Ex = torch.linalg.matrix_exp(1j * eps * H)
+            # one Gram-Schmidt clean-up of the rows (A12): matrix_exp leaves ~1e-14 of non-unitarity
+            u = Ex[:, 0] / Ex[:, 0].abs().pow(2).sum(-1, keepdim=True).sqrt()
+            v = Ex[:, 1] - (u.conj() * Ex[:, 1]).sum(-1, keepdim=True) * u
+            v = v / v.abs().pow(2).sum(-1, keepdim=True).sqrt()
+            Ex = torch.stack([u, v, torch.linalg.cross(u, v).conj()], dim=1)
+            U[a:b, mu] = h[a:b] @ Ex @ hf[a:b]
+    return U
 
 
 def wilson(dims, beta: float, sweeps: int, seed: int, device: str = "cpu", hot: bool = False):

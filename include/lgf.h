@@ -55,21 +55,25 @@ typedef enum {
 /* Precision of link storage and of the per-site arithmetic.  LGF_FP64: the paper's setting.
  * LGF_FP32: links and field stored as float, every kernel computes in float; the
  * lattice sums (theta, F) and the p^2 filter weights stay double.  Half the HBM bytes per iteration; theta bottoms out
- * near 1e-12 (fp32 rounding of Delta), so theta < 1e-15 is not reachable in this precision alone.  Host- and
+ * between 1e-14 and 1e-12 (fp32 rounding of Delta, amplified by p2max/p2min ~ L^2), so theta < 1e-15 is not reachable in
+ * this precision alone.  Host- and
  * device-side link and field arrays of this API are double in every precision (converted on load and on get).
  * LGF_MIXED: an fp64 context (everything above holds: fp64 links, fp64 lgf_iterate) whose lgf_fix runs in two phases:
- * a float copy of the links is fixed in fp32 down to theta = max(theta_tol, 1e-12) while the update accumulates the
- * total gauge transformation G(x); then the fp64 links receive U_mu(x) <- G(x) U_mu(x) G(x+mu)^dagger with G
+ * a float copy of the links is fixed in fp32 down to theta = max(theta_tol, 1e-12) -- or until theta stops falling, so
+ * a stalled fp32 phase never eats the max_iter budget -- while the update accumulates the total gauge transformation G(x); then the fp64 links receive U_mu(x) <- G(x) U_mu(x) G(x+mu)^dagger with G
  * re-orthonormalised in double -- an exact gauge copy of the input, at the fp32 noise level of theta -- and the fp64
  * iteration continues to theta_tol.  n_iter is the total; lgf_get_option(LGF_OPT_MIXED_FP32_ITERS) gives the fp32
  * share; lgf_get_history covers the fp64 phase.  Needs the workspaces of both precisions. */
 typedef enum { LGF_FP64 = 0, LGF_FP32 = 1, LGF_MIXED = 2 } lgf_precision;
 typedef enum { LGF_STORE_18 = 18, LGF_STORE_12 = 12 } lgf_storage;
 
-/* Bytes of device workspace a context for these parameters needs (0 if the parameters are unsupported). */
+/* Bytes of device workspace a context for these parameters needs (0 if the parameters are unsupported).
+ * [layout: SURVEY.md 8(a) S0; 12-real storage PAPER.md:45,51] */
 size_t lgf_workspace_bytes(const int dims[4], lgf_precision p, lgf_storage s);
 
-/* Create a context.  dims: HOST, {L0,L1,L2,L3}.  The library allocates its own device memory (cudaMalloc)
+/* Create a context: lgf_create(dims, precision, storage) of the north star; lattice, precision and link storage as the
+ * paper names them (PAPER.md:45 "12 real number representation", :47 lattice volume, :51 double precision).
+ * dims: HOST, {L0,L1,L2,L3}.  The library allocates its own device memory (cudaMalloc)
  * on the current device and creates its own stream. */
 lgf_status lgf_create(const int dims[4], lgf_precision p, lgf_storage s, lgf_ctx **out);
 
@@ -81,27 +85,29 @@ lgf_status lgf_create_ex(const int dims[4], lgf_precision p, lgf_storage s,
 
 void lgf_destroy(lgf_ctx *ctx);
 
-/* Load links.  host_links: HOST, canonical order, V*4*18 doubles.  Stored as given -- no reprojection; in
+/* Load links U_mu(x) (the gauge configuration of PAPER.md:37-39; layout S0, reading A9: no reprojection).
+ * host_links: HOST, canonical order, V*4*18 doubles.  Stored as given -- no reprojection; in
  * 12-real storage rows 0,1 are kept and row 2 is dropped (it is rebuilt as conj(row0 x row1) on use). */
 lgf_status lgf_load_links(lgf_ctx *ctx, const double *host_links);
 /* Same from DEVICE memory (canonical order). */
 lgf_status lgf_load_links_device(lgf_ctx *ctx, const double *dev_links);
 
-/* Read the links back, canonical order, always full 18 reals per link (row 2 rebuilt in 12-real storage). */
+/* Read the gauge-fixed links back (the transformed U of PAPER.md:39), canonical order, always full 18 reals per link (row 2 rebuilt in 12-real storage). */
 lgf_status lgf_get_links(lgf_ctx *ctx, double *host_links);
 lgf_status lgf_get_links_device(lgf_ctx *ctx, double *dev_links);
 
-/* Apply exactly n iterations S1-S4 with step alpha (no stop test), then measure once more.
+/* Apply exactly n iterations S1-S4 (north star steps 1-4; steepest descent with Fourier acceleration) with
+ * step alpha, no stop test, then measure once more (reading A5).
  * F, theta (HOST, may be NULL): the functional and theta of the links AFTER the n-th update.  n >= 0. */
 lgf_status lgf_iterate(lgf_ctx *ctx, int n, double alpha, double *F, double *theta);
 
-/* Iterate until theta < theta_tol (strict) or max_iter updates.  n_iter (HOST): number of link updates applied
+/* Iterate until theta < theta_tol (strict; "theta < 10^-15", alpha = 0.08 there) or max_iter updates (S5).  n_iter (HOST): number of link updates applied
  * before the first measurement with theta < theta_tol (0 if the links already satisfy it).  F, theta: that
  * measurement.  Returns LGF_OK, or LGF_NOT_CONVERGED when max_iter updates did not reach theta_tol. */
 lgf_status lgf_fix(lgf_ctx *ctx, double alpha, double theta_tol, int max_iter,
                    int *n_iter, double *F, double *theta);
 
-/* F, theta and the average plaquette of the current links; no state change.  Any out pointer may be NULL. */
+/* F (PAPER.md:39 with g = 1), theta (north star step 1) and the average plaquette of the current links; no state change.  Any out pointer may be NULL. */
 lgf_status lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette);
 
 /* (F_k, theta_k) of the measurements made by the last lgf_iterate/lgf_fix call, k = 0..min(n_iter, cap-1);
@@ -115,68 +121,26 @@ lgf_status lgf_get_history(lgf_ctx *ctx, double *hist, int capacity, int *n_out)
 typedef enum { LGF_FIELD_DELTA = 0, LGF_FIELD_X = 1, LGF_FIELD_G = 2 } lgf_field;
 lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *host_field);
 
-/* Kernel selection (for ncu comparisons; results are identical up to rounding order).
- *   LGF_OPT_FUSE_DELTA_FFT  1: Delta is computed inside FFT pass A (default when the plane fits), 0: separate kernel
- *   LGF_OPT_STORE_G         1: pass C stores g(x) and the update reads it, 0: the update recomputes g from X
- *   LGF_OPT_GRAPH           1: replay iterations through a CUDA graph (default), 0: plain launches
- *   LGF_OPT_BATCH           iterations enqueued between two reads of the device stop flag (default 8)
- *   LGF_OPT_FAST_FFT        1 (default): use the compile-time-sized FFT passes where the lattice allows (extents 16,
- *                           32 or 64 on the axis pair of a pass; a 64 extent in the (x0,x1) plane keeps S1 separate), 0: always the generic passes.  lgf_get_option returns a
- *                           bit mask of the passes that run fast: 1 pass A (fused Delta), 2 pass B, 4 pass C
- *   LGF_OPT_FUSE_UPDATE     0 (default: the separate kernels measured faster on B200), 1: where the
- *                           compile-time-sized passes cover the (x0,x1) plane, S3/S4 of one iteration
- *                           are fused with S1 and FFT pass A of the next (double-buffered links, g stored by pass C:
- *                           the links cross HBM twice per iteration instead of three times), 0: separate kernels.
- *                           lgf_get_option returns whether the fused path is the one that runs.
- *   LGF_OPT_PINGPONG        bit mask (1 pass A, 2 pass B, 4 pass C): run that compile-time-sized pass as a
- *                           persistent kernel, one CTA per SM, whose two thread groups alternate their global-memory
- *                           and shared-memory phases (fft_fast.cuh); 0 bits: one work item per CTA.
- *                           lgf_get_option returns the mask of the passes that run this way.  Default 0: measured on
- *                           B200 the strict alternation is slower for pass A and neutral for B and C.
- *   LGF_OPT_FUSE_FINALIZE   where the final theta/F reduction and the S5 stop test run.  0: k_finalize, a one-CTA kernel
- *                           between S1 and pass B.  2 (default): inside the first CTA of pass B, where pass B is one of
- *                           the compile-time-sized kernels -- the partials are complete when pass B starts, pass B
- *                           itself does not need the decision, pass C and the update see it: one launch fewer per
- *                           iteration, no fence.  1: inside the CTA of the compile-time-sized pass A that finishes
- *                           S1 last (needs a gpu-scope fence per CTA, which costs pass A more than the launch it
- *                           saves).  Summation order as in k_finalize up to the CTA's thread count.
- *                           lgf_get_option returns the mode that runs.
- *   LGF_OPT_QUAD_UPDATE     1 (default): S3+S4 with one thread per link, the four directions of 32 sites per CTA, g(x)
- *                           taken from the thread that built it as g((x-0)+0) (4 Gram-Schmidt per site, k_update_quad),
- *                           0: one thread per site (5 Gram-Schmidt per site, k_update).  Applies when g is recomputed
- *                           from X (LGF_OPT_STORE_G = 0, LGF_OPT_FUSE_UPDATE = 0); lgf_get_option returns whether it runs.
- *   LGF_OPT_PDL             1 (default): the kernels of an iteration are launched with programmatic dependent launch
- *                           (each waits on the device for the complete end of its predecessor, so results are
- *                           unchanged; launch latency and CTA ramp-up overlap the predecessor's tail), 0: plain
- *                           stream-ordered launches.
- *   LGF_OPT_FOURIER_ACCEL   1 (default): the paper's method, X = IFFT[(p2max/p2) FFT[Delta]].  0: plain steepest
- *                           descent, X = Delta (the method Fourier acceleration is measured against, PAPER.md:41 refs
- *                           [1],[2]): S2 drops out, an iteration is S1, S5, S3+S4.  Converges for alpha < 2/p2max = 1/8,
- *                           with a rate that degrades with the volume (critical slowing down).
- *   LGF_OPT_GAUGE_DIRECTIONS 4 (default): Landau gauge, the paper's problem.  3: Coulomb gauge -- the gauge
- *                           condition, Delta, F (normalised by 3 N_c V) and p^2 run over mu = 0..2 only, p2max = 12, the
- *                           spatial zero mode of every time slice is dropped, all four link directions are transformed.
- *                           Same kernels; the transform pair along axis 3 cancels -- k_fr_mid skips it (every axis-2 line
- *                           is finished in registers), the other pass-B kernels keep it as a no-op pair.
- *                           LGF_OPT_FUSE_UPDATE is Landau only and is ignored in Coulomb gauge.
- *   LGF_OPT_LINE_FFT        1 (default): FFT pass B on extents 16/32 keeps whole lines in registers (one thread = one line
- *                           of an axis, twiddles as instruction operands; the tile is written and read twice per point
- *                           instead of four times, two barriers instead of five; k_fr_mid), 0: the stage-wise pass B
- *                           (k_fa_mid), 2: half a line per thread, lane pairs exchanging by shuffle (k_fh_mid; Landau
- *                           only; measured slower).  lgf_get_option returns the form that runs.
- *   LGF_OPT_QUAD_DELTA      1: where S1 is a kernel of its own (64-extent planes, LGF_OPT_FUSE_DELTA_FFT = 0, plain
- *                           steepest descent, lgf_measure) it runs with one thread per link pair (k_delta_quad:
- *                           4 directions x 32 sites per CTA step, contributions summed through shared memory),
- *                           0 (default; measured faster): one thread per site (k_delta).
- *   LGF_OPT_CLUSTER_PASS_A  1 (default): on 64 x 64 (x0,x1) planes S1 is fused into FFT pass A on CTA pairs (thread-block
- *                           clusters of 2: each CTA keeps two of the four component tiles and writes the other two
- *                           into its partner's shared memory; k_cl_delta_fwd), needs LGF_OPT_FUSE_DELTA_FFT = 1;
- *                           0: S1 as its own kernel + one-component plane passes.  get: whether it runs. */
-typedef enum { LGF_OPT_FUSE_DELTA_FFT = 0, LGF_OPT_STORE_G = 1, LGF_OPT_GRAPH = 2, LGF_OPT_BATCH = 3, LGF_OPT_FAST_FFT = 4,
-               LGF_OPT_FUSE_UPDATE = 5, LGF_OPT_PINGPONG = 6, LGF_OPT_FUSE_FINALIZE = 7,
-               LGF_OPT_QUAD_UPDATE = 8, LGF_OPT_PDL = 9, LGF_OPT_FOURIER_ACCEL = 10,
-               LGF_OPT_MIXED_FP32_ITERS = 11 /* read-only */, LGF_OPT_GAUGE_DIRECTIONS = 12, LGF_OPT_LINE_FFT = 13,
-               LGF_OPT_QUAD_DELTA = 14, LGF_OPT_CLUSTER_PASS_A = 15 } lgf_option;
+/* Options.  The method itself (what is computed):
+ *   LGF_OPT_FOURIER_ACCEL    1 (default): the paper's method, X = IFFT[(p2max/p2) FFT[Delta]].  0: plain
+ *                            steepest descent, X = Delta (what Fourier acceleration is measured against, PAPER.md:41
+ *                            refs [1],[2]); converges for alpha < 2/p2max = 1/8, rate degrades with the volume.
+ *   LGF_OPT_GAUGE_DIRECTIONS 4 (default): Landau gauge, the paper's problem.  3: Coulomb gauge -- the
+ *                            gauge condition, Delta, F (normalised by 3 N_c V) and p^2 run over mu = 0..2, p2max = 12, the
+ *                            spatial zero mode of every time slice is dropped, all four link directions are transformed.
+ * How it runs (results identical up to rounding order; DESIGN.md section 6 holds the measured A/B numbers):
+ *   LGF_OPT_STORE_G          0 (default): S3+S4 rebuild g(x+mu) from X.  1: pass C stores g(x) (96 B/site) and S4 reads it.
+ *   LGF_OPT_GRAPH            1 (default): iterations are replayed through a CUDA graph.  0: plain launches.
+ *   LGF_OPT_BATCH            iterations enqueued between two reads of the device stop flag (default 8, 1..1024).
+ *   LGF_OPT_PDL              1 (default): programmatic dependent launch between the kernels of an iteration.  0: off.
+ *   LGF_OPT_FAST_FFT         1 (default): compile-time-sized FFT passes where the lattice allows (extents 16/32/64).
+ *                            0: the generic passes.  get: bit mask of the passes that run fast (1 A, 2 B, 4 C).
+ *   LGF_OPT_MIXED_FP32_ITERS read-only: fp32 iterations of the last LGF_MIXED lgf_fix.
+ *   LGF_OPT_MIXED_SWITCH     LGF_MIXED: the fp32 phase aims at theta = 10^-value (default 12, 4..20) and hands over to fp64
+ *                            there, or earlier when theta stops falling (it has not halved within 256 iterations). */
+typedef enum { LGF_OPT_STORE_G = 0, LGF_OPT_GRAPH = 1, LGF_OPT_BATCH = 2, LGF_OPT_PDL = 3, LGF_OPT_FAST_FFT = 4,
+               LGF_OPT_FOURIER_ACCEL = 5, LGF_OPT_GAUGE_DIRECTIONS = 6, LGF_OPT_MIXED_FP32_ITERS = 7,
+               LGF_OPT_MIXED_SWITCH = 8 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

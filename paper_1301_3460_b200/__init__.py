@@ -19,8 +19,8 @@ __all__ = [
     "LgfError", "lib", "library_path", "GaugeFixer", "copy_peak_gbs", "stream_peak_gbs",
     "LGF_OK", "LGF_NOT_CONVERGED", "LGF_FP64", "LGF_FP32", "LGF_MIXED", "LGF_STORE_12", "LGF_STORE_18",
     "LGF_FIELD_DELTA", "LGF_FIELD_X", "LGF_FIELD_G",
-    "LGF_OPT_FUSE_DELTA_FFT", "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_FAST_FFT", "LGF_OPT_FUSE_UPDATE",
-    "LGF_OPT_PINGPONG", "LGF_OPT_FUSE_FINALIZE", "LGF_OPT_QUAD_UPDATE", "LGF_OPT_PDL", "LGF_OPT_FOURIER_ACCEL", "LGF_OPT_MIXED_FP32_ITERS", "LGF_OPT_GAUGE_DIRECTIONS", "LGF_OPT_LINE_FFT", "LGF_OPT_QUAD_DELTA", "LGF_OPT_CLUSTER_PASS_A",
+    "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_PDL", "LGF_OPT_FAST_FFT", "LGF_OPT_FOURIER_ACCEL",
+    "LGF_OPT_GAUGE_DIRECTIONS", "LGF_OPT_MIXED_FP32_ITERS", "LGF_OPT_MIXED_SWITCH",
     "EXPORTS",
 ]
 
@@ -35,10 +35,8 @@ LGF_NOT_CONVERGED = 100
 LGF_FP64, LGF_FP32, LGF_MIXED = 0, 1, 2
 LGF_STORE_18, LGF_STORE_12 = 18, 12
 LGF_FIELD_DELTA, LGF_FIELD_X, LGF_FIELD_G = 0, 1, 2
-LGF_OPT_FUSE_DELTA_FFT, LGF_OPT_STORE_G, LGF_OPT_GRAPH, LGF_OPT_BATCH, LGF_OPT_FAST_FFT, LGF_OPT_FUSE_UPDATE = 0, 1, 2, 3, 4, 5
-LGF_OPT_PINGPONG, LGF_OPT_FUSE_FINALIZE, LGF_OPT_QUAD_UPDATE, LGF_OPT_PDL, LGF_OPT_FOURIER_ACCEL = 6, 7, 8, 9, 10
-LGF_OPT_MIXED_FP32_ITERS, LGF_OPT_GAUGE_DIRECTIONS, LGF_OPT_LINE_FFT = 11, 12, 13
-LGF_OPT_QUAD_DELTA, LGF_OPT_CLUSTER_PASS_A = 14, 15
+LGF_OPT_STORE_G, LGF_OPT_GRAPH, LGF_OPT_BATCH, LGF_OPT_PDL, LGF_OPT_FAST_FFT = 0, 1, 2, 3, 4
+LGF_OPT_FOURIER_ACCEL, LGF_OPT_GAUGE_DIRECTIONS, LGF_OPT_MIXED_FP32_ITERS, LGF_OPT_MIXED_SWITCH = 5, 6, 7, 8
 LGF_MAX_KERNELS = 32
 
 # every symbol include/lgf.h declares (checked by tests/test_abi.py against the header text)
@@ -78,9 +76,13 @@ def lib():
     if _lib is not None:
         return _lib
     path = library_path()
-    if not os.path.exists(path):
+    if not os.environ.get("LGF_LIBRARY"):
         from . import _build
-        _build.build()
+        if _build.have_nvcc():
+            _build.build()                    # no-op when the .so is newer than every source
+        elif os.path.exists(path) and not _build.up_to_date():
+            import warnings
+            warnings.warn("paper_1301_3460_b200/liblgf.so is older than its sources and nvcc is not available")
     if not os.path.exists(path):
         raise ImportError("paper_1301_3460_b200/liblgf.so is missing; run python -m paper_1301_3460_b200._build")
     L = C.CDLL(path)
@@ -218,6 +220,9 @@ class GaugeFixer:
         """Returns complex128 [V,4,3,3] (canonical order)."""
         if out is None:
             out = np.empty((self.V, 4, 3, 3), dtype=np.complex128)
+        elif not (isinstance(out, np.ndarray) and out.flags.c_contiguous and out.flags.writeable
+                  and out.dtype in (np.complex128, np.float64)):
+            raise TypeError("out must be a writeable C-contiguous complex128 [V,4,3,3] or float64 [V,4,3,3,2] array")
         a = _host_f64(out, self.V * 72)
         self._ck(lib().lgf_get_links(self._h, a.ctypes.data), "lgf_get_links")
         return out

@@ -47,8 +47,7 @@
 namespace lgf {
 
 // A group of NT threads that works on one tile: thread index within the group and the named barrier the group
-// synchronises on.  A whole CTA is the group {threadIdx.x, 0} (bar.sync 0 over all threads = __syncthreads());
-// the ping-pong kernels of fft_pp.cuh run two groups per CTA on barriers 1 and 2.
+// synchronises on.  A whole CTA is the group {threadIdx.x, 0} (bar.sync 0 over all threads = __syncthreads()).
 struct Grp { int tid; int bar; };
 template <int NT> __device__ __forceinline__ void gsync(const Grp& g) {
     asm volatile("bar.sync %0, %1;" ::"r"(g.bar), "n"(NT) : "memory");
@@ -267,41 +266,21 @@ __device__ __forceinline__ void pass_a_delta(const cplx* __restrict__ links, con
     gsync<NT>(g);
 }
 
-// S5 inside pass A: the CTA that takes the last ticket sums the plane partials in the order k_finalize uses (strided per
-// thread, then the fixed tree: the result is bit-identical), writes F, theta and the history and raises the stop flag.
-// Every CTA of the grid has passed its ctl->done test by then, and the next kernel starts after this one ends.
+// S5 by one whole CTA (all its threads call this): sums the partials in the order k_finalize uses (strided per thread,
+// then the fixed tree: bit-identical), writes F, theta and the history and raises the stop flag.
+// FinArgs::on = number of partials the first CTA of pass B has to reduce (0: k_finalize already did it).
 struct FinArgs { double2* hist; double inv3V, inv12V; int on; };
-// The reduction and the S5 decision by one whole CTA (all its threads call this).
 template <int NT>
 __device__ __forceinline__ void finalize_cta(const double2* partials, int n, Ctl* ctl, const FinArgs& fa, double* red) {
     double a = 0, b = 0;
     for (int i = threadIdx.x; i < n; i += NT) { const double2 p = __ldcg(partials + i); a += p.x; b += p.y; }
     block_sum2(a, b, red);
     if (threadIdx.x == 0) {
-        const double theta = a * fa.inv3V, F = b * fa.inv12V;
-        ctl->theta = theta; ctl->F = F; ctl->ticket = 0;
-        const int k = ctl->n_meas;
-        if (k < ctl->hist_cap) fa.hist[k] = make_double2(F, theta);
-        ctl->n_meas = k + 1;
-        if (!(isfinite(theta) && isfinite(F))) { ctl->nonfinite = 1; ctl->done = 1; }
-        else if (theta < ctl->theta_tol) { ctl->converged = 1; ctl->done = 1; }
-        else if (ctl->iters >= ctl->max_iter) { ctl->done = 1; }
+        s5_decide(ctl, fa.hist, a * fa.inv3V, b * fa.inv12V);
     }
     __syncthreads();
 }
-template <int NT>
-__device__ __forceinline__ void finalize_last_cta(const double2* partials, int n, Ctl* ctl, const FinArgs& fa, double* red) {
-    __shared__ int is_last;
-    if (threadIdx.x == 0) {
-        __threadfence();                                   // this CTA's partial is visible before its ticket
-        is_last = (atomicAdd(&ctl->ticket, 1u) == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!is_last) return;
-    __threadfence();
-    finalize_cta<NT>(partials, n, ctl, fa, red);
-}
-// S5 inside pass B (LGF_OPT_FUSE_FINALIZE = 2): the partials of pass A are complete when pass B starts, so its CTA 0 does
+// S5 inside pass B: the partials of pass A are complete when pass B starts, so its CTA 0 does
 // the reduction and the stop decision before its own tile -- no k_finalize launch, no fence.  Pass B itself never needs
 // the decision (it only transforms the scratch field; a CTA that already sees the flag may skip its tile, which nobody
 // reads once the flag is up); pass C and the update start after this kernel has ended and see it.
@@ -330,7 +309,7 @@ __device__ __forceinline__ void pass_b_entry(const double2* partials, const FinA
 // Pass A: S1 (Delta, theta/F partials) + forward FFT over axes 0,1 of one (x2,x3) plane, all 4 components.
 template <int LG0, int LG1, int NC, int NT>
 __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
-                                                     Geom G, FftTables T, Ctl* ctl, FinArgs fa) {
+                                                     Geom G, FftTables T, const Ctl* __restrict__ ctl) {
     pdl_enter();
     if (ctl->done) return;
     constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
@@ -340,23 +319,9 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cp
     cplx* tw1 = tw0 + L0;
     __shared__ double red[64];
     const Grp g{(int)threadIdx.x, 0};
-#if defined(LGF_A_PREFETCH) && LGF_A_PREFETCH
-    if (threadIdx.x < 4 * NC)     // experiment: DRAM -> L2 bulk prefetch of the CTA's own plane
-        prefetch_l2(links + (long long)threadIdx.x * G.V + ((long long)blockIdx.x << (LG0 + LG1)), (unsigned)(L0 * L1 * sizeof(cplx)));
-#endif
     for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
     for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
-#if defined(LGF_DBG_A) && LGF_DBG_A == 2      // timing experiment: no S1 (tile filled with constants)
-    for (int e = threadIdx.x; e < 4 * SC; e += NT) tile[e] = mk((real)(1e-3 * (e & 15)), (real)1e-3);
-    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(1.0, 1.0);
-    __syncthreads();
-#else
     pass_a_delta<LG0, LG1, NC, NT>(links, G, blockIdx.x, tile, red, partials, g);
-#endif
-    if (fa.on) finalize_last_cta<NT>(partials, gridDim.x, ctl, fa, red);
-#if defined(LGF_DBG_A) && LGF_DBG_A == 1      // timing experiment: no FFT, no field store
-    return;
-#endif
     plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)blockIdx.x << (LG0 + LG1), g);
 }
 
@@ -899,320 +864,6 @@ __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ f
         cplx* gq = gbase + i0 + ((long long)i3 << sh3);
 #pragma unroll
         for (int m = 0; m < L2; m++) st_field(gq + ((long long)m << sh2), v[m]);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// Pass B with HALF a line per thread: two adjacent lanes (h = 0, 1) share a line of L = R1 R2 points.  Stage 1 needs no
-// exchange (lane h takes the butterflies ja in [h R2/2, (h+1) R2/2)); before stage 2 the pair swaps half of its values
-// through one round of shuffles so that lane h owns the complete blocks ba in [h R1/2, (h+1) R1/2).  Half the registers
-// of k_fr_mid per thread (16 points instead of 32), hence twice the resident warps.
-//   "stage-1 layout":  a[jl][k]  <->  position (h J + jl) + k R2,      J = R2/2, jl < J, k < R1
-//   "stage-2 layout":  b[kl][j]  <->  position (h K + kl) R2 + j,      K = R1/2, kl < K, j < R2
-template <int LG> __device__ __forceinline__ cplx ctw_rt(int k) {       // run-time index: constant-cache load
-    if constexpr (LG == 4) return mk(c_tw16[k][0], c_tw16[k][1]);
-    else return mk(c_tw32[k][0], c_tw32[k][1]);
-}
-__device__ __forceinline__ cplx shfl_pair(cplx v) {
-    return mk(__shfl_xor_sync(0xffffffffu, v.x, 1), __shfl_xor_sync(0xffffffffu, v.y, 1));
-}
-__device__ __forceinline__ cplx csel(bool c, cplx a, cplx b) { return mk(c ? a.x : b.x, c ? a.y : b.y); }
-
-template <int LG, bool B>
-__device__ __forceinline__ void half_fft_forward(const cplx (&a)[(1 << LG) / 2], cplx (&b)[(1 << LG) / 2], int h) {
-    using P = Plan2<LG, B>;
-    constexpr int R1 = P::R1, R2 = P::R2, J = R2 / 2, K = R1 / 2;
-    cplx s[J][R1];
-#pragma unroll
-    for (int jl = 0; jl < J; jl++) {
-        cplx x[R1];
-#pragma unroll
-        for (int k = 0; k < R1; k++) x[k] = a[jl * R1 + k];
-        bfly<R1, false>(x);
-        const int ja = h * J + jl;
-#pragma unroll
-        for (int k = 1; k < R1; k++) x[k] = cmul(x[k], ctw_rt<LG>(k * ja));
-#pragma unroll
-        for (int k = 0; k < R1; k++) s[jl][k] = x[k];
-    }
-#pragma unroll
-    for (int kl = 0; kl < K; kl++) {
-        cplx x[R2];
-#pragma unroll
-        for (int jl = 0; jl < J; jl++) {
-            const cplx keep = csel(h, s[jl][K + kl], s[jl][kl]);
-            const cplx recv = shfl_pair(csel(h, s[jl][kl], s[jl][K + kl]));
-            x[jl] = csel(h, recv, keep);
-            x[J + jl] = csel(h, keep, recv);
-        }
-        bfly<R2, false>(x);
-#pragma unroll
-        for (int j = 0; j < R2; j++) b[kl * R2 + j] = x[j];
-    }
-}
-template <int LG, bool B>
-__device__ __forceinline__ void half_fft_inverse(const cplx (&b)[(1 << LG) / 2], cplx (&a)[(1 << LG) / 2], int h) {
-    using P = Plan2<LG, B>;
-    constexpr int R1 = P::R1, R2 = P::R2, J = R2 / 2, K = R1 / 2;
-    cplx s[J][R1];
-#pragma unroll
-    for (int kl = 0; kl < K; kl++) {
-        cplx x[R2];
-#pragma unroll
-        for (int j = 0; j < R2; j++) x[j] = b[kl * R2 + j];
-        bfly<R2, true>(x);
-#pragma unroll
-        for (int jl = 0; jl < J; jl++) {
-            const cplx keep = csel(h, x[J + jl], x[jl]);
-            const cplx recv = shfl_pair(csel(h, x[jl], x[J + jl]));
-            s[jl][kl] = csel(h, recv, keep);
-            s[jl][K + kl] = csel(h, keep, recv);
-        }
-    }
-#pragma unroll
-    for (int jl = 0; jl < J; jl++) {
-        cplx x[R1];
-#pragma unroll
-        for (int k = 0; k < R1; k++) x[k] = s[jl][k];
-        const int ja = h * J + jl;
-#pragma unroll
-        for (int k = 1; k < R1; k++) x[k] = cmulc(x[k], ctw_rt<LG>(k * ja));
-        bfly<R1, true>(x);
-#pragma unroll
-        for (int k = 0; k < R1; k++) a[jl * R1 + k] = x[k];
-    }
-}
-
-#ifndef LGF_FH_MINB
-#define LGF_FH_MINB 2
-#endif
-template <int LG2, int LG3, int LGC, int NT>
-__global__ void __launch_bounds__(NT, LGF_FH_MINB) k_fh_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, Ctl* ctl, const double2* partials, FinArgs fa) {
-    pdl_enter();
-    __shared__ int s_done;
-    pass_b_entry<NT>(partials, fa, ctl, &s_done);
-    using MG = MidGeom<LG2, LGC>;
-    using P2 = Plan2<LG2, false>;
-    using P3 = Plan2<LG3, true>;
-    constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
-    constexpr int J2 = P2::R2 / 2, K2 = P2::R1 / 2, J3 = P3::R2 / 2, K3 = P3::R1 / 2;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx* tile = reinterpret_cast<cplx*>(smem_raw);
-    double* s2 = reinterpret_cast<double*>(tile + S2 * L3);
-    double* s3 = s2 + L2;
-    for (int i = threadIdx.x; i < L2; i += NT) s2[i] = T.s[2][i];
-    for (int i = threadIdx.x; i < L3; i += NT) s3[i] = T.s[3][i];
-    const int lgChunks = G.lg[0] - LGC;
-    const int chunk = blockIdx.x & ((1 << lgChunks) - 1);
-    const int x1 = (blockIdx.x >> lgChunks) & (G.L[1] - 1);
-    const int comp = blockIdx.x >> (lgChunks + G.lg[1]);
-    cplx* gbase = field + (long long)comp * G.V + (chunk << LGC) + ((long long)x1 << G.sh[1]);
-    const int sh2 = G.sh[2], sh3 = G.sh[3];
-    const int h = threadIdx.x & 1;
-    // phase 1: axis-2 lines, one per (i0, i3) and lane pair: global -> forward -> tile
-#pragma unroll 1
-    for (int ln = threadIdx.x >> 1; ln < C0 * L3; ln += NT / 2) {
-        const int i0 = ln % C0, i3 = ln / C0;
-        const cplx* gq = gbase + i0 + ((long long)i3 << sh3);
-        cplx a[L2 / 2], b[L2 / 2];
-#pragma unroll
-        for (int jl = 0; jl < J2; jl++)
-#pragma unroll
-            for (int k = 0; k < P2::R1; k++) a[jl * P2::R1 + k] = ld_field(gq + ((long long)((h * J2 + jl) + k * P2::R2) << sh2));
-        half_fft_forward<LG2, false>(a, b, h);
-        cplx* p = tile + i0 + i3 * S2;
-#pragma unroll
-        for (int kl = 0; kl < K2; kl++)
-#pragma unroll
-            for (int j = 0; j < P2::R2; j++) p[((h * K2 + kl) * P2::R2 + j) * S1] = b[kl * P2::R2 + j];
-    }
-    __syncthreads();
-    if (s_done) return;
-    // phase 2: axis-3 lines, one per (i0, i2) and lane pair: forward, filter at the stored positions, inverse, in place
-#pragma unroll 1
-    for (int ln = threadIdx.x >> 1; ln < C0 * L2; ln += NT / 2) {
-        const int i0 = ln % C0, i2 = ln / C0;
-        cplx* p = tile + i0 + i2 * S1;
-        cplx a[L3 / 2], b[L3 / 2];
-#pragma unroll
-        for (int jl = 0; jl < J3; jl++)
-#pragma unroll
-            for (int k = 0; k < P3::R1; k++) a[jl * P3::R1 + k] = p[((h * J3 + jl) + k * P3::R2) * S2];
-        half_fft_forward<LG3, true>(a, b, h);
-        const double s012 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1] + s2[i2];
-#pragma unroll
-        for (int kl = 0; kl < K3; kl++)
-#pragma unroll
-            for (int j = 0; j < P3::R2; j++) {
-                const double p2 = s012 + s3[(h * K3 + kl) * P3::R2 + j];
-                b[kl * P3::R2 + j] = cscale(b[kl * P3::R2 + j], (real)((p2 > 0.0) ? scale / p2 : 0.0));
-            }
-        half_fft_inverse<LG3, true>(b, a, h);
-#pragma unroll
-        for (int jl = 0; jl < J3; jl++)
-#pragma unroll
-            for (int k = 0; k < P3::R1; k++) p[((h * J3 + jl) + k * P3::R2) * S2] = a[jl * P3::R1 + k];
-    }
-    __syncthreads();
-    // phase 3: axis-2 lines again: tile -> inverse -> global
-#pragma unroll 1
-    for (int ln = threadIdx.x >> 1; ln < C0 * L3; ln += NT / 2) {
-        const int i0 = ln % C0, i3 = ln / C0;
-        const cplx* p = tile + i0 + i3 * S2;
-        cplx a[L2 / 2], b[L2 / 2];
-#pragma unroll
-        for (int kl = 0; kl < K2; kl++)
-#pragma unroll
-            for (int j = 0; j < P2::R2; j++) b[kl * P2::R2 + j] = p[((h * K2 + kl) * P2::R2 + j) * S1];
-        half_fft_inverse<LG2, false>(b, a, h);
-        cplx* gq = gbase + i0 + ((long long)i3 << sh3);
-#pragma unroll
-        for (int jl = 0; jl < J2; jl++)
-#pragma unroll
-            for (int k = 0; k < P2::R1; k++) st_field(gq + ((long long)((h * J2 + jl) + k * P2::R2) << sh2), a[jl * P2::R1 + k]);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// Ping-pong persistent passes.  With one work item per CTA every resident CTA starts together and stays in phase:
-// all of them read global memory at once, then all of them sit in the shared-memory stages with HBM idle (measured
-// on B200 at 32^4: pass A takes 17.2 us per plane per SM at 1 CTA/SM and 2 x 15.6 at 2 CTAs/SM, i.e. the phases add
-// instead of overlapping).  Here one CTA per SM runs two groups of NT threads, each with its own tile, which take the
-// CTA's work items alternately and pass a token so that their MEMORY phases alternate: while group 0 is in the
-// on-chip stages of item k, group 1 is loading item k+1.  The token is a pair of named barriers (3: "group 0 may
-// load", 4: "group 1 may load"): bar.sync by the waiting group, bar.arrive by the releasing one.
-// Work items of CTA b: b, b + gridDim, b + 2 gridDim, ...  (148 CTAs x 6.92 planes at 32^4: 7 rounds, 1 % tail).
-#ifndef LGF_PP_TOKEN
-#define LGF_PP_TOKEN 1
-#endif
-#ifndef LGF_PP_PREFETCH
-#define LGF_PP_PREFETCH 0
-#endif
-template <int NT> struct PingPong {
-    int grp;
-    __device__ __forceinline__ void acquire(int round) const {
-        if (!LGF_PP_TOKEN) return;
-        if (grp == 1 || round > 0) asm volatile("bar.sync %0, %1;" ::"r"(3 + grp), "n"(2 * NT) : "memory");
-    }
-    // last: no later acquire of the other group will consume this release
-    __device__ __forceinline__ void release(bool last) const {
-        if (!LGF_PP_TOKEN) return;
-        if (grp == 0 || !last) asm volatile("bar.arrive %0, %1;" ::"r"(3 + (grp ^ 1)), "n"(2 * NT) : "memory");
-    }
-};
-
-template <int LG0, int LG1, int NC, int NT>
-__global__ void __launch_bounds__(2 * NT, 1) k_pp_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
-                                                            Geom G, FftTables T, const Ctl* __restrict__ ctl) {
-    pdl_enter();
-    if (ctl->done) return;
-    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double red2[2][64];
-    const int grp = threadIdx.x / NT;
-    const Grp g{(int)threadIdx.x % NT, 1 + grp};
-    const PingPong<NT> pp{grp};
-    cplx* tile = reinterpret_cast<cplx*>(smem_raw) + grp * 4 * SC;
-    cplx* tw0 = reinterpret_cast<cplx*>(smem_raw) + 8 * SC;
-    cplx* tw1 = tw0 + L0;
-    for (int i = threadIdx.x; i < L0; i += 2 * NT) tw0[i] = T.tw[0][i];
-    for (int i = threadIdx.x; i < L1; i += 2 * NT) tw1[i] = T.tw[1][i];
-    __syncthreads();
-    const int n_all = G.L[2] * G.L[3];
-    const int n_items = (n_all - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
-    const int rounds = (n_items + 1) >> 1;
-#pragma unroll 1
-    for (int r = 0; r < rounds; r++) {
-        const int k = 2 * r + grp;
-        const bool active = k < n_items;
-        const int plane = blockIdx.x + k * gridDim.x;
-        pp.acquire(r);
-        if (active) pass_a_delta<LG0, LG1, NC, NT>(links, G, plane, tile, red2[grp], partials, g);
-        pp.release(r == rounds - 1);
-        if (LGF_PP_PREFETCH && k + 2 < n_items && g.tid < 4 * NC) {
-            // DRAM -> L2 prefetch of the group's next plane (4*NC contiguous runs of L0*L1 entries) while it transforms this one
-            const long long xn = (long long)(plane + 2 * (int)gridDim.x) << (LG0 + LG1);
-            prefetch_l2(links + (long long)g.tid * G.V + xn, (unsigned)(L0 * L1 * sizeof(cplx)));
-        }
-        if (active) {
-            plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)plane << (LG0 + LG1), g);
-            gsync<NT>(g);      // the tile is free for the group's next item
-        }
-    }
-}
-
-template <int LG0, int LG1, int NT>
-__global__ void __launch_bounds__(2 * NT, 1) k_pp_inv(cplx* __restrict__ field, Geom G, FftTables T, const Ctl* __restrict__ ctl) {
-    pdl_enter();
-    if (ctl->done) return;
-    constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int grp = threadIdx.x / NT;
-    const Grp g{(int)threadIdx.x % NT, 1 + grp};
-    const PingPong<NT> pp{grp};
-    cplx* tile = reinterpret_cast<cplx*>(smem_raw) + grp * 4 * SC;
-    cplx* tw0 = reinterpret_cast<cplx*>(smem_raw) + 8 * SC;
-    cplx* tw1 = tw0 + L0;
-    for (int i = threadIdx.x; i < L0; i += 2 * NT) tw0[i] = T.tw[0][i];
-    for (int i = threadIdx.x; i < L1; i += 2 * NT) tw1[i] = T.tw[1][i];
-    __syncthreads();
-    const int n_all = G.L[2] * G.L[3];
-    const int n_items = (n_all - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
-    const int rounds = (n_items + 1) >> 1;
-#pragma unroll 1
-    for (int r = 0; r < rounds; r++) {
-        const int k = 2 * r + grp;
-        const bool active = k < n_items;
-        cplx* fbase = field + ((long long)(blockIdx.x + k * gridDim.x) << (LG0 + LG1));
-        pp.acquire(r);
-        if (active) pass_c_load<LG0, LG1, 4, NT>(fbase, G.V, tile, g);
-        pp.release(r == rounds - 1);
-        if (active) {
-            pass_c_finish<LG0, LG1, 4, NT, false>(fbase, nullptr, 0.0, G.V, tile, tw0, tw1, g);
-            gsync<NT>(g);
-        }
-    }
-}
-
-template <int LG2, int LG3, int LGC, int NT>
-__global__ void __launch_bounds__(2 * NT, 1) k_pp_mid(cplx* __restrict__ field, Geom G, FftTables T, double scale, const Ctl* __restrict__ ctl) {
-    pdl_enter();
-    if (ctl->done) return;
-    using MG = MidGeom<LG2, LGC>;
-    constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = MG::C0, TILE = MG::S2 * L3;
-    static_assert(NT % C0 == 0, "a thread keeps its x0 offset");
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int grp = threadIdx.x / NT;
-    const Grp g{(int)threadIdx.x % NT, 1 + grp};
-    const PingPong<NT> pp{grp};
-    cplx* tile = reinterpret_cast<cplx*>(smem_raw) + grp * TILE;
-    cplx* tw2 = reinterpret_cast<cplx*>(smem_raw) + 2 * TILE;
-    cplx* tw3 = tw2 + L2;
-    double* s2 = reinterpret_cast<double*>(tw3 + L3);
-    double* s3 = s2 + L2;
-    for (int i = threadIdx.x; i < L2; i += 2 * NT) { tw2[i] = T.tw[2][i]; s2[i] = T.s[2][i]; }
-    for (int i = threadIdx.x; i < L3; i += 2 * NT) { tw3[i] = T.tw[3][i]; s3[i] = T.s[3][i]; }
-    __syncthreads();
-    const int i0 = g.tid % C0;
-    const int n_all = 4 * G.L[1] * (G.L[0] >> LGC);
-    const int n_items = (n_all - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
-    const int rounds = (n_items + 1) >> 1;
-    const int sh2 = G.sh[2], sh3 = G.sh[3];
-#pragma unroll 1
-    for (int r = 0; r < rounds; r++) {
-        const int k = 2 * r + grp;
-        const bool active = k < n_items;
-        MidItem it;
-        pp.acquire(r);
-        if (active) {
-            it = mid_item<LGC>(field, G, T, blockIdx.x + k * gridDim.x, i0);
-            pass_b_load<LG2, LG3, LGC, NT>(it.gp, sh2, sh3, tile + i0, tw2, g);
-        }
-        pp.release(r == rounds - 1);
-        if (active) {
-            pass_b_finish<LG2, LG3, LGC, NT>(it.gp, it.s01, sh2, sh3, scale, tile + i0, tw2, tw3, s2, s3, g);
-            gsync<NT>(g);
-        }
     }
 }
 

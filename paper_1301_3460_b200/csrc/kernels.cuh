@@ -14,7 +14,8 @@
 //                  MODE_DELTA_FWD computes Delta of the plane itself (S1 fused), MODE_INV_G writes g (S3 fused)
 //   k_fft23_mid    S2a+S2b+S2c on axes 2,3 for a chunk of x0: forward, p2max/p2 filter, inverse
 //   k_finalize     deterministic final reduction of the partials, S5 stop flag
-//   k_update       S3+S4: rebuild (or read) g(x), g(x+mu) and rotate the four links of a site in place
+//   k_update_quad  S3+S4: rebuild g(x+mu) from X, one thread per link, rotate the link in place (default)
+//   k_update_g     S3+S4 with g read from gbuf (LGF_OPT_STORE_G)
 //   k_layout_in/out, k_plaquette, k_unpack_field, k_copy: boundary helpers
 #pragma once
 #include "su3.cuh"
@@ -66,13 +67,8 @@ __device__ __forceinline__ void delta_site_nd(const cplx* __restrict__ links, co
         load_link<NC>(links, G.V, mu, x, u);
         retr += u[0].x + u[4].x + u[8].x;
         acc_link(u, real(-1), d01, d02, d12, i0, i1, i2);
-#if defined(LGF_DBG_D)          // timing experiment: bit mu set -> no backward load for that direction
-        if (!((LGF_DBG_D >> mu) & 1))
-#endif
-        {
         load_link<NC>(links, G.V, mu, bwd(G, x, mu), u);
         acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
-        }
     }
     // D_jj = 2i Im A_jj; Delta_jj = D_jj - Tr D / 3
     const real tr3 = real(2.0 / 3.0) * (i0 + i1 + i2);
@@ -103,59 +99,26 @@ __global__ void __launch_bounds__(128) k_delta(const cplx* __restrict__ links, c
     if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
 }
 
-// S1 with one thread per link pair: a CTA is 4 warps = the 4 directions of 32 consecutive sites.  Thread (x, mu) loads
-// U_mu(x-mu) and U_mu(x) (12 loads instead of 48 per thread: more resident warps, shorter dependency chains), forms the
-// packed contribution of the pair to Delta(x) and hands it over through shared memory; thread (x, c) then sums the four
-// directions of packed component c and writes it: 4 coalesced V-arrays.  In Coulomb gauge the mu = 3 warp contributes 0.
-#ifndef LGF_DELTAQ_MINB
-#define LGF_DELTAQ_MINB 8
-#endif
-template <int NC>
-__global__ void __launch_bounds__(128, LGF_DELTAQ_MINB) k_delta_quad(const cplx* __restrict__ links, cplx* __restrict__ field, double2* __restrict__ partials,
-                                                                    Geom G, const Ctl* __restrict__ ctl) {
-    pdl_enter();
-    if (ctl->done) return;
-    __shared__ cplx sc[4][4][32];          // [direction][packed component][site]
-    __shared__ double red[64];
-    const int lane = threadIdx.x & 31, mu = threadIdx.x >> 5;
-    double th = 0, fs = 0;
-#pragma unroll 1
-    for (int it = 0; it < 4; it++) {       // 4 groups of 32 sites per CTA: one partial per 128 sites, as k_delta
-        const long long x = ((long long)blockIdx.x * 4 + it) * 32 + lane;
-        cplx d01 = mk(0, 0), d02 = mk(0, 0), d12 = mk(0, 0);
-        real i0 = 0, i1 = 0, i2 = 0, retr = 0;
-        if (mu < G.nd) {
-            cplx u[9];
-            load_link<NC>(links, G.V, mu, x, u);
-            retr = u[0].x + u[4].x + u[8].x;
-            acc_link(u, real(-1), d01, d02, d12, i0, i1, i2);
-            load_link<NC>(links, G.V, mu, bwd(G, x, mu), u);
-            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
-        }
-        // the diagonal part is linear too: e_j = 2 i_j - (2/3)(i0 + i1 + i2)
-        const real tr3 = real(2.0 / 3.0) * (i0 + i1 + i2);
-        if (it) __syncthreads();           // the previous group's sums have been read
-        sc[mu][0][lane] = d01; sc[mu][1][lane] = d02; sc[mu][2][lane] = d12;
-        sc[mu][3][lane] = mk(real(2) * i0 - tr3, real(2) * i1 - tr3);
-        __syncthreads();
-        const int c = mu;                  // this thread now owns packed component c of site x
-        const cplx f = cadd(cadd(sc[0][c][lane], sc[1][c][lane]), cadd(sc[2][c][lane], sc[3][c][lane]));
-        field[(long long)c * G.V + x] = f;
-        if (c < 3) th += (double)(real(2) * cnorm2(f));
-        else { const real e2 = -(f.x + f.y); th += (double)(f.x * f.x + f.y * f.y + e2 * e2); }
-        fs += (double)retr;
+// ------------------------------------------------------------------------------------------------ S5
+// The S5 decision, by one thread: record (F, theta), raise the stop flag when theta < theta_tol (converged), max_iter
+// updates have been applied, theta or F is not finite, or the stagnation guard fires.
+__device__ __forceinline__ void s5_decide(Ctl* ctl, double2* hist, double theta, double F) {
+    ctl->theta = theta; ctl->F = F;
+    const int k = ctl->n_meas;
+    if (k < ctl->hist_cap) hist[k] = make_double2(F, theta);
+    ctl->n_meas = k + 1;
+    if (!(isfinite(theta) && isfinite(F))) { ctl->nonfinite = 1; ctl->done = 1; }
+    else if (theta < ctl->theta_tol) { ctl->converged = 1; ctl->done = 1; }
+    else if (ctl->iters >= ctl->max_iter) { ctl->done = 1; }
+    else if (ctl->stall_window > 0) {
+        if (k == 0 || theta < 0.5 * ctl->theta_mark) { ctl->theta_mark = theta; ctl->stall_count = 0; }
+        else if (++ctl->stall_count >= ctl->stall_window) { ctl->stalled = 1; ctl->done = 1; }
     }
-    block_sum2(th, fs, red);
-    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
 }
 
-// ------------------------------------------------------------------------------------------------ S5
 // One block.  Sums the partials in a fixed order (strided per thread, then tree), writes F, theta, history,
 // and raises the stop flag: theta < theta_tol (converged), or max_iter updates applied, or non-finite.
-// advance != 0: the measured links are the result of an update applied by the same iteration body (fused update,
-// fused_update.cuh): count it and make the buffer it wrote the current one.
-__global__ void __launch_bounds__(1024) k_finalize(const double2* __restrict__ partials, int n, Ctl* ctl, double2* hist, double inv3V, double inv12V,
-                                                  int advance) {
+__global__ void __launch_bounds__(1024) k_finalize(const double2* __restrict__ partials, int n, Ctl* ctl, double2* hist, double inv3V, double inv12V) {
     pdl_enter();
     if (ctl->done) return;
     __shared__ double red[64];
@@ -163,15 +126,7 @@ __global__ void __launch_bounds__(1024) k_finalize(const double2* __restrict__ p
     for (int i = threadIdx.x; i < n; i += blockDim.x) { double2 p = partials[i]; a += p.x; b += p.y; }
     block_sum2(a, b, red);
     if (threadIdx.x == 0) {
-        const double theta = a * inv3V, F = b * inv12V;
-        ctl->theta = theta; ctl->F = F;
-        if (advance) { ctl->iters = ctl->iters + 1; ctl->parity = ctl->parity ^ 1; }
-        const int k = ctl->n_meas;
-        if (k < ctl->hist_cap) hist[k] = make_double2(F, theta);
-        ctl->n_meas = k + 1;
-        if (!(isfinite(theta) && isfinite(F))) { ctl->nonfinite = 1; ctl->done = 1; }
-        else if (theta < ctl->theta_tol) { ctl->converged = 1; ctl->done = 1; }
-        else if (ctl->iters >= ctl->max_iter) { ctl->done = 1; }
+        s5_decide(ctl, hist, a * inv3V, b * inv12V);
     }
 }
 
@@ -327,41 +282,27 @@ __global__ void __launch_bounds__(256) k_fft23_mid(cplx* __restrict__ field, Geo
 }
 
 // ------------------------------------------------------------------------------------------------ S3 + S4
-// One thread per site.  STORE_G = 0: g(x) and g(x+mu) are rebuilt from the packed X field (5 Gram-Schmidt per
-// site, 64 B/site read once from HBM, neighbours from L1/L2).  STORE_G = 1: rows 0,1 of g are read from gbuf
-// (96 B/site) and row 2 is rebuilt.  Each link (x,mu) is read and written by exactly one thread: in place.
-#ifndef LGF_UPD_NT
-#define LGF_UPD_NT 128
-#endif
-#ifndef LGF_UPD_MINB
-#define LGF_UPD_MINB 3
-#endif
-template <int NC, int STORE_G>
-__global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G, double half_alpha, Ctl* ctl) {
+// S3+S4 with a stored g field (LGF_OPT_STORE_G): one thread per site reads rows 0,1 of g(x) and g(x+mu) from gbuf
+// (96 B/site, written by pass C), rebuilds row 2 and rotates the four links of the site in place.  Each link (x,mu) is
+// read and written by exactly one thread.
+template <int NC>
+__global__ void __launch_bounds__(128, 3) k_update_g(cplx* links, const cplx* __restrict__ gbuf, Geom G, Ctl* ctl) {
     pdl_enter();
     if (ctl->done) return;
     const long long x = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long V = G.V;
     cplx g[9];
-    if (STORE_G) {
 #pragma unroll
-        for (int c = 0; c < 6; c++) g[c] = ldg2(src + (long long)c * V + x);
-        third_row(g);
-    } else {
-        build_g(ldc_field(src + x), ldc_field(src + V + x), ldc_field(src + 2 * V + x), ldc_field(src + 3 * V + x), (real)half_alpha, g);
-    }
+    for (int c = 0; c < 6; c++) g[c] = ldg2(gbuf + (long long)c * V + x);
+    third_row(g);
 #pragma unroll
     for (int mu = 0; mu < 4; mu++) {
         const long long xf = fwd(G, x, mu);
         cplx gp[9], u[9], r[9];
-        load_link<NC>(links, V, mu, x, u);
-        if (STORE_G) {
+        load_link<NC, false>(links, V, mu, x, u);
 #pragma unroll
-            for (int c = 0; c < 6; c++) gp[c] = ldg2(src + (long long)c * V + xf);
-            third_row(gp);
-        } else {
-            build_g(ldc_field(src + xf), ldc_field(src + V + xf), ldc_field(src + 2 * V + xf), ldc_field(src + 3 * V + xf), (real)half_alpha, gp);
-        }
+        for (int c = 0; c < 6; c++) gp[c] = ldg2(gbuf + (long long)c * V + xf);
+        third_row(gp);
         rotate_link<(NC == 6) ? 2 : 3>(g, u, gp, r);
         store_link<NC>(links, V, mu, x, r);
     }
@@ -370,7 +311,7 @@ __global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __res
 
 // One thread per link, four warps per CTA = the four directions of 32 consecutive sites.  Thread (x, mu) builds
 // g(x+mu) only; g(x) is what the mu = 0 thread of the site x-0 built (its forward neighbour is x), handed over
-// through shared memory: 4 Gram-Schmidt per site instead of 5 (one thread per site) or 8 (k_update_link).
+// through shared memory: 4 Gram-Schmidt per site instead of 5 (one thread per site) or 8 (no sharing).
 // A CTA covers whole x0 rows (NS = max(32, L0) sites, 4 NS threads), so the site x-0 is always in the same CTA.
 // Measured on B200 at 32^4 (CUDA events per launch): 149 us at 5 CTAs/SM (96 registers), 157 at 4, 157 at 6 (spills),
 // against 161 for one thread per site (k_update<NC,0>, 12 warps/SM); the IEEE 1/sqrt costs nothing measurable.
@@ -393,7 +334,7 @@ __global__ void __launch_bounds__(LGF_UPD_NT, LGF_UPD_MINB) k_update(cplx* __res
 // ACC: the mu = 1 thread of each site also accumulates the total gauge transformation, Gacc(x) <- g(x) Gacc(x)
 // (rows 0,1 in gacc, 6 V-arrays; mixed precision, lgf_api.cu): +2 x 6 complex per site.
 template <int NC, int NS, int ACC = 0>      // NS = sites per CTA = max(32, L0): 4 * NS threads, thread = (mu, site)
-__global__ void __launch_bounds__(4 * NS, (NS == 32) ? LGF_UPDQ_MINB : ((NS == 64) ? LGF_UPDQ_MINB64 : 1)) k_update_quad(cplx* __restrict__ links, const cplx* __restrict__ src, Geom G,
+__global__ void __launch_bounds__(4 * NS, (NS == 32) ? LGF_UPDQ_MINB : ((NS == 64) ? LGF_UPDQ_MINB64 : 1)) k_update_quad(cplx* links, const cplx* __restrict__ src, Geom G,
                                                                                        double half_alpha, Ctl* ctl, cplx* __restrict__ gacc = nullptr) {
     pdl_enter();
     if (ctl->done) return;
@@ -413,7 +354,7 @@ __global__ void __launch_bounds__(4 * NS, (NS == 32) ? LGF_UPDQ_MINB : ((NS == 6
         }
     }
 #endif
-    load_link<NC>(links, V, mu, x, u);
+    load_link<NC, false>(links, V, mu, x, u);
     build_g(ldc_field(src + xf), ldc_field(src + V + xf), ldc_field(src + 2 * V + xf), ldc_field(src + 3 * V + xf), (real)half_alpha, gp);
     if (mu == 0) {
         const int m = G.L[0] - 1;                             // L0 <= NS: the x0 row of a site lies inside its CTA
@@ -476,11 +417,11 @@ __device__ __forceinline__ void load_gacc64(const float2* __restrict__ gacc, lon
     third_row(g);
 }
 template <int NC>
-__global__ void __launch_bounds__(128) k_apply_gacc(cplx* __restrict__ links, const float2* __restrict__ gacc, Geom G) {
+__global__ void __launch_bounds__(128) k_apply_gacc(cplx* links, const float2* __restrict__ gacc, Geom G) {
     const int mu = blockIdx.x & 3;
     const long long x = (long long)(blockIdx.x >> 2) * 128 + threadIdx.x;
     cplx g[9], gp[9], u[9], r[9];
-    load_link<NC>(links, G.V, mu, x, u);
+    load_link<NC, false>(links, G.V, mu, x, u);
     load_gacc64(gacc, G.V, x, g);
     load_gacc64(gacc, G.V, fwd(G, x, mu), gp);
     rotate_link<(NC == 6) ? 2 : 3>(g, u, gp, r);

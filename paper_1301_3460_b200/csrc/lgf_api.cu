@@ -69,7 +69,6 @@ void* lgf32_x_gacc(lgf_ctx* c);
 
 #include "kernels.cuh"
 #include "fft_fast.cuh"
-#include "fused_update.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -83,17 +82,22 @@ using namespace lgf;
 namespace {
 
 enum KernelSlot {
-    K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_X, K_UPDATE_G,
-    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G, K_FU_UPDATE,
-    K_PP_DELTA_FWD, K_PP_MID, K_PP_INV, K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_FH_MID, K_NSLOTS
+    K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_G,
+    K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G,
+    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
-    "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_x", "k_update_g",
-    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g", "k_fu_update_delta_fwd",
-    "k_pp_delta_fwd", "k_pp_mid", "k_pp_inv", "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_fh_mid"};
+    "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_g",
+    "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g",
+    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd"};
 
 constexpr int HIST_CAP = 1 << 16;
+// mixed precision: the fp32 phase ends when theta has not halved within this many iterations (a rough thermalised
+// configuration at beta = 5.7 halves theta every ~30 iterations at alpha = 0.08; a wrong "stalled" only hands over early)
+#ifndef LGF_MIXED_STALL_WINDOW
+#define LGF_MIXED_STALL_WINDOW 256
+#endif
 constexpr long long STAGE_SITES = 1 << 17;   // sites per staging chunk of the boundary copies
 constexpr int MAX_SMEM = 200 * 1024;
 
@@ -101,7 +105,6 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {   // offsets into the workspace
     size_t links, field, gbuf, partials, ctl, hist, tables, scratch, staging, total;
-    size_t link_buf;        // bytes of one link buffer; the links region holds two (fused update: read one, write the other)
     int n_partials;
     long long stage_sites;
 };
@@ -121,8 +124,7 @@ Layout make_layout(const int dims[4], int NC) {
     Layout o;
     const long long V = (long long)dims[0] * dims[1] * dims[2] * dims[3];
     size_t off = 0;
-    o.link_buf = align_up((size_t)V * 4 * NC * sizeof(cplx), 256);
-    o.links = off; off += 2 * o.link_buf;
+    o.links = off; off = align_up(off + (size_t)V * 4 * NC * sizeof(cplx), 256);
     o.field = off; off = align_up(off + (size_t)V * 4 * sizeof(cplx), 256);
     o.gbuf = off; off = align_up(off + (size_t)V * 6 * sizeof(cplx), 256);
     o.n_partials = (int)(V / 128);                       // k_delta / k_plaquette: one per 128-site block
@@ -188,21 +190,23 @@ struct lgf_ctx {
     char* shadow_ws;        // its workspace when this context allocated it
     int acc_g;              // fp32 build: the update also accumulates Gacc(x) <- g(x) Gacc(x) in gbuf
     int mixed_n32;          // fp32 iterations of the last mixed lgf_fix
+    int mixed_switch;       // the fp32 phase aims at theta = 10^-mixed_switch (LGF_OPT_MIXED_SWITCH)
+    int stall_window;       // fp32 build, mixed precision: stagnation guard of the fp32 phase (Ctl::stall_window), 0 = off
     int pending_np;         // S5 inside pass B: partials of the S1 just enqueued that no k_finalize has reduced yet
-    // options
-    int opt_fuse, opt_store_g, opt_graph, opt_batch, opt_fast, opt_fuse_update, opt_pingpong, opt_fuse_fin, opt_quad, opt_pdl, opt_accel, opt_line, opt_delta_quad, opt_cluster;
-    int sms;                // SMs of the device: grid of the persistent passes
-    int parity;             // link buffer holding the current links (host mirror of Ctl::parity)
-    // fast (compile-time-sized) FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
-    bool fast_a, fast_b, fast_c, pp_b_ok, big_p, cl_ok;
-    size_t smem_fa, smem_fb, smem_fc, smem_fu, smem_pa, smem_pb, smem_p1, smem_cl;
+    // options (include/lgf.h lgf_option)
+    int opt_store_g, opt_graph, opt_batch, opt_fast, opt_pdl, opt_accel;
+    int sms;                // SMs of the device
+    // compile-time-sized FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
+    bool fast_a, fast_b, fast_c, big_p, cl_ok;
+    size_t smem_fa, smem_fb, smem_fc, smem_p1, smem_cl;
     int fb_lgC;
-    // derived launch parameters
+    // derived launch parameters of the generic passes
     int fft01_ncomp_fused_ok, fft01_ncomp, fft01_threads, fft23_lgC, fft23_S1, fft23_S2, fft23_threads;
     size_t smem01_fused, smem01, smem23;
-    // graph cache
+    // graph cache: the executable graph of opt_batch iteration bodies and the full selection it was captured with
+    struct GraphKey { double half_alpha; int nb, nd, acc_g, store_g, fast, pdl, accel; };
     cudaGraphExec_t graph_exec;
-    int graph_key;
+    GraphKey graph_key;
     // profiling
     int profiling;
     cudaEvent_t ev0, ev1;
@@ -227,8 +231,6 @@ namespace {
             return LGF_ERR_CUDA;                                                                           \
         }                                                                                                  \
     } while (0)
-
-cplx* cur_links(const lgf_ctx* c) { return c->links + (size_t)c->parity * (c->lay.link_buf / sizeof(cplx)); }
 
 // Profiling: resolve the event pairs recorded so far (one synchronisation for the whole batch, so the kernels run
 // back to back on the device and the pairs measure device time, not launch latency).
@@ -278,56 +280,24 @@ void launch_k(lgf_ctx* c, void (*kern)(KArgs...), unsigned grid, unsigned block,
     cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
-#ifndef LGF_CARVEOUT
-#define LGF_CARVEOUT 0
-#endif
 template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
-    // prefer the largest shared-memory carveout: the tile passes are limited by resident CTAs, not by L1
-    if (LGF_CARVEOUT) cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, LGF_CARVEOUT);
     return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
 }
 
-// ---- fast (compile-time-sized) FFT passes: the lattices they cover, and their launchers -----------------------
-#ifndef LGF_FA_NT
-#define LGF_FA_NT 256
-#endif
-#ifndef LGF_FC_NT
-#define LGF_FC_NT 256
-#endif
-constexpr int FA_NT = 256;            // group size of the ping-pong passes
-constexpr int FAD_NT = LGF_FA_NT;     // threads per CTA of pass A (k_fa_delta_fwd)
-constexpr int FC_NT = LGF_FC_NT;      // threads per CTA of pass C (k_fa_inv)
-#ifndef LGF_CL_NT
-#define LGF_CL_NT 256
-#endif
-constexpr int CL_NT = LGF_CL_NT;      // threads per CTA of the CTA-pair pass A (k_cl_delta_fwd)
-// (lg of the fast axis, lg of the slow axis) pairs instantiated for each pass
+// ---- compile-time-sized FFT passes (fft_fast.cuh): the lattices they cover, and their launchers ----------------
+constexpr int FAD_NT = 256;           // threads per CTA of pass A (k_fa_delta_fwd)
+constexpr int FC_NT = 256;            // threads per CTA of pass C (k_fa_inv) and of the one-component plane passes
+constexpr int CL_NT = 256;            // threads per CTA of the CTA-pair pass A (k_cl_delta_fwd)
+constexpr int FB_NT = 256;            // threads per CTA of the stage-wise pass B when its tile is below 100 KB
+// (lg of the fast axis, lg of the slow axis) pairs instantiated for each pass: extents 16 and 32 ...
 #define LGF_FAST_PAIRS(X) X(4, 4) X(4, 5) X(5, 4) X(5, 5)
-#ifndef LGF_FB_LGC55
-#ifdef LGF_F32_LGC55
-#define LGF_FB_LGC55 LGF_F32_LGC55
-#else
-#define LGF_FB_LGC55 2
-#endif
-#endif
-#ifndef LGF_FB_NT
-#define LGF_FB_NT 256
-#endif
-constexpr int FB_NT = LGF_FB_NT;
-// 64 extents: the (x0,x1) plane passes take one component per CTA (S1 stays a separate kernel: four 64 x 64 tiles do
-// not fit one SM), the (x2,x3) pass takes a shorter x0 chunk
+// ... and pairs with a 64 extent: the (x0,x1) plane passes take one component per CTA (four 64-wide tiles do not fit
+// one SM; 64 x 64 planes run S1 on CTA pairs, the others keep S1 a separate kernel), the (x2,x3) pass takes a shorter
+// x0 chunk
 #define LGF_BIG_PAIRS(X) X(5, 6) X(6, 5) X(6, 6)
-#ifndef LGF_FB_LGC11
-#define LGF_FB_LGC11 2
-#endif
-#ifndef LGF_FB_LGC12
-#define LGF_FB_LGC12 1
-#endif
 // x0 chunk of pass B (2^lgC sites): tile = 2^(lga+lgb+lgC) * 16 B
-constexpr int fast_mid_lgC(int lga, int lgb) {
-    return (lga + lgb <= 9) ? 3 : ((lga + lgb == 10) ? LGF_FB_LGC55 : ((lga + lgb == 11) ? LGF_FB_LGC11 : LGF_FB_LGC12));
-}
-// threads per CTA of pass B: one 512-thread CTA per SM when the tile is above 100 KB, else 2 x 256
+constexpr int fast_mid_lgC(int lga, int lgb) { return (lga + lgb <= 9) ? 3 : ((lga + lgb == 10) ? 2 : ((lga + lgb == 11) ? 2 : 1)); }
+// threads per CTA of the stage-wise pass B: one 512-thread CTA per SM when the tile is above 100 KB, else 2 x 256
 constexpr int fast_mid_nt(int lga, int lgb) { return ((16 << (lga + lgb + fast_mid_lgC(lga, lgb))) > 100 * 1024) ? 512 : FB_NT; }
 bool fast_pair(int lga, int lgb) {
 #define X(A, B) if (lga == A && lgb == B) return true;
@@ -347,13 +317,11 @@ size_t smem_fast_mid(int lga, int lgb, int lgC) {
     return (size_t)(S2 * (1 << lgb) + (1 << lga) + (1 << lgb)) * sizeof(cplx) + (size_t)((1 << lga) + (1 << lgb)) * 8;
 }
 
-// fin: the last CTA also does S5 (no k_finalize launch)
-template <int NC> void launch_fa_delta_fwd(lgf_ctx* c, bool fin) {
+template <int NC> void launch_fa_delta_fwd(lgf_ctx* c) {
     LaunchScope ls(c, K_FA_DELTA_FWD);
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
-    const FinArgs fa{c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (3.0 * (double)c->G.nd * (double)c->G.V), fin ? 1 : 0};
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        launch_k(c, k_fa_delta_fwd<A, B, NC, FAD_NT>, grid, FAD_NT, c->smem_fa, cur_links(c), c->field, c->partials, c->G, c->T, c->ctl, fa);
+        launch_k(c, k_fa_delta_fwd<A, B, NC, FAD_NT>, grid, FAD_NT, c->smem_fa, c->links, c->field, c->partials, c->G, c->T, c->ctl);
     LGF_FAST_PAIRS(X)
 #undef X
 }
@@ -377,7 +345,7 @@ void launch_fa_inv_g(lgf_ctx* c, double half_alpha) {
 template <int NC> void launch_cl_delta_fwd(lgf_ctx* c) {
     LaunchScope ls(c, K_CL_DELTA_FWD);
     const unsigned grid = (unsigned)(2 * c->G.L[2] * c->G.L[3]);
-    launch_k(c, k_cl_delta_fwd<6, 6, NC, CL_NT>, grid, CL_NT, c->smem_cl, cur_links(c), c->field, c->partials, c->G, c->T, c->ctl);
+    launch_k(c, k_cl_delta_fwd<6, 6, NC, CL_NT>, grid, CL_NT, c->smem_cl, c->links, c->field, c->partials, c->G, c->T, c->ctl);
 }
 // planes with a 64 extent: one component per CTA
 void launch_fa_fwd1(lgf_ctx* c) {
@@ -396,22 +364,13 @@ void launch_fa_inv1(lgf_ctx* c) {
     LGF_BIG_PAIRS(X)
 #undef X
 }
-// S3/S4 of this iteration + S1 and pass A of the next (fused_update.cuh); reads link buffer Ctl::parity, writes the other
-template <int NC> void launch_fu_update(lgf_ctx* c) {
-    LaunchScope ls(c, K_FU_UPDATE);
-    const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3]);
-    const long long stride = (long long)(c->lay.link_buf / sizeof(cplx));
-#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        launch_k(c, k_fu_update_delta_fwd<A, B, NC, LGF_FU_NT>, grid, LGF_FU_NT, c->smem_fu, c->links, stride, c->gbuf, c->field, c->partials, c->G, c->T, c->ctl);
-    LGF_FAST_PAIRS(X)
-#undef X
-}
 // S5 inside pass B: the pending number of partials of the S1 that just ran (0: k_finalize already did it)
 FinArgs pending_fin(lgf_ctx* c) {
     const FinArgs fa{c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (3.0 * (double)c->G.nd * (double)c->G.V), c->pending_np};
     c->pending_np = 0;
     return fa;
 }
+// pass B, stage-wise through shared memory: 64 extents
 void launch_fa_mid(lgf_ctx* c) {
     LaunchScope ls(c, K_FA_MID);
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
@@ -419,22 +378,10 @@ void launch_fa_mid(lgf_ctx* c) {
     const FinArgs fa = pending_fin(c);
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
         launch_k(c, k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, grid, fast_mid_nt(A, B), c->smem_fb, c->field, c->G, c->T, scale, c->ctl, c->partials, fa);
-    LGF_FAST_PAIRS(X) LGF_BIG_PAIRS(X)
+    LGF_BIG_PAIRS(X)
 #undef X
 }
-
 // pass B with whole lines in registers (fft_fast.cuh k_fr_mid): 16/32 extents
-// pass B with half a line per thread (k_fh_mid): LGF_OPT_LINE_FFT = 2
-void launch_fh_mid(lgf_ctx* c) {
-    LaunchScope ls(c, K_FH_MID);
-    const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
-    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
-    const FinArgs fa = pending_fin(c);
-#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        launch_k(c, k_fh_mid<A, B, fast_mid_lgC(A, B), 256>, grid, 256, c->smem_fb, c->field, c->G, c->T, scale, c->ctl, c->partials, fa);
-    LGF_FAST_PAIRS(X)
-#undef X
-}
 void launch_fr_mid(lgf_ctx* c) {
     LaunchScope ls(c, K_FR_MID);
     const unsigned grid = (unsigned)(4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
@@ -447,64 +394,27 @@ void launch_fr_mid(lgf_ctx* c) {
 #undef X
 }
 
-// persistent ping-pong forms of the three passes (fft_fast.cuh): one CTA per SM, two groups of FA_NT threads
-unsigned pp_grid(const lgf_ctx* c, long long items) { return (unsigned)(items < c->sms ? items : c->sms); }
-template <int NC> void launch_pp_delta_fwd(lgf_ctx* c) {
-    LaunchScope ls(c, K_PP_DELTA_FWD);
-    const unsigned grid = pp_grid(c, c->G.L[2] * c->G.L[3]);
-#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        launch_k(c, k_pp_delta_fwd<A, B, NC, FA_NT>, grid, 2 * FA_NT, c->smem_pa, cur_links(c), c->field, c->partials, c->G, c->T, c->ctl);
-    LGF_FAST_PAIRS(X)
-#undef X
-}
-void launch_pp_inv(lgf_ctx* c) {
-    LaunchScope ls(c, K_PP_INV);
-    const unsigned grid = pp_grid(c, c->G.L[2] * c->G.L[3]);
-#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        launch_k(c, k_pp_inv<A, B, FA_NT>, grid, 2 * FA_NT, c->smem_pa, c->field, c->G, c->T, c->ctl);
-    LGF_FAST_PAIRS(X)
-#undef X
-}
-void launch_pp_mid(lgf_ctx* c) {
-    LaunchScope ls(c, K_PP_MID);
-    const unsigned grid = pp_grid(c, 4LL * c->G.L[1] * (c->G.L[0] >> c->fb_lgC));
-    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
-#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        launch_k(c, k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, grid, 2 * FA_NT, c->smem_pb, c->field, c->G, c->T, scale, c->ctl);
-    LGF_FAST_PAIRS(X)
-#undef X
-}
-
 lgf_status setup_fast(lgf_ctx* c) {
     const Geom& G = c->G;
     c->fast_a = c->fast_c = fast_pair(G.lg[0], G.lg[1]);
     c->fast_b = fast_pair(G.lg[2], G.lg[3]) || big_pair(G.lg[2], G.lg[3]);
-    c->big_p = big_pair(G.lg[0], G.lg[1]);               // plane passes with one component per CTA, S1 separate
+    c->big_p = big_pair(G.lg[0], G.lg[1]);               // plane passes with one component per CTA
     c->smem_p1 = smem_fast_plane(G.lg[0], G.lg[1], 1);
     c->fb_lgC = fast_mid_lgC(G.lg[2], G.lg[3]);
     if (c->fb_lgC > G.lg[0]) c->fast_b = false;          // the x0 extent must hold one chunk
-    c->smem_fa = c->smem_fc = c->smem_fu = smem_fast_plane(G.lg[0], G.lg[1], 4);
+    c->smem_fa = c->smem_fc = smem_fast_plane(G.lg[0], G.lg[1], 4);
     c->smem_fb = smem_fast_mid(G.lg[2], G.lg[3], c->fb_lgC);
-    // two tiles + one set of tables
-    c->smem_pa = 2 * c->smem_fa - (size_t)(G.L[0] + G.L[1]) * sizeof(cplx);
-    c->smem_pb = 2 * c->smem_fb - ((size_t)(G.L[2] + G.L[3]) * sizeof(cplx) + (size_t)(G.L[2] + G.L[3]) * 8);
-    c->pp_b_ok = c->smem_pb <= (size_t)227 * 1024 && fast_pair(G.lg[2], G.lg[3]);
     if (c->fast_a) {
 #define X(A, B) if (G.lg[0] == A && G.lg[1] == B) { \
             CK(set_smem(k_fa_delta_fwd<A, B, 6, FAD_NT>, c->smem_fa)); CK(set_smem(k_fa_delta_fwd<A, B, 9, FAD_NT>, c->smem_fa)); \
-            CK(set_smem(k_fa_inv<A, B, 4, FC_NT, false>, c->smem_fc)); CK(set_smem(k_fa_inv<A, B, 4, FC_NT, true>, c->smem_fc)); \
-            CK(set_smem(k_fu_update_delta_fwd<A, B, 6, LGF_FU_NT>, c->smem_fu)); CK(set_smem(k_fu_update_delta_fwd<A, B, 9, LGF_FU_NT>, c->smem_fu)); \
-            CK(set_smem(k_pp_delta_fwd<A, B, 6, FA_NT>, c->smem_pa)); CK(set_smem(k_pp_delta_fwd<A, B, 9, FA_NT>, c->smem_pa)); \
-            CK(set_smem(k_pp_inv<A, B, FA_NT>, c->smem_pa)); }
+            CK(set_smem(k_fa_inv<A, B, 4, FC_NT, false>, c->smem_fc)); CK(set_smem(k_fa_inv<A, B, 4, FC_NT, true>, c->smem_fc)); }
         LGF_FAST_PAIRS(X)
 #undef X
     }
     if (c->fast_b) {
-#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) { CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb)); \
+#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) { \
             CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, false>, c->smem_fb)); \
-            CK(set_smem(k_fh_mid<A, B, fast_mid_lgC(A, B), 256>, c->smem_fb)); \
-            CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, true>, c->smem_fb)); \
-            if (c->pp_b_ok) CK(set_smem(k_pp_mid<A, B, fast_mid_lgC(A, B), FA_NT>, c->smem_pb)); }
+            CK(set_smem(k_fr_mid<A, B, fast_mid_lgC(A, B), LGF_FR_NT, true>, c->smem_fb)); }
         LGF_FAST_PAIRS(X)
 #undef X
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb));
@@ -594,19 +504,18 @@ lgf_status build_tables(lgf_ctx* c) {
     return LGF_OK;
 }
 
-// ---- kernel launchers ---------------------------------------------------------------------------------------
+// ---- generic kernel launchers -------------------------------------------------------------------------------
 template <int NC> void launch_delta(lgf_ctx* c) {
     LaunchScope ls(c, K_DELTA);
-    if (c->opt_delta_quad) { launch_k(c, k_delta_quad<NC>, (unsigned)(c->G.V / 128), 128, 0, cur_links(c), c->field, c->partials, c->G, c->ctl); return; }
-    launch_k(c, k_delta<NC>, (unsigned)(c->G.V / 128), 128, 0, cur_links(c), c->field, c->partials, c->G, c->ctl);
+    launch_k(c, k_delta<NC>, (unsigned)(c->G.V / 128), 128, 0, c->links, c->field, c->partials, c->G, c->ctl);
 }
 template <int MODE, int NC> void launch_fft01(lgf_ctx* c, int slot, double half_alpha) {
     LaunchScope ls(c, slot);
     const bool fused = (MODE == MODE_DELTA_FWD || MODE == MODE_INV_G);
     const int ncomp = fused ? 4 : c->fft01_ncomp;
     const unsigned grid = (unsigned)(c->G.L[2] * c->G.L[3] * (4 / ncomp));
-    launch_k(c, k_fft01<MODE, NC>, grid, c->fft01_threads, fused ? c->smem01_fused : c->smem01, 
-        c->field, cur_links(c), c->gbuf, c->partials, c->G, c->T, ncomp, half_alpha, c->ctl);
+    launch_k(c, k_fft01<MODE, NC>, grid, c->fft01_threads, fused ? c->smem01_fused : c->smem01,
+        c->field, c->links, c->gbuf, c->partials, c->G, c->T, ncomp, half_alpha, c->ctl);
 }
 void launch_fft23(lgf_ctx* c) {
     LaunchScope ls(c, K_FFT23_MID);
@@ -614,47 +523,47 @@ void launch_fft23(lgf_ctx* c) {
     launch_k(c, k_fft23_mid, grid, c->fft23_threads, c->smem23, c->field, c->G, c->T, c->fft23_lgC, c->fft23_S1, c->fft23_S2,
                                                                    4.0 * (double)c->G.nd / (double)c->G.V, c->ctl);
 }
-void launch_finalize(lgf_ctx* c, int n_partials, int advance = 0) {
+void launch_finalize(lgf_ctx* c, int n_partials) {
     LaunchScope ls(c, K_FINALIZE);
-    launch_k(c, k_finalize, 1, n_partials > 8192 ? 1024 : 256, 0, c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (3.0 * (double)c->G.nd * (double)c->G.V), advance);
+    launch_k(c, k_finalize, 1, n_partials > 8192 ? 1024 : 256, 0, c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (3.0 * (double)c->G.nd * (double)c->G.V));
 }
-template <int NC, int SG> void launch_update(lgf_ctx* c, double half_alpha) {
-    if (!SG && c->opt_quad) {
-        LaunchScope ls(c, K_UPDATE_QUAD);
-        cplx* const no_acc = nullptr;
-        if (c->acc_g) {
-            if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32, 1>, (unsigned)(c->G.V / 32), 128, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, c->gbuf);
-            else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64, 1>, (unsigned)(c->G.V / 64), 256, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, c->gbuf);
-            else launch_k(c, k_update_quad<NC, 128, 1>, (unsigned)(c->G.V / 128), 512, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, c->gbuf);
-        }
-        else if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32>, (unsigned)(c->G.V / 32), 128, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, no_acc);
-        else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64>, (unsigned)(c->G.V / 64), 256, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, no_acc);
-        else launch_k(c, k_update_quad<NC, 128>, (unsigned)(c->G.V / 128), 512, 0, cur_links(c), c->field, c->G, half_alpha, c->ctl, no_acc);
-        return;
+// S3+S4, g rebuilt from X: one thread per link
+template <int NC> void launch_update_quad(lgf_ctx* c, double half_alpha) {
+    LaunchScope ls(c, K_UPDATE_QUAD);
+    cplx* const no_acc = nullptr;
+    if (c->acc_g) {
+        if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32, 1>, (unsigned)(c->G.V / 32), 128, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
+        else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64, 1>, (unsigned)(c->G.V / 64), 256, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
+        else launch_k(c, k_update_quad<NC, 128, 1>, (unsigned)(c->G.V / 128), 512, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
     }
-    LaunchScope ls(c, SG ? K_UPDATE_G : K_UPDATE_X);
-    launch_k(c, k_update<NC, SG>, (unsigned)(c->G.V / LGF_UPD_NT), LGF_UPD_NT, 0, cur_links(c), SG ? c->gbuf : c->field, c->G, half_alpha, c->ctl);
+    else if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32>, (unsigned)(c->G.V / 32), 128, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
+    else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64>, (unsigned)(c->G.V / 64), 256, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
+    else launch_k(c, k_update_quad<NC, 128>, (unsigned)(c->G.V / 128), 512, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
+}
+// S3+S4 with g read from gbuf (LGF_OPT_STORE_G)
+template <int NC> void launch_update_g(lgf_ctx* c) {
+    LaunchScope ls(c, K_UPDATE_G);
+    launch_k(c, k_update_g<NC>, (unsigned)(c->G.V / 128), 128, 0, c->links, c->gbuf, c->G, c->ctl);
 }
 
-bool use_fused(const lgf_ctx* c) { return c->opt_fuse && c->fft01_ncomp_fused_ok; }
-bool use_store_g(const lgf_ctx* c) { return c->opt_store_g && c->fft01_ncomp_fused_ok; }
-bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a && use_fused(c); }
+// ---- kernel selection ------------------------------------------------------------------------------------------
+// S1 is fused into pass A wherever the four component tiles of a plane fit one SM (or a CTA pair at 64 x 64)
+bool use_fused(const lgf_ctx* c) { return c->fft01_ncomp_fused_ok; }
+// the accumulating update of the mixed-precision fp32 phase is k_update_quad only
+bool use_store_g(const lgf_ctx* c) { return c->opt_store_g && c->fft01_ncomp_fused_ok && !c->acc_g; }
+bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a; }
 bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
-bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c && !use_store_g(c); }
-bool use_fused_update(const lgf_ctx* c) { return c->opt_accel && c->G.nd == 4 && c->opt_fuse_update && c->opt_fast && c->fast_a; }
-bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p && !use_store_g(c); }
-bool use_cluster_a(const lgf_ctx* c) { return use_big_p(c) && c->cl_ok && c->opt_cluster && c->opt_fuse; }
-bool use_pp_a(const lgf_ctx* c) { return (c->opt_pingpong & 1) && use_fast_a(c); }
-bool use_pp_b(const lgf_ctx* c) { return (c->opt_pingpong & 2) && use_fast_b(c) && c->pp_b_ok; }
-bool use_pp_c(const lgf_ctx* c) { return (c->opt_pingpong & 4) && use_fast_c(c); }
+bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c; }
+bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p; }
+bool use_cluster_a(const lgf_ctx* c) { return use_big_p(c) && c->cl_ok; }
+bool use_line_b(const lgf_ctx* c) { return use_fast_b(c) && fast_pair(c->G.lg[2], c->G.lg[3]); }
+// S5 inside pass B's first CTA, where pass B is one of the compile-time-sized kernels
+bool use_fin_b(const lgf_ctx* c) { return c->opt_accel && use_fast_b(c); }
 
-// S5 inside pass B's first CTA: LGF_OPT_FUSE_FINALIZE = 2, where pass B is one of the compile-time-sized kernels
-bool use_fin_b(const lgf_ctx* c) { return c->opt_fuse_fin == 2 && c->opt_accel && use_fast_b(c) && !use_pp_b(c) && !use_fused_update(c); }
-// S1 (+ pass A) and the reduction.  Returns the number of partials written.
+// S1 (+ pass A) and, unless pass B does it, the reduction.
 template <int NC> void enqueue_head(lgf_ctx* c) {
     int np;
-    if (use_pp_a(c)) { launch_pp_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
-    else if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c, c->opt_fuse_fin == 1); if (c->opt_fuse_fin == 1) return; np = c->G.L[2] * c->G.L[3]; }
+    if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
     else if (use_cluster_a(c)) { launch_cl_delta_fwd<NC>(c); np = 2 * c->G.L[2] * c->G.L[3]; }
     else if (use_big_p(c)) { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fa_fwd1(c); }
     else if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
@@ -662,60 +571,45 @@ template <int NC> void enqueue_head(lgf_ctx* c) {
     if (use_fin_b(c)) { c->pending_np = np; return; }     // pass B's CTA 0 reduces them (every head here is followed by a pass B)
     launch_finalize(c, np);
 }
-// pass B, pass C, update
-bool use_line_b(const lgf_ctx* c) { return c->opt_line && use_fast_b(c) && fast_pair(c->G.lg[2], c->G.lg[3]); }
-void launch_mid_once(lgf_ctx* c);
 void launch_mid(lgf_ctx* c) {
-    launch_mid_once(c);
-#ifdef LGF_DBG_MID2          // timing experiment: a second pass B right behind the first (field then L2-resident)
-    launch_mid_once(c);
-#endif
-}
-void launch_mid_once(lgf_ctx* c) {
-    if (use_pp_b(c)) launch_pp_mid(c); else if (use_line_b(c) && c->opt_line == 2 && c->G.nd == 4) launch_fh_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
+    if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
 }
 void launch_inv_x(lgf_ctx* c) {
-    if (use_pp_c(c)) launch_pp_inv(c); else if (use_fast_c(c)) launch_fa_inv(c); else if (use_big_p(c)) launch_fa_inv1(c);
+    if (use_fast_c(c)) launch_fa_inv(c); else if (use_big_p(c)) launch_fa_inv1(c);
     else launch_fft01<MODE_INV, 6>(c, K_FFT01_INV, 0.0);
+}
+// pass C ending in g (rows 0,1 -> gbuf)
+void launch_inv_g(lgf_ctx* c, double half_alpha) {
+    if (use_fast_c(c)) launch_fa_inv_g(c, half_alpha); else launch_fft01<MODE_INV_G, 6>(c, K_FFT01_INV_G, half_alpha);
 }
 template <int NC> void enqueue_tail(lgf_ctx* c, double half_alpha) {
     launch_mid(c);
-    if (use_store_g(c)) { launch_fft01<MODE_INV_G, 6>(c, K_FFT01_INV_G, half_alpha); launch_update<NC, 1>(c, half_alpha); }
-    else { launch_inv_x(c); launch_update<NC, 0>(c, half_alpha); }
+    if (use_store_g(c)) { launch_inv_g(c, half_alpha); launch_update_g<NC>(c); }
+    else { launch_inv_x(c); launch_update_quad<NC>(c, half_alpha); }
 }
 void enqueue_body(lgf_ctx* c, double half_alpha) {
     if (!c->opt_accel) {
         // plain steepest descent (no Fourier acceleration, PAPER.md:41 refs [1],[2]): X = Delta, so S2 drops out
-        if (c->NC == 6) { launch_delta<6>(c); launch_finalize(c, (int)(c->G.V / 128)); launch_update<6, 0>(c, half_alpha); }
-        else { launch_delta<9>(c); launch_finalize(c, (int)(c->G.V / 128)); launch_update<9, 0>(c, half_alpha); }
-        return;
-    }
-    if (use_fused_update(c)) {
-        // pass B, pass C ending in g, then update + next Delta + next pass A, and the measurement of the updated links
-        launch_mid(c);
-        launch_fa_inv_g(c, half_alpha);
-        if (c->NC == 6) launch_fu_update<6>(c); else launch_fu_update<9>(c);
-        launch_finalize(c, c->G.L[2] * c->G.L[3], 1);
+        if (c->NC == 6) { launch_delta<6>(c); launch_finalize(c, (int)(c->G.V / 128)); launch_update_quad<6>(c, half_alpha); }
+        else { launch_delta<9>(c); launch_finalize(c, (int)(c->G.V / 128)); launch_update_quad<9>(c, half_alpha); }
         return;
     }
     if (c->NC == 6) { enqueue_head<6>(c); enqueue_tail<6>(c, half_alpha); }
     else { enqueue_head<9>(c); enqueue_tail<9>(c, half_alpha); }
 }
-bool use_fused_fin(const lgf_ctx* c) { return (c->opt_fuse_fin == 1 && use_fast_a(c) && !use_pp_a(c)) || use_fin_b(c); }
 int launches_per_body(const lgf_ctx* c) {
     if (!c->opt_accel) return 3;
-    if (use_fused_update(c)) return 4;
     int n;                                               // with a k_finalize launch
-    if (use_pp_a(c) || use_fast_a(c) || use_cluster_a(c)) n = 5;
+    if (use_fast_a(c) || use_cluster_a(c)) n = 5;
     else if (use_big_p(c)) n = 6;
     else n = use_fused(c) ? 5 : 6;
-    if (use_fused_fin(c)) n -= 1;                        // S5 inside pass A's last CTA or pass B's first
+    if (use_fin_b(c)) n -= 1;                            // S5 inside pass B's first CTA
     return n;
 }
 
 lgf_status reset_ctl(lgf_ctx* c, double tol, int max_iter) {
     Ctl h; memset(&h, 0, sizeof h);
-    h.theta_tol = tol; h.max_iter = max_iter; h.hist_cap = HIST_CAP; h.parity = c->parity;
+    h.theta_tol = tol; h.max_iter = max_iter; h.hist_cap = HIST_CAP; h.stall_window = c->stall_window;
     *c->h_ctl = h;
     CK(cudaMemcpyAsync(c->ctl, c->h_ctl, sizeof(Ctl), cudaMemcpyHostToDevice, c->stream));
     return LGF_OK;
@@ -723,7 +617,6 @@ lgf_status reset_ctl(lgf_ctx* c, double tol, int max_iter) {
 lgf_status read_ctl(lgf_ctx* c) {
     CK(cudaMemcpyAsync(c->h_ctl, c->ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
-    c->parity = c->h_ctl->parity;
     return LGF_OK;
 }
 
@@ -736,12 +629,14 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
         CK(cudaGetLastError());
         return LGF_OK;
     }
-    // alpha enters the graph as a kernel argument, so it is part of the key
-    union { double d; unsigned long long u; } au; au.d = half_alpha;
-    // the separate kernels take the current link buffer as an argument, so its parity is part of the key too
-    const int key = (int)((au.u ^ (au.u >> 32)) & 0x7fffffff) ^ (use_fused(c) << 1) ^ (use_store_g(c) << 2) ^ (c->opt_fast << 3) ^
-                    (use_fused_update(c) << 4) ^ (c->parity << 5) ^ (nb << 8) ^ (c->opt_pingpong << 20) ^ (c->opt_fuse_fin << 24) ^ (c->opt_quad << 25) ^ (c->opt_pdl << 26) ^ (c->opt_accel << 27) ^ (c->acc_g << 28) ^ ((c->G.nd == 3) << 29) ^ (c->opt_line << 30) ^ (c->opt_delta_quad << 19) ^ (c->opt_cluster << 18);
-    if (!c->graph_exec || c->graph_key != key) {
+    // Everything that is baked into the captured launches (alpha as a kernel argument, the kernel selection) is kept
+    // as a full tuple beside the executable graph and compared member by member: a hash could collide and silently
+    // replay a stale graph.
+    lgf_ctx::GraphKey key;
+    memset(&key, 0, sizeof key);
+    key.half_alpha = half_alpha; key.nb = nb; key.nd = c->G.nd; key.acc_g = c->acc_g; key.store_g = use_store_g(c) ? 1 : 0;
+    key.fast = c->opt_fast; key.pdl = c->opt_pdl; key.accel = c->opt_accel;
+    if (!c->graph_exec || memcmp(&c->graph_key, &key, sizeof key) != 0) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
         CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
@@ -765,13 +660,6 @@ lgf_status run(lgf_ctx* c, double alpha, double tol, int max_iter, bool poll) {
     if (st != LGF_OK) return st;
     const double ha = 0.5 * alpha;
     long long bodies_left = (long long)max_iter + 1;
-    if (use_fused_update(c)) {
-        // measurement 0 (S1 + pass A of the first iteration); every later measurement is made by the fused update
-        if (c->NC == 6) enqueue_head<6>(c); else enqueue_head<9>(c);
-        CK(cudaGetLastError());
-        bodies_left = max_iter;
-        if (bodies_left == 0) { st = read_ctl(c); if (st != LGF_OK) return st; }
-    }
     while (bodies_left > 0) {
         int nb = (int)(bodies_left < c->opt_batch ? bodies_left : c->opt_batch);
         st = enqueue_bodies(c, nb, ha);
@@ -810,11 +698,10 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_fuse = 1; c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_fuse_update = 0; c->opt_pingpong = 0; c->opt_fuse_fin = 2; c->opt_quad = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_line = 1; c->opt_delta_quad = 0; c->opt_cluster = 1;
+    c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_pdl = 1; c->opt_accel = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
-    c->parity = 0;
-    c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0; c->pending_np = 0;
-    c->graph_exec = nullptr; c->graph_key = 0; c->profiling = 0; c->launches = 0; c->capturing = false;
+    c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0; c->mixed_switch = 12; c->pending_np = 0; c->stall_window = 0;
+    c->graph_exec = nullptr; memset(&c->graph_key, 0, sizeof c->graph_key); c->profiling = 0; c->launches = 0; c->capturing = false;
     c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
 
@@ -848,7 +735,6 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
 
 lgf_status load_from_device_chunks(lgf_ctx* c, const double* src, bool src_is_host) {
     const long long V = c->G.V, S = c->lay.stage_sites;
-    c->parity = 0;          // a load fills link buffer 0
     for (long long off = 0; off < V; off += S) {
         const long long n = (V - off < S) ? V - off : S;
         const dcplx* aos;
@@ -877,8 +763,8 @@ lgf_status get_to_chunks(lgf_ctx* c, double* dst, bool dst_is_host) {
         {
             LaunchScope ls(c, K_LAYOUT_OUT);
             const unsigned grid = (unsigned)((n * 4 + 255) / 256);
-            if (c->NC == 6) k_layout_out<6><<<grid, 256, 0, c->stream>>>(cur_links(c), aos, V, off, n);
-            else k_layout_out<9><<<grid, 256, 0, c->stream>>>(cur_links(c), aos, V, off, n);
+            if (c->NC == 6) k_layout_out<6><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n);
+            else k_layout_out<9><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n);
         }
         CK(cudaGetLastError());
         if (dst_is_host) CK(cudaMemcpyAsync(dst + off * 72, c->staging, (size_t)n * 576, cudaMemcpyDeviceToHost, c->stream));
@@ -989,8 +875,8 @@ lgf_status lgf_get_links_device(lgf_ctx* c, double* dev_links) {
 
 #ifdef LGF_F32
 void* lgf32_x_begin(lgf_ctx* c) {
-    c->parity = 0; c->loaded = true; c->acc_g = 1;
-    c->opt_quad = 1; c->opt_store_g = 0; c->opt_fuse_update = 0;
+    c->loaded = true; c->acc_g = 1;
+    c->stall_window = LGF_MIXED_STALL_WINDOW;
     LaunchScope ls(c, K_MISC);
     k_init_gacc<<<(unsigned)((c->G.V + 255) / 256), 256, 0, c->stream>>>(c->gbuf, c->G.V);
     return c->links;
@@ -1016,14 +902,18 @@ lgf_status lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int
     int n32 = 0;
 #ifndef LGF_F32
     if (c->shadow) {
-        // Mixed precision.  Phase 1: a float copy of the links is fixed in fp32 down to theta_sw (above the fp32 floor of
-        // ~1e-14) while the fp32 update accumulates the total transformation Gacc(x).  Phase 2: the fp64 links receive
-        // Gacc in one step (re-orthonormalised in double: an exact gauge copy of the input) and the fp64 iteration
-        // takes theta from the fp32 noise level to theta_tol.
-        const double theta_sw = theta_tol > 1e-12 ? theta_tol : 1e-12;
+        // Mixed precision.  Phase 1: a float copy of the links is fixed in fp32 down to theta_sw while the fp32 update
+        // accumulates the total transformation Gacc(x).  The fp32 floor of theta is 1e-14..1e-12 (round-off of Delta
+        // amplified by p2max/p2min, which grows as L^2), so theta_sw may be out of reach: the phase also ends when theta
+        // has not halved within LGF_MIXED_STALL_WINDOW iterations (stagnation guard, Ctl::stall_window) -- never by
+        // exhausting max_iter on a stalled fp32 run.  Phase 2: the fp64 links receive Gacc in one step (re-orthonormalised
+        // in double: an exact gauge copy of the input) and the fp64 iteration takes theta to theta_tol with the remaining
+        // budget.
+        const double sw = pow(10.0, -(double)c->mixed_switch);
+        const double theta_sw = theta_tol > sw ? theta_tol : sw;
         float2* l32 = static_cast<float2*>(lgf32_x_begin(c->shadow));
         const long long n = 4LL * c->NC * c->G.V;
-        { LaunchScope ls(c, K_MISC); k_demote<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(cur_links(c), l32, n); }
+        { LaunchScope ls(c, K_MISC); k_demote<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->links, l32, n); }
         CK(cudaGetLastError());
         double F32v = 0, th32 = 0;
         lgf_status s1 = lgf32_fix(c->shadow, alpha, theta_sw, max_iter, &n32, &F32v, &th32);
@@ -1031,8 +921,8 @@ lgf_status lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int
         {
             LaunchScope ls(c, K_MISC);
             const float2* ga = static_cast<const float2*>(lgf32_x_gacc(c->shadow));
-            if (c->NC == 6) k_apply_gacc<6><<<(unsigned)(4 * (c->G.V / 128)), 128, 0, c->stream>>>(cur_links(c), ga, c->G);
-            else k_apply_gacc<9><<<(unsigned)(4 * (c->G.V / 128)), 128, 0, c->stream>>>(cur_links(c), ga, c->G);
+            if (c->NC == 6) k_apply_gacc<6><<<(unsigned)(4 * (c->G.V / 128)), 128, 0, c->stream>>>(c->links, ga, c->G);
+            else k_apply_gacc<9><<<(unsigned)(4 * (c->G.V / 128)), 128, 0, c->stream>>>(c->links, ga, c->G);
         }
         CK(cudaGetLastError());
         c->mixed_n32 = n32;
@@ -1057,8 +947,8 @@ lgf_status lgf_measure(lgf_ctx* c, double* F, double* theta, double* plaq) {
     launch_finalize(c, (int)(c->G.V / 128));
     {
         LaunchScope ls(c, K_PLAQUETTE);
-        if (c->NC == 6) k_plaquette<6><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(cur_links(c), c->partials, c->G);
-        else k_plaquette<9><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(cur_links(c), c->partials, c->G);
+        if (c->NC == 6) k_plaquette<6><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, c->partials, c->G);
+        else k_plaquette<9><<<(unsigned)(c->G.V / 128), 128, 0, c->stream>>>(c->links, c->partials, c->G);
     }
     double* sums = reinterpret_cast<double*>(c->ws + c->lay.scratch);
     {
@@ -1103,7 +993,7 @@ lgf_status lgf_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host
     } else {
         if (c->NC == 6) enqueue_head<6>(c); else enqueue_head<9>(c);
         launch_mid(c);
-        if (which == LGF_FIELD_G && use_store_g(c)) { launch_fft01<MODE_INV_G, 6>(c, K_FFT01_INV_G, ha); g_from_buf = true; }
+        if (which == LGF_FIELD_G && use_store_g(c)) { launch_inv_g(c, ha); g_from_buf = true; }
         else launch_inv_x(c);
     }
     CK(cudaGetLastError());
@@ -1134,20 +1024,13 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
     }
 #endif
     switch (opt) {
-        case LGF_OPT_FUSE_DELTA_FFT: c->opt_fuse = value ? 1 : 0; break;
         case LGF_OPT_STORE_G: c->opt_store_g = value ? 1 : 0; break;
         case LGF_OPT_GRAPH: c->opt_graph = value ? 1 : 0; break;
         case LGF_OPT_BATCH: if (value < 1 || value > 1024) return LGF_ERR_INVALID_ARG; c->opt_batch = value; break;
-        case LGF_OPT_FAST_FFT: c->opt_fast = value ? 1 : 0; break;
-        case LGF_OPT_FUSE_UPDATE: c->opt_fuse_update = value ? 1 : 0; break;
-        case LGF_OPT_PINGPONG: if (value < 0 || value > 7) return LGF_ERR_INVALID_ARG; c->opt_pingpong = value; break;
-        case LGF_OPT_FUSE_FINALIZE: if (value < 0 || value > 2) return LGF_ERR_INVALID_ARG; c->opt_fuse_fin = value; break;
-        case LGF_OPT_QUAD_UPDATE: c->opt_quad = value ? 1 : 0; break;
         case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
+        case LGF_OPT_FAST_FFT: c->opt_fast = value ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
-        case LGF_OPT_LINE_FFT: if (value < 0 || value > 2) return LGF_ERR_INVALID_ARG; c->opt_line = value; break;
-        case LGF_OPT_QUAD_DELTA: c->opt_delta_quad = value ? 1 : 0; break;
-        case LGF_OPT_CLUSTER_PASS_A: c->opt_cluster = value ? 1 : 0; break;
+        case LGF_OPT_MIXED_SWITCH: if (value < 4 || value > 20) return LGF_ERR_INVALID_ARG; c->mixed_switch = value; break;
         case LGF_OPT_GAUGE_DIRECTIONS: {
             if (value != 3 && value != 4) return LGF_ERR_INVALID_ARG;
             c->G.nd = value;
@@ -1163,22 +1046,15 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
     FWD32(lgf32_get_option(c, opt, value))
     if (!c || !value) return LGF_ERR_INVALID_ARG;
     switch (opt) {
-        case LGF_OPT_FUSE_DELTA_FFT: *value = use_fused(c); break;
-        case LGF_OPT_STORE_G: *value = use_store_g(c); break;
+        case LGF_OPT_STORE_G: *value = use_store_g(c) ? 1 : 0; break;
         case LGF_OPT_GRAPH: *value = c->opt_graph; break;
         case LGF_OPT_BATCH: *value = c->opt_batch; break;
-        case LGF_OPT_FAST_FFT: *value = ((use_fast_a(c) || use_big_p(c)) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | ((use_fast_c(c) || use_big_p(c)) ? 4 : 0); break;
-        case LGF_OPT_FUSE_UPDATE: *value = use_fused_update(c) ? 1 : 0; break;
-        case LGF_OPT_PINGPONG: *value = (use_pp_a(c) ? 1 : 0) | (use_pp_b(c) ? 2 : 0) | (use_pp_c(c) ? 4 : 0); break;
-        case LGF_OPT_FUSE_FINALIZE: *value = use_fin_b(c) ? 2 : ((c->opt_fuse_fin == 1 && use_fast_a(c) && !use_pp_a(c)) ? 1 : 0); break;
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
+        case LGF_OPT_FAST_FFT: *value = ((use_fast_a(c) || use_big_p(c)) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | ((use_fast_c(c) || use_big_p(c)) ? 4 : 0); break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
-        case LGF_OPT_QUAD_DELTA: *value = c->opt_delta_quad; break;
-        case LGF_OPT_CLUSTER_PASS_A: *value = use_cluster_a(c) ? 1 : 0; break;
-        case LGF_OPT_LINE_FFT: *value = (use_line_b(c) && !use_pp_b(c)) ? ((c->opt_line == 2 && c->G.nd == 4) ? 2 : 1) : 0; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;
-        case LGF_OPT_QUAD_UPDATE: *value = (c->opt_quad && !use_store_g(c) && !use_fused_update(c)) ? 1 : 0; break;
+        case LGF_OPT_MIXED_SWITCH: *value = c->mixed_switch; break;
         default: return LGF_ERR_INVALID_ARG;
     }
     return LGF_OK;
@@ -1200,7 +1076,7 @@ lgf_status lgf_get_profile(lgf_ctx* c, double ms[LGF_MAX_KERNELS], long long n[L
     return LGF_OK;
 }
 #ifndef LGF_F32
-const char* lgf_kernel_name(int slot) { return (slot >= 0 && slot < LGF_MAX_KERNELS) ? kKernelNames[slot] : ""; }
+const char* lgf_kernel_name(int slot) { return (slot >= 0 && slot < K_NSLOTS) ? kKernelNames[slot] : ""; }
 #endif
 long long lgf_launch_count(lgf_ctx* c) {
     FWD32(lgf32_launch_count(c))

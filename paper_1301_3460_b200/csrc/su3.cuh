@@ -53,63 +53,11 @@ __device__ __forceinline__ void third_row(cplx (&u)[9]) {
 // 128-bit loads/stores of one complex double
 __device__ __forceinline__ cplx ldg2(const cplx* p) { return __ldg(p); }
 
-// L2 residency control (createpolicy + ld/st .L2::cache_hint).  The packed field (64 B/site: 67 MB at 32^4) is
-// touched by every kernel of an iteration and fits the 126 MB L2; the links (384 B/site) are streamed once per
-// kernel and do not.  LGF_L2HINT bit 0: field accesses evict_last; bit 1: link accesses evict_first.
-#ifndef LGF_L2HINT
-#define LGF_L2HINT 0
-#endif
-#ifdef LGF_F32
-#undef LGF_L2HINT
-#define LGF_L2HINT 0        // the hinted accesses below are written for 16-byte complex
-#endif
-__device__ __forceinline__ unsigned long long l2_policy_last() {
-    unsigned long long p; asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
-}
-__device__ __forceinline__ unsigned long long l2_policy_first() {
-    unsigned long long p; asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
-}
-#ifndef LGF_F32
-__device__ __forceinline__ cplx ld_hint(const cplx* p, unsigned long long pol) {
-    cplx v; asm volatile("ld.global.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol)); return v;
-}
-__device__ __forceinline__ cplx ldnc_hint(const cplx* p, unsigned long long pol) {
-    cplx v; asm("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol)); return v;
-}
-__device__ __forceinline__ void st_hint(cplx* p, cplx v, unsigned long long pol) {
-    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
-}
-#else
-__device__ __forceinline__ cplx ld_hint(const cplx* p, unsigned long long) { return *p; }
-__device__ __forceinline__ cplx ldnc_hint(const cplx* p, unsigned long long) { return __ldg(p); }
-__device__ __forceinline__ void st_hint(cplx* p, cplx v, unsigned long long) { *p = v; }
-#endif
 // field (Delta~ / X~ / X) accesses: ld_field where the same kernel later overwrites the location (plain load),
 // ldc_field where the field is read-only for the kernel (non-coherent path)
-__device__ __forceinline__ cplx ld_field(const cplx* p) {
-    if (LGF_L2HINT & 1) return ld_hint(p, l2_policy_last());
-    return *p;
-}
-__device__ __forceinline__ cplx ldc_field(const cplx* p) {
-    if (LGF_L2HINT & 1) return ldnc_hint(p, l2_policy_last());
-    return __ldg(p);
-}
-__device__ __forceinline__ void st_field(cplx* p, cplx v) {
-    if (LGF_L2HINT & 1) st_hint(p, v, l2_policy_last()); else *p = v;
-}
-__device__ __forceinline__ cplx ld_lnk(const cplx* p) {
-    if (LGF_L2HINT & 2) return ldnc_hint(p, l2_policy_first());
-    return __ldg(p);
-}
-__device__ __forceinline__ void st_lnk(cplx* p, cplx v) {
-    if (LGF_L2HINT & 2) st_hint(p, v, l2_policy_first()); else *p = v;
-}
-
-// Asynchronous DRAM -> L2 prefetch of `bytes` contiguous bytes (multiple of 16, 16-byte aligned): no register or
-// shared-memory destination, so the bytes in flight are not bounded by the register file (sm_90+ bulk prefetch).
-__device__ __forceinline__ void prefetch_l2(const void* p, unsigned bytes) {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
-}
+__device__ __forceinline__ cplx ld_field(const cplx* p) { return *p; }
+__device__ __forceinline__ cplx ldc_field(const cplx* p) { return __ldg(p); }
+__device__ __forceinline__ void st_field(cplx* p, cplx v) { *p = v; }
 
 // Line prefetch into L2 (no destination register): used to pull a thread's NEXT site towards the SM while it works on
 // the current one, so that the later loads see L2 latency instead of DRAM latency.
@@ -124,18 +72,21 @@ __device__ __forceinline__ bool prefetch_lane() {
 
 // Load link (x, mu) from the structure-of-arrays store: entry c of direction mu is the V-array at
 // links + (mu*NC + c)*V, NC = 6 (12-real: rows 0,1) or 9 (18-real).  Row 2 is rebuilt for NC = 6.
-template <int NC>
-__device__ __forceinline__ void load_link(const cplx* __restrict__ links, long long V, int mu, long long x, cplx (&u)[9]) {
+// RO = true: the links are read-only for the whole kernel (S1, read-outs): non-coherent loads (ld.global.nc).
+// RO = false: the kernel also writes the links (the in-place update kernels): plain loads, as ld.global.nc is specified
+// for data nobody writes during the kernel's lifetime.
+template <int NC, bool RO = true>
+__device__ __forceinline__ void load_link(const cplx* links, long long V, int mu, long long x, cplx (&u)[9]) {
     const cplx* p = links + (long long)(mu * NC) * V + x;
 #pragma unroll
-    for (int c = 0; c < NC; c++) u[c] = ld_lnk(p + (long long)c * V);
+    for (int c = 0; c < NC; c++) u[c] = RO ? __ldg(p + (long long)c * V) : p[(long long)c * V];
     if (NC == 6) third_row(u);
 }
 template <int NC>
-__device__ __forceinline__ void store_link(cplx* __restrict__ links, long long V, int mu, long long x, const cplx (&u)[9]) {
+__device__ __forceinline__ void store_link(cplx* links, long long V, int mu, long long x, const cplx (&u)[9]) {
     cplx* p = links + (long long)(mu * NC) * V + x;
 #pragma unroll
-    for (int c = 0; c < NC; c++) st_lnk(p + (long long)c * V, u[c]);
+    for (int c = 0; c < NC; c++) p[(long long)c * V] = u[c];
 }
 
 // S3: g = rowGramSchmidt(M), M = 1 + (alpha/2) X, X given by its packed independent components
@@ -226,8 +177,11 @@ struct Ctl {
     int nonfinite;         // theta or F not finite
     int n_meas;            // measurements made (index into the history)
     int hist_cap;
-    unsigned int ticket;   // block counter of the fused reduction
-    int parity;            // which of the two link buffers holds the current links (fused update: flipped per update)
+    // stagnation guard (the fp32 phase of LGF_MIXED): stop when theta has not halved within stall_window measurements
+    int stall_window;      // 0: off
+    int stall_count;       // measurements since theta last fell below half of theta_mark
+    int stalled;           // 1: stopped by the guard
+    double theta_mark;
 };
 
 }  // namespace lgf

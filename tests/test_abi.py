@@ -31,8 +31,8 @@ def test_status_strings_and_kernel_names():
     L = lgf.lib()
     for st in (0, 1, 2, 3, 4, 5, 6, 100):
         assert len(L.lgf_status_string(st)) > 0
-    names = [L.lgf_kernel_name(i).decode() for i in range(16)]
-    assert "k_update_x" in names and "k_fft23_mid" in names
+    names = [L.lgf_kernel_name(i).decode() for i in range(lgf.LGF_MAX_KERNELS)]
+    assert "k_update_quad" in names and "k_fft23_mid" in names and "k_fa_delta_fwd" in names
     assert L.lgf_kernel_name(99) == b""
 
 
@@ -42,14 +42,14 @@ def test_workspace_bytes_and_supported_sizes():
     V = 32 ** 4
     n12 = L.lgf_workspace_bytes(d(32, 32, 32, 32), lgf.LGF_FP64, lgf.LGF_STORE_12)
     n18 = L.lgf_workspace_bytes(d(32, 32, 32, 32), lgf.LGF_FP64, lgf.LGF_STORE_18)
-    # links 384 / 576 B per site, two buffers (the fused update reads one and writes the other)
-    assert n12 >= V * (2 * 384 + 64) and n18 - n12 == 2 * V * 192
+    # links 384 / 576 B per site, one buffer (updated in place), field 64 B, stored g 96 B
+    assert V * (384 + 64) <= n12 <= V * (384 + 64 + 96) + (80 << 20) and n18 - n12 == V * 192
     assert L.lgf_workspace_bytes(d(64, 64, 64, 64), lgf.LGF_FP64, lgf.LGF_STORE_12) >= 64 ** 4 * 448
     assert L.lgf_workspace_bytes(d(32, 32, 32, 64), lgf.LGF_FP64, lgf.LGF_STORE_12) > 0
     assert L.lgf_workspace_bytes(d(8, 8, 8, 8), lgf.LGF_FP64, lgf.LGF_STORE_18) > 0
     # fp32 (LGF_FP32): half the link and field bytes
     n12f = L.lgf_workspace_bytes(d(32, 32, 32, 32), lgf.LGF_FP32, lgf.LGF_STORE_12)
-    assert V * (2 * 192 + 32) <= n12f < n12 - V * 384
+    assert V * (192 + 32) <= n12f < n12 - V * 192
     # unsupported: non power of two, too small, bad precision, bad storage
     assert L.lgf_workspace_bytes(d(12, 8, 8, 8), lgf.LGF_FP64, lgf.LGF_STORE_12) == 0
     assert L.lgf_workspace_bytes(d(2, 8, 8, 8), lgf.LGF_FP64, lgf.LGF_STORE_12) == 0

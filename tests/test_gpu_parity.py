@@ -24,43 +24,19 @@ def theta_close(t_gpu, t_ref):
 
 
 def all_variants(gf):
-    """Every kernel selection the library offers:
-    (fuse Delta into FFT pass A, store g, CUDA graph, compile-time-sized FFT passes, fused update + next Delta
-    [, ping-pong mask of the persistent passes; default 0 [, where S5 runs: 0 k_finalize, 1 pass A, 2 pass B; default 2
-    [, one thread per link in S3/S4; default 1 [, pass B with whole lines in registers; default 1]]]])."""
+    """Every kernel selection the library offers, as (store g, CUDA graph, compile-time-sized FFT passes, PDL)."""
     if gf.V > (1 << 18):
-        return [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 0, 0), (0, 1, 1, 1, 0), (0, 0, 0, 0, 0),
-                (1, 0, 1, 1, 0, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 1, 0), (0, 0, 1, 1, 0, 0, 0, 1, 1, 1)]
-    out = []
-    for fast in (1, 0):
-        for fuse in (1, 0):
-            for store_g in (0, 1):
-                for graph in (1, 0):
-                    out.append((fuse, store_g, graph, fast, 0))
-    out += [(1, 0, 1, 1, 1), (1, 0, 0, 1, 1)]       # the fused update needs the fast passes; the other switches do not enter
-    # the persistent ping-pong passes, all or one at a time; S5 inside pass A
-    out += [(1, 0, 1, 1, 0, 7), (0, 0, 0, 1, 0, 7), (1, 0, 1, 1, 0, 1), (1, 0, 1, 1, 0, 2), (1, 0, 0, 1, 0, 4), (1, 0, 1, 1, 0, 0, 1), (1, 0, 0, 1, 0, 0, 1)]
-    out += [(1, 0, 1, 1, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]      # one thread per site in S3/S4 (and k_finalize)
-    out += [(1, 0, 1, 1, 0, 0, 0), (0, 0, 0, 1, 0, 0, 0), (1, 1, 1, 1, 0, 0, 0)]   # k_finalize as a kernel of its own
-    out += [(1, 0, 1, 1, 0, 0, 0, 1, 0), (0, 1, 0, 1, 0, 0, 0, 1, 0)]   # stage-wise pass B
-    out += [(1, 0, 1, 1, 0, 0, 2, 1, 2), (0, 0, 0, 1, 0, 0, 0, 1, 2)]   # pass B with half a line per thread
-    out += [(0, 0, 1, 1, 0, 0, 0, 1, 1, 1), (0, 0, 0, 0, 0, 0, 0, 0, 1, 1)]   # S1 as its own kernel with one thread per link pair
-    out += [(1, 0, 1, 1, 0, 0, 0, 1, 1, 0, 0)]                               # 64 x 64 planes without the CTA-pair pass A
+        return [(0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0)]
+    out = [(sg, graph, fast, 1) for fast in (1, 0) for sg in (0, 1) for graph in (1, 0)]
+    out += [(0, 1, 1, 0), (1, 0, 0, 0)]
     return out
 
 
 def set_variant(gf, v):
-    gf.set_option(lgf.LGF_OPT_FUSE_DELTA_FFT, v[0])
-    gf.set_option(lgf.LGF_OPT_STORE_G, v[1])
-    gf.set_option(lgf.LGF_OPT_GRAPH, v[2])
-    gf.set_option(lgf.LGF_OPT_FAST_FFT, v[3])
-    gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, v[4])
-    gf.set_option(lgf.LGF_OPT_PINGPONG, v[5] if len(v) > 5 else 0)
-    gf.set_option(lgf.LGF_OPT_FUSE_FINALIZE, v[6] if len(v) > 6 else 2)
-    gf.set_option(lgf.LGF_OPT_QUAD_UPDATE, v[7] if len(v) > 7 else 1)
-    gf.set_option(lgf.LGF_OPT_LINE_FFT, v[8] if len(v) > 8 else 1)
-    gf.set_option(lgf.LGF_OPT_QUAD_DELTA, v[9] if len(v) > 9 else 0)
-    gf.set_option(lgf.LGF_OPT_CLUSTER_PASS_A, v[10] if len(v) > 10 else 1)
+    gf.set_option(lgf.LGF_OPT_STORE_G, v[0])
+    gf.set_option(lgf.LGF_OPT_GRAPH, v[1])
+    gf.set_option(lgf.LGF_OPT_FAST_FFT, v[2])
+    gf.set_option(lgf.LGF_OPT_PDL, v[3] if len(v) > 3 else 1)
 
 
 # ------------------------------------------------------------------ boundary: load -> get
@@ -172,8 +148,7 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
     assert hist_ref[n_ref, 1] < TOL, "oracle did not converge inside the trajectory"
 
     gf = lgf.GaugeFixer(dims, storage)
-    for v in [(1, 0, 1, 1, 1), (1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 7), (1, 0, 1, 1, 0, 0, 1), (1, 0, 1, 1, 0, 0, 0), (0, 1, 0, 0, 0), (1, 0, 1, 1, 0, 0, 0, 0),
-              (1, 0, 1, 1, 0, 0, 0, 1, 0), (1, 0, 1, 1, 0, 0, 2, 1, 2)]:
+    for v in [(0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0)]:
         set_variant(gf, v)
         gf.load_links(U)
         done = 0
@@ -337,9 +312,9 @@ def test_plain_steepest_descent_variant(dims, storage):
     X_ref = o.fa_field()
     r_ref = o.fix(ALPHA, 0.0, 20, history=True)
     gf = lgf.GaugeFixer(dims, storage)
-    for quad in (1, 0):
+    for graph in (1, 0):
         gf.set_option(lgf.LGF_OPT_FOURIER_ACCEL, 0)
-        gf.set_option(lgf.LGF_OPT_QUAD_UPDATE, quad)
+        gf.set_option(lgf.LGF_OPT_GRAPH, graph)
         assert gf.get_option(lgf.LGF_OPT_FOURIER_ACCEL) == 0
         gf.load_links(U)
         assert np.abs(gf.get_field(lgf.LGF_FIELD_X) - X_ref).max() <= 1e-13 * np.abs(X_ref).max()
@@ -366,12 +341,12 @@ def test_plain_steepest_descent_variant(dims, storage):
 
 # ------------------------------------------------------------------ many short runs across the kernel selections
 def test_kernel_selections_agree_over_many_configurations():
-    """Several hundred lgf_fix runs on seeded device-generated configurations: every kernel selection (pass B forms, where S5
-    runs, PDL, graph batching) must stop at the same iteration with the same F, and the mixed-precision run must reach
+    """A few hundred lgf_fix runs on seeded device-generated configurations: every kernel selection (generic or sized passes,
+    stored g, PDL, graph batching) must stop at the same iteration with the same F, and the mixed-precision run must reach
     the same F.  The stop flag is raised and observed in a different kernel or CTA in each selection; this is the test
     that goes through that transition many times (a per-thread read of the flag once hung an experimental build)."""
-    variants = [{}, {"LGF_OPT_LINE_FFT": 0}, {"LGF_OPT_LINE_FFT": 2}, {"LGF_OPT_FUSE_FINALIZE": 0}, {"LGF_OPT_FUSE_FINALIZE": 1},
-                {"LGF_OPT_PDL": 0}, {"LGF_OPT_BATCH": 1}, {"LGF_OPT_BATCH": 3}, {"LGF_OPT_GRAPH": 0}, {"LGF_OPT_QUAD_UPDATE": 0}]
+    variants = [{}, {"LGF_OPT_FAST_FFT": 0}, {"LGF_OPT_STORE_G": 1}, {"LGF_OPT_PDL": 0}, {"LGF_OPT_BATCH": 1}, {"LGF_OPT_BATCH": 3},
+                {"LGF_OPT_GRAPH": 0}]
     for dims, nseeds in [((16, 16, 16, 16), 24), ((32, 32, 16, 16), 8), ((64, 64, 4, 4), 4)]:
         gfs = []
         for opts in variants:
@@ -416,7 +391,7 @@ def test_trajectory_on_thermalised_wilson_configuration(dims, beta, sweeps, seed
     href = np.array(r_ref["history"])
     assert r_ref["status"] == 0 and r_ref["n_iter"] > 30
     gf = lgf.GaugeFixer(dims, 12)
-    for v in [(1, 0, 1, 1, 0), (1, 0, 1, 1, 0, 0, 0, 0, 0), (0, 0, 0, 0, 0, 0, 0, 0)]:
+    for v in [(0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1)]:
         set_variant(gf, v)
         gf.load_links(U)
         r = gf.fix(ALPHA, TOL, 5000)
@@ -450,7 +425,7 @@ def test_coulomb_gauge_against_the_oracle(dims, storage):
     gf = lgf.GaugeFixer(dims, storage)
     gf.set_option(lgf.LGF_OPT_GAUGE_DIRECTIONS, 3)
     assert gf.get_option(lgf.LGF_OPT_GAUGE_DIRECTIONS) == 3
-    for v in [(1, 0, 1, 1, 0), (0, 0, 0, 0, 0, 0, 0, 0), (0, 1, 1, 1, 0), (1, 0, 0, 1, 0, 7), (1, 0, 1, 1, 1)]:
+    for v in [(0, 1, 1, 1), (0, 0, 0, 1), (1, 1, 1, 1), (1, 0, 0, 0)]:
         set_variant(gf, v)
         gf.load_links(U)
         F, th, _ = gf.measure()
@@ -473,7 +448,7 @@ def test_coulomb_gauge_against_the_oracle(dims, storage):
     assert r["status"] == lgf.LGF_OK and r["theta"] < TOL and abs(r["F"] - r_ref["F"]) <= 1e-10
     # back to Landau on the same context
     gf.set_option(lgf.LGF_OPT_GAUGE_DIRECTIONS, 4)
-    set_variant(gf, (1, 0, 1, 1, 0))
+    set_variant(gf, (0, 1, 1, 1))
     gf.load_links(U)
     o.set_gauge(4)
     o.load(U)
@@ -502,7 +477,7 @@ def test_fp32_stage_and_trajectory_against_the_fp64_oracle(dims, storage):
     href = np.array(r["history"])
     U10 = o.get()
     gf = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_FP32)
-    for v in [(1, 0, 1, 1, 0), (0, 0, 0, 0, 0, 0, 0, 0), (1, 1, 1, 1, 0), (1, 0, 1, 1, 0, 7)]:
+    for v in [(0, 1, 1, 1), (0, 0, 0, 1), (1, 1, 1, 1)]:
         set_variant(gf, v)
         gf.load_links(U)
         F, th, _ = gf.measure()
@@ -573,6 +548,30 @@ def test_mixed_precision_fix_is_an_exact_gauge_copy_at_the_same_maximum(name):
     F, th = gf.iterate(3, ALPHA)
     F_ref, th_ref = o.iterate(3, ALPHA)
     assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref) and np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
+
+
+def test_mixed_precision_hands_over_when_the_fp32_phase_stalls():
+    """the fp32 phase must not eat the max_iter budget when it cannot reach its target.  With the switch
+    threshold set to 1e-16 (below the fp32 floor of theta, ~1e-14) the fp32 phase stalls; the stagnation guard (theta
+    has not halved within 256 iterations) ends it and the fp64 phase converges with the remaining budget -- where an
+    unguarded fp32 phase would have used all of max_iter and returned LGF_NOT_CONVERGED."""
+    U, cfg = E.make_config("C1")
+    dims, storage = cfg["dims"], cfg["storage"]
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    o.load(U)
+    r_ref = o.fix(ALPHA, TOL, 1000)
+    gf = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_MIXED)
+    assert gf.get_option(lgf.LGF_OPT_MIXED_SWITCH) == 12
+    gf.set_option(lgf.LGF_OPT_MIXED_SWITCH, 16)
+    gf.load_links(U)
+    r = gf.fix(ALPHA, TOL, 2000)
+    n32 = gf.get_option(lgf.LGF_OPT_MIXED_FP32_ITERS)
+    assert r["status"] == lgf.LGF_OK and r["theta"] < TOL, r
+    assert r_ref["n_iter"] < n32 <= r_ref["n_iter"] + 256 + 64, (n32, r_ref["n_iter"])     # stalled, then stopped by the guard
+    assert r["n_iter"] - n32 <= 12                                                        # a short fp64 polish
+    assert abs(r["F"] - r_ref["F"]) <= F_TOL
+    with pytest.raises(lgf.LgfError):
+        gf.set_option(lgf.LGF_OPT_MIXED_SWITCH, 3)
 
 
 def test_C1_ten_iterations_against_the_naive_dft_oracle():
@@ -715,8 +714,7 @@ def test_launch_count_and_profile():
     gf.load_links(U)
     n0 = gf.launch_count()
     gf.iterate(8, ALPHA)
-    per_body = 5 if gf.get_option(lgf.LGF_OPT_FUSE_DELTA_FFT) else 6
-    assert gf.launch_count() - n0 == 9 * per_body
+    assert gf.launch_count() - n0 == 9 * 5       # generic passes at 8^4: S1+A, S5, B, C, S3+S4
     gf.set_profiling(True)
     gf.iterate(4, ALPHA)
     prof = gf.get_profile()
@@ -727,56 +725,30 @@ def test_launch_count_and_profile():
     assert lgf.stream_peak_gbs(1 << 18, False, 3) > 500.0 and lgf.stream_peak_gbs(1 << 18, True, 3) > 500.0
 
 
-def test_fused_update_buffers_and_counts():
-    """The fused update double-buffers the links: whatever the parity after a call, every later call --
-    read-back, measurement, stage read-out, more iterations on either path, a reload -- sees the current links."""
+def test_option_changes_between_calls_never_replay_a_stale_graph():
+    """The CUDA-graph cache is keyed by the full selection tuple and alpha (a hashed key collided): after any
+    change of option or alpha on one context, the next call must give what a fresh context with those settings gives."""
     dims, storage = (16, 16, 16, 16), 12
     U = E.noisy(dims, 49, 0.35)
-    o = oracle.Oracle(dims, storage, fft_mode=1)
     gf = lgf.GaugeFixer(dims, storage)
-    assert gf.get_option(lgf.LGF_OPT_FUSE_UPDATE) == 0   # measured slower on B200 (DESIGN.md): off by default
-    gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, 1)
-    assert gf.get_option(lgf.LGF_OPT_FUSE_UPDATE) == 1
-    gf.load_links(U)
-    o.load(U)
-    n0 = gf.launch_count()
-    F, th = gf.iterate(3, ALPHA)                          # odd: the current links are in the second buffer
-    head = 1 if gf.get_option(lgf.LGF_OPT_FUSE_FINALIZE) else 2
-    assert gf.launch_count() - n0 == head + 4 * 3         # measurement 0 (pass A [+ k_finalize]) + 3 bodies of 4
-    F_ref, th_ref = o.iterate(3, ALPHA)
-    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
-    U3 = gf.get_links()
-    assert np.abs(U3 - o.get()).max() <= LINK_TOL
-    Fm, thm, _ = gf.measure()
-    assert abs(Fm - F) <= 1e-14 and abs(thm - th) <= 1e-12 * th
-    assert np.abs(gf.get_field(lgf.LGF_FIELD_DELTA) - o.delta()).max() <= 1e-13
-    F0, th0 = gf.iterate(0, ALPHA)
-    assert abs(F0 - F) <= 1e-14
-    gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, 0)             # separate kernels continue from the second buffer, in place
-    F, th = gf.iterate(2, ALPHA)
-    F_ref, th_ref = o.iterate(2, ALPHA)
-    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
-    gf.set_option(lgf.LGF_OPT_FUSE_UPDATE, 1)
-    F, th = gf.iterate(4, ALPHA)
-    F_ref, th_ref = o.iterate(4, ALPHA)
-    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref)
-    assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
-    gf.load_links(U)                                      # a reload starts from buffer 0 again
-    assert np.array_equal(gf.get_links()[:, :, :2], U[:, :, :2])
-    r = gf.fix(ALPHA, TOL, 1000)
-    o.load(U)
-    r_ref = o.fix(ALPHA, TOL, 1000)
-    assert r["status"] == lgf.LGF_OK and r["n_iter"] == r_ref["n_iter"]
-    assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
-    h = gf.get_history()
-    assert len(h) == r["n_iter"] + 1 and h[-1, 1] < TOL and np.all(h[:-1, 1] >= TOL)
-    # profile names of the fused path
-    gf.set_profiling(True)
-    gf.iterate(2, ALPHA)
-    prof = gf.get_profile()
-    gf.set_profiling(False)
-    assert prof["k_fu_update_delta_fwd"]["launches"] == 2 and prof["k_fa_inv_g"]["launches"] == 2
-    assert prof["k_fa_delta_fwd"]["launches"] == 1 and prof["k_finalize"]["launches"] == 3
+    seq = [({}, 0.08), ({"LGF_OPT_STORE_G": 1}, 0.08), ({"LGF_OPT_STORE_G": 0}, 0.05), ({"LGF_OPT_FAST_FFT": 0}, 0.05),
+           ({"LGF_OPT_FAST_FFT": 1, "LGF_OPT_PDL": 0}, 0.08), ({"LGF_OPT_FOURIER_ACCEL": 0}, 0.08),
+           ({"LGF_OPT_FOURIER_ACCEL": 1, "LGF_OPT_GAUGE_DIRECTIONS": 3}, 0.08), ({"LGF_OPT_GAUGE_DIRECTIONS": 4, "LGF_OPT_PDL": 1}, 0.0625)]
+    state = {}
+    for opts, alpha in seq:
+        state.update(opts)
+        for k, v in opts.items():
+            gf.set_option(getattr(lgf, k), v)
+        fresh = lgf.GaugeFixer(dims, storage)
+        for k, v in state.items():
+            fresh.set_option(getattr(lgf, k), v)
+        gf.load_links(U)
+        fresh.load_links(U)
+        a = gf.iterate(16, alpha)
+        b = fresh.iterate(16, alpha)
+        assert a == b, (state, alpha, a, b)
+        assert np.array_equal(gf.get_links(), fresh.get_links()), (state, alpha)
+        fresh.destroy()
 
 
 def test_fast_fft_pass_selection_64_extents():
@@ -784,7 +756,6 @@ def test_fast_fft_pass_selection_64_extents():
     for dims, mask in [((64, 64, 4, 4), 5), ((4, 4, 64, 64), 2), ((32, 64, 32, 64), 7), ((8, 8, 64, 32), 2), ((64, 32, 16, 16), 7)]:
         gf = lgf.GaugeFixer(dims, 12)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
-        assert gf.get_option(lgf.LGF_OPT_CLUSTER_PASS_A) == (1 if dims[:2] == (64, 64) else 0), dims
         gf.destroy()
 
 
@@ -794,11 +765,5 @@ def test_fast_fft_pass_selection():
                        ((16, 32, 4, 8), 5), ((4, 8, 16, 32), 0), ((8, 8, 8, 8), 0)]:
         gf = lgf.GaugeFixer(dims, 12)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
-        assert gf.get_option(lgf.LGF_OPT_PINGPONG) == 0, dims
-        gf.set_option(lgf.LGF_OPT_PINGPONG, 7)
-        assert gf.get_option(lgf.LGF_OPT_PINGPONG) == mask, dims      # every fast pass has a persistent form
-        gf.set_option(lgf.LGF_OPT_PINGPONG, 2)
-        assert gf.get_option(lgf.LGF_OPT_PINGPONG) == (mask & 2), dims
         gf.set_option(lgf.LGF_OPT_FAST_FFT, 0)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == 0
-        assert gf.get_option(lgf.LGF_OPT_PINGPONG) == 0

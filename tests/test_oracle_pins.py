@@ -530,3 +530,53 @@ def test_coulomb_trajectory_invariants():
     assert np.all(np.diff(h[:, 0]) >= -1e-14)
     assert abs(o.plaquette() - p0) <= 1e-12
     assert max(o.unitarity()) <= 1e-13
+
+
+# ------------------------------------------------------------------ utility read-outs (plaquette, unitarity)
+def test_plaquette_equals_an_independent_numpy_evaluation_and_the_heatbath_measurement():
+    """orc_plaquette (the invariant of pin P11 and the number DESIGN.md section 4 reports per ensemble) on non-trivial
+    links: (1/18V) sum_x sum_{mu<nu} Re Tr[U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag] written out with explicit
+    np.roll shifts on a 4-D array, and the same number from ensembles.heatbath.average_plaquette (torch, written for the
+    Wilson action, shares no code with the oracle).  An anisotropic lattice catches swapped directions or shifts."""
+    import torch
+    from ensembles import heatbath as H
+    for dims, eps in [((4, 4, 4, 4), 0.35), ((4, 6, 2, 8), 0.6)]:
+        U = E.noisy(dims, 71, eps)
+        L0, L1, L2, L3 = dims
+        U4 = U.reshape(L3, L2, L1, L0, 4, 3, 3)
+        s = 0.0
+        for mu in range(4):
+            for nu in range(mu + 1, 4):
+                Um, Un = U4[..., mu, :, :], U4[..., nu, :, :]
+                Un_xmu = np.roll(Un, -1, axis=3 - mu)         # U_nu(x + mu)
+                Um_xnu = np.roll(Um, -1, axis=3 - nu)         # U_mu(x + nu)
+                P = Um @ Un_xmu @ dag(Um_xnu) @ dag(Un)
+                s += np.trace(P, axis1=-2, axis2=-1).real.sum()
+        want = s / (18.0 * U.shape[0])
+        o = oracle.Oracle(dims, 18)
+        o.load(U)
+        got = o.plaquette()
+        assert abs(got - want) < 1e-14, (dims, got, want)
+        assert 0.1 < got < 0.95                                # non-trivial links: neither 1 nor 0
+        assert abs(H.average_plaquette(torch.from_numpy(U), dims) - got) < 1e-13
+        # a single perturbed link changes exactly the 6 plaquettes through it
+        U2 = U.copy()
+        U2[5, 2] = U2[5, 2] @ E.expi_hermitian(E.gaussian_su3_algebra(np.random.default_rng(3), 1), 0.4)[0]
+        o.load(U2)
+        assert abs(o.plaquette() - got) > 1e-6
+
+
+def test_unitarity_readout_equals_numpy():
+    """orc_unitarity = (max |U U^dag - 1|, max |det U - 1|) over all links, against numpy on links that are off the
+    group by a known amount."""
+    dims = (4, 4, 4, 4)
+    U = E.noisy(dims, 72, 0.3)
+    rng = np.random.default_rng(5)
+    U = U + 1e-3 * (rng.standard_normal(U.shape) + 1j * rng.standard_normal(U.shape))
+    o = oracle.Oracle(dims, 18)
+    o.load(U)
+    uu, dd = o.unitarity()
+    want_uu = np.abs(U @ dag(U) - np.eye(3)).max()
+    want_dd = np.abs(np.linalg.det(U) - 1.0).max()
+    assert abs(uu - want_uu) < 1e-15 and abs(dd - want_dd) < 1e-14
+    assert 1e-4 < uu < 1e-1 and 1e-4 < dd < 1e-1
