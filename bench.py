@@ -10,7 +10,8 @@ BASELINE.json configs[2]); value = N * K * inner / (max over ranks of the CUDA-e
 N > 1: one independent configuration per GPU (replicas, weak scaling), no collective on the
 data path.  The JSON line also carries: e2e (host buffers through the C ABI), roofline (dominant kernel, live
 CUDA-event timing), kernels (every kernel), iteration (whole-iteration HBM fraction), time_to_theta (lgf_fix),
-cpu_baseline (the oracle timed on the host cores), clocks, gpu_launches.
+cpu_baseline (the oracle timed on the host cores), clocks, gpu_launches, and other_configs (C3: iterate(500), C4: iterate(200) and
+lgf_fix, each on its own BASELINE.json ensemble with its own kernel table, HBM fraction and clocks).
 
 --impl reference times the CPU oracle (oracle/, radix-2 FFT mode) on the host cores on the same workload.
 """
@@ -61,8 +62,7 @@ def kernel_bytes_per_site(nc: int, cb: int = 16) -> dict:
         "k_fr_mid": 2 * fld,                 # pass B with whole lines in registers: same traffic
         "k_fa_inv": 2 * fld,
         "k_fa_inv_g": fld + g,               # read X~ field, write rows 0,1 of g
-        # fused S3/S4 + next S1 + next pass A (fused_update.cuh): g, links read once + written once, field written
-        "k_fu_update_delta_fwd": g + 2 * lk + fld,
+        "k_tb_mid": 2 * fld,                 # pass B on TMA-staged tiles: same traffic
     }
 
 
@@ -74,18 +74,23 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic(kernel: str):
-    """DRAM bytes (read + write) per launch of `kernel` from the committed ncu --set full capture
-    (profiles/r01_ncu_traffic.csv; the command that made it is in profiles/r01_README.md), or None."""
+TRAFFIC_CSV = "profiles/r02_ncu_traffic.csv"
+
+
+def ncu_traffic(kernel: str, workload: str):
+    """(DRAM bytes read + written per launch of `kernel` on `workload`, the commit the capture was taken at) from the
+    committed ncu --set full capture (TRAFFIC_CSV; the command that made it is in the .md beside it), or (None, None).
+    The number is NOT measured in this run (a bench value is never taken under a profiler): it is stamped with the
+    commit of its capture so that a reader can tell whether the kernel has changed since."""
     import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "r01_ncu_traffic.csv")) as f:
+        with open(os.path.join(ROOT, TRAFFIC_CSV)) as f:
             for r in csv.DictReader(f):
-                if r["kernel"] == kernel:
-                    return int(r["dram_read_bytes"]) + int(r["dram_write_bytes"])
+                if r["kernel"] == kernel and r.get("workload", "C2b") == workload:
+                    return int(r["dram_read_bytes"]) + int(r["dram_write_bytes"]), r.get("commit")
     except Exception:
         pass
-    return None
+    return None, None
 
 
 class ClockSampler:
@@ -167,6 +172,26 @@ def dims_name(dims):
     return "x".join(str(d) for d in dims)
 
 
+# ---------------------------------------------------------------------------------------------- shared by both arms
+def workload_config(name: str, cfg: dict, links: str, inner: int, world: int, beta=None, sweeps=None) -> dict:
+    """The `config` object of the JSON line; both arms print the same one for the same workload."""
+    dims, storage = cfg["dims"], cfg["storage"]
+    V = int(np.prod(dims))
+    nc = 6 if storage == 12 else 9
+    if links == "wilson":
+        src = f"Wilson-action heat bath beta={beta}, {sweeps} sweeps (ensembles.wilson)"
+    elif links == "device":
+        src = "device-generated links (ensembles.device_su3)"
+    elif links == "noisy_device":
+        src = f"eps={cfg.get('eps')} (ensembles.noisy_device: the configs[1] recipe on torch's generator, reading A12b)"
+    else:
+        src = f"eps={cfg.get('eps')}"
+    return {"workload": f"{name}: SU(3) {dims_name(dims)} {storage}-real, {src}, seed={cfg['seed']}, alpha=0.08",
+            "iterations_per_step": inner,
+            "l2": "inputs larger than L2 (links %.0f MB + field %.0f MB per GPU)" % (V * nc * 64 / 1e6, V * 64 / 1e6),
+            "parallelism": "replicas" if world > 1 else "single"}
+
+
 # ---------------------------------------------------------------------------------------------- reference arm
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
@@ -187,12 +212,14 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     val = args.steps * per_step / dt
     cores = oracle.num_threads()
-    sample = f"{per_step} iteration(s) per step of {args.workload} ({dims_name(dims)}, {storage}-real), oracle radix-2 FFT mode"
+    sample = (f"{per_step} iteration(s) per timed step (a bounded sample of the workload's {args.inner}) of {args.workload} "
+              f"({dims_name(dims)}, {storage}-real), oracle radix-2 FFT mode")
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, alpha=0.08", "iterations_per_step": per_step},
+        "config": workload_config(args.workload, cfg, "host", args.inner, 1),
+        "sample_iterations_per_step": per_step,
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -202,6 +229,91 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------------- our arm
+# kernels of the closing (inner+1)-th body of lgf_iterate(inner): launched inner+1 times, the last one returns at once
+# on the stop flag, so their per-iteration time is the accumulated time over `inner`
+TAIL_KERNELS = {"k_fa_inv", "k_fa_inv1", "k_fft01_inv", "k_fa_inv_g", "k_fft01_inv_g", "k_update_quad", "k_update_g"}
+
+
+def profile_kernels(gf, reload, V: int, kb: dict, inner: int, peak: float):
+    """Per-kernel device times: CUDA events around every launch on the library's stream (plain launches)."""
+    reload()
+    gf.iterate(10, ALPHA)
+    gf.set_profiling(True)
+    gf.iterate(inner, ALPHA)
+    prof = gf.get_profile()
+    gf.set_profiling(False)
+    kernels = {}
+    tot_ms = sum(v["ms"] for v in prof.values())
+    for name, v in prof.items():
+        n_eff = inner if (name in TAIL_KERNELS and v["launches"] == inner + 1) else v["launches"]
+        us = v["ms"] / n_eff * 1e3
+        b = kb.get(name, 0) * V
+        kernels[name] = {"launches": v["launches"], "avg_us": us, "share": v["ms"] / tot_ms,
+                         "bytes_per_launch": b, "gbs": b / us / 1e3 if us > 0 else None,
+                         "frac": (b / us / 1e3) / peak if us > 0 else None}
+    dom = max((k for k in kernels if kb.get(k, 0) > 0), key=lambda k: prof[k]["ms"])
+    iter_bytes = sum(kb[k] * V for k in kernels if k in kb)      # each of them runs once per iteration
+    return kernels, dom, iter_bytes
+
+
+def iteration_block(iter_bytes: int, V: int, it_s: float, peak: float) -> dict:
+    return {"bytes_per_site": iter_bytes // V, "bytes": iter_bytes, "gbs": iter_bytes * it_s / 1e9,
+            "frac_of_measured": iter_bytes * it_s / 1e9 / peak, "frac_of_spec_8000": iter_bytes * it_s / 1e9 / 8000.0}
+
+
+def timed_fix(gf, reload, tol: float) -> dict:
+    """lgf_fix from freshly loaded links, wall clock with all syncs (time to theta < tol)."""
+    import torch
+    reload()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    r = gf.fix(ALPHA, tol, 100000)
+    torch.cuda.synchronize()
+    return {"ms": (time.perf_counter() - t0) * 1e3, "n_iter": r["n_iter"], "status": r["status"], "F": r["F"],
+            "theta": r["theta"], "theta_tol": tol}
+
+
+def other_config(lgf, E, name: str, n_iter: int, peak: float, local: int) -> dict:
+    """One of the other BASELINE.json configs (C3: iterate(500); C4: iterate(200)), links resident, on the config's own
+    ensemble generated on the device (ensembles.noisy_device, reading A12b): throughput of `n_iter` iterations in one
+    lgf_iterate call, per-kernel table, whole-iteration HBM fraction, time to theta < 1e-15, clocks."""
+    import torch
+    cfg = dict(E.CONFIGS[name])
+    dims, storage = cfg["dims"], cfg["storage"]
+    V = int(np.prod(dims))
+    nc = 6 if storage == 12 else 9
+    d_in = E.noisy_device(dims, cfg["seed"], cfg["eps"], cfg.get("stream", 0))
+    gf = lgf.GaugeFixer(dims, storage)
+
+    def reload():
+        gf.load_links_device(d_in.data_ptr())
+
+    reload()
+    _, _, plaq = gf.measure()
+    gf.iterate(20, ALPHA)                                       # warm-up: graph capture, clocks
+    reps = 3
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(gf.stream)
+    for _ in range(reps):
+        gf.iterate(n_iter, ALPHA)
+    e1.record(gf.stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / reps
+    it_s = n_iter / (ms * 1e-3)
+    kernels, dom, iter_bytes = profile_kernels(gf, reload, V, kernel_bytes_per_site(nc, 16), min(n_iter, 50), peak)
+    ttt = timed_fix(gf, reload, THETA_TOL)
+    ttt["plaquette"] = plaq
+    gf.destroy()
+    del d_in
+    torch.cuda.empty_cache()
+    return {"config": workload_config(name, cfg, "noisy_device", n_iter, 1), "value": it_s, "unit": UNIT,
+            "ms_per_step": ms, "steps": reps, "iteration": iteration_block(iter_bytes, V, it_s, peak),
+            "dominant_kernel": dom, "kernels": kernels, "time_to_theta": ttt, "clocks": clocks}
+
+
 def run_ours(args):
     import torch
     import paper_1301_3460_b200 as lgf
@@ -226,10 +338,10 @@ def run_ours(args):
         return max_over_ranks(x, dist, "cuda")
 
     import ensembles as E
-    device_links = args.links in ("device", "wilson")
+    device_links = args.links in ("device", "wilson", "noisy_device")
     if device_links:
-        # seeded links generated on the device (ensembles.device_su3): for the large shapes (C3, C4), whose host recipe
-        # takes minutes; throughput does not depend on the configuration.  No end-to-end leg, no CPU baseline.
+        # seeded links generated on the device: for the large shapes (C3, C4), whose host recipe takes minutes;
+        # throughput does not depend on the configuration.  No end-to-end leg, no CPU baseline.
         cfg = dict(E.CONFIGS[args.workload])
         U = None
     else:
@@ -243,6 +355,8 @@ def run_ours(args):
     if device_links:
         if args.links == "wilson":
             d_in = E.wilson(dims, args.beta, args.sweeps, cfg["seed"] + 100 * rank, device="cuda")
+        elif args.links == "noisy_device":
+            d_in = E.noisy_device(dims, cfg["seed"], cfg["eps"], rank_stream(cfg, rank))
         else:
             d_in = E.device_su3(dims, cfg["seed"] + 100 * rank, 0.15)
         h_in = h_out = None
@@ -275,7 +389,6 @@ def run_ours(args):
 
     # ---- device-resident throughput (links already in HBM)
     sampler = ClockSampler(local) if rank == 0 else None
-    n0 = gf.launch_count()
     res = {}
 
     def step():
@@ -306,38 +419,17 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = measured_peak()
         kb = kernel_bytes_per_site(nc, 8 if fp32 else 16)
-        # ---- per-kernel device times: CUDA events around every launch on the library's stream (plain launches)
-        reload()
-        gf.iterate(10, ALPHA)
-        gf.set_profiling(True)
-        gf.iterate(inner, ALPHA)
-        prof = gf.get_profile()
-        gf.set_profiling(False)
-        kernels = {}
-        tot_ms = sum(v["ms"] for v in prof.values())
-        for name, v in prof.items():
-            us = v["ms"] / v["launches"] * 1e3
-            b = kb.get(name, 0) * V
-            kernels[name] = {"launches": v["launches"], "avg_us": us, "share": v["ms"] / tot_ms,
-                             "bytes_per_launch": b, "gbs": b / us / 1e3 if us > 0 else None,
-                             "frac": (b / us / 1e3) / peak if us > 0 else None}
-        dom = max((k for k in kernels if kb.get(k, 0) > 0), key=lambda k: prof[k]["ms"])
+        kernels, dom, iter_bytes = profile_kernels(gf, reload, V, kb, inner, peak)
         try:
             copy_gbs = lgf.copy_peak_gbs(1 << 30, 10)
             stream_gbs = {"read": lgf.stream_peak_gbs(V, False, 10), "read_write_in_place": lgf.stream_peak_gbs(V, True, 10)}
         except Exception:
             copy_gbs, stream_gbs = None, None
-        # bytes of one iteration = the kernels that actually ran (each launched once per iteration)
-        iter_bytes = sum(kb[k] * V for k in kernels if k in kb)
         it_s_1 = value / world
         # ---- time to theta < 1e-15 (lgf_fix, links resident, all syncs included)
-        reload()
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        r = gf.fix(ALPHA, 1e-10 if fp32 else THETA_TOL, 100000)      # fp32 bottoms out near theta = 1e-14
-        torch.cuda.synchronize()
-        ttt = {"ms": (time.perf_counter() - t0) * 1e3, "n_iter": r["n_iter"], "status": r["status"], "F": r["F"],
-               "theta": r["theta"], "theta_tol": 1e-10 if fp32 else THETA_TOL, "plaquette": plaq, "ensemble": args.workload}
+        tol = 1e-10 if fp32 else THETA_TOL                           # fp32 bottoms out near theta = 1e-14
+        ttt = timed_fix(gf, reload, tol)
+        ttt.update({"plaquette": plaq, "ensemble": args.workload})
         # ---- the same with LGF_MIXED (fp32 phase + fp64 polish), fp64 workloads only
         if not fp32:
             try:
@@ -370,27 +462,39 @@ def run_ours(args):
             dt = time.perf_counter() - t0
             cpu = {"value": n_cpu / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                    "sample": f"{n_cpu} iterations of {args.workload} ({dims_name(dims)}, {storage}-real), oracle radix-2 FFT mode, after 1 warm-up"}
+            del o
+        # ---- the other BASELINE.json configs (C3: iterate(500), C4: iterate(200) + lgf_fix), each on its own ensemble
+        others = None
+        if world == 1 and not fp32 and args.workload == "C2b" and not args.no_other_configs:
+            gf.destroy()
+            del h_in, h_out
+            others = {}
+            for nm, n_it in (("C3", 500), ("C4", 200)):
+                try:
+                    others[nm] = other_config(lgf, E, nm, n_it, peak, local)
+                except Exception as e:                   # reported, never fatal for the headline number
+                    others[nm] = {"error": f"{type(e).__name__}: {e}"}
+        traffic, traffic_commit = ncu_traffic(dom, args.workload) if not fp32 else (None, None)
         line = {
             "metric": METRIC.replace("fp64", "fp32") if fp32 else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if fp32 else "f64", "data": "synthetic",
-            "config": {"workload": f"{args.workload}: SU(3) {dims_name(dims)} {storage}-real, " + ((f"Wilson-action heat bath beta={args.beta}, {args.sweeps} sweeps (ensembles.wilson)" if args.links == "wilson" else "device-generated links (ensembles.device_su3)") if device_links else f"eps={cfg.get('eps')}") + f", seed={cfg['seed']}, alpha=0.08",
-                       "iterations_per_step": inner, "l2": "inputs larger than L2 (links %.0f MB + field %.0f MB per GPU)" % (V * nc * 64 / 1e6, V * 64 / 1e6),
-                       "parallelism": "replicas" if world > 1 else "single"},
+            "config": workload_config(args.workload, cfg, args.links, inner, world, args.beta, args.sweeps),
             "e2e": None if device_links else {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": V * 576, "d2h_bytes_per_step": V * 576 + 16,
                                               "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                         "frac": kernels[dom]["frac"], "traffic": ncu_traffic(dom) if (args.workload.startswith("C2") and not fp32) else None,
-                         "traffic_source": "profiles/r01_ncu_traffic.csv (ncu --set full, one launch, cold caches)", "peak_source": peak_src,
+                         "frac": kernels[dom]["frac"], "traffic": traffic,
+                         "traffic_source": f"{TRAFFIC_CSV} (ncu --set full, one launch, cold caches; NOT measured in this run: captured at commit {traffic_commit})",
+                         "peak_source": peak_src,
                          "bytes_per_launch": kernels[dom]["bytes_per_launch"], "avg_us": kernels[dom]["avg_us"],
                          "copy_kernel_gbs": copy_gbs, "stream_yardstick_gbs": stream_gbs},
-            "iteration": {"bytes_per_site": iter_bytes // V, "bytes": iter_bytes, "gbs": iter_bytes * it_s_1 / 1e9,
-                          "frac_of_measured": iter_bytes * it_s_1 / 1e9 / peak, "frac_of_spec_8000": iter_bytes * it_s_1 / 1e9 / 8000.0},
+            "iteration": iteration_block(iter_bytes, V, it_s_1, peak),
             "kernels": kernels,
             "time_to_theta": ttt,
             "cpu_baseline": cpu,
+            "other_configs": others,
             "final": {"F": res["F"], "theta": res["theta"]},
         }
         print(json.dumps(line), flush=True)
@@ -409,12 +513,13 @@ def main():
     ap.add_argument("--workload", default="C2b", help="ensemble name from ensembles.CONFIGS (C2b = 32^4, eps 0.35)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the C3 / C4 blocks of the default C2b run")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
                     help="fp64: the BASELINE.json metric (default); fp32: LGF_FP32 storage and arithmetic (SURVEY.md 8(f) NEXT-1), "
                          "reported with dtype f32 and its own byte model; time_to_theta then stops at theta < 1e-10")
     ap.add_argument("--beta", type=float, default=6.0, help="--links wilson: coupling of the Wilson action")
     ap.add_argument("--sweeps", type=int, default=20, help="--links wilson: heat-bath sweeps from a cold start")
-    ap.add_argument("--links", default="host", choices=["host", "device", "wilson"],
+    ap.add_argument("--links", default="host", choices=["host", "device", "noisy_device", "wilson"],
                     help="host: the seeded BASELINE.json ensemble built with numpy (default); device: seeded links generated on the GPU "
                          "(large shapes C3, C4; no e2e leg, no CPU baseline); wilson: a thermalised Wilson-action configuration generated on the GPU "
                          "(ensembles.wilson: the kind of input the paper fixes), for time_to_theta on realistic links")

@@ -135,12 +135,16 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_PDL              1 (default): programmatic dependent launch between the kernels of an iteration.  0: off.
  *   LGF_OPT_FAST_FFT         1 (default): compile-time-sized FFT passes where the lattice allows (extents 16/32/64).
  *                            0: the generic passes.  get: bit mask of the passes that run fast (1 A, 2 B, 4 C).
+ *   LGF_OPT_TMA              1: pass B (axes 2,3) runs persistent, one CTA per SM, with the next tile staged by the Tensor
+ *                            Memory Accelerator (cp.async.bulk.tensor + mbarrier) while the current one is transformed.
+ *                            0 (default; measured faster): one CTA per tile, plain loads.
+ *                            get: 1 when the TMA pass actually runs for this lattice.
  *   LGF_OPT_MIXED_FP32_ITERS read-only: fp32 iterations of the last LGF_MIXED lgf_fix.
  *   LGF_OPT_MIXED_SWITCH     LGF_MIXED: the fp32 phase aims at theta = 10^-value (default 12, 4..20) and hands over to fp64
  *                            there, or earlier when theta stops falling (it has not halved within 256 iterations). */
 typedef enum { LGF_OPT_STORE_G = 0, LGF_OPT_GRAPH = 1, LGF_OPT_BATCH = 2, LGF_OPT_PDL = 3, LGF_OPT_FAST_FFT = 4,
                LGF_OPT_FOURIER_ACCEL = 5, LGF_OPT_GAUGE_DIRECTIONS = 6, LGF_OPT_MIXED_FP32_ITERS = 7,
-               LGF_OPT_MIXED_SWITCH = 8 } lgf_option;
+               LGF_OPT_MIXED_SWITCH = 8, LGF_OPT_TMA = 9 } lgf_option;
 lgf_status lgf_set_option(lgf_ctx *ctx, lgf_option opt, int value);
 lgf_status lgf_get_option(lgf_ctx *ctx, lgf_option opt, int *value);
 

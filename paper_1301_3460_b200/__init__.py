@@ -20,7 +20,7 @@ __all__ = [
     "LGF_OK", "LGF_NOT_CONVERGED", "LGF_FP64", "LGF_FP32", "LGF_MIXED", "LGF_STORE_12", "LGF_STORE_18",
     "LGF_FIELD_DELTA", "LGF_FIELD_X", "LGF_FIELD_G",
     "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_PDL", "LGF_OPT_FAST_FFT", "LGF_OPT_FOURIER_ACCEL",
-    "LGF_OPT_GAUGE_DIRECTIONS", "LGF_OPT_MIXED_FP32_ITERS", "LGF_OPT_MIXED_SWITCH",
+    "LGF_OPT_GAUGE_DIRECTIONS", "LGF_OPT_MIXED_FP32_ITERS", "LGF_OPT_MIXED_SWITCH", "LGF_OPT_TMA",
     "EXPORTS",
 ]
 
@@ -36,7 +36,7 @@ LGF_FP64, LGF_FP32, LGF_MIXED = 0, 1, 2
 LGF_STORE_18, LGF_STORE_12 = 18, 12
 LGF_FIELD_DELTA, LGF_FIELD_X, LGF_FIELD_G = 0, 1, 2
 LGF_OPT_STORE_G, LGF_OPT_GRAPH, LGF_OPT_BATCH, LGF_OPT_PDL, LGF_OPT_FAST_FFT = 0, 1, 2, 3, 4
-LGF_OPT_FOURIER_ACCEL, LGF_OPT_GAUGE_DIRECTIONS, LGF_OPT_MIXED_FP32_ITERS, LGF_OPT_MIXED_SWITCH = 5, 6, 7, 8
+LGF_OPT_FOURIER_ACCEL, LGF_OPT_GAUGE_DIRECTIONS, LGF_OPT_MIXED_FP32_ITERS, LGF_OPT_MIXED_SWITCH, LGF_OPT_TMA = 5, 6, 7, 8, 9
 LGF_MAX_KERNELS = 32
 
 # every symbol include/lgf.h declares (checked by tests/test_abi.py against the header text)

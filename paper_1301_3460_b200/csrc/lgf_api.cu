@@ -69,6 +69,7 @@ void* lgf32_x_gacc(lgf_ctx* c);
 
 #include "kernels.cuh"
 #include "fft_fast.cuh"
+#include "fft_tma.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -84,13 +85,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G,
-    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_NSLOTS
+    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_TB_MID, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g",
-    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd"};
+    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_tb_mid"};
 
 constexpr int HIST_CAP = 1 << 16;
 // mixed precision: the fp32 phase ends when theta has not halved within this many iterations (a rough thermalised
@@ -194,7 +195,10 @@ struct lgf_ctx {
     int stall_window;       // fp32 build, mixed precision: stagnation guard of the fp32 phase (Ctl::stall_window), 0 = off
     int pending_np;         // S5 inside pass B: partials of the S1 just enqueued that no k_finalize has reduced yet
     // options (include/lgf.h lgf_option)
-    int opt_store_g, opt_graph, opt_batch, opt_fast, opt_pdl, opt_accel;
+    int opt_store_g, opt_graph, opt_batch, opt_fast, opt_pdl, opt_accel, opt_tma;
+    // pass B on TMA-staged tiles (fft_tma.cuh): the field as a 5-D tensor map, whether it could be built
+    CUtensorMap tm_field;
+    bool tma_b;
     int sms;                // SMs of the device
     // compile-time-sized FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
     bool fast_a, fast_b, fast_c, big_p, cl_ok;
@@ -204,7 +208,7 @@ struct lgf_ctx {
     int fft01_ncomp_fused_ok, fft01_ncomp, fft01_threads, fft23_lgC, fft23_S1, fft23_S2, fft23_threads;
     size_t smem01_fused, smem01, smem23;
     // graph cache: the executable graph of opt_batch iteration bodies and the full selection it was captured with
-    struct GraphKey { double half_alpha; int nb, nd, acc_g, store_g, fast, pdl, accel; };
+    struct GraphKey { double half_alpha; int nb, nd, acc_g, store_g, fast, pdl, accel, tma; };
     cudaGraphExec_t graph_exec;
     GraphKey graph_key;
     // profiling
@@ -394,6 +398,42 @@ void launch_fr_mid(lgf_ctx* c) {
 #undef X
 }
 
+// pass B on TMA-staged tiles (fft_tma.cuh): 16/32 extents, one persistent CTA per SM
+void launch_tb_mid(lgf_ctx* c) {
+    LaunchScope ls(c, K_TB_MID);
+    const int n_tiles = 4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC);
+    const unsigned grid = (unsigned)(n_tiles < c->sms ? n_tiles : c->sms);
+    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
+    const FinArgs fa = pending_fin(c);
+#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
+        launch_k(c, k_tb_mid<A, B, fast_mid_lgC(A, B), LGF_TB_NT>, grid, LGF_TB_NT, TmaMidGeom<A, B, fast_mid_lgC(A, B)>::SMEM, c->tm_field, c->field, c->G, c->T, scale, c->ctl, c->partials, fa, n_tiles);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+
+// The field as a 5-D tensor of reals (2 L0, L1, L2, L3, 4 components) with the pass-B tile as its box.  The encoder is
+// a driver entry point fetched at run time, so the library does not link against libcuda.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+bool make_field_tensor_map(lgf_ctx* c, int lgC) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    const Geom& G = c->G;
+    const cuuint64_t esz = sizeof(cplx);
+    const cuuint64_t dims[5] = {(cuuint64_t)2 * G.L[0], (cuuint64_t)G.L[1], (cuuint64_t)G.L[2], (cuuint64_t)G.L[3], 4};
+    const cuuint64_t strides[4] = {esz * G.L[0], esz * G.L[0] * G.L[1], esz * G.L[0] * G.L[1] * G.L[2], esz * (cuuint64_t)G.V};
+    const cuuint32_t box[5] = {(cuuint32_t)(2 << lgC), 1, (cuuint32_t)G.L[2], (cuuint32_t)G.L[3], 1};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(&c->tm_field, sizeof(real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+        5, c->field, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
 lgf_status setup_fast(lgf_ctx* c) {
     const Geom& G = c->G;
     c->fast_a = c->fast_c = fast_pair(G.lg[0], G.lg[1]);
@@ -420,6 +460,15 @@ lgf_status setup_fast(lgf_ctx* c) {
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) CK(set_smem(k_fa_mid<A, B, fast_mid_lgC(A, B), fast_mid_nt(A, B)>, c->smem_fb));
         LGF_BIG_PAIRS(X)
 #undef X
+    }
+    c->tma_b = false;
+    if (c->fast_b && fast_pair(G.lg[2], G.lg[3]) && make_field_tensor_map(c, c->fb_lgC)) {
+        c->tma_b = true;
+#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) \
+            c->tma_b = set_smem(k_tb_mid<A, B, fast_mid_lgC(A, B), LGF_TB_NT>, TmaMidGeom<A, B, fast_mid_lgC(A, B)>::SMEM) == cudaSuccess;
+        LGF_FAST_PAIRS(X)
+#undef X
+        if (!c->tma_b) cudaGetLastError();
     }
     c->cl_ok = false;
     if (c->big_p && G.lg[0] == 6 && G.lg[1] == 6) {
@@ -557,6 +606,8 @@ bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c; }
 bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p; }
 bool use_cluster_a(const lgf_ctx* c) { return use_big_p(c) && c->cl_ok; }
 bool use_line_b(const lgf_ctx* c) { return use_fast_b(c) && fast_pair(c->G.lg[2], c->G.lg[3]); }
+// ... on TMA-staged tiles (Landau gauge: the Coulomb pass B has no axis-3 phase and keeps the plain-load kernel)
+bool use_tma_b(const lgf_ctx* c) { return use_line_b(c) && c->opt_tma && c->tma_b && c->G.nd == 4; }
 // S5 inside pass B's first CTA, where pass B is one of the compile-time-sized kernels
 bool use_fin_b(const lgf_ctx* c) { return c->opt_accel && use_fast_b(c); }
 
@@ -572,7 +623,7 @@ template <int NC> void enqueue_head(lgf_ctx* c) {
     launch_finalize(c, np);
 }
 void launch_mid(lgf_ctx* c) {
-    if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
+    if (use_tma_b(c)) launch_tb_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
 }
 void launch_inv_x(lgf_ctx* c) {
     if (use_fast_c(c)) launch_fa_inv(c); else if (use_big_p(c)) launch_fa_inv1(c);
@@ -635,7 +686,7 @@ lgf_status enqueue_bodies(lgf_ctx* c, int nb, double half_alpha) {
     lgf_ctx::GraphKey key;
     memset(&key, 0, sizeof key);
     key.half_alpha = half_alpha; key.nb = nb; key.nd = c->G.nd; key.acc_g = c->acc_g; key.store_g = use_store_g(c) ? 1 : 0;
-    key.fast = c->opt_fast; key.pdl = c->opt_pdl; key.accel = c->opt_accel;
+    key.fast = c->opt_fast; key.pdl = c->opt_pdl; key.accel = c->opt_accel; key.tma = c->opt_tma;
     if (!c->graph_exec || memcmp(&c->graph_key, &key, sizeof key) != 0) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         cudaGraph_t g = nullptr;
@@ -698,7 +749,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_pdl = 1; c->opt_accel = 1;
+    c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_tma = 0;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0; c->mixed_switch = 12; c->pending_np = 0; c->stall_window = 0;
     c->graph_exec = nullptr; memset(&c->graph_key, 0, sizeof c->graph_key); c->profiling = 0; c->launches = 0; c->capturing = false;
@@ -1029,6 +1080,7 @@ lgf_status lgf_set_option(lgf_ctx* c, lgf_option opt, int value) {
         case LGF_OPT_BATCH: if (value < 1 || value > 1024) return LGF_ERR_INVALID_ARG; c->opt_batch = value; break;
         case LGF_OPT_PDL: c->opt_pdl = value ? 1 : 0; break;
         case LGF_OPT_FAST_FFT: c->opt_fast = value ? 1 : 0; break;
+        case LGF_OPT_TMA: c->opt_tma = value ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: c->opt_accel = value ? 1 : 0; break;
         case LGF_OPT_MIXED_SWITCH: if (value < 4 || value > 20) return LGF_ERR_INVALID_ARG; c->mixed_switch = value; break;
         case LGF_OPT_GAUGE_DIRECTIONS: {
@@ -1051,6 +1103,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_BATCH: *value = c->opt_batch; break;
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_FAST_FFT: *value = ((use_fast_a(c) || use_big_p(c)) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | ((use_fast_c(c) || use_big_p(c)) ? 4 : 0); break;
+        case LGF_OPT_TMA: *value = use_tma_b(c) ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;

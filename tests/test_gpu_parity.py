@@ -26,9 +26,9 @@ def theta_close(t_gpu, t_ref):
 def all_variants(gf):
     """Every kernel selection the library offers, as (store g, CUDA graph, compile-time-sized FFT passes, PDL)."""
     if gf.V > (1 << 18):
-        return [(0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0)]
+        return [(0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0), (0, 1, 1, 1, 1)]
     out = [(sg, graph, fast, 1) for fast in (1, 0) for sg in (0, 1) for graph in (1, 0)]
-    out += [(0, 1, 1, 0), (1, 0, 0, 0)]
+    out += [(0, 1, 1, 0), (1, 0, 0, 0), (0, 1, 1, 1, 1), (0, 0, 1, 0, 1)]      # the last two: pass B on TMA-staged tiles
     return out
 
 
@@ -37,6 +37,7 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_GRAPH, v[1])
     gf.set_option(lgf.LGF_OPT_FAST_FFT, v[2])
     gf.set_option(lgf.LGF_OPT_PDL, v[3] if len(v) > 3 else 1)
+    gf.set_option(lgf.LGF_OPT_TMA, v[4] if len(v) > 4 else 0)
 
 
 # ------------------------------------------------------------------ boundary: load -> get
@@ -140,7 +141,7 @@ def oracle_trajectory(U, dims, storage, checkpoints, fft_mode):
     return np.array(hist), links
 
 
-def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
+def check_trajectory(name, fft_mode, checkpoints=(10, 100), variants=((0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0), (0, 1, 1, 1, 1))):
     U, cfg = E.make_config(name)
     dims, storage = cfg["dims"], cfg["storage"]
     hist_ref, links_ref = oracle_trajectory(U, dims, storage, checkpoints, fft_mode)
@@ -148,7 +149,9 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
     assert hist_ref[n_ref, 1] < TOL, "oracle did not converge inside the trajectory"
 
     gf = lgf.GaugeFixer(dims, storage)
-    for v in [(0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0)]:
+    _, _, plaq = gf_plaquette(gf, U)
+    print(f"{name}: average plaquette {plaq:.6f}, oracle stop iteration {n_ref}, F = {hist_ref[n_ref, 0]:.12f}")
+    for v in variants:
         set_variant(gf, v)
         gf.load_links(U)
         done = 0
@@ -178,6 +181,11 @@ def check_trajectory(name, fft_mode, checkpoints=(10, 100)):
         assert r["theta"] < TOL
         assert np.abs(gf.get_links() - oracle_links_at(U, dims, storage, n_ref, fft_mode)).max() <= LINK_TOL
     return hist_ref, n_ref
+
+
+def gf_plaquette(gf, U):
+    gf.load_links(U)
+    return gf.measure()
 
 
 _cache = {}
@@ -215,9 +223,91 @@ def test_trajectory_C2b_headline_config():
     check_trajectory("C2b", fft_mode=1)
 
 
+@pytest.mark.parametrize("name", ["C2a", "C2c"])
+def test_trajectory_C2a_C2c(name):
+    """BASELINE.json configs[2], eps = 0.25 and 0.45: the other two of the three seeded 32^4 ensembles that stand in
+    for the paper's three beta values; default path and the store-g path."""
+    check_trajectory(name, fft_mode=1, variants=((0, 1, 1, 1), (1, 0, 0, 0)))
+
+
 def test_trajectory_C3_anisotropic():
     """BASELINE.json configs[3], 32^3 x 64: uneven FFT axes, non-cubic p^2 filter, 64-extent pass B."""
     check_trajectory("C3", fft_mode=1, checkpoints=(10, 60))
+
+
+# ------------------------------------------------------------------ C4 as BASELINE.json states it (64^4, eps 0.35, seed 5)
+def _c4_inputs():
+    """configs[4] on its own ensemble: the configs[1] recipe generated on the device (ensembles.noisy_device, reading
+    A12b: the numpy recipe takes minutes at 64^4), copied to the host ONCE; the same array goes to the oracle and to
+    lgf_load_links."""
+    import torch
+    cfg = E.CONFIGS["C4"]
+    Ud = E.noisy_device(cfg["dims"], cfg["seed"], cfg["eps"], cfg.get("stream", 0))
+    U = Ud.cpu().numpy()
+    del Ud
+    torch.cuda.empty_cache()
+    return U, cfg["dims"], cfg["storage"]
+
+
+def test_C4_first_iterations_on_the_full_lattice():
+    """64^4 at full size against the radix-2-FFT-mode oracle (itself pinned to the naive DFT on the CPU): Delta and X of
+    the first iteration element by element on all 16.8 M sites, then F, theta and every link after 1 and 3 iterations."""
+    U, dims, storage = _c4_inputs()
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    o.load(U)
+    gf = lgf.GaugeFixer(dims, storage)
+    gf.load_links(U)
+    F0, th0, plaq = gf.measure()
+    F0_ref, th0_ref = o.measure()
+    print(f"C4: average plaquette {plaq:.6f}, F0 = {F0:.12f}, theta0 = {th0:.6e}")
+    assert abs(F0 - F0_ref) <= F_TOL and abs(th0 - th0_ref) <= 1e-12 * th0_ref
+    D_ref = o.delta()
+    D = gf.get_field(lgf.LGF_FIELD_DELTA)
+    assert np.abs(D - D_ref).max() <= 1e-14 * np.abs(D_ref).max()
+    del D, D_ref
+    X_ref = o.fa_field()
+    X = gf.get_field(lgf.LGF_FIELD_X)
+    assert np.abs(X - X_ref).max() <= 1e-13 * np.abs(X_ref).max()
+    del X, X_ref
+    done = 0
+    for k in (1, 3):
+        F_ref, th_ref = o.iterate(k - done, ALPHA)
+        F, th = gf.iterate(k - done, ALPHA)
+        done = k
+        assert abs(F - F_ref) <= F_TOL, (k, F, F_ref)
+        assert theta_close(th, th_ref), (k, th, th_ref)
+        assert np.abs(gf.get_links() - o.get()).max() <= 1e-13 * k, k
+    gf.destroy()
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(not __import__("os").environ.get("LGF_RUN_SLOW"), reason="about 10 minutes of oracle time at 64^4: set LGF_RUN_SLOW=1 "
+                    "(the log of the last run is profiles/r02_C4_full_run.txt)")
+def test_C4_full_run_to_the_stop_iteration():
+    """configs[4] in full: lgf_fix to theta < 1e-15 against the FFT-mode oracle -- the stop iteration (exact, A19), F
+    within 1e-12, theta per A14 at every iteration, every link within 1e-11 at the stop."""
+    U, dims, storage = _c4_inputs()
+    o = oracle.Oracle(dims, storage, fft_mode=1)
+    o.load(U)
+    r_ref = o.fix(ALPHA, TOL, 1000, history=True)
+    assert r_ref["status"] == 0
+    gf = lgf.GaugeFixer(dims, storage)
+    gf.load_links(U)
+    r = gf.fix(ALPHA, TOL, 1000)
+    h = gf.get_history()
+    h_ref = np.array(r_ref["history"])
+    print(f"C4 full run: n_iter {r['n_iter']} (oracle {r_ref['n_iter']}), F {r['F']:.15f} (oracle {r_ref['F']:.15f}), "
+          f"theta {r['theta']:.3e} (oracle {r_ref['theta']:.3e})")
+    assert r["status"] == lgf.LGF_OK and r["n_iter"] == r_ref["n_iter"]
+    assert abs(r["F"] - r_ref["F"]) <= F_TOL and theta_close(r["theta"], r_ref["theta"])
+    assert len(h) == len(h_ref)
+    assert np.abs(h[:, 0] - h_ref[:, 0]).max() <= F_TOL
+    for k in range(len(h)):
+        assert theta_close(h[k, 1], h_ref[k, 1]), (k, h[k, 1], h_ref[k, 1])
+    dmax = np.abs(gf.get_links() - o.get()).max()
+    print(f"C4 full run: max link difference at the stop {dmax:.3e}")
+    assert dmax <= LINK_TOL
+    gf.destroy()
 
 
 # ------------------------------------------------------------------ full-size lattices on sampled sites
@@ -765,5 +855,10 @@ def test_fast_fft_pass_selection():
                        ((16, 32, 4, 8), 5), ((4, 8, 16, 32), 0), ((8, 8, 8, 8), 0)]:
         gf = lgf.GaugeFixer(dims, 12)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
+        # pass B on TMA-staged tiles (an option) wherever the (x2,x3) extents are 16 or 32 and the x0 extent holds a chunk
+        assert gf.get_option(lgf.LGF_OPT_TMA) == 0
+        gf.set_option(lgf.LGF_OPT_TMA, 1)
+        assert gf.get_option(lgf.LGF_OPT_TMA) == (1 if (mask & 2) else 0), dims
         gf.set_option(lgf.LGF_OPT_FAST_FFT, 0)
+        assert gf.get_option(lgf.LGF_OPT_TMA) == 0
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == 0
