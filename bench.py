@@ -63,6 +63,7 @@ def kernel_bytes_per_site(nc: int, cb: int = 16) -> dict:
         "k_fa_inv": 2 * fld,
         "k_fa_inv_g": fld + g,               # read X~ field, write rows 0,1 of g
         "k_tb_mid": 2 * fld,                 # pass B on TMA-staged tiles: same traffic
+        "k_tm_mid": 2 * fld,                 # ... 64 extents
     }
 
 
@@ -352,6 +353,9 @@ def run_ours(args):
     inner = args.inner
     fp32 = args.precision == "fp32"
     gf = lgf.GaugeFixer(dims, storage, precision=lgf.LGF_FP32 if fp32 else lgf.LGF_FP64)
+    for kv in args.opt:                                   # kernel-selection switches (include/lgf.h lgf_option), e.g. --opt TMA=1
+        k, v = kv.split("=")
+        gf.set_option(getattr(lgf, "LGF_OPT_" + k.upper()), int(v))
     if device_links:
         if args.links == "wilson":
             d_in = E.wilson(dims, args.beta, args.sweeps, cfg["seed"] + 100 * rank, device="cuda")
@@ -479,7 +483,7 @@ def run_ours(args):
             "metric": METRIC.replace("fp64", "fp32") if fp32 else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if fp32 else "f64", "data": "synthetic",
-            "config": workload_config(args.workload, cfg, args.links, inner, world, args.beta, args.sweeps),
+            "config": dict(workload_config(args.workload, cfg, args.links, inner, world, args.beta, args.sweeps), **({"options": args.opt} if args.opt else {})),
             "e2e": None if device_links else {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": V * 576, "d2h_bytes_per_step": V * 576 + 16,
                                               "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
             "gpu_launches": int(launches),
@@ -514,6 +518,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the C3 / C4 blocks of the default C2b run")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="set a library option on the timed context (lgf_option without the LGF_OPT_ prefix), e.g. --opt TMA=1; A/B runs and profiles")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
                     help="fp64: the BASELINE.json metric (default); fp32: LGF_FP32 storage and arithmetic (SURVEY.md 8(f) NEXT-1), "
                          "reported with dtype f32 and its own byte model; time_to_theta then stops at theta < 1e-10")

@@ -92,6 +92,13 @@ lgf_status lgf_load_links(lgf_ctx *ctx, const double *host_links);
 /* Same from DEVICE memory (canonical order). */
 lgf_status lgf_load_links_device(lgf_ctx *ctx, const double *dev_links);
 
+/* The same pair in the two-row host format (the paper's "12 real number representation", carried to the
+ * boundary): host_rows: HOST, double [V][4][2][3][2] = rows 0,1 of every link, V*4*12 doubles; a third of the bytes of the
+ * canonical array stays off the PCIe link.  Only for contexts created with LGF_STORE_12 (else LGF_ERR_UNSUPPORTED); the
+ * caller rebuilds row 2 = conj(row0 x row1) where it needs it. */
+lgf_status lgf_load_links_12(lgf_ctx *ctx, const double *host_rows);
+lgf_status lgf_get_links_12(lgf_ctx *ctx, double *host_rows);
+
 /* Read the gauge-fixed links back (the transformed U of PAPER.md:39), canonical order, always full 18 reals per link (row 2 rebuilt in 12-real storage). */
 lgf_status lgf_get_links(lgf_ctx *ctx, double *host_links);
 lgf_status lgf_get_links_device(lgf_ctx *ctx, double *dev_links);
@@ -135,10 +142,10 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_PDL              1 (default): programmatic dependent launch between the kernels of an iteration.  0: off.
  *   LGF_OPT_FAST_FFT         1 (default): compile-time-sized FFT passes where the lattice allows (extents 16/32/64).
  *                            0: the generic passes.  get: bit mask of the passes that run fast (1 A, 2 B, 4 C).
- *   LGF_OPT_TMA              1: pass B (axes 2,3) runs persistent, one CTA per SM, with the next tile staged by the Tensor
- *                            Memory Accelerator (cp.async.bulk.tensor + mbarrier) while the current one is transformed.
- *                            0 (default; measured faster): one CTA per tile, plain loads.
- *                            get: 1 when the TMA pass actually runs for this lattice.
+ *   LGF_OPT_TMA              1 (default): pass B (axes 2,3) runs persistent, one CTA per SM, its tiles staged by the Tensor
+ *                            Memory Accelerator (cp.async.bulk.tensor + mbarrier): at 16/32 extents the next tiles stream in
+ *                            while the current ones are transformed; at 64 extents the tile goes in and out through the TMA
+ *                            unit.  0: one CTA per tile, plain loads and stores.  get: 1 when a TMA pass actually runs.
  *   LGF_OPT_MIXED_FP32_ITERS read-only: fp32 iterations of the last LGF_MIXED lgf_fix.
  *   LGF_OPT_MIXED_SWITCH     LGF_MIXED: the fp32 phase aims at theta = 10^-value (default 12, 4..20) and hands over to fp64
  *                            there, or earlier when theta stops falling (it has not halved within 256 iterations). */

@@ -42,7 +42,7 @@ LGF_MAX_KERNELS = 32
 # every symbol include/lgf.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [
     "lgf_workspace_bytes", "lgf_create", "lgf_create_ex", "lgf_destroy", "lgf_load_links", "lgf_load_links_device",
-    "lgf_get_links", "lgf_get_links_device", "lgf_iterate", "lgf_fix", "lgf_measure", "lgf_get_history",
+    "lgf_get_links", "lgf_get_links_device", "lgf_load_links_12", "lgf_get_links_12", "lgf_iterate", "lgf_fix", "lgf_measure", "lgf_get_history",
     "lgf_get_field", "lgf_set_option", "lgf_get_option", "lgf_set_profiling", "lgf_get_profile", "lgf_kernel_name",
     "lgf_launch_count", "lgf_copy_peak", "lgf_stream_peak", "lgf_status_string", "lgf_last_error",
 ]
@@ -98,6 +98,8 @@ def lib():
     L.lgf_load_links_device.argtypes = [P, P]
     L.lgf_get_links.argtypes = [P, P]
     L.lgf_get_links_device.argtypes = [P, P]
+    L.lgf_load_links_12.argtypes = [P, P]
+    L.lgf_get_links_12.argtypes = [P, P]
     L.lgf_iterate.argtypes = [P, C.c_int, C.c_double, D, D]
     L.lgf_fix.argtypes = [P, C.c_double, C.c_double, C.c_int, I, D, D]
     L.lgf_measure.argtypes = [P, D, D, D]
@@ -225,6 +227,22 @@ class GaugeFixer:
             raise TypeError("out must be a writeable C-contiguous complex128 [V,4,3,3] or float64 [V,4,3,3,2] array")
         a = _host_f64(out, self.V * 72)
         self._ck(lib().lgf_get_links(self._h, a.ctypes.data), "lgf_get_links")
+        return out
+
+    def load_links_12(self, host_rows):
+        """Two-row host format: complex128 [V,4,2,3] (rows 0,1 of every link); LGF_STORE_12 contexts only."""
+        a = _host_f64(host_rows, self.V * 48)
+        self._ck(lib().lgf_load_links_12(self._h, a.ctypes.data), "lgf_load_links_12")
+
+    def get_links_12(self, out=None) -> np.ndarray:
+        """Returns complex128 [V,4,2,3]: rows 0,1 of every link (two-row host format)."""
+        if out is None:
+            out = np.empty((self.V, 4, 2, 3), dtype=np.complex128)
+        elif not (isinstance(out, np.ndarray) and out.flags.c_contiguous and out.flags.writeable
+                  and out.dtype in (np.complex128, np.float64)):
+            raise TypeError("out must be a writeable C-contiguous complex128 [V,4,2,3] or float64 [V,4,2,3,2] array")
+        a = _host_f64(out, self.V * 48)
+        self._ck(lib().lgf_get_links_12(self._h, a.ctypes.data), "lgf_get_links_12")
         return out
 
     def get_links_device(self, dev_ptr: int):

@@ -61,21 +61,32 @@ template <int LG, bool B> struct Plan2 {
     static constexpr int R1 = 1 << LG1, R2 = 1 << LG2, L = 1 << LG;
 };
 
+// Plan of an axis inside pass B (axes 2,3): as Plan2, except that a 64-point axis is 16 x 4 (axis 2) or 4 x 16 (axis 3)
+// with the radix-16 stage done as 4 x 4 in registers (bfly16: the stored order of the generic plan [4,4,4], lgf_api.cu
+// make_plan), so that the last stage of axis 2 and the first of axis 3 are always one 16-point register block: the tile
+// crosses shared memory 4 times per direction... 8 passes in all at 64 x 64 instead of 12 with 8 x 8.
+template <int LG, bool B> struct PlanM {
+    static_assert(LG >= 4 && LG <= 6, "fast FFT passes cover L = 16, 32, 64");
+    static constexpr int LG1 = (LG == 6) ? (B ? 2 : 4) : Plan2<LG, B>::LG1;
+    static constexpr int LG2 = LG - LG1;
+    static constexpr int R1 = 1 << LG1, R2 = 1 << LG2, L = 1 << LG;
+};
+
 // Forward stage on registers: y = DFT_R(v), then y_k *= tw[k*t]  (t = j * L/N: W_N^{jk} = tw[k t]).
-// Inverse stage: v_k *= conj(tw[k t]), then y = IDFT_R(v).
+// Inverse stage: v_k *= conj(tw[k t]), then y = IDFT_R(v).  Slot s of a radix-16 butterfly holds frequency slot_freq(s).
 template <int R, bool INV, bool TW>
 __device__ __forceinline__ void stage_regs(cplx (&v)[R], const cplx* __restrict__ tw, int t) {
     if constexpr (INV) {
         if constexpr (TW) {
 #pragma unroll
-            for (int k = 1; k < R; k++) v[k] = cmulc(v[k], tw[k * t]);
+            for (int k = 1; k < R; k++) v[k] = cmulc(v[k], tw[slot_freq<R>(k) * t]);
         }
         bfly<R, true>(v);
     } else {
         bfly<R, false>(v);
         if constexpr (TW) {
 #pragma unroll
-            for (int k = 1; k < R; k++) v[k] = cmul(v[k], tw[k * t]);
+            for (int k = 1; k < R; k++) v[k] = cmul(v[k], tw[slot_freq<R>(k) * t]);
         }
     }
 }
@@ -347,7 +358,14 @@ k_cl_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2
     __shared__ double red[64];
     const int r = (int)cluster.block_rank();             // which half of the rows, which pair of components
     cplx* peer = cluster.map_shared_rank(tile, r ^ 1);
-    const int plane = blockIdx.x >> 1;
+    // The planes are walked in x2 bands of 16: x2 fastest inside a band, then x3, then the bands.  The backward neighbours
+    // U_2(x-2) and U_3(x-3) live in the planes (x2-1, x3) and (x2, x3-1); in plain order the latter was read 64 planes =
+    // 100 MB of links earlier and has left L2 (ncu at 64^4: 7.90 GB of DRAM reads against 6.44 GB of links), here 16.
+    int plane = blockIdx.x >> 1;
+    if (G.L[2] >= 32) {
+        const int x2l = plane & 15, x3 = (plane >> 4) & (G.L[3] - 1), bnd = plane >> (4 + G.lg[3]);
+        plane = (bnd * 16 + x2l) + (x3 << G.lg[2]);
+    }
     const long long xbase = (long long)plane << (LG0 + LG1);
     const Grp g{(int)threadIdx.x, 0};
     for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
@@ -366,7 +384,7 @@ k_cl_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2
         else { oth[0] = f[0]; oth[SC] = f[1]; own[0] = f[2]; own[SC] = f[3]; }
     }
     block_sum2(th, fs, red);
-    if (threadIdx.x == 0) partials[blockIdx.x] = make_double2(th, fs);
+    if (threadIdx.x == 0) partials[2 * plane + r] = make_double2(th, fs);
     cluster.sync();                                      // both halves of both tiles are in place (release/acquire)
     plane_forward_store<LG0, LG1, NT, 2>(tile, tw0, tw1, field + (long long)(2 * r) * G.V, G.V, xbase, g);
 }
@@ -534,8 +552,8 @@ __device__ __forceinline__ MidItem mid_item(cplx* __restrict__ field, const Geom
 // group barrier.  tl = tile + i0.
 template <int LG2, int LG3, int LGC, int NT>
 __device__ __forceinline__ void pass_b_load(const cplx* __restrict__ gp, int sh2, int sh3, cplx* __restrict__ tl, const cplx* __restrict__ tw2, const Grp& g) {
-    using PA = Plan2<LG2, false>;
-    using PB = Plan2<LG3, true>;
+    using PA = PlanM<LG2, false>;
+    using PB = PlanM<LG3, true>;
     using MG = MidGeom<LG2, LGC>;
     constexpr int L3 = PB::L, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
     constexpr int NW = C0 * PA::R2 * L3;
@@ -562,8 +580,8 @@ template <int LG2, int LG3, int LGC, int NT>
 __device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01, int sh2, int sh3, double scale, cplx* __restrict__ tl,
                                               const cplx* __restrict__ tw2, const cplx* __restrict__ tw3, const double* __restrict__ s2,
                                               const double* __restrict__ s3, const Grp& g) {
-    using PA = Plan2<LG2, false>;
-    using PB = Plan2<LG3, true>;
+    using PA = PlanM<LG2, false>;
+    using PB = PlanM<LG3, true>;
     using MG = MidGeom<LG2, LGC>;
     constexpr int L2 = PA::L, L3 = PB::L, C0 = MG::C0, S1 = MG::S1, S2 = MG::S2;
     // middle stages, forward and (after the filter) inverse

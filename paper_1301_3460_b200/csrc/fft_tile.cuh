@@ -62,10 +62,55 @@ template <bool INV> __device__ __forceinline__ void bfly8(cplx (&v)[8]) {
     v[3] = cadd(e3, w3); v[7] = csub(e3, w3);
 }
 
+// 16 points as 4 x 4 in place, DIGIT-REVERSED frequency order: forward takes the points x_m (m = c + 4r) in v[m] and leaves
+// F_k = sum_m x_m W16^{km}, k = q + 4p, in v[p + 4q]; the inverse is the exact mirror (frequencies in, points out).
+// This is the order two successive radix-4 stages of the generic passes produce, so a radix-16 stage here and the
+// plan [4,4] there store the same frequency at the same position.
+template <bool INV> __device__ __forceinline__ cplx mul_w16(cplx a, int e) {      // a * W16^e (forward) or a * conj(W16^e); e = q c <= 9
+    const real c1 = (real)0.92387953251128675613, s1 = (real)0.38268343236508977173, h = (real)0.70710678118654752440;
+    // W16^e = (cos, -sin)(2 pi e / 16)
+    real wr, wi;
+    switch (e) {
+        case 0: return a;
+        case 1: wr = c1; wi = -s1; break;
+        case 2: wr = h; wi = -h; break;
+        case 3: wr = s1; wi = -c1; break;
+        case 4: return mul_i<INV>(a);
+        case 6: wr = -h; wi = -h; break;
+        default: wr = -c1; wi = s1; break;      // 9
+    }
+    if (INV) wi = -wi;
+    return mk(a.x * wr - a.y * wi, a.x * wi + a.y * wr);
+}
+template <bool INV> __device__ __forceinline__ void bfly16(cplx (&v)[16]) {
+    if constexpr (!INV) {
+#pragma unroll
+        for (int c = 0; c < 4; c++) bfly4<false>(v[c], v[c + 4], v[c + 8], v[c + 12]);      // over r: t[c][q] in v[c + 4q]
+#pragma unroll
+        for (int q = 1; q < 4; q++)
+#pragma unroll
+            for (int c = 1; c < 4; c++) v[c + 4 * q] = mul_w16<false>(v[c + 4 * q], q * c);
+#pragma unroll
+        for (int q = 0; q < 4; q++) bfly4<false>(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);   // over c: F_{q+4p} in v[p + 4q]
+    } else {
+#pragma unroll
+        for (int q = 0; q < 4; q++) bfly4<true>(v[4 * q], v[4 * q + 1], v[4 * q + 2], v[4 * q + 3]);
+#pragma unroll
+        for (int q = 1; q < 4; q++)
+#pragma unroll
+            for (int c = 1; c < 4; c++) v[c + 4 * q] = mul_w16<true>(v[c + 4 * q], q * c);
+#pragma unroll
+        for (int c = 0; c < 4; c++) bfly4<true>(v[c], v[c + 4], v[c + 8], v[c + 12]);
+    }
+}
+// frequency digit held in slot s of a radix-R butterfly's output (input of the inverse)
+template <int R> __host__ __device__ constexpr int slot_freq(int s) { return (R == 16) ? ((s >> 2) + 4 * (s & 3)) : s; }
+
 template <int R, bool INV> __device__ __forceinline__ void bfly(cplx (&v)[R]) {
     if constexpr (R == 2) bfly2<INV>(v[0], v[1]);
     if constexpr (R == 4) bfly4<INV>(v[0], v[1], v[2], v[3]);
     if constexpr (R == 8) bfly8<INV>(v);
+    if constexpr (R == 16) bfly16<INV>(v);
 }
 
 // One radix-R stage on sub-blocks of length N = 2^lgN for every line of the tile.  The caller syncs.

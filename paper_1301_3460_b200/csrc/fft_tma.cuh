@@ -3,12 +3,12 @@
 // The register-line pass B of fft_fast.cuh (k_fr_mid) is bound by latency, not by DRAM, the FP64 pipe or shared memory
 // (ncu, profiles/r01_ncu_full_summary.txt: DRAM 21 %, FP64 36 %, issue active 26 % at 7 warps per SM): a CTA loads its
 // tile with 32 dependent-latency global loads per thread, transforms it, stores it, and nothing overlaps the three.
-// Here one persistent CTA per SM walks over its tiles and the NEXT tile is always in flight: one elected thread issues
-// a 5-D cp.async.bulk.tensor (box = 2^LGC x0 sites x all of x2 x all of x3 of one component and one x1) into the other
-// of two staging buffers and arms an mbarrier with the byte count; the copy costs neither registers nor issue slots
-// and completes on the barrier while all warps transform the current tile.  Phase 1 reads its axis-2 lines from the
-// (dense) staging buffer and writes the padded work tile; phases 2 and 3 are those of k_fr_mid; phase 3 stores straight
-// from registers (plain stores retire asynchronously).  Same arithmetic, same stored order, same results as k_fr_mid.
+// Here one persistent CTA per SM walks over its tiles and the next tiles are always in flight: one elected thread issues
+// a 5-D cp.async.bulk.tensor (box = 2^LGC x0 sites x all of x2 x all of x3 of one component and one x1) into a free tile
+// buffer and arms an mbarrier with the byte count; the copy costs neither registers nor issue slots and completes on
+// the barrier while the warps transform other tiles.  The three phases are those of k_fr_mid, in place in the buffer
+// the TMA unit filled; phase 3 stores straight from registers (plain stores retire asynchronously).  Same arithmetic,
+// same stored order, same results as k_fr_mid.
 #pragma once
 #include <cuda.h>        // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint, lgf_api.cu)
 #include <cstdint>
@@ -49,94 +49,109 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tm) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(tm) : "memory");
 }
 
-// Geometry of a pass-B tile: staging buffer dense [i3][i2][i0] (what the TMA box writes), work tile padded as MidGeom.
+// Geometry of a pass-B tile in shared memory: dense [i3][i2][i0], exactly what the TMA box writes.
 template <int LG2, int LG3, int LGC> struct TmaMidGeom {
-    using MG = MidGeom<LG2, LGC>;
     static constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = 1 << LGC;
     static constexpr int TILE = C0 * L2 * L3;                       // complex numbers per tile
     static constexpr unsigned TILE_BYTES = TILE * sizeof(cplx);
-    static constexpr int WORK = MG::S2 * L3;
-    // shared memory: two staging buffers, the work tile, the p^2 tables of axes 2,3
-    // (+ slack: the kernel rounds the dynamic shared-memory base up to the 128 bytes a TMA destination needs)
-    static constexpr size_t SMEM = (size_t)(2 * TILE + WORK) * sizeof(cplx) + (size_t)(L2 + L3) * 8 + 128;
+    static constexpr int NBUF = 3;
+    // shared memory: three tile buffers, the p^2 tables of axes 2,3 (+ slack: the kernel rounds the dynamic
+    // shared-memory base up to the 128 bytes a TMA destination needs)
+    static constexpr size_t SMEM = (size_t)(NBUF * TILE) * sizeof(cplx) + (size_t)(L2 + L3) * 8 + 128;
 };
 
 #ifndef LGF_TB_NT
-#define LGF_TB_NT 128
+#define LGF_TB_NT 256
 #endif
 
 // The field as a 5-D tensor of reals for the TMA unit: (2 L0 reals, L1, L2, L3, 4 components); a pass-B tile is the box
 // (2 C0, 1, L2, L3, 1) at (2 C0 chunk, x1, 0, 0, comp).  n_tiles = 4 L1 (L0 / C0); tile index = chunk + nChunks (x1 + L1 comp).
+//
+// One persistent CTA per SM, NT = 256 threads = two groups of 128 (a thread = one whole line in registers needs up to 255
+// of them, so 8 warps is what an SM holds; with ONE group the FP64 dependency stalls are exposed: 60.6 us at 32^4, ncu
+// "wait" 1.7 cycles per issue at 4 warps per SM).  The CTA's tiles form a sequence j = 0, 1, 2, ...; tile j is transformed
+// by group j mod 2, in place, in buffer j mod 3.  When a group has finished tile j (phase 3 has read the buffer), its
+// thread 0 starts the copy of tile j + 3 into the same buffer and arms the buffer's mbarrier; the group that transforms
+// tile j + 3 waits on that barrier.  So each group always finds its next tile already in shared memory, the copies cost
+// neither registers nor issue slots, and the two groups' phases interleave on the FP64 pipe.
+// Bank conflicts: the dense TMA layout makes lanes (i0, i3) and (i0, i3 + 1) of an axis-2 line collide (C0 = 4: 2-way) on
+// the phase-1 reads only; phase 1 writes element m of line (i0, i3) at position m ^ (i3 & 1) -- inside the same line -- which
+// makes its own writes, both accesses of phase 2 and the reads of phase 3 conflict-free.
 template <int LG2, int LG3, int LGC, int NT>
 __global__ void __launch_bounds__(NT, 1) k_tb_mid(const __grid_constant__ CUtensorMap tmap, cplx* __restrict__ field, Geom G, FftTables T,
                                                   double scale, Ctl* ctl, const double2* partials, FinArgs fa, int n_tiles) {
+    static_assert(NT == 256, "two groups of 128 threads");
     pdl_enter();
     __shared__ int s_done;
-    __shared__ __align__(8) uint64_t full[2];
+    __shared__ __align__(8) uint64_t full[3];
     pass_b_entry<NT>(partials, fa, ctl, &s_done);
     using TG = TmaMidGeom<LG2, LG3, LGC>;
-    using MG = MidGeom<LG2, LGC>;
-    constexpr int L2 = TG::L2, L3 = TG::L3, C0 = TG::C0, S1 = MG::S1, S2 = MG::S2, TILE = TG::TILE;
+    constexpr int L2 = TG::L2, L3 = TG::L3, C0 = TG::C0, TILE = TG::TILE, GT = 128;
+    constexpr int SW = (C0 < 8) ? 1 : 0;                 // C0 = 8: 128-byte rows, no conflicts, no swizzle
     extern __shared__ __align__(16) unsigned char smem_raw[];
     // a TMA destination must be 128-byte aligned; the dynamic shared memory starts behind the static variables
-    cplx* stage = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u));      // [2][TILE]
-    cplx* work = stage + 2 * TILE;
-    double* s2 = reinterpret_cast<double*>(work + TG::WORK);
+    cplx* bufs = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u));      // [3][TILE]
+    double* s2 = reinterpret_cast<double*>(bufs + TG::NBUF * TILE);
     double* s3 = s2 + L2;
     for (int i = threadIdx.x; i < L2; i += NT) s2[i] = T.s[2][i];
     for (int i = threadIdx.x; i < L3; i += NT) s3[i] = T.s[3][i];
     const int lgChunks = G.lg[0] - LGC;
-    auto issue = [&](int tile, int buf) {                              // one thread: arm the barrier, start the copy
+    const int n_seq = (n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;      // tiles of this CTA
+    auto issue = [&](int j) {                            // one thread: arm the barrier of buffer j mod 3, start the copy of tile j
+        const int tile = blockIdx.x + j * gridDim.x, b = j % 3;
         const int chunk = tile & ((1 << lgChunks) - 1);
         const int x1 = (tile >> lgChunks) & (G.L[1] - 1);
         const int comp = tile >> (lgChunks + G.lg[1]);
-        mbar_expect_tx(&full[buf], TG::TILE_BYTES);
-        tma_load_5d(stage + buf * TILE, &tmap, &full[buf], chunk << (LGC + 1), x1, 0, 0, comp);
+        mbar_expect_tx(&full[b], TG::TILE_BYTES);
+        tma_load_5d(bufs + b * TILE, &tmap, &full[b], chunk << (LGC + 1), x1, 0, 0, comp);
     };
-    int tile = blockIdx.x;
     if (threadIdx.x == 0) {
-        mbar_init(&full[0], 1); mbar_init(&full[1], 1);
+        mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_init(&full[2], 1);
         mbar_init_fence();
         // a copy in flight must never outlive its CTA: nothing is issued when the run is already over
-        if (!s_done && tile < n_tiles) issue(tile, 0);
+        if (!s_done)
+            for (int j = 0; j < 3 && j < n_seq; j++) issue(j);
     }
     __syncthreads();
     if (s_done) return;                                  // one reading per CTA, behind a barrier (pass_b_entry)
     const int sh2 = G.sh[2], sh3 = G.sh[3];
+    const Grp g{(int)threadIdx.x % GT, 1 + (int)threadIdx.x / GT};      // named barriers 1 and 2
 #pragma unroll 1
-    for (int it = 0; tile < n_tiles; it++, tile += gridDim.x) {
-        const int buf = it & 1;
-        // the other staging buffer was last read in phase 1 of the previous tile, two barriers ago
-        if (threadIdx.x == 0 && tile + (int)gridDim.x < n_tiles) issue(tile + gridDim.x, buf ^ 1);
+    for (int j = threadIdx.x / GT; j < n_seq; j += 2) {
+        const int tile = blockIdx.x + j * gridDim.x, b = j % 3;
         const int chunk = tile & ((1 << lgChunks) - 1);
         const int x1 = (tile >> lgChunks) & (G.L[1] - 1);
         const int comp = tile >> (lgChunks + G.lg[1]);
         cplx* gbase = field + (long long)comp * G.V + (chunk << LGC) + ((long long)x1 << G.sh[1]);
-        const cplx* st = stage + buf * TILE;
-        mbar_wait(&full[buf], (it >> 1) & 1);
-        // phase 1: lines along axis 2, one per (i0, i3), from the staging buffer: forward -> work tile
+        cplx* tl = bufs + b * TILE;
+        mbar_wait(&full[b], (j / 3) & 1);
+        // phase 1: lines along axis 2, one per (i0, i3): forward, in place (element m -> position m ^ (i3 & 1))
 #pragma unroll 1
-        for (int ln = threadIdx.x; ln < C0 * L3; ln += NT) {
+        for (int ln = g.tid; ln < C0 * L3; ln += GT) {
             const int i0 = ln % C0, i3 = ln / C0;
-            const cplx* q = st + i0 + i3 * (C0 * L2);
+            cplx* q = tl + i0 + i3 * (C0 * L2);
             cplx v[L2];
 #pragma unroll
             for (int m = 0; m < L2; m++) v[m] = q[m * C0];
             line_fft<LG2, false, false>(v);
-            cplx* p = work + i0 + i3 * S2;
+            const int par = SW * (i3 & 1) * C0;
+            cplx* qe = q + par;                          // even m: position m + par
+            cplx* qo = q - par;                          // odd m:  position m - par
 #pragma unroll
-            for (int m = 0; m < L2; m++) p[m * S1] = v[m];
+            for (int m = 0; m < L2; m++) ((m & 1) ? qo : qe)[m * C0] = v[m];
         }
-        __syncthreads();
+        gsync<GT>(g);
         // phase 2: lines along axis 3, one per (i0, i2): forward, filter X~ = (p2max / (V p2)) Delta~ at the stored
         // positions (zero mode -> 0), inverse                                                       [north_star step 2]
 #pragma unroll 1
-        for (int ln = threadIdx.x; ln < C0 * L2; ln += NT) {
+        for (int ln = g.tid; ln < C0 * L2; ln += GT) {
             const int i0 = ln % C0, i2 = ln / C0;
-            cplx* p = work + i0 + i2 * S1;
+            // element (i2, i3 = m) sits at position i2 ^ (m & 1) of its axis-2 line
+            cplx* pe = tl + i0 + i2 * C0;
+            cplx* po = tl + i0 + (i2 ^ SW) * C0;
             cplx v[L3];
 #pragma unroll
-            for (int m = 0; m < L3; m++) v[m] = p[m * S2];
+            for (int m = 0; m < L3; m++) v[m] = ((m & 1) ? po : pe)[m * (C0 * L2)];
             line_fft<LG3, true, false>(v);
             const double s012 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1] + s2[i2];
 #pragma unroll
@@ -146,24 +161,222 @@ __global__ void __launch_bounds__(NT, 1) k_tb_mid(const __grid_constant__ CUtens
             }
             line_fft<LG3, true, true>(v);
 #pragma unroll
-            for (int m = 0; m < L3; m++) p[m * S2] = v[m];
+            for (int m = 0; m < L3; m++) ((m & 1) ? po : pe)[m * (C0 * L2)] = v[m];
         }
-        __syncthreads();
+        gsync<GT>(g);
         // phase 3: lines along axis 2 again: inverse, straight to global memory
 #pragma unroll 1
-        for (int ln = threadIdx.x; ln < C0 * L3; ln += NT) {
+        for (int ln = g.tid; ln < C0 * L3; ln += GT) {
             const int i0 = ln % C0, i3 = ln / C0;
-            const cplx* p = work + i0 + i3 * S2;
+            const cplx* q = tl + i0 + i3 * (C0 * L2);
+            const int par = SW * (i3 & 1) * C0;
+            const cplx* qe = q + par;
+            const cplx* qo = q - par;
             cplx v[L2];
 #pragma unroll
-            for (int m = 0; m < L2; m++) v[m] = p[m * S1];
+            for (int m = 0; m < L2; m++) v[m] = ((m & 1) ? qo : qe)[m * C0];
             line_fft<LG2, false, true>(v);
             cplx* gq = gbase + i0 + ((long long)i3 << sh3);
 #pragma unroll
             for (int m = 0; m < L2; m++) st_field(gq + ((long long)m << sh2), v[m]);
         }
-        __syncthreads();                                 // the work tile is rewritten by the next tile's phase 1
+        gsync<GT>(g);                                    // every thread of the group has read the buffer
+        if (g.tid == 0 && j + 3 < n_seq) issue(j + 3);   // same buffer, next tile of the chain
     }
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------
+// Pass B for (x2,x3) tiles with a 64 extent: the tile (2^LGC x0 sites x L2 x L3, 128 KB) fills the SM, so there is one
+// buffer and no second tile in flight -- but the plain-load version of this pass (k_fa_mid) is bound by the L1 queue for
+// global memory instructions (ncu at 64^4: lg_throttle 4.1 cycles per issue; a warp-wide load of 2-site chunks touches 16
+// different 128-byte lines).  Here the tile comes in and goes out through the TMA unit (one 5-D bulk tensor copy each
+// way), which takes the 32/64-byte rows off the LSU, and the stages are those of k_fa_mid with PlanM's radices
+// (16 x 4 | 4 x 16 at 64: the tile crosses shared memory 8 times).  The TMA box is dense, [i3][i2][i0]; between the
+// first and the last stage element (i2, i3) of an (x2,x3) plane sits at position i2 ^ (i3 & SWM), SWM = 8/C0 - 1, inside
+// its own axis-2 line, which makes every stage's accesses conflict-free without padding.
+__device__ __forceinline__ void tma_store_5d(const CUtensorMap* tm, const void* src, int c0, int c1, int c2, int c3, int c4) {
+    asm volatile("cp.async.bulk.tensor.5d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5, %6}], [%1];"
+                 ::"l"(tm), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4) : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+template <int LG2, int LG3, int LGC> struct TmaBigGeom {
+    static constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = 1 << LGC;
+    static constexpr int TILE = C0 * L2 * L3;
+    static constexpr unsigned TILE_BYTES = TILE * sizeof(cplx);
+    static constexpr size_t SMEM = (size_t)(TILE + L2 + L3) * sizeof(cplx) + (size_t)(L2 + L3) * 8 + 128;
+};
+
+template <int LG2, int LG3, int LGC, int NT>
+__global__ void __launch_bounds__(NT, 1) k_tm_mid(const __grid_constant__ CUtensorMap tmap, cplx* __restrict__ field, Geom G, FftTables T,
+                                                  double scale, Ctl* ctl, const double2* partials, FinArgs fa, int n_tiles) {
+    pdl_enter();
+    __shared__ int s_done;
+    __shared__ __align__(8) uint64_t full;
+    pass_b_entry<NT>(partials, fa, ctl, &s_done);
+    using PA = PlanM<LG2, false>;
+    using PB = PlanM<LG3, true>;
+    using TG = TmaBigGeom<LG2, LG3, LGC>;
+    constexpr int L2 = TG::L2, L3 = TG::L3, C0 = TG::C0, TILE = TG::TILE;
+    constexpr int SI2 = C0, SI3 = C0 * L2;               // element strides of i2 and i3 in the dense tile
+    constexpr int SWM = (C0 < 8) ? (8 / C0 - 1) : 0;
+    static_assert(PA::R2 == 4 && PB::R1 == 4, "one 16-point block between the axes");
+    static_assert(NT % C0 == 0, "a thread keeps its x0 offset");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* tile = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u));
+    cplx* tw2 = tile + TILE;
+    cplx* tw3 = tw2 + L2;
+    double* s2 = reinterpret_cast<double*>(tw3 + L3);
+    double* s3 = s2 + L2;
+    for (int i = threadIdx.x; i < L2; i += NT) { tw2[i] = T.tw[2][i]; s2[i] = T.s[2][i]; }
+    for (int i = threadIdx.x; i < L3; i += NT) { tw3[i] = T.tw[3][i]; s3[i] = T.s[3][i]; }
+    const int lgChunks = G.lg[0] - LGC;
+    if (threadIdx.x == 0) { mbar_init(&full, 1); mbar_init_fence(); }
+    __syncthreads();
+    if (s_done) return;                                  // one reading per CTA, behind a barrier (pass_b_entry)
+    const int i0 = threadIdx.x % C0;
+    cplx* tl = tile + i0;
+    int it = 0;
+#pragma unroll 1
+    for (int tileno = blockIdx.x; tileno < n_tiles; tileno += gridDim.x, it++) {
+        const int chunk = tileno & ((1 << lgChunks) - 1);
+        const int x1 = (tileno >> lgChunks) & (G.L[1] - 1);
+        const int comp = tileno >> (lgChunks + G.lg[1]);
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(&full, TG::TILE_BYTES);
+            tma_load_5d(tile, &tmap, &full, chunk << (LGC + 1), x1, 0, 0, comp);
+        }
+        const double s01 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1];
+        mbar_wait(&full, it & 1);
+        // axis-2 stage 1 (points i2 = ja + m R2, twiddles tw2[k ja]): dense in, swizzled out
+        {
+            constexpr int NW = C0 * PA::R2 * L3, NI = (NW + NT - 1) / NT;
+            static_assert(NW % NT == 0, "whole items per thread");
+            cplx v[NI][PA::R1];
+#pragma unroll
+            for (int k = 0; k < NI; k++) {
+                const int w = k * NT + threadIdx.x;
+                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+                const cplx* p = tl + ja * SI2 + i3 * SI3;
+#pragma unroll
+                for (int m = 0; m < PA::R1; m++) v[k][m] = p[m * PA::R2 * SI2];
+                stage_regs<PA::R1, false, true>(v[k], tw2, ja);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < NI; k++) {
+                const int w = k * NT + threadIdx.x;
+                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+                cplx* p = tl + (ja ^ (i3 & SWM)) * SI2 + i3 * SI3;
+#pragma unroll
+                for (int m = 0; m < PA::R1; m++) p[m * PA::R2 * SI2] = v[k][m];
+            }
+            __syncthreads();
+        }
+        // 16-point block: last stage of axis 2 (contiguous sub-blocks of 4) x first stage of axis 3 (points jb + mb R2b)
+        auto block = [&](auto inv_tag) {
+            constexpr bool INV = decltype(inv_tag)::value;
+            constexpr int NW = C0 * PB::R2 * PA::R1;
+#pragma unroll
+            for (int w0 = 0; w0 < NW; w0 += NT) {
+                const int w = w0 + threadIdx.x;
+                if (NW % NT == 0 || w < NW) {
+                    const int jb = (w / C0) % PB::R2, ba = w / (C0 * PB::R2);
+                    const int sw = jb & SWM;
+                    cplx v[4][4];                        // [mb][ma]
+#pragma unroll
+                    for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+                        for (int ma = 0; ma < 4; ma++) v[mb][ma] = tl[((ba * 4 + ma) ^ sw) * SI2 + (jb + mb * PB::R2) * SI3];
+                    if constexpr (!INV) {
+#pragma unroll
+                        for (int mb = 0; mb < 4; mb++) bfly<4, false>(v[mb]);
+                    }
+#pragma unroll
+                    for (int ma = 0; ma < 4; ma++) {
+                        cplx c[4];
+#pragma unroll
+                        for (int mb = 0; mb < 4; mb++) c[mb] = v[mb][ma];
+                        stage_regs<4, INV, true>(c, tw3, jb);
+#pragma unroll
+                        for (int mb = 0; mb < 4; mb++) v[mb][ma] = c[mb];
+                    }
+                    if constexpr (INV) {
+#pragma unroll
+                        for (int mb = 0; mb < 4; mb++) bfly<4, true>(v[mb]);
+                    }
+#pragma unroll
+                    for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+                        for (int ma = 0; ma < 4; ma++) tl[((ba * 4 + ma) ^ sw) * SI2 + (jb + mb * PB::R2) * SI3] = v[mb][ma];
+                }
+            }
+            __syncthreads();
+        };
+        block(std::false_type{});
+        // axis-3 stage 2 forward, S2b filter X~ = (p2max / (V p2)) Delta~ at the stored positions (zero mode -> 0), axis-3
+        // stage 2 inverse, on the same registers                                                   [north_star step 2]
+        {
+            constexpr int NW = C0 * L2 * PB::R1;
+#pragma unroll
+            for (int w0 = 0; w0 < NW; w0 += NT) {
+                const int w = w0 + threadIdx.x;
+                if (NW % NT == 0 || w < NW) {
+                    const int i2 = (w / C0) % L2, bb = w / (C0 * L2);
+                    cplx v[PB::R2];
+#pragma unroll
+                    for (int m = 0; m < PB::R2; m++) v[m] = tl[(i2 ^ (m & SWM)) * SI2 + (bb * PB::R2 + m) * SI3];
+                    bfly<PB::R2, false>(v);
+                    const double s012 = s01 + s2[i2];
+#pragma unroll
+                    for (int m = 0; m < PB::R2; m++) {
+                        const double p2 = s012 + s3[bb * PB::R2 + m];
+                        v[m] = cscale(v[m], (real)((p2 > 0.0) ? scale / p2 : 0.0));
+                    }
+                    bfly<PB::R2, true>(v);
+#pragma unroll
+                    for (int m = 0; m < PB::R2; m++) tl[(i2 ^ (m & SWM)) * SI2 + (bb * PB::R2 + m) * SI3] = v[m];
+                }
+            }
+            __syncthreads();
+        }
+        block(std::true_type{});
+        // axis-2 stage 1 inverse: swizzled in, dense out, then the tile goes back through the TMA unit
+        {
+            constexpr int NW = C0 * PA::R2 * L3, NI = (NW + NT - 1) / NT;
+            cplx v[NI][PA::R1];
+#pragma unroll
+            for (int k = 0; k < NI; k++) {
+                const int w = k * NT + threadIdx.x;
+                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+                const cplx* p = tl + (ja ^ (i3 & SWM)) * SI2 + i3 * SI3;
+#pragma unroll
+                for (int m = 0; m < PA::R1; m++) v[k][m] = p[m * PA::R2 * SI2];
+                stage_regs<PA::R1, true, true>(v[k], tw2, ja);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < NI; k++) {
+                const int w = k * NT + threadIdx.x;
+                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+                cplx* p = tl + ja * SI2 + i3 * SI3;
+#pragma unroll
+                for (int m = 0; m < PA::R1; m++) p[m * PA::R2 * SI2] = v[k][m];
+            }
+        }
+        fence_proxy_async();                             // the generic-proxy writes above, before the async proxy reads them
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            tma_store_5d(&tmap, tile, chunk << (LGC + 1), x1, 0, 0, comp);
+            tma_store_wait_read();                       // the buffer is free again once the store has read it
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) tma_store_wait_all();
 }
 
 }  // namespace lgf

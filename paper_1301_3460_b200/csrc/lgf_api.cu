@@ -19,6 +19,8 @@
 #define lgf_load_links lgf32_load_links
 #define lgf_get_links_device lgf32_get_links_device
 #define lgf_get_links lgf32_get_links
+#define lgf_load_links_12 lgf32_load_links_12
+#define lgf_get_links_12 lgf32_get_links_12
 #define lgf_iterate lgf32_iterate
 #define lgf_fix lgf32_fix
 #define lgf_measure lgf32_measure
@@ -45,6 +47,8 @@ void lgf32_destroy(lgf_ctx* c);
 lgf_status lgf32_load_links(lgf_ctx* c, const double* host_links);
 lgf_status lgf32_load_links_device(lgf_ctx* c, const double* dev_links);
 lgf_status lgf32_get_links(lgf_ctx* c, double* host_links);
+lgf_status lgf32_load_links_12(lgf_ctx* c, const double* host_rows);
+lgf_status lgf32_get_links_12(lgf_ctx* c, double* host_rows);
 lgf_status lgf32_get_links_device(lgf_ctx* c, double* dev_links);
 lgf_status lgf32_iterate(lgf_ctx* c, int n, double alpha, double* F, double* theta);
 lgf_status lgf32_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int* n_iter, double* F, double* theta);
@@ -73,6 +77,7 @@ void* lgf32_x_gacc(lgf_ctx* c);
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -85,13 +90,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G,
-    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_TB_MID, K_NSLOTS
+    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_TB_MID, K_TM_MID, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g",
-    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_tb_mid"};
+    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_tb_mid", "k_tm_mid"};
 
 constexpr int HIST_CAP = 1 << 16;
 // mixed precision: the fp32 phase ends when theta has not halved within this many iterations (a rough thermalised
@@ -141,10 +146,12 @@ Layout make_layout(const int dims[4], int NC) {
     return o;
 }
 
-// Stage radices of an axis of length 2^lgL; b_axis: axes 1 and 3 (see fft_tile.cuh).
-AxisPlan make_plan(int lgL, bool b_axis) {
+// Stage radices of an axis of length 2^lgL; b_axis: axes 1 and 3 (see fft_tile.cuh); mid: axes 2,3 (pass B), whose
+// 64-point plan is [4,4,4] -- the stored order of the 16 x 4 / 4 x 16 stages of the compile-time-sized pass B (PlanM).
+AxisPlan make_plan(int lgL, bool b_axis, bool mid) {
     AxisPlan p; p.nst = 0; p.lgr[0] = p.lgr[1] = p.lgr[2] = 0;
     if (lgL == 5 && b_axis) { p.nst = 2; p.lgr[0] = 2; p.lgr[1] = 3; return p; }
+    if (lgL == 6 && mid) { p.nst = 3; p.lgr[0] = p.lgr[1] = p.lgr[2] = 2; return p; }
     int lgN = lgL;
     while (lgN > 0) {
         const int lgR = (lgN == 1) ? 1 : ((lgN == 2 || lgN == 4) ? 2 : 3);
@@ -179,6 +186,8 @@ struct lgf_ctx {
     char* ws;               // workspace base (device)
     bool own_ws, own_stream;
     cudaStream_t stream;
+    cudaStream_t copy_stream;           // boundary copies (overlap with the layout kernels on `stream`)
+    cudaEvent_t ev_copy[2], ev_kern[2]; // per staging half: copy done / layout kernel done
     cplx *links, *field, *gbuf;
     dcplx* staging;         // host-facing double complex (AoS chunks of the boundary copies)
     double2 *partials, *hist;
@@ -411,6 +420,20 @@ void launch_tb_mid(lgf_ctx* c) {
 #undef X
 }
 
+// pass B on TMA-staged tiles, 64 extents: the tile goes in and out through the TMA unit (fft_tma.cuh k_tm_mid)
+constexpr int TM_NT = 512;
+void launch_tm_mid(lgf_ctx* c) {
+    LaunchScope ls(c, K_TM_MID);
+    const int n_tiles = 4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC);
+    const unsigned grid = (unsigned)(n_tiles < c->sms ? n_tiles : c->sms);
+    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
+    const FinArgs fa = pending_fin(c);
+#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
+        launch_k(c, k_tm_mid<A, B, fast_mid_lgC(A, B), TM_NT>, grid, TM_NT, TmaBigGeom<A, B, fast_mid_lgC(A, B)>::SMEM, c->tm_field, c->field, c->G, c->T, scale, c->ctl, c->partials, fa, n_tiles);
+    LGF_BIG_PAIRS(X)
+#undef X
+}
+
 // The field as a 5-D tensor of reals (2 L0, L1, L2, L3, 4 components) with the pass-B tile as its box.  The encoder is
 // a driver entry point fetched at run time, so the library does not link against libcuda.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
@@ -462,11 +485,15 @@ lgf_status setup_fast(lgf_ctx* c) {
 #undef X
     }
     c->tma_b = false;
-    if (c->fast_b && fast_pair(G.lg[2], G.lg[3]) && make_field_tensor_map(c, c->fb_lgC)) {
+    if (c->fast_b && make_field_tensor_map(c, c->fb_lgC)) {
         c->tma_b = true;
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) \
             c->tma_b = set_smem(k_tb_mid<A, B, fast_mid_lgC(A, B), LGF_TB_NT>, TmaMidGeom<A, B, fast_mid_lgC(A, B)>::SMEM) == cudaSuccess;
         LGF_FAST_PAIRS(X)
+#undef X
+#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) \
+            c->tma_b = set_smem(k_tm_mid<A, B, fast_mid_lgC(A, B), TM_NT>, TmaBigGeom<A, B, fast_mid_lgC(A, B)>::SMEM) == cudaSuccess;
+        LGF_BIG_PAIRS(X)
 #undef X
         if (!c->tma_b) cudaGetLastError();
     }
@@ -526,7 +553,7 @@ lgf_status setup_kernels(lgf_ctx* c) {
 lgf_status build_tables(lgf_ctx* c) {
     std::vector<real> tw(4 * 128 * 2, real(0));
     std::vector<double> s(4 * 128, 0.0);
-    for (int mu = 0; mu < 4; mu++) c->T.plan[mu] = make_plan(c->G.lg[mu], (mu & 1) != 0);
+    for (int mu = 0; mu < 4; mu++) c->T.plan[mu] = make_plan(c->G.lg[mu], (mu & 1) != 0, mu >= 2);
     const long double pi = 3.141592653589793238462643383279502884L;
     for (int mu = 0; mu < 4; mu++) {
         const int L = c->G.L[mu];
@@ -577,15 +604,26 @@ void launch_finalize(lgf_ctx* c, int n_partials) {
     launch_k(c, k_finalize, 1, n_partials > 8192 ? 1024 : 256, 0, c->partials, n_partials, c->ctl, c->hist, 1.0 / (3.0 * (double)c->G.V), 1.0 / (3.0 * (double)c->G.nd * (double)c->G.V));
 }
 // S3+S4, g rebuilt from X: one thread per link
+// rows walked in bands of 8 values of x2 (k_update_quad<..., LGB = 3>) when a CTA is one x0 row and a time slice of
+// links + X outgrows the L2 share
+bool update_banded(const lgf_ctx* c) {
+    const Geom& G = c->G;
+    if (const char* e = getenv("LGF_UPD_BAND")) return atoi(e) != 0;
+    if (G.L[0] < 64 || G.L[2] < 16) return false;
+    const double slice_mb = (double)G.L[0] * G.L[1] * G.L[2] * (2.0 * 4 * c->NC + 4) * sizeof(cplx) / 1e6;
+    return slice_mb > 48.0;
+}
 template <int NC> void launch_update_quad(lgf_ctx* c, double half_alpha) {
     LaunchScope ls(c, K_UPDATE_QUAD);
     cplx* const no_acc = nullptr;
+    const bool banded = update_banded(c);
     if (c->acc_g) {
         if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32, 1>, (unsigned)(c->G.V / 32), 128, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
         else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64, 1>, (unsigned)(c->G.V / 64), 256, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
         else launch_k(c, k_update_quad<NC, 128, 1>, (unsigned)(c->G.V / 128), 512, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
     }
     else if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32>, (unsigned)(c->G.V / 32), 128, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
+    else if (c->G.L[0] == 64 && banded) launch_k(c, k_update_quad<NC, 64, 0, 3>, (unsigned)(c->G.V / 64), 256, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
     else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64>, (unsigned)(c->G.V / 64), 256, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
     else launch_k(c, k_update_quad<NC, 128>, (unsigned)(c->G.V / 128), 512, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
 }
@@ -608,6 +646,8 @@ bool use_cluster_a(const lgf_ctx* c) { return use_big_p(c) && c->cl_ok; }
 bool use_line_b(const lgf_ctx* c) { return use_fast_b(c) && fast_pair(c->G.lg[2], c->G.lg[3]); }
 // ... on TMA-staged tiles (Landau gauge: the Coulomb pass B has no axis-3 phase and keeps the plain-load kernel)
 bool use_tma_b(const lgf_ctx* c) { return use_line_b(c) && c->opt_tma && c->tma_b && c->G.nd == 4; }
+// 64 extents: the stage-wise pass B with the tile going in and out through the TMA unit (either gauge)
+bool use_tma_big(const lgf_ctx* c) { return use_fast_b(c) && !use_line_b(c) && c->opt_tma && c->tma_b; }
 // S5 inside pass B's first CTA, where pass B is one of the compile-time-sized kernels
 bool use_fin_b(const lgf_ctx* c) { return c->opt_accel && use_fast_b(c); }
 
@@ -623,7 +663,7 @@ template <int NC> void enqueue_head(lgf_ctx* c) {
     launch_finalize(c, np);
 }
 void launch_mid(lgf_ctx* c) {
-    if (use_tma_b(c)) launch_tb_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
+    if (use_tma_b(c)) launch_tb_mid(c); else if (use_tma_big(c)) launch_tm_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
 }
 void launch_inv_x(lgf_ctx* c) {
     if (use_fast_c(c)) launch_fa_inv(c); else if (use_big_p(c)) launch_fa_inv1(c);
@@ -749,11 +789,12 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->lay = make_layout(dims, c->NC);
     c->own_ws = own; c->own_stream = own;
     c->loaded = false;
-    c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_tma = 0;
+    c->opt_store_g = 0; c->opt_graph = 1; c->opt_batch = 8; c->opt_fast = 1; c->opt_pdl = 1; c->opt_accel = 1; c->opt_tma = 1;
     { int dev = 0; c->sms = 148; cudaGetDevice(&dev); cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev); if (c->sms < 1) c->sms = 1; }
     c->shadow = nullptr; c->shadow_ws = nullptr; c->acc_g = 0; c->mixed_n32 = 0; c->mixed_switch = 12; c->pending_np = 0; c->stall_window = 0;
     c->graph_exec = nullptr; memset(&c->graph_key, 0, sizeof c->graph_key); c->profiling = 0; c->launches = 0; c->capturing = false;
-    c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr;
+    c->ev0 = c->ev1 = nullptr; c->h_ctl = nullptr; c->ws = nullptr; c->stream = nullptr; c->copy_stream = nullptr;
+    c->ev_copy[0] = c->ev_copy[1] = c->ev_kern[0] = c->ev_kern[1] = nullptr;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
 
     auto fail = [&](lgf_status st) { lgf_destroy(c); return st; };
@@ -774,6 +815,10 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->ctl = reinterpret_cast<Ctl*>(c->ws + c->lay.ctl);
     if (cudaHostAlloc(&c->h_ctl, sizeof(Ctl), cudaHostAllocDefault) != cudaSuccess) return fail(LGF_ERR_OOM);
     if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) return fail(LGF_ERR_CUDA);
+    if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(LGF_ERR_CUDA);
+    for (int k = 0; k < 2; k++)
+        if (cudaEventCreateWithFlags(&c->ev_copy[k], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->ev_kern[k], cudaEventDisableTiming) != cudaSuccess) return fail(LGF_ERR_CUDA);
     lgf_status st = setup_kernels(c);
     if (st != LGF_OK) return fail(st);
     st = build_tables(c);
@@ -784,42 +829,68 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     return LGF_OK;
 }
 
-lgf_status load_from_device_chunks(lgf_ctx* c, const double* src, bool src_is_host) {
-    const long long V = c->G.V, S = c->lay.stage_sites;
-    for (long long off = 0; off < V; off += S) {
+// Boundary copies.  The canonical array (array of structs, NE = 9 entries per link; the two-row host format: NE = 6) is
+// converted to and from the structure-of-arrays store by k_layout_in/out chunk by chunk.  Host arrays go through two
+// staging halves in the workspace: the copies run on the context's copy stream, the layout kernels on its main stream,
+// chained by events, so the copy of chunk k+1 overlaps the layout kernel of chunk k (load) and the layout kernel of chunk
+// k+1 overlaps the copy of chunk k (get).
+lgf_status load_from_device_chunks(lgf_ctx* c, const double* src, bool src_is_host, int NE = 9) {
+    const long long V = c->G.V;
+    const long long S = src_is_host ? (c->lay.stage_sites + 1) / 2 : c->lay.stage_sites;
+    const size_t site_bytes = (size_t)4 * NE * 16;
+    if (src_is_host) { CK(cudaEventRecord(c->ev_kern[0], c->stream)); CK(cudaStreamWaitEvent(c->copy_stream, c->ev_kern[0], 0)); }
+    int k = 0;
+    for (long long off = 0; off < V; off += S, k++) {
         const long long n = (V - off < S) ? V - off : S;
+        const int b = k & 1;
         const dcplx* aos;
         if (src_is_host) {
-            CK(cudaMemcpyAsync(c->staging, src + off * 72, (size_t)n * 576, cudaMemcpyHostToDevice, c->stream));
-            aos = c->staging;
-        } else aos = reinterpret_cast<const dcplx*>(src) + off * 36;
+            dcplx* half = c->staging + (size_t)b * S * 36;
+            if (k >= 2) CK(cudaStreamWaitEvent(c->copy_stream, c->ev_kern[b], 0));      // the layout kernel of chunk k-2 has read this half
+            CK(cudaMemcpyAsync(half, src + off * (4 * NE * 2), (size_t)n * site_bytes, cudaMemcpyHostToDevice, c->copy_stream));
+            CK(cudaEventRecord(c->ev_copy[b], c->copy_stream));
+            CK(cudaStreamWaitEvent(c->stream, c->ev_copy[b], 0));
+            aos = half;
+        } else aos = reinterpret_cast<const dcplx*>(src) + off * (4 * NE);
         {
             LaunchScope ls(c, K_LAYOUT_IN);
             const unsigned grid = (unsigned)((n * 4 + 255) / 256);
-            if (c->NC == 6) k_layout_in<6><<<grid, 256, 0, c->stream>>>(aos, c->links, V, off, n);
-            else k_layout_in<9><<<grid, 256, 0, c->stream>>>(aos, c->links, V, off, n);
+            if (c->NC == 6) k_layout_in<6><<<grid, 256, 0, c->stream>>>(aos, c->links, V, off, n, NE);
+            else k_layout_in<9><<<grid, 256, 0, c->stream>>>(aos, c->links, V, off, n, NE);
         }
         CK(cudaGetLastError());
+        if (src_is_host) CK(cudaEventRecord(c->ev_kern[b], c->stream));
     }
     CK(cudaStreamSynchronize(c->stream));
     c->loaded = true;
     return LGF_OK;
 }
 
-lgf_status get_to_chunks(lgf_ctx* c, double* dst, bool dst_is_host) {
-    const long long V = c->G.V, S = c->lay.stage_sites;
-    for (long long off = 0; off < V; off += S) {
+lgf_status get_to_chunks(lgf_ctx* c, double* dst, bool dst_is_host, int NE = 9) {
+    const long long V = c->G.V;
+    const long long S = dst_is_host ? (c->lay.stage_sites + 1) / 2 : c->lay.stage_sites;
+    const size_t site_bytes = (size_t)4 * NE * 16;
+    int k = 0;
+    for (long long off = 0; off < V; off += S, k++) {
         const long long n = (V - off < S) ? V - off : S;
-        dcplx* aos = dst_is_host ? c->staging : reinterpret_cast<dcplx*>(dst) + off * 36;
+        const int b = k & 1;
+        dcplx* aos = dst_is_host ? c->staging + (size_t)b * S * 36 : reinterpret_cast<dcplx*>(dst) + off * (4 * NE);
+        if (dst_is_host && k >= 2) CK(cudaStreamWaitEvent(c->stream, c->ev_copy[b], 0));            // the copy of chunk k-2 has left this half
         {
             LaunchScope ls(c, K_LAYOUT_OUT);
             const unsigned grid = (unsigned)((n * 4 + 255) / 256);
-            if (c->NC == 6) k_layout_out<6><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n);
-            else k_layout_out<9><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n);
+            if (c->NC == 6) k_layout_out<6><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n, NE);
+            else k_layout_out<9><<<grid, 256, 0, c->stream>>>(c->links, aos, V, off, n, NE);
         }
         CK(cudaGetLastError());
-        if (dst_is_host) CK(cudaMemcpyAsync(dst + off * 72, c->staging, (size_t)n * 576, cudaMemcpyDeviceToHost, c->stream));
+        if (dst_is_host) {
+            CK(cudaEventRecord(c->ev_kern[b], c->stream));
+            CK(cudaStreamWaitEvent(c->copy_stream, c->ev_kern[b], 0));
+            CK(cudaMemcpyAsync(dst + off * (4 * NE * 2), aos, (size_t)n * site_bytes, cudaMemcpyDeviceToHost, c->copy_stream));
+            CK(cudaEventRecord(c->ev_copy[b], c->copy_stream));
+        }
     }
+    if (dst_is_host) CK(cudaStreamSynchronize(c->copy_stream));
     CK(cudaStreamSynchronize(c->stream));
     return LGF_OK;
 }
@@ -895,6 +966,8 @@ void lgf_destroy(lgf_ctx* c) {
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    for (int k = 0; k < 2; k++) { if (c->ev_copy[k]) cudaEventDestroy(c->ev_copy[k]); if (c->ev_kern[k]) cudaEventDestroy(c->ev_kern[k]); }
+    if (c->copy_stream) { cudaStreamSynchronize(c->copy_stream); cudaStreamDestroy(c->copy_stream); }
     if (c->h_ctl) cudaFreeHost(c->h_ctl);
     if (c->own_ws && c->ws) cudaFree(c->ws);
     if (c->own_stream && c->stream) cudaStreamDestroy(c->stream);
@@ -910,6 +983,19 @@ lgf_status lgf_load_links_device(lgf_ctx* c, const double* dev_links) {
     FWD32(lgf32_load_links_device(c, dev_links))
     if (!c || !dev_links) return LGF_ERR_INVALID_ARG;
     return load_from_device_chunks(c, dev_links, false);
+}
+lgf_status lgf_load_links_12(lgf_ctx* c, const double* host_rows) {
+    FWD32(lgf32_load_links_12(c, host_rows))
+    if (!c || !host_rows) return LGF_ERR_INVALID_ARG;
+    if (c->NC != 6) return LGF_ERR_UNSUPPORTED;          // the two-row host format goes with two-row storage
+    return load_from_device_chunks(c, host_rows, true, 6);
+}
+lgf_status lgf_get_links_12(lgf_ctx* c, double* host_rows) {
+    FWD32(lgf32_get_links_12(c, host_rows))
+    if (!c || !host_rows) return LGF_ERR_INVALID_ARG;
+    if (c->NC != 6) return LGF_ERR_UNSUPPORTED;
+    if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    return get_to_chunks(c, host_rows, true, 6);
 }
 lgf_status lgf_get_links(lgf_ctx* c, double* host_links) {
     FWD32(lgf32_get_links(c, host_links))
@@ -1103,7 +1189,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_BATCH: *value = c->opt_batch; break;
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_FAST_FFT: *value = ((use_fast_a(c) || use_big_p(c)) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | ((use_fast_c(c) || use_big_p(c)) ? 4 : 0); break;
-        case LGF_OPT_TMA: *value = use_tma_b(c) ? 1 : 0; break;
+        case LGF_OPT_TMA: *value = (use_tma_b(c) || use_tma_big(c)) ? 1 : 0; break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;

@@ -26,9 +26,9 @@ def theta_close(t_gpu, t_ref):
 def all_variants(gf):
     """Every kernel selection the library offers, as (store g, CUDA graph, compile-time-sized FFT passes, PDL)."""
     if gf.V > (1 << 18):
-        return [(0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0), (0, 1, 1, 1, 1)]
+        return [(0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0), (0, 1, 1, 1, 0)]
     out = [(sg, graph, fast, 1) for fast in (1, 0) for sg in (0, 1) for graph in (1, 0)]
-    out += [(0, 1, 1, 0), (1, 0, 0, 0), (0, 1, 1, 1, 1), (0, 0, 1, 0, 1)]      # the last two: pass B on TMA-staged tiles
+    out += [(0, 1, 1, 0), (1, 0, 0, 0), (0, 1, 1, 1, 0), (0, 0, 1, 0, 0)]      # the last two: pass B with plain loads instead of TMA
     return out
 
 
@@ -37,7 +37,7 @@ def set_variant(gf, v):
     gf.set_option(lgf.LGF_OPT_GRAPH, v[1])
     gf.set_option(lgf.LGF_OPT_FAST_FFT, v[2])
     gf.set_option(lgf.LGF_OPT_PDL, v[3] if len(v) > 3 else 1)
-    gf.set_option(lgf.LGF_OPT_TMA, v[4] if len(v) > 4 else 0)
+    gf.set_option(lgf.LGF_OPT_TMA, v[4] if len(v) > 4 else 1)
 
 
 # ------------------------------------------------------------------ boundary: load -> get
@@ -141,7 +141,7 @@ def oracle_trajectory(U, dims, storage, checkpoints, fft_mode):
     return np.array(hist), links
 
 
-def check_trajectory(name, fft_mode, checkpoints=(10, 100), variants=((0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0), (0, 1, 1, 1, 1))):
+def check_trajectory(name, fft_mode, checkpoints=(10, 100), variants=((0, 1, 1, 1), (1, 1, 1, 1), (0, 0, 0, 1), (1, 0, 0, 0), (0, 1, 1, 1, 0))):
     U, cfg = E.make_config(name)
     dims, storage = cfg["dims"], cfg["storage"]
     hist_ref, links_ref = oracle_trajectory(U, dims, storage, checkpoints, fft_mode)
@@ -855,9 +855,7 @@ def test_fast_fft_pass_selection():
                        ((16, 32, 4, 8), 5), ((4, 8, 16, 32), 0), ((8, 8, 8, 8), 0)]:
         gf = lgf.GaugeFixer(dims, 12)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
-        # pass B on TMA-staged tiles (an option) wherever the (x2,x3) extents are 16 or 32 and the x0 extent holds a chunk
-        assert gf.get_option(lgf.LGF_OPT_TMA) == 0
-        gf.set_option(lgf.LGF_OPT_TMA, 1)
+        # pass B on TMA-staged tiles wherever the (x2,x3) extents are 16, 32 or 64 and the x0 extent holds a chunk
         assert gf.get_option(lgf.LGF_OPT_TMA) == (1 if (mask & 2) else 0), dims
         gf.set_option(lgf.LGF_OPT_FAST_FFT, 0)
         assert gf.get_option(lgf.LGF_OPT_TMA) == 0
