@@ -174,13 +174,14 @@ def dims_name(dims):
 
 
 # ---------------------------------------------------------------------------------------------- shared by both arms
-def workload_config(name: str, cfg: dict, links: str, inner: int, world: int, beta=None, sweeps=None) -> dict:
+def workload_config(name: str, cfg: dict, links: str, inner: int, world: int, beta=None, sweeps=None, overrelax=0) -> dict:
     """The `config` object of the JSON line; both arms print the same one for the same workload."""
     dims, storage = cfg["dims"], cfg["storage"]
     V = int(np.prod(dims))
     nc = 6 if storage == 12 else 9
     if links == "wilson":
-        src = f"Wilson-action heat bath beta={beta}, {sweeps} sweeps (ensembles.wilson)"
+        src = f"Wilson-action heat bath beta={beta}, {sweeps} sweeps (ensembles.wilson)" if not overrelax else \
+              f"Wilson-action heat bath + {overrelax} over-relaxation sweeps each, beta={beta}, {sweeps} compound sweeps (ensembles.wilson)"
     elif links == "device":
         src = "device-generated links (ensembles.device_su3)"
     elif links == "noisy_device":
@@ -358,7 +359,8 @@ def run_ours(args):
         gf.set_option(getattr(lgf, "LGF_OPT_" + k.upper()), int(v))
     if device_links:
         if args.links == "wilson":
-            d_in = E.wilson(dims, args.beta, args.sweeps, cfg["seed"] + 100 * rank, device="cuda")
+            wilson_hist = []
+            d_in = E.wilson(dims, args.beta, args.sweeps, cfg["seed"] + 100 * rank, device="cuda", overrelax=args.overrelax, history=wilson_hist)
         elif args.links == "noisy_device":
             d_in = E.noisy_device(dims, cfg["seed"], cfg["eps"], rank_stream(cfg, rank))
         else:
@@ -406,18 +408,36 @@ def run_ours(args):
     clocks = sampler.stop() if sampler else None
     value = whole_job_value(world, args.steps, inner, ms)
 
-    # ---- end to end through the C ABI with host buffers: H2D of the links, the iterations, D2H of the result
-    def step_e2e():
+    # ---- end to end through the C ABI with host buffers: H2D of the links, the iterations, D2H of the result.
+    # Two-row storage goes with the two-row host format (lgf_load_links_12 / lgf_get_links_12: rows 0,1 of every link, 384
+    # instead of 576 bytes per site over PCIe); the canonical 18-real format is timed beside it (e2e_canonical).
+    def step_e2e_canonical():
         gf.load_links(h_in.numpy())
         gf.iterate(inner, ALPHA)
         gf.get_links(h_out.numpy().view(np.complex128).reshape(V, 4, 3, 3))
 
     e2e_steps = max(2, min(args.steps, 5))
-    if device_links:
-        ms_e2e, e2e_value = None, None
-    else:
-        ms_e2e = timed(step_e2e, e2e_steps, 1)
-        e2e_value = whole_job_value(world, e2e_steps, inner, ms_e2e)
+    e2e = e2e_canon = None
+    if not device_links:
+        ms_c = timed(step_e2e_canonical, e2e_steps, 1)
+        e2e_canon = {"value": whole_job_value(world, e2e_steps, inner, ms_c), "unit": UNIT, "h2d_bytes_per_step": V * 576,
+                     "d2h_bytes_per_step": V * 576 + 16, "ms_per_step": ms_c / e2e_steps, "steps": e2e_steps,
+                     "host_format": "canonical [V][4][3][3][2] (lgf_load_links / lgf_get_links)"}
+        e2e = e2e_canon
+        if storage == 12:
+            rows_in = torch.from_numpy(np.ascontiguousarray(h_in.numpy().view(np.complex128).reshape(V, 4, 3, 3)[:, :, :2]).view(np.float64).reshape(-1)).pin_memory()
+            rows_out = torch.empty_like(rows_in).pin_memory()
+
+            def step_e2e_rows():
+                gf.load_links_12(rows_in.numpy())
+                gf.iterate(inner, ALPHA)
+                gf.get_links_12(rows_out.numpy().view(np.complex128).reshape(V, 4, 2, 3))
+
+            ms_r = timed(step_e2e_rows, e2e_steps, 1)
+            e2e = {"value": whole_job_value(world, e2e_steps, inner, ms_r), "unit": UNIT, "h2d_bytes_per_step": V * 384,
+                   "d2h_bytes_per_step": V * 384 + 16, "ms_per_step": ms_r / e2e_steps, "steps": e2e_steps,
+                   "host_format": "two-row [V][4][2][3][2] (lgf_load_links_12 / lgf_get_links_12; PAPER.md:45 12-real representation)"}
+            del rows_in, rows_out
 
     line = None
     if rank == 0:
@@ -434,6 +454,23 @@ def run_ours(args):
         tol = 1e-10 if fp32 else THETA_TOL                           # fp32 bottoms out near theta = 1e-14
         ttt = timed_fix(gf, reload, tol)
         ttt.update({"plaquette": plaq, "ensemble": args.workload})
+        if args.links == "wilson":
+            # thermalisation statement for the generated configuration: plaquette after every sweep, and the plateau test
+            from ensembles.heatbath import plateau
+            mean, spread, drift = plateau(wilson_hist, window=min(5, max(1, len(wilson_hist) // 2)))
+            ttt["thermalisation"] = {"beta": args.beta, "sweeps": args.sweeps, "overrelax_per_sweep": args.overrelax,
+                                     "plaquette_last_sweeps": wilson_hist[-10:], "plateau_mean": mean, "plateau_spread": spread,
+                                     "drift_between_last_two_windows": drift, "thermalised": bool(abs(drift) <= max(spread, 1e-4))}
+        # ---- step-size scan (lgf_scan_alpha): iteration counts from the same start, one lgf_fix per alpha
+        if args.scan_alpha:
+            alphas = [float(v) for v in args.scan_alpha.split(",")]
+            reload()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            sc = gf.scan_alpha(alphas, tol, 20000)
+            torch.cuda.synchronize()
+            sc["ms"] = (time.perf_counter() - t0) * 1e3
+            ttt["alpha_scan"] = sc
         # ---- the same with LGF_MIXED (fp32 phase + fp64 polish), fp64 workloads only
         if not fp32:
             try:
@@ -483,9 +520,9 @@ def run_ours(args):
             "metric": METRIC.replace("fp64", "fp32") if fp32 else METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if fp32 else "f64", "data": "synthetic",
-            "config": dict(workload_config(args.workload, cfg, args.links, inner, world, args.beta, args.sweeps), **({"options": args.opt} if args.opt else {})),
-            "e2e": None if device_links else {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": V * 576, "d2h_bytes_per_step": V * 576 + 16,
-                                              "ms_per_step": ms_e2e / e2e_steps, "steps": e2e_steps},
+            "config": dict(workload_config(args.workload, cfg, args.links, inner, world, args.beta, args.sweeps, args.overrelax), **({"options": args.opt} if args.opt else {})),
+            "e2e": e2e,
+            "e2e_canonical": e2e_canon,
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["gbs"], "peak": peak, "unit": "GB/s",
@@ -518,6 +555,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the C3 / C4 blocks of the default C2b run")
+    ap.add_argument("--scan-alpha", default="", metavar="A1,A2,...", help="also run lgf_scan_alpha over these step sizes (time_to_theta.alpha_scan)")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="set a library option on the timed context (lgf_option without the LGF_OPT_ prefix), e.g. --opt TMA=1; A/B runs and profiles")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32"],
@@ -525,6 +563,7 @@ def main():
                          "reported with dtype f32 and its own byte model; time_to_theta then stops at theta < 1e-10")
     ap.add_argument("--beta", type=float, default=6.0, help="--links wilson: coupling of the Wilson action")
     ap.add_argument("--sweeps", type=int, default=20, help="--links wilson: heat-bath sweeps from a cold start")
+    ap.add_argument("--overrelax", type=int, default=0, help="--links wilson: over-relaxation sweeps after every heat-bath sweep")
     ap.add_argument("--links", default="host", choices=["host", "device", "noisy_device", "wilson"],
                     help="host: the seeded BASELINE.json ensemble built with numpy (default); device: seeded links generated on the GPU "
                          "(large shapes C3, C4; no e2e leg, no CPU baseline); wilson: a thermalised Wilson-action configuration generated on the GPU "

@@ -265,9 +265,11 @@ def noisy_device(dims, seed: int, eps: float, stream: int = 0, device: str = "cu
     return U
 
 
-def wilson(dims, beta: float, sweeps: int, seed: int, device: str = "cpu", hot: bool = False):
+def wilson(dims, beta: float, sweeps: int, seed: int, device: str = "cpu", hot: bool = False, overrelax: int = 0, history=None):
     """Thermalised Wilson-action configuration (ensembles/heatbath.py: Cabibbo-Marinari heat bath, Kennedy-Pendleton
-    SU(2) updates) -- the kind of input the paper fixes, at a beta of the caller's choice.  Returns a
-    torch complex128 tensor [V, 4, 3, 3] on `device` (use .cpu().numpy() for the host entry points)."""
+    SU(2) updates, `overrelax` over-relaxation sweeps after each heat-bath sweep) -- the kind of input the paper fixes
+    (generated as in its ref. [6]), at a beta of the caller's choice.  `history` (a list)
+    receives the average plaquette after every sweep (thermalisation check: heatbath.plateau).  Returns a torch
+    complex128 tensor [V, 4, 3, 3] on `device` (use .cpu().numpy() for the host entry points)."""
     from .heatbath import thermalise
-    return thermalise(dims, beta, sweeps, seed, device=device, hot=hot)
+    return thermalise(dims, beta, sweeps, seed, device=device, hot=hot, overrelax=overrelax, history=history)

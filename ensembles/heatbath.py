@@ -16,7 +16,7 @@ from __future__ import annotations
 
 import math
 
-__all__ = ["thermalise", "average_plaquette"]
+__all__ = ["thermalise", "average_plaquette", "overrelax_sweep", "plateau"]
 
 
 def _axis(mu: int) -> int:
@@ -95,7 +95,14 @@ def _su2_heatbath(W, i, j, beta, gen):
     b1 = -x0 * v1 + x1 * v0 + x2 * v3 - x3 * v2
     b2 = -x0 * v2 + x2 * v0 + x3 * v1 - x1 * v3
     b3 = -x0 * v3 + x3 * v0 + x1 * v2 - x2 * v1
-    al = torch.zeros(n, 3, 3, dtype=W.dtype, device=W.device)
+    return _embed_su2(b0, b1, b2, b3, i, j, W.dtype, W.device)
+
+
+def _embed_su2(b0, b1, b2, b3, i, j, dtype, device):
+    """The SU(2) element b0 + i b.sigma on rows/columns i, j of a 3x3 identity."""
+    import torch
+    n = b0.numel()
+    al = torch.zeros(n, 3, 3, dtype=dtype, device=device)
     for d in range(3):
         al[:, d, d] = 1.0
     al[:, i, i] = torch.complex(b0, b3)
@@ -103,6 +110,21 @@ def _su2_heatbath(W, i, j, beta, gen):
     al[:, j, i] = torch.complex(-b2, b1)
     al[:, j, j] = torch.complex(b0, -b3)
     return al
+
+
+def _su2_overrelax(W, i, j):
+    """Micro-canonical (over-relaxation) update of the subgroup (i, j): with the SU(2) part of W = U A written as k V,
+    alpha = (V^dagger)^2 reflects U about the minimum of the local action; tr(alpha k V) = k tr(V^dagger) = k tr(V), so
+    Re Tr[U A] -- and with it the Wilson action -- is unchanged (ref. [6]: heat bath + over-relaxation)."""
+    import torch
+    w00, w01, w10, w11 = W[:, i, i], W[:, i, j], W[:, j, i], W[:, j, j]
+    a0 = 0.5 * (w00.real + w11.real)
+    a1 = 0.5 * (w01.imag + w10.imag)
+    a2 = 0.5 * (w01.real - w10.real)
+    a3 = 0.5 * (w00.imag - w11.imag)
+    k = torch.sqrt(a0 * a0 + a1 * a1 + a2 * a2 + a3 * a3).clamp_min(1e-300)
+    v0, v1, v2, v3 = a0 / k, a1 / k, a2 / k, a3 / k
+    return _embed_su2(2.0 * v0 * v0 - 1.0, -2.0 * v0 * v1, -2.0 * v0 * v2, -2.0 * v0 * v3, i, j, W.dtype, W.device)
 
 
 def _reunitarise(U):
@@ -127,8 +149,53 @@ def average_plaquette(links, dims):
     return float(tot) / 18.0
 
 
-def thermalise(dims, beta: float, sweeps: int, seed: int, device: str = "cpu", hot: bool = False):
-    """`sweeps` heat-bath sweeps at coupling beta from a cold (identity) or hot (random) start.
+def _parity_masks(shape, device):
+    import torch
+    ar = [torch.arange(n, device=device) for n in shape]
+    parity = (ar[0][:, None, None, None] + ar[1][None, :, None, None] + ar[2][None, None, :, None] + ar[3][None, None, None, :]) % 2
+    return [(parity == p).reshape(-1) for p in (0, 1)]
+
+
+def _sweep(U, shape, masks, update):
+    """One sweep over all links: direction by direction, parity by parity; `update(W, i, j)` gives the SU(2) factor."""
+    for mu in range(4):
+        for p in (0, 1):
+            A = _staples(U, mu).reshape(-1, 3, 3)[masks[p]]
+            Ul = U[..., mu, :, :].reshape(-1, 3, 3)[masks[p]]
+            for (i, j) in ((0, 1), (0, 2), (1, 2)):
+                Ul = update(Ul @ A, i, j) @ Ul
+            flat = U[..., mu, :, :].reshape(-1, 3, 3).clone()
+            flat[masks[p]] = Ul
+            U[..., mu, :, :] = flat.reshape(*shape, 3, 3)
+    return U
+
+
+def overrelax_sweep(links, dims):
+    """One micro-canonical over-relaxation sweep of links [V,4,3,3] (torch): every link reflected in each SU(2) subgroup.
+    Deterministic; leaves the Wilson action unchanged up to rounding (no re-orthonormalisation here, so that the
+    conservation can be checked to rounding; thermalise() re-orthonormalises after its sweeps)."""
+    L0, L1, L2, L3 = (int(d) for d in dims)
+    shape = (L3, L2, L1, L0)
+    U = links.reshape(*shape, 4, 3, 3).clone()
+    U = _sweep(U, shape, _parity_masks(shape, U.device), _su2_overrelax)
+    return U.reshape(-1, 4, 3, 3)
+
+
+def plateau(history, window: int = 5):
+    """Thermalisation check on a plaquette history (one value per sweep): (mean of the last `window` values, their
+    spread max - min, the drift between the means of the two last windows).  A thermalised run shows a drift no larger
+    than the spread."""
+    import numpy as np
+    h = np.asarray(history, dtype=float)
+    if len(h) < 2 * window:
+        return float(h[-window:].mean()), float(np.ptp(h[-window:])), float("nan")
+    return float(h[-window:].mean()), float(np.ptp(h[-window:])), float(h[-window:].mean() - h[-2 * window:-window].mean())
+
+
+def thermalise(dims, beta: float, sweeps: int, seed: int, device: str = "cpu", hot: bool = False, overrelax: int = 0, history=None):
+    """`sweeps` compound sweeps at coupling beta from a cold (identity) or hot (random) start, each one heat-bath sweep
+    followed by `overrelax` over-relaxation sweeps (the usual mix, PAPER.md:72 ref. [6]).  `history`: a list that
+    receives the average plaquette after every compound sweep (for the thermalisation check, plateau()).
     Returns a torch complex128 tensor [V, 4, 3, 3] on `device`."""
     import torch
     gen = torch.Generator(device=device)
@@ -141,19 +208,12 @@ def thermalise(dims, beta: float, sweeps: int, seed: int, device: str = "cpu", h
     if hot:
         A = torch.view_as_complex(torch.randn(*shape, 4, 3, 3, 2, dtype=torch.float64, device=device, generator=gen))
         U = _reunitarise(A)
-    ar = [torch.arange(n, device=device) for n in shape]
-    parity = (ar[0][:, None, None, None] + ar[1][None, :, None, None] + ar[2][None, None, :, None] + ar[3][None, None, None, :]) % 2
-    masks = [(parity == p).reshape(-1) for p in (0, 1)]
+    masks = _parity_masks(shape, device)
     for _ in range(int(sweeps)):
-        for mu in range(4):
-            for p in (0, 1):
-                A = _staples(U, mu).reshape(-1, 3, 3)[masks[p]]
-                Ul = U[..., mu, :, :].reshape(-1, 3, 3)[masks[p]]
-                for (i, j) in ((0, 1), (0, 2), (1, 2)):
-                    al = _su2_heatbath(Ul @ A, i, j, float(beta), gen)
-                    Ul = al @ Ul
-                flat = U[..., mu, :, :].reshape(-1, 3, 3).clone()
-                flat[masks[p]] = Ul
-                U[..., mu, :, :] = flat.reshape(*shape, 3, 3)
+        U = _sweep(U, shape, masks, lambda W, i, j: _su2_heatbath(W, i, j, float(beta), gen))
+        for _ in range(int(overrelax)):
+            U = _sweep(U, shape, masks, _su2_overrelax)
         U = _reunitarise(U)
+        if history is not None:
+            history.append(average_plaquette(U.reshape(-1, 4, 3, 3), dims))
     return U.reshape(-1, 4, 3, 3)

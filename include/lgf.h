@@ -114,6 +114,16 @@ lgf_status lgf_iterate(lgf_ctx *ctx, int n, double alpha, double *F, double *the
 lgf_status lgf_fix(lgf_ctx *ctx, double alpha, double theta_tol, int max_iter,
                    int *n_iter, double *F, double *theta);
 
+/* Step-size scan (the paper runs one alpha = 0.08; tuning it is the subject of its refs [1],[2]):
+ * from the links now in the context, one lgf_fix(alphas[k], theta_tol, max_iter) per k, each from the same start.
+ * alphas: HOST, n values > 0.  counts: HOST, n ints: the iteration count of each run, -1 where max_iter updates did not
+ * reach theta_tol, -2 where the iteration diverged (non-finite theta or F).  F_final: HOST, n doubles (may be NULL): F at
+ * the stop.  best: HOST (may be NULL): index of the smallest count, -1 if no run converged.  The context's links are the
+ * same before and after the call (the start is kept in a temporary device buffer of the size of the link store:
+ * LGF_ERR_OOM if that cannot be allocated). */
+lgf_status lgf_scan_alpha(lgf_ctx *ctx, const double *alphas, int n, double theta_tol, int max_iter,
+                          int *counts, double *F_final, int *best);
+
 /* F (PAPER.md:39 with g = 1), theta (north star step 1) and the average plaquette of the current links; no state change.  Any out pointer may be NULL. */
 lgf_status lgf_measure(lgf_ctx *ctx, double *F, double *theta, double *plaquette);
 

@@ -42,7 +42,7 @@ LGF_MAX_KERNELS = 32
 # every symbol include/lgf.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [
     "lgf_workspace_bytes", "lgf_create", "lgf_create_ex", "lgf_destroy", "lgf_load_links", "lgf_load_links_device",
-    "lgf_get_links", "lgf_get_links_device", "lgf_load_links_12", "lgf_get_links_12", "lgf_iterate", "lgf_fix", "lgf_measure", "lgf_get_history",
+    "lgf_get_links", "lgf_get_links_device", "lgf_load_links_12", "lgf_get_links_12", "lgf_iterate", "lgf_fix", "lgf_scan_alpha", "lgf_measure", "lgf_get_history",
     "lgf_get_field", "lgf_set_option", "lgf_get_option", "lgf_set_profiling", "lgf_get_profile", "lgf_kernel_name",
     "lgf_launch_count", "lgf_copy_peak", "lgf_stream_peak", "lgf_status_string", "lgf_last_error",
 ]
@@ -103,6 +103,7 @@ def lib():
     L.lgf_iterate.argtypes = [P, C.c_int, C.c_double, D, D]
     L.lgf_fix.argtypes = [P, C.c_double, C.c_double, C.c_int, I, D, D]
     L.lgf_measure.argtypes = [P, D, D, D]
+    L.lgf_scan_alpha.argtypes = [P, D, C.c_int, C.c_double, C.c_int, I, D, I]
     L.lgf_get_history.argtypes = [P, P, C.c_int, I]
     L.lgf_get_field.argtypes = [P, C.c_int, C.c_double, P]
     L.lgf_set_option.argtypes = [P, C.c_int, C.c_int]
@@ -260,6 +261,18 @@ class GaugeFixer:
         st = self._ck(lib().lgf_fix(self._h, float(alpha), float(theta_tol), int(max_iter), C.byref(n), C.byref(F), C.byref(th)),
                       "lgf_fix", ok=(LGF_OK, LGF_NOT_CONVERGED))
         return dict(status=st, n_iter=n.value, F=F.value, theta=th.value)
+
+    def scan_alpha(self, alphas, theta_tol: float, max_iter: int) -> dict:
+        """One lgf_fix per alpha from the links now loaded (which the call leaves unchanged): iteration counts
+        (-1: not converged within max_iter, -2: diverged), F at the stop, index of the best alpha (-1: none)."""
+        a = np.ascontiguousarray(alphas, dtype=np.float64)
+        n = len(a)
+        counts = (C.c_int * n)()
+        F = (C.c_double * n)()
+        best = C.c_int(-1)
+        self._ck(lib().lgf_scan_alpha(self._h, a.ctypes.data_as(C.POINTER(C.c_double)), n, float(theta_tol), int(max_iter), counts, F, C.byref(best)),
+                 "lgf_scan_alpha")
+        return dict(alphas=[float(v) for v in a], counts=[int(v) for v in counts], F=[float(v) for v in F], best=int(best.value))
 
     def measure(self):
         F, th, p = C.c_double(), C.c_double(), C.c_double()

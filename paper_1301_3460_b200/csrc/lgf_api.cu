@@ -24,6 +24,7 @@
 #define lgf_iterate lgf32_iterate
 #define lgf_fix lgf32_fix
 #define lgf_measure lgf32_measure
+#define lgf_scan_alpha lgf32_scan_alpha
 #define lgf_get_history lgf32_get_history
 #define lgf_get_field lgf32_get_field
 #define lgf_set_option lgf32_set_option
@@ -53,6 +54,7 @@ lgf_status lgf32_get_links_device(lgf_ctx* c, double* dev_links);
 lgf_status lgf32_iterate(lgf_ctx* c, int n, double alpha, double* F, double* theta);
 lgf_status lgf32_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int* n_iter, double* F, double* theta);
 lgf_status lgf32_measure(lgf_ctx* c, double* F, double* theta, double* plaq);
+lgf_status lgf32_scan_alpha(lgf_ctx* c, const double* alphas, int n, double theta_tol, int max_iter, int* counts, double* F_final, int* best);
 lgf_status lgf32_get_history(lgf_ctx* c, double* hist, int capacity, int* n_out);
 lgf_status lgf32_get_field(lgf_ctx* c, lgf_field which, double alpha, double* host_field);
 lgf_status lgf32_set_option(lgf_ctx* c, lgf_option opt, int value);
@@ -1072,6 +1074,38 @@ lgf_status lgf_fix(lgf_ctx* c, double alpha, double theta_tol, int max_iter, int
     if (F) *F = c->h_ctl->F;
     if (theta) *theta = c->h_ctl->theta;
     return c->h_ctl->converged ? LGF_OK : LGF_NOT_CONVERGED;
+}
+
+// Step-size scan (PAPER.md:47 fixes one alpha = 0.08, its refs [1],[2] tune it): the same start,
+// one lgf_fix per alpha, the iteration counts side by side.  The start is kept in a temporary device copy of the link
+// store and put back at the end, so the context's links are unchanged by the call.
+lgf_status lgf_scan_alpha(lgf_ctx* c, const double* alphas, int n, double theta_tol, int max_iter, int* counts, double* F_final, int* best) {
+    FWD32(lgf32_scan_alpha(c, alphas, n, theta_tol, max_iter, counts, F_final, best))
+    if (!c || !alphas || !counts || n < 1 || max_iter < 0 || !(theta_tol >= 0.0)) return LGF_ERR_INVALID_ARG;
+    for (int k = 0; k < n; k++) if (!(alphas[k] > 0.0) || !std::isfinite(alphas[k])) return LGF_ERR_INVALID_ARG;
+    if (!c->loaded) return LGF_ERR_NOT_LOADED;
+    const size_t bytes = (size_t)c->G.V * 4 * c->NC * sizeof(cplx);
+    void* keep = nullptr;
+    if (cudaMalloc(&keep, bytes) != cudaSuccess) { cudaGetLastError(); return LGF_ERR_OOM; }
+    lgf_status out = LGF_OK;
+    auto copy = [&](void* dst, const void* src) { return cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToDevice, c->stream) == cudaSuccess; };
+    if (!copy(keep, c->links)) out = LGF_ERR_CUDA;
+    int arg = -1;
+    for (int k = 0; k < n && out == LGF_OK; k++) {
+        if (k > 0 && !copy(c->links, keep)) { out = LGF_ERR_CUDA; break; }
+        int it = 0; double F = 0, th = 0;
+        const lgf_status st = lgf_fix(c, alphas[k], theta_tol, max_iter, &it, &F, &th);
+        if (st == LGF_OK) { counts[k] = it; if (arg < 0 || it < counts[arg]) arg = k; }
+        else if (st == LGF_NOT_CONVERGED) counts[k] = -1;         // max_iter updates did not reach theta_tol
+        else if (st == LGF_ERR_NUMERIC) counts[k] = -2;           // this alpha diverges
+        else { out = st; break; }
+        if (F_final) F_final[k] = (st == LGF_ERR_NUMERIC) ? 0.0 : F;
+    }
+    if (!copy(c->links, keep) && out == LGF_OK) out = LGF_ERR_CUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess && out == LGF_OK) out = LGF_ERR_CUDA;
+    cudaFree(keep);
+    if (out == LGF_OK && best) *best = arg;
+    return out;
 }
 
 lgf_status lgf_measure(lgf_ctx* c, double* F, double* theta, double* plaq) {

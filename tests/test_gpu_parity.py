@@ -59,6 +59,13 @@ def test_load_get_roundtrip(dims):
     o12.load(bad)
     assert np.abs(out[:, :, 2] - o12.get()[:, :, 2]).max() < 5e-16
     assert np.abs(out[:, :, 2] - U[:, :, 2]).max() < 1e-14
+    # two-row host format: rows 0,1 in, rows 0,1 out, bit exact; the same state as the canonical load
+    rows = np.ascontiguousarray(U[:, :, :2])
+    g12.load_links_12(rows)
+    assert np.array_equal(g12.get_links_12(), rows)
+    assert np.array_equal(g12.get_links(), out)
+    with pytest.raises(lgf.LgfError):
+        g18.load_links_12(rows)                                     # LGF_ERR_UNSUPPORTED with full storage
     # float64 [V,4,3,3,2] view is accepted as well
     g18.load_links(E.as_real(U))
     assert np.array_equal(g18.get_links(), U)
@@ -192,14 +199,14 @@ _cache = {}
 
 
 def oracle_links_at(U, dims, storage, n, fft_mode):
-    key = (id(U), n)
-    if key not in _cache:
+    key = (id(U), tuple(dims), storage, n, fft_mode)
+    if key not in _cache or _cache[key][0] is not U:          # the array itself is kept: an id can be reused after garbage collection
         o = oracle.Oracle(dims, storage, fft_mode=fft_mode)
         o.load(U)
         o.iterate(n, ALPHA)
         _cache.clear()
-        _cache[key] = o.get()
-    return _cache[key]
+        _cache[key] = (U, o.get())
+    return _cache[key][1]
 
 
 def test_trajectory_C0_pure_gauge_fixed_point():
@@ -233,6 +240,34 @@ def test_trajectory_C2a_C2c(name):
 def test_trajectory_C3_anisotropic():
     """BASELINE.json configs[3], 32^3 x 64: uneven FFT axes, non-cubic p^2 filter, 64-extent pass B."""
     check_trajectory("C3", fft_mode=1, checkpoints=(10, 60))
+
+
+# ------------------------------------------------------------------ step-size scan (NEXT-3)
+def test_alpha_scan_counts_equal_the_oracle():
+    """lgf_scan_alpha on C1: one lgf_fix per alpha from the same start; every count equals the oracle's for that alpha
+    (A19: exact), the best alpha is the oracle's best, a diverging alpha is reported as such, and the links in the
+    context are the same before and after."""
+    U, cfg = E.make_config("C1")
+    dims, storage = cfg["dims"], cfg["storage"]
+    alphas = [0.05, 0.0625, 0.08, 0.10, 0.2]                   # 0.2 > 1/8: beyond the stability bound of the linearised map
+    gf = lgf.GaugeFixer(dims, storage)
+    gf.load_links(U)
+    before = gf.get_links()
+    r = gf.scan_alpha(alphas, TOL, 400)
+    assert np.array_equal(gf.get_links(), before)
+    ref = []
+    for a in alphas[:-1]:
+        o = oracle.Oracle(dims, storage, fft_mode=1)
+        o.load(U)
+        rr = o.fix(a, TOL, 400)
+        assert rr["status"] == 0
+        ref.append((rr["n_iter"], rr["F"]))
+    assert r["counts"][:-1] == [n for n, _ in ref], (r, ref)
+    assert max(abs(f - fr) for f, (_, fr) in zip(r["F"][:-1], ref)) <= F_TOL
+    assert r["counts"][-1] < 0                                  # alpha = 0.2 does not converge
+    assert r["best"] == int(np.argmin([n for n, _ in ref]))
+    print("alpha scan C1:", dict(zip(alphas, r["counts"])))
+    gf.destroy()
 
 
 # ------------------------------------------------------------------ C4 as BASELINE.json states it (64^4, eps 0.35, seed 5)
