@@ -188,6 +188,28 @@ lgf_status lgf_copy_peak(void *dev_dst, const void *dev_src, size_t bytes, int r
  * launch: 384 * n_sites * (1 + write).  Same errors as lgf_copy_peak. */
 lgf_status lgf_stream_peak(void *dev_buf, size_t n_sites, int write, int reps, void *cuda_stream, double *ms);
 
+/* ---- Slab-decomposed context (the paper's CPU comparator is this decomposition over MPI +
+ * PFFT).  The lattice is cut along axis 3 into n_ranks slabs; every rank has its own workspace and runs
+ * S1, the plane passes and S3+S4 on its slab; per iteration the ranks exchange one time slice of U_3 (for S1), one time
+ * slice of X (for S3) and transpose the 64 B/site field twice (so that pass B finds axis 3 local).  This build runs the
+ * ranks as VIRTUAL ranks on the current device (one stream, n_ranks separate allocations); the only code that crosses
+ * rank boundaries is one copy function and one table of peer pointers, written for GPUs with peer access
+ * (csrc/lgf_slab.inl).  fp64, Landau gauge, the generic FFT passes.  n_ranks: a power of two <= 16 dividing L1 and L3;
+ * L0 <= 64.  Same semantics, tolerances and error codes as the single-context calls of the same names. */
+typedef struct lgf_slab_ctx lgf_slab_ctx;
+lgf_status lgf_create_sharded(const int dims[4], int n_ranks, lgf_storage s, lgf_slab_ctx **out);
+void       lgf_destroy_sharded(lgf_slab_ctx *ctx);
+int        lgf_sharded_ranks(lgf_slab_ctx *ctx);
+lgf_status lgf_load_links_sharded(lgf_slab_ctx *ctx, const double *host_links);   /* HOST, canonical order: rank r takes x3 in [r L3/P, (r+1) L3/P) */
+lgf_status lgf_get_links_sharded(lgf_slab_ctx *ctx, double *host_links);
+lgf_status lgf_iterate_sharded(lgf_slab_ctx *ctx, int n, double alpha, double *F, double *theta);
+lgf_status lgf_fix_sharded(lgf_slab_ctx *ctx, double alpha, double theta_tol, int max_iter, int *n_iter, double *F, double *theta);
+lgf_status lgf_get_history_sharded(lgf_slab_ctx *ctx, double *hist, int capacity, int *n_out);
+/* out (HOST, 5 values): bytes ONE rank sends per iteration for [0] the U_3 halo, [1] the X halo, [2] the two transposes;
+ * [3] kernels launched and [4] inter-rank copies issued by the context so far. */
+lgf_status lgf_sharded_traffic(lgf_slab_ctx *ctx, long long out[5]);
+const char *lgf_last_error_sharded(lgf_slab_ctx *ctx);
+
 const char *lgf_status_string(lgf_status s);
 const char *lgf_last_error(lgf_ctx *ctx); /* detail of the last LGF_ERR_CUDA (static or ctx-owned string) */
 

@@ -16,7 +16,7 @@ import os
 import numpy as np
 
 __all__ = [
-    "LgfError", "lib", "library_path", "GaugeFixer", "copy_peak_gbs", "stream_peak_gbs",
+    "LgfError", "lib", "library_path", "GaugeFixer", "ShardedGaugeFixer", "copy_peak_gbs", "stream_peak_gbs",
     "LGF_OK", "LGF_NOT_CONVERGED", "LGF_FP64", "LGF_FP32", "LGF_MIXED", "LGF_STORE_12", "LGF_STORE_18",
     "LGF_FIELD_DELTA", "LGF_FIELD_X", "LGF_FIELD_G",
     "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_PDL", "LGF_OPT_FAST_FFT", "LGF_OPT_FOURIER_ACCEL",
@@ -45,6 +45,8 @@ EXPORTS = [
     "lgf_get_links", "lgf_get_links_device", "lgf_load_links_12", "lgf_get_links_12", "lgf_iterate", "lgf_fix", "lgf_scan_alpha", "lgf_measure", "lgf_get_history",
     "lgf_get_field", "lgf_set_option", "lgf_get_option", "lgf_set_profiling", "lgf_get_profile", "lgf_kernel_name",
     "lgf_launch_count", "lgf_copy_peak", "lgf_stream_peak", "lgf_status_string", "lgf_last_error",
+    "lgf_create_sharded", "lgf_destroy_sharded", "lgf_sharded_ranks", "lgf_load_links_sharded", "lgf_get_links_sharded",
+    "lgf_iterate_sharded", "lgf_fix_sharded", "lgf_get_history_sharded", "lgf_sharded_traffic", "lgf_last_error_sharded",
 ]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -120,6 +122,18 @@ def lib():
     L.lgf_status_string.argtypes = [C.c_int]
     L.lgf_last_error.restype = C.c_char_p
     L.lgf_last_error.argtypes = [P]
+    L.lgf_create_sharded.argtypes = [I4, C.c_int, C.c_int, C.POINTER(P)]
+    L.lgf_destroy_sharded.restype = None
+    L.lgf_destroy_sharded.argtypes = [P]
+    L.lgf_sharded_ranks.argtypes = [P]
+    L.lgf_load_links_sharded.argtypes = [P, P]
+    L.lgf_get_links_sharded.argtypes = [P, P]
+    L.lgf_iterate_sharded.argtypes = [P, C.c_int, C.c_double, D, D]
+    L.lgf_fix_sharded.argtypes = [P, C.c_double, C.c_double, C.c_int, I, D, D]
+    L.lgf_get_history_sharded.argtypes = [P, P, C.c_int, I]
+    L.lgf_sharded_traffic.argtypes = [P, C.POINTER(C.c_longlong)]
+    L.lgf_last_error_sharded.restype = C.c_char_p
+    L.lgf_last_error_sharded.argtypes = [P]
     _lib = L
     return L
 
@@ -180,7 +194,7 @@ class GaugeFixer:
             where = "lgf_create"
         if st != LGF_OK:
             self._h = C.c_void_p()
-            raise LgfError(st, where, f"dims={self.dims}")
+            raise LgfError(st, where, f"dims={self.dims} " + L.lgf_last_error(None).decode())
 
     # ---- lifetime
     def destroy(self):
@@ -315,6 +329,68 @@ class GaugeFixer:
 
     def launch_count(self) -> int:
         return int(lib().lgf_launch_count(self._h))
+
+
+class ShardedGaugeFixer:
+    """Slab-decomposed context (include/lgf.h lgf_*_sharded): n_ranks virtual ranks on the current device, each with its
+    own workspace; argument marshalling only."""
+
+    def __init__(self, dims, n_ranks: int, storage: int = LGF_STORE_12):
+        self.dims = _dims(dims)
+        self.V = int(np.prod(self.dims))
+        self.n_ranks = int(n_ranks)
+        h = C.c_void_p()
+        st = lib().lgf_create_sharded((C.c_int * 4)(*self.dims), self.n_ranks, int(storage), C.byref(h))
+        if st != LGF_OK:
+            raise LgfError(st, "lgf_create_sharded")
+        self._h = h
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().lgf_destroy_sharded(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def _ck(self, st: int, where: str, ok=(LGF_OK,)):
+        if st not in ok:
+            raise LgfError(st, where, lib().lgf_last_error_sharded(self._h).decode())
+        return st
+
+    def load_links(self, host_links):
+        a = _host_f64(host_links, self.V * 72)
+        self._ck(lib().lgf_load_links_sharded(self._h, a.ctypes.data), "lgf_load_links_sharded")
+
+    def get_links(self) -> np.ndarray:
+        out = np.empty((self.V, 4, 3, 3), dtype=np.complex128)
+        self._ck(lib().lgf_get_links_sharded(self._h, out.ctypes.data), "lgf_get_links_sharded")
+        return out
+
+    def iterate(self, n: int, alpha: float):
+        F, th = C.c_double(), C.c_double()
+        self._ck(lib().lgf_iterate_sharded(self._h, int(n), float(alpha), C.byref(F), C.byref(th)), "lgf_iterate_sharded")
+        return F.value, th.value
+
+    def fix(self, alpha: float, theta_tol: float, max_iter: int) -> dict:
+        F, th, n = C.c_double(), C.c_double(), C.c_int()
+        st = self._ck(lib().lgf_fix_sharded(self._h, float(alpha), float(theta_tol), int(max_iter), C.byref(n), C.byref(F), C.byref(th)),
+                      "lgf_fix_sharded", ok=(LGF_OK, LGF_NOT_CONVERGED))
+        return dict(status=st, n_iter=n.value, F=F.value, theta=th.value)
+
+    def get_history(self, capacity: int = 65536) -> np.ndarray:
+        h = np.zeros((capacity, 2))
+        n = C.c_int()
+        self._ck(lib().lgf_get_history_sharded(self._h, h.ctypes.data, capacity, C.byref(n)), "lgf_get_history_sharded")
+        return h[: n.value].copy()
+
+    def traffic(self) -> dict:
+        o = (C.c_longlong * 5)()
+        self._ck(lib().lgf_sharded_traffic(self._h, o), "lgf_sharded_traffic")
+        return dict(halo_u_bytes=int(o[0]), halo_x_bytes=int(o[1]), transpose_bytes=int(o[2]), launches=int(o[3]), copies=int(o[4]))
 
 
 def copy_peak_gbs(nbytes: int = 1 << 30, reps: int = 10) -> float:

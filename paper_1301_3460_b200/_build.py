@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "liblgf.so")
 SOURCES = [os.path.join(CSRC, "lgf_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "fft_tile.cuh", "fft_fast.cuh", "fft_tma.cuh", "su3.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "fft_tile.cuh", "fft_fast.cuh", "fft_tma.cuh", "su3.cuh", "slab.cuh", "lgf_slab.inl")] + [
     os.path.join(os.path.dirname(HERE), "include", "lgf.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -295,8 +295,22 @@ void launch_k(lgf_ctx* c, void (*kern)(KArgs...), unsigned grid, unsigned block,
     cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
+// Opt a kernel in to large dynamic shared memory.  The attribute is a per-function CAP shared by every context in the
+// process, so it is always raised to the device's opt-in maximum -- setting it to one context's tile size would lower it
+// under the feet of another live context with a larger lattice.
 template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
-    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    static int optin = 0;
+    if (!optin) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess || optin <= 0) { optin = 0; return cudaErrorInvalidValue; }
+    }
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, kern);
+    if (e != cudaSuccess) return e;
+    const long long cap = (long long)optin - (long long)fa.sharedSizeBytes;      // static + dynamic <= the opt-in maximum
+    if (cap < (long long)bytes) return cudaErrorInvalidValue;
+    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cap);
 }
 
 // ---- compile-time-sized FFT passes (fft_fast.cuh): the lattices they cover, and their launchers ----------------
@@ -768,6 +782,9 @@ lgf_status run(lgf_ctx* c, double alpha, double tol, int max_iter, bool poll) {
     return LGF_OK;
 }
 
+// detail of the last failed lgf_create* of this thread (the context it belonged to is gone): lgf_last_error(NULL)
+thread_local std::string g_create_err;
+
 lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* wsp, size_t ws_bytes, void* stream, bool own, lgf_ctx** out) {
     if (!dims || !out) return LGF_ERR_INVALID_ARG;
     *out = nullptr;
@@ -799,7 +816,7 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->ev_copy[0] = c->ev_copy[1] = c->ev_kern[0] = c->ev_kern[1] = nullptr;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
 
-    auto fail = [&](lgf_status st) { lgf_destroy(c); return st; };
+    auto fail = [&](lgf_status st) { g_create_err = c->err; lgf_destroy(c); return st; };
     if (own) {
         if (cudaMalloc(&c->ws, c->lay.total) != cudaSuccess) { cudaGetLastError(); return fail(LGF_ERR_OOM); }
         if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(LGF_ERR_CUDA);
@@ -1315,7 +1332,11 @@ const char* lgf_status_string(lgf_status s) {
 #endif
 const char* lgf_last_error(lgf_ctx* c) {
     FWD32(lgf32_last_error(c))
-    return c ? c->err.c_str() : "";
+    return c ? c->err.c_str() : g_create_err.c_str();
 }
 
 }  // extern "C"
+
+#ifndef LGF_F32
+#include "lgf_slab.inl"
+#endif
