@@ -58,6 +58,7 @@ def kernel_bytes_per_site(nc: int, cb: int = 16) -> dict:
         # compile-time-sized passes (fft_fast.cuh): same traffic as the generic passes they replace
         "k_fa_delta_fwd": lk + fld,
         "k_cl_delta_fwd": lk + fld,          # 64 x 64 planes: S1 + pass A on CTA pairs
+        "k_ta_delta_fwd": lk + fld,          # S1 + pass A with the links staged by the TMA unit
         "k_fa_mid": 2 * fld,
         "k_fr_mid": 2 * fld,                 # pass B with whole lines in registers: same traffic
         "k_fa_inv": 2 * fld,

@@ -152,10 +152,12 @@ lgf_status lgf_get_field(lgf_ctx *ctx, lgf_field which, double alpha, double *ho
  *   LGF_OPT_PDL              1 (default): programmatic dependent launch between the kernels of an iteration.  0: off.
  *   LGF_OPT_FAST_FFT         1 (default): compile-time-sized FFT passes where the lattice allows (extents 16/32/64).
  *                            0: the generic passes.  get: bit mask of the passes that run fast (1 A, 2 B, 4 C).
- *   LGF_OPT_TMA              1 (default): pass B (axes 2,3) runs persistent, one CTA per SM, its tiles staged by the Tensor
- *                            Memory Accelerator (cp.async.bulk.tensor + mbarrier): at 16/32 extents the next tiles stream in
- *                            while the current ones are transformed; at 64 extents the tile goes in and out through the TMA
- *                            unit.  0: one CTA per tile, plain loads and stores.  get: 1 when a TMA pass actually runs.
+ *   LGF_OPT_TMA              1 (default): the FFT passes run persistent, one CTA per SM, fed by the Tensor Memory Accelerator
+ *                            (cp.async.bulk.tensor + mbarrier).  Pass A (S1 + axes 0,1; 16/32 extents, two-row storage): the
+ *                            links stream into shared memory stage by stage while the warps compute Delta and transform.
+ *                            Pass B (axes 2,3): at 16/32 extents the next tiles stream in while the current ones are
+ *                            transformed; at 64 extents the tile goes in and out through the TMA unit.  0: one CTA per plane
+ *                            or tile, plain loads and stores.  get: bit mask of the TMA passes that actually run (1 B, 2 A).
  *   LGF_OPT_MIXED_FP32_ITERS read-only: fp32 iterations of the last LGF_MIXED lgf_fix.
  *   LGF_OPT_MIXED_SWITCH     LGF_MIXED: the fp32 phase aims at theta = 10^-value (default 12, 4..20) and hands over to fp64
  *                            there, or earlier when theta stops falling (it has not halved within 256 iterations). */

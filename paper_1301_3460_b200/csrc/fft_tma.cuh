@@ -380,3 +380,142 @@ __global__ void __launch_bounds__(NT, 1) k_tm_mid(const __grid_constant__ CUtens
 }
 
 }  // namespace lgf
+
+namespace lgf {
+
+// ---------------------------------------------------------------------------------------------------------------
+// Pass A (S1 + forward FFT over axes 0,1) with the links staged by the TMA unit.
+//
+// k_fa_delta_fwd is bound by the latency of S1's loads (ncu, profiles/r01: long_scoreboard 9.6 cycles per issue at 14.5
+// warps per SM; 48 loads per site, each warp waits for all of them before it computes).  Here one persistent CTA per SM
+// walks over its (x2,x3) planes and the links arrive by bulk tensor copies, stage by stage, while the warps work: a
+// stage is 128 consecutive sites of the plane (R = 128/L0 rows) and holds, as dense arrays [stream][site],
+//   own   the 4 NC streams of the sites' own links U_mu(x)                       one copy, box (256 reals, 1 plane, 4 NC streams)
+//   nb2   U_2(x-2): the NC streams of direction 2 in the plane (x2-1, x3)        box (256, 1, NC)
+//   nb3   U_3(x-3): direction 3 in the plane (x2, x3-1)                          box (256, 1, NC)
+//   row1  U_1 of the row below the stage's first row (U_1(x-1) of that row)      box (2 L0, 1, NC)
+// (U_0(x-0), and U_1(x-1) of the other rows, are inside `own`).  The links are a 3-D tensor for the TMA unit:
+// (2 L0 L1 reals of a plane, L2 L3 planes, 4 NC streams).  NT = 256 threads = two groups of 128, a thread = one site of
+// a stage; group g takes the stages s = g (mod 2) into ITS OWN buffer, and when all its threads have read the buffer its
+// thread 0 starts the copies of stage s + 2 -- of the same plane or the CTA's next one -- and arms the buffer's mbarrier.
+// So two stages (150 KB at 32 x 32, fp64) are always in flight or being consumed, also while all warps transform the
+// finished tile, and no warp ever waits on a global load.
+struct LinkMaps { CUtensorMap own, nb, row; };
+
+template <int LG0, int LG1, int NC> struct TmaPlaneGeom {
+    static constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1, nP = L0 * L1;
+    static constexpr int SS = 128;                                   // sites per stage
+    static constexpr int NST = nP / SS;                              // stages per plane
+    static constexpr int OWN = 4 * NC * SS, NB = NC * SS, ROW = NC * L0;      // complex numbers
+    static constexpr int STAGE = OWN + 2 * NB + ROW;
+    static constexpr unsigned STAGE_BYTES = STAGE * sizeof(cplx);
+    static_assert(NST >= 2 && NST % 2 == 0, "each group takes every other stage");
+    static_assert((OWN * sizeof(cplx)) % 128 == 0 && (NB * sizeof(cplx)) % 128 == 0, "TMA destinations are 128-byte aligned");
+    static constexpr size_t SMEM = (size_t)(2 * STAGE + 4 * SC + L0 + L1) * sizeof(cplx) + 128;
+};
+
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+template <int NC> __device__ __forceinline__ void load_link_smem(const cplx* __restrict__ p, int stride, cplx (&u)[9]) {
+#pragma unroll
+    for (int c = 0; c < NC; c++) u[c] = p[c * stride];
+    if (NC == 6) third_row(u);
+}
+
+template <int LG0, int LG1, int NC, int NT>
+__global__ void __launch_bounds__(NT, 1) k_ta_delta_fwd(const __grid_constant__ LinkMaps maps, cplx* __restrict__ field, double2* __restrict__ partials,
+                                                        Geom G, FftTables T, const Ctl* __restrict__ ctl, int n_planes) {
+    static_assert(NT == 256, "two groups of 128 threads");
+    pdl_enter();
+    if (ctl->done) return;                               // uniform over the grid; nothing has been issued yet
+    using PG = TmaPlaneGeom<LG0, LG1, NC>;
+    constexpr int L0 = PG::L0, L1 = PG::L1, S = PG::S, SC = PG::SC, SS = PG::SS, NST = PG::NST, GT = 128;
+    __shared__ __align__(8) uint64_t full[2];
+    __shared__ double red[64];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* stage = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u));      // [2][STAGE]
+    cplx* tile = stage + 2 * PG::STAGE;
+    cplx* tw0 = tile + 4 * SC;
+    cplx* tw1 = tw0 + L0;
+    for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
+    for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
+    const int n_seq = (n_planes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;      // planes of this CTA
+    const int n_stage = n_seq * NST;
+    // stage t of this CTA: plane blockIdx.x + (t / NST) gridDim.x, rows [(t % NST) R, ...), buffer t & 1
+    auto issue = [&](int t) {
+        const int plane = blockIdx.x + (t / NST) * gridDim.x, s = t % NST, b = t & 1;
+        const int x2 = plane & (G.L[2] - 1), x3 = plane >> G.lg[2];
+        const int pl2 = ((x2 + G.L[2] - 1) & (G.L[2] - 1)) + (x3 << G.lg[2]);
+        const int pl3 = x2 + (((x3 + G.L[3] - 1) & (G.L[3] - 1)) << G.lg[2]);
+        const int r0 = 2 * SS * s;                                      // first real of the stage inside the plane
+        const int rowb = 2 * L0 * (((s * (SS / L0)) + L1 - 1) & (L1 - 1));   // the row below the stage's first row
+        cplx* d = stage + b * PG::STAGE;
+        mbar_expect_tx(&full[b], PG::STAGE_BYTES);
+        tma_load_3d(d, &maps.own, &full[b], r0, plane, 0);
+        tma_load_3d(d + PG::OWN, &maps.nb, &full[b], r0, pl2, 2 * NC);
+        tma_load_3d(d + PG::OWN + PG::NB, &maps.nb, &full[b], r0, pl3, 3 * NC);
+        tma_load_3d(d + PG::OWN + 2 * PG::NB, &maps.row, &full[b], rowb, plane, NC);
+    };
+    if (threadIdx.x == 0) {
+        mbar_init(&full[0], 1); mbar_init(&full[1], 1);
+        mbar_init_fence();
+        for (int t = 0; t < 2 && t < n_stage; t++) issue(t);
+    }
+    __syncthreads();
+    const int grp = threadIdx.x / GT;
+    const Grp g{(int)threadIdx.x % GT, 1 + grp};
+    const Grp all{(int)threadIdx.x, 0};
+    const int j = g.tid;                                               // site of the stage
+    const int jx = j & (L0 - 1), jr = j >> LG0;                        // x0, row inside the stage
+    const int jm0 = (j & ~(L0 - 1)) | ((jx + L0 - 1) & (L0 - 1));      // x - 0 (periodic inside the row)
+#pragma unroll 1
+    for (int q = 0; q < n_seq; q++) {
+        const int plane = blockIdx.x + q * gridDim.x;
+        double th = 0, fs = 0;
+#pragma unroll 1
+        for (int s = grp; s < NST; s += 2) {
+            const int t = q * NST + s;
+            const cplx* own = stage + grp * PG::STAGE;                 // buffer t & 1 = grp (NST is even)
+            const cplx* nb2 = own + PG::OWN;
+            const cplx* nb3 = nb2 + PG::NB;
+            const cplx* row1 = nb3 + PG::NB;
+            mbar_wait(&full[grp], (t >> 1) & 1);
+            cplx d01 = mk(0, 0), d02 = mk(0, 0), d12 = mk(0, 0);
+            real i0 = 0, i1 = 0, i2 = 0, retr = 0;
+            cplx u[9];
+#pragma unroll
+            for (int mu = 0; mu < 4; mu++) {
+                load_link_smem<NC>(own + mu * NC * SS + j, SS, u);
+                retr += u[0].x + u[4].x + u[8].x;
+                acc_link(u, real(-1), d01, d02, d12, i0, i1, i2);
+            }
+            load_link_smem<NC>(own + jm0, SS, u);                                      // U_0(x-0)
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
+            if (jr == 0) load_link_smem<NC>(row1 + jx, L0, u);                          // U_1(x-1)
+            else load_link_smem<NC>(own + NC * SS + j - L0, SS, u);
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
+            load_link_smem<NC>(nb2 + j, SS, u);                                        // U_2(x-2)
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
+            load_link_smem<NC>(nb3 + j, SS, u);                                        // U_3(x-3)
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
+            const real tr3 = real(2.0 / 3.0) * (i0 + i1 + i2);
+            const real e0 = real(2) * i0 - tr3, e1 = real(2) * i1 - tr3, e2 = real(2) * i2 - tr3;
+            th += (double)(real(2) * (cnorm2(d01) + cnorm2(d02) + cnorm2(d12)) + e0 * e0 + e1 * e1 + e2 * e2);
+            fs += (double)retr;
+            const int o = jx + (s * (SS / L0) + jr) * S;
+            tile[o] = d01; tile[SC + o] = d02; tile[2 * SC + o] = d12; tile[3 * SC + o] = mk(e0, e1);
+            gsync<GT>(g);                                              // every thread of the group has read the buffer
+            if (g.tid == 0 && t + 2 < n_stage) issue(t + 2);
+        }
+        group_sum2<NT>(th, fs, red, all);                              // its barrier also completes the tile
+        if (threadIdx.x == 0) partials[plane] = make_double2(th, fs);
+        gsync<NT>(all);
+        plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)plane << (LG0 + LG1), all);
+        gsync<NT>(all);                                                // the tile is rewritten by the next plane's S1
+    }
+}
+
+}  // namespace lgf

@@ -92,13 +92,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G,
-    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_TB_MID, K_TM_MID, K_NSLOTS
+    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_TB_MID, K_TM_MID, K_TA_DELTA_FWD, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g",
-    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_tb_mid", "k_tm_mid"};
+    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_tb_mid", "k_tm_mid", "k_ta_delta_fwd"};
 
 constexpr int HIST_CAP = 1 << 16;
 // mixed precision: the fp32 phase ends when theta has not halved within this many iterations (a rough thermalised
@@ -210,6 +210,8 @@ struct lgf_ctx {
     // pass B on TMA-staged tiles (fft_tma.cuh): the field as a 5-D tensor map, whether it could be built
     CUtensorMap tm_field;
     bool tma_b;
+    LinkMaps tm_links;      // pass A with the links staged by the TMA unit (k_ta_delta_fwd)
+    bool tma_a;
     int sms;                // SMs of the device
     // compile-time-sized FFT passes available for this lattice: pass A (fused Delta), B (middle), C (inverse)
     bool fast_a, fast_b, fast_c, big_p, cl_ok;
@@ -436,6 +438,17 @@ void launch_tb_mid(lgf_ctx* c) {
 #undef X
 }
 
+// pass A with TMA-staged links (fft_tma.cuh k_ta_delta_fwd): 16/32 extents, one persistent CTA per SM
+template <int NC> void launch_ta_delta_fwd(lgf_ctx* c) {
+    LaunchScope ls(c, K_TA_DELTA_FWD);
+    const int n_planes = c->G.L[2] * c->G.L[3];
+    const unsigned grid = (unsigned)(n_planes < c->sms ? n_planes : c->sms);
+#define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
+        launch_k(c, k_ta_delta_fwd<A, B, NC, 256>, grid, 256, TmaPlaneGeom<A, B, NC>::SMEM, c->tm_links, c->field, c->partials, c->G, c->T, c->ctl, n_planes);
+    LGF_FAST_PAIRS(X)
+#undef X
+}
+
 // pass B on TMA-staged tiles, 64 extents: the tile goes in and out through the TMA unit (fft_tma.cuh k_tm_mid)
 constexpr int TM_NT = 512;
 void launch_tm_mid(lgf_ctx* c) {
@@ -471,6 +484,31 @@ bool make_field_tensor_map(lgf_ctx* c, int lgC) {
         5, c->field, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
+}
+
+// The link store as a 3-D tensor of reals (2 L0 L1 reals of a plane, L2 L3 planes, 4 NC streams) with the three boxes of
+// a pass-A stage: 128 sites x all streams, 128 sites x the NC streams of one direction, one x0 row x NC streams.
+bool make_link_tensor_maps(lgf_ctx* c) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    const Geom& G = c->G;
+    const cuuint64_t esz = sizeof(cplx);
+    const cuuint64_t plane = (cuuint64_t)G.L[0] * G.L[1];
+    const cuuint64_t dims[3] = {2 * plane, (cuuint64_t)G.L[2] * G.L[3], (cuuint64_t)(4 * c->NC)};
+    const cuuint64_t strides[2] = {esz * plane, esz * (cuuint64_t)G.V};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    const CUtensorMapDataType dt = sizeof(real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    const cuuint32_t boxes[3][3] = {{256, 1, (cuuint32_t)(4 * c->NC)}, {256, 1, (cuuint32_t)c->NC}, {(cuuint32_t)(2 * G.L[0]), 1, (cuuint32_t)c->NC}};
+    CUtensorMap* maps[3] = {&c->tm_links.own, &c->tm_links.nb, &c->tm_links.row};
+    for (int k = 0; k < 3; k++)
+        if (reinterpret_cast<EncodeTiledFn>(fn)(maps[k], dt, 3, c->links, dims, strides, boxes[k], estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return false;
+    return true;
 }
 
 lgf_status setup_fast(lgf_ctx* c) {
@@ -512,6 +550,15 @@ lgf_status setup_fast(lgf_ctx* c) {
         LGF_BIG_PAIRS(X)
 #undef X
         if (!c->tma_b) cudaGetLastError();
+    }
+    c->tma_a = false;
+    if (c->fast_a && make_link_tensor_maps(c)) {
+#define X(A, B) if (G.lg[0] == A && G.lg[1] == B) \
+            c->tma_a = (c->NC == 6) ? set_smem(k_ta_delta_fwd<A, B, 6, 256>, TmaPlaneGeom<A, B, 6>::SMEM) == cudaSuccess \
+                                    : set_smem(k_ta_delta_fwd<A, B, 9, 256>, TmaPlaneGeom<A, B, 9>::SMEM) == cudaSuccess;
+        LGF_FAST_PAIRS(X)
+#undef X
+        if (!c->tma_a) cudaGetLastError();               // e.g. 18-real links at 32 x 32: two stages do not fit one SM
     }
     c->cl_ok = false;
     if (c->big_p && G.lg[0] == 6 && G.lg[1] == 6) {
@@ -656,6 +703,12 @@ bool use_fused(const lgf_ctx* c) { return c->fft01_ncomp_fused_ok; }
 bool use_store_g(const lgf_ctx* c) { return c->opt_store_g && c->fft01_ncomp_fused_ok && !c->acc_g; }
 bool use_fast_a(const lgf_ctx* c) { return c->opt_fast && c->fast_a; }
 bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
+// pass A with TMA-staged links (Landau gauge; the Coulomb S1 keeps the plain-load kernel)
+// -- from two planes per SM on: the persistent grid has one CTA per SM, and below that its tail costs more than the staging
+// gains (16^4, 256 planes on 148 SMs: 12.7 against 10.7 us)
+bool use_tma_a(const lgf_ctx* c) {
+    return c->opt_fast && c->fast_a && c->opt_tma && c->tma_a && c->G.nd == 4 && c->G.L[2] * c->G.L[3] >= 2 * c->sms;
+}
 bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c; }
 bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p; }
 bool use_cluster_a(const lgf_ctx* c) { return use_big_p(c) && c->cl_ok; }
@@ -670,7 +723,8 @@ bool use_fin_b(const lgf_ctx* c) { return c->opt_accel && use_fast_b(c); }
 // S1 (+ pass A) and, unless pass B does it, the reduction.
 template <int NC> void enqueue_head(lgf_ctx* c) {
     int np;
-    if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
+    if (use_tma_a(c)) { launch_ta_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
+    else if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
     else if (use_cluster_a(c)) { launch_cl_delta_fwd<NC>(c); np = 2 * c->G.L[2] * c->G.L[3]; }
     else if (use_big_p(c)) { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fa_fwd1(c); }
     else if (use_fused(c)) { launch_fft01<MODE_DELTA_FWD, NC>(c, K_FFT01_DELTA_FWD, 0.0); np = c->G.L[2] * c->G.L[3]; }
@@ -1240,7 +1294,7 @@ lgf_status lgf_get_option(lgf_ctx* c, lgf_option opt, int* value) {
         case LGF_OPT_BATCH: *value = c->opt_batch; break;
         case LGF_OPT_PDL: *value = c->opt_pdl; break;
         case LGF_OPT_FAST_FFT: *value = ((use_fast_a(c) || use_big_p(c)) ? 1 : 0) | (use_fast_b(c) ? 2 : 0) | ((use_fast_c(c) || use_big_p(c)) ? 4 : 0); break;
-        case LGF_OPT_TMA: *value = (use_tma_b(c) || use_tma_big(c)) ? 1 : 0; break;
+        case LGF_OPT_TMA: *value = ((use_tma_b(c) || use_tma_big(c)) ? 1 : 0) | (use_tma_a(c) ? 2 : 0); break;
         case LGF_OPT_FOURIER_ACCEL: *value = c->opt_accel; break;
         case LGF_OPT_GAUGE_DIRECTIONS: *value = c->G.nd; break;
         case LGF_OPT_MIXED_FP32_ITERS: *value = c->mixed_n32; break;
