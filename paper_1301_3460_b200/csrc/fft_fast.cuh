@@ -645,7 +645,7 @@ __device__ __forceinline__ void pass_b_finish(cplx* __restrict__ gp, double s01,
 #pragma unroll
                 for (int m = 0; m < PB::R2; m++) {
                     const double p2 = s012 + s3[bb * PB::R2 + m];
-                    const double wgt = (p2 > 0.0) ? scale / p2 : 0.0;
+                    const double wgt = filter_weight(scale, p2);
                     v[m] = cscale(v[m], (real)wgt);
                 }
                 bfly<PB::R2, true>(v);
@@ -826,7 +826,7 @@ __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ f
 #pragma unroll
             for (int m = 0; m < L2; m++) {
                 const double p2 = s01 + s2[m];
-                v[m] = cscale(v[m], (real)((p2 > 0.0) ? scale * (double)L3 / p2 : 0.0));      // no 1/L3: axis 3 is not transformed
+                v[m] = cscale(v[m], (real)filter_weight(scale * (double)L3, p2));      // no 1/L3: axis 3 is not transformed
             }
             line_fft<LG2, false, true>(v);
 #pragma unroll
@@ -863,7 +863,7 @@ __global__ void __launch_bounds__(NT, LGF_FR_MINB) k_fr_mid(cplx* __restrict__ f
 #pragma unroll
         for (int m = 0; m < L3; m++) {
             const double p2 = s012 + s3[m];
-            v[m] = cscale(v[m], (real)((p2 > 0.0) ? scale / p2 : 0.0));
+            v[m] = cscale(v[m], (real)filter_weight(scale, p2));
         }
         line_fft<LG3, true, true>(v);
 #pragma unroll

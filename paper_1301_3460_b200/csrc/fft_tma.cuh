@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(NT, 1) k_tb_mid(const __grid_constant__ CUtens
 #pragma unroll
             for (int m = 0; m < L3; m++) {
                 const double p2 = s012 + s3[m];
-                v[m] = cscale(v[m], (real)((p2 > 0.0) ? scale / p2 : 0.0));
+                v[m] = cscale(v[m], (real)filter_weight(scale, p2));
             }
             line_fft<LG3, true, true>(v);
 #pragma unroll
@@ -335,7 +335,7 @@ __global__ void __launch_bounds__(NT, 1) k_tm_mid(const __grid_constant__ CUtens
 #pragma unroll
                     for (int m = 0; m < PB::R2; m++) {
                         const double p2 = s012 + s3[bb * PB::R2 + m];
-                        v[m] = cscale(v[m], (real)((p2 > 0.0) ? scale / p2 : 0.0));
+                        v[m] = cscale(v[m], (real)filter_weight(scale, p2));
                     }
                     bfly<PB::R2, true>(v);
 #pragma unroll

@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(256) k_fft23_mid(cplx* __restrict__ field, Geo
         const int i0 = e & (C0 - 1), r = e >> lgC;
         const int i2 = r & (L2 - 1), i3 = r >> G.lg[2];
         const double p2 = (T.s[0][p0base + i0] + s01_base) + (s2[i2] + s3[i3]);
-        const double w = (p2 > 0.0) ? scale / p2 : 0.0;
+        const double w = filter_weight(scale, p2);
         cplx* q = tile + i0 + i2 * S1 + i3 * S2;
         cplx v = *q;
         *q = cscale(v, (real)w);

@@ -132,6 +132,21 @@ __device__ __forceinline__ void rotate_link(const cplx (&g)[9], const cplx (&u)[
     }
 }
 
+// S2b filter weight scale / p2 (scale = p2max / V), 0 for the zero mode.  p2 lies in [4 sin^2(pi/128), 16]: no special
+// cases, so the division is a reciprocal seed (MUFU.RCP64H, ~20 bits) and two Newton steps -- within 2 ulp of the IEEE
+// quotient at a quarter of its instructions (the IEEE fp64 division was a quarter of pass B's instruction stream).
+// Every pass-B kernel, generic or compile-time-sized, uses this one function, so all kernel selections agree bit for bit.
+__device__ __forceinline__ double filter_weight(double scale, double p2) {
+    if (!(p2 > 0.0)) return 0.0;
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(p2));
+    double e = fma(-p2, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-p2, r, 1.0);
+    r = fma(r, e, r);
+    return scale * r;
+}
+
 // Lattice geometry: every L_mu is a power of two, x = x0 + L0*(x1 + L1*(x2 + L2*x3)).
 struct Geom {
     int L[4];
