@@ -890,8 +890,10 @@ def test_fast_fft_pass_selection():
                        ((16, 32, 4, 8), 5), ((4, 8, 16, 32), 0), ((8, 8, 8, 8), 0)]:
         gf = lgf.GaugeFixer(dims, 12)
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == mask, dims
-        # TMA-staged passes: bit 1 pass B (wherever the compile-time-sized pass B runs), bit 2 pass A (16/32-extent planes)
-        assert gf.get_option(lgf.LGF_OPT_TMA) == ((1 if (mask & 2) else 0) | (2 if (mask & 1) else 0)), dims
+        # TMA-staged passes: bit 1 pass B (wherever the compile-time-sized pass B runs), bit 2 pass A (16/32-extent planes,
+        # from two planes per SM on: 32^4 has 1024, 16^4 256)
+        tma_a = 2 if ((mask & 1) and dims[2] * dims[3] >= 512) else 0
+        assert gf.get_option(lgf.LGF_OPT_TMA) == ((1 if (mask & 2) else 0) | tma_a), dims
         gf.set_option(lgf.LGF_OPT_FAST_FFT, 0)
         assert gf.get_option(lgf.LGF_OPT_TMA) == 0
         assert gf.get_option(lgf.LGF_OPT_FAST_FFT) == 0
