@@ -65,6 +65,7 @@ def kernel_bytes_per_site(nc: int, cb: int = 16) -> dict:
         "k_fa_inv_g": fld + g,               # read X~ field, write rows 0,1 of g
         "k_tb_mid": 2 * fld,                 # pass B on TMA-staged tiles: same traffic
         "k_tm_mid": 2 * fld,                 # ... 64 extents
+        "k_tr_mid": 2 * fld,                 # ... 64 extents, ring of half-chunk tiles
     }
 
 

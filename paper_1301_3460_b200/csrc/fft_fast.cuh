@@ -52,6 +52,11 @@ struct Grp { int tid; int bar; };
 template <int NT> __device__ __forceinline__ void gsync(const Grp& g) {
     asm volatile("bar.sync %0, %1;" ::"r"(g.bar), "n"(NT) : "memory");
 }
+// Compile-time group: BAR = 0 is the whole CTA (__syncthreads), else a named barrier over NT threads.
+template <int NT, int BAR> __device__ __forceinline__ void gsync_c() {
+    if constexpr (BAR == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(NT) : "memory");
+}
 
 // Two-stage plan of an axis of length 2^LG (LG = 4, 5, 6); B = axis 1 or 3.  Must agree with make_plan().
 template <int LG, bool B> struct Plan2 {

@@ -211,6 +211,142 @@ template <int LG2, int LG3, int LGC> struct TmaBigGeom {
     static constexpr size_t SMEM = (size_t)(TILE + L2 + L3) * sizeof(cplx) + (size_t)(L2 + L3) * 8 + 128;
 };
 
+// The stages of pass B on one dense tile (entry: the TMA box [i3][i2][i0]; exit: the same layout, transformed), run by
+// the GT threads of group g; tl = tile + the thread's x0 offset (g.tid % C0).  Ends behind the group's last writes (the
+// caller fences and synchronises before the tile is handed to the TMA unit).
+template <int LG2, int LG3, int LGC, int GT, int BAR>
+__device__ __forceinline__ void mid_tile_stages(cplx* tl, const cplx* tw2, const cplx* tw3, const double* s2, const double* s3, double s01, double scale,
+                                                int gtid) {
+    using PA = PlanM<LG2, false>;
+    using PB = PlanM<LG3, true>;
+    constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = 1 << LGC;
+    constexpr int SI2 = C0, SI3 = C0 * L2;               // element strides of i2 and i3 in the dense tile
+    constexpr int SWM = (C0 < 8) ? (8 / C0 - 1) : 0;
+    static_assert(PA::R2 == 4 && PB::R1 == 4, "one 16-point block between the axes");
+    static_assert(GT % C0 == 0, "a thread keeps its x0 offset");
+    // axis-2 stage 1 (points i2 = ja + m R2, twiddles tw2[k ja]): dense in, swizzled out
+    {
+        constexpr int NW = C0 * PA::R2 * L3, NI = (NW + GT - 1) / GT;
+        static_assert(NW % GT == 0, "whole items per thread");
+        cplx v[NI][PA::R1];
+#pragma unroll
+        for (int k = 0; k < NI; k++) {
+            const int w = k * GT + gtid;
+            const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+            const cplx* p = tl + ja * SI2 + i3 * SI3;
+#pragma unroll
+            for (int m = 0; m < PA::R1; m++) v[k][m] = p[m * PA::R2 * SI2];
+            stage_regs<PA::R1, false, true>(v[k], tw2, ja);
+        }
+        gsync_c<GT, BAR>();
+#pragma unroll
+        for (int k = 0; k < NI; k++) {
+            const int w = k * GT + gtid;
+            const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+            // position (ja + 4 m) ^ sw = (ja ^ (sw & 3)) + 4 (m ^ (sw >> 2)): two base pointers, static offsets
+            const int sw = i3 & SWM, hb = (sw >> 2) * 4 * SI2;
+            cplx* pe = tl + (ja ^ (sw & 3)) * SI2 + i3 * SI3 + hb;
+            cplx* po = pe - 2 * hb;
+#pragma unroll
+            for (int m = 0; m < PA::R1; m++) ((m & 1) ? po : pe)[m * PA::R2 * SI2] = v[k][m];
+        }
+        gsync_c<GT, BAR>();
+    }
+    // 16-point block: last stage of axis 2 (contiguous sub-blocks of 4) x first stage of axis 3 (points jb + mb R2b)
+    auto block = [&](auto inv_tag) {
+        constexpr bool INV = decltype(inv_tag)::value;
+        constexpr int NW = C0 * PB::R2 * PA::R1;
+#pragma unroll
+        for (int w0 = 0; w0 < NW; w0 += GT) {
+            const int w = w0 + gtid;
+            if (NW % GT == 0 || w < NW) {
+                const int jb = (w / C0) % PB::R2, ba = w / (C0 * PB::R2);
+                const int sw = jb & SWM;
+                cplx v[4][4];                        // [mb][ma]
+#pragma unroll
+                for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+                    for (int ma = 0; ma < 4; ma++) v[mb][ma] = tl[((ba * 4 + ma) ^ sw) * SI2 + (jb + mb * PB::R2) * SI3];
+                if constexpr (!INV) {
+#pragma unroll
+                    for (int mb = 0; mb < 4; mb++) bfly<4, false>(v[mb]);
+                }
+#pragma unroll
+                for (int ma = 0; ma < 4; ma++) {
+                    cplx c[4];
+#pragma unroll
+                    for (int mb = 0; mb < 4; mb++) c[mb] = v[mb][ma];
+                    stage_regs<4, INV, true>(c, tw3, jb);
+#pragma unroll
+                    for (int mb = 0; mb < 4; mb++) v[mb][ma] = c[mb];
+                }
+                if constexpr (INV) {
+#pragma unroll
+                    for (int mb = 0; mb < 4; mb++) bfly<4, true>(v[mb]);
+                }
+#pragma unroll
+                for (int mb = 0; mb < 4; mb++)
+#pragma unroll
+                    for (int ma = 0; ma < 4; ma++) tl[((ba * 4 + ma) ^ sw) * SI2 + (jb + mb * PB::R2) * SI3] = v[mb][ma];
+            }
+        }
+        gsync_c<GT, BAR>();
+    };
+    block(std::false_type{});
+    // axis-3 stage 2 forward, S2b filter X~ = (p2max / (V p2)) Delta~ at the stored positions (zero mode -> 0), axis-3
+    // stage 2 inverse, on the same registers                                                   [north_star step 2]
+    {
+        constexpr int NW = C0 * L2 * PB::R1;
+#pragma unroll
+        for (int w0 = 0; w0 < NW; w0 += GT) {
+            const int w = w0 + gtid;
+            if (NW % GT == 0 || w < NW) {
+                const int i2 = (w / C0) % L2, bb = w / (C0 * L2);
+                cplx v[PB::R2];
+#pragma unroll
+                for (int m = 0; m < PB::R2; m++) v[m] = tl[(i2 ^ (m & SWM)) * SI2 + (bb * PB::R2 + m) * SI3];
+                bfly<PB::R2, false>(v);
+                const double s012 = s01 + s2[i2];
+#pragma unroll
+                for (int m = 0; m < PB::R2; m++) {
+                    const double p2 = s012 + s3[bb * PB::R2 + m];
+                    v[m] = cscale(v[m], (real)filter_weight(scale, p2));
+                }
+                bfly<PB::R2, true>(v);
+#pragma unroll
+                for (int m = 0; m < PB::R2; m++) tl[(i2 ^ (m & SWM)) * SI2 + (bb * PB::R2 + m) * SI3] = v[m];
+            }
+        }
+        gsync_c<GT, BAR>();
+    }
+    block(std::true_type{});
+    // axis-2 stage 1 inverse: swizzled in, dense out, then the tile goes back through the TMA unit
+    {
+        constexpr int NW = C0 * PA::R2 * L3, NI = (NW + GT - 1) / GT;
+        cplx v[NI][PA::R1];
+#pragma unroll
+        for (int k = 0; k < NI; k++) {
+            const int w = k * GT + gtid;
+            const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+            const int sw = i3 & SWM, hb = (sw >> 2) * 4 * SI2;
+            const cplx* pe = tl + (ja ^ (sw & 3)) * SI2 + i3 * SI3 + hb;
+            const cplx* po = pe - 2 * hb;
+#pragma unroll
+            for (int m = 0; m < PA::R1; m++) v[k][m] = ((m & 1) ? po : pe)[m * PA::R2 * SI2];
+            stage_regs<PA::R1, true, true>(v[k], tw2, ja);
+        }
+        gsync_c<GT, BAR>();
+#pragma unroll
+        for (int k = 0; k < NI; k++) {
+            const int w = k * GT + gtid;
+            const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
+            cplx* p = tl + ja * SI2 + i3 * SI3;
+#pragma unroll
+            for (int m = 0; m < PA::R1; m++) p[m * PA::R2 * SI2] = v[k][m];
+        }
+    }
+}
+
 template <int LG2, int LG3, int LGC, int NT>
 __global__ void __launch_bounds__(NT, 1) k_tm_mid(const __grid_constant__ CUtensorMap tmap, cplx* __restrict__ field, Geom G, FftTables T,
                                                   double scale, Ctl* ctl, const double2* partials, FinArgs fa, int n_tiles) {
@@ -252,122 +388,7 @@ __global__ void __launch_bounds__(NT, 1) k_tm_mid(const __grid_constant__ CUtens
         }
         const double s01 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1];
         mbar_wait(&full, it & 1);
-        // axis-2 stage 1 (points i2 = ja + m R2, twiddles tw2[k ja]): dense in, swizzled out
-        {
-            constexpr int NW = C0 * PA::R2 * L3, NI = (NW + NT - 1) / NT;
-            static_assert(NW % NT == 0, "whole items per thread");
-            cplx v[NI][PA::R1];
-#pragma unroll
-            for (int k = 0; k < NI; k++) {
-                const int w = k * NT + threadIdx.x;
-                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
-                const cplx* p = tl + ja * SI2 + i3 * SI3;
-#pragma unroll
-                for (int m = 0; m < PA::R1; m++) v[k][m] = p[m * PA::R2 * SI2];
-                stage_regs<PA::R1, false, true>(v[k], tw2, ja);
-            }
-            __syncthreads();
-#pragma unroll
-            for (int k = 0; k < NI; k++) {
-                const int w = k * NT + threadIdx.x;
-                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
-                cplx* p = tl + (ja ^ (i3 & SWM)) * SI2 + i3 * SI3;
-#pragma unroll
-                for (int m = 0; m < PA::R1; m++) p[m * PA::R2 * SI2] = v[k][m];
-            }
-            __syncthreads();
-        }
-        // 16-point block: last stage of axis 2 (contiguous sub-blocks of 4) x first stage of axis 3 (points jb + mb R2b)
-        auto block = [&](auto inv_tag) {
-            constexpr bool INV = decltype(inv_tag)::value;
-            constexpr int NW = C0 * PB::R2 * PA::R1;
-#pragma unroll
-            for (int w0 = 0; w0 < NW; w0 += NT) {
-                const int w = w0 + threadIdx.x;
-                if (NW % NT == 0 || w < NW) {
-                    const int jb = (w / C0) % PB::R2, ba = w / (C0 * PB::R2);
-                    const int sw = jb & SWM;
-                    cplx v[4][4];                        // [mb][ma]
-#pragma unroll
-                    for (int mb = 0; mb < 4; mb++)
-#pragma unroll
-                        for (int ma = 0; ma < 4; ma++) v[mb][ma] = tl[((ba * 4 + ma) ^ sw) * SI2 + (jb + mb * PB::R2) * SI3];
-                    if constexpr (!INV) {
-#pragma unroll
-                        for (int mb = 0; mb < 4; mb++) bfly<4, false>(v[mb]);
-                    }
-#pragma unroll
-                    for (int ma = 0; ma < 4; ma++) {
-                        cplx c[4];
-#pragma unroll
-                        for (int mb = 0; mb < 4; mb++) c[mb] = v[mb][ma];
-                        stage_regs<4, INV, true>(c, tw3, jb);
-#pragma unroll
-                        for (int mb = 0; mb < 4; mb++) v[mb][ma] = c[mb];
-                    }
-                    if constexpr (INV) {
-#pragma unroll
-                        for (int mb = 0; mb < 4; mb++) bfly<4, true>(v[mb]);
-                    }
-#pragma unroll
-                    for (int mb = 0; mb < 4; mb++)
-#pragma unroll
-                        for (int ma = 0; ma < 4; ma++) tl[((ba * 4 + ma) ^ sw) * SI2 + (jb + mb * PB::R2) * SI3] = v[mb][ma];
-                }
-            }
-            __syncthreads();
-        };
-        block(std::false_type{});
-        // axis-3 stage 2 forward, S2b filter X~ = (p2max / (V p2)) Delta~ at the stored positions (zero mode -> 0), axis-3
-        // stage 2 inverse, on the same registers                                                   [north_star step 2]
-        {
-            constexpr int NW = C0 * L2 * PB::R1;
-#pragma unroll
-            for (int w0 = 0; w0 < NW; w0 += NT) {
-                const int w = w0 + threadIdx.x;
-                if (NW % NT == 0 || w < NW) {
-                    const int i2 = (w / C0) % L2, bb = w / (C0 * L2);
-                    cplx v[PB::R2];
-#pragma unroll
-                    for (int m = 0; m < PB::R2; m++) v[m] = tl[(i2 ^ (m & SWM)) * SI2 + (bb * PB::R2 + m) * SI3];
-                    bfly<PB::R2, false>(v);
-                    const double s012 = s01 + s2[i2];
-#pragma unroll
-                    for (int m = 0; m < PB::R2; m++) {
-                        const double p2 = s012 + s3[bb * PB::R2 + m];
-                        v[m] = cscale(v[m], (real)filter_weight(scale, p2));
-                    }
-                    bfly<PB::R2, true>(v);
-#pragma unroll
-                    for (int m = 0; m < PB::R2; m++) tl[(i2 ^ (m & SWM)) * SI2 + (bb * PB::R2 + m) * SI3] = v[m];
-                }
-            }
-            __syncthreads();
-        }
-        block(std::true_type{});
-        // axis-2 stage 1 inverse: swizzled in, dense out, then the tile goes back through the TMA unit
-        {
-            constexpr int NW = C0 * PA::R2 * L3, NI = (NW + NT - 1) / NT;
-            cplx v[NI][PA::R1];
-#pragma unroll
-            for (int k = 0; k < NI; k++) {
-                const int w = k * NT + threadIdx.x;
-                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
-                const cplx* p = tl + (ja ^ (i3 & SWM)) * SI2 + i3 * SI3;
-#pragma unroll
-                for (int m = 0; m < PA::R1; m++) v[k][m] = p[m * PA::R2 * SI2];
-                stage_regs<PA::R1, true, true>(v[k], tw2, ja);
-            }
-            __syncthreads();
-#pragma unroll
-            for (int k = 0; k < NI; k++) {
-                const int w = k * NT + threadIdx.x;
-                const int ja = (w / C0) % PA::R2, i3 = w / (C0 * PA::R2);
-                cplx* p = tl + ja * SI2 + i3 * SI3;
-#pragma unroll
-                for (int m = 0; m < PA::R1; m++) p[m * PA::R2 * SI2] = v[k][m];
-            }
-        }
+        mid_tile_stages<LG2, LG3, LGC, NT, 0>(tl, tw2, tw3, s2, s3, s01, scale, (int)threadIdx.x);
         fence_proxy_async();                             // the generic-proxy writes above, before the async proxy reads them
         __syncthreads();
         if (threadIdx.x == 0) {
@@ -382,6 +403,87 @@ __global__ void __launch_bounds__(NT, 1) k_tm_mid(const __grid_constant__ CUtens
 }  // namespace lgf
 
 namespace lgf {
+
+// ---------------------------------------------------------------------------------------------------------------
+// Pass B for 32 x 64 and 64 x 32 tiles as a RING: tiles of HALF the x0 chunk of k_tm_mid (64 KB: two sites x 32 x 64),
+// three buffers, NT = 512 threads = two groups of 256.  (Measured: 74.6 against 106.3 us at 32^3 x 64.  For 64 x 64 the
+// half chunk is ONE site, the rows of the TMA box are 16 bytes, and the ring measured slower than k_tm_mid -- 1065
+// against 999 us at 64^4 -- so that shape keeps the single-buffered kernel.)  As in k_tb_mid, tile j of the CTA's sequence is
+// transformed in place in buffer j mod 3 by group j mod 2 (the stages of mid_tile_stages on the group's named barrier),
+// goes back to the field by a bulk tensor store, and when that store has read the buffer the group's thread 0 starts the
+// copy of tile j + 3 into it.  So the load and the store of a tile overlap the other group's stages instead of standing
+// in front of and behind the tile's own (k_tm_mid: about a quarter of the tile's time).  The CTA takes its tiles in
+// PAIRS of neighbouring x0 chunks (j and j + 1 share their 32- or 64-byte sectors), so the second copy of a pair finds its
+// sectors in L2 and the two partial-sector stores meet there before they go to DRAM.
+template <int LG2, int LG3, int LGC> struct TmaRingGeom {
+    static constexpr int L2 = 1 << LG2, L3 = 1 << LG3, C0 = 1 << LGC;
+    static constexpr int TILE = C0 * L2 * L3;
+    static constexpr unsigned TILE_BYTES = TILE * sizeof(cplx);
+    static constexpr size_t SMEM = (size_t)(3 * TILE + L2 + L3) * sizeof(cplx) + (size_t)(L2 + L3) * 8 + 128;
+};
+
+template <int LG2, int LG3, int LGC, int NT>
+__global__ void __launch_bounds__(NT, 1) k_tr_mid(const __grid_constant__ CUtensorMap tmap, cplx* __restrict__ field, Geom G, FftTables T,
+                                                  double scale, Ctl* ctl, const double2* partials, FinArgs fa, int n_tiles) {
+    static_assert(NT == 512, "two groups of 256 threads");
+    pdl_enter();
+    __shared__ int s_done;
+    __shared__ __align__(8) uint64_t full[3];
+    pass_b_entry<NT>(partials, fa, ctl, &s_done);
+    using TG = TmaRingGeom<LG2, LG3, LGC>;
+    constexpr int L2 = TG::L2, L3 = TG::L3, C0 = TG::C0, TILE = TG::TILE, GT = 256;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* bufs = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u));      // [3][TILE]
+    cplx* tw2 = bufs + 3 * TILE;
+    cplx* tw3 = tw2 + L2;
+    double* s2 = reinterpret_cast<double*>(tw3 + L3);
+    double* s3 = s2 + L2;
+    for (int i = threadIdx.x; i < L2; i += NT) { tw2[i] = T.tw[2][i]; s2[i] = T.s[2][i]; }
+    for (int i = threadIdx.x; i < L3; i += NT) { tw3[i] = T.tw[3][i]; s3[i] = T.s[3][i]; }
+    const int lgChunks = G.lg[0] - LGC;
+    // tile j of this CTA: the (j & 1)-th of the pair blockIdx.x + (j >> 1) gridDim.x
+    const int n_pairs = n_tiles >> 1;
+    const int n_seq = 2 * ((n_pairs - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x);
+    auto tile_of = [&](int j) { return 2 * ((int)blockIdx.x + (j >> 1) * (int)gridDim.x) + (j & 1); };
+    auto issue = [&](int j) {
+        const int tile = tile_of(j), b = j % 3;
+        const int chunk = tile & ((1 << lgChunks) - 1);
+        const int x1 = (tile >> lgChunks) & (G.L[1] - 1);
+        const int comp = tile >> (lgChunks + G.lg[1]);
+        mbar_expect_tx(&full[b], TG::TILE_BYTES);
+        tma_load_5d(bufs + b * TILE, &tmap, &full[b], chunk << (LGC + 1), x1, 0, 0, comp);
+    };
+    if (threadIdx.x == 0) {
+        mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_init(&full[2], 1);
+        mbar_init_fence();
+        if (!s_done)
+            for (int j = 0; j < 3 && j < n_seq; j++) issue(j);
+    }
+    __syncthreads();
+    if (s_done) return;                                  // one reading per CTA, behind a barrier (pass_b_entry)
+    const int grp = threadIdx.x / GT, gtid = threadIdx.x % GT;
+    const int i0 = gtid % C0;
+#pragma unroll 1
+    for (int j = grp; j < n_seq; j += 2) {
+        const int tile = tile_of(j), b = j % 3;
+        const int chunk = tile & ((1 << lgChunks) - 1);
+        const int x1 = (tile >> lgChunks) & (G.L[1] - 1);
+        const int comp = tile >> (lgChunks + G.lg[1]);
+        cplx* tbuf = bufs + b * TILE;
+        const double s01 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1];
+        mbar_wait(&full[b], (j / 3) & 1);
+        if (grp == 0) mid_tile_stages<LG2, LG3, LGC, GT, 1>(tbuf + i0, tw2, tw3, s2, s3, s01, scale, gtid);
+        else mid_tile_stages<LG2, LG3, LGC, GT, 2>(tbuf + i0, tw2, tw3, s2, s3, s01, scale, gtid);
+        fence_proxy_async();                             // the generic-proxy writes above, before the async proxy reads them
+        if (grp == 0) gsync_c<GT, 1>(); else gsync_c<GT, 2>();
+        if (gtid == 0) {
+            tma_store_5d(&tmap, tbuf, chunk << (LGC + 1), x1, 0, 0, comp);
+            tma_store_wait_read();                       // this group's only outstanding store has read the buffer ...
+            if (j + 3 < n_seq) issue(j + 3);             // ... which takes the next tile of its chain
+        }
+    }
+    if (gtid == 0) tma_store_wait_all();
+}
 
 // ---------------------------------------------------------------------------------------------------------------
 // Pass A (S1 + forward FFT over axes 0,1) with the links staged by the TMA unit.

@@ -92,13 +92,13 @@ namespace {
 enum KernelSlot {
     K_DELTA = 0, K_FFT01_FWD, K_FFT01_DELTA_FWD, K_FINALIZE, K_FFT23_MID, K_FFT01_INV, K_FFT01_INV_G, K_UPDATE_G,
     K_LAYOUT_IN, K_LAYOUT_OUT, K_PLAQUETTE, K_MISC, K_FA_DELTA_FWD, K_FA_MID, K_FA_INV, K_FA_INV_G,
-    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_TB_MID, K_TM_MID, K_TA_DELTA_FWD, K_NSLOTS
+    K_UPDATE_QUAD, K_FA_FWD1, K_FA_INV1, K_FR_MID, K_CL_DELTA_FWD, K_TB_MID, K_TM_MID, K_TA_DELTA_FWD, K_TR_MID, K_NSLOTS
 };
 static_assert(K_NSLOTS <= LGF_MAX_KERNELS, "kernel slot table");
 const char* const kKernelNames[LGF_MAX_KERNELS] = {
     "k_delta", "k_fft01_fwd", "k_fft01_delta_fwd", "k_finalize", "k_fft23_mid", "k_fft01_inv", "k_fft01_inv_g", "k_update_g",
     "k_layout_in", "k_layout_out", "k_plaquette", "misc", "k_fa_delta_fwd", "k_fa_mid", "k_fa_inv", "k_fa_inv_g",
-    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_tb_mid", "k_tm_mid", "k_ta_delta_fwd"};
+    "k_update_quad", "k_fa_fwd1", "k_fa_inv1", "k_fr_mid", "k_cl_delta_fwd", "k_tb_mid", "k_tm_mid", "k_ta_delta_fwd", "k_tr_mid"};
 
 constexpr int HIST_CAP = 1 << 16;
 // mixed precision: the fp32 phase ends when theta has not halved within this many iterations (a rough thermalised
@@ -208,8 +208,8 @@ struct lgf_ctx {
     // options (include/lgf.h lgf_option)
     int opt_store_g, opt_graph, opt_batch, opt_fast, opt_pdl, opt_accel, opt_tma;
     // pass B on TMA-staged tiles (fft_tma.cuh): the field as a 5-D tensor map, whether it could be built
-    CUtensorMap tm_field;
-    bool tma_b;
+    CUtensorMap tm_field, tm_field_half;
+    bool tma_b, ring_b;
     LinkMaps tm_links;      // pass A with the links staged by the TMA unit (k_ta_delta_fwd)
     bool tma_a;
     int sms;                // SMs of the device
@@ -463,11 +463,25 @@ void launch_tm_mid(lgf_ctx* c) {
 #undef X
 }
 
+// ... as a ring of half-chunk tiles (fft_tma.cuh k_tr_mid)
+void launch_tr_mid(lgf_ctx* c) {
+    LaunchScope ls(c, K_TR_MID);
+    const int n_tiles = 4 * c->G.L[1] * (c->G.L[0] >> (c->fb_lgC - 1));
+    const int n_pairs = n_tiles / 2;
+    const unsigned grid = (unsigned)(n_pairs < c->sms ? n_pairs : c->sms);
+    const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
+    const FinArgs fa = pending_fin(c);
+#define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
+        launch_k(c, k_tr_mid<A, B, fast_mid_lgC(A, B) - 1, TM_NT>, grid, TM_NT, TmaRingGeom<A, B, fast_mid_lgC(A, B) - 1>::SMEM, c->tm_field_half, c->field, c->G, c->T, scale, c->ctl, c->partials, fa, n_tiles);
+    LGF_BIG_PAIRS(X)
+#undef X
+}
+
 // The field as a 5-D tensor of reals (2 L0, L1, L2, L3, 4 components) with the pass-B tile as its box.  The encoder is
 // a driver entry point fetched at run time, so the library does not link against libcuda.
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-bool make_field_tensor_map(lgf_ctx* c, int lgC) {
+bool make_field_tensor_map(lgf_ctx* c, int lgC, CUtensorMap* out) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn || qres != cudaDriverEntryPointSuccess) {
@@ -480,7 +494,7 @@ bool make_field_tensor_map(lgf_ctx* c, int lgC) {
     const cuuint64_t strides[4] = {esz * G.L[0], esz * G.L[0] * G.L[1], esz * G.L[0] * G.L[1] * G.L[2], esz * (cuuint64_t)G.V};
     const cuuint32_t box[5] = {(cuuint32_t)(2 << lgC), 1, (cuuint32_t)G.L[2], (cuuint32_t)G.L[3], 1};
     const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-    const CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(&c->tm_field, sizeof(real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+    const CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(out, sizeof(real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
         5, c->field, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS;
@@ -539,7 +553,7 @@ lgf_status setup_fast(lgf_ctx* c) {
 #undef X
     }
     c->tma_b = false;
-    if (c->fast_b && make_field_tensor_map(c, c->fb_lgC)) {
+    if (c->fast_b && make_field_tensor_map(c, c->fb_lgC, &c->tm_field)) {
         c->tma_b = true;
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) \
             c->tma_b = set_smem(k_tb_mid<A, B, fast_mid_lgC(A, B), LGF_TB_NT>, TmaMidGeom<A, B, fast_mid_lgC(A, B)>::SMEM) == cudaSuccess;
@@ -550,6 +564,17 @@ lgf_status setup_fast(lgf_ctx* c) {
         LGF_BIG_PAIRS(X)
 #undef X
         if (!c->tma_b) cudaGetLastError();
+        // the ring form of the 64-extent pass (k_tr_mid): tiles of half the chunk
+        c->ring_b = false;
+        // (from 2-site chunks on: with 1-site chunks -- 64 x 64 -- the TMA box rows are 16 bytes and the ring measured
+        // slower than k_tm_mid, 1065 against 999 us at 64^4)
+        if (c->tma_b && big_pair(G.lg[2], G.lg[3]) && c->fb_lgC >= 2 && make_field_tensor_map(c, c->fb_lgC - 1, &c->tm_field_half)) {
+#define X(A, B) if (G.lg[2] == A && G.lg[3] == B) \
+                c->ring_b = set_smem(k_tr_mid<A, B, fast_mid_lgC(A, B) - 1, TM_NT>, TmaRingGeom<A, B, fast_mid_lgC(A, B) - 1>::SMEM) == cudaSuccess;
+            LGF_BIG_PAIRS(X)
+#undef X
+            if (!c->ring_b) cudaGetLastError();
+        }
     }
     c->tma_a = false;
     if (c->fast_a && make_link_tensor_maps(c)) {
@@ -733,7 +758,7 @@ template <int NC> void enqueue_head(lgf_ctx* c) {
     launch_finalize(c, np);
 }
 void launch_mid(lgf_ctx* c) {
-    if (use_tma_b(c)) launch_tb_mid(c); else if (use_tma_big(c)) launch_tm_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
+    if (use_tma_b(c)) launch_tb_mid(c); else if (use_tma_big(c) && c->ring_b) launch_tr_mid(c); else if (use_tma_big(c)) launch_tm_mid(c); else if (use_line_b(c)) launch_fr_mid(c); else if (use_fast_b(c)) launch_fa_mid(c); else launch_fft23(c);
 }
 void launch_inv_x(lgf_ctx* c) {
     if (use_fast_c(c)) launch_fa_inv(c); else if (use_big_p(c)) launch_fa_inv1(c);
