@@ -318,7 +318,7 @@ template <typename K> cudaError_t set_smem(K kern, size_t bytes) {
 // ---- compile-time-sized FFT passes (fft_fast.cuh): the lattices they cover, and their launchers ----------------
 constexpr int FAD_NT = 256;           // threads per CTA of pass A (k_fa_delta_fwd)
 constexpr int FC_NT = 256;            // threads per CTA of pass C (k_fa_inv) and of the one-component plane passes
-constexpr int CL_NT = 256;            // threads per CTA of the CTA-pair pass A (k_cl_delta_fwd)
+constexpr int CL_NT = 512;            // threads per CTA of the CTA-pair pass A (k_cl_delta_fwd)
 constexpr int FB_NT = 256;            // threads per CTA of the stage-wise pass B when its tile is below 100 KB
 // (lg of the fast axis, lg of the slow axis) pairs instantiated for each pass: extents 16 and 32 ...
 #define LGF_FAST_PAIRS(X) X(4, 4) X(4, 5) X(5, 4) X(5, 5)
@@ -326,6 +326,8 @@ constexpr int FB_NT = 256;            // threads per CTA of the stage-wise pass 
 // one SM; 64 x 64 planes run S1 on CTA pairs, the others keep S1 a separate kernel), the (x2,x3) pass takes a shorter
 // x0 chunk
 #define LGF_BIG_PAIRS(X) X(5, 6) X(6, 5) X(6, 6)
+// ... of which the 64-extent pass B also runs as a ring of half-chunk tiles (k_tr_mid)
+#define LGF_RING_PAIRS(X) X(5, 6) X(6, 5)
 // x0 chunk of pass B (2^lgC sites): tile = 2^(lga+lgb+lgC) * 16 B
 constexpr int fast_mid_lgC(int lga, int lgb) { return (lga + lgb <= 9) ? 3 : ((lga + lgb == 10) ? 2 : ((lga + lgb == 11) ? 2 : 1)); }
 // threads per CTA of the stage-wise pass B: one 512-thread CTA per SM when the tile is above 100 KB, else 2 x 256
@@ -473,7 +475,7 @@ void launch_tr_mid(lgf_ctx* c) {
     const FinArgs fa = pending_fin(c);
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
         launch_k(c, k_tr_mid<A, B, fast_mid_lgC(A, B) - 1, TM_NT>, grid, TM_NT, TmaRingGeom<A, B, fast_mid_lgC(A, B) - 1>::SMEM, c->tm_field_half, c->field, c->G, c->T, scale, c->ctl, c->partials, fa, n_tiles);
-    LGF_BIG_PAIRS(X)
+    LGF_RING_PAIRS(X)
 #undef X
 }
 
@@ -571,7 +573,7 @@ lgf_status setup_fast(lgf_ctx* c) {
         if (c->tma_b && big_pair(G.lg[2], G.lg[3]) && c->fb_lgC >= 2 && make_field_tensor_map(c, c->fb_lgC - 1, &c->tm_field_half)) {
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) \
                 c->ring_b = set_smem(k_tr_mid<A, B, fast_mid_lgC(A, B) - 1, TM_NT>, TmaRingGeom<A, B, fast_mid_lgC(A, B) - 1>::SMEM) == cudaSuccess;
-            LGF_BIG_PAIRS(X)
+            LGF_RING_PAIRS(X)
 #undef X
             if (!c->ring_b) cudaGetLastError();
         }
