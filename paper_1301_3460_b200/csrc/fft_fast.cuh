@@ -337,8 +337,10 @@ __global__ void __launch_bounds__(NT, LGF_FA_MINB_DELTA) k_fa_delta_fwd(const cp
     const Grp g{(int)threadIdx.x, 0};
     for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
     for (int i = threadIdx.x; i < L1; i += NT) tw1[i] = T.tw[1][i];
-    pass_a_delta<LG0, LG1, NC, NT>(links, G, blockIdx.x, tile, red, partials, g);
-    plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)blockIdx.x << (LG0 + LG1), g);
+    // planes from the last one down: the link update before this kernel walks upwards and leaves its last planes in L2
+    const int plane = (int)gridDim.x - 1 - (int)blockIdx.x;
+    pass_a_delta<LG0, LG1, NC, NT>(links, G, plane, tile, red, partials, g);
+    plane_forward_store<LG0, LG1, NT>(tile, tw0, tw1, field, G.V, (long long)plane << (LG0 + LG1), g);
 }
 
 // Pass A for 64 x 64 planes on a CTA PAIR (thread-block cluster of 2, distributed shared memory): the four component

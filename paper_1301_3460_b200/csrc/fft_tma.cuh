@@ -502,6 +502,9 @@ __global__ void __launch_bounds__(NT, 1) k_tr_mid(const __grid_constant__ CUtens
 // thread 0 starts the copies of stage s + 2 -- of the same plane or the CTA's next one -- and arms the buffer's mbarrier.
 // So two stages (150 KB at 32 x 32, fp64) are always in flight or being consumed, also while all warps transform the
 // finished tile, and no warp ever waits on a global load.
+// The planes are walked from the LAST one down: the link update before this kernel walks the lattice upwards, so the
+// last ~100 MB of links it wrote are still in L2 and this kernel starts on exactly those (measured at 32^4: 92.9 against
+// 97.3 us; walking the update downwards instead gives pass A the same hits but costs the update its own on X).
 struct LinkMaps { CUtensorMap own, nb, row; };
 
 // sites per stage: 128 (a thread = one site, each group owns one buffer; default) or 64 (two threads per site -- one takes
@@ -571,7 +574,7 @@ __global__ void __launch_bounds__(NT, 1) k_ta_delta_fwd(const __grid_constant__ 
     // Stage t of this CTA: plane blockIdx.x + (t / NST) gridDim.x, sites [(t % NST) SS, ...).  Group g = t & 1 takes it as
     // its k-th stage, k = t >> 1, in its buffer k mod NBG.
     auto issue = [&](int t) {
-        const int plane = blockIdx.x + (t / NST) * gridDim.x, s = t % NST, b = (t & 1) * NBG + ((t >> 1) % NBG);
+        const int plane = n_planes - 1 - ((int)blockIdx.x + (t / NST) * (int)gridDim.x), s = t % NST, b = (t & 1) * NBG + ((t >> 1) % NBG);
         const int x2 = plane & (G.L[2] - 1), x3 = plane >> G.lg[2];
         const int pl2 = ((x2 + G.L[2] - 1) & (G.L[2] - 1)) + (x3 << G.lg[2]);
         const int pl3 = x2 + (((x3 + G.L[3] - 1) & (G.L[3] - 1)) << G.lg[2]);
@@ -602,7 +605,7 @@ __global__ void __launch_bounds__(NT, 1) k_ta_delta_fwd(const __grid_constant__ 
     const int jm0 = (j & ~(L0 - 1)) | ((jx + L0 - 1) & (L0 - 1));      // x - 0 (periodic inside the row)
 #pragma unroll 1
     for (int q = 0; q < n_seq; q++) {
-        const int plane = blockIdx.x + q * gridDim.x;
+        const int plane = n_planes - 1 - ((int)blockIdx.x + q * (int)gridDim.x);
         double th = 0, fs = 0;
 #pragma unroll 1
         for (int s = grp; s < NST; s += 2) {

@@ -441,14 +441,20 @@ void launch_tb_mid(lgf_ctx* c) {
 }
 
 // pass A with TMA-staged links (fft_tma.cuh k_ta_delta_fwd): 16/32 extents, one persistent CTA per SM
-template <int NC> void launch_ta_delta_fwd(lgf_ctx* c) {
+// (instantiated for fp64 two-row storage only: two stages of 18-real links do not fit one SM, and the fp32 build keeps
+// the plain-load pass A, which measured faster there)
+void launch_ta_delta_fwd(lgf_ctx* c) {
+#ifndef LGF_F32
     LaunchScope ls(c, K_TA_DELTA_FWD);
     const int n_planes = c->G.L[2] * c->G.L[3];
     const unsigned grid = (unsigned)(n_planes < c->sms ? n_planes : c->sms);
 #define X(A, B) if (c->G.lg[0] == A && c->G.lg[1] == B) \
-        launch_k(c, k_ta_delta_fwd<A, B, NC, 256>, grid, 256, TmaPlaneGeom<A, B, NC>::SMEM, c->tm_links, c->field, c->partials, c->G, c->T, c->ctl, n_planes);
+        launch_k(c, k_ta_delta_fwd<A, B, 6, 256>, grid, 256, TmaPlaneGeom<A, B, 6>::SMEM, c->tm_links, c->field, c->partials, c->G, c->T, c->ctl, n_planes);
     LGF_FAST_PAIRS(X)
 #undef X
+#else
+    (void)c;
+#endif
 }
 
 // pass B on TMA-staged tiles, 64 extents: the tile goes in and out through the TMA unit (fft_tma.cuh k_tm_mid)
@@ -579,14 +585,14 @@ lgf_status setup_fast(lgf_ctx* c) {
         }
     }
     c->tma_a = false;
-    if (c->fast_a && make_link_tensor_maps(c)) {
-#define X(A, B) if (G.lg[0] == A && G.lg[1] == B) \
-            c->tma_a = (c->NC == 6) ? set_smem(k_ta_delta_fwd<A, B, 6, 256>, TmaPlaneGeom<A, B, 6>::SMEM) == cudaSuccess \
-                                    : set_smem(k_ta_delta_fwd<A, B, 9, 256>, TmaPlaneGeom<A, B, 9>::SMEM) == cudaSuccess;
+#ifndef LGF_F32
+    if (c->fast_a && c->NC == 6 && make_link_tensor_maps(c)) {       // 18-real links: two stages do not fit one SM
+#define X(A, B) if (G.lg[0] == A && G.lg[1] == B) c->tma_a = set_smem(k_ta_delta_fwd<A, B, 6, 256>, TmaPlaneGeom<A, B, 6>::SMEM) == cudaSuccess;
         LGF_FAST_PAIRS(X)
 #undef X
-        if (!c->tma_a) cudaGetLastError();               // e.g. 18-real links at 32 x 32: two stages do not fit one SM
+        if (!c->tma_a) cudaGetLastError();
     }
+#endif
     c->cl_ok = false;
     if (c->big_p && G.lg[0] == 6 && G.lg[1] == 6) {
         c->smem_cl = smem_fast_plane(6, 6, 2);
@@ -707,12 +713,15 @@ template <int NC> void launch_update_quad(lgf_ctx* c, double half_alpha) {
     LaunchScope ls(c, K_UPDATE_QUAD);
     cplx* const no_acc = nullptr;
     const bool banded = update_banded(c);
-    if (c->acc_g) {
+#ifdef LGF_F32
+    if (c->acc_g) {                                      // the fp32 phase of LGF_MIXED accumulates the transformation
         if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32, 1>, (unsigned)(c->G.V / 32), 128, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
         else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64, 1>, (unsigned)(c->G.V / 64), 256, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
         else launch_k(c, k_update_quad<NC, 128, 1>, (unsigned)(c->G.V / 128), 512, 0, c->links, c->field, c->G, half_alpha, c->ctl, c->gbuf);
+        return;
     }
-    else if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32>, (unsigned)(c->G.V / 32), 128, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
+#endif
+    if (c->G.L[0] <= 32) launch_k(c, k_update_quad<NC, 32>, (unsigned)(c->G.V / 32), 128, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
     else if (c->G.L[0] == 64 && banded) launch_k(c, k_update_quad<NC, 64, 0, 3>, (unsigned)(c->G.V / 64), 256, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
     else if (c->G.L[0] == 64) launch_k(c, k_update_quad<NC, 64>, (unsigned)(c->G.V / 64), 256, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
     else launch_k(c, k_update_quad<NC, 128>, (unsigned)(c->G.V / 128), 512, 0, c->links, c->field, c->G, half_alpha, c->ctl, no_acc);
@@ -733,8 +742,9 @@ bool use_fast_b(const lgf_ctx* c) { return c->opt_fast && c->fast_b; }
 // pass A with TMA-staged links (Landau gauge; the Coulomb S1 keeps the plain-load kernel)
 // -- from two planes per SM on: the persistent grid has one CTA per SM, and below that its tail costs more than the staging
 // gains (16^4, 256 planes on 148 SMs: 12.7 against 10.7 us)
+// (fp64 only: in the fp32 build the plain-load pass A with its next-site L2 prefetch measured faster, 61.8 against 66.0 us)
 bool use_tma_a(const lgf_ctx* c) {
-    return c->opt_fast && c->fast_a && c->opt_tma && c->tma_a && c->G.nd == 4 && c->G.L[2] * c->G.L[3] >= 2 * c->sms;
+    return sizeof(real) == 8 && c->NC == 6 && c->opt_fast && c->fast_a && c->opt_tma && c->tma_a && c->G.nd == 4 && c->G.L[2] * c->G.L[3] >= 2 * c->sms;
 }
 bool use_fast_c(const lgf_ctx* c) { return c->opt_fast && c->fast_c; }
 bool use_big_p(const lgf_ctx* c) { return c->opt_fast && c->big_p; }
@@ -750,7 +760,7 @@ bool use_fin_b(const lgf_ctx* c) { return c->opt_accel && use_fast_b(c); }
 // S1 (+ pass A) and, unless pass B does it, the reduction.
 template <int NC> void enqueue_head(lgf_ctx* c) {
     int np;
-    if (use_tma_a(c)) { launch_ta_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
+    if (use_tma_a(c)) { launch_ta_delta_fwd(c); np = c->G.L[2] * c->G.L[3]; }
     else if (use_fast_a(c)) { launch_fa_delta_fwd<NC>(c); np = c->G.L[2] * c->G.L[3]; }
     else if (use_cluster_a(c)) { launch_cl_delta_fwd<NC>(c); np = 2 * c->G.L[2] * c->G.L[3]; }
     else if (use_big_p(c)) { launch_delta<NC>(c); np = (int)(c->G.V / 128); launch_fa_fwd1(c); }
