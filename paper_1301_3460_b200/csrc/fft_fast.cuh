@@ -368,7 +368,7 @@ k_cl_delta_fwd(const cplx* __restrict__ links, cplx* __restrict__ field, double2
     // The planes are walked in x2 bands of 16: x2 fastest inside a band, then x3, then the bands.  The backward neighbours
     // U_2(x-2) and U_3(x-3) live in the planes (x2-1, x3) and (x2, x3-1); in plain order the latter was read 64 planes =
     // 100 MB of links earlier and has left L2 (ncu at 64^4: 7.90 GB of DRAM reads against 6.44 GB of links), here 16.
-    int plane = blockIdx.x >> 1;
+    int plane = (int)(gridDim.x >> 1) - 1 - (int)(blockIdx.x >> 1);      // from the last plane down (see k_fa_delta_fwd)
     if (G.L[2] >= 32) {
         const int x2l = plane & 15, x3 = (plane >> 4) & (G.L[3] - 1), bnd = plane >> (4 + G.lg[3]);
         plane = (bnd * 16 + x2l) + (x3 << G.lg[2]);
