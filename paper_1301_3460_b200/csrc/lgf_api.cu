@@ -704,7 +704,6 @@ void launch_finalize(lgf_ctx* c, int n_partials) {
 // links + X outgrows the L2 share
 bool update_banded(const lgf_ctx* c) {
     const Geom& G = c->G;
-    if (const char* e = getenv("LGF_UPD_BAND")) return atoi(e) != 0;
     if (G.L[0] < 64 || G.L[2] < 16) return false;
     const double slice_mb = (double)G.L[0] * G.L[1] * G.L[2] * (2.0 * 4 * c->NC + 4) * sizeof(cplx) / 1e6;
     return slice_mb > 48.0;
