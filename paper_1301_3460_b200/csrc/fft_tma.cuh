@@ -1,14 +1,18 @@
-// fft_tma.cuh -- pass B (axes 2,3: forward, p2max/p2 filter, inverse) on tiles staged by the Tensor Memory Accelerator.
+// fft_tma.cuh -- the FFT passes fed by the Tensor Memory Accelerator (cp.async.bulk.tensor + mbarrier), persistent, one CTA
+// per SM:
+//   k_tb_mid        pass B (axes 2,3: forward, p2max/p2 filter, inverse) for 16/32 extents: ring of three tiles, two thread
+//                   groups, whole lines in registers
+//   k_tm_mid        pass B for 64 x 64 tiles: the 128 KB tile in and out through the TMA unit, radix-16 stages
+//   k_tr_mid        pass B for 32 x 64 / 64 x 32 tiles: ring of three 64 KB tiles, two thread groups, the same stages
+//   k_ta_delta_fwd  pass A (S1 + forward FFT over axes 0,1) for 16/32-extent planes: the links staged 128 sites at a time
 //
-// The register-line pass B of fft_fast.cuh (k_fr_mid) is bound by latency, not by DRAM, the FP64 pipe or shared memory
-// (ncu, profiles/r01_ncu_full_summary.txt: DRAM 21 %, FP64 36 %, issue active 26 % at 7 warps per SM): a CTA loads its
-// tile with 32 dependent-latency global loads per thread, transforms it, stores it, and nothing overlaps the three.
-// Here one persistent CTA per SM walks over its tiles and the next tiles are always in flight: one elected thread issues
-// a 5-D cp.async.bulk.tensor (box = 2^LGC x0 sites x all of x2 x all of x3 of one component and one x1) into a free tile
-// buffer and arms an mbarrier with the byte count; the copy costs neither registers nor issue slots and completes on
-// the barrier while the warps transform other tiles.  The three phases are those of k_fr_mid, in place in the buffer
-// the TMA unit filled; phase 3 stores straight from registers (plain stores retire asynchronously).  Same arithmetic,
-// same stored order, same results as k_fr_mid.
+// Why: the plain-load passes of fft_fast.cuh are bound by latency, not by DRAM, the FP64 pipe or shared memory (ncu,
+// profiles/r01_ncu_full_summary.txt: pass B DRAM 21 %, FP64 36 %, issue active 26 % at 7 warps per SM; pass A
+// long_scoreboard 9.6 cycles per issue): a CTA loads its tile with dependent-latency global loads, transforms it, stores
+// it, and nothing overlaps the three.  Here one elected thread issues a bulk tensor copy into a free shared-memory buffer
+// and arms an mbarrier with the byte count; the copy costs neither registers nor issue slots and completes on the
+// barrier while the warps work on other buffers.  Same arithmetic, same stored order, same results as the plain-load
+// kernels (LGF_OPT_TMA = 0), against which every one of these is parity-tested.
 #pragma once
 #include <cuda.h>        // CUtensorMap (type only: the encoder is fetched through cudaGetDriverEntryPoint, lgf_api.cu)
 #include <cstdint>

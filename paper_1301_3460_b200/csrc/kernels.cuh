@@ -17,6 +17,8 @@
 //   k_update_quad  S3+S4: rebuild g(x+mu) from X, one thread per link, rotate the link in place (default)
 //   k_update_g     S3+S4 with g read from gbuf (LGF_OPT_STORE_G)
 //   k_layout_in/out, k_plaquette, k_unpack_field, k_copy: boundary helpers
+// The compile-time-sized passes live in fft_fast.cuh, their TMA-fed persistent forms (the default path) in fft_tma.cuh,
+// the kernels of the slab-decomposed context in slab.cuh.
 #pragma once
 #include "su3.cuh"
 #include "fft_tile.cuh"
