@@ -458,7 +458,10 @@ void launch_ta_delta_fwd(lgf_ctx* c) {
 }
 
 // pass B on TMA-staged tiles, 64 extents: the tile goes in and out through the TMA unit (fft_tma.cuh k_tm_mid)
-constexpr int TM_NT = 512;
+constexpr int TM_NT = 512;             // the ring (k_tr_mid): two groups of 256
+// the single-buffered 64 x 64 pass: 256 threads with two items per thread and stage (961 against 997 us at 64^4 for 512
+// threads with one: the second item's shared-memory loads overlap the first one's butterflies)
+constexpr int TM1_NT = 256;
 void launch_tm_mid(lgf_ctx* c) {
     LaunchScope ls(c, K_TM_MID);
     const int n_tiles = 4 * c->G.L[1] * (c->G.L[0] >> c->fb_lgC);
@@ -466,7 +469,7 @@ void launch_tm_mid(lgf_ctx* c) {
     const double scale = 4.0 * (double)c->G.nd / (double)c->G.V;      // p2max / V
     const FinArgs fa = pending_fin(c);
 #define X(A, B) if (c->G.lg[2] == A && c->G.lg[3] == B) \
-        launch_k(c, k_tm_mid<A, B, fast_mid_lgC(A, B), TM_NT>, grid, TM_NT, TmaBigGeom<A, B, fast_mid_lgC(A, B)>::SMEM, c->tm_field, c->field, c->G, c->T, scale, c->ctl, c->partials, fa, n_tiles);
+        launch_k(c, k_tm_mid<A, B, fast_mid_lgC(A, B), TM1_NT>, grid, TM1_NT, TmaBigGeom<A, B, fast_mid_lgC(A, B)>::SMEM, c->tm_field, c->field, c->G, c->T, scale, c->ctl, c->partials, fa, n_tiles);
     LGF_BIG_PAIRS(X)
 #undef X
 }
@@ -568,7 +571,7 @@ lgf_status setup_fast(lgf_ctx* c) {
         LGF_FAST_PAIRS(X)
 #undef X
 #define X(A, B) if (G.lg[2] == A && G.lg[3] == B) \
-            c->tma_b = set_smem(k_tm_mid<A, B, fast_mid_lgC(A, B), TM_NT>, TmaBigGeom<A, B, fast_mid_lgC(A, B)>::SMEM) == cudaSuccess;
+            c->tma_b = set_smem(k_tm_mid<A, B, fast_mid_lgC(A, B), TM1_NT>, TmaBigGeom<A, B, fast_mid_lgC(A, B)>::SMEM) == cudaSuccess;
         LGF_BIG_PAIRS(X)
 #undef X
         if (!c->tma_b) cudaGetLastError();
