@@ -97,6 +97,8 @@ STAGE_CASES = [
     ((64, 64, 4, 4), 12), ((4, 4, 64, 64), 18), ((32, 64, 4, 8), 12), ((64, 32, 8, 4), 18), ((8, 4, 32, 64), 12), ((4, 8, 64, 32), 12),
     ((8, 8, 16, 32), 12), ((4, 8, 16, 32), 18), ((32, 4, 8, 4), 12), ((4, 4, 4, 4), 12), ((16, 32, 4, 8), 18),
     ((32, 16, 16, 32), 12), ((16, 32, 32, 16), 18), ((32, 32, 16, 16), 12), ((16, 16, 32, 32), 18), ((32, 32, 32, 32), 12),
+    # two-row storage with at least two (x2,x3) planes per SM: the TMA-staged pass A on 16 x 32 and 16 x 16 planes
+    ((16, 32, 32, 16), 12), ((16, 16, 32, 16), 12),
 ]
 
 
