@@ -451,6 +451,10 @@ def run_ours(args):
             stream_gbs = {"read": lgf.stream_peak_gbs(V, False, 10), "read_write_in_place": lgf.stream_peak_gbs(V, True, 10)}
         except Exception:
             copy_gbs, stream_gbs = None, None
+        try:
+            fp64_tflops = lgf.fp64_peak_tflops(5)
+        except Exception:
+            fp64_tflops = None
         it_s_1 = value / world
         # ---- time to theta < 1e-15 (lgf_fix, links resident, all syncs included)
         tol = 1e-10 if fp32 else THETA_TOL                           # fp32 bottoms out near theta = 1e-14
@@ -532,7 +536,8 @@ def run_ours(args):
                          "traffic_source": f"{TRAFFIC_CSV} (ncu --set full, one launch, cold caches; NOT measured in this run: captured at commit {traffic_commit})",
                          "peak_source": peak_src,
                          "bytes_per_launch": kernels[dom]["bytes_per_launch"], "avg_us": kernels[dom]["avg_us"],
-                         "copy_kernel_gbs": copy_gbs, "stream_yardstick_gbs": stream_gbs},
+                         "copy_kernel_gbs": copy_gbs, "stream_yardstick_gbs": stream_gbs,
+                         "fp64_fma_tflops": fp64_tflops},
             "iteration": iteration_block(iter_bytes, V, it_s_1, peak),
             "kernels": kernels,
             "time_to_theta": ttt,

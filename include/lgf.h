@@ -212,6 +212,11 @@ lgf_status lgf_get_history_sharded(lgf_slab_ctx *ctx, double *hist, int capacity
 lgf_status lgf_sharded_traffic(lgf_slab_ctx *ctx, long long out[5]);
 const char *lgf_last_error_sharded(lgf_slab_ctx *ctx);
 
+/* Third yardstick: the FP64 FMA rate of the device (8 independent chains of dependent fused multiply-adds per thread, 64
+ * warps per SM, no memory traffic), in TFLOP/s, averaged over `reps` launches on cuda_stream.  The arithmetic roof of the
+ * FFT passes: the path is HBM-bound, but pass B is within a factor of two of this one as well. */
+lgf_status lgf_fp64_peak(int reps, void *cuda_stream, double *tflops);
+
 const char *lgf_status_string(lgf_status s);
 const char *lgf_last_error(lgf_ctx *ctx); /* detail of the last LGF_ERR_CUDA (static or ctx-owned string) */
 

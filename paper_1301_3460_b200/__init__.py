@@ -16,7 +16,7 @@ import os
 import numpy as np
 
 __all__ = [
-    "LgfError", "lib", "library_path", "GaugeFixer", "ShardedGaugeFixer", "copy_peak_gbs", "stream_peak_gbs",
+    "LgfError", "lib", "library_path", "GaugeFixer", "ShardedGaugeFixer", "copy_peak_gbs", "stream_peak_gbs", "fp64_peak_tflops",
     "LGF_OK", "LGF_NOT_CONVERGED", "LGF_FP64", "LGF_FP32", "LGF_MIXED", "LGF_STORE_12", "LGF_STORE_18",
     "LGF_FIELD_DELTA", "LGF_FIELD_X", "LGF_FIELD_G",
     "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_PDL", "LGF_OPT_FAST_FFT", "LGF_OPT_FOURIER_ACCEL",
@@ -44,7 +44,7 @@ EXPORTS = [
     "lgf_workspace_bytes", "lgf_create", "lgf_create_ex", "lgf_destroy", "lgf_load_links", "lgf_load_links_device",
     "lgf_get_links", "lgf_get_links_device", "lgf_load_links_12", "lgf_get_links_12", "lgf_iterate", "lgf_fix", "lgf_scan_alpha", "lgf_measure", "lgf_get_history",
     "lgf_get_field", "lgf_set_option", "lgf_get_option", "lgf_set_profiling", "lgf_get_profile", "lgf_kernel_name",
-    "lgf_launch_count", "lgf_copy_peak", "lgf_stream_peak", "lgf_status_string", "lgf_last_error",
+    "lgf_launch_count", "lgf_copy_peak", "lgf_stream_peak", "lgf_fp64_peak", "lgf_status_string", "lgf_last_error",
     "lgf_create_sharded", "lgf_destroy_sharded", "lgf_sharded_ranks", "lgf_load_links_sharded", "lgf_get_links_sharded",
     "lgf_iterate_sharded", "lgf_fix_sharded", "lgf_get_history_sharded", "lgf_sharded_traffic", "lgf_last_error_sharded",
 ]
@@ -118,6 +118,7 @@ def lib():
     L.lgf_launch_count.argtypes = [P]
     L.lgf_copy_peak.argtypes = [P, P, C.c_size_t, C.c_int, P, D]
     L.lgf_stream_peak.argtypes = [P, C.c_size_t, C.c_int, C.c_int, P, D]
+    L.lgf_fp64_peak.argtypes = [C.c_int, P, D]
     L.lgf_status_string.restype = C.c_char_p
     L.lgf_status_string.argtypes = [C.c_int]
     L.lgf_last_error.restype = C.c_char_p
@@ -405,6 +406,16 @@ def copy_peak_gbs(nbytes: int = 1 << 30, reps: int = 10) -> float:
     if st != LGF_OK:
         raise LgfError(st, "lgf_copy_peak")
     return 2.0 * nbytes / ms.value / 1e6
+
+
+def fp64_peak_tflops(reps: int = 5) -> float:
+    """FP64 FMA rate of the device in TFLOP/s (lgf_fp64_peak)."""
+    import torch
+    v = C.c_double()
+    st = lib().lgf_fp64_peak(int(reps), C.c_void_p(torch.cuda.current_stream().cuda_stream), C.byref(v))
+    if st != LGF_OK:
+        raise LgfError(st, "lgf_fp64_peak")
+    return v.value
 
 
 def stream_peak_gbs(n_sites: int = 1 << 20, write: bool = False, reps: int = 10) -> float:

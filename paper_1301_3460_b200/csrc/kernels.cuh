@@ -584,6 +584,19 @@ __global__ void __launch_bounds__(128) k_streams(double2* __restrict__ a, long l
     }
 }
 
+// FP64 FMA yardstick: every thread runs 8 independent chains of dependent DFMAs in registers (no memory traffic);
+// 2 * 8 * iters flops per thread.  The second roof of the FFT passes.
+__global__ void __launch_bounds__(256) k_fma64(double* __restrict__ sink, int iters, double a, double b) {
+    double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+#pragma unroll 4
+    for (int i = 0; i < iters; i++) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 1.2345e300) sink[0] = s;                                 // never true: keeps the chains alive
+}
+
 #endif  // LGF_F32
 
 }  // namespace lgf

@@ -1409,6 +1409,29 @@ lgf_status lgf_stream_peak(void* buf, size_t n_sites, int write, int reps, void*
     return LGF_OK;
 }
 
+lgf_status lgf_fp64_peak(int reps, void* stream, double* tflops) {
+    if (!tflops || reps < 1) return LGF_ERR_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return LGF_ERR_CUDA;
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev); cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    double* sink = nullptr;
+    if (cudaMalloc(&sink, 8) != cudaSuccess) { cudaGetLastError(); cudaEventDestroy(a); cudaEventDestroy(b); return LGF_ERR_OOM; }
+    const int iters = 4096;
+    const unsigned grid = (unsigned)(sms * 8);                        // 8 CTAs of 256 threads per SM: 64 warps
+    k_fma64<<<grid, 256, 0, s>>>(sink, iters, 0.999999, 1e-9);        // warm-up
+    cudaEventRecord(a, s);
+    for (int i = 0; i < reps; i++) k_fma64<<<grid, 256, 0, s>>>(sink, iters, 0.999999, 1e-9);
+    cudaEventRecord(b, s);
+    cudaError_t e = cudaEventSynchronize(b);
+    float t = 0; cudaEventElapsedTime(&t, a, b);
+    cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(sink);
+    if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) return LGF_ERR_CUDA;
+    *tflops = 2.0 * 8.0 * iters * 256.0 * grid * reps / ((double)t * 1e-3) / 1e12;
+    return LGF_OK;
+}
+
 const char* lgf_status_string(lgf_status s) {
     switch (s) {
         case LGF_OK: return "ok";
