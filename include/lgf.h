@@ -217,6 +217,35 @@ const char *lgf_last_error_sharded(lgf_slab_ctx *ctx);
  * FFT passes: the path is HBM-bound, but pass B is within a factor of two of this one as well. */
 lgf_status lgf_fp64_peak(int reps, void *cuda_stream, double *tflops);
 
+/* ---- theta and F without any allocation (csrc/lgf_static.cu).
+ * Every call above that needs device memory gets it from cudaMalloc, at lgf_create or (lgf_scan_alpha) per call.  Some
+ * programs cannot let a library do that: a production Monte Carlo job whose own pool took all of the HBM at start-up (a
+ * library cudaMalloc then fails although the job has memory to spare), a program under a framework's caching allocator
+ * (what the framework has cached is invisible to cudaMalloc), or a measurement hook inside a running update loop (cudaMalloc
+ * and cudaFree synchronise the whole device and would stall the job's other streams on every call).  For them the lattice
+ * sums of step S1 -- the gauge-fixing monitor theta and the functional F (PAPER.md:39 with g = 1; theta as in PAPER.md:47) --
+ * are one stateless call.  It needs no context, creates no stream or event, and calls no cudaMalloc/cudaFree: its only
+ * scratch memory, one partial sum per 128 sites, is a fixed array inside the library image.
+ *   dev_links   DEVICE, canonical order, V*4*18 doubles, 16-byte aligned; read only.  All three rows are read (no 12-real
+ *               rebuild), nothing is reprojected.
+ *   dims        HOST, {L0,L1,L2,L3}, every L_mu >= 1 (any integers, not only powers of two), V = L0 L1 L2 L3 <=
+ *               LGF_STATIC_MAX_SITES; a larger lattice returns LGF_ERR_UNSUPPORTED and launches nothing.
+ *   cuda_stream a cudaStream_t of the current device cast to void* (NULL: the default stream).
+ *   dev_out     DEVICE, 2 doubles: dev_out[0] = F, dev_out[1] = theta (Landau gauge, the normalisations of lgf_measure).
+ * Unlike the context calls this one does not wait: it enqueues two kernels on cuda_stream and returns; dev_out is final
+ * when the stream has run them.  Returns LGF_OK, LGF_ERR_INVALID_ARG (NULL pointer, extent < 1), LGF_ERR_UNSUPPORTED (too
+ * many sites), LGF_ERR_CUDA (no device, failed launch); lgf_measure_static_error() gives the text of the calling thread's
+ * last failure ("" after a success).
+ * Cost and sharing: the array is LGF_STATIC_MAX_SITES/128 * 16 B = 2 MiB of every GPU the process uses, from the moment the
+ * library is loaded until exit.  The first call on a device looks up the array's address on that device and keeps it:
+ * make that first call before beginning any stream capture.  All calls on a device use the same array, which keeps the
+ * previous call's partial sums; a call overwrites every entry it later reads, so nothing needs clearing -- but calls that
+ * overlap on the GPU (two streams, or two host threads without ordering between their streams) race on it and both
+ * results are then undefined.  Calls on one stream, or ordered by events, are safe. */
+#define LGF_STATIC_MAX_SITES (1 << 24)   /* 64^4, the largest lattice of BASELINE.json */
+lgf_status lgf_measure_static(const double *dev_links, const int dims[4], void *cuda_stream, double *dev_out);
+const char *lgf_measure_static_error(void);
+
 const char *lgf_status_string(lgf_status s);
 const char *lgf_last_error(lgf_ctx *ctx); /* detail of the last LGF_ERR_CUDA (static or ctx-owned string) */
 

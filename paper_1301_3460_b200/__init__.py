@@ -16,7 +16,7 @@ import os
 import numpy as np
 
 __all__ = [
-    "LgfError", "lib", "library_path", "GaugeFixer", "ShardedGaugeFixer", "copy_peak_gbs", "stream_peak_gbs", "fp64_peak_tflops",
+    "LgfError", "lib", "library_path", "GaugeFixer", "ShardedGaugeFixer", "measure_static", "LGF_STATIC_MAX_SITES", "copy_peak_gbs", "stream_peak_gbs", "fp64_peak_tflops",
     "LGF_OK", "LGF_NOT_CONVERGED", "LGF_FP64", "LGF_FP32", "LGF_MIXED", "LGF_STORE_12", "LGF_STORE_18",
     "LGF_FIELD_DELTA", "LGF_FIELD_X", "LGF_FIELD_G",
     "LGF_OPT_STORE_G", "LGF_OPT_GRAPH", "LGF_OPT_BATCH", "LGF_OPT_PDL", "LGF_OPT_FAST_FFT", "LGF_OPT_FOURIER_ACCEL",
@@ -38,6 +38,7 @@ LGF_FIELD_DELTA, LGF_FIELD_X, LGF_FIELD_G = 0, 1, 2
 LGF_OPT_STORE_G, LGF_OPT_GRAPH, LGF_OPT_BATCH, LGF_OPT_PDL, LGF_OPT_FAST_FFT = 0, 1, 2, 3, 4
 LGF_OPT_FOURIER_ACCEL, LGF_OPT_GAUGE_DIRECTIONS, LGF_OPT_MIXED_FP32_ITERS, LGF_OPT_MIXED_SWITCH, LGF_OPT_TMA = 5, 6, 7, 8, 9
 LGF_MAX_KERNELS = 32
+LGF_STATIC_MAX_SITES = 1 << 24
 
 # every symbol include/lgf.h declares (checked by tests/test_abi.py against the header text)
 EXPORTS = [
@@ -47,6 +48,7 @@ EXPORTS = [
     "lgf_launch_count", "lgf_copy_peak", "lgf_stream_peak", "lgf_fp64_peak", "lgf_status_string", "lgf_last_error",
     "lgf_create_sharded", "lgf_destroy_sharded", "lgf_sharded_ranks", "lgf_load_links_sharded", "lgf_get_links_sharded",
     "lgf_iterate_sharded", "lgf_fix_sharded", "lgf_get_history_sharded", "lgf_sharded_traffic", "lgf_last_error_sharded",
+    "lgf_measure_static", "lgf_measure_static_error",
 ]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -135,6 +137,9 @@ def lib():
     L.lgf_sharded_traffic.argtypes = [P, C.POINTER(C.c_longlong)]
     L.lgf_last_error_sharded.restype = C.c_char_p
     L.lgf_last_error_sharded.argtypes = [P]
+    L.lgf_measure_static.argtypes = [P, I4, P, P]
+    L.lgf_measure_static_error.restype = C.c_char_p
+    L.lgf_measure_static_error.argtypes = []
     _lib = L
     return L
 
@@ -392,6 +397,20 @@ class ShardedGaugeFixer:
         o = (C.c_longlong * 5)()
         self._ck(lib().lgf_sharded_traffic(self._h, o), "lgf_sharded_traffic")
         return dict(halo_u_bytes=int(o[0]), halo_x_bytes=int(o[1]), transpose_bytes=int(o[2]), launches=int(o[3]), copies=int(o[4]))
+
+
+def measure_static(dev_links_ptr: int, dims, dev_out_ptr: int, cuda_stream: int = 0) -> None:
+    """lgf_measure_static: F and theta of the links at ``dev_links_ptr`` (DEVICE, canonical [V,4,3,3] complex128) into the
+    two doubles at ``dev_out_ptr`` (DEVICE: F, theta), for callers that cannot let the library allocate -- their own pool
+    or a framework's caching allocator holds the HBM, or they run inside a loop that a device-wide cudaMalloc/cudaFree
+    synchronisation would stall.  No context and no allocation: the scratch memory is a fixed 2 MiB array inside the library, so at most
+    ``LGF_STATIC_MAX_SITES`` sites.  The call only enqueues work on ``cuda_stream`` (a raw cudaStream_t as int, 0 = default
+    stream) and does not wait; calls that overlap on the GPU share the scratch array and race, so keep them on one
+    stream.  Make the first call on a device before any stream capture.  Marshalling only."""
+    L = lib()
+    st = L.lgf_measure_static(C.c_void_p(int(dev_links_ptr)), _dims(dims), C.c_void_p(int(cuda_stream)), C.c_void_p(int(dev_out_ptr)))
+    if st != LGF_OK:
+        raise LgfError(st, "lgf_measure_static", L.lgf_measure_static_error().decode())
 
 
 def copy_peak_gbs(nbytes: int = 1 << 30, reps: int = 10) -> float:

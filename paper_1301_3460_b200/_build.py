@@ -9,14 +9,15 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "liblgf.so")
 SOURCES = [os.path.join(CSRC, "lgf_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("kernels.cuh", "fft_tile.cuh", "fft_fast.cuh", "fft_tma.cuh", "su3.cuh", "slab.cuh", "lgf_slab.inl")] + [
+STATIC_SOURCE = os.path.join(CSRC, "lgf_static.cu")      # lgf_measure_static: the entry point that allocates nothing
+DEPS = SOURCES + [STATIC_SOURCE] + [os.path.join(CSRC, f) for f in ("kernels.cuh", "fft_tile.cuh", "fft_fast.cuh", "fft_tma.cuh", "su3.cuh", "slab.cuh", "lgf_slab.inl")] + [
     os.path.join(os.path.dirname(HERE), "include", "lgf.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v",
 ]
 # lgf_api.cu is compiled twice: fp64 (public lgf_* entry points) and, with -DLGF_F32, fp32 (lgf32_* twins)
-OBJECTS = [("lgf_api_f64.o", []), ("lgf_api_f32.o", ["-DLGF_F32"])]
+OBJECTS = [("lgf_api_f64.o", SOURCES, []), ("lgf_api_f32.o", SOURCES, ["-DLGF_F32"]), ("lgf_static.o", [STATIC_SOURCE], [])]
 
 
 def nvcc() -> str:
@@ -43,8 +44,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return OUT
     procs = []
-    for obj, extra in OBJECTS:
-        cmd = [nvcc()] + NVCC_FLAGS + extra + ["-c"] + SOURCES + ["-o", os.path.join(HERE, obj)]
+    for obj, src, extra in OBJECTS:
+        cmd = [nvcc()] + NVCC_FLAGS + extra + ["-c"] + src + ["-o", os.path.join(HERE, obj)]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
     log = ""
     for cmd, p in procs:
@@ -54,7 +55,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(out + err)
         if p.returncode != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared"] + [os.path.join(HERE, o) for o, _ in OBJECTS] + ["-o", OUT]
+    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared"] + [os.path.join(HERE, o) for o, _, _ in OBJECTS] + ["-o", OUT]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
