@@ -41,25 +41,54 @@ def up_to_date() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile and link liblgf.so unless it is newer than every source.  Safe when several processes arrive at once
+    (torchrun ranks, pytest-xdist workers): one of them builds under an exclusive file lock while the others wait and then
+    find the library up to date; objects and the library are written under temporary names and moved into place, so no
+    process ever loads a half-written file."""
     if not force and up_to_date():
         return OUT
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and up_to_date():       # another process built it while this one waited for the lock
+                return OUT
+            return _build_locked(verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(verbose: bool) -> str:
+    tag = ".tmp%d" % os.getpid()
     procs = []
     for obj, src, extra in OBJECTS:
-        cmd = [nvcc()] + NVCC_FLAGS + extra + ["-c"] + src + ["-o", os.path.join(HERE, obj)]
+        cmd = [nvcc()] + NVCC_FLAGS + extra + ["-c"] + src + ["-o", os.path.join(HERE, obj + tag)]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
     log = ""
+    failed = None
     for cmd, p in procs:
         out, err = p.communicate()
-        log += "# " + " ".join(cmd) + "\n" + err
+        log += "# " + " ".join(cmd).replace(tag, "") + "\n" + err
         if verbose or p.returncode != 0:
             sys.stderr.write(out + err)
-        if p.returncode != 0:
-            raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared"] + [os.path.join(HERE, o) for o, _, _ in OBJECTS] + ["-o", OUT]
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-        raise RuntimeError("link failed: " + " ".join(cmd))
+        if p.returncode != 0 and failed is None:
+            failed = "nvcc failed: " + " ".join(cmd)
+    objs = [os.path.join(HERE, o) for o, _, _ in OBJECTS]
+    try:
+        if failed:
+            raise RuntimeError(failed)
+        for o in objs:
+            os.replace(o + tag, o)
+        cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared"] + objs + ["-o", OUT + tag]
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError("link failed: " + " ".join(cmd))
+        os.replace(OUT + tag, OUT)
+    finally:
+        for f in [o + tag for o in objs] + [OUT + tag]:
+            if os.path.exists(f):
+                os.remove(f)
     with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
         f.write(log)
     return OUT
