@@ -9,7 +9,8 @@ closing measurement (reading A5).  metric = iterations/s at 32^4 SU(3) fp64, 12-
 BASELINE.json configs[2]); value = N * K * inner / (max over ranks of the CUDA-event time of the K steps).
 N > 1: one independent configuration per GPU (replicas, weak scaling), no collective on the
 data path.  The JSON line also carries: e2e (host buffers through the C ABI), roofline (dominant kernel, live
-CUDA-event timing), kernels (every kernel), iteration (whole-iteration HBM fraction), time_to_theta (lgf_fix),
+CUDA-event timing), kernels (every kernel), iteration (whole iteration: effective = algorithmic bytes over time, and dram =
+the DRAM bytes of the committed ncu capture over the same time), time_to_theta (lgf_fix),
 cpu_baseline (the oracle timed on the host cores), clocks, gpu_launches, and other_configs (C3: iterate(500), C4: iterate(200) and
 lgf_fix, each on its own BASELINE.json ensemble with its own kernel table, HBM fraction and clocks).
 
@@ -86,6 +87,7 @@ def ncu_traffic(kernel: str, workload: str):
     The number is NOT measured in this run (a bench value is never taken under a profiler): it is stamped with the
     commit of its capture so that a reader can tell whether the kernel has changed since."""
     import csv
+    kernel = {"k_fa_inv1": "k_fa_inv"}.get(kernel, kernel)      # profiling slot name -> function name ncu prints (k_fa_inv<6,6,1>)
     try:
         with open(os.path.join(ROOT, TRAFFIC_CSV)) as f:
             for r in csv.DictReader(f):
@@ -94,6 +96,20 @@ def ncu_traffic(kernel: str, workload: str):
     except Exception:
         pass
     return None, None
+
+
+def ncu_iteration_traffic(kernel_names, workload: str):
+    """DRAM bytes of one whole iteration on `workload` from the same committed captures: the sum over the kernels this run
+    launched (`kernel_names`), or (None, ...) when one of them has no capture for this workload.  Returns (bytes, the
+    per-kernel bytes, the capture commits).  Like roofline.traffic: cold-cache single launches, not measured in this run."""
+    per, commits = {}, set()
+    for k in kernel_names:
+        b, c = ncu_traffic(k, workload)
+        if b is None:
+            return None, {}, []
+        per[k] = b
+        commits.add(c)
+    return sum(per.values()), per, sorted(c for c in commits if c)
 
 
 class ClockSampler:
@@ -192,7 +208,10 @@ def workload_config(name: str, cfg: dict, links: str, inner: int, world: int, be
         src = f"eps={cfg.get('eps')}"
     return {"workload": f"{name}: SU(3) {dims_name(dims)} {storage}-real, {src}, seed={cfg['seed']}, alpha=0.08",
             "iterations_per_step": inner,
-            "l2": "inputs larger than L2 (links %.0f MB + field %.0f MB per GPU)" % (V * nc * 64 / 1e6, V * 64 / 1e6),
+            "l2": ("no flush between iterations: the links (%.0f MB per GPU, read and written every iteration) are %s the 126 MB L2; "
+                   "the field (%.0f MB) %s -- iteration.dram_frac_of_measured is the HBM figure, iteration.effective_* counts algorithmic bytes"
+                   % (V * nc * 64 / 1e6, "larger than" if V * nc * 64 > 126e6 else "NOT larger than", V * 64 / 1e6,
+                      "is larger too" if V * 64 > 126e6 else "fits in L2, so passes B and C are partly L2-fed")),
             "parallelism": "replicas" if world > 1 else "single"}
 
 
@@ -260,9 +279,23 @@ def profile_kernels(gf, reload, V: int, kb: dict, inner: int, peak: float):
     return kernels, dom, iter_bytes
 
 
-def iteration_block(iter_bytes: int, V: int, it_s: float, peak: float) -> dict:
-    return {"bytes_per_site": iter_bytes // V, "bytes": iter_bytes, "gbs": iter_bytes * it_s / 1e9,
-            "frac_of_measured": iter_bytes * it_s / 1e9 / peak, "frac_of_spec_8000": iter_bytes * it_s / 1e9 / 8000.0}
+def iteration_block(iter_bytes: int, V: int, it_s: float, peak: float, kernel_names=(), workload: str = "") -> dict:
+    """Whole-iteration figures.  `effective_*`: ALGORITHMIC bytes (every array each kernel must read or
+    write, once) x iterations/s -- a model fraction, which counts bytes an L2-resident field never moves through HBM (at
+    32^4 the 67 MB field stays in the 126 MB L2 between passes, so passes B and C write ~15 MB each instead of 67).
+    `dram_*`: the DRAM bytes ncu counted for the same kernels (committed capture) x the iterations/s
+    of THIS run -- the HBM throughput the iteration really sustains."""
+    out = {"bytes_per_site": iter_bytes // V, "bytes": iter_bytes, "basis": "effective = algorithmic bytes / time; dram = ncu DRAM bytes / time",
+           "effective_gbs": iter_bytes * it_s / 1e9, "effective_frac_of_measured": iter_bytes * it_s / 1e9 / peak,
+           "effective_frac_of_spec_8000": iter_bytes * it_s / 1e9 / 8000.0}
+    dram, per, commits = ncu_iteration_traffic([k for k in kernel_names], workload) if kernel_names else (None, {}, [])
+    out["dram_bytes_ncu"] = dram
+    out["dram_gbs_ncu"] = dram * it_s / 1e9 if dram else None
+    out["dram_frac_of_measured"] = dram * it_s / 1e9 / peak if dram else None
+    out["dram_bytes_ncu_per_kernel"] = per or None
+    out["dram_source"] = (f"{TRAFFIC_CSV} (ncu --set full, one cold-cache launch per kernel; NOT measured in this run: captured at commit {','.join(commits)})"
+                          if dram else f"no capture of every kernel of this workload in {TRAFFIC_CSV}")
+    return out
 
 
 def timed_fix(gf, reload, tol: float) -> dict:
@@ -277,7 +310,7 @@ def timed_fix(gf, reload, tol: float) -> dict:
             "theta": r["theta"], "theta_tol": tol}
 
 
-def other_config(lgf, E, name: str, n_iter: int, peak: float, local: int) -> dict:
+def other_config(lgf, E, name: str, n_iter: int, peak: float, local: int, n_cpu: int = 0) -> dict:
     """One of the other BASELINE.json configs (C3: iterate(500); C4: iterate(200)), links resident, on the config's own
     ensemble generated on the device (ensembles.noisy_device, reading A12b): throughput of `n_iter` iterations in one
     lgf_iterate call, per-kernel table, whole-iteration HBM fraction, time to theta < 1e-15, clocks."""
@@ -311,10 +344,23 @@ def other_config(lgf, E, name: str, n_iter: int, peak: float, local: int) -> dic
     ttt = timed_fix(gf, reload, THETA_TOL)
     ttt["plaquette"] = plaq
     gf.destroy()
+    cpu = None
+    if n_cpu > 0:
+        # the oracle as it stands on the host cores, on the same links (5 iterations at C3, 3 at C4)
+        import oracle
+        o = oracle.Oracle(dims, storage, fft_mode=1)
+        o.load(d_in.cpu().numpy())
+        o.iterate(1, ALPHA)
+        t0 = time.perf_counter()
+        o.iterate(n_cpu, ALPHA)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n_cpu / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{n_cpu} iterations of {name} ({dims_name(dims)}, {storage}-real), oracle radix-2 FFT mode, after 1 warm-up"}
+        del o
     del d_in
     torch.cuda.empty_cache()
-    return {"config": workload_config(name, cfg, "noisy_device", n_iter, 1), "value": it_s, "unit": UNIT,
-            "ms_per_step": ms, "steps": reps, "iteration": iteration_block(iter_bytes, V, it_s, peak),
+    return {"config": workload_config(name, cfg, "noisy_device", n_iter, 1), "value": it_s, "unit": UNIT, "cpu_baseline": cpu,
+            "ms_per_step": ms, "steps": reps, "iteration": iteration_block(iter_bytes, V, it_s, peak, [k for k in kernels if kernels[k]["bytes_per_launch"] > 0], name),
             "dominant_kernel": dom, "kernels": kernels, "time_to_theta": ttt, "clocks": clocks}
 
 
@@ -440,6 +486,10 @@ def run_ours(args):
                    "d2h_bytes_per_step": V * 384 + 16, "ms_per_step": ms_r / e2e_steps, "steps": e2e_steps,
                    "host_format": "two-row [V][4][2][3][2] (lgf_load_links_12 / lgf_get_links_12; PAPER.md:45 12-real representation)"}
             del rows_in, rows_out
+        # e2e is quoted on the context's own host format (two-row for 12-real storage: the paper's representation);
+        # the SURVEY.md 8(b) calls lgf_load_links / lgf_get_links (canonical 18-real) ride inside the same object
+        if e2e is not e2e_canon:
+            e2e["canonical"] = e2e_canon
 
     line = None
     if rank == 0:
@@ -516,9 +566,9 @@ def run_ours(args):
             gf.destroy()
             del h_in, h_out
             others = {}
-            for nm, n_it in (("C3", 500), ("C4", 200)):
+            for nm, n_it, n_cpu in (("C3", 500, 5), ("C4", 200, 3)):
                 try:
-                    others[nm] = other_config(lgf, E, nm, n_it, peak, local)
+                    others[nm] = other_config(lgf, E, nm, n_it, peak, local, 0 if args.no_cpu_baseline else n_cpu)
                 except Exception as e:                   # reported, never fatal for the headline number
                     others[nm] = {"error": f"{type(e).__name__}: {e}"}
         traffic, traffic_commit = ncu_traffic(dom, args.workload) if not fp32 else (None, None)
@@ -538,7 +588,7 @@ def run_ours(args):
                          "bytes_per_launch": kernels[dom]["bytes_per_launch"], "avg_us": kernels[dom]["avg_us"],
                          "copy_kernel_gbs": copy_gbs, "stream_yardstick_gbs": stream_gbs,
                          "fp64_fma_tflops": fp64_tflops},
-            "iteration": iteration_block(iter_bytes, V, it_s_1, peak),
+            "iteration": iteration_block(iter_bytes, V, it_s_1, peak, [k for k in kernels if kernels[k]["bytes_per_launch"] > 0], args.workload) if not fp32 else iteration_block(iter_bytes, V, it_s_1, peak),
             "kernels": kernels,
             "time_to_theta": ttt,
             "cpu_baseline": cpu,
