@@ -210,7 +210,7 @@ lgf_status lgf_get_history_sharded(lgf_slab_ctx *ctx, double *hist, int capacity
 /* out (HOST, 5 values): bytes ONE rank sends per iteration for [0] the U_3 halo, [1] the X halo, [2] the two transposes;
  * [3] kernels launched and [4] inter-rank copies issued by the context so far. */
 lgf_status lgf_sharded_traffic(lgf_slab_ctx *ctx, long long out[5]);
-const char *lgf_last_error_sharded(lgf_slab_ctx *ctx);
+const char *lgf_last_error_sharded(lgf_slab_ctx *ctx);   /* ctx == NULL: text of the calling thread's last failed lgf_create_sharded */
 
 /* Third yardstick: the FP64 FMA rate of the device (8 independent chains of dependent fused multiply-adds per thread, 64
  * warps per SM, no memory traffic), in TFLOP/s, averaged over `reps` launches on cuda_stream.  The arithmetic roof of the

@@ -348,7 +348,7 @@ class ShardedGaugeFixer:
         h = C.c_void_p()
         st = lib().lgf_create_sharded((C.c_int * 4)(*self.dims), self.n_ranks, int(storage), C.byref(h))
         if st != LGF_OK:
-            raise LgfError(st, "lgf_create_sharded")
+            raise LgfError(st, "lgf_create_sharded", f"dims={tuple(self.dims)} n_ranks={self.n_ranks} " + lib().lgf_last_error_sharded(None).decode())
         self._h = h
 
     def destroy(self):

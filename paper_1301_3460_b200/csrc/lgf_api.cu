@@ -876,22 +876,28 @@ lgf_status run(lgf_ctx* c, double alpha, double tol, int max_iter, bool poll) {
 }
 
 // detail of the last failed lgf_create* of this thread (the context it belonged to is gone): lgf_last_error(NULL)
-thread_local std::string g_create_err;
+thread_local std::string g_create_err;     // text of this thread's last failed create ("" after a successful one)
+#ifndef LGF_F32
+thread_local int g_create_from32 = 0;      // 1: that create ran (and failed) in the fp32 translation unit, which keeps its own text
+#endif
 
 lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* wsp, size_t ws_bytes, void* stream, bool own, lgf_ctx** out) {
-    if (!dims || !out) return LGF_ERR_INVALID_ARG;
+    // lgf_last_error(NULL) speaks of the LAST create of this thread: cleared here, set on every failing return below
+    g_create_err.clear();
+    auto refuse = [&](lgf_status st, const char* why) { g_create_err = why; return st; };
+    if (!dims || !out) return refuse(LGF_ERR_INVALID_ARG, "lgf_create: dims or out is NULL");
     *out = nullptr;
-    if (p != LGF_FP64 && p != LGF_FP32 && p != LGF_MIXED) return LGF_ERR_INVALID_ARG;
-    if (s != LGF_STORE_12 && s != LGF_STORE_18) return LGF_ERR_INVALID_ARG;
-    for (int k = 0; k < 4; k++) if (dims[k] < 1) return LGF_ERR_INVALID_ARG;
-    if (p != LGF_THIS_PREC) return LGF_ERR_UNSUPPORTED;
+    if (p != LGF_FP64 && p != LGF_FP32 && p != LGF_MIXED) return refuse(LGF_ERR_INVALID_ARG, "lgf_create: precision is not LGF_FP64, LGF_FP32 or LGF_MIXED");
+    if (s != LGF_STORE_12 && s != LGF_STORE_18) return refuse(LGF_ERR_INVALID_ARG, "lgf_create: storage is not LGF_STORE_12 or LGF_STORE_18");
+    for (int k = 0; k < 4; k++) if (dims[k] < 1) return refuse(LGF_ERR_INVALID_ARG, "lgf_create: an extent is smaller than 1");
+    if (p != LGF_THIS_PREC) return refuse(LGF_ERR_UNSUPPORTED, "lgf_create: precision not built into this translation unit");
     int lg[4];
-    if (!dims_ok(dims, lg)) return LGF_ERR_UNSUPPORTED;
+    if (!dims_ok(dims, lg)) return refuse(LGF_ERR_UNSUPPORTED, "lgf_create: extents must be powers of two, 4 <= L <= 128, L0*L1 <= 4096, L2*L3 <= 4096");
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return LGF_ERR_CUDA;   // no CPU fallback
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return refuse(LGF_ERR_CUDA, "lgf_create: no CUDA device (there is no CPU fallback)"); }
 
     lgf_ctx* c = new (std::nothrow) lgf_ctx();
-    if (!c) return LGF_ERR_OOM;
+    if (!c) return refuse(LGF_ERR_OOM, "lgf_create: host allocation of the context failed");
     c->precision = (int)LGF_THIS_PREC;
     int shv = 0;
     for (int k = 0; k < 4; k++) { c->G.L[k] = dims[k]; c->G.lg[k] = lg[k]; c->G.sh[k] = shv; shv += lg[k]; }
@@ -909,12 +915,16 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->ev_copy[0] = c->ev_copy[1] = c->ev_kern[0] = c->ev_kern[1] = nullptr;
     memset(c->prof_ms, 0, sizeof c->prof_ms); memset(c->prof_n, 0, sizeof c->prof_n);
 
-    auto fail = [&](lgf_status st) { g_create_err = c->err; lgf_destroy(c); return st; };
+    auto fail = [&](lgf_status st, const char* why = nullptr) {
+        g_create_err = !c->err.empty() ? c->err : std::string(why ? why : "lgf_create: set-up failed");
+        lgf_destroy(c);
+        return st;
+    };
     if (own) {
-        if (cudaMalloc(&c->ws, c->lay.total) != cudaSuccess) { cudaGetLastError(); return fail(LGF_ERR_OOM); }
-        if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(LGF_ERR_CUDA);
+        if (cudaMalloc(&c->ws, c->lay.total) != cudaSuccess) { cudaGetLastError(); return fail(LGF_ERR_OOM, "lgf_create: cudaMalloc of the workspace failed"); }
+        if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(LGF_ERR_CUDA, "lgf_create: cudaStreamCreate failed");
     } else {
-        if (!wsp || ((size_t)wsp & 255) || ws_bytes < c->lay.total) return fail(LGF_ERR_INVALID_ARG);
+        if (!wsp || ((size_t)wsp & 255) || ws_bytes < c->lay.total) return fail(LGF_ERR_INVALID_ARG, "lgf_create_ex: workspace is NULL, not 256-byte aligned, or smaller than lgf_workspace_bytes()");
         c->ws = static_cast<char*>(wsp);
         c->stream = static_cast<cudaStream_t>(stream);
     }
@@ -925,12 +935,12 @@ lgf_status create_impl(const int dims[4], lgf_precision p, lgf_storage s, void* 
     c->partials = reinterpret_cast<double2*>(c->ws + c->lay.partials);
     c->hist = reinterpret_cast<double2*>(c->ws + c->lay.hist);
     c->ctl = reinterpret_cast<Ctl*>(c->ws + c->lay.ctl);
-    if (cudaHostAlloc(&c->h_ctl, sizeof(Ctl), cudaHostAllocDefault) != cudaSuccess) return fail(LGF_ERR_OOM);
-    if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) return fail(LGF_ERR_CUDA);
-    if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(LGF_ERR_CUDA);
+    if (cudaHostAlloc(&c->h_ctl, sizeof(Ctl), cudaHostAllocDefault) != cudaSuccess) return fail(LGF_ERR_OOM, "lgf_create: cudaHostAlloc of the control block failed");
+    if (cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess) return fail(LGF_ERR_CUDA, "lgf_create: cudaEventCreate failed");
+    if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(LGF_ERR_CUDA, "lgf_create: cudaStreamCreate (copy stream) failed");
     for (int k = 0; k < 2; k++)
         if (cudaEventCreateWithFlags(&c->ev_copy[k], cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&c->ev_kern[k], cudaEventDisableTiming) != cudaSuccess) return fail(LGF_ERR_CUDA);
+            cudaEventCreateWithFlags(&c->ev_kern[k], cudaEventDisableTiming) != cudaSuccess) return fail(LGF_ERR_CUDA, "lgf_create: cudaEventCreate failed");
     lgf_status st = setup_kernels(c);
     if (st != LGF_OK) return fail(st);
     st = build_tables(c);
@@ -1027,7 +1037,8 @@ size_t lgf_workspace_bytes(const int dims[4], lgf_precision p, lgf_storage s) {
 #ifndef LGF_F32
 // LGF_MIXED: an fp64 context that owns an fp32 shadow context on the same stream
 static lgf_status create_mixed(const int dims[4], lgf_storage s, void* ws, size_t bytes, void* stream, bool own, lgf_ctx** out) {
-    if (!dims || !out) return LGF_ERR_INVALID_ARG;
+    g_create_err.clear();
+    if (!dims || !out) { g_create_err = "lgf_create: dims or out is NULL"; return LGF_ERR_INVALID_ARG; }
     *out = nullptr;
     const size_t n64 = lgf_workspace_bytes(dims, LGF_FP64, s), n32 = lgf32_workspace_bytes(dims, LGF_FP32, s);
     lgf_ctx* c = nullptr;
@@ -1035,17 +1046,17 @@ static lgf_status create_mixed(const int dims[4], lgf_storage s, void* ws, size_
     if (own) st = create_impl(dims, LGF_FP64, s, nullptr, 0, nullptr, true, &c);
     else {
         if (n64 == 0 || n32 == 0) return create_impl(dims, LGF_FP64, s, ws, bytes, stream, false, &c);   // reports the argument error
-        if (!ws || bytes < align_up(n64, 256) + n32) return LGF_ERR_INVALID_ARG;
+        if (!ws || bytes < align_up(n64, 256) + n32) { g_create_err = "lgf_create_ex: LGF_MIXED workspace is NULL or smaller than lgf_workspace_bytes()"; return LGF_ERR_INVALID_ARG; }
         st = create_impl(dims, LGF_FP64, s, ws, align_up(n64, 256), stream, false, &c);
     }
     if (st != LGF_OK) return st;
     char* ws32;
     if (own) {
-        if (cudaMalloc(&c->shadow_ws, n32) != cudaSuccess) { cudaGetLastError(); lgf_destroy(c); return LGF_ERR_OOM; }
+        if (cudaMalloc(&c->shadow_ws, n32) != cudaSuccess) { cudaGetLastError(); lgf_destroy(c); g_create_err = "lgf_create: cudaMalloc of the fp32 workspace of LGF_MIXED failed"; return LGF_ERR_OOM; }
         ws32 = c->shadow_ws;
     } else ws32 = static_cast<char*>(ws) + align_up(n64, 256);
     st = lgf32_create_ex(dims, LGF_FP32, s, ws32, n32, c->stream, &c->shadow);
-    if (st != LGF_OK) { c->shadow = nullptr; lgf_destroy(c); return st; }
+    if (st != LGF_OK) { c->shadow = nullptr; lgf_destroy(c); g_create_from32 = 1; return st; }   // the text is the fp32 unit's
     *out = c;
     return LGF_OK;
 }
@@ -1053,6 +1064,7 @@ static lgf_status create_mixed(const int dims[4], lgf_storage s, void* ws, size_
 
 lgf_status lgf_create(const int dims[4], lgf_precision p, lgf_storage s, lgf_ctx** out) {
 #ifndef LGF_F32
+    g_create_from32 = (p == LGF_FP32);
     if (p == LGF_FP32) return lgf32_create(dims, p, s, out);
     if (p == LGF_MIXED) return create_mixed(dims, s, nullptr, 0, nullptr, true, out);
 #endif
@@ -1060,6 +1072,7 @@ lgf_status lgf_create(const int dims[4], lgf_precision p, lgf_storage s, lgf_ctx
 }
 lgf_status lgf_create_ex(const int dims[4], lgf_precision p, lgf_storage s, void* ws, size_t bytes, void* stream, lgf_ctx** out) {
 #ifndef LGF_F32
+    g_create_from32 = (p == LGF_FP32);
     if (p == LGF_FP32) return lgf32_create_ex(dims, p, s, ws, bytes, stream, out);
     if (p == LGF_MIXED) return create_mixed(dims, s, ws, bytes, stream, false, out);
 #endif
@@ -1448,6 +1461,9 @@ const char* lgf_status_string(lgf_status s) {
 #endif
 const char* lgf_last_error(lgf_ctx* c) {
     FWD32(lgf32_last_error(c))
+#ifndef LGF_F32
+    if (!c && g_create_from32) return lgf32_last_error(nullptr);     // the last create of this thread failed in the fp32 unit
+#endif
     return c ? c->err.c_str() : g_create_err.c_str();
 }
 

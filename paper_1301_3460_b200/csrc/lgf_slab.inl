@@ -27,10 +27,14 @@ struct lgf_slab_ctx {
     size_t smem01, smem23;
     bool loaded;
     long long launches, copies;
+    cudaError_t copy_err;                // first failed inter-rank copy since the last slab_run began (cudaSuccess: none)
+    const char* copy_what;
     std::string err;
 };
 
 namespace {
+
+thread_local std::string g_slab_create_err;      // text of this thread's last failed lgf_create_sharded ("" after a success)
 
 #define SCK(call)                                                                                          \
     do {                                                                                                   \
@@ -48,6 +52,14 @@ namespace {
 // (the runtime routes it over NVLink), or an ncclSend/ncclRecv pair of the packed rows.
 cudaError_t slab_copy2d(void* dst, size_t dpitch, const void* src, size_t spitch, size_t row_bytes, size_t rows, cudaStream_t s) {
     return cudaMemcpy2DAsync(dst, dpitch, src, spitch, row_bytes, rows, cudaMemcpyDefault, s);
+}
+
+// The halo exchanges are enqueued from functions that return nothing; a failed copy is remembered here and turned into
+// LGF_ERR_CUDA by slab_run before any result is read.
+void slab_exchange(lgf_slab_ctx* c, const char* what, void* dst, size_t dpitch, const void* src, size_t spitch, size_t row_bytes, size_t rows) {
+    const cudaError_t e = slab_copy2d(dst, dpitch, src, spitch, row_bytes, rows, c->stream);
+    if (e != cudaSuccess && c->copy_err == cudaSuccess) { c->copy_err = e; c->copy_what = what; }
+    c->copies++;
 }
 
 void slab_geom(Geom& G, int l0, int l1, int l2, int l3, int nd) {
@@ -77,8 +89,7 @@ template <int NC> void slab_measure(lgf_slab_ctx* c) {
     for (int r = 0; r < P; r++) {                        // halo 1: U_3 of the last slice of rank r-1 -> rank r
         const int q = (r + P - 1) % P;
         const cplx* src = c->links[q] + (long long)(3 * NC) * c->Vl + (c->Vl - c->S);
-        slab_copy2d(c->halo_u[r], (size_t)c->S * sizeof(cplx), src, (size_t)c->Vl * sizeof(cplx), (size_t)c->S * sizeof(cplx), NC, c->stream);
-        c->copies++;
+        slab_exchange(c, "U_3 halo", c->halo_u[r], (size_t)c->S * sizeof(cplx), src, (size_t)c->Vl * sizeof(cplx), (size_t)c->S * sizeof(cplx), NC);
     }
     for (int r = 0; r < P; r++) {
         k_delta_slab<NC><<<(unsigned)c->nb, 128, 0, c->stream>>>(c->links[r], c->halo_u[r], c->field[r], c->partials + (size_t)r * c->nb, c->Gl, c->ctl);
@@ -122,8 +133,7 @@ template <int NC> void slab_body(lgf_slab_ctx* c, double half_alpha) {
     }
     for (int r = 0; r < P; r++) {                        // halo 2: X of the first slice of rank r+1 -> rank r
         const int q = (r + 1) % P;
-        slab_copy2d(c->halo_x[r], (size_t)c->S * sizeof(cplx), c->field[q], (size_t)c->Vl * sizeof(cplx), (size_t)c->S * sizeof(cplx), 4, c->stream);
-        c->copies++;
+        slab_exchange(c, "X halo", c->halo_x[r], (size_t)c->S * sizeof(cplx), c->field[q], (size_t)c->Vl * sizeof(cplx), (size_t)c->S * sizeof(cplx), 4);
     }
     for (int r = 0; r < P; r++) {                        // S3 + S4
         if (Gl.L[0] <= 32) k_update_slab<NC, 32><<<(unsigned)(c->Vl / 32), 128, 0, c->stream>>>(c->links[r], c->field[r], c->halo_x[r], Gl, half_alpha, c->ctl, r == 0);
@@ -135,10 +145,19 @@ template <int NC> void slab_body(lgf_slab_ctx* c, double half_alpha) {
 lgf_status slab_run(lgf_slab_ctx* c, double alpha, double tol, int max_iter, bool poll) {
     lgf_status st = slab_reset_ctl(c, tol, max_iter);
     if (st != LGF_OK) return st;
+    c->copy_err = cudaSuccess; c->copy_what = "";
     long long left = (long long)max_iter + 1;
     while (left > 0) {
         const int nb = (int)(left < 8 ? left : 8);
         for (int i = 0; i < nb; i++) { if (c->NC == 6) slab_body<6>(c, 0.5 * alpha); else slab_body<9>(c, 0.5 * alpha); }
+        if (c->copy_err != cudaSuccess) {        // a halo never arrived: the links are no longer a gauge copy of the input
+            char b[256];
+            snprintf(b, sizeof b, "inter-rank copy (%s) failed: %s", c->copy_what, cudaGetErrorString(c->copy_err));
+            c->err = b;
+            cudaStreamSynchronize(c->stream); cudaGetLastError();
+            c->loaded = false;
+            return LGF_ERR_CUDA;
+        }
         SCK(cudaGetLastError());
         left -= nb;
         if (poll || left == 0) {
@@ -165,19 +184,23 @@ void lgf_destroy_sharded(lgf_slab_ctx* c) {
 }
 
 lgf_status lgf_create_sharded(const int dims[4], int n_ranks, lgf_storage s, lgf_slab_ctx** out) {
-    if (!dims || !out) return LGF_ERR_INVALID_ARG;
+    g_slab_create_err.clear();                   // lgf_last_error_sharded(NULL): the text of this thread's last failed create
+    auto refuse = [&](lgf_status st, const char* why) { g_slab_create_err = why; return st; };
+    if (!dims || !out) return refuse(LGF_ERR_INVALID_ARG, "lgf_create_sharded: dims or out is NULL");
     *out = nullptr;
-    if (s != LGF_STORE_12 && s != LGF_STORE_18) return LGF_ERR_INVALID_ARG;
-    if (n_ranks < 1 || n_ranks > SLAB_MAX_RANKS || (n_ranks & (n_ranks - 1))) return LGF_ERR_INVALID_ARG;
-    for (int k = 0; k < 4; k++) if (dims[k] < 1) return LGF_ERR_INVALID_ARG;
+    if (s != LGF_STORE_12 && s != LGF_STORE_18) return refuse(LGF_ERR_INVALID_ARG, "lgf_create_sharded: storage is not LGF_STORE_12 or LGF_STORE_18");
+    if (n_ranks < 1 || n_ranks > SLAB_MAX_RANKS || (n_ranks & (n_ranks - 1))) return refuse(LGF_ERR_INVALID_ARG, "lgf_create_sharded: n_ranks must be a power of two between 1 and 16");
+    for (int k = 0; k < 4; k++) if (dims[k] < 1) return refuse(LGF_ERR_INVALID_ARG, "lgf_create_sharded: an extent is smaller than 1");
     int lg[4];
-    if (!dims_ok(dims, lg)) return LGF_ERR_UNSUPPORTED;
+    if (!dims_ok(dims, lg)) return refuse(LGF_ERR_UNSUPPORTED, "lgf_create_sharded: extents must be powers of two, 4 <= L <= 128, L0*L1 <= 4096, L2*L3 <= 4096");
     int lgP = 0; while ((1 << lgP) < n_ranks) lgP++;
-    if (lgP > lg[3] || lgP > lg[1] || dims[0] > 64) return LGF_ERR_UNSUPPORTED;      // every rank needs a time slice and an x1 row; x0 rows of <= 64 sites
+    if (lgP > lg[3] || lgP > lg[1] || dims[0] > 64)      // every rank needs a time slice and an x1 row; x0 rows of <= 64 sites
+        return refuse(LGF_ERR_UNSUPPORTED, "lgf_create_sharded: n_ranks must not exceed L1 or L3, and L0 must be at most 64");
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return LGF_ERR_CUDA;   // no CPU fallback
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return refuse(LGF_ERR_CUDA, "lgf_create_sharded: no CUDA device (there is no CPU fallback)"); }
     lgf_slab_ctx* c = new (std::nothrow) lgf_slab_ctx();
-    if (!c) return LGF_ERR_OOM;
+    if (!c) return refuse(LGF_ERR_OOM, "lgf_create_sharded: host allocation of the context failed");
+    c->copy_err = cudaSuccess; c->copy_what = "";
     c->P = n_ranks; c->lgP = lgP; c->NC = (s == LGF_STORE_12) ? 6 : 9;
     for (int r = 0; r < SLAB_MAX_RANKS; r++) c->ws[r] = nullptr;
     c->shared = nullptr; c->h_ctl = nullptr; c->stream = nullptr; c->loaded = false; c->launches = 0; c->copies = 0;
@@ -186,7 +209,15 @@ lgf_status lgf_create_sharded(const int dims[4], int n_ranks, lgf_storage s, lgf
     slab_geom(c->Gt, lg[0], lg[1] - lgP, lg[2], lg[3], 4);
     c->Vl = c->Gl.V; c->S = 1LL << c->Gl.sh[3];
     c->nb = (int)(c->Vl / 128);
-    auto fail = [&](lgf_status st) { lgf_destroy_sharded(c); return st; };
+    auto fail = [&](lgf_status st) {
+        const cudaError_t e = cudaGetLastError();
+        g_slab_create_err = !c->err.empty() ? c->err
+            : st == LGF_ERR_OOM ? std::string("lgf_create_sharded: device or pinned-host allocation failed")
+            : st == LGF_ERR_UNSUPPORTED ? std::string("lgf_create_sharded: a rank's slab is too small (< 128 sites) or its FFT tile exceeds shared memory")
+            : std::string("lgf_create_sharded: CUDA set-up failed") + (e != cudaSuccess ? std::string(": ") + cudaGetErrorString(e) : std::string());
+        lgf_destroy_sharded(c);
+        return st;
+    };
     if (c->nb < 1) return fail(LGF_ERR_UNSUPPORTED);
     if (cudaStreamCreateWithFlags(&c->stream, cudaStreamNonBlocking) != cudaSuccess) return fail(LGF_ERR_CUDA);
     // per-rank workspaces
@@ -346,6 +377,6 @@ lgf_status lgf_sharded_traffic(lgf_slab_ctx* c, long long out[5]) {
     out[4] = c->copies;
     return LGF_OK;
 }
-const char* lgf_last_error_sharded(lgf_slab_ctx* c) { return c ? c->err.c_str() : ""; }
+const char* lgf_last_error_sharded(lgf_slab_ctx* c) { return c ? c->err.c_str() : g_slab_create_err.c_str(); }
 
 }  // extern "C"

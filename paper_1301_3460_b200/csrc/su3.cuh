@@ -135,7 +135,10 @@ __device__ __forceinline__ void rotate_link(const cplx (&g)[9], const cplx (&u)[
 // S2b filter weight scale / p2 (scale = p2max / V), 0 for the zero mode.  p2 lies in [4 sin^2(pi/128), 16]: no special
 // cases, so the division is a reciprocal seed (MUFU.RCP64H, ~20 bits) and two Newton steps -- within 2 ulp of the IEEE
 // quotient at a quarter of its instructions (the IEEE fp64 division was a quarter of pass B's instruction stream).
-// Every pass-B kernel, generic or compile-time-sized, uses this one function, so all kernel selections agree bit for bit.
+// Every pass-B kernel, generic or compile-time-sized, takes the weight from this one function.  Its argument is not summed
+// in one order everywhere (k_tb_mid forms p2 as ((s0+s1)+s2)+s3, k_fft23_mid as (s0+s1)+(s2+s3)), so two kernel
+// selections can differ in the last bit of p2 and hence of the weight: they agree to rounding, not bit for bit (the
+// parity tests bound X at 1e-13 relative for every selection).
 __device__ __forceinline__ double filter_weight(double scale, double p2) {
     if (!(p2 > 0.0)) return 0.0;
     double r;

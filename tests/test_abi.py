@@ -81,6 +81,43 @@ def test_argument_errors_before_any_device_work():
     L.lgf_destroy(None)
 
 
+def test_create_error_text_belongs_to_the_last_create():
+    """lgf_last_error(NULL) describes the LAST lgf_create* of the calling thread on every failing path -- argument
+    errors and fp32 contexts included -- and never a stale text of an earlier one."""
+    L = lgf.lib()
+    h = C.c_void_p()
+    d = lambda *v: (C.c_int * 4)(*v)
+    assert L.lgf_create(d(8, 8, 6, 8), lgf.LGF_FP64, 12, C.byref(h)) == lgf.LGF_ERR_UNSUPPORTED
+    assert b"powers of two" in L.lgf_last_error(None)
+    assert L.lgf_create(d(8, 8, 8, 8), 7, 12, C.byref(h)) == lgf.LGF_ERR_INVALID_ARG
+    assert b"precision" in L.lgf_last_error(None)                        # not the text of the call before
+    assert L.lgf_create(d(8, 8, 8, 8), lgf.LGF_FP64, 13, C.byref(h)) == lgf.LGF_ERR_INVALID_ARG
+    assert b"storage" in L.lgf_last_error(None)
+    assert L.lgf_create(d(8, 8, 6, 8), lgf.LGF_FP32, 12, C.byref(h)) == lgf.LGF_ERR_UNSUPPORTED
+    assert b"powers of two" in L.lgf_last_error(None)                    # forwarded from the fp32 translation unit
+    assert L.lgf_create_ex(d(8, 8, 8, 8), lgf.LGF_MIXED, 12, None, 0, None, C.byref(h)) == lgf.LGF_ERR_INVALID_ARG
+    assert b"workspace" in L.lgf_last_error(None)
+    st = L.lgf_create(d(8, 8, 8, 8), lgf.LGF_FP64, 12, C.byref(h))
+    if st == lgf.LGF_OK:                                                 # a device is present: a success leaves no text
+        assert L.lgf_last_error(None) == b""
+        L.lgf_destroy(h)
+    else:
+        assert st == lgf.LGF_ERR_CUDA and b"no CUDA device" in L.lgf_last_error(None)
+
+
+def test_sharded_create_failures_leave_a_text():
+    L = lgf.lib()
+    h = C.c_void_p()
+    d = lambda *v: (C.c_int * 4)(*v)
+    assert L.lgf_create_sharded(d(8, 8, 8, 8), 3, 12, C.byref(h)) == lgf.LGF_ERR_INVALID_ARG
+    assert b"power of two" in L.lgf_last_error_sharded(None)
+    assert L.lgf_create_sharded(d(16, 4, 16, 16), 8, 12, C.byref(h)) == lgf.LGF_ERR_UNSUPPORTED
+    assert b"n_ranks must not exceed" in L.lgf_last_error_sharded(None)
+    with pytest.raises(lgf.LgfError) as e:
+        lgf.ShardedGaugeFixer((16, 16, 16, 16), 3)
+    assert "power of two" in str(e.value)
+
+
 def test_no_cpu_fallback_without_a_device():
     import torch
     if torch.cuda.is_available():
