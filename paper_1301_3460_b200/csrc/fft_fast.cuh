@@ -22,11 +22,6 @@
 #ifndef LGF_FA_MINB_DELTA
 #define LGF_FA_MINB_DELTA 2
 #endif
-// 1: pass A runs its middle stages as two 8-point-or-smaller stages instead of one 16-point register block (fewer
-// registers per thread, one more shared-memory round trip)
-#ifndef LGF_FA_NOBLOCK16
-#define LGF_FA_NOBLOCK16 0
-#endif
 // 1: pass A prefetches the own links of a thread's next site into L2 (prefetch.global.L2) before it works on the current
 // one.  Measured on B200 at 32^4: fp32 61.5 against 65.8 us, fp64 115.5 against 106 us (the extra L1TEX requests cost
 // more than the latency they save) -- so it is on in the fp32 build only.
@@ -149,7 +144,7 @@ __device__ __forceinline__ void plane_middle(cplx* __restrict__ t, const cplx* _
     using PA = Plan2<LGA, false>;
     using PB = Plan2<LGB, true>;
     constexpr int LA = PA::L, LB = PB::L, S = LA + 1, SC = S * LB;
-    if constexpr (PA::R2 * PB::R1 <= 16 && !(LGF_FA_NOBLOCK16 && !INV)) {
+    if constexpr (PA::R2 * PB::R1 <= 16) {
         // lanes run over jb (rows, odd stride S: conflict-free), then over the a-blocks
         constexpr int NW = NCOMP * PA::R1 * PB::R2;
 #pragma unroll

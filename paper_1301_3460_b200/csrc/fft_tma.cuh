@@ -75,9 +75,15 @@ template <int LG2, int LG3, int LGC> struct TmaMidGeom {
 // of them, so 8 warps is what an SM holds; with ONE group the FP64 dependency stalls are exposed: 60.6 us at 32^4, ncu
 // "wait" 1.7 cycles per issue at 4 warps per SM).  The CTA's tiles form a sequence j = 0, 1, 2, ...; tile j is transformed
 // by group j mod 2, in place, in buffer j mod 3.  When a group has finished tile j (phase 3 has read the buffer), its
-// thread 0 starts the copy of tile j + 3 into the same buffer and arms the buffer's mbarrier; the group that transforms
-// tile j + 3 waits on that barrier.  So each group always finds its next tile already in shared memory, the copies cost
+// thread 0 starts the copy of tile j + 3 into the same buffer and arms that tile's mbarrier; the group that transforms
+// tile j + 3 waits on it.  So each group always finds its next tile already in shared memory, the copies cost
 // neither registers nor issue slots, and the two groups' phases interleave on the FP64 pipe.
+// Barriers: tile j uses full[j mod 6] in phase j / 6 -- one barrier per (buffer, consuming group) pair, as 3 is odd and
+// a buffer's consecutive tiles alternate between the groups.  Each barrier is therefore waited on by ONE group, phase after
+// phase, and re-armed (tile j + 6) only after that group has consumed tile j: when the group arrives for phase k it has
+// itself seen phase k - 1 complete, so a parity wait cannot be satisfied by an older phase.  (With one barrier per
+// buffer the group that takes tile j + 3 had never waited for tile j, and its parity-1 wait would have passed on a
+// barrier still in phase 0 had tile j not landed yet -- excluded only by timing.)  k_tr_mid uses the same scheme.
 // Bank conflicts: the dense TMA layout makes lanes (i0, i3) and (i0, i3 + 1) of an axis-2 line collide (C0 = 4: 2-way) on
 // the phase-1 reads only; phase 1 writes element m of line (i0, i3) at position m ^ (i3 & 1) -- inside the same line -- which
 // makes its own writes, both accesses of phase 2 and the reads of phase 3 conflict-free.
@@ -87,7 +93,7 @@ __global__ void __launch_bounds__(NT, 1) k_tb_mid(const __grid_constant__ CUtens
     static_assert(NT == 256, "two groups of 128 threads");
     pdl_enter();
     __shared__ int s_done;
-    __shared__ __align__(8) uint64_t full[3];
+    __shared__ __align__(8) uint64_t full[6];          // one per (buffer j mod 3, consuming group j mod 2): index j mod 6
     pass_b_entry<NT>(partials, fa, ctl, &s_done);
     using TG = TmaMidGeom<LG2, LG3, LGC>;
     constexpr int L2 = TG::L2, L3 = TG::L3, C0 = TG::C0, TILE = TG::TILE, GT = 128;
@@ -106,11 +112,12 @@ __global__ void __launch_bounds__(NT, 1) k_tb_mid(const __grid_constant__ CUtens
         const int chunk = tile & ((1 << lgChunks) - 1);
         const int x1 = (tile >> lgChunks) & (G.L[1] - 1);
         const int comp = tile >> (lgChunks + G.lg[1]);
-        mbar_expect_tx(&full[b], TG::TILE_BYTES);
-        tma_load_5d(bufs + b * TILE, &tmap, &full[b], chunk << (LGC + 1), x1, 0, 0, comp);
+        mbar_expect_tx(&full[j % 6], TG::TILE_BYTES);
+        tma_load_5d(bufs + b * TILE, &tmap, &full[j % 6], chunk << (LGC + 1), x1, 0, 0, comp);
     };
     if (threadIdx.x == 0) {
-        mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_init(&full[2], 1);
+#pragma unroll
+        for (int i = 0; i < 6; i++) mbar_init(&full[i], 1);
         mbar_init_fence();
         // a copy in flight must never outlive its CTA: nothing is issued when the run is already over
         if (!s_done)
@@ -128,7 +135,7 @@ __global__ void __launch_bounds__(NT, 1) k_tb_mid(const __grid_constant__ CUtens
         const int comp = tile >> (lgChunks + G.lg[1]);
         cplx* gbase = field + (long long)comp * G.V + (chunk << LGC) + ((long long)x1 << G.sh[1]);
         cplx* tl = bufs + b * TILE;
-        mbar_wait(&full[b], (j / 3) & 1);
+        mbar_wait(&full[j % 6], (j / 6) & 1);
         // phase 1: lines along axis 2, one per (i0, i3): forward, in place (element m -> position m ^ (i3 & 1))
 #pragma unroll 1
         for (int ln = g.tid; ln < C0 * L3; ln += GT) {
@@ -432,7 +439,7 @@ __global__ void __launch_bounds__(NT, 1) k_tr_mid(const __grid_constant__ CUtens
     static_assert(NT == 512, "two groups of 256 threads");
     pdl_enter();
     __shared__ int s_done;
-    __shared__ __align__(8) uint64_t full[3];
+    __shared__ __align__(8) uint64_t full[6];          // one per (buffer j mod 3, consuming group j mod 2): index j mod 6
     pass_b_entry<NT>(partials, fa, ctl, &s_done);
     using TG = TmaRingGeom<LG2, LG3, LGC>;
     constexpr int L2 = TG::L2, L3 = TG::L3, C0 = TG::C0, TILE = TG::TILE, GT = 256;
@@ -454,11 +461,12 @@ __global__ void __launch_bounds__(NT, 1) k_tr_mid(const __grid_constant__ CUtens
         const int chunk = tile & ((1 << lgChunks) - 1);
         const int x1 = (tile >> lgChunks) & (G.L[1] - 1);
         const int comp = tile >> (lgChunks + G.lg[1]);
-        mbar_expect_tx(&full[b], TG::TILE_BYTES);
-        tma_load_5d(bufs + b * TILE, &tmap, &full[b], chunk << (LGC + 1), x1, 0, 0, comp);
+        mbar_expect_tx(&full[j % 6], TG::TILE_BYTES);
+        tma_load_5d(bufs + b * TILE, &tmap, &full[j % 6], chunk << (LGC + 1), x1, 0, 0, comp);
     };
     if (threadIdx.x == 0) {
-        mbar_init(&full[0], 1); mbar_init(&full[1], 1); mbar_init(&full[2], 1);
+#pragma unroll
+        for (int i = 0; i < 6; i++) mbar_init(&full[i], 1);
         mbar_init_fence();
         if (!s_done)
             for (int j = 0; j < 3 && j < n_seq; j++) issue(j);
@@ -475,7 +483,7 @@ __global__ void __launch_bounds__(NT, 1) k_tr_mid(const __grid_constant__ CUtens
         const int comp = tile >> (lgChunks + G.lg[1]);
         cplx* tbuf = bufs + b * TILE;
         const double s01 = T.s[0][(chunk << LGC) + i0] + T.s[1][x1];
-        mbar_wait(&full[b], (j / 3) & 1);
+        mbar_wait(&full[j % 6], (j / 6) & 1);
         if (grp == 0) mid_tile_stages<LG2, LG3, LGC, GT, 1>(tbuf + i0, tw2, tw3, s2, s3, s01, scale, gtid);
         else mid_tile_stages<LG2, LG3, LGC, GT, 2>(tbuf + i0, tw2, tw3, s2, s3, s01, scale, gtid);
         fence_proxy_async();                             // the generic-proxy writes above, before the async proxy reads them
@@ -511,32 +519,27 @@ __global__ void __launch_bounds__(NT, 1) k_tr_mid(const __grid_constant__ CUtens
 // 97.3 us; walking the update downwards instead gives pass A the same hits but costs the update its own on X).
 struct LinkMaps { CUtensorMap own, nb, row; };
 
-// sites per stage: 128 (a thread = one site, each group owns one buffer; default) or 64 (two threads per site -- one takes
-// the site's own four links, the other the four backward neighbours, summed by a lane-pair shuffle -- and each group
-// owns TWO buffers, so that its next stage is landing while it works on the current one).  Measured at 32^4: 98.6-99.4
-// against 100.6-101.7 us: the finer pipeline does not pay, because what is exposed is not the per-buffer load/compute
+// Sites per stage: 128 -- a thread = one site, each group owns one buffer.  A variant with 64-site stages (two threads per
+// site, summed by a lane-pair shuffle, two buffers per group so that a group's next stage lands while it works on the
+// current one) was built, measured and removed in round 3 (history: commit d75b9c7): at 32^4 98.6-99.4 against
+// 100.6-101.7 us.  The finer pipeline does not pay, because what is exposed is not the per-buffer load/compute
 // cycle but the transform of the finished tile: leaving phases out gives 78.5 us for the staged copies alone (0.92 of the
 // measured HBM peak on the kernel's 470 MB), 90.6 with the transform, 100 with S1 as well -- while all warps transform a
 // tile the 150 KB of stage buffers fill up and the SM's share of HBM idles for the rest of the phase; a second tile or
 // deeper buffers do not fit (222 KB used), and pulling stages further ahead into L2 with cp.async.bulk.prefetch.tensor
 // made it slower at every distance tried (102.5 at one stage ahead of the window, 119 at a plane ahead).
-#ifndef LGF_TA_SS
-#define LGF_TA_SS 128
-#endif
+constexpr int TA_SS = 128;
 template <int LG0, int LG1, int NC> struct TmaPlaneGeom {
     static constexpr int L0 = 1 << LG0, L1 = 1 << LG1, S = L0 + 1, SC = S * L1, nP = L0 * L1;
-    static constexpr int SS = LGF_TA_SS;                             // sites per stage
-    static constexpr int TPS = 128 / SS;                             // threads per site
-    static constexpr int NBG = TPS;                                  // stage buffers per thread group
+    static constexpr int SS = TA_SS;                                 // sites per stage = threads per group
     static constexpr int NST = nP / SS;                              // stages per plane
     static constexpr int OWN = 4 * NC * SS, NB = NC * SS, ROW = NC * L0;      // complex numbers
     static constexpr int STAGE = OWN + 2 * NB + ROW;
     static constexpr unsigned STAGE_BYTES = STAGE * sizeof(cplx);
-    static_assert(SS == 64 || SS == 128, "one or two threads per site");
     static_assert(SS % L0 == 0, "a stage is whole x0 rows");
     static_assert(NST >= 2 && NST % 2 == 0, "each group takes every other stage");
     static_assert((OWN * sizeof(cplx)) % 128 == 0 && (NB * sizeof(cplx)) % 128 == 0 && (STAGE * sizeof(cplx)) % 128 == 0, "TMA destinations are 128-byte aligned");
-    static constexpr size_t SMEM = (size_t)(2 * NBG * STAGE + 4 * SC + L0 + L1) * sizeof(cplx) + 128;
+    static constexpr size_t SMEM = (size_t)(2 * STAGE + 4 * SC + L0 + L1) * sizeof(cplx) + 128;
 };
 
 __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2) {
@@ -550,12 +553,6 @@ template <int NC> __device__ __forceinline__ void load_link_smem(const cplx* __r
     if (NC == 6) third_row(u);
 }
 
-template <int NC> __device__ __forceinline__ void load_link_smem_rt(const cplx* __restrict__ p, int stride, cplx (&u)[9]) {
-#pragma unroll
-    for (int c = 0; c < NC; c++) u[c] = p[c * stride];
-    if (NC == 6) third_row(u);
-}
-
 template <int LG0, int LG1, int NC, int NT>
 __global__ void __launch_bounds__(NT, 1) k_ta_delta_fwd(const __grid_constant__ LinkMaps maps, cplx* __restrict__ field, double2* __restrict__ partials,
                                                         Geom G, FftTables T, const Ctl* __restrict__ ctl, int n_planes) {
@@ -563,12 +560,13 @@ __global__ void __launch_bounds__(NT, 1) k_ta_delta_fwd(const __grid_constant__ 
     pdl_enter();
     if (ctl->done) return;                               // uniform over the grid; nothing has been issued yet
     using PG = TmaPlaneGeom<LG0, LG1, NC>;
-    constexpr int L0 = PG::L0, L1 = PG::L1, S = PG::S, SC = PG::SC, SS = PG::SS, NST = PG::NST, GT = 128, TPS = PG::TPS, NBG = PG::NBG;
-    __shared__ __align__(8) uint64_t full[2 * NBG];
+    constexpr int L0 = PG::L0, L1 = PG::L1, S = PG::S, SC = PG::SC, SS = PG::SS, NST = PG::NST, GT = 128;
+    static_assert(SS == GT, "a thread of a group = one site of its stage");
+    __shared__ __align__(8) uint64_t full[2];            // one per group: only that group waits on it, phase after phase
     __shared__ double red[64];
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx* stage = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u));      // [2 NBG][STAGE]
-    cplx* tile = stage + 2 * NBG * PG::STAGE;
+    cplx* stage = reinterpret_cast<cplx*>(smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u));      // [2][STAGE]
+    cplx* tile = stage + 2 * PG::STAGE;
     cplx* tw0 = tile + 4 * SC;
     cplx* tw1 = tw0 + L0;
     for (int i = threadIdx.x; i < L0; i += NT) tw0[i] = T.tw[0][i];
@@ -576,9 +574,9 @@ __global__ void __launch_bounds__(NT, 1) k_ta_delta_fwd(const __grid_constant__ 
     const int n_seq = (n_planes - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;      // planes of this CTA
     const int n_stage = n_seq * NST;
     // Stage t of this CTA: plane blockIdx.x + (t / NST) gridDim.x, sites [(t % NST) SS, ...).  Group g = t & 1 takes it as
-    // its k-th stage, k = t >> 1, in its buffer k mod NBG.
+    // its k-th stage, k = t >> 1, in its own buffer.
     auto issue = [&](int t) {
-        const int plane = n_planes - 1 - ((int)blockIdx.x + (t / NST) * (int)gridDim.x), s = t % NST, b = (t & 1) * NBG + ((t >> 1) % NBG);
+        const int plane = n_planes - 1 - ((int)blockIdx.x + (t / NST) * (int)gridDim.x), s = t % NST, b = t & 1;
         const int x2 = plane & (G.L[2] - 1), x3 = plane >> G.lg[2];
         const int pl2 = ((x2 + G.L[2] - 1) & (G.L[2] - 1)) + (x3 << G.lg[2]);
         const int pl3 = x2 + (((x3 + G.L[3] - 1) & (G.L[3] - 1)) << G.lg[2]);
@@ -592,19 +590,15 @@ __global__ void __launch_bounds__(NT, 1) k_ta_delta_fwd(const __grid_constant__ 
         tma_load_3d(d + PG::OWN + 2 * PG::NB, &maps.row, &full[b], rowb, plane, NC);
     };
     if (threadIdx.x == 0) {
-#pragma unroll
-        for (int b = 0; b < 2 * NBG; b++) mbar_init(&full[b], 1);
+        mbar_init(&full[0], 1); mbar_init(&full[1], 1);
         mbar_init_fence();
-        for (int t = 0; t < 2 * NBG && t < n_stage; t++) issue(t);
+        for (int t = 0; t < 2 && t < n_stage; t++) issue(t);
     }
     __syncthreads();
     const int grp = threadIdx.x / GT;
     const Grp g{(int)threadIdx.x % GT, 1 + grp};
     const Grp all{(int)threadIdx.x, 0};
-    // a thread's site of the stage and, with two threads per site, its half: 0 = the own links, 1 = the backward neighbours
-    const int lane = threadIdx.x & 31;
-    const int j = (TPS == 1) ? g.tid : ((g.tid >> 5) * 16 + (lane & 15));
-    const int h = (TPS == 1) ? 0 : (lane >> 4);
+    const int j = g.tid;                                               // a thread's site of the stage
     const int jx = j & (L0 - 1), jr = j >> LG0;                        // x0, row inside the stage
     const int jm0 = (j & ~(L0 - 1)) | ((jx + L0 - 1) & (L0 - 1));      // x - 0 (periodic inside the row)
 #pragma unroll 1
@@ -613,69 +607,37 @@ __global__ void __launch_bounds__(NT, 1) k_ta_delta_fwd(const __grid_constant__ 
         double th = 0, fs = 0;
 #pragma unroll 1
         for (int s = grp; s < NST; s += 2) {
-            const int t = q * NST + s, k = t >> 1, b = grp * NBG + (k % NBG);
+            const int t = q * NST + s, k = t >> 1, b = grp;
             const cplx* own = stage + b * PG::STAGE;
             const cplx* nb2 = own + PG::OWN;
             const cplx* nb3 = nb2 + PG::NB;
             const cplx* row1 = nb3 + PG::NB;
-            mbar_wait(&full[b], (k / NBG) & 1);
+            mbar_wait(&full[b], k & 1);
             cplx d01 = mk(0, 0), d02 = mk(0, 0), d12 = mk(0, 0);
             real i0 = 0, i1 = 0, i2 = 0, retr = 0;
             cplx u[9];
-            if constexpr (TPS == 1) {
 #pragma unroll
-                for (int mu = 0; mu < 4; mu++) {                       // the site's own links: - U_mu(x)
-                    load_link_smem<NC>(own + mu * NC * SS + j, SS, u);
-                    retr += u[0].x + u[4].x + u[8].x;
-                    acc_link(u, real(-1), d01, d02, d12, i0, i1, i2);
-                }
-                load_link_smem<NC>(own + jm0, SS, u);                  // the backward neighbours: + U_mu(x-mu)
-                acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
-                load_link_smem_rt<NC>(jr == 0 ? row1 + jx : own + NC * SS + j - L0, jr == 0 ? L0 : SS, u);
-                acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
-                load_link_smem<NC>(nb2 + j, SS, u);
-                acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
-                load_link_smem<NC>(nb3 + j, SS, u);
-                acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
-            } else {
-                // One instruction stream for both halves of a warp: four links through per-lane pointers.  Half 0: the
-                // site's own U_mu(x), mu = 0..3, sign -1, and Re Tr for F.  Half 1: U_0(x-0), U_1(x-1), U_2(x-2), U_3(x-3), sign +1.
-                const cplx* p0 = h ? own + jm0 : own + j;
-                const cplx* p1 = h ? (jr == 0 ? row1 + jx : own + NC * SS + j - L0) : own + NC * SS + j;
-                const int st1 = (h && jr == 0) ? L0 : SS;
-                const cplx* p2 = h ? nb2 + j : own + 2 * NC * SS + j;
-                const cplx* p3 = h ? nb3 + j : own + 3 * NC * SS + j;
-                const real sg = h ? real(1) : real(-1), rf = h ? real(0) : real(1);
-                load_link_smem<NC>(p0, SS, u);
-                retr = fma(rf, u[0].x + u[4].x + u[8].x, retr);
-                acc_link(u, sg, d01, d02, d12, i0, i1, i2);
-                load_link_smem_rt<NC>(p1, st1, u);
-                retr = fma(rf, u[0].x + u[4].x + u[8].x, retr);
-                acc_link(u, sg, d01, d02, d12, i0, i1, i2);
-                load_link_smem<NC>(p2, SS, u);
-                retr = fma(rf, u[0].x + u[4].x + u[8].x, retr);
-                acc_link(u, sg, d01, d02, d12, i0, i1, i2);
-                load_link_smem<NC>(p3, SS, u);
-                retr = fma(rf, u[0].x + u[4].x + u[8].x, retr);
-                acc_link(u, sg, d01, d02, d12, i0, i1, i2);
+            for (int mu = 0; mu < 4; mu++) {                           // the site's own links: - U_mu(x)
+                load_link_smem<NC>(own + mu * NC * SS + j, SS, u);
+                retr += u[0].x + u[4].x + u[8].x;
+                acc_link(u, real(-1), d01, d02, d12, i0, i1, i2);
             }
-            if (TPS == 2) {                                            // the two halves of a site sit 16 lanes apart
-                d01.x += __shfl_xor_sync(0xffffffffu, d01.x, 16); d01.y += __shfl_xor_sync(0xffffffffu, d01.y, 16);
-                d02.x += __shfl_xor_sync(0xffffffffu, d02.x, 16); d02.y += __shfl_xor_sync(0xffffffffu, d02.y, 16);
-                d12.x += __shfl_xor_sync(0xffffffffu, d12.x, 16); d12.y += __shfl_xor_sync(0xffffffffu, d12.y, 16);
-                i0 += __shfl_xor_sync(0xffffffffu, i0, 16); i1 += __shfl_xor_sync(0xffffffffu, i1, 16); i2 += __shfl_xor_sync(0xffffffffu, i2, 16);
-            }
+            load_link_smem<NC>(own + jm0, SS, u);                      // the backward neighbours: + U_mu(x-mu)
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
+            load_link_smem<NC>(jr == 0 ? row1 + jx : own + NC * SS + j - L0, jr == 0 ? L0 : SS, u);
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
+            load_link_smem<NC>(nb2 + j, SS, u);
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
+            load_link_smem<NC>(nb3 + j, SS, u);
+            acc_link(u, real(1), d01, d02, d12, i0, i1, i2);
             const real tr3 = real(2.0 / 3.0) * (i0 + i1 + i2);
             const real e0 = real(2) * i0 - tr3, e1 = real(2) * i1 - tr3, e2 = real(2) * i2 - tr3;
             const int o = jx + (s * (SS / L0) + jr) * S;
-            if (h == 0) {
-                th += (double)(real(2) * (cnorm2(d01) + cnorm2(d02) + cnorm2(d12)) + e0 * e0 + e1 * e1 + e2 * e2);
-                fs += (double)retr;
-                tile[o] = d01; tile[SC + o] = d02;
-                if (TPS == 1) { tile[2 * SC + o] = d12; tile[3 * SC + o] = mk(e0, e1); }
-            } else { tile[2 * SC + o] = d12; tile[3 * SC + o] = mk(e0, e1); }
+            th += (double)(real(2) * (cnorm2(d01) + cnorm2(d02) + cnorm2(d12)) + e0 * e0 + e1 * e1 + e2 * e2);
+            fs += (double)retr;
+            tile[o] = d01; tile[SC + o] = d02; tile[2 * SC + o] = d12; tile[3 * SC + o] = mk(e0, e1);
             gsync<GT>(g);                                              // every thread of the group has read the buffer
-            if (g.tid == 0 && t + 2 * NBG < n_stage) issue(t + 2 * NBG);
+            if (g.tid == 0 && t + 2 < n_stage) issue(t + 2);
         }
         group_sum2<NT>(th, fs, red, all);                              // its barrier also completes the tile
         if (threadIdx.x == 0) partials[plane] = make_double2(th, fs);

@@ -527,7 +527,7 @@ bool make_link_tensor_maps(lgf_ctx* c) {
     const cuuint64_t strides[2] = {esz * plane, esz * (cuuint64_t)G.V};
     const cuuint32_t estr[3] = {1, 1, 1};
     const CUtensorMapDataType dt = sizeof(real) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-    const cuuint32_t boxes[3][3] = {{2 * LGF_TA_SS, 1, (cuuint32_t)(4 * c->NC)}, {2 * LGF_TA_SS, 1, (cuuint32_t)c->NC}, {(cuuint32_t)(2 * G.L[0]), 1, (cuuint32_t)c->NC}};
+    const cuuint32_t boxes[3][3] = {{2 * TA_SS, 1, (cuuint32_t)(4 * c->NC)}, {2 * TA_SS, 1, (cuuint32_t)c->NC}, {(cuuint32_t)(2 * G.L[0]), 1, (cuuint32_t)c->NC}};
     CUtensorMap* maps[3] = {&c->tm_links.own, &c->tm_links.nb, &c->tm_links.row};
     for (int k = 0; k < 3; k++)
         if (reinterpret_cast<EncodeTiledFn>(fn)(maps[k], dt, 3, c->links, dims, strides, boxes[k], estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
