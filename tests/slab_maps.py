@@ -1,7 +1,8 @@
 """Index maps of the slab decomposition (include/lgf.h lgf_*_sharded; kernels k_slab_scatter / k_slab_gather of
 csrc/slab.cuh), as plain integer arithmetic.  No arithmetic of the method is here: these are the owner and position
 maps a rank needs to pack what it sends and to place what it receives when the ranks are separate processes
-(torch.distributed all_to_all over NCCL between GPUs; over gloo in tests/test_slab_maps.py).
+(torch.distributed all_to_all over NCCL between GPUs; over gloo in tests/test_slab_maps.py).  Test infrastructure: it
+lives under tests/ because only the tests use it -- the library's sharded context runs its ranks inside one process.
 
 Lattice (L0, L1, L2, L3), site x = x0 + L0 (x1 + L1 (x2 + L2 x3)); P ranks, P | L1 and P | L3.
   slab layout        rank r owns x3 in [r L3/P, (r+1) L3/P): local array [L3/P][L2][L1][L0]       (x0 fastest)

@@ -236,12 +236,12 @@ def test_trajectory_C2b_headline_config():
 def test_trajectory_C2a_C2c(name):
     """BASELINE.json configs[2], eps = 0.25 and 0.45: the other two of the three seeded 32^4 ensembles that stand in
     for the paper's three beta values; default path and the store-g path."""
-    check_trajectory(name, fft_mode=1, variants=((0, 1, 1, 1), (1, 0, 0, 0)))
+    check_trajectory(name, fft_mode=1, checkpoints=(10, 60), variants=((0, 1, 1, 1), (1, 0, 0, 0)))
 
 
 def test_trajectory_C3_anisotropic():
     """BASELINE.json configs[3], 32^3 x 64: uneven FFT axes, non-cubic p^2 filter, 64-extent pass B."""
-    check_trajectory("C3", fft_mode=1, checkpoints=(10, 60))
+    check_trajectory("C3", fft_mode=1, checkpoints=(10, 100))
 
 
 # ------------------------------------------------------------------ step-size scan (NEXT-3)
@@ -286,9 +286,11 @@ def _c4_inputs():
     return U, cfg["dims"], cfg["storage"]
 
 
-def test_C4_first_iterations_on_the_full_lattice():
+def test_C4_full_lattice_first_iterations_and_full_run():
     """64^4 at full size against the radix-2-FFT-mode oracle (itself pinned to the naive DFT on the CPU): Delta and X of
-    the first iteration element by element on all 16.8 M sites, then F, theta and every link after 1 and 3 iterations."""
+    the first iteration element by element on all 16.8 M sites, then F, theta and every link after 1, 3 and 10
+    iterations, then the whole run to theta < 1e-15 with the stop iteration.  One set of inputs and ONE oracle
+    trajectory for all of it (about 7 s of host time per oracle iteration)."""
     U, dims, storage = _c4_inputs()
     o = oracle.Oracle(dims, storage, fft_mode=1)
     o.load(U)
@@ -314,33 +316,30 @@ def test_C4_first_iterations_on_the_full_lattice():
         assert abs(F - F_ref) <= F_TOL, (k, F, F_ref)
         assert theta_close(th, th_ref), (k, th, th_ref)
         assert np.abs(gf.get_links() - o.get()).max() <= 1e-13 * k, k
-    gf.destroy()
-
-
-@pytest.mark.slow
-@pytest.mark.skipif(not __import__("os").environ.get("LGF_RUN_SLOW"), reason="about 10 minutes of oracle time at 64^4: set LGF_RUN_SLOW=1 "
-                    "(the log of the last run is profiles/r02_C4_full_run.txt)")
-def test_C4_full_run_to_the_stop_iteration():
-    """configs[4] in full: lgf_fix to theta < 1e-15 against the FFT-mode oracle -- the stop iteration (exact, A19), F
-    within 1e-12, theta per A14 at every iteration, every link within 1e-11 at the stop."""
-    U, dims, storage = _c4_inputs()
-    o = oracle.Oracle(dims, storage, fft_mode=1)
-    o.load(U)
+    # the north star's checkpoint after 10 iterations: F, theta, every link
+    F_ref, th_ref = o.iterate(10 - done, ALPHA)
+    F, th = gf.iterate(10 - done, ALPHA)
+    assert abs(F - F_ref) <= F_TOL and theta_close(th, th_ref), (10, F, F_ref, th, th_ref)
+    assert np.abs(gf.get_links() - o.get()).max() <= LINK_TOL
+    # the full run to theta < 1e-15 (configs[4]): the oracle goes on from its iteration 10 to its stop, the
+    # library runs lgf_fix from the start -- stop iteration exact (A19), F and theta of every iteration from 10 on, every
+    # link at the stop.  (C4 stops before 100 iterations, so the stop takes the place of the second checkpoint.)
     r_ref = o.fix(ALPHA, TOL, 1000, history=True)
     assert r_ref["status"] == 0
-    gf = lgf.GaugeFixer(dims, storage)
+    n_ref = 10 + r_ref["n_iter"]
+    h_ref = np.array(r_ref["history"])                     # h_ref[i] = (F, theta) after 10 + i iterations
     gf.load_links(U)
     r = gf.fix(ALPHA, TOL, 1000)
     h = gf.get_history()
-    h_ref = np.array(r_ref["history"])
-    print(f"C4 full run: n_iter {r['n_iter']} (oracle {r_ref['n_iter']}), F {r['F']:.15f} (oracle {r_ref['F']:.15f}), "
+    print(f"C4 full run: n_iter {r['n_iter']} (oracle {n_ref}), F {r['F']:.15f} (oracle {r_ref['F']:.15f}), "
           f"theta {r['theta']:.3e} (oracle {r_ref['theta']:.3e})")
-    assert r["status"] == lgf.LGF_OK and r["n_iter"] == r_ref["n_iter"]
-    assert abs(r["F"] - r_ref["F"]) <= F_TOL and theta_close(r["theta"], r_ref["theta"])
-    assert len(h) == len(h_ref)
-    assert np.abs(h[:, 0] - h_ref[:, 0]).max() <= F_TOL
-    for k in range(len(h)):
-        assert theta_close(h[k, 1], h_ref[k, 1]), (k, h[k, 1], h_ref[k, 1])
+    assert r["status"] == lgf.LGF_OK and r["n_iter"] == n_ref
+    assert abs(r["F"] - r_ref["F"]) <= F_TOL and theta_close(r["theta"], r_ref["theta"]) and r["theta"] < TOL
+    assert len(h) == n_ref + 1 and len(h_ref) == n_ref - 10 + 1
+    assert abs(h[0, 0] - F0_ref) <= F_TOL and theta_close(h[0, 1], th0_ref)
+    assert np.abs(h[10:, 0] - h_ref[:, 0]).max() <= F_TOL
+    for i in range(len(h_ref)):
+        assert theta_close(h[10 + i, 1], h_ref[i, 1]), (10 + i, h[10 + i, 1], h_ref[i, 1])
     dmax = np.abs(gf.get_links() - o.get()).max()
     print(f"C4 full run: max link difference at the stop {dmax:.3e}")
     assert dmax <= LINK_TOL

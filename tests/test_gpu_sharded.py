@@ -7,7 +7,7 @@ import pytest
 import ensembles as E
 import oracle
 import paper_1301_3460_b200 as lgf
-from paper_1301_3460_b200 import slab
+import slab_maps as slab
 
 pytestmark = pytest.mark.gpu
 

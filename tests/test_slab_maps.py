@@ -1,4 +1,4 @@
-"""Host logic of the slab decomposition (paper_1301_3460_b200/slab.py) at world size 2 over gloo on the CPU: the two
+"""Host logic of the slab decomposition (tests/slab_maps.py) at world size 2 over gloo on the CPU: the two
 all-to-all transposes built from the send/place maps reproduce the global re-distribution, the halo sources are the
 periodic neighbours, and the byte counts are those the C library reports (include/lgf.h lgf_sharded_traffic)."""
 import os
@@ -10,7 +10,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_1301_3460_b200 import slab
+import slab_maps as slab
 
 
 def _free_port():
