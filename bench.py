@@ -78,7 +78,7 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-TRAFFIC_CSV = "profiles/r02_ncu_traffic.csv"
+TRAFFIC_CSV = "profiles/r03_ncu_traffic.csv"
 
 
 def ncu_traffic(kernel: str, workload: str):
